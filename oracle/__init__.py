@@ -1,0 +1,150 @@
+"""ctypes loader for the CPU oracle (oracle/painn_oracle.cpp).
+
+TEST INFRASTRUCTURE ONLY: imported by tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs.  The product (paper_2604_15380_b200/) never imports it.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "painn_oracle.cpp")
+_LIB = os.path.join(_HERE, "_build", "libpainn_oracle.so")
+_lock = threading.Lock()
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2 -fopenmp, no BLAS (BASELINE.md "CPU-baseline plan")."""
+    os.makedirs(os.path.dirname(_LIB), exist_ok=True)
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(["g++", "-std=c++17", "-O2", "-fopenmp", "-fPIC", "-shared", _SRC, "-o", tmp])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    with _lock:
+        if _lib is None:
+            lib = ctypes.CDLL(build())
+            lib.oracle_weights_count.restype = ctypes.c_int64
+            lib.oracle_neighbours.restype = ctypes.c_int64
+            lib.oracle_eval.restype = ctypes.c_int64
+            lib.oracle_forces_dual.restype = None
+            lib.oracle_rbf_cutoff.restype = None
+            _lib = lib
+    return _lib
+
+
+def _p(a, ct):
+    return None if a is None else a.ctypes.data_as(ctypes.POINTER(ct))
+
+
+def _cfg_arrays(mc):
+    ic = np.array([mc.F, mc.T, mc.K, mc.H, mc.Zmax], np.int32)
+    dc = np.array([mc.cutoff, mc.norm_eps], np.float64)
+    return ic, dc
+
+
+def num_threads() -> int:
+    """Threads the oracle's OpenMP loops use (OMP_NUM_THREADS or all cores in the affinity mask)."""
+    v = os.environ.get("OMP_NUM_THREADS")
+    if v:
+        return int(v.split(",")[0])
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def rbf_cutoff(d: float, K: int, rc: float):
+    """(g_k(d) [K], c(d)) exactly as the forward pass evaluates them."""
+    lib = _load()
+    g = np.zeros(K, np.float64)
+    c = np.zeros(1, np.float64)
+    lib.oracle_rbf_cutoff(ctypes.c_double(d), ctypes.c_int32(K), ctypes.c_double(rc), _p(g, ctypes.c_double),
+                          _p(c, ctypes.c_double))
+    return g, float(c[0])
+
+
+def weights_count(mc) -> int:
+    ic, _ = _cfg_arrays(mc)
+    return int(_load().oracle_weights_count(_p(ic, ctypes.c_int32)))
+
+
+def _prep(batch):
+    Z = np.ascontiguousarray(batch.Z, np.int32)
+    pos = np.ascontiguousarray(batch.pos, np.float64)
+    sp = np.ascontiguousarray(batch.struct_ptr, np.int32)
+    head = np.ascontiguousarray(batch.head, np.int32)
+    cell = None if batch.cell is None else np.ascontiguousarray(batch.cell, np.float64)
+    pbc = None if batch.pbc is None else np.ascontiguousarray(batch.pbc, np.uint8)
+    return Z, pos, sp, head, cell, pbc
+
+
+def neighbours(batch, cutoff: float):
+    """Brute-force radius graph. Returns dict(rowptr, recv, send, shift, rvec)."""
+    lib = _load()
+    Z, pos, sp, head, cell, pbc = _prep(batch)
+    N, S = Z.shape[0], head.shape[0]
+    rowptr = np.zeros(N + 1, np.int32)
+    E = lib.oracle_neighbours(ctypes.c_int32(N), ctypes.c_int32(S), _p(pos, ctypes.c_double), _p(sp, ctypes.c_int32),
+                              _p(cell, ctypes.c_double), _p(pbc, ctypes.c_uint8), ctypes.c_double(cutoff),
+                              _p(rowptr, ctypes.c_int32), None, None, None, None)
+    recv = np.zeros(E, np.int32)
+    send = np.zeros(E, np.int32)
+    shift = np.zeros((E, 3), np.int8)
+    rvec = np.zeros((E, 3), np.float64)
+    lib.oracle_neighbours(ctypes.c_int32(N), ctypes.c_int32(S), _p(pos, ctypes.c_double), _p(sp, ctypes.c_int32),
+                          _p(cell, ctypes.c_double), _p(pbc, ctypes.c_uint8), ctypes.c_double(cutoff),
+                          _p(rowptr, ctypes.c_int32), _p(recv, ctypes.c_int32), _p(send, ctypes.c_int32),
+                          _p(shift, ctypes.c_int8), _p(rvec, ctypes.c_double))
+    return dict(rowptr=rowptr, recv=recv, send=send, shift=shift, rvec=rvec)
+
+
+def evaluate(mc, weights, batch, forces: bool = True, features: bool = False):
+    """Energy [S], forces [N,3] (or None); with features=True also s [N,F], v [N,3,F], eatom [N]."""
+    lib = _load()
+    ic, dc = _cfg_arrays(mc)
+    w = np.ascontiguousarray(weights, np.float64)
+    assert w.size == weights_count(mc), "weight blob size mismatch"
+    Z, pos, sp, head, cell, pbc = _prep(batch)
+    N, S = Z.shape[0], head.shape[0]
+    assert Z.min(initial=1) >= 1 and Z.max(initial=1) <= mc.Zmax
+    assert head.min(initial=0) >= 0 and head.max(initial=0) < mc.H
+    energy = np.zeros(S, np.float64)
+    frc = np.zeros((N, 3), np.float64) if forces else None
+    s_out = np.zeros((N, mc.F), np.float64) if features else None
+    v_out = np.zeros((N, 3, mc.F), np.float64) if features else None
+    eatom = np.zeros(N, np.float64) if features else None
+    E = lib.oracle_eval(_p(ic, ctypes.c_int32), _p(dc, ctypes.c_double), _p(w, ctypes.c_double), ctypes.c_int32(N),
+                        ctypes.c_int32(S), _p(Z, ctypes.c_int32), _p(pos, ctypes.c_double), _p(sp, ctypes.c_int32),
+                        _p(cell, ctypes.c_double), _p(pbc, ctypes.c_uint8), _p(head, ctypes.c_int32),
+                        _p(energy, ctypes.c_double), _p(frc, ctypes.c_double), _p(s_out, ctypes.c_double),
+                        _p(v_out, ctypes.c_double), _p(eatom, ctypes.c_double))
+    out = dict(energy=energy, forces=frc, n_edges=int(E))
+    if features:
+        out.update(s=s_out, v=v_out, eatom=eatom)
+    return out
+
+
+def forces_dual(mc, weights, batch):
+    """Forces by forward-mode dual numbers (3N forward evaluations; tiny inputs only)."""
+    lib = _load()
+    ic, dc = _cfg_arrays(mc)
+    w = np.ascontiguousarray(weights, np.float64)
+    Z, pos, sp, head, cell, pbc = _prep(batch)
+    N, S = Z.shape[0], head.shape[0]
+    frc = np.zeros((N, 3), np.float64)
+    lib.oracle_forces_dual(_p(ic, ctypes.c_int32), _p(dc, ctypes.c_double), _p(w, ctypes.c_double), ctypes.c_int32(N),
+                           ctypes.c_int32(S), _p(Z, ctypes.c_int32), _p(pos, ctypes.c_double), _p(sp, ctypes.c_int32),
+                           _p(cell, ctypes.c_double), _p(pbc, ctypes.c_uint8), _p(head, ctypes.c_int32),
+                           _p(frc, ctypes.c_double))
+    return frc
