@@ -1,0 +1,133 @@
+/* include/pnn.h — C ABI of the B200-native batched PaiNN energy+force library (libpnn.so).
+ *
+ * The path (the paper names the backbone and the problem only:
+ * PAPER.md:147 "PaiNN" [48], PAPER.md:53 forces = energy gradients w.r.t. positions,
+ * PAPER.md:126/232 shared trunk + 16 per-dataset heads, PAPER.md:229-231 radial basis / cutoff,
+ * PAPER.md:269 periodic boundary conditions, PAPER.md:172 BF16/FP32/FP64):
+ *
+ *   (Z, positions, optional cell/PBC, per-structure head index, weights, precision)
+ *        -> (per-structure energy, per-atom forces = -dE/dx)
+ *
+ * Conventions
+ *   - Every function returns int: 0 = PNN_OK, < 0 = error (pnn_status_string()).  No exceptions, no aborts.
+ *   - "DEVICE" pointers are CUDA device pointers owned by the caller (e.g. torch allocations); the library
+ *     never frees them and does not use them after the stream work of the call has run.  "HOST" pointers are
+ *     ordinary host memory, read or written synchronously inside the call.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls only enqueue work and do
+ *     not synchronise unless stated.
+ *   - Atoms of a structure are contiguous: struct_ptr[0] = 0, struct_ptr[S] = N.  Units: Angstrom; energies in
+ *     the (arbitrary) units of the weights.  Positions are FP64 at the boundary for every model precision so
+ *     that the cutoff predicate is evaluated in FP64 (bit-exact edge sets).
+ *   - Row-major everywhere.  Weight blob: flat FP64, matrices [out][in], y = W x + b, in the order
+ *       emb[Zmax+1][F] (row 0 unused)
+ *       per block t: msg_W1[F][F] msg_b1[F] msg_W2[3F][F] msg_b2[3F] flt_W[3F][K] flt_b[3F]
+ *                    upd_U[F][F] upd_V[F][F] upd_A1[F][2F] upd_c1[F] upd_A2[3F][F] upd_c2[3F]
+ *       per head h:  out_W1[F/2][F] out_b1[F/2] out_w2[F/2] out_b2[1]
+ *     3F chunks: rows [0,F) scalar (ss), [F,2F) direction (vs), [2F,3F) vector (vv); upd_A2 rows
+ *     [0,F) a_vv, [F,2F) a_sv, [2F,3F) a_ss.
+ */
+#ifndef PNN_H_
+#define PNN_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PNN_OK 0
+#define PNN_ERR_INVALID_ARG (-1) /* null pointer, negative size, F not a multiple of 32 or > 256, K > 32 ...  */
+#define PNN_ERR_CAPACITY (-2)    /* N / E / S exceed what the workspace was created for                        */
+#define PNN_ERR_CUDA (-3)        /* a CUDA runtime call failed; pnn_last_cuda_error() has the text             */
+#define PNN_ERR_UNSUPPORTED (-4) /* feature not available in this build / for this precision                   */
+#define PNN_ERR_NO_GRAPH (-5)    /* pnn_eval called before pnn_build_graph for these sizes                     */
+#define PNN_ERR_BAD_INPUT (-6)   /* device-side check failed: Z outside [1,Zmax] or head outside [0,H)         */
+
+typedef enum { PNN_BF16 = 0, PNN_FP32 = 1, PNN_FP64 = 2 } pnn_precision;
+
+/* F feature width (multiple of 32, 32..256), T interaction blocks, K Gaussian radial basis functions (2..32),
+ * H heads, Zmax largest atomic number, cutoff r_c [A], norm_eps the epsilon under the sqrt of the update block. */
+typedef struct {
+  int32_t F, T, K, H, Zmax;
+  double cutoff;
+  double norm_eps;
+  int32_t prec; /* pnn_precision */
+} pnn_config;
+
+typedef struct pnn_model pnn_model;         /* opaque; owns device copies of the weights in model precision */
+typedef struct pnn_workspace pnn_workspace; /* opaque; owns CSR graph, activations and adjoints             */
+
+/* Number of FP64 scalars in the weight blob for this configuration (layout above). */
+int pnn_weights_count(const pnn_config* cfg, int64_t* n_scalars);
+
+/* Uploads (and converts / transposes) the weights.  weights_host: HOST, FP64, n_scalars must equal
+ * pnn_weights_count().  Synchronous. */
+int pnn_model_create(const pnn_config* cfg, const double* weights_host, int64_t n_scalars, pnn_model** out);
+void pnn_model_destroy(pnn_model* m);
+
+/* Allocates all device memory needed for batches of up to max_atoms atoms, max_edges directed edges and
+ * max_structs structures.  want_forces != 0 also allocates the per-block tape and the adjoint buffers
+ * (SURVEY.md §8(a) a7).  Synchronous. */
+int pnn_workspace_create(const pnn_model* m, int64_t max_atoms, int64_t max_edges, int64_t max_structs,
+                         int want_forces, pnn_workspace** out);
+void pnn_workspace_destroy(pnn_workspace* ws);
+/* Bytes of device memory the workspace holds. */
+int64_t pnn_workspace_bytes(const pnn_workspace* ws);
+
+/* a1 — radius graph (PAPER.md:230 cutoff, PAPER.md:269 PBC).  All ordered pairs (i, j),
+ * i != j, in the same structure, with |x_j - x_i + shift.C| < r_c (strict, FP64); under PBC the shift is the
+ * per-axis minimum-image rounding of the fractional difference.  Built by a cell list (cells >= r_c wide; a
+ * structure narrower than 3 cells along an axis uses one cell on that axis) and emitted as receiver-sorted CSR
+ * held inside the workspace, together with the per-edge unit vector and distance in model precision.
+ *   pos        DEVICE [N,3] f64        struct_ptr DEVICE [S+1] i32
+ *   cell       DEVICE [S,3,3] f64 (rows = lattice vectors) or NULL    pbc DEVICE [S,3] u8 or NULL
+ * Edge overflow (E > max_edges) is detected on the device and reported by pnn_check_async_errors /
+ * pnn_graph_view.  Asynchronous. */
+int pnn_build_graph(pnn_workspace* ws, int64_t n_atoms, int64_t n_structs, const double* pos,
+                    const int32_t* struct_ptr, const double* cell, const uint8_t* pbc, void* cuda_stream);
+
+/* DEVICE views of the last graph: rowptr [N+1] i32 (receiver i owns edges rowptr[i]..rowptr[i+1]), col [E] i32
+ * (global sender index), shift [E,3] i8 (integer lattice shift of the sender image).  *n_edges is a host value:
+ * this call synchronises the stream of the last pnn_build_graph.  Any out pointer may be NULL. */
+int pnn_graph_view(const pnn_workspace* ws, const int32_t** rowptr, const int32_t** col, const int8_t** shift,
+                   int64_t* n_edges);
+
+/* Copies the last graph into caller-owned buffers (HOST or DEVICE, sized from pnn_graph_view's n_edges):
+ * rowptr [N+1] i32, col [E] i32, shift [E,3] i8.  Any pointer may be NULL.  Synchronous. */
+int pnn_graph_copy(const pnn_workspace* ws, int32_t* rowptr, int32_t* col, int8_t* shift);
+
+#define PNN_ENERGY 1
+#define PNN_FORCES 2
+
+/* a2..a7 — embedding, T x (message, update), multi-head readout, and (with PNN_FORCES) the analytic reverse
+ * sweep.  Uses the graph last built in the workspace (same n_atoms, n_structs
+ * and pos; PNN_ERR_NO_GRAPH otherwise).
+ *   Z DEVICE [N] i32 in [1,Zmax]     head DEVICE [S] i32 in [0,H)
+ *   energy DEVICE [S], forces DEVICE [N,3]: f64 for a PNN_FP64 model, f32 for PNN_FP32 and PNN_BF16.
+ *   forces may be NULL unless flags has PNN_FORCES (which needs a workspace created with want_forces).
+ * Asynchronous. */
+int pnn_eval(const pnn_model* m, pnn_workspace* ws, int64_t n_atoms, int64_t n_structs, const int32_t* Z,
+             const double* pos, const int32_t* struct_ptr, const int32_t* head, int flags, void* energy,
+             void* forces, void* cuda_stream);
+
+/* Convenience for callers with HOST buffers (bench.py's e2e leg): copies Z, pos, struct_ptr, head (and cell /
+ * pbc when not NULL) to the device, runs pnn_build_graph + pnn_eval and copies energy [S] / forces [N,3] back.
+ * energy_host / forces_host have the dtype pnn_eval documents.  Synchronous. */
+int pnn_eval_host(const pnn_model* m, pnn_workspace* ws, int64_t n_atoms, int64_t n_structs, const int32_t* Z,
+                  const double* pos, const int32_t* struct_ptr, const int32_t* head, const double* cell,
+                  const uint8_t* pbc, int flags, void* energy_host, void* forces_host, void* cuda_stream);
+
+/* Reads the device error flags (edge overflow -> PNN_ERR_CAPACITY, bad Z / head -> PNN_ERR_BAD_INPUT) and
+ * clears them.  Synchronises the device. */
+int pnn_check_async_errors(pnn_workspace* ws);
+
+/* Number of kernels the library has launched on behalf of this workspace since it was created. */
+int64_t pnn_launch_count(const pnn_workspace* ws);
+
+const char* pnn_status_string(int status);
+const char* pnn_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PNN_H_ */

@@ -1,0 +1,278 @@
+"""ctypes binding of include/pnn.h.  Argument marshalling only: every step of the path runs inside libpnn.so.
+
+Pointers: DEVICE arguments are passed as integers (`tensor.data_ptr()`); HOST arguments as C-contiguous
+numpy arrays.  `PaiNN` is a small convenience holder (model + workspace) used by the tests and bench.py; it
+only allocates output tensors with torch and forwards pointers.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import numpy as np
+
+__all__ = [
+    "PNN_OK", "PNN_BF16", "PNN_FP32", "PNN_FP64", "PNN_ENERGY", "PNN_FORCES", "PnnError", "pnn_config", "lib",
+    "lib_path", "pnn_status_string", "pnn_last_cuda_error", "pnn_weights_count", "pnn_model_create",
+    "pnn_model_destroy", "pnn_workspace_create", "pnn_workspace_destroy", "pnn_workspace_bytes", "pnn_build_graph",
+    "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_eval_host", "pnn_check_async_errors", "pnn_launch_count",
+    "PaiNN", "PRECISIONS",
+]
+
+PNN_OK = 0
+PNN_BF16, PNN_FP32, PNN_FP64 = 0, 1, 2
+PNN_ENERGY, PNN_FORCES = 1, 2
+PRECISIONS = {"bf16": PNN_BF16, "fp32": PNN_FP32, "fp64": PNN_FP64}
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libpnn.so")
+_lib = None
+
+
+class PnnError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = f"{where}: {pnn_status_string(status)} ({status})"
+        if status == -3:
+            msg += f" — {pnn_last_cuda_error()}"
+        super().__init__(msg)
+
+
+class pnn_config(ctypes.Structure):
+    _fields_ = [("F", ctypes.c_int32), ("T", ctypes.c_int32), ("K", ctypes.c_int32), ("H", ctypes.c_int32),
+                ("Zmax", ctypes.c_int32), ("cutoff", ctypes.c_double), ("norm_eps", ctypes.c_double),
+                ("prec", ctypes.c_int32)]
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def lib():
+    """Loads libpnn.so (built in-tree by paper_2604_15380_b200.build).  Raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise ImportError(f"{_LIB_PATH} not found: build it with `python -m paper_2604_15380_b200.build` "
+                              "(the CUDA library is the product; there is no fallback)")
+        L = ctypes.CDLL(_LIB_PATH)
+        vp, i64, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
+        L.pnn_status_string.restype = ctypes.c_char_p
+        L.pnn_status_string.argtypes = [i32]
+        L.pnn_last_cuda_error.restype = ctypes.c_char_p
+        L.pnn_last_cuda_error.argtypes = []
+        L.pnn_weights_count.argtypes = [ctypes.POINTER(pnn_config), ctypes.POINTER(i64)]
+        L.pnn_model_create.argtypes = [ctypes.POINTER(pnn_config), vp, i64, ctypes.POINTER(vp)]
+        L.pnn_model_destroy.argtypes = [vp]
+        L.pnn_model_destroy.restype = None
+        L.pnn_workspace_create.argtypes = [vp, i64, i64, i64, i32, ctypes.POINTER(vp)]
+        L.pnn_workspace_destroy.argtypes = [vp]
+        L.pnn_workspace_destroy.restype = None
+        L.pnn_workspace_bytes.argtypes = [vp]
+        L.pnn_workspace_bytes.restype = i64
+        L.pnn_build_graph.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
+        L.pnn_graph_view.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp),
+                                     ctypes.POINTER(i64)]
+        L.pnn_graph_copy.argtypes = [vp, vp, vp, vp]
+        L.pnn_eval.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, i32, vp, vp, vp]
+        L.pnn_eval_host.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp]
+        L.pnn_check_async_errors.argtypes = [vp]
+        L.pnn_launch_count.argtypes = [vp]
+        L.pnn_launch_count.restype = i64
+        _lib = L
+    return _lib
+
+
+def _check(st: int, where: str):
+    if st != PNN_OK:
+        raise PnnError(st, where)
+
+
+def _ptr(x) -> Optional[int]:
+    """int / None pass through; numpy arrays give their host address; torch tensors their data_ptr()."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if isinstance(x, np.ndarray):
+        assert x.flags["C_CONTIGUOUS"]
+        return x.ctypes.data
+    return x.data_ptr()
+
+
+def pnn_status_string(status: int) -> str:
+    return lib().pnn_status_string(status).decode()
+
+
+def pnn_last_cuda_error() -> str:
+    return lib().pnn_last_cuda_error().decode()
+
+
+def pnn_weights_count(cfg: pnn_config) -> int:
+    n = ctypes.c_int64(0)
+    _check(lib().pnn_weights_count(ctypes.byref(cfg), ctypes.byref(n)), "pnn_weights_count")
+    return n.value
+
+
+def pnn_model_create(cfg: pnn_config, weights_host: np.ndarray) -> int:
+    w = np.ascontiguousarray(weights_host, np.float64)
+    out = ctypes.c_void_p()
+    _check(lib().pnn_model_create(ctypes.byref(cfg), w.ctypes.data, w.size, ctypes.byref(out)), "pnn_model_create")
+    return out.value
+
+
+def pnn_model_destroy(model: int) -> None:
+    lib().pnn_model_destroy(model)
+
+
+def pnn_workspace_create(model: int, max_atoms: int, max_edges: int, max_structs: int, want_forces: bool) -> int:
+    out = ctypes.c_void_p()
+    _check(lib().pnn_workspace_create(model, max_atoms, max_edges, max_structs, int(bool(want_forces)),
+                                      ctypes.byref(out)), "pnn_workspace_create")
+    return out.value
+
+
+def pnn_workspace_destroy(ws: int) -> None:
+    lib().pnn_workspace_destroy(ws)
+
+
+def pnn_workspace_bytes(ws: int) -> int:
+    return lib().pnn_workspace_bytes(ws)
+
+
+def pnn_build_graph(ws: int, n_atoms: int, n_structs: int, pos, struct_ptr, cell=None, pbc=None, stream=None):
+    _check(lib().pnn_build_graph(ws, n_atoms, n_structs, _ptr(pos), _ptr(struct_ptr), _ptr(cell), _ptr(pbc),
+                                 stream), "pnn_build_graph")
+
+
+def pnn_graph_view(ws: int):
+    """(rowptr_ptr, col_ptr, shift_ptr, n_edges); synchronises the build stream."""
+    r, c, s = ctypes.c_void_p(), ctypes.c_void_p(), ctypes.c_void_p()
+    n = ctypes.c_int64(0)
+    _check(lib().pnn_graph_view(ws, ctypes.byref(r), ctypes.byref(c), ctypes.byref(s), ctypes.byref(n)),
+           "pnn_graph_view")
+    return r.value, c.value, s.value, n.value
+
+
+def pnn_graph_copy(ws: int, rowptr=None, col=None, shift=None):
+    _check(lib().pnn_graph_copy(ws, _ptr(rowptr), _ptr(col), _ptr(shift)), "pnn_graph_copy")
+
+
+def pnn_eval(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, struct_ptr, head, flags: int, energy,
+             forces=None, stream=None):
+    _check(lib().pnn_eval(model, ws, n_atoms, n_structs, _ptr(Z), _ptr(pos), _ptr(struct_ptr), _ptr(head), flags,
+                          _ptr(energy), _ptr(forces), stream), "pnn_eval")
+
+
+def pnn_eval_host(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, struct_ptr, head, cell, pbc,
+                  flags: int, energy_host, forces_host=None, stream=None):
+    _check(lib().pnn_eval_host(model, ws, n_atoms, n_structs, _ptr(Z), _ptr(pos), _ptr(struct_ptr), _ptr(head),
+                               _ptr(cell), _ptr(pbc), flags, _ptr(energy_host), _ptr(forces_host), stream),
+           "pnn_eval_host")
+
+
+def pnn_check_async_errors(ws: int) -> None:
+    _check(lib().pnn_check_async_errors(ws), "pnn_check_async_errors")
+
+
+def pnn_launch_count(ws: int) -> int:
+    return lib().pnn_launch_count(ws)
+
+
+class PaiNN:
+    """Model + workspace holder.  Marshals torch tensors / numpy arrays into the C ABI; no arithmetic here."""
+
+    def __init__(self, F: int, T: int, K: int, H: int, weights: np.ndarray, *, precision: str = "fp32",
+                 cutoff: float = 5.0, Zmax: int = 86, norm_eps: float = 1e-8, max_atoms: int, max_edges: int,
+                 max_structs: int, forces: bool = True):
+        self.cfg = pnn_config(F, T, K, H, Zmax, cutoff, norm_eps, PRECISIONS[precision])
+        self.precision = precision
+        self.want_forces = bool(forces)
+        self.model = pnn_model_create(self.cfg, weights)
+        try:
+            self.ws = pnn_workspace_create(self.model, max_atoms, max_edges, max_structs, forces)
+        except Exception:
+            pnn_model_destroy(self.model)
+            self.model = None
+            raise
+        self.max_atoms, self.max_edges, self.max_structs = max_atoms, max_edges, max_structs
+
+    def close(self):
+        if getattr(self, "ws", None):
+            pnn_workspace_destroy(self.ws)
+            self.ws = None
+        if getattr(self, "model", None):
+            pnn_model_destroy(self.model)
+            self.model = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def out_dtype(self):
+        import torch
+        return torch.float64 if self.precision == "fp64" else torch.float32
+
+    @property
+    def out_np_dtype(self):
+        return np.float64 if self.precision == "fp64" else np.float32
+
+    @staticmethod
+    def _stream():
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+
+    def build_graph(self, pos, struct_ptr, cell=None, pbc=None):
+        """pos [N,3] f64, struct_ptr [S+1] i32, cell [S,3,3] f64, pbc [S,3] u8: CUDA tensors."""
+        N, S = int(pos.shape[0]), int(struct_ptr.shape[0]) - 1
+        pnn_build_graph(self.ws, N, S, pos, struct_ptr, cell, pbc, self._stream())
+
+    def graph(self):
+        """Host copies (numpy) of rowptr [N+1], col [E], shift [E,3]."""
+        _, _, _, E = pnn_graph_view(self.ws)
+        N = self._last_N
+        rowptr = np.zeros(N + 1, np.int32)
+        col = np.zeros(E, np.int32)
+        shift = np.zeros((E, 3), np.int8)
+        pnn_graph_copy(self.ws, rowptr, col, shift)
+        return rowptr, col, shift
+
+    def eval(self, Z, pos, struct_ptr, head, cell=None, pbc=None, forces: Optional[bool] = None, build: bool = True):
+        """CUDA tensors in, CUDA tensors out: (energy [S], forces [N,3] or None)."""
+        import torch
+        forces = self.want_forces if forces is None else forces
+        N, S = int(Z.shape[0]), int(head.shape[0])
+        self._last_N = N
+        if build:
+            self.build_graph(pos, struct_ptr, cell, pbc)
+        energy = torch.empty(S, dtype=self.out_dtype, device=pos.device)
+        frc = torch.empty((N, 3), dtype=self.out_dtype, device=pos.device) if forces else None
+        flags = PNN_ENERGY | (PNN_FORCES if forces else 0)
+        pnn_eval(self.model, self.ws, N, S, Z, pos, struct_ptr, head, flags, energy, frc, self._stream())
+        return energy, frc
+
+    def eval_host(self, Z, pos, struct_ptr, head, cell=None, pbc=None, forces: Optional[bool] = None,
+                  energy_out=None, forces_out=None):
+        """Host numpy arrays (or pinned torch CPU tensors) in and out; H2D/D2H copies happen inside the library."""
+        forces = self.want_forces if forces is None else forces
+        N, S = int(Z.shape[0]), int(head.shape[0])
+        self._last_N = N
+        if energy_out is None:
+            energy_out = np.empty(S, self.out_np_dtype)
+        if forces and forces_out is None:
+            forces_out = np.empty((N, 3), self.out_np_dtype)
+        flags = PNN_ENERGY | (PNN_FORCES if forces else 0)
+        pnn_eval_host(self.model, self.ws, N, S, Z, pos, struct_ptr, head, cell, pbc, flags, energy_out,
+                      forces_out if forces else None, self._stream())
+        return energy_out, (forces_out if forces else None)
+
+    def check(self):
+        pnn_check_async_errors(self.ws)
+
+    @property
+    def launches(self) -> int:
+        return pnn_launch_count(self.ws)

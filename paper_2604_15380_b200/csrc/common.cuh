@@ -1,0 +1,147 @@
+// common.cuh — shared declarations of the CUDA library (internal; the public boundary is include/pnn.h).
+#pragma once
+
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace pnn {
+
+// Records the first failed kernel launch (checked with cudaPeekAtLastError after every launch); pnn_api.cu
+// turns it into PNN_ERR_CUDA.
+void note_launch(const char* where);
+#define PNN_KCHECK(name) ::pnn::note_launch(name)
+
+// device-side error flags (workspace->d_err)
+enum : int { ERRF_EDGE_OVERFLOW = 1, ERRF_BAD_Z = 2, ERRF_BAD_HEAD = 4 };
+
+// Per-edge geometry in model precision: unit vector receiver->sender image and distance.
+template <typename T>
+struct __align__(sizeof(T) * 4) Geom {
+  T ux, uy, uz, d;
+};
+
+// Per-structure cell-grid descriptor written by the graph builder.
+struct GridDesc {
+  double C[9];      // lattice rows (identity when not periodic)
+  double Ci[9];     // inverse
+  double fmin[3];   // fractional origin of the binning box (0 on periodic axes)
+  double fscale[3]; // cells per unit of fractional coordinate on each axis
+  int32_t dim[3];   // cells per axis
+  int32_t per[3];   // axis is periodic
+  int32_t periodic; // any axis periodic
+  int32_t ncell;    // dim[0]*dim[1]*dim[2]
+};
+
+template <typename T>
+__device__ __forceinline__ T silu_f(T x) {
+  return x / (T(1) + exp(-x));
+}
+template <>
+__device__ __forceinline__ float silu_f<float>(float x) {
+  return x / (1.0f + expf(-x));
+}
+// silu'(x) = sg (1 + x (1 - sg)), sg = 1/(1+e^-x)
+template <typename T>
+__device__ __forceinline__ T dsilu_f(T x) {
+  const T sg = T(1) / (T(1) + exp(-x));
+  return sg * (T(1) + x * (T(1) - sg));
+}
+template <>
+__device__ __forceinline__ float dsilu_f<float>(float x) {
+  const float sg = 1.0f / (1.0f + expf(-x));
+  return sg * (1.0f + x * (1.0f - sg));
+}
+
+// ---------------------------------------------------------------------------------------------
+// launch wrappers (one per kernel family); every wrapper returns the number of kernels launched
+// ---------------------------------------------------------------------------------------------
+
+// graph.cu
+struct GraphBuffers {
+  int32_t* a2s;        // [N] atom -> structure
+  GridDesc* desc;      // [S]
+  int32_t* ncell;      // [S+1] cells per structure, then exclusive scan in cell_off
+  int32_t* cell_off;   // [S+1]
+  int32_t* cid;        // [N] global cell of atom
+  int32_t* cell_cnt;   // [N+S+1]
+  int32_t* cell_start; // [N+S+2]
+  int32_t* cell_fill;  // [N+S+1]
+  int32_t* sorted;     // [N] atoms ordered by (structure, cell, index)
+  int32_t* deg;        // [N+1]
+  int32_t* rowptr;     // [N+1]
+  int32_t* col;        // [Emax]
+  int8_t* shift;       // [Emax,3]
+  void* geom;          // [Emax] Geom<T>
+  int32_t* scan_tmp;   // scratch for the scans
+  int64_t max_edges;
+  int* d_err;
+};
+int launch_graph_build(const GraphBuffers& g, int64_t N, int64_t S, const double* pos, const int32_t* struct_ptr,
+                       const double* cell, const uint8_t* pbc, double rc, int prec, cudaStream_t st);
+
+// gemm_simt.cu :  C[M,N] (ldc) = epi( A[M,K] (lda) * B[K,N] (ldb) )
+enum : int { ACT_NONE = 0, ACT_SILU = 1, ACT_MUL_DSILU = 2 };
+template <typename T>
+struct GemmEpi {
+  const T* bias = nullptr; // [N] added before the activation
+  int act = ACT_NONE;
+  T* pre = nullptr;        // ACT_SILU: also store the pre-activation here (ld = ldpre)
+  int64_t ldpre = 0;
+  const T* aux = nullptr;  // ACT_MUL_DSILU: result *= silu'(aux[m][n]) (ld = ldaux)
+  int64_t ldaux = 0;
+  int accumulate = 0;      // C += result
+};
+template <typename T>
+int launch_gemm(int64_t M, int N, int K, const T* A, int64_t lda, const T* B, int64_t ldb, T* C, int64_t ldc,
+                const GemmEpi<T>& epi, cudaStream_t st);
+
+// edge.cu
+template <typename T>
+struct EdgeArgs {
+  int64_t N;
+  int F, K;
+  double rc;
+  const int32_t* rowptr;
+  const int32_t* col;
+  const Geom<T>* geom;
+  const T* fltW; // [3F][K]
+  const T* fltb; // [3F]
+  const int* d_err;
+};
+// forward message step (B3b): s1 = s_in + sum, v1 = v_in + sum.  s_in/s1 have leading dimensions.
+template <typename T>
+int launch_edge_fwd(const EdgeArgs<T>& a, const T* phi, const T* s_in, int64_t ld_sin, const T* v_in, T* s1,
+                    int64_t ld_s1, T* v1, cudaStream_t st);
+// reverse message step (R3 + R4 partial): from sb1 [N,F], vb1 [N,3F] and the forward phi, v_in produce
+// phib [N,3F], vb_in [N,3F] and add this block's force contribution into fpart [nslab][N][3].
+template <typename T>
+int launch_edge_bwd(const EdgeArgs<T>& a, const T* phi, const T* v_in, const T* sb1, const T* vb1, T* phib, T* vb_in,
+                    T* fpart, int first_block, cudaStream_t st);
+int edge_num_slabs(int F);
+
+// node.cu
+template <typename T>
+int launch_embed(int64_t N, int F, int Zmax, const int32_t* Z, const T* emb, T* s, int* d_err, cudaStream_t st);
+template <typename T>
+int launch_norm(int64_t N, int F, const T* PQ, T* sn, T eps, cudaStream_t st);
+template <typename T>
+int launch_update(int64_t N, int F, const T* sn, const T* v1, const T* PQ, const T* a, T* s_out, T* v_out,
+                  cudaStream_t st);
+template <typename T>
+int launch_update_bwd1(int64_t N, int F, const T* sb, const T* vb, const T* a, const T* PQ, T* ab, T* PQb,
+                       cudaStream_t st);
+template <typename T>
+int launch_update_bwd2(int64_t N, int F, const T* zb, const T* PQ, T eps, T* sb, T* PQb, cudaStream_t st);
+// readout (B5 / R1).  W1t: [H][F][F/2] (transposed), W1: [H][F/2][F], b1 [H][F/2], w2 [H][F/2], b2 [H].
+template <typename T>
+int launch_readout(int64_t N, int64_t S, int F, int H, const T* s, const int32_t* a2s, const int32_t* head,
+                   const int32_t* struct_ptr, const T* W1t, const T* b1, const T* w2, const T* b2, T* opre, T* eatom,
+                   T* energy, int* d_err, cudaStream_t st);
+template <typename T>
+int launch_readout_bwd(int64_t N, int F, int H, const T* opre, const int32_t* a2s, const int32_t* head, const T* W1,
+                       const T* w2, T* sb, cudaStream_t st);
+template <typename T>
+int launch_force_assemble(int64_t N, int nslab, const T* fpart, T* forces, cudaStream_t st);
+
+} // namespace pnn

@@ -1,0 +1,175 @@
+// gemm_simt.cu — FP32 / FP64 dense node contractions (a3, a5 and their adjoints) on the ordinary ALUs.
+//
+//   C[M,N] = epi( A[M,K] * B[K,N] ),  all row-major, K a multiple of 16, N a multiple of 4.
+//
+// tcgen05 has no FP64 kind and no true-FP32 kind (SURVEY.md §7 hard part 2), so the FP32 and FP64 models run
+// their Linear layers here: a register-blocked, shared-memory tiled FFMA / DFMA kernel with a double-buffered
+// global->register->shared pipeline.  The BF16 model uses gemm_tc.cu (tcgen05 + TMA + TMEM) instead.
+// Epilogues fuse what follows each Linear in SURVEY.md §8(c): bias, SiLU (+ store of the pre-activation for the
+// reverse sweep), multiplication by silu'(stored pre-activation), and accumulation into C (residual adjoints).
+#include "common.cuh"
+
+namespace pnn {
+
+namespace {
+
+template <typename T> struct V4;
+template <> struct V4<float> { using type = float4; };
+template <> struct V4<double> { using type = double4; };
+
+template <typename T, int BM, int BN, int TM, int TN, int BK>
+__global__ void __launch_bounds__((BM / TM) * (BN / TN))
+gemm_k(int64_t M, int N, int K, const T* __restrict__ A, int64_t lda, const T* __restrict__ B, int64_t ldb,
+       T* __restrict__ C, int64_t ldc, GemmEpi<T> epi) {
+  constexpr int NT = (BM / TM) * (BN / TN);
+  constexpr int PAD = 4;
+  using V = typename V4<T>::type;
+  static_assert(TM % 4 == 0 && TN % 4 == 0, "micro tile in units of 4");
+  static_assert((BM * BK / 4) % NT == 0 && (BK * BN / 4) % NT == 0, "tile loads must divide evenly");
+  constexpr int A_LD = (BM * BK / 4) / NT; // vector loads per thread for the A tile
+  constexpr int B_LD = (BK * BN / 4) / NT;
+
+  __shared__ __align__(32) T As[2][BK][BM + PAD]; // transposed A tile
+  __shared__ __align__(32) T Bs[2][BK][BN + PAD];
+
+  const int tid = threadIdx.x;
+  const int tx = tid % (BN / TN), ty = tid / (BN / TN);
+  const int64_t m0 = (int64_t)blockIdx.x * BM;
+  const int n0 = blockIdx.y * BN;
+
+  T acc[TM][TN];
+#pragma unroll
+  for (int i = 0; i < TM; ++i)
+#pragma unroll
+    for (int j = 0; j < TN; ++j) acc[i][j] = T(0);
+
+  V ra[A_LD], rb[B_LD];
+  auto gload = [&](int k0) {
+#pragma unroll
+    for (int q = 0; q < A_LD; ++q) {
+      const int v = tid + q * NT;          // vector index in the BM x (BK/4) tile
+      const int r = v / (BK / 4), kq = v % (BK / 4);
+      const int64_t m = m0 + r;
+      if (m < M) ra[q] = *reinterpret_cast<const V*>(A + m * lda + k0 + kq * 4);
+      else ra[q] = V{T(0), T(0), T(0), T(0)};
+    }
+#pragma unroll
+    for (int q = 0; q < B_LD; ++q) {
+      const int v = tid + q * NT;          // vector index in the BK x (BN/4) tile
+      const int r = v / (BN / 4), nq = v % (BN / 4);
+      const int n = n0 + nq * 4;
+      if (n < N) rb[q] = *reinterpret_cast<const V*>(B + (int64_t)(k0 + r) * ldb + n);
+      else rb[q] = V{T(0), T(0), T(0), T(0)};
+    }
+  };
+  auto sstore = [&](int buf) {
+#pragma unroll
+    for (int q = 0; q < A_LD; ++q) {
+      const int v = tid + q * NT;
+      const int r = v / (BK / 4), kq = v % (BK / 4);
+      As[buf][kq * 4 + 0][r] = ra[q].x; As[buf][kq * 4 + 1][r] = ra[q].y;
+      As[buf][kq * 4 + 2][r] = ra[q].z; As[buf][kq * 4 + 3][r] = ra[q].w;
+    }
+#pragma unroll
+    for (int q = 0; q < B_LD; ++q) {
+      const int v = tid + q * NT;
+      const int r = v / (BN / 4), nq = v % (BN / 4);
+      *reinterpret_cast<V*>(&Bs[buf][r][nq * 4]) = rb[q];
+    }
+  };
+
+  // micro-tile ownership: TM/4 groups of 4 rows spaced BM/(TM/4) apart, same for columns (conflict-free LDS.128)
+  constexpr int GM = TM / 4, GN = TN / 4;
+  constexpr int SM_ = BM / GM, SN_ = BN / GN;
+
+  gload(0);
+  sstore(0);
+  __syncthreads();
+  const int nk = K / BK;
+  for (int kt = 0; kt < nk; ++kt) {
+    const int buf = kt & 1;
+    if (kt + 1 < nk) gload((kt + 1) * BK);
+#pragma unroll
+    for (int k = 0; k < BK; ++k) {
+      T a[TM], b[TN];
+#pragma unroll
+      for (int gi = 0; gi < GM; ++gi) {
+        const V t = *reinterpret_cast<const V*>(&As[buf][k][gi * SM_ + ty * 4]);
+        a[gi * 4 + 0] = t.x; a[gi * 4 + 1] = t.y; a[gi * 4 + 2] = t.z; a[gi * 4 + 3] = t.w;
+      }
+#pragma unroll
+      for (int gj = 0; gj < GN; ++gj) {
+        const V t = *reinterpret_cast<const V*>(&Bs[buf][k][gj * SN_ + tx * 4]);
+        b[gj * 4 + 0] = t.x; b[gj * 4 + 1] = t.y; b[gj * 4 + 2] = t.z; b[gj * 4 + 3] = t.w;
+      }
+#pragma unroll
+      for (int i = 0; i < TM; ++i)
+#pragma unroll
+        for (int j = 0; j < TN; ++j) acc[i][j] = fma(a[i], b[j], acc[i][j]);
+    }
+    if (kt + 1 < nk) {
+      sstore(buf ^ 1);
+      __syncthreads();
+    }
+  }
+
+  // epilogue
+#pragma unroll
+  for (int gi = 0; gi < GM; ++gi)
+#pragma unroll
+    for (int ii = 0; ii < 4; ++ii) {
+      const int64_t m = m0 + gi * SM_ + ty * 4 + ii;
+      if (m >= M) continue;
+#pragma unroll
+      for (int gj = 0; gj < GN; ++gj) {
+        const int n = n0 + gj * SN_ + tx * 4;
+        if (n >= N) continue;
+        T r[4];
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) r[jj] = acc[gi * 4 + ii][gj * 4 + jj];
+        if (epi.bias) {
+          const V bv = *reinterpret_cast<const V*>(epi.bias + n);
+          r[0] += bv.x; r[1] += bv.y; r[2] += bv.z; r[3] += bv.w;
+        }
+        if (epi.act == ACT_SILU) {
+          if (epi.pre) *reinterpret_cast<V*>(epi.pre + m * epi.ldpre + n) = V{r[0], r[1], r[2], r[3]};
+#pragma unroll
+          for (int jj = 0; jj < 4; ++jj) r[jj] = silu_f<T>(r[jj]);
+        } else if (epi.act == ACT_MUL_DSILU) {
+          const V xv = *reinterpret_cast<const V*>(epi.aux + m * epi.ldaux + n);
+          r[0] *= dsilu_f<T>(xv.x); r[1] *= dsilu_f<T>(xv.y); r[2] *= dsilu_f<T>(xv.z); r[3] *= dsilu_f<T>(xv.w);
+        }
+        V* cp = reinterpret_cast<V*>(C + m * ldc + n);
+        if (epi.accumulate) {
+          const V cv = *cp;
+          r[0] += cv.x; r[1] += cv.y; r[2] += cv.z; r[3] += cv.w;
+        }
+        *cp = V{r[0], r[1], r[2], r[3]};
+      }
+    }
+}
+
+} // namespace
+
+template <typename T>
+int launch_gemm(int64_t M, int N, int K, const T* A, int64_t lda, const T* B, int64_t ldb, T* C, int64_t ldc,
+                const GemmEpi<T>& epi, cudaStream_t st) {
+  if (M <= 0) return 0;
+  // Large problems: 128x128 tiles (8x8 per thread).  Small ones (fewer than ~2 waves of big tiles): 64x64.
+  const int64_t big_tiles = ((M + 127) / 128) * ((N + 127) / 128);
+  if (big_tiles >= 2 * 148 && N >= 128) {
+    dim3 grid((unsigned)((M + 127) / 128), (unsigned)((N + 127) / 128));
+    gemm_k<T, 128, 128, 8, 8, (sizeof(T) == 8 ? 8 : 16)><<<grid, 256, 0, st>>>(M, N, K, A, lda, B, ldb, C, ldc, epi); PNN_KCHECK("gemm_k");
+  } else {
+    dim3 grid((unsigned)((M + 63) / 64), (unsigned)((N + 63) / 64));
+    gemm_k<T, 64, 64, 4, 4, 16><<<grid, 256, 0, st>>>(M, N, K, A, lda, B, ldb, C, ldc, epi); PNN_KCHECK("gemm_k");
+  }
+  return 1;
+}
+
+template int launch_gemm<float>(int64_t, int, int, const float*, int64_t, const float*, int64_t, float*, int64_t,
+                                const GemmEpi<float>&, cudaStream_t);
+template int launch_gemm<double>(int64_t, int, int, const double*, int64_t, const double*, int64_t, double*, int64_t,
+                                 const GemmEpi<double>&, cudaStream_t);
+
+} // namespace pnn

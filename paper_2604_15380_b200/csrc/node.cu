@@ -1,0 +1,331 @@
+// node.cu — per-atom element-wise pieces of the path, FP32 / FP64:
+//   a2 embedding (B2), the non-GEMM parts of the update block a5 (B4: n = sqrt(sum_a Q_a^2 + eps), gated
+//   scalar-vector products) and of its adjoint (R2), a6 multi-head readout + per-structure segmented sum (B5)
+//   and its adjoint (R1), and the final force assembly (R4).  Formulas: SURVEY.md §8(c).
+// All are streaming kernels: one thread per (atom, feature), consecutive threads on consecutive features.
+#include "common.cuh"
+
+namespace pnn {
+
+namespace {
+
+constexpr int RT = 16; // atoms per readout tile
+
+template <typename T>
+__global__ void __launch_bounds__(256) embed_k(int64_t N, int F, int Zmax, const int32_t* __restrict__ Z,
+                                               const T* __restrict__ emb, T* __restrict__ s, int* d_err) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= N * F) return;
+  const int64_t i = idx / F;
+  const int f = (int)(idx % F);
+  int z = Z[i];
+  if (z < 1 || z > Zmax) {
+    if (f == 0) atomicOr(d_err, ERRF_BAD_Z);
+    z = 1;
+  }
+  s[idx] = emb[(int64_t)z * F + f];
+}
+
+// PQ [N][3][2F] (P | Q)  ->  sn[:, F:2F] = sqrt(sum_a Q_a^2 + eps)          (B4)
+template <typename T>
+__global__ void __launch_bounds__(256) norm_k(int64_t N, int F, const T* __restrict__ PQ, T* __restrict__ sn, T eps) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= N * F) return;
+  const int64_t i = idx / F;
+  const int f = (int)(idx % F);
+  const T q0 = PQ[(i * 3 + 0) * 2 * F + F + f], q1 = PQ[(i * 3 + 1) * 2 * F + F + f], q2 = PQ[(i * 3 + 2) * 2 * F + F + f];
+  sn[i * 2 * F + F + f] = sqrt(q0 * q0 + q1 * q1 + q2 * q2 + eps);
+}
+
+// s'' = s' + a_sv <P,Q> + a_ss ;  v'' = v' + a_vv P                          (B4)
+template <typename T>
+__global__ void __launch_bounds__(256) update_k(int64_t N, int F, const T* __restrict__ sn, const T* __restrict__ v1,
+                                                const T* __restrict__ PQ, const T* __restrict__ a,
+                                                T* __restrict__ s_out, T* __restrict__ v_out) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= N * F) return;
+  const int64_t i = idx / F;
+  const int f = (int)(idx % F);
+  const T avv = a[i * 3 * F + f], asv = a[i * 3 * F + F + f], ass = a[i * 3 * F + 2 * F + f];
+  T dot = T(0);
+#pragma unroll
+  for (int ax = 0; ax < 3; ++ax) {
+    const T p = PQ[(i * 3 + ax) * 2 * F + f], q = PQ[(i * 3 + ax) * 2 * F + F + f];
+    dot = fma(p, q, dot);
+    if (v_out) v_out[(i * 3 + ax) * F + f] = fma(avv, p, v1[(i * 3 + ax) * F + f]);
+  }
+  s_out[idx] = sn[i * 2 * F + f] + asv * dot + ass;
+}
+
+// R2, first half: a-bar [N,3F] and the direct parts of P-bar, Q-bar [N][3][2F]
+template <typename T>
+__global__ void __launch_bounds__(256) update_bwd1_k(int64_t N, int F, const T* __restrict__ sb,
+                                                     const T* __restrict__ vb, const T* __restrict__ a,
+                                                     const T* __restrict__ PQ, T* __restrict__ ab,
+                                                     T* __restrict__ PQb) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= N * F) return;
+  const int64_t i = idx / F;
+  const int f = (int)(idx % F);
+  const T sbf = sb[idx];
+  const T avv = a[i * 3 * F + f], asv = a[i * 3 * F + F + f];
+  T p[3], q[3], vbf[3];
+  T dot = T(0), avvb = T(0);
+#pragma unroll
+  for (int ax = 0; ax < 3; ++ax) {
+    p[ax] = PQ[(i * 3 + ax) * 2 * F + f];
+    q[ax] = PQ[(i * 3 + ax) * 2 * F + F + f];
+    vbf[ax] = vb ? vb[(i * 3 + ax) * F + f] : T(0);
+    dot = fma(p[ax], q[ax], dot);
+    avvb = fma(vbf[ax], p[ax], avvb);
+  }
+  ab[i * 3 * F + f] = avvb;
+  ab[i * 3 * F + F + f] = sbf * dot;
+  ab[i * 3 * F + 2 * F + f] = sbf;
+  const T dotb = sbf * asv;
+#pragma unroll
+  for (int ax = 0; ax < 3; ++ax) {
+    PQb[(i * 3 + ax) * 2 * F + f] = vbf[ax] * avv + dotb * q[ax];
+    PQb[(i * 3 + ax) * 2 * F + F + f] = dotb * p[ax];
+  }
+}
+
+// R2, second half: s-bar' = s-bar'' + z-bar[0:F];  Q-bar += n-bar Q / n
+template <typename T>
+__global__ void __launch_bounds__(256) update_bwd2_k(int64_t N, int F, const T* __restrict__ zb,
+                                                     const T* __restrict__ PQ, T eps, T* __restrict__ sb,
+                                                     T* __restrict__ PQb) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= N * F) return;
+  const int64_t i = idx / F;
+  const int f = (int)(idx % F);
+  sb[idx] += zb[i * 2 * F + f];
+  const T nb = zb[i * 2 * F + F + f];
+  const T q0 = PQ[(i * 3 + 0) * 2 * F + F + f], q1 = PQ[(i * 3 + 1) * 2 * F + F + f], q2 = PQ[(i * 3 + 2) * 2 * F + F + f];
+  const T r = nb / sqrt(q0 * q0 + q1 * q1 + q2 * q2 + eps);
+  PQb[(i * 3 + 0) * 2 * F + F + f] += r * q0;
+  PQb[(i * 3 + 1) * 2 * F + F + f] += r * q1;
+  PQb[(i * 3 + 2) * 2 * F + F + f] += r * q2;
+}
+
+// ------------------------------------------------------------------------------------------ readout
+// One CTA per tile of RT consecutive atoms.  Atoms of a structure are contiguous and share a head, so the tile
+// splits into a few runs of equal head; each run is a small [run x F] x [F x F/2] product with the head's W1.
+template <typename T>
+__global__ void __launch_bounds__(128) readout_k(int64_t N, int F, int H, const T* __restrict__ s,
+                                                 const int32_t* __restrict__ a2s, const int32_t* __restrict__ head,
+                                                 const T* __restrict__ W1t, const T* __restrict__ b1,
+                                                 const T* __restrict__ w2, const T* __restrict__ b2,
+                                                 T* __restrict__ opre, T* __restrict__ eatom, int* d_err) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* S = reinterpret_cast<T*>(smem_raw);      // [RT][F]
+  T* Eo = S + RT * F;                         // [RT][Fh]
+  __shared__ int Hs[RT];
+  const int Fh = F / 2;
+  const int64_t i0 = (int64_t)blockIdx.x * RT;
+  const int nt = (int)min((int64_t)RT, N - i0);
+  for (int q = threadIdx.x; q < nt * F; q += blockDim.x) S[q] = s[i0 * F + q];
+  if (threadIdx.x < nt) {
+    int h = head[a2s[i0 + threadIdx.x]];
+    if (h < 0 || h >= H) { atomicOr(d_err, ERRF_BAD_HEAD); h = 0; }
+    Hs[threadIdx.x] = h;
+  }
+  __syncthreads();
+  for (int o = threadIdx.x; o < Fh; o += blockDim.x) {
+    int r0 = 0;
+    while (r0 < nt) {
+      const int h = Hs[r0];
+      int r1 = r0 + 1;
+      while (r1 < nt && Hs[r1] == h) ++r1;
+      T acc[RT];
+#pragma unroll
+      for (int r = 0; r < RT; ++r) acc[r] = T(0);
+      const T* Wp = W1t + (int64_t)h * F * Fh + o;
+      for (int k = 0; k < F; ++k) {
+        const T wv = Wp[(int64_t)k * Fh];
+#pragma unroll
+        for (int r = 0; r < RT; ++r)
+          if (r0 + r < r1) acc[r] = fma(wv, S[(r0 + r) * F + k], acc[r]);
+      }
+      const T bb = b1[h * Fh + o], ww = w2[h * Fh + o];
+#pragma unroll
+      for (int r = 0; r < RT; ++r)
+        if (r0 + r < r1) {
+          const T pre = acc[r] + bb;
+          if (opre) opre[(i0 + r0 + r) * Fh + o] = pre;
+          Eo[(r0 + r) * Fh + o] = ww * silu_f<T>(pre);
+        }
+      r0 = r1;
+    }
+  }
+  __syncthreads();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  for (int r = warp; r < nt; r += 4) {
+    T e = T(0);
+    for (int o = lane; o < Fh; o += 32) e += Eo[r * Fh + o];
+    for (int sft = 16; sft; sft >>= 1) e += __shfl_xor_sync(0xffffffffu, e, sft);
+    if (lane == 0) eatom[i0 + r] = e + b2[Hs[r]];
+  }
+}
+
+// E_g = sum of the structure's atom energies (segmented sum, fixed tree order)
+template <typename T>
+__global__ void __launch_bounds__(128) struct_sum_k(const int32_t* __restrict__ sptr, const T* __restrict__ eatom,
+                                                    T* __restrict__ energy) {
+  const int g = blockIdx.x;
+  const int a0 = sptr[g], a1 = sptr[g + 1];
+  T e = T(0);
+  for (int i = a0 + threadIdx.x; i < a1; i += 128) e += eatom[i];
+  for (int sft = 16; sft; sft >>= 1) e += __shfl_xor_sync(0xffffffffu, e, sft);
+  __shared__ T ws[4];
+  if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = e;
+  __syncthreads();
+  if (threadIdx.x == 0) energy[g] = (ws[0] + ws[1]) + (ws[2] + ws[3]);
+}
+
+// R1: s-bar_i = out_W1^T (out_w2 o silu'(pre_i))
+template <typename T>
+__global__ void __launch_bounds__(256) readout_bwd_k(int64_t N, int F, int H, const T* __restrict__ opre,
+                                                     const int32_t* __restrict__ a2s,
+                                                     const int32_t* __restrict__ head, const T* __restrict__ W1,
+                                                     const T* __restrict__ w2, T* __restrict__ sb) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T* Pb = reinterpret_cast<T*>(smem_raw); // [RT][Fh]
+  __shared__ int Hs[RT];
+  const int Fh = F / 2;
+  const int64_t i0 = (int64_t)blockIdx.x * RT;
+  const int nt = (int)min((int64_t)RT, N - i0);
+  if (threadIdx.x < nt) {
+    int h = head[a2s[i0 + threadIdx.x]];
+    if (h < 0 || h >= H) h = 0;
+    Hs[threadIdx.x] = h;
+  }
+  __syncthreads();
+  for (int q = threadIdx.x; q < nt * Fh; q += blockDim.x) {
+    const int r = q / Fh, o = q % Fh;
+    Pb[q] = w2[Hs[r] * Fh + o] * dsilu_f<T>(opre[(i0 + r) * Fh + o]);
+  }
+  __syncthreads();
+  for (int k = threadIdx.x; k < F; k += blockDim.x) {
+    int r0 = 0;
+    while (r0 < nt) {
+      const int h = Hs[r0];
+      int r1 = r0 + 1;
+      while (r1 < nt && Hs[r1] == h) ++r1;
+      T acc[RT];
+#pragma unroll
+      for (int r = 0; r < RT; ++r) acc[r] = T(0);
+      const T* Wp = W1 + (int64_t)h * Fh * F + k;
+      for (int o = 0; o < Fh; ++o) {
+        const T wv = Wp[(int64_t)o * F];
+#pragma unroll
+        for (int r = 0; r < RT; ++r)
+          if (r0 + r < r1) acc[r] = fma(wv, Pb[(r0 + r) * Fh + o], acc[r]);
+      }
+#pragma unroll
+      for (int r = 0; r < RT; ++r)
+        if (r0 + r < r1) sb[(i0 + r0 + r) * F + k] = acc[r];
+      r0 = r1;
+    }
+  }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) force_assemble_k(int64_t n3, int nslab, const T* __restrict__ fpart,
+                                                        T* __restrict__ forces) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n3) return;
+  T s = T(0);
+  for (int b = 0; b < nslab; ++b) s += fpart[(int64_t)b * n3 + idx];
+  forces[idx] = s;
+}
+
+inline unsigned nblk(int64_t n, int b) { return (unsigned)((n + b - 1) / b); }
+
+} // namespace
+
+template <typename T>
+int launch_embed(int64_t N, int F, int Zmax, const int32_t* Z, const T* emb, T* s, int* d_err, cudaStream_t st) {
+  if (N == 0) return 0;
+  embed_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, Zmax, Z, emb, s, d_err); PNN_KCHECK("embed_k");
+  return 1;
+}
+template <typename T>
+int launch_norm(int64_t N, int F, const T* PQ, T* sn, T eps, cudaStream_t st) {
+  if (N == 0) return 0;
+  norm_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, PQ, sn, eps); PNN_KCHECK("norm_k");
+  return 1;
+}
+template <typename T>
+int launch_update(int64_t N, int F, const T* sn, const T* v1, const T* PQ, const T* a, T* s_out, T* v_out,
+                  cudaStream_t st) {
+  if (N == 0) return 0;
+  update_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, sn, v1, PQ, a, s_out, v_out); PNN_KCHECK("update_k");
+  return 1;
+}
+template <typename T>
+int launch_update_bwd1(int64_t N, int F, const T* sb, const T* vb, const T* a, const T* PQ, T* ab, T* PQb,
+                       cudaStream_t st) {
+  if (N == 0) return 0;
+  update_bwd1_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, sb, vb, a, PQ, ab, PQb); PNN_KCHECK("update_bwd1_k");
+  return 1;
+}
+template <typename T>
+int launch_update_bwd2(int64_t N, int F, const T* zb, const T* PQ, T eps, T* sb, T* PQb, cudaStream_t st) {
+  if (N == 0) return 0;
+  update_bwd2_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, zb, PQ, eps, sb, PQb); PNN_KCHECK("update_bwd2_k");
+  return 1;
+}
+template <typename T>
+int launch_readout(int64_t N, int64_t S, int F, int H, const T* s, const int32_t* a2s, const int32_t* head,
+                   const int32_t* struct_ptr, const T* W1t, const T* b1, const T* w2, const T* b2, T* opre, T* eatom,
+                   T* energy, int* d_err, cudaStream_t st) {
+  int nl = 0;
+  if (N > 0) {
+    const size_t smem = sizeof(T) * (RT * F + RT * (F / 2));
+    static bool attr_set = false;
+    if (!attr_set) {
+      cudaFuncSetAttribute(readout_k<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+      attr_set = true;
+    }
+    readout_k<T><<<nblk(N, RT), 128, smem, st>>>(N, F, H, s, a2s, head, W1t, b1, w2, b2, opre, eatom, d_err); PNN_KCHECK("readout_k");
+    ++nl;
+  }
+  if (S > 0) {
+    struct_sum_k<T><<<(unsigned)S, 128, 0, st>>>(struct_ptr, eatom, energy); PNN_KCHECK("struct_sum_k");
+    ++nl;
+  }
+  return nl;
+}
+template <typename T>
+int launch_readout_bwd(int64_t N, int F, int H, const T* opre, const int32_t* a2s, const int32_t* head, const T* W1,
+                       const T* w2, T* sb, cudaStream_t st) {
+  if (N == 0) return 0;
+  const size_t smem = sizeof(T) * (RT * (F / 2));
+  readout_bwd_k<T><<<nblk(N, RT), F < 256 ? (F < 64 ? 64 : F) : 256, smem, st>>>(N, F, H, opre, a2s, head, W1, w2, sb); PNN_KCHECK("readout_bwd_k");
+  return 1;
+}
+template <typename T>
+int launch_force_assemble(int64_t N, int nslab, const T* fpart, T* forces, cudaStream_t st) {
+  if (N == 0) return 0;
+  force_assemble_k<T><<<nblk(N * 3, 256), 256, 0, st>>>(N * 3, nslab, fpart, forces); PNN_KCHECK("force_assemble_k");
+  return 1;
+}
+
+#define PNN_INST(T)                                                                                                  \
+  template int launch_embed<T>(int64_t, int, int, const int32_t*, const T*, T*, int*, cudaStream_t);                 \
+  template int launch_norm<T>(int64_t, int, const T*, T*, T, cudaStream_t);                                          \
+  template int launch_update<T>(int64_t, int, const T*, const T*, const T*, const T*, T*, T*, cudaStream_t);         \
+  template int launch_update_bwd1<T>(int64_t, int, const T*, const T*, const T*, const T*, T*, T*, cudaStream_t);    \
+  template int launch_update_bwd2<T>(int64_t, int, const T*, const T*, T, T*, T*, cudaStream_t);                     \
+  template int launch_readout<T>(int64_t, int64_t, int, int, const T*, const int32_t*, const int32_t*,               \
+                                 const int32_t*, const T*, const T*, const T*, const T*, T*, T*, T*, int*,           \
+                                 cudaStream_t);                                                                      \
+  template int launch_readout_bwd<T>(int64_t, int, int, const T*, const int32_t*, const int32_t*, const T*,          \
+                                     const T*, T*, cudaStream_t);                                                    \
+  template int launch_force_assemble<T>(int64_t, int, const T*, T*, cudaStream_t);
+PNN_INST(float)
+PNN_INST(double)
+#undef PNN_INST
+
+} // namespace pnn

@@ -1,0 +1,533 @@
+// pnn_api.cu — the C ABI of include/pnn.h: model upload, workspace arena, and the launch sequences of the hot path
+// (SURVEY.md §8(a) a1..a7).  Every step of the path runs in this library's kernels; there is no CPU fallback.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/pnn.h"
+#include "common.cuh"
+#include "gemm_tc.cuh"
+
+using namespace pnn;
+
+namespace {
+thread_local std::string g_last_cuda_error;
+thread_local bool g_launch_failed_flag = false;
+} // namespace
+
+namespace pnn {
+void note_launch(const char* where) {
+  const cudaError_t e = cudaPeekAtLastError();
+  if (e != cudaSuccess && !g_launch_failed_flag) {
+    g_launch_failed_flag = true;
+    g_last_cuda_error = std::string("launch of ") + where + ": " + cudaGetErrorString(e);
+    cudaGetLastError();
+  }
+}
+} // namespace pnn
+
+namespace {
+
+bool cuda_ok(cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return true;
+  g_last_cuda_error = std::string(what) + ": " + cudaGetErrorString(e);
+  return false;
+}
+#define PNN_TRY(call)                                      \
+  do {                                                     \
+    if (!cuda_ok((call), #call)) return PNN_ERR_CUDA;      \
+  } while (0)
+
+bool launch_failed() {
+  const bool f = g_launch_failed_flag;
+  g_launch_failed_flag = false;
+  return f;
+}
+
+size_t elem_size(int prec) { return prec == PNN_FP64 ? 8 : 4; }
+
+bool config_ok(const pnn_config* c) {
+  if (!c) return false;
+  if (c->F < 32 || c->F > 256 || c->F % 32) return false;
+  if (c->T < 1 || c->T > 64 || c->K < 2 || c->K > 32 || c->H < 1 || c->Zmax < 1) return false;
+  if (!(c->cutoff > 0.0) || !(c->norm_eps >= 0.0)) return false;
+  if (c->prec != PNN_BF16 && c->prec != PNN_FP32 && c->prec != PNN_FP64) return false;
+  return true;
+}
+
+int64_t weights_count(const pnn_config* c) {
+  const int64_t F = c->F, K = c->K;
+  const int64_t per_block = 11 * F * F + 3 * F * K + 11 * F;
+  const int64_t per_head = (F / 2) * F + (F / 2) + (F / 2) + 1;
+  return (int64_t)(c->Zmax + 1) * F + c->T * per_block + c->H * per_head;
+}
+
+// element offsets of one block's arrays inside the device weight buffer
+struct BlockW {
+  int64_t W1t, b1, W2t, b2, fltW, fltb, UVt, A1t, c1, A2t, c2; // forward (transposed: [in][out])
+  int64_t A2, A1, UV, W2, W1;                                   // reverse (original: [out][in])
+};
+
+} // namespace
+
+struct pnn_model {
+  pnn_config cfg;
+  void* d_w = nullptr; // all weights, model precision (FP32 for the BF16 model; BF16 copies live in tc)
+  int64_t n_elem = 0;
+  int64_t emb = 0;
+  std::vector<BlockW> blk;
+  int64_t oW1t = 0, oW1 = 0, ob1 = 0, ow2 = 0, ob2 = 0; // heads: [H][F][Fh], [H][Fh][F], [H][Fh], [H][Fh], [H]
+  TcModel* tc = nullptr;                                // BF16 tensor-core operands (gemm_tc.cu), or null
+};
+
+struct pnn_workspace {
+  const pnn_model* model = nullptr;
+  int64_t maxN = 0, maxE = 0, maxS = 0;
+  int want_forces = 0;
+  char* arena = nullptr;
+  int64_t arena_bytes = 0;
+  GraphBuffers g{};
+  int64_t graph_N = -1, graph_S = -1;
+  cudaStream_t graph_stream = nullptr;
+  int64_t launches = 0;
+  // activations (element type = model state type)
+  void *s_cur, *h, *sn, *v1, *k, *vping[2], *eatom, *opre;
+  struct Tape { void *v_in, *hpre, *phi, *PQ, *kpre, *a; };
+  std::vector<Tape> tape;
+  // adjoints
+  void *sb, *vb, *vb2, *ab, *PQb, *kb, *zb, *phib, *hb, *fpart;
+  // staging for pnn_eval_host
+  int32_t *st_Z, *st_sptr, *st_head;
+  double *st_pos, *st_cell;
+  uint8_t* st_pbc;
+  void *st_energy, *st_forces;
+  TcWorkspace* tc = nullptr;
+};
+
+extern "C" {
+
+const char* pnn_status_string(int st) {
+  switch (st) {
+    case PNN_OK: return "ok";
+    case PNN_ERR_INVALID_ARG: return "invalid argument";
+    case PNN_ERR_CAPACITY: return "capacity exceeded (atoms, edges or structures larger than the workspace)";
+    case PNN_ERR_CUDA: return "CUDA error (see pnn_last_cuda_error)";
+    case PNN_ERR_UNSUPPORTED: return "unsupported";
+    case PNN_ERR_NO_GRAPH: return "no graph built for these sizes (call pnn_build_graph first)";
+    case PNN_ERR_BAD_INPUT: return "bad input on device (atomic number or head index out of range)";
+    default: return "unknown status";
+  }
+}
+
+const char* pnn_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
+
+int pnn_weights_count(const pnn_config* cfg, int64_t* n) {
+  if (!config_ok(cfg) || !n) return PNN_ERR_INVALID_ARG;
+  *n = weights_count(cfg);
+  return PNN_OK;
+}
+
+int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, pnn_model** out) {
+  if (!config_ok(cfg) || !w || !out) return PNN_ERR_INVALID_ARG;
+  if (n_scalars != weights_count(cfg)) return PNN_ERR_INVALID_ARG;
+  const int64_t F = cfg->F, K = cfg->K, Fh = F / 2;
+  pnn_model* m = new (std::nothrow) pnn_model();
+  if (!m) return PNN_ERR_INVALID_ARG;
+  m->cfg = *cfg;
+  std::vector<double> hb;
+  auto reserve = [&](int64_t n) {
+    const int64_t off = ((int64_t)hb.size() + 63) / 64 * 64;
+    hb.resize(off + n, 0.0);
+    return off;
+  };
+  auto put = [&](const double* src, int64_t n) {
+    const int64_t off = reserve(n);
+    std::memcpy(hb.data() + off, src, sizeof(double) * n);
+    return off;
+  };
+  auto put_t = [&](const double* src, int64_t rows, int64_t cols) { // src [rows][cols] -> [cols][rows]
+    const int64_t off = reserve(rows * cols);
+    for (int64_t r = 0; r < rows; ++r)
+      for (int64_t c = 0; c < cols; ++c) hb[off + c * rows + r] = src[r * cols + c];
+    return off;
+  };
+  const double* p = w;
+  auto take = [&](int64_t n) { const double* q = p; p += n; return q; };
+  m->emb = put(take((cfg->Zmax + 1) * F), (cfg->Zmax + 1) * F);
+  m->blk.resize(cfg->T);
+  for (int t = 0; t < cfg->T; ++t) {
+    BlockW& b = m->blk[t];
+    const double* W1 = take(F * F);     const double* b1 = take(F);
+    const double* W2 = take(3 * F * F); const double* b2 = take(3 * F);
+    const double* fW = take(3 * F * K); const double* fb = take(3 * F);
+    const double* U = take(F * F);      const double* V = take(F * F);
+    const double* A1 = take(2 * F * F); const double* c1 = take(F);
+    const double* A2 = take(3 * F * F); const double* c2 = take(3 * F);
+    b.W1t = put_t(W1, F, F); b.b1 = put(b1, F);
+    b.W2t = put_t(W2, 3 * F, F); b.b2 = put(b2, 3 * F);
+    b.fltW = put(fW, 3 * F * K); b.fltb = put(fb, 3 * F);
+    { // [U;V] stacked [2F][F] and its transpose [F][2F]
+      std::vector<double> uv(2 * F * F);
+      std::memcpy(uv.data(), U, sizeof(double) * F * F);
+      std::memcpy(uv.data() + F * F, V, sizeof(double) * F * F);
+      b.UV = put(uv.data(), 2 * F * F);
+      b.UVt = put_t(uv.data(), 2 * F, F);
+    }
+    b.A1t = put_t(A1, F, 2 * F); b.c1 = put(c1, F);
+    b.A2t = put_t(A2, 3 * F, F); b.c2 = put(c2, 3 * F);
+    b.A2 = put(A2, 3 * F * F); b.A1 = put(A1, 2 * F * F); b.W2 = put(W2, 3 * F * F); b.W1 = put(W1, F * F);
+  }
+  {
+    const int H = cfg->H;
+    m->oW1t = reserve(H * F * Fh); m->oW1 = reserve(H * Fh * F);
+    m->ob1 = reserve(H * Fh); m->ow2 = reserve(H * Fh); m->ob2 = reserve(H);
+    for (int h = 0; h < H; ++h) {
+      const double* W1 = take(Fh * F); const double* b1 = take(Fh);
+      const double* w2 = take(Fh);     const double* b2 = take(1);
+      for (int64_t o = 0; o < Fh; ++o)
+        for (int64_t k = 0; k < F; ++k) {
+          hb[m->oW1 + (h * Fh + o) * F + k] = W1[o * F + k];
+          hb[m->oW1t + (h * F + k) * Fh + o] = W1[o * F + k];
+        }
+      for (int64_t o = 0; o < Fh; ++o) { hb[m->ob1 + h * Fh + o] = b1[o]; hb[m->ow2 + h * Fh + o] = w2[o]; }
+      hb[m->ob2 + h] = b2[0];
+    }
+  }
+  m->n_elem = (int64_t)hb.size();
+  const size_t es = elem_size(cfg->prec);
+  if (!cuda_ok(cudaMalloc(&m->d_w, m->n_elem * es), "cudaMalloc(weights)")) { delete m; return PNN_ERR_CUDA; }
+  cudaError_t e;
+  if (cfg->prec == PNN_FP64) {
+    e = cudaMemcpy(m->d_w, hb.data(), m->n_elem * 8, cudaMemcpyHostToDevice);
+  } else {
+    std::vector<float> hf(hb.begin(), hb.end());
+    e = cudaMemcpy(m->d_w, hf.data(), m->n_elem * 4, cudaMemcpyHostToDevice);
+  }
+  if (!cuda_ok(e, "cudaMemcpy(weights)")) { cudaFree(m->d_w); delete m; return PNN_ERR_CUDA; }
+  if (cfg->prec == PNN_BF16) {
+    const int rc = tc_model_create(cfg, w, &m->tc);
+    if (rc != PNN_OK) { cudaFree(m->d_w); delete m; return rc; }
+  }
+  *out = m;
+  return PNN_OK;
+}
+
+void pnn_model_destroy(pnn_model* m) {
+  if (!m) return;
+  if (m->tc) tc_model_destroy(m->tc);
+  cudaFree(m->d_w);
+  delete m;
+}
+
+int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t maxS, int want_forces,
+                         pnn_workspace** out) {
+  if (!m || !out || maxN < 0 || maxE < 0 || maxS < 0) return PNN_ERR_INVALID_ARG;
+  if (maxN > 0x7fffffffLL / 32 || maxE > 0x7fffffffLL - 64 || maxS > 0x7fffffffLL - 64) return PNN_ERR_CAPACITY;
+  pnn_workspace* ws = new (std::nothrow) pnn_workspace();
+  if (!ws) return PNN_ERR_INVALID_ARG;
+  ws->model = m; ws->maxN = maxN; ws->maxE = maxE; ws->maxS = maxS; ws->want_forces = want_forces ? 1 : 0;
+  const int64_t F = m->cfg.F, T = m->cfg.T;
+  const size_t es = elem_size(m->cfg.prec);
+  const int64_t N = maxN > 0 ? maxN : 1, E = maxE > 0 ? maxE : 1, S = maxS > 0 ? maxS : 1;
+  // two passes over the same carving code: first to size the arena, then to assign pointers
+  for (int pass = 0; pass < 2; ++pass) {
+    int64_t off = 0;
+    auto carve = [&](int64_t bytes) -> void* {
+      const int64_t o = off;
+      off += (bytes + 255) / 256 * 256;
+      return pass ? (void*)(ws->arena + o) : nullptr;
+    };
+    GraphBuffers& g = ws->g;
+    g.a2s = (int32_t*)carve(4 * N);
+    g.desc = (GridDesc*)carve(sizeof(GridDesc) * S);
+    g.ncell = (int32_t*)carve(4 * (S + 1));
+    g.cell_off = (int32_t*)carve(4 * (S + 1));
+    g.cid = (int32_t*)carve(4 * N);
+    g.cell_cnt = (int32_t*)carve(4 * (N + S + 2));
+    g.cell_start = (int32_t*)carve(4 * (N + S + 2));
+    g.cell_fill = (int32_t*)carve(4 * (N + S + 2));
+    g.sorted = (int32_t*)carve(4 * N);
+    g.deg = (int32_t*)carve(4 * (N + 1));
+    g.rowptr = (int32_t*)carve(4 * (N + 1));
+    g.col = (int32_t*)carve(4 * E);
+    g.shift = (int8_t*)carve(3 * E);
+    g.geom = carve(4 * es * E);
+    g.scan_tmp = (int32_t*)carve(4 * ((N + S + 2) / 1024 + 4));
+    g.d_err = (int*)carve(256);
+    g.max_edges = maxE;
+    ws->s_cur = carve(es * N * F);
+    ws->h = carve(es * N * F);
+    ws->sn = carve(es * N * 2 * F);
+    ws->v1 = carve(es * N * 3 * F);
+    ws->k = carve(es * N * F);
+    ws->eatom = carve(es * N);
+    ws->tape.resize(want_forces ? T : 1);
+    if (want_forces) {
+      ws->opre = carve(es * N * (F / 2));
+      for (int t = 0; t < T; ++t) {
+        pnn_workspace::Tape& tp = ws->tape[t];
+        tp.v_in = (t == 0) ? nullptr : carve(es * N * 3 * F);
+        tp.hpre = carve(es * N * F);
+        tp.phi = carve(es * N * 3 * F);
+        tp.PQ = carve(es * N * 6 * F);
+        tp.kpre = carve(es * N * F);
+        tp.a = carve(es * N * 3 * F);
+      }
+      ws->vping[0] = ws->vping[1] = nullptr;
+      ws->sb = carve(es * N * F);
+      ws->vb = carve(es * N * 3 * F);
+      ws->vb2 = carve(es * N * 3 * F);
+      ws->ab = carve(es * N * 3 * F);
+      ws->PQb = carve(es * N * 6 * F);
+      ws->kb = carve(es * N * F);
+      ws->zb = carve(es * N * 2 * F);
+      ws->phib = carve(es * N * 3 * F);
+      ws->hb = carve(es * N * F);
+      ws->fpart = carve(es * N * 3 * edge_num_slabs((int)F));
+    } else {
+      ws->opre = nullptr;
+      pnn_workspace::Tape& tp = ws->tape[0];
+      tp.v_in = nullptr;
+      tp.hpre = nullptr;
+      tp.phi = carve(es * N * 3 * F);
+      tp.PQ = carve(es * N * 6 * F);
+      tp.kpre = nullptr;
+      tp.a = carve(es * N * 3 * F);
+      ws->vping[0] = carve(es * N * 3 * F);
+      ws->vping[1] = carve(es * N * 3 * F);
+      ws->sb = ws->vb = ws->vb2 = ws->ab = ws->PQb = ws->kb = ws->zb = ws->phib = ws->hb = ws->fpart = nullptr;
+    }
+    ws->st_Z = (int32_t*)carve(4 * N);
+    ws->st_sptr = (int32_t*)carve(4 * (S + 1));
+    ws->st_head = (int32_t*)carve(4 * S);
+    ws->st_pos = (double*)carve(24 * N);
+    ws->st_cell = (double*)carve(72 * S);
+    ws->st_pbc = (uint8_t*)carve(3 * S);
+    ws->st_energy = carve(es * S);
+    ws->st_forces = carve(es * 3 * N);
+    if (pass == 0) {
+      ws->arena_bytes = off;
+      if (!cuda_ok(cudaMalloc((void**)&ws->arena, off), "cudaMalloc(workspace)")) { delete ws; return PNN_ERR_CUDA; }
+      if (!cuda_ok(cudaMemset(ws->arena, 0, off), "cudaMemset(workspace)")) {
+        cudaFree(ws->arena); delete ws; return PNN_ERR_CUDA;
+      }
+    }
+  }
+  if (m->cfg.prec == PNN_BF16) {
+    const int rc = tc_workspace_create(m->tc, N, &ws->tc);
+    if (rc != PNN_OK) { cudaFree(ws->arena); delete ws; return rc; }
+  }
+  *out = ws;
+  return PNN_OK;
+}
+
+void pnn_workspace_destroy(pnn_workspace* ws) {
+  if (!ws) return;
+  if (ws->tc) tc_workspace_destroy(ws->tc);
+  cudaFree(ws->arena);
+  delete ws;
+}
+
+int64_t pnn_workspace_bytes(const pnn_workspace* ws) { return ws ? ws->arena_bytes + (ws->tc ? tc_workspace_bytes(ws->tc) : 0) : 0; }
+int64_t pnn_launch_count(const pnn_workspace* ws) { return ws ? ws->launches : 0; }
+
+int pnn_build_graph(pnn_workspace* ws, int64_t N, int64_t S, const double* pos, const int32_t* sptr,
+                    const double* cell, const uint8_t* pbc, void* stream) {
+  if (!ws || N < 0 || S < 0) return PNN_ERR_INVALID_ARG;
+  if (N > ws->maxN || S > ws->maxS) return PNN_ERR_CAPACITY;
+  if ((N > 0 && !pos) || !sptr) return PNN_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  ws->launches += launch_graph_build(ws->g, N, S, pos, sptr, cell, pbc, ws->model->cfg.cutoff, ws->model->cfg.prec, st);
+  ws->graph_N = N; ws->graph_S = S; ws->graph_stream = st;
+  if (launch_failed()) return PNN_ERR_CUDA;
+  PNN_TRY(cudaGetLastError());
+  return PNN_OK;
+}
+
+int pnn_graph_view(const pnn_workspace* ws, const int32_t** rowptr, const int32_t** col, const int8_t** shift,
+                   int64_t* n_edges) {
+  if (!ws) return PNN_ERR_INVALID_ARG;
+  if (ws->graph_N < 0) return PNN_ERR_NO_GRAPH;
+  if (rowptr) *rowptr = ws->g.rowptr;
+  if (col) *col = ws->g.col;
+  if (shift) *shift = ws->g.shift;
+  if (n_edges) {
+    PNN_TRY(cudaStreamSynchronize(ws->graph_stream));
+    int32_t e = 0;
+    PNN_TRY(cudaMemcpy(&e, ws->g.rowptr + ws->graph_N, 4, cudaMemcpyDeviceToHost));
+    *n_edges = e;
+    if (e > ws->maxE) return PNN_ERR_CAPACITY;
+  }
+  return PNN_OK;
+}
+
+int pnn_graph_copy(const pnn_workspace* ws, int32_t* rowptr, int32_t* col, int8_t* shift) {
+  if (!ws) return PNN_ERR_INVALID_ARG;
+  int64_t E = 0;
+  const int rc = pnn_graph_view(ws, nullptr, nullptr, nullptr, &E);
+  if (rc != PNN_OK) return rc;
+  if (rowptr) PNN_TRY(cudaMemcpy(rowptr, ws->g.rowptr, 4 * (ws->graph_N + 1), cudaMemcpyDefault));
+  if (col && E > 0) PNN_TRY(cudaMemcpy(col, ws->g.col, 4 * E, cudaMemcpyDefault));
+  if (shift && E > 0) PNN_TRY(cudaMemcpy(shift, ws->g.shift, 3 * E, cudaMemcpyDefault));
+  return PNN_OK;
+}
+
+int pnn_check_async_errors(pnn_workspace* ws) {
+  if (!ws) return PNN_ERR_INVALID_ARG;
+  PNN_TRY(cudaDeviceSynchronize());
+  int flags = 0;
+  PNN_TRY(cudaMemcpy(&flags, ws->g.d_err, 4, cudaMemcpyDeviceToHost));
+  PNN_TRY(cudaMemset(ws->g.d_err, 0, 4));
+  if (flags & ERRF_EDGE_OVERFLOW) return PNN_ERR_CAPACITY;
+  if (flags & (ERRF_BAD_Z | ERRF_BAD_HEAD)) return PNN_ERR_BAD_INPUT;
+  return PNN_OK;
+}
+
+} // extern "C"
+
+// ------------------------------------------------------------------------------------------------ the path
+namespace {
+
+template <typename T>
+int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const int32_t* sptr,
+              const int32_t* head, int flags, T* energy, T* forces, cudaStream_t st) {
+  const pnn_config& c = m->cfg;
+  const int F = c.F, T_ = c.T;
+  const bool want_f = (flags & PNN_FORCES) != 0;
+  const T* W = (const T*)m->d_w;
+  int nl = 0;
+  EdgeArgs<T> ea;
+  ea.N = N; ea.F = F; ea.K = c.K; ea.rc = c.cutoff;
+  ea.rowptr = ws->g.rowptr; ea.col = ws->g.col; ea.geom = (const Geom<T>*)ws->g.geom; ea.d_err = ws->g.d_err;
+  T* s_cur = (T*)ws->s_cur; T* h = (T*)ws->h; T* sn = (T*)ws->sn; T* v1 = (T*)ws->v1; T* k = (T*)ws->k;
+  const bool taped = ws->want_forces != 0;
+
+  nl += launch_embed<T>(N, F, c.Zmax, Z, W + m->emb, s_cur, ws->g.d_err, st);
+  for (int t = 0; t < T_; ++t) {
+    const BlockW& b = m->blk[t];
+    const pnn_workspace::Tape& tp = ws->tape[taped ? t : 0];
+    const T* v_in;
+    T* v_out;
+    if (taped) {
+      v_in = (const T*)tp.v_in;
+      v_out = (t + 1 < T_) ? (T*)ws->tape[t + 1].v_in : nullptr;
+    } else {
+      v_in = (t == 0) ? nullptr : (const T*)ws->vping[(t - 1) & 1];
+      v_out = (t + 1 < T_) ? (T*)ws->vping[t & 1] : nullptr;
+    }
+    T* phi = (T*)tp.phi; T* PQ = (T*)tp.PQ; T* a = (T*)tp.a;
+    GemmEpi<T> e1; e1.bias = W + b.b1; e1.act = ACT_SILU; e1.pre = (T*)tp.hpre; e1.ldpre = F;
+    nl += launch_gemm<T>(N, F, F, s_cur, F, W + b.W1t, F, h, F, e1, st);                 // B3a, first Linear + SiLU
+    GemmEpi<T> e2; e2.bias = W + b.b2;
+    nl += launch_gemm<T>(N, 3 * F, F, h, F, W + b.W2t, 3 * F, phi, 3 * F, e2, st);       // B3a, second Linear
+    ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
+    nl += launch_edge_fwd<T>(ea, phi, s_cur, F, v_in, sn, 2 * F, v1, st);                // B3b -> s' in sn[:, :F], v'
+    GemmEpi<T> e3;
+    nl += launch_gemm<T>(3 * N, 2 * F, F, v1, F, W + b.UVt, 2 * F, PQ, 2 * F, e3, st);   // B4: P | Q
+    nl += launch_norm<T>(N, F, PQ, sn, (T)c.norm_eps, st);                               // n -> sn[:, F:]
+    GemmEpi<T> e4; e4.bias = W + b.c1; e4.act = ACT_SILU; e4.pre = (T*)tp.kpre; e4.ldpre = F;
+    nl += launch_gemm<T>(N, F, 2 * F, sn, 2 * F, W + b.A1t, F, k, F, e4, st);
+    GemmEpi<T> e5; e5.bias = W + b.c2;
+    nl += launch_gemm<T>(N, 3 * F, F, k, F, W + b.A2t, 3 * F, a, 3 * F, e5, st);
+    nl += launch_update<T>(N, F, sn, v1, PQ, a, s_cur, v_out, st);
+  }
+  nl += launch_readout<T>(N, S, F, c.H, s_cur, ws->g.a2s, head, sptr, W + m->oW1t, W + m->ob1, W + m->ow2,
+                          W + m->ob2, (T*)ws->opre, (T*)ws->eatom, energy, ws->g.d_err, st);
+  if (want_f) {
+    T* sb = (T*)ws->sb; T* vb = (T*)ws->vb; T* vb2 = (T*)ws->vb2; T* ab = (T*)ws->ab; T* PQb = (T*)ws->PQb;
+    T* kb = (T*)ws->kb; T* zb = (T*)ws->zb; T* phib = (T*)ws->phib; T* hb = (T*)ws->hb; T* fpart = (T*)ws->fpart;
+    nl += launch_readout_bwd<T>(N, F, c.H, (const T*)ws->opre, ws->g.a2s, head, W + m->oW1, W + m->ow2, sb, st); // R1
+    for (int t = T_ - 1; t >= 0; --t) {
+      const BlockW& b = m->blk[t];
+      const pnn_workspace::Tape& tp = ws->tape[t];
+      const bool last = (t == T_ - 1);
+      // R2
+      nl += launch_update_bwd1<T>(N, F, sb, last ? nullptr : vb, (const T*)tp.a, (const T*)tp.PQ, ab, PQb, st);
+      GemmEpi<T> g1; g1.act = ACT_MUL_DSILU; g1.aux = (const T*)tp.kpre; g1.ldaux = F;
+      nl += launch_gemm<T>(N, F, 3 * F, ab, 3 * F, W + b.A2, F, kb, F, g1, st);
+      GemmEpi<T> g2;
+      nl += launch_gemm<T>(N, 2 * F, F, kb, F, W + b.A1, 2 * F, zb, 2 * F, g2, st);
+      nl += launch_update_bwd2<T>(N, F, zb, (const T*)tp.PQ, (T)c.norm_eps, sb, PQb, st);
+      GemmEpi<T> g3; g3.accumulate = last ? 0 : 1;
+      nl += launch_gemm<T>(3 * N, F, 2 * F, PQb, 2 * F, W + b.UV, F, vb, F, g3, st);
+      // R3 + R4
+      ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
+      nl += launch_edge_bwd<T>(ea, (const T*)tp.phi, (const T*)tp.v_in, sb, vb, t > 0 ? phib : nullptr, vb2, fpart,
+                               last ? 1 : 0, st);
+      if (t > 0) {
+        GemmEpi<T> g4; g4.act = ACT_MUL_DSILU; g4.aux = (const T*)tp.hpre; g4.ldaux = F;
+        nl += launch_gemm<T>(N, F, 3 * F, phib, 3 * F, W + b.W2, F, hb, F, g4, st);
+        GemmEpi<T> g5; g5.accumulate = 1;
+        nl += launch_gemm<T>(N, F, F, hb, F, W + b.W1, F, sb, F, g5, st);
+        T* tmp = vb; vb = vb2; vb2 = tmp;
+      }
+    }
+    nl += launch_force_assemble<T>(N, edge_num_slabs(F), fpart, forces, st);
+  }
+  ws->launches += nl;
+  return PNN_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+int pnn_eval(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const double* pos,
+             const int32_t* sptr, const int32_t* head, int flags, void* energy, void* forces, void* stream) {
+  (void)pos;
+  if (!m || !ws || ws->model != m || N < 0 || S < 0) return PNN_ERR_INVALID_ARG;
+  if (!(flags & (PNN_ENERGY | PNN_FORCES))) return PNN_ERR_INVALID_ARG;
+  if (N > ws->maxN || S > ws->maxS) return PNN_ERR_CAPACITY;
+  if ((N > 0 && !Z) || !sptr || (S > 0 && (!head || !energy))) return PNN_ERR_INVALID_ARG;
+  if ((flags & PNN_FORCES) && (!ws->want_forces || (N > 0 && !forces))) return PNN_ERR_INVALID_ARG;
+  if (ws->graph_N != N || ws->graph_S != S) return PNN_ERR_NO_GRAPH;
+  cudaStream_t st = (cudaStream_t)stream;
+  int rc;
+  if (m->cfg.prec == PNN_FP64)
+    rc = eval_simt<double>(m, ws, N, S, Z, sptr, head, flags, (double*)energy, (double*)forces, st);
+  else if (m->cfg.prec == PNN_FP32)
+    rc = eval_simt<float>(m, ws, N, S, Z, sptr, head, flags, (float*)energy, (float*)forces, st);
+  else
+    return PNN_ERR_UNSUPPORTED;
+  if (rc != PNN_OK) return rc;
+  if (launch_failed()) return PNN_ERR_CUDA;
+  PNN_TRY(cudaGetLastError());
+  return PNN_OK;
+}
+
+int pnn_eval_host(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const double* pos,
+                  const int32_t* sptr, const int32_t* head, const double* cell, const uint8_t* pbc, int flags,
+                  void* energy_host, void* forces_host, void* stream) {
+  if (!m || !ws || N < 0 || S < 0) return PNN_ERR_INVALID_ARG;
+  if (N > ws->maxN || S > ws->maxS) return PNN_ERR_CAPACITY;
+  if ((N > 0 && (!Z || !pos)) || !sptr || (S > 0 && (!head || !energy_host))) return PNN_ERR_INVALID_ARG;
+  if ((flags & PNN_FORCES) && N > 0 && !forces_host) return PNN_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t es = elem_size(m->cfg.prec);
+  if (N > 0) {
+    PNN_TRY(cudaMemcpyAsync(ws->st_Z, Z, 4 * N, cudaMemcpyHostToDevice, st));
+    PNN_TRY(cudaMemcpyAsync(ws->st_pos, pos, 24 * N, cudaMemcpyHostToDevice, st));
+  }
+  PNN_TRY(cudaMemcpyAsync(ws->st_sptr, sptr, 4 * (S + 1), cudaMemcpyHostToDevice, st));
+  if (S > 0) PNN_TRY(cudaMemcpyAsync(ws->st_head, head, 4 * S, cudaMemcpyHostToDevice, st));
+  const bool periodic = cell && pbc && S > 0;
+  if (periodic) {
+    PNN_TRY(cudaMemcpyAsync(ws->st_cell, cell, 72 * S, cudaMemcpyHostToDevice, st));
+    PNN_TRY(cudaMemcpyAsync(ws->st_pbc, pbc, 3 * S, cudaMemcpyHostToDevice, st));
+  }
+  int rc = pnn_build_graph(ws, N, S, ws->st_pos, ws->st_sptr, periodic ? ws->st_cell : nullptr,
+                           periodic ? ws->st_pbc : nullptr, stream);
+  if (rc != PNN_OK) return rc;
+  rc = pnn_eval(m, ws, N, S, ws->st_Z, ws->st_pos, ws->st_sptr, ws->st_head, flags, ws->st_energy, ws->st_forces,
+                stream);
+  if (rc != PNN_OK) return rc;
+  if (S > 0) PNN_TRY(cudaMemcpyAsync(energy_host, ws->st_energy, es * S, cudaMemcpyDeviceToHost, st));
+  if ((flags & PNN_FORCES) && N > 0)
+    PNN_TRY(cudaMemcpyAsync(forces_host, ws->st_forces, es * 3 * N, cudaMemcpyDeviceToHost, st));
+  PNN_TRY(cudaStreamSynchronize(st));
+  return PNN_OK;
+}
+
+} // extern "C"

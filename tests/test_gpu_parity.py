@@ -1,0 +1,171 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the FP64 CPU oracle, element by element on the
+same seeded inputs.  Tolerances are BASELINE.json's: edge sets bit-exact after canonical sort; energies/forces
+relative 1e-10 (FP64), 1e-5 / 1e-4 (FP32), 2e-2 (BF16), with the denominators of DESIGN.md reading Q20."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import gen
+import oracle
+from gpu_common import gpu_edge_set, run_gpu
+from helpers import edge_set, energy_rel_err, force_rel_err, single
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"fp64": (1e-10, 1e-10), "fp32": (1e-5, 1e-4), "bf16": (2e-2, 2e-2)}
+
+
+def big_molecule(n=400, seed=7):
+    """One non-periodic 'molecule' large enough for the multi-cell (non-periodic) branch of the cell list."""
+    c = dict(gen.CONFIGS[2])
+    return gen.make_molecules(2, [1000 + seed], n, n, density=0.05, box=None, z_choices=np.arange(1, 87), H=16,
+                              cutoff=5.0, seed=gen.BASE_SEED)
+
+
+def check_graph(batch, rc, out):
+    nb = oracle.neighbours(batch, rc)
+    assert np.array_equal(out["rowptr"], nb["rowptr"])
+    assert gpu_edge_set(out["rowptr"], out["col"], out["shift"]) == edge_set(nb)
+    assert len(out["col"]) == len(nb["send"])           # no duplicates
+    return len(nb["send"])
+
+
+def check_values(mc, w, batch, out, precision, forces=True):
+    ref = oracle.evaluate(mc, w, batch, forces=forces)
+    te, tf = TOL[precision]
+    ee = energy_rel_err(out["energy"], ref["energy"])
+    assert ee.max(initial=0.0) < te, f"energy rel err {ee.max()} ({precision})"
+    if forces:
+        fe = force_rel_err(out["forces"], ref["forces"], batch.struct_ptr)
+        assert fe.max(initial=0.0) < tf, f"force rel err {fe.max()} ({precision})"
+    return ref
+
+
+# ------------------------------------------------------------------------------------------- graphs (a1)
+@pytest.mark.parametrize("case", ["cfg1", "cfg2", "cfg3", "cfg5_small", "bigmol", "mixed"])
+def test_graph_bit_exact(case):
+    if case == "cfg1":
+        b, rc = gen.make_batch(1), 5.0
+    elif case == "cfg2":
+        b, rc = gen.make_batch(2, 0, 64), 5.0
+    elif case == "cfg3":
+        b, rc = gen.make_batch(3, 0, 6), 6.0
+    elif case == "cfg5_small":
+        b, rc = gen.make_batch(5, n_atoms=3000), 5.0          # L = 33.5 A: 6 cells per axis, periodic wrap
+    elif case == "bigmol":
+        b, rc = big_molecule(700), 5.0                        # 24 A cube: 4 cells per axis, clipped stencil
+    else:
+        b = gen.concat_batches([gen.make_batch(2, 0, 5), gen.make_batch(5, n_atoms=1500), big_molecule(300),
+                                gen.make_batch(3, 0, 2), gen.make_batch(2, 5, 3)])
+        rc = 5.0
+    mc = dataclasses.replace(gen.model_cfg(1), cutoff=rc, H=16)
+    out = run_gpu(mc, gen.make_weights(mc, 1), b, "fp32", forces=False, want_graph=True)
+    E = check_graph(b, rc, out)
+    assert E > 0
+
+
+def test_graph_partial_pbc_and_triclinic():
+    rng = np.random.default_rng(5)
+    n = 600
+    C = np.array([[30.0, 0.0, 0.0], [6.0, 28.0, 0.0], [0.0, 0.0, 40.0]])
+    pos = rng.uniform(0, 1, (n, 3)) @ C
+    pos[:, 2] = rng.uniform(0, 22.0, n)                        # slab: z not periodic
+    b = single(rng.integers(1, 87, n), pos, 0, C, [1, 1, 0])
+    mc = dataclasses.replace(gen.model_cfg(1), cutoff=5.0)
+    out = run_gpu(mc, gen.make_weights(mc, 1), b, "fp64", forces=False, want_graph=True)
+    check_graph(b, 5.0, out)
+
+
+# ------------------------------------------------------------------------------------------- values
+def test_cfg1_fp64_against_oracle_and_golden():
+    mc, b = gen.model_cfg(1), gen.make_batch(1)
+    w = gen.make_weights(mc, 1)
+    out = run_gpu(mc, w, b, "fp64", want_graph=True)
+    check_graph(b, mc.cutoff, out)
+    check_values(mc, w, b, out, "fp64")
+    import os
+    gold = np.load(os.path.join(os.path.dirname(__file__), "golden", "cfg1_oracle.npz"))
+    assert np.abs(out["energy"] - gold["energy"]).max() < 1e-10 * np.abs(gold["energy"]).max()
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_cfg2_molecular(precision):
+    mc, b = gen.model_cfg(2), gen.make_batch(2, 0, 48)
+    w = gen.make_weights(mc, 2)
+    out = run_gpu(mc, w, b, precision)
+    check_values(mc, w, b, out, precision)
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_cfg3_crystals(precision):
+    mc, b = gen.model_cfg(3), gen.make_batch(3, 0, 3)
+    w = gen.make_weights(mc, 3)
+    out = run_gpu(mc, w, b, precision)
+    check_values(mc, w, b, out, precision)
+
+
+def test_cfg5_scaled_fp64():
+    mc, b = gen.model_cfg(5), gen.make_batch(5, n_atoms=1200)
+    w = gen.make_weights(mc, 5)
+    out = run_gpu(mc, w, b, "fp64")
+    check_values(mc, w, b, out, "fp64")
+
+
+def test_energy_only_workspace_matches():
+    mc, b = gen.model_cfg(2), gen.make_batch(2, 100, 16)
+    w = gen.make_weights(mc, 2)
+    out = run_gpu(mc, w, b, "fp64", forces=False)
+    check_values(mc, w, b, out, "fp64", forces=False)
+
+
+# ------------------------------------------------------------------------------------------- edge cases
+def test_degenerate_structures():
+    """single atoms (no edges), an isolated pair beyond the cutoff, an empty structure, ragged sizes."""
+    mc = dataclasses.replace(gen.model_cfg(1), H=3)
+    w = gen.make_weights(mc, 9)
+    parts = [single([6], [[0.0, 0.0, 0.0]], 0), single([1, 8], [[0, 0, 0], [0, 0, 9.0]], 1),
+             gen.Batch(np.zeros(0, np.int32), np.zeros((0, 3)), np.array([0, 0], np.int32), np.array([2], np.int32)),
+             single([1, 1, 8], [[0, 0, 0], [0.96, 0, 0], [-0.24, 0.93, 0]], 2), single([7], [[1.0, 2.0, 3.0]], 1)]
+    b = gen.concat_batches(parts)
+    out = run_gpu(mc, w, b, "fp64", want_graph=True)
+    assert check_graph(b, mc.cutoff, out) == 6
+    ref = check_values(mc, w, b, out, "fp64")
+    assert out["energy"][2] == 0.0 == ref["energy"][2]
+    assert np.abs(out["forces"][:3]).max() == 0.0            # no neighbours: exactly zero force
+
+
+def test_empty_batch():
+    mc = gen.model_cfg(1)
+    b = gen.Batch(np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(1, np.int32), np.zeros(0, np.int32))
+    out = run_gpu(mc, gen.make_weights(mc, 1), b, "fp32")
+    assert out["energy"].shape == (0,) and out["forces"].shape == (0, 3)
+
+
+def test_error_reporting():
+    import paper_2604_15380_b200 as pnn
+    mc, b = gen.model_cfg(1), gen.make_batch(1)
+    w = gen.make_weights(mc, 1)
+    with pytest.raises(pnn.PnnError) as ei:                   # edge capacity overflow, detected on the device
+        run_gpu(mc, w, b, "fp64", max_edges=100)
+    assert ei.value.status == -2
+    bad = dataclasses.replace(b, Z=np.where(np.arange(b.n_atoms) == 5, 99, b.Z).astype(np.int32))
+    with pytest.raises(pnn.PnnError) as ei:
+        run_gpu(mc, w, bad, "fp64")
+    assert ei.value.status == -6
+    with pytest.raises(pnn.PnnError):                         # F not a multiple of 32
+        pnn.pnn_weights_count(pnn.pnn_config(48, 2, 20, 1, 86, 5.0, 1e-8, pnn.PNN_FP32))
+
+
+def test_host_entry_point_matches_device_entry_point():
+    from gpu_common import make_model, to_device
+    import torch
+    mc, b = gen.model_cfg(2), gen.make_batch(2, 7, 9)
+    w = gen.make_weights(mc, 2)
+    net = make_model(mc, w, "fp32", b.n_atoms, b.n_atoms * 64, b.n_structs)
+    t = to_device(b)
+    e, f = net.eval(t["Z"], t["pos"], t["struct_ptr"], t["head"])
+    torch.cuda.synchronize()
+    eh, fh = net.eval_host(b.Z, b.pos, b.struct_ptr, b.head)
+    assert np.array_equal(e.cpu().numpy(), eh) and np.array_equal(f.cpu().numpy(), fh)
+    net.close()
