@@ -121,6 +121,13 @@ int pnn_eval_host(const pnn_model* m, pnn_workspace* ws, int64_t n_atoms, int64_
  * clears them.  Synchronises the device. */
 int pnn_check_async_errors(pnn_workspace* ws);
 
+/* Optional per-kernel-family timing: when enabled, pnn_build_graph / pnn_eval bracket each kernel family with CUDA
+ * events on the launch stream.  pnn_profile_read synchronises the device, aggregates the records since the last
+ * read by family name (names: max_entries x 32 bytes, NUL-padded; total_ms; launches) and clears them. */
+int pnn_profile_enable(pnn_workspace* ws, int on);
+int pnn_profile_read(pnn_workspace* ws, int max_entries, char* names, double* total_ms, int64_t* launches,
+                     int* n_entries);
+
 /* Number of kernels the library has launched on behalf of this workspace since it was created. */
 int64_t pnn_launch_count(const pnn_workspace* ws);
 

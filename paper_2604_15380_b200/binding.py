@@ -16,7 +16,8 @@ __all__ = [
     "PNN_OK", "PNN_BF16", "PNN_FP32", "PNN_FP64", "PNN_ENERGY", "PNN_FORCES", "PnnError", "pnn_config", "lib",
     "lib_path", "pnn_status_string", "pnn_last_cuda_error", "pnn_weights_count", "pnn_model_create",
     "pnn_model_destroy", "pnn_workspace_create", "pnn_workspace_destroy", "pnn_workspace_bytes", "pnn_build_graph",
-    "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_eval_host", "pnn_check_async_errors", "pnn_launch_count",
+    "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_eval_host", "pnn_check_async_errors", "pnn_launch_count", "pnn_profile_enable",
+    "pnn_profile_read",
     "PaiNN", "PRECISIONS",
 ]
 
@@ -78,6 +79,8 @@ def lib():
         L.pnn_eval.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, i32, vp, vp, vp]
         L.pnn_eval_host.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp]
         L.pnn_check_async_errors.argtypes = [vp]
+        L.pnn_profile_enable.argtypes = [vp, i32]
+        L.pnn_profile_read.argtypes = [vp, i32, vp, vp, vp, ctypes.POINTER(i32)]
         L.pnn_launch_count.argtypes = [vp]
         L.pnn_launch_count.restype = i64
         _lib = L
@@ -178,6 +181,21 @@ def pnn_check_async_errors(ws: int) -> None:
 
 def pnn_launch_count(ws: int) -> int:
     return lib().pnn_launch_count(ws)
+
+
+def pnn_profile_enable(ws: int, on: bool) -> None:
+    _check(lib().pnn_profile_enable(ws, int(bool(on))), "pnn_profile_enable")
+
+
+def pnn_profile_read(ws: int, max_entries: int = 32) -> dict:
+    """{family: (total_ms, launches)} since the last read."""
+    names = ctypes.create_string_buffer(32 * max_entries)
+    ms = (ctypes.c_double * max_entries)()
+    nl = (ctypes.c_int64 * max_entries)()
+    n = ctypes.c_int(0)
+    _check(lib().pnn_profile_read(ws, max_entries, ctypes.addressof(names), ctypes.addressof(ms),
+                                  ctypes.addressof(nl), ctypes.byref(n)), "pnn_profile_read")
+    return {names.raw[32 * q:32 * q + 32].split(b"\0")[0].decode(): (ms[q], nl[q]) for q in range(n.value)}
 
 
 class PaiNN:

@@ -104,7 +104,32 @@ struct pnn_workspace {
   uint8_t* st_pbc;
   void *st_energy, *st_forces;
   TcWorkspace* tc = nullptr;
+  // optional per-kernel-family timing (pnn_profile_enable)
+  bool profile = false;
+  struct ProfRec { const char* name; cudaEvent_t a, b; int launches; };
+  std::vector<ProfRec> prof;
+  std::vector<cudaEvent_t> ev_pool;
 };
+
+namespace {
+// Brackets the launches of one kernel family with CUDA events on the launch stream when profiling is on.
+struct ProfScope {
+  pnn_workspace* ws; cudaStream_t st; const char* name; int64_t l0; cudaEvent_t a = nullptr;
+  ProfScope(pnn_workspace* w, cudaStream_t s, const char* n) : ws(w), st(s), name(n), l0(0) {
+    if (!ws->profile) return;
+    a = take(); cudaEventRecord(a, st);
+  }
+  cudaEvent_t take() {
+    if (!ws->ev_pool.empty()) { cudaEvent_t e = ws->ev_pool.back(); ws->ev_pool.pop_back(); return e; }
+    cudaEvent_t e; cudaEventCreate(&e); return e;
+  }
+  void done(int launches) {
+    if (!ws->profile) return;
+    cudaEvent_t b = take(); cudaEventRecord(b, st);
+    ws->prof.push_back({name, a, b, launches});
+  }
+};
+} // namespace
 
 extern "C" {
 
@@ -325,6 +350,8 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
 
 void pnn_workspace_destroy(pnn_workspace* ws) {
   if (!ws) return;
+  for (auto& r : ws->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+  for (auto e : ws->ev_pool) cudaEventDestroy(e);
   if (ws->tc) tc_workspace_destroy(ws->tc);
   cudaFree(ws->arena);
   delete ws;
@@ -339,7 +366,12 @@ int pnn_build_graph(pnn_workspace* ws, int64_t N, int64_t S, const double* pos, 
   if (N > ws->maxN || S > ws->maxS) return PNN_ERR_CAPACITY;
   if ((N > 0 && !pos) || !sptr) return PNN_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
-  ws->launches += launch_graph_build(ws->g, N, S, pos, sptr, cell, pbc, ws->model->cfg.cutoff, ws->model->cfg.prec, st);
+  {
+    ProfScope ps(ws, st, "graph_build");
+    const int nl = launch_graph_build(ws->g, N, S, pos, sptr, cell, pbc, ws->model->cfg.cutoff, ws->model->cfg.prec, st);
+    ws->launches += nl;
+    ps.done(nl);
+  }
   ws->graph_N = N; ws->graph_S = S; ws->graph_stream = st;
   if (launch_failed()) return PNN_ERR_CUDA;
   PNN_TRY(cudaGetLastError());
@@ -374,6 +406,37 @@ int pnn_graph_copy(const pnn_workspace* ws, int32_t* rowptr, int32_t* col, int8_
   return PNN_OK;
 }
 
+int pnn_profile_enable(pnn_workspace* ws, int on) {
+  if (!ws) return PNN_ERR_INVALID_ARG;
+  ws->profile = on != 0;
+  return PNN_OK;
+}
+
+int pnn_profile_read(pnn_workspace* ws, int max_entries, char* names, double* total_ms, int64_t* launches,
+                     int* n_entries) {
+  if (!ws || !names || !total_ms || !launches || !n_entries || max_entries < 0) return PNN_ERR_INVALID_ARG;
+  PNN_TRY(cudaDeviceSynchronize());
+  int n = 0;
+  for (auto& r : ws->prof) {
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, r.a, r.b);
+    int idx = -1;
+    for (int q = 0; q < n; ++q)
+      if (std::strncmp(names + 32 * q, r.name, 31) == 0) { idx = q; break; }
+    if (idx < 0 && n < max_entries) {
+      idx = n++;
+      std::memset(names + 32 * idx, 0, 32);
+      std::strncpy(names + 32 * idx, r.name, 31);
+      total_ms[idx] = 0.0; launches[idx] = 0;
+    }
+    if (idx >= 0) { total_ms[idx] += ms; launches[idx] += r.launches; }
+    ws->ev_pool.push_back(r.a); ws->ev_pool.push_back(r.b);
+  }
+  ws->prof.clear();
+  *n_entries = n;
+  return PNN_OK;
+}
+
 int pnn_check_async_errors(pnn_workspace* ws) {
   if (!ws) return PNN_ERR_INVALID_ARG;
   PNN_TRY(cudaDeviceSynchronize());
@@ -404,7 +467,9 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
   T* s_cur = (T*)ws->s_cur; T* h = (T*)ws->h; T* sn = (T*)ws->sn; T* v1 = (T*)ws->v1; T* k = (T*)ws->k;
   const bool taped = ws->want_forces != 0;
 
-  nl += launch_embed<T>(N, F, c.Zmax, Z, W + m->emb, s_cur, ws->g.d_err, st);
+  { ProfScope ps_(ws, st, "embed");
+  const int l_ = launch_embed<T>(N, F, c.Zmax, Z, W + m->emb, s_cur, ws->g.d_err, st);
+    nl += l_; ps_.done(l_); }
   for (int t = 0; t < T_; ++t) {
     const BlockW& b = m->blk[t];
     const pnn_workspace::Tape& tp = ws->tape[taped ? t : 0];
@@ -419,52 +484,90 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     }
     T* phi = (T*)tp.phi; T* PQ = (T*)tp.PQ; T* a = (T*)tp.a;
     GemmEpi<T> e1; e1.bias = W + b.b1; e1.act = ACT_SILU; e1.pre = (T*)tp.hpre; e1.ldpre = F;
-    nl += launch_gemm<T>(N, F, F, s_cur, F, W + b.W1t, F, h, F, e1, st);                 // B3a, first Linear + SiLU
+    { ProfScope ps_(ws, st, "gemm_N");
+    const int l_ = launch_gemm<T>(N, F, F, s_cur, F, W + b.W1t, F, h, F, e1, st);                 // B3a, first Linear + SiLU
+      nl += l_; ps_.done(l_); }
     GemmEpi<T> e2; e2.bias = W + b.b2;
-    nl += launch_gemm<T>(N, 3 * F, F, h, F, W + b.W2t, 3 * F, phi, 3 * F, e2, st);       // B3a, second Linear
+    { ProfScope ps_(ws, st, "gemm_N");
+    const int l_ = launch_gemm<T>(N, 3 * F, F, h, F, W + b.W2t, 3 * F, phi, 3 * F, e2, st);       // B3a, second Linear
+      nl += l_; ps_.done(l_); }
     ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
-    nl += launch_edge_fwd<T>(ea, phi, s_cur, F, v_in, sn, 2 * F, v1, st);                // B3b -> s' in sn[:, :F], v'
+    { ProfScope ps_(ws, st, "edge_fwd");
+    const int l_ = launch_edge_fwd<T>(ea, phi, s_cur, F, v_in, sn, 2 * F, v1, st);                // B3b -> s' in sn[:, :F], v'
+      nl += l_; ps_.done(l_); }
     GemmEpi<T> e3;
-    nl += launch_gemm<T>(3 * N, 2 * F, F, v1, F, W + b.UVt, 2 * F, PQ, 2 * F, e3, st);   // B4: P | Q
-    nl += launch_norm<T>(N, F, PQ, sn, (T)c.norm_eps, st);                               // n -> sn[:, F:]
+    { ProfScope ps_(ws, st, "gemm_3N");
+    const int l_ = launch_gemm<T>(3 * N, 2 * F, F, v1, F, W + b.UVt, 2 * F, PQ, 2 * F, e3, st);   // B4: P | Q
+      nl += l_; ps_.done(l_); }
+    { ProfScope ps_(ws, st, "update_elementwise");
+    const int l_ = launch_norm<T>(N, F, PQ, sn, (T)c.norm_eps, st);                               // n -> sn[:, F:]
+      nl += l_; ps_.done(l_); }
     GemmEpi<T> e4; e4.bias = W + b.c1; e4.act = ACT_SILU; e4.pre = (T*)tp.kpre; e4.ldpre = F;
-    nl += launch_gemm<T>(N, F, 2 * F, sn, 2 * F, W + b.A1t, F, k, F, e4, st);
+    { ProfScope ps_(ws, st, "gemm_N");
+    const int l_ = launch_gemm<T>(N, F, 2 * F, sn, 2 * F, W + b.A1t, F, k, F, e4, st);
+      nl += l_; ps_.done(l_); }
     GemmEpi<T> e5; e5.bias = W + b.c2;
-    nl += launch_gemm<T>(N, 3 * F, F, k, F, W + b.A2t, 3 * F, a, 3 * F, e5, st);
-    nl += launch_update<T>(N, F, sn, v1, PQ, a, s_cur, v_out, st);
+    { ProfScope ps_(ws, st, "gemm_N");
+    const int l_ = launch_gemm<T>(N, 3 * F, F, k, F, W + b.A2t, 3 * F, a, 3 * F, e5, st);
+      nl += l_; ps_.done(l_); }
+    { ProfScope ps_(ws, st, "update_elementwise");
+    const int l_ = launch_update<T>(N, F, sn, v1, PQ, a, s_cur, v_out, st);
+      nl += l_; ps_.done(l_); }
   }
-  nl += launch_readout<T>(N, S, F, c.H, s_cur, ws->g.a2s, head, sptr, W + m->oW1t, W + m->ob1, W + m->ow2,
+  { ProfScope ps_(ws, st, "readout");
+  const int l_ = launch_readout<T>(N, S, F, c.H, s_cur, ws->g.a2s, head, sptr, W + m->oW1t, W + m->ob1, W + m->ow2,
                           W + m->ob2, (T*)ws->opre, (T*)ws->eatom, energy, ws->g.d_err, st);
+    nl += l_; ps_.done(l_); }
   if (want_f) {
     T* sb = (T*)ws->sb; T* vb = (T*)ws->vb; T* vb2 = (T*)ws->vb2; T* ab = (T*)ws->ab; T* PQb = (T*)ws->PQb;
     T* kb = (T*)ws->kb; T* zb = (T*)ws->zb; T* phib = (T*)ws->phib; T* hb = (T*)ws->hb; T* fpart = (T*)ws->fpart;
-    nl += launch_readout_bwd<T>(N, F, c.H, (const T*)ws->opre, ws->g.a2s, head, W + m->oW1, W + m->ow2, sb, st); // R1
+    { ProfScope ps_(ws, st, "readout_bwd");
+    const int l_ = launch_readout_bwd<T>(N, F, c.H, (const T*)ws->opre, ws->g.a2s, head, W + m->oW1, W + m->ow2, sb, st); // R1
+      nl += l_; ps_.done(l_); }
     for (int t = T_ - 1; t >= 0; --t) {
       const BlockW& b = m->blk[t];
       const pnn_workspace::Tape& tp = ws->tape[t];
       const bool last = (t == T_ - 1);
       // R2
-      nl += launch_update_bwd1<T>(N, F, sb, last ? nullptr : vb, (const T*)tp.a, (const T*)tp.PQ, ab, PQb, st);
+      { ProfScope ps_(ws, st, "update_bwd_elementwise");
+      const int l_ = launch_update_bwd1<T>(N, F, sb, last ? nullptr : vb, (const T*)tp.a, (const T*)tp.PQ, ab, PQb, st);
+        nl += l_; ps_.done(l_); }
       GemmEpi<T> g1; g1.act = ACT_MUL_DSILU; g1.aux = (const T*)tp.kpre; g1.ldaux = F;
-      nl += launch_gemm<T>(N, F, 3 * F, ab, 3 * F, W + b.A2, F, kb, F, g1, st);
+      { ProfScope ps_(ws, st, "gemm_N");
+      const int l_ = launch_gemm<T>(N, F, 3 * F, ab, 3 * F, W + b.A2, F, kb, F, g1, st);
+        nl += l_; ps_.done(l_); }
       GemmEpi<T> g2;
-      nl += launch_gemm<T>(N, 2 * F, F, kb, F, W + b.A1, 2 * F, zb, 2 * F, g2, st);
-      nl += launch_update_bwd2<T>(N, F, zb, (const T*)tp.PQ, (T)c.norm_eps, sb, PQb, st);
+      { ProfScope ps_(ws, st, "gemm_N");
+      const int l_ = launch_gemm<T>(N, 2 * F, F, kb, F, W + b.A1, 2 * F, zb, 2 * F, g2, st);
+        nl += l_; ps_.done(l_); }
+      { ProfScope ps_(ws, st, "update_bwd_elementwise");
+      const int l_ = launch_update_bwd2<T>(N, F, zb, (const T*)tp.PQ, (T)c.norm_eps, sb, PQb, st);
+        nl += l_; ps_.done(l_); }
       GemmEpi<T> g3; g3.accumulate = last ? 0 : 1;
-      nl += launch_gemm<T>(3 * N, F, 2 * F, PQb, 2 * F, W + b.UV, F, vb, F, g3, st);
+      { ProfScope ps_(ws, st, "gemm_3N");
+      const int l_ = launch_gemm<T>(3 * N, F, 2 * F, PQb, 2 * F, W + b.UV, F, vb, F, g3, st);
+        nl += l_; ps_.done(l_); }
       // R3 + R4
       ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
-      nl += launch_edge_bwd<T>(ea, (const T*)tp.phi, (const T*)tp.v_in, sb, vb, t > 0 ? phib : nullptr, vb2, fpart,
+      { ProfScope ps_(ws, st, "edge_bwd");
+      const int l_ = launch_edge_bwd<T>(ea, (const T*)tp.phi, (const T*)tp.v_in, sb, vb, t > 0 ? phib : nullptr, vb2, fpart,
                                last ? 1 : 0, st);
+        nl += l_; ps_.done(l_); }
       if (t > 0) {
         GemmEpi<T> g4; g4.act = ACT_MUL_DSILU; g4.aux = (const T*)tp.hpre; g4.ldaux = F;
-        nl += launch_gemm<T>(N, F, 3 * F, phib, 3 * F, W + b.W2, F, hb, F, g4, st);
+        { ProfScope ps_(ws, st, "gemm_N");
+        const int l_ = launch_gemm<T>(N, F, 3 * F, phib, 3 * F, W + b.W2, F, hb, F, g4, st);
+          nl += l_; ps_.done(l_); }
         GemmEpi<T> g5; g5.accumulate = 1;
-        nl += launch_gemm<T>(N, F, F, hb, F, W + b.W1, F, sb, F, g5, st);
+        { ProfScope ps_(ws, st, "gemm_N");
+        const int l_ = launch_gemm<T>(N, F, F, hb, F, W + b.W1, F, sb, F, g5, st);
+          nl += l_; ps_.done(l_); }
         T* tmp = vb; vb = vb2; vb2 = tmp;
       }
     }
-    nl += launch_force_assemble<T>(N, edge_num_slabs(F), fpart, forces, st);
+    { ProfScope ps_(ws, st, "force_assemble");
+    const int l_ = launch_force_assemble<T>(N, edge_num_slabs(F), fpart, forces, st);
+      nl += l_; ps_.done(l_); }
   }
   ws->launches += nl;
   return PNN_OK;
