@@ -128,6 +128,14 @@ int pnn_profile_enable(pnn_workspace* ws, int on);
 int pnn_profile_read(pnn_workspace* ws, int max_entries, char* names, double* total_ms, int64_t* launches,
                      int* n_entries);
 
+/* The BF16 node contraction on its own (a3 / a5 building block; also used by the tests and bench.py to measure the
+ * tensor pipe): C[M,N] = act( A[M,K] . Wt[N,K]^T + bias ), A / Wt DEVICE BF16 row-major with row strides lda / ldw
+ * (elements), FP32 accumulation on tcgen05 tensor cores.  bias DEVICE f32 [N] or NULL; act 0 = none, 1 = SiLU.
+ * C DEVICE f32 (row stride ldc) and / or Cb DEVICE bf16 (row stride ldcb); either may be NULL.  N and K multiples of
+ * 32, lda / ldw multiples of 8.  Asynchronous. */
+int pnn_gemm_bf16(int64_t M, int32_t N, int32_t K, const void* A, int64_t lda, const void* Wt, int64_t ldw,
+                  const float* bias, int32_t act, float* C, int64_t ldc, void* Cb, int64_t ldcb, void* cuda_stream);
+
 /* Number of kernels the library has launched on behalf of this workspace since it was created. */
 int64_t pnn_launch_count(const pnn_workspace* ws);
 

@@ -17,7 +17,7 @@ __all__ = [
     "lib_path", "pnn_status_string", "pnn_last_cuda_error", "pnn_weights_count", "pnn_model_create",
     "pnn_model_destroy", "pnn_workspace_create", "pnn_workspace_destroy", "pnn_workspace_bytes", "pnn_build_graph",
     "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_eval_host", "pnn_check_async_errors", "pnn_launch_count", "pnn_profile_enable",
-    "pnn_profile_read",
+    "pnn_profile_read", "pnn_gemm_bf16",
     "PaiNN", "PRECISIONS",
 ]
 
@@ -81,6 +81,7 @@ def lib():
         L.pnn_check_async_errors.argtypes = [vp]
         L.pnn_profile_enable.argtypes = [vp, i32]
         L.pnn_profile_read.argtypes = [vp, i32, vp, vp, vp, ctypes.POINTER(i32)]
+        L.pnn_gemm_bf16.argtypes = [i64, i32, i32, vp, i64, vp, i64, vp, i32, vp, i64, vp, i64, vp]
         L.pnn_launch_count.argtypes = [vp]
         L.pnn_launch_count.restype = i64
         _lib = L
@@ -196,6 +197,12 @@ def pnn_profile_read(ws: int, max_entries: int = 32) -> dict:
     _check(lib().pnn_profile_read(ws, max_entries, ctypes.addressof(names), ctypes.addressof(ms),
                                   ctypes.addressof(nl), ctypes.byref(n)), "pnn_profile_read")
     return {names.raw[32 * q:32 * q + 32].split(b"\0")[0].decode(): (ms[q], nl[q]) for q in range(n.value)}
+
+
+def pnn_gemm_bf16(M: int, N: int, K: int, A, lda: int, Wt, ldw: int, bias=None, act: int = 0, C=None, ldc: int = 0,
+                  Cb=None, ldcb: int = 0, stream=None) -> None:
+    _check(lib().pnn_gemm_bf16(M, N, K, _ptr(A), lda, _ptr(Wt), ldw, _ptr(bias), act, _ptr(C), ldc, _ptr(Cb), ldcb,
+                               stream), "pnn_gemm_bf16")
 
 
 class PaiNN:

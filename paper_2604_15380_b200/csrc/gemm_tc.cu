@@ -1,12 +1,318 @@
-// gemm_tc.cu — BF16 tensor-core GEMMs (placeholder until the tcgen05 path lands: reports UNSUPPORTED).
+// gemm_tc.cu — BF16 node contractions (a3, a5 and their adjoints) on the 5th-generation tensor cores.
+//
+//   C[M,N] = epi( A[M,K] * Wt[N,K]^T ),  BF16 operands, FP32 accumulation.
+//
+// One CTA computes a 128 x BN tile (BN = largest of 256/128/64/32 dividing N).  Warp roles:
+//   warp 0    TMA producer: cp.async.bulk.tensor.2d of the A tile [128 x 64] and the Wt tile [BN x 64] per k-block into
+//             a ring of shared-memory stages (SWIZZLE_128B, K-major), completion on the stage's "full" mbarrier;
+//   warp 1    MMA issuer: one thread issues tcgen05.mma.cta_group::1.kind::f16 (M = 128, N = BN, K = 16) four times per
+//             k-block, accumulator in TMEM; tcgen05.commit frees the stage ("empty" mbarrier) and finally signals
+//             the epilogue ("accumulator full" mbarrier);
+//   warps 2-5 epilogue: tcgen05.ld (32 lanes x 32 columns per warp), transposition through shared memory so that
+//             global accesses are row-contiguous, then bias / SiLU / silu' / accumulate and FP32 / BF16 stores.
+//             Warp 2 also allocates and frees the TMEM columns.
+// K <= 768 here (at most 12 k-blocks), so a CTA is short; two CTAs share an SM (TMEM 2 x 256 columns, shared memory
+// 2 x <= 113 KB) so one tile's epilogue overlaps the other's loads and MMAs.
+#include <cuda.h>
+
+#include <mutex>
+#include <unordered_map>
+
+#include "common.cuh"
 #include "gemm_tc.cuh"
 
 namespace pnn {
-struct TcModel { int dummy; };
-struct TcWorkspace { int dummy; };
-int tc_model_create(const pnn_config*, const double*, TcModel**) { return PNN_ERR_UNSUPPORTED; }
-void tc_model_destroy(TcModel*) {}
-int tc_workspace_create(const TcModel*, int64_t, TcWorkspace**) { return PNN_ERR_UNSUPPORTED; }
-void tc_workspace_destroy(TcWorkspace*) {}
-int64_t tc_workspace_bytes(const TcWorkspace*) { return 0; }
+
+namespace {
+
+constexpr int BM = 128, BK = 64;
+constexpr int NTHREADS = 192;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tm)), "r"(bar), "r"(c0), "r"(c1)
+      : "memory");
+}
+// shared-memory matrix descriptor: K-major, SWIZZLE_128B, 8-row groups 1024 B apart (sm_100 descriptor version 1)
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3FFFFu) >> 4);
+  d |= (uint64_t)1 << 16;           // leading byte offset (unused for swizzled K-major)
+  d |= (uint64_t)(1024 >> 4) << 32; // stride byte offset
+  d |= (uint64_t)1 << 46;           // descriptor version
+  d |= (uint64_t)2 << 61;           // SWIZZLE_128B
+  return d;
+}
+__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                          uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr)
+      : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+template <int BN, int STAGES>
+struct TcSmem {
+  static constexpr int A_BYTES = BM * BK * 2;
+  static constexpr int B_BYTES = BN * BK * 2;
+  static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+  static constexpr int EPI_BYTES = 4 * 32 * 33 * 4; // transposition buffers of the four epilogue warps
+  static constexpr int PIPE_BYTES = STAGES * STAGE_BYTES;
+  static constexpr int TOTAL = (PIPE_BYTES > EPI_BYTES ? PIPE_BYTES : EPI_BYTES) + 1024 /*alignment slack*/ + 256;
+};
+
+template <int BN, int STAGES>
+__global__ void __launch_bounds__(NTHREADS)
+tc_gemm_k(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int64_t M, int N, int K,
+          int n_tiles, TcEpi epi) {
+  using L = TcSmem<BN, STAGES>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const uint32_t raw = smem_u32(smem_raw);
+  const uint32_t tiles = (raw + 1023u) & ~1023u;                 // 1024-byte aligned stage ring
+  unsigned char* tiles_ptr = smem_raw + (tiles - raw);
+  const uint32_t PIPE = (L::PIPE_BYTES > L::EPI_BYTES ? L::PIPE_BYTES : L::EPI_BYTES);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tiles_ptr + PIPE); // full[STAGES], empty[STAGES], accfull
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 1);
+  const uint32_t bar0 = smem_u32(bars);
+  auto full_bar = [&](int s) { return bar0 + 8u * s; };
+  auto empty_bar = [&](int s) { return bar0 + 8u * (STAGES + s); };
+  const uint32_t acc_bar = bar0 + 8u * (2 * STAGES);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t m_tile = blockIdx.x / n_tiles;
+  const int n_tile = blockIdx.x % n_tiles;
+  const int64_t m0 = m_tile * BM;
+  const int n0 = n_tile * BN;
+  const int nkb = (K + BK - 1) / BK;
+
+  if (warp == 1 && lane == 0) {
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    mbar_init(acc_bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 2) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(BN)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      for (int kb = 0; kb < nkb; ++kb) {
+        const int s = kb % STAGES;
+        const uint32_t ph = (kb / STAGES) & 1;
+        mbar_wait(empty_bar(s), ph ^ 1u);
+        const uint32_t sa = tiles + s * L::STAGE_BYTES;
+        mbar_expect_tx(full_bar(s), L::STAGE_BYTES);
+        tma_load_2d(sa, &tmA, full_bar(s), kb * BK, (int)m0);
+        tma_load_2d(sa + L::A_BYTES, &tmB, full_bar(s), kb * BK, n0);
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      // instruction descriptor: D = F32, A = B = BF16, both K-major, N = BN, M = 128
+      const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+      for (int kb = 0; kb < nkb; ++kb) {
+        const int s = kb % STAGES;
+        const uint32_t ph = (kb / STAGES) & 1;
+        mbar_wait(full_bar(s), ph);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const uint32_t sa = tiles + s * L::STAGE_BYTES;
+        const uint64_t ad = umma_desc_sw128(sa), bd = umma_desc_sw128(sa + L::A_BYTES);
+#pragma unroll
+        for (int k = 0; k < BK / 16; ++k)
+          umma_bf16(tmem_base, ad + (uint64_t)(k * 2), bd + (uint64_t)(k * 2), idesc, (kb | k) ? 1u : 0u);
+        umma_commit(empty_bar(s));
+      }
+      umma_commit(acc_bar);
+    }
+  } else {
+    // epilogue warps 2..5: TMEM lane quadrant = warp % 4
+    const int q = warp & 3;
+    mbar_wait(acc_bar, 0);
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    float* Tb = reinterpret_cast<float*>(tiles_ptr) + (warp - 2) * 32 * 33; // stage ring is free once acc_bar fired
+    const int64_t mrow0 = m0 + q * 32;
+#pragma unroll 1
+    for (int c0 = 0; c0 < BN; c0 += 32) {
+      uint32_t r[32];
+      tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)c0, r);
+#pragma unroll
+      for (int j = 0; j < 32; ++j) Tb[lane * 33 + j] = __uint_as_float(r[j]);
+      __syncwarp();
+      const int n = n0 + c0 + lane;
+      const float bv = epi.bias ? epi.bias[n] : 0.0f;
+#pragma unroll 4
+      for (int rr = 0; rr < 32; ++rr) {
+        const int64_t m = mrow0 + rr;
+        if (m >= M) break;
+        float x = Tb[rr * 33 + lane] + bv;
+        if (epi.act == ACT_SILU) {
+          if (epi.pre) epi.pre[m * epi.ldpre + n] = x;
+          x = silu_f<float>(x);
+        } else if (epi.act == ACT_MUL_DSILU) {
+          x *= dsilu_f<float>(epi.aux[m * epi.ldaux + n]);
+        }
+        if (epi.accumulate) x += epi.C[m * epi.ldc + n];
+        if (epi.C) epi.C[m * epi.ldc + n] = x;
+        if (epi.Cb) epi.Cb[m * epi.ldcb + n] = __float2bfloat16_rn(x);
+      }
+      __syncwarp();
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  }
+  __syncthreads();
+  if (warp == 2) {
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(BN) : "memory");
+  }
+}
+
+__global__ void __launch_bounds__(256) f32_to_bf16_k(int64_t n, const float* __restrict__ src,
+                                                     __nv_bfloat16* __restrict__ dst) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) dst[i] = __float2bfloat16_rn(src[i]);
+}
+
+// ------------------------------------------------------------------------------------------ TMA descriptors
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  });
+  return fn;
+}
+
+struct MapKey {
+  const void* ptr; int64_t rows, ld; int cols, box_rows;
+  bool operator==(const MapKey& o) const {
+    return ptr == o.ptr && rows == o.rows && ld == o.ld && cols == o.cols && box_rows == o.box_rows;
+  }
+};
+struct MapKeyHash {
+  size_t operator()(const MapKey& k) const {
+    size_t h = std::hash<const void*>()(k.ptr);
+    h = h * 1000003u ^ std::hash<int64_t>()(k.rows);
+    h = h * 1000003u ^ std::hash<int64_t>()(k.ld);
+    h = h * 1000003u ^ std::hash<int>()(k.cols * 512 + k.box_rows);
+    return h;
+  }
+};
+
+// BF16 row-major [rows][cols] with row stride ld (elements); box = [box_rows][64], 128-byte swizzle, OOB zero fill.
+bool get_tensor_map(const __nv_bfloat16* ptr, int64_t rows, int cols, int64_t ld, int box_rows, CUtensorMap* out) {
+  static std::unordered_map<MapKey, CUtensorMap, MapKeyHash> cache;
+  static std::mutex mu;
+  const MapKey key{ptr, rows, ld, cols, box_rows};
+  std::lock_guard<std::mutex> lock(mu);
+  auto it = cache.find(key);
+  if (it != cache.end()) { *out = it->second; return true; }
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return false;
+  CUtensorMap tm;
+  const cuuint64_t gdim[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  const cuuint64_t gstride[1] = {(cuuint64_t)ld * 2};
+  const cuuint32_t box[2] = {(cuuint32_t)BK, (cuuint32_t)box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = fn(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<__nv_bfloat16*>(ptr), gdim, gstride, box,
+                        estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                        CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return false;
+  if (cache.size() > 4096) cache.clear();
+  cache.emplace(key, tm);
+  *out = tm;
+  return true;
+}
+
+template <int BN, int STAGES>
+int launch_cfg(int64_t M, int N, int K, const CUtensorMap& ta, const CUtensorMap& tb, const TcEpi& epi,
+               cudaStream_t st) {
+  using L = TcSmem<BN, STAGES>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(tc_gemm_k<BN, STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, L::TOTAL);
+    attr_set = true;
+  }
+  const int n_tiles = N / BN;
+  const int64_t m_tiles = (M + BM - 1) / BM;
+  tc_gemm_k<BN, STAGES><<<(unsigned)(m_tiles * n_tiles), NTHREADS, L::TOTAL, st>>>(ta, tb, M, N, K, n_tiles, epi);
+  PNN_KCHECK("tc_gemm_k");
+  return 1;
+}
+
+} // namespace
+
+int launch_gemm_tc(int64_t M, int N, int K, const __nv_bfloat16* A, int64_t lda, const __nv_bfloat16* Wt, int64_t ldw,
+                   const TcEpi& epi, cudaStream_t st) {
+  if (M <= 0) return 0;
+  const int bn = (N % 256 == 0) ? 256 : (N % 128 == 0) ? 128 : (N % 64 == 0) ? 64 : 32;
+  CUtensorMap ta, tb;
+  if (!get_tensor_map(A, M, K, lda, BM, &ta) || !get_tensor_map(Wt, N, K, ldw, bn, &tb)) return -1;
+  switch (bn) {
+    case 256: return launch_cfg<256, 2>(M, N, K, ta, tb, epi, st);
+    case 128: return launch_cfg<128, 3>(M, N, K, ta, tb, epi, st);
+    case 64: return launch_cfg<64, 4>(M, N, K, ta, tb, epi, st);
+    default: return launch_cfg<32, 4>(M, N, K, ta, tb, epi, st);
+  }
+}
+
+int launch_f32_to_bf16(int64_t n, const float* src, __nv_bfloat16* dst, cudaStream_t st) {
+  if (n <= 0) return 0;
+  f32_to_bf16_k<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, src, dst);
+  PNN_KCHECK("f32_to_bf16_k");
+  return 1;
+}
+
 } // namespace pnn

@@ -79,7 +79,7 @@ struct pnn_model {
   int64_t emb = 0;
   std::vector<BlockW> blk;
   int64_t oW1t = 0, oW1 = 0, ob1 = 0, ow2 = 0, ob2 = 0; // heads: [H][F][Fh], [H][Fh][F], [H][Fh], [H][Fh], [H]
-  TcModel* tc = nullptr;                                // BF16 tensor-core operands (gemm_tc.cu), or null
+  __nv_bfloat16* d_wb = nullptr;                        // BF16 copy of d_w (same offsets): tcgen05 GEMM operands
 };
 
 struct pnn_workspace {
@@ -103,7 +103,6 @@ struct pnn_workspace {
   double *st_pos, *st_cell;
   uint8_t* st_pbc;
   void *st_energy, *st_forces;
-  TcWorkspace* tc = nullptr;
   // optional per-kernel-family timing (pnn_profile_enable)
   bool profile = false;
   struct ProfRec { const char* name; cudaEvent_t a, b; int launches; };
@@ -232,8 +231,13 @@ int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, 
   }
   if (!cuda_ok(e, "cudaMemcpy(weights)")) { cudaFree(m->d_w); delete m; return PNN_ERR_CUDA; }
   if (cfg->prec == PNN_BF16) {
-    const int rc = tc_model_create(cfg, w, &m->tc);
-    if (rc != PNN_OK) { cudaFree(m->d_w); delete m; return rc; }
+    if (!cuda_ok(cudaMalloc((void**)&m->d_wb, m->n_elem * 2), "cudaMalloc(bf16 weights)")) {
+      cudaFree(m->d_w); delete m; return PNN_ERR_CUDA;
+    }
+    launch_f32_to_bf16(m->n_elem, (const float*)m->d_w, m->d_wb, nullptr);
+    if (!cuda_ok(cudaDeviceSynchronize(), "bf16 weight conversion") || launch_failed()) {
+      cudaFree(m->d_wb); cudaFree(m->d_w); delete m; return PNN_ERR_CUDA;
+    }
   }
   *out = m;
   return PNN_OK;
@@ -241,7 +245,7 @@ int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, 
 
 void pnn_model_destroy(pnn_model* m) {
   if (!m) return;
-  if (m->tc) tc_model_destroy(m->tc);
+  cudaFree(m->d_wb);
   cudaFree(m->d_w);
   delete m;
 }
@@ -340,10 +344,6 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
       }
     }
   }
-  if (m->cfg.prec == PNN_BF16) {
-    const int rc = tc_workspace_create(m->tc, N, &ws->tc);
-    if (rc != PNN_OK) { cudaFree(ws->arena); delete ws; return rc; }
-  }
   *out = ws;
   return PNN_OK;
 }
@@ -352,12 +352,11 @@ void pnn_workspace_destroy(pnn_workspace* ws) {
   if (!ws) return;
   for (auto& r : ws->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (auto e : ws->ev_pool) cudaEventDestroy(e);
-  if (ws->tc) tc_workspace_destroy(ws->tc);
   cudaFree(ws->arena);
   delete ws;
 }
 
-int64_t pnn_workspace_bytes(const pnn_workspace* ws) { return ws ? ws->arena_bytes + (ws->tc ? tc_workspace_bytes(ws->tc) : 0) : 0; }
+int64_t pnn_workspace_bytes(const pnn_workspace* ws) { return ws ? ws->arena_bytes : 0; }
 int64_t pnn_launch_count(const pnn_workspace* ws) { return ws ? ws->launches : 0; }
 
 int pnn_build_graph(pnn_workspace* ws, int64_t N, int64_t S, const double* pos, const int32_t* sptr,
@@ -630,6 +629,21 @@ int pnn_eval_host(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, c
   if ((flags & PNN_FORCES) && N > 0)
     PNN_TRY(cudaMemcpyAsync(forces_host, ws->st_forces, es * 3 * N, cudaMemcpyDeviceToHost, st));
   PNN_TRY(cudaStreamSynchronize(st));
+  return PNN_OK;
+}
+
+int pnn_gemm_bf16(int64_t M, int32_t N, int32_t K, const void* A, int64_t lda, const void* Wt, int64_t ldw,
+                  const float* bias, int32_t act, float* C, int64_t ldc, void* Cb, int64_t ldcb, void* stream) {
+  if (M < 0 || N < 32 || K < 32 || N % 32 || K % 32 || lda % 8 || ldw % 8 || lda < K || ldw < K) return PNN_ERR_INVALID_ARG;
+  if (M > 0 && (!A || !Wt || (!C && !Cb))) return PNN_ERR_INVALID_ARG;
+  if (act != ACT_NONE && act != ACT_SILU) return PNN_ERR_INVALID_ARG;
+  TcEpi e;
+  e.bias = bias; e.act = act; e.C = C; e.ldc = ldc; e.Cb = (__nv_bfloat16*)Cb; e.ldcb = ldcb;
+  const int nl = launch_gemm_tc(M, N, K, (const __nv_bfloat16*)A, lda, (const __nv_bfloat16*)Wt, ldw, e,
+                                (cudaStream_t)stream);
+  if (nl < 0) return PNN_ERR_UNSUPPORTED;
+  if (launch_failed()) return PNN_ERR_CUDA;
+  PNN_TRY(cudaGetLastError());
   return PNN_OK;
 }
 

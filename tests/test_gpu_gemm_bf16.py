@@ -1,0 +1,48 @@
+"""-m gpu: the tcgen05 BF16 GEMM building block (pnn_gemm_bf16) against an FP64 matmul of the same BF16 operands.
+Products of BF16 numbers are exact in FP32 and the accumulation is FP32, so the only error is summation rounding:
+|err| <= ~K * 2^-24 * sum|a||w| — the bound used below."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("M,N,K", [(128, 32, 32), (1000, 96, 96), (300, 128, 256), (4133, 384, 128), (2500, 768, 256),
+                                   (777, 256, 512), (129, 512, 768), (1, 64, 64)])
+@pytest.mark.parametrize("act", [0, 1])
+def test_gemm_bf16_matches_fp64(M, N, K, act):
+    import torch
+    import paper_2604_15380_b200 as pnn
+    g = torch.Generator(device="cpu").manual_seed(M * 7 + N * 3 + K + act)
+    A = torch.randn(M, K, generator=g).to(torch.bfloat16).cuda()
+    W = (torch.randn(N, K, generator=g) / K ** 0.5).to(torch.bfloat16).cuda()
+    bias = torch.randn(N, generator=g).cuda()
+    C = torch.full((M, N), float("nan"), device="cuda")
+    Cb = torch.zeros((M, N), dtype=torch.bfloat16, device="cuda")
+    pnn.pnn_gemm_bf16(M, N, K, A, K, W, K, bias, act, C, N, Cb, N, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    ref = A.double() @ W.double().T + bias.double()
+    bound = (A.double().abs() @ W.double().abs().T + bias.double().abs()) * (K * 2.0 ** -24) + 1e-30
+    if act == 1:
+        ref = torch.nn.functional.silu(ref)
+        bound = bound * 1.2 + 2e-7 * ref.abs()
+    err = (C.double() - ref).abs()
+    assert torch.isfinite(C).all()
+    assert (err <= bound * 2 + 1e-7).all(), float((err / bound).max())
+    assert ((Cb.double() - ref).abs() <= ref.abs() * 2.0 ** -8 + bound * 2 + 1e-7).all()
+
+
+def test_gemm_bf16_strided_and_outputs_optional():
+    import torch
+    import paper_2604_15380_b200 as pnn
+    M, N, K, lda = 515, 128, 64, 192
+    g = torch.Generator(device="cpu").manual_seed(3)
+    Abig = torch.randn(M, lda, generator=g).to(torch.bfloat16).cuda()
+    W = torch.randn(N, K, generator=g).to(torch.bfloat16).cuda()
+    C = torch.zeros((M, 2 * N), device="cuda")
+    pnn.pnn_gemm_bf16(M, N, K, Abig[:, 64:], lda, W, K, None, 0, C[:, N:], 2 * N, None, 0,
+                      torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    ref = Abig[:, 64:128].double() @ W.double().T
+    assert (C[:, :N] == 0).all()
+    assert ((C[:, N:].double() - ref).abs() <= 1e-4 * (1 + ref.abs())).all()
