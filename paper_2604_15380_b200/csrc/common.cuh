@@ -109,30 +109,41 @@ struct EdgeArgs {
   const T* fltb; // [3F]
   const int* d_err;
 };
-// forward message step (B3b): s1 = s_in + sum, v1 = v_in + sum.  s_in/s1 have leading dimensions.
-template <typename T>
-int launch_edge_fwd(const EdgeArgs<T>& a, const T* phi, const T* s_in, int64_t ld_sin, const T* v_in, T* s1,
-                    int64_t ld_s1, T* v1, cudaStream_t st);
+// optional BF16 copies of the forward outputs (BF16 model: operands of the next GEMMs)
+struct EdgeMirror {
+  __nv_bfloat16* s1 = nullptr;
+  int64_t ld_s1 = 0;
+  __nv_bfloat16* v1 = nullptr;
+};
+// forward message step (B3b): s1 = s_in + sum, v1 = v_res + sum.  s_in/s1 have leading dimensions.  phi and v_in
+// are the gathered sender payloads (type PT = T, or BF16 in the BF16 model); v_res is the receiver's own row of v.
+template <typename T, typename PT>
+int launch_edge_fwd(const EdgeArgs<T>& a, const PT* phi, const T* s_in, int64_t ld_sin, const PT* v_in,
+                    const T* v_res, T* s1, int64_t ld_s1, T* v1, const EdgeMirror& mir, cudaStream_t st);
 // reverse message step (R3 + R4 partial): from sb1 [N,F], vb1 [N,3F] and the forward phi, v_in produce
 // phib [N,3F], vb_in [N,3F] and add this block's force contribution into fpart [nslab][N][3].
-template <typename T>
-int launch_edge_bwd(const EdgeArgs<T>& a, const T* phi, const T* v_in, const T* sb1, const T* vb1, T* phib, T* vb_in,
-                    T* fpart, int first_block, cudaStream_t st);
+// (phib16 != null: phib is written there in BF16 instead of to phib.)
+template <typename T, typename PT>
+int launch_edge_bwd(const EdgeArgs<T>& a, const PT* phi, const PT* v_in, const T* sb1, const T* vb1, T* phib,
+                    T* vb_in, T* fpart, int first_block, __nv_bfloat16* phib16, cudaStream_t st);
 int edge_num_slabs(int F);
 
 // node.cu
+// (the trailing BF16 pointers are optional copies / replacements of an output for the BF16 model's GEMM operands)
 template <typename T>
-int launch_embed(int64_t N, int F, int Zmax, const int32_t* Z, const T* emb, T* s, int* d_err, cudaStream_t st);
+int launch_embed(int64_t N, int F, int Zmax, const int32_t* Z, const T* emb, T* s, int* d_err, cudaStream_t st,
+                 __nv_bfloat16* s16 = nullptr);
 template <typename T>
-int launch_norm(int64_t N, int F, const T* PQ, T* sn, T eps, cudaStream_t st);
+int launch_norm(int64_t N, int F, const T* PQ, T* sn, T eps, cudaStream_t st, __nv_bfloat16* sn16 = nullptr);
 template <typename T>
 int launch_update(int64_t N, int F, const T* sn, const T* v1, const T* PQ, const T* a, T* s_out, T* v_out,
-                  cudaStream_t st);
+                  cudaStream_t st, __nv_bfloat16* s16 = nullptr, __nv_bfloat16* v16 = nullptr);
 template <typename T>
 int launch_update_bwd1(int64_t N, int F, const T* sb, const T* vb, const T* a, const T* PQ, T* ab, T* PQb,
-                       cudaStream_t st);
+                       cudaStream_t st, __nv_bfloat16* ab16 = nullptr);
 template <typename T>
-int launch_update_bwd2(int64_t N, int F, const T* zb, const T* PQ, T eps, T* sb, T* PQb, cudaStream_t st);
+int launch_update_bwd2(int64_t N, int F, const T* zb, const T* PQ, T eps, T* sb, T* PQb, cudaStream_t st,
+                       __nv_bfloat16* PQb16 = nullptr);
 // readout (B5 / R1).  W1t: [H][F][F/2] (transposed), W1: [H][F/2][F], b1 [H][F/2], w2 [H][F/2], b2 [H].
 template <typename T>
 int launch_readout(int64_t N, int64_t S, int F, int H, const T* s, const int32_t* a2s, const int32_t* head,

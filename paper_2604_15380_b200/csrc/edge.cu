@@ -30,6 +30,12 @@ template <typename T> __device__ __forceinline__ void t_sincos(T x, T* s, T* c);
 template <> __device__ __forceinline__ void t_sincos<float>(float x, float* s, float* c) { sincosf(x, s, c); }
 template <> __device__ __forceinline__ void t_sincos<double>(double x, double* s, double* c) { sincos(x, s, c); }
 
+// gathered payloads (phi_j, v_j) may be stored narrower than the arithmetic type (BF16 model, reading Q19)
+template <typename T, typename PT> __device__ __forceinline__ T ldp(const PT* p) { return (T)(*p); }
+template <> __device__ __forceinline__ float ldp<float, __nv_bfloat16>(const __nv_bfloat16* p) {
+  return __bfloat162float(*p);
+}
+
 template <typename T, int KP>
 __device__ __forceinline__ void load_filter_row(const EdgeArgs<T>& a, int row, T (&w)[KP], T& bias) {
 #pragma unroll
@@ -61,10 +67,11 @@ __device__ __forceinline__ double dotK(const double (&w)[KP], const double* __re
 }
 
 // ------------------------------------------------------------------------------------------ forward
-template <typename T, int KP>
+template <typename T, int KP, typename PT>
 __global__ void __launch_bounds__(384)
-edge_fwd_k(EdgeArgs<T> a, int FS, int RB, const T* __restrict__ phi, const T* __restrict__ s_in, int64_t ld_sin,
-           const T* __restrict__ v_in, T* __restrict__ s1, int64_t ld_s1, T* __restrict__ v1) {
+edge_fwd_k(EdgeArgs<T> a, int FS, int RB, const PT* __restrict__ phi, const T* __restrict__ s_in, int64_t ld_sin,
+           const PT* __restrict__ v_in, const T* __restrict__ v_res, T* __restrict__ s1, int64_t ld_s1,
+           T* __restrict__ v1, EdgeMirror mir) {
   if (*a.d_err & ERRF_EDGE_OVERFLOW) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* G = reinterpret_cast<T*>(smem_raw);            // [ET][KP]
@@ -129,17 +136,17 @@ edge_fwd_k(EdgeArgs<T> a, int FS, int RB, const T* __restrict__ phi, const T* __
         const int64_t j = J[q];
         const T wv = fma(bias, Cc[q], dotK<KP>(w, G + q * KP));
         if (c == 0) {
-          acc0 = fma(phi[j * 3 * F + f], wv, acc0);
+          acc0 = fma(ldp<T, PT>(phi + j * 3 * F + f), wv, acc0);
         } else if (c == 1) {
-          const T x = phi[j * 3 * F + F + f] * wv;
+          const T x = ldp<T, PT>(phi + j * 3 * F + F + f) * wv;
           acc0 = fma(x, U[q * 4 + 0], acc0);
           acc1 = fma(x, U[q * 4 + 1], acc1);
           acc2 = fma(x, U[q * 4 + 2], acc2);
         } else if (v_in != nullptr) {
-          const T x = phi[j * 3 * F + 2 * F + f] * wv;
-          acc0 = fma(x, v_in[(j * 3 + 0) * F + f], acc0);
-          acc1 = fma(x, v_in[(j * 3 + 1) * F + f], acc1);
-          acc2 = fma(x, v_in[(j * 3 + 2) * F + f], acc2);
+          const T x = ldp<T, PT>(phi + j * 3 * F + 2 * F + f) * wv;
+          acc0 = fma(x, ldp<T, PT>(v_in + (j * 3 + 0) * F + f), acc0);
+          acc1 = fma(x, ldp<T, PT>(v_in + (j * 3 + 1) * F + f), acc1);
+          acc2 = fma(x, ldp<T, PT>(v_in + (j * 3 + 2) * F + f), acc2);
         }
       }
     }
@@ -152,21 +159,25 @@ edge_fwd_k(EdgeArgs<T> a, int FS, int RB, const T* __restrict__ phi, const T* __
       const int64_t i = i0 + rr;
       const int fo = blockIdx.y * FS + ff;
       if (comp == 0) {
-        s1[i * ld_s1 + fo] = s_in[i * ld_sin + fo] + Acc[(rr * 7 + 0) * FS + ff];
+        const T r = s_in[i * ld_sin + fo] + Acc[(rr * 7 + 0) * FS + ff];
+        s1[i * ld_s1 + fo] = r;
+        if (mir.s1) mir.s1[i * mir.ld_s1 + fo] = __float2bfloat16_rn((float)r);
       } else {
-        const T vin = v_in ? v_in[(i * 3 + (comp - 1)) * F + fo] : T(0);
-        v1[(i * 3 + (comp - 1)) * F + fo] = vin + Acc[(rr * 7 + comp) * FS + ff] + Acc[(rr * 7 + 3 + comp) * FS + ff];
+        const T vin = v_res ? v_res[(i * 3 + (comp - 1)) * F + fo] : T(0);
+        const T r = vin + Acc[(rr * 7 + comp) * FS + ff] + Acc[(rr * 7 + 3 + comp) * FS + ff];
+        v1[(i * 3 + (comp - 1)) * F + fo] = r;
+        if (mir.v1) mir.v1[(i * 3 + (comp - 1)) * F + fo] = __float2bfloat16_rn((float)r);
       }
     }
   }
 }
 
 // ------------------------------------------------------------------------------------------ reverse
-template <typename T, int KP>
+template <typename T, int KP, typename PT>
 __global__ void __launch_bounds__(384)
-edge_bwd_k(EdgeArgs<T> a, int FS, int RB, const T* __restrict__ phi, const T* __restrict__ v_in,
+edge_bwd_k(EdgeArgs<T> a, int FS, int RB, const PT* __restrict__ phi, const PT* __restrict__ v_in,
            const T* __restrict__ sb1, const T* __restrict__ vb1, T* __restrict__ phib, T* __restrict__ vb_in,
-           T* __restrict__ fpart, int first_block) {
+           T* __restrict__ fpart, int first_block, __nv_bfloat16* __restrict__ phib16) {
   if (*a.d_err & ERRF_EDGE_OVERFLOW) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   T* G1 = reinterpret_cast<T*>(smem_raw);           // [ET][KP]  g_k c
@@ -204,12 +215,13 @@ edge_bwd_k(EdgeArgs<T> a, int FS, int RB, const T* __restrict__ phi, const T* __
     T li0 = T(0), li1 = T(0), li2 = T(0), lv0 = T(0), lv1 = T(0), lv2 = T(0), lph = T(0);
     auto load_local = [&]() {
       const int64_t i = i0 + r;
-      lph = phi[i * 3 * F + c * F + f];
+      lph = ldp<T, PT>(phi + i * 3 * F + c * F + f);
       if (c == 0) li0 = sb1[i * F + f];
       else {
         li0 = vb1[(i * 3 + 0) * F + f]; li1 = vb1[(i * 3 + 1) * F + f]; li2 = vb1[(i * 3 + 2) * F + f];
         if (c == 2 && has_v) {
-          lv0 = v_in[(i * 3 + 0) * F + f]; lv1 = v_in[(i * 3 + 1) * F + f]; lv2 = v_in[(i * 3 + 2) * F + f];
+          lv0 = ldp<T, PT>(v_in + (i * 3 + 0) * F + f); lv1 = ldp<T, PT>(v_in + (i * 3 + 1) * F + f);
+          lv2 = ldp<T, PT>(v_in + (i * 3 + 2) * F + f);
         }
       }
     };
@@ -258,7 +270,7 @@ edge_bwd_k(EdgeArgs<T> a, int FS, int RB, const T* __restrict__ phi, const T* __
         const T wv = fma(bias, Cc[q], dotK<KP>(w, G1 + q * KP));
         const T dw = fma(bias, Cp[q], dotK<KP>(w, G2 + q * KP));
         const T ux = U[q * 4 + 0], uy = U[q * 4 + 1], uz = U[q * 4 + 2];
-        const T phj = phi[j * 3 * F + c * F + f];
+        const T phj = ldp<T, PT>(phi + j * 3 * F + c * F + f);
         if (c == 0) {
           const T sbj = sb1[j * F + f];
           acc0 = fma(sbj, wv, acc0);
@@ -281,8 +293,8 @@ edge_bwd_k(EdgeArgs<T> a, int FS, int RB, const T* __restrict__ phi, const T* __
           } else {
             acc0 = fma(b0, wv, acc0); acc1 = fma(b1, wv, acc1); acc2 = fma(b2, wv, acc2);
             if (has_v) {
-              const T vj0 = v_in[(j * 3 + 0) * F + f], vj1 = v_in[(j * 3 + 1) * F + f],
-                      vj2 = v_in[(j * 3 + 2) * F + f];
+              const T vj0 = ldp<T, PT>(v_in + (j * 3 + 0) * F + f), vj1 = ldp<T, PT>(v_in + (j * 3 + 1) * F + f),
+                      vj2 = ldp<T, PT>(v_in + (j * 3 + 2) * F + f);
               const T Dp = ((li0 * vj0 + li1 * vj1 + li2 * vj2) * phj + (b0 * lv0 + b1 * lv1 + b2 * lv2) * lph) * dw;
               fp0 = fma(Dp, ux, fp0); fp1 = fma(Dp, uy, fp1); fp2 = fma(Dp, uz, fp2);
             }
@@ -300,7 +312,7 @@ edge_bwd_k(EdgeArgs<T> a, int FS, int RB, const T* __restrict__ phi, const T* __
       T* dst = fpart + ((int64_t)blockIdx.y * a.N + i0 + rr) * 3 + ax;
       *dst = first_block ? s : (*dst + s);
     }
-    if (phib != nullptr) {
+    if (phib != nullptr || phib16 != nullptr) {
       // node adjoints: item (r, comp, fl): comp 0,1 phib ss/vs; 2 phib vv; 3..5 vb_in[a]
       for (int idx = tid; idx < nrecv * 6 * FS; idx += nthr) {
         const int rr = idx / (6 * FS), rem = idx % (6 * FS);
@@ -308,17 +320,19 @@ edge_bwd_k(EdgeArgs<T> a, int FS, int RB, const T* __restrict__ phi, const T* __
         const int64_t i = i0 + rr;
         const int fo = blockIdx.y * FS + ff;
         const T* A = Acc + (size_t)(rr * 5) * FS;
-        if (comp < 2) {
-          phib[i * 3 * F + comp * F + fo] = A[comp * FS + ff];
-        } else if (comp == 2) {
+        if (comp < 3) {
           T s = T(0);
-          if (has_v)
-            s = v_in[(i * 3 + 0) * F + fo] * A[2 * FS + ff] + v_in[(i * 3 + 1) * F + fo] * A[3 * FS + ff] +
-                v_in[(i * 3 + 2) * F + fo] * A[4 * FS + ff];
-          phib[i * 3 * F + 2 * F + fo] = s;
+          if (comp < 2) s = A[comp * FS + ff];
+          else if (has_v)
+            s = ldp<T, PT>(v_in + (i * 3 + 0) * F + fo) * A[2 * FS + ff] +
+                ldp<T, PT>(v_in + (i * 3 + 1) * F + fo) * A[3 * FS + ff] +
+                ldp<T, PT>(v_in + (i * 3 + 2) * F + fo) * A[4 * FS + ff];
+          if (phib16) phib16[i * 3 * F + comp * F + fo] = __float2bfloat16_rn((float)s);
+          else phib[i * 3 * F + comp * F + fo] = s;
         } else {
           const int ax = comp - 3;
-          vb_in[(i * 3 + ax) * F + fo] = vb1[(i * 3 + ax) * F + fo] + phi[i * 3 * F + 2 * F + fo] * A[(2 + ax) * FS + ff];
+          vb_in[(i * 3 + ax) * F + fo] =
+              vb1[(i * 3 + ax) * F + fo] + ldp<T, PT>(phi + i * 3 * F + 2 * F + fo) * A[(2 + ax) * FS + ff];
         }
       }
     }
@@ -334,9 +348,9 @@ int pick_rb() { return sizeof(T) == 8 ? 4 : 8; }
 
 int edge_num_slabs(int F) { return (F + 127) / 128; }
 
-template <typename T>
-int launch_edge_fwd(const EdgeArgs<T>& a, const T* phi, const T* s_in, int64_t ld_sin, const T* v_in, T* s1,
-                    int64_t ld_s1, T* v1, cudaStream_t st) {
+template <typename T, typename PT>
+int launch_edge_fwd(const EdgeArgs<T>& a, const PT* phi, const T* s_in, int64_t ld_sin, const PT* v_in,
+                    const T* v_res, T* s1, int64_t ld_s1, T* v1, const EdgeMirror& mir, cudaStream_t st) {
   if (a.N == 0) return 0;
   const int nslab = edge_num_slabs(a.F), FS = a.F / nslab, RB = pick_rb<T>(), KP = pick_kp(a.K);
   const int64_t nwork = (a.N + RB - 1) / RB;
@@ -346,10 +360,11 @@ int launch_edge_fwd(const EdgeArgs<T>& a, const T* phi, const T* s_in, int64_t l
   {                                                                                                           \
     static bool attr_set = false;                                                                             \
     if (!attr_set) {                                                                                          \
-      cudaFuncSetAttribute(edge_fwd_k<T, KPV>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);       \
+      cudaFuncSetAttribute(edge_fwd_k<T, KPV, PT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);   \
       attr_set = true;                                                                                        \
     }                                                                                                         \
-    edge_fwd_k<T, KPV><<<grid, 3 * FS, smem, st>>>(a, FS, RB, phi, s_in, ld_sin, v_in, s1, ld_s1, v1); PNN_KCHECK("edge_fwd_k");\
+    edge_fwd_k<T, KPV, PT><<<grid, 3 * FS, smem, st>>>(a, FS, RB, phi, s_in, ld_sin, v_in, v_res, s1, ld_s1,  \
+                                                       v1, mir); PNN_KCHECK("edge_fwd_k");                    \
   }
   switch (KP) {
     case 8: PNN_LAUNCH_FWD(8) break;
@@ -362,9 +377,9 @@ int launch_edge_fwd(const EdgeArgs<T>& a, const T* phi, const T* s_in, int64_t l
   return 1;
 }
 
-template <typename T>
-int launch_edge_bwd(const EdgeArgs<T>& a, const T* phi, const T* v_in, const T* sb1, const T* vb1, T* phib, T* vb_in,
-                    T* fpart, int first_block, cudaStream_t st) {
+template <typename T, typename PT>
+int launch_edge_bwd(const EdgeArgs<T>& a, const PT* phi, const PT* v_in, const T* sb1, const T* vb1, T* phib,
+                    T* vb_in, T* fpart, int first_block, __nv_bfloat16* phib16, cudaStream_t st) {
   if (a.N == 0) return 0;
   const int nslab = edge_num_slabs(a.F), FS = a.F / nslab, RB = pick_rb<T>(), KP = pick_kp(a.K);
   const int64_t nwork = (a.N + RB - 1) / RB;
@@ -375,11 +390,11 @@ int launch_edge_bwd(const EdgeArgs<T>& a, const T* phi, const T* v_in, const T* 
   {                                                                                                           \
     static bool attr_set = false;                                                                             \
     if (!attr_set) {                                                                                          \
-      cudaFuncSetAttribute(edge_bwd_k<T, KPV>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);       \
+      cudaFuncSetAttribute(edge_bwd_k<T, KPV, PT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);   \
       attr_set = true;                                                                                        \
     }                                                                                                         \
-    edge_bwd_k<T, KPV><<<grid, 3 * FS, smem, st>>>(a, FS, RB, phi, v_in, sb1, vb1, phib, vb_in, fpart,         \
-                                                   first_block); PNN_KCHECK("edge_bwd_k");                    \
+    edge_bwd_k<T, KPV, PT><<<grid, 3 * FS, smem, st>>>(a, FS, RB, phi, v_in, sb1, vb1, phib, vb_in, fpart,     \
+                                                       first_block, phib16); PNN_KCHECK("edge_bwd_k");        \
   }
   switch (KP) {
     case 8: PNN_LAUNCH_BWD(8) break;
@@ -392,13 +407,14 @@ int launch_edge_bwd(const EdgeArgs<T>& a, const T* phi, const T* v_in, const T* 
   return 1;
 }
 
-template int launch_edge_fwd<float>(const EdgeArgs<float>&, const float*, const float*, int64_t, const float*, float*,
-                                    int64_t, float*, cudaStream_t);
-template int launch_edge_fwd<double>(const EdgeArgs<double>&, const double*, const double*, int64_t, const double*,
-                                     double*, int64_t, double*, cudaStream_t);
-template int launch_edge_bwd<float>(const EdgeArgs<float>&, const float*, const float*, const float*, const float*,
-                                    float*, float*, float*, int, cudaStream_t);
-template int launch_edge_bwd<double>(const EdgeArgs<double>&, const double*, const double*, const double*,
-                                     const double*, double*, double*, double*, int, cudaStream_t);
+#define PNN_INST_EDGE(T, PT)                                                                                        \
+  template int launch_edge_fwd<T, PT>(const EdgeArgs<T>&, const PT*, const T*, int64_t, const PT*, const T*, T*,    \
+                                      int64_t, T*, const EdgeMirror&, cudaStream_t);                               \
+  template int launch_edge_bwd<T, PT>(const EdgeArgs<T>&, const PT*, const PT*, const T*, const T*, T*, T*, T*,    \
+                                      int, __nv_bfloat16*, cudaStream_t);
+PNN_INST_EDGE(float, float)
+PNN_INST_EDGE(double, double)
+PNN_INST_EDGE(float, __nv_bfloat16)
+#undef PNN_INST_EDGE
 
 } // namespace pnn

@@ -1,0 +1,33 @@
+// edge_mma.cuh — edge kernels of the BF16 model with the filter contraction on the tensor cores (edge_mma.cu).
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "common.cuh"
+
+namespace pnn {
+
+struct EdgeMmaArgs {
+  int64_t N;
+  int F, K;
+  float rc;
+  const int32_t* rowptr;
+  const int32_t* col;
+  const Geom<float>* geom;
+  // Filter of one block packed for the MMA B operand, BF16: KP = edge_mma_kp(K) columns per row
+  // (k < K: flt_W[row][k]; k == K: flt_b[row]; then zeros), rows ordered [chunk c][32-feature slab s][n-tile nt][g]
+  // with feature f = s*32 + (g>>1)*8 + nt*2 + (g&1)  — the column permutation that gives every thread of the
+  // accumulator fragment 8 contiguous features.
+  const __nv_bfloat16* fltP;
+  const int* d_err;
+};
+
+int edge_mma_kp(int K);
+void pack_filter_bf16(int F, int K, const double* fltW, const double* fltb, uint16_t* out);
+
+int launch_edge_fwd_mma(const EdgeMmaArgs& a, const __nv_bfloat16* phi, const float* s_in, int64_t ld_sin,
+                        const __nv_bfloat16* v_in, const float* v_res, float* s1, int64_t ld_s1, float* v1,
+                        const EdgeMirror& mir, cudaStream_t st);
+
+} // namespace pnn

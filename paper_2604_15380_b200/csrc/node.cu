@@ -13,7 +13,8 @@ constexpr int RT = 16; // atoms per readout tile
 
 template <typename T>
 __global__ void __launch_bounds__(256) embed_k(int64_t N, int F, int Zmax, const int32_t* __restrict__ Z,
-                                               const T* __restrict__ emb, T* __restrict__ s, int* d_err) {
+                                               const T* __restrict__ emb, T* __restrict__ s, int* d_err,
+                                               __nv_bfloat16* __restrict__ s16) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= N * F) return;
   const int64_t i = idx / F;
@@ -23,25 +24,31 @@ __global__ void __launch_bounds__(256) embed_k(int64_t N, int F, int Zmax, const
     if (f == 0) atomicOr(d_err, ERRF_BAD_Z);
     z = 1;
   }
-  s[idx] = emb[(int64_t)z * F + f];
+  const T e = emb[(int64_t)z * F + f];
+  s[idx] = e;
+  if (s16) s16[idx] = __float2bfloat16_rn((float)e);
 }
 
 // PQ [N][3][2F] (P | Q)  ->  sn[:, F:2F] = sqrt(sum_a Q_a^2 + eps)          (B4)
 template <typename T>
-__global__ void __launch_bounds__(256) norm_k(int64_t N, int F, const T* __restrict__ PQ, T* __restrict__ sn, T eps) {
+__global__ void __launch_bounds__(256) norm_k(int64_t N, int F, const T* __restrict__ PQ, T* __restrict__ sn, T eps,
+                                              __nv_bfloat16* __restrict__ sn16) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= N * F) return;
   const int64_t i = idx / F;
   const int f = (int)(idx % F);
   const T q0 = PQ[(i * 3 + 0) * 2 * F + F + f], q1 = PQ[(i * 3 + 1) * 2 * F + F + f], q2 = PQ[(i * 3 + 2) * 2 * F + F + f];
-  sn[i * 2 * F + F + f] = sqrt(q0 * q0 + q1 * q1 + q2 * q2 + eps);
+  const T n = sqrt(q0 * q0 + q1 * q1 + q2 * q2 + eps);
+  if (sn16) sn16[i * 2 * F + F + f] = __float2bfloat16_rn((float)n);
+  else sn[i * 2 * F + F + f] = n;
 }
 
 // s'' = s' + a_sv <P,Q> + a_ss ;  v'' = v' + a_vv P                          (B4)
 template <typename T>
 __global__ void __launch_bounds__(256) update_k(int64_t N, int F, const T* __restrict__ sn, const T* __restrict__ v1,
                                                 const T* __restrict__ PQ, const T* __restrict__ a,
-                                                T* __restrict__ s_out, T* __restrict__ v_out) {
+                                                T* __restrict__ s_out, T* __restrict__ v_out,
+                                                __nv_bfloat16* __restrict__ s16, __nv_bfloat16* __restrict__ v16) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= N * F) return;
   const int64_t i = idx / F;
@@ -52,9 +59,15 @@ __global__ void __launch_bounds__(256) update_k(int64_t N, int F, const T* __res
   for (int ax = 0; ax < 3; ++ax) {
     const T p = PQ[(i * 3 + ax) * 2 * F + f], q = PQ[(i * 3 + ax) * 2 * F + F + f];
     dot = fma(p, q, dot);
-    if (v_out) v_out[(i * 3 + ax) * F + f] = fma(avv, p, v1[(i * 3 + ax) * F + f]);
+    if (v_out) {
+      const T r = fma(avv, p, v1[(i * 3 + ax) * F + f]);
+      v_out[(i * 3 + ax) * F + f] = r;
+      if (v16) v16[(i * 3 + ax) * F + f] = __float2bfloat16_rn((float)r);
+    }
   }
-  s_out[idx] = sn[i * 2 * F + f] + asv * dot + ass;
+  const T r = sn[i * 2 * F + f] + asv * dot + ass;
+  s_out[idx] = r;
+  if (s16) s16[idx] = __float2bfloat16_rn((float)r);
 }
 
 // R2, first half: a-bar [N,3F] and the direct parts of P-bar, Q-bar [N][3][2F]
@@ -62,7 +75,7 @@ template <typename T>
 __global__ void __launch_bounds__(256) update_bwd1_k(int64_t N, int F, const T* __restrict__ sb,
                                                      const T* __restrict__ vb, const T* __restrict__ a,
                                                      const T* __restrict__ PQ, T* __restrict__ ab,
-                                                     T* __restrict__ PQb) {
+                                                     T* __restrict__ PQb, __nv_bfloat16* __restrict__ ab16) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= N * F) return;
   const int64_t i = idx / F;
@@ -79,9 +92,15 @@ __global__ void __launch_bounds__(256) update_bwd1_k(int64_t N, int F, const T* 
     dot = fma(p[ax], q[ax], dot);
     avvb = fma(vbf[ax], p[ax], avvb);
   }
-  ab[i * 3 * F + f] = avvb;
-  ab[i * 3 * F + F + f] = sbf * dot;
-  ab[i * 3 * F + 2 * F + f] = sbf;
+  if (ab16) {
+    ab16[i * 3 * F + f] = __float2bfloat16_rn((float)avvb);
+    ab16[i * 3 * F + F + f] = __float2bfloat16_rn((float)(sbf * dot));
+    ab16[i * 3 * F + 2 * F + f] = __float2bfloat16_rn((float)sbf);
+  } else {
+    ab[i * 3 * F + f] = avvb;
+    ab[i * 3 * F + F + f] = sbf * dot;
+    ab[i * 3 * F + 2 * F + f] = sbf;
+  }
   const T dotb = sbf * asv;
 #pragma unroll
   for (int ax = 0; ax < 3; ++ax) {
@@ -94,7 +113,7 @@ __global__ void __launch_bounds__(256) update_bwd1_k(int64_t N, int F, const T* 
 template <typename T>
 __global__ void __launch_bounds__(256) update_bwd2_k(int64_t N, int F, const T* __restrict__ zb,
                                                      const T* __restrict__ PQ, T eps, T* __restrict__ sb,
-                                                     T* __restrict__ PQb) {
+                                                     T* __restrict__ PQb, __nv_bfloat16* __restrict__ PQb16) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= N * F) return;
   const int64_t i = idx / F;
@@ -103,9 +122,18 @@ __global__ void __launch_bounds__(256) update_bwd2_k(int64_t N, int F, const T* 
   const T nb = zb[i * 2 * F + F + f];
   const T q0 = PQ[(i * 3 + 0) * 2 * F + F + f], q1 = PQ[(i * 3 + 1) * 2 * F + F + f], q2 = PQ[(i * 3 + 2) * 2 * F + F + f];
   const T r = nb / sqrt(q0 * q0 + q1 * q1 + q2 * q2 + eps);
-  PQb[(i * 3 + 0) * 2 * F + F + f] += r * q0;
-  PQb[(i * 3 + 1) * 2 * F + F + f] += r * q1;
-  PQb[(i * 3 + 2) * 2 * F + F + f] += r * q2;
+  const T qq[3] = {q0, q1, q2};
+#pragma unroll
+  for (int ax = 0; ax < 3; ++ax) {
+    const int64_t o = (i * 3 + ax) * 2 * F + f;
+    const T qb = PQb[o + F] + r * qq[ax];
+    if (PQb16) {
+      PQb16[o] = __float2bfloat16_rn((float)PQb[o]);
+      PQb16[o + F] = __float2bfloat16_rn((float)qb);
+    } else {
+      PQb[o + F] = qb;
+    }
+  }
 }
 
 // ------------------------------------------------------------------------------------------ readout
@@ -245,35 +273,37 @@ inline unsigned nblk(int64_t n, int b) { return (unsigned)((n + b - 1) / b); }
 } // namespace
 
 template <typename T>
-int launch_embed(int64_t N, int F, int Zmax, const int32_t* Z, const T* emb, T* s, int* d_err, cudaStream_t st) {
+int launch_embed(int64_t N, int F, int Zmax, const int32_t* Z, const T* emb, T* s, int* d_err, cudaStream_t st,
+                 __nv_bfloat16* s16) {
   if (N == 0) return 0;
-  embed_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, Zmax, Z, emb, s, d_err); PNN_KCHECK("embed_k");
+  embed_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, Zmax, Z, emb, s, d_err, s16); PNN_KCHECK("embed_k");
   return 1;
 }
 template <typename T>
-int launch_norm(int64_t N, int F, const T* PQ, T* sn, T eps, cudaStream_t st) {
+int launch_norm(int64_t N, int F, const T* PQ, T* sn, T eps, cudaStream_t st, __nv_bfloat16* sn16) {
   if (N == 0) return 0;
-  norm_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, PQ, sn, eps); PNN_KCHECK("norm_k");
+  norm_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, PQ, sn, eps, sn16); PNN_KCHECK("norm_k");
   return 1;
 }
 template <typename T>
 int launch_update(int64_t N, int F, const T* sn, const T* v1, const T* PQ, const T* a, T* s_out, T* v_out,
-                  cudaStream_t st) {
+                  cudaStream_t st, __nv_bfloat16* s16, __nv_bfloat16* v16) {
   if (N == 0) return 0;
-  update_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, sn, v1, PQ, a, s_out, v_out); PNN_KCHECK("update_k");
+  update_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, sn, v1, PQ, a, s_out, v_out, s16, v16); PNN_KCHECK("update_k");
   return 1;
 }
 template <typename T>
 int launch_update_bwd1(int64_t N, int F, const T* sb, const T* vb, const T* a, const T* PQ, T* ab, T* PQb,
-                       cudaStream_t st) {
+                       cudaStream_t st, __nv_bfloat16* ab16) {
   if (N == 0) return 0;
-  update_bwd1_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, sb, vb, a, PQ, ab, PQb); PNN_KCHECK("update_bwd1_k");
+  update_bwd1_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, sb, vb, a, PQ, ab, PQb, ab16); PNN_KCHECK("update_bwd1_k");
   return 1;
 }
 template <typename T>
-int launch_update_bwd2(int64_t N, int F, const T* zb, const T* PQ, T eps, T* sb, T* PQb, cudaStream_t st) {
+int launch_update_bwd2(int64_t N, int F, const T* zb, const T* PQ, T eps, T* sb, T* PQb, cudaStream_t st,
+                       __nv_bfloat16* PQb16) {
   if (N == 0) return 0;
-  update_bwd2_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, zb, PQ, eps, sb, PQb); PNN_KCHECK("update_bwd2_k");
+  update_bwd2_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, zb, PQ, eps, sb, PQb, PQb16); PNN_KCHECK("update_bwd2_k");
   return 1;
 }
 template <typename T>
@@ -313,11 +343,14 @@ int launch_force_assemble(int64_t N, int nslab, const T* fpart, T* forces, cudaS
 }
 
 #define PNN_INST(T)                                                                                                  \
-  template int launch_embed<T>(int64_t, int, int, const int32_t*, const T*, T*, int*, cudaStream_t);                 \
-  template int launch_norm<T>(int64_t, int, const T*, T*, T, cudaStream_t);                                          \
-  template int launch_update<T>(int64_t, int, const T*, const T*, const T*, const T*, T*, T*, cudaStream_t);         \
-  template int launch_update_bwd1<T>(int64_t, int, const T*, const T*, const T*, const T*, T*, T*, cudaStream_t);    \
-  template int launch_update_bwd2<T>(int64_t, int, const T*, const T*, T, T*, T*, cudaStream_t);                     \
+  template int launch_embed<T>(int64_t, int, int, const int32_t*, const T*, T*, int*, cudaStream_t,                  \
+                               __nv_bfloat16*);                                                                      \
+  template int launch_norm<T>(int64_t, int, const T*, T*, T, cudaStream_t, __nv_bfloat16*);                          \
+  template int launch_update<T>(int64_t, int, const T*, const T*, const T*, const T*, T*, T*, cudaStream_t,          \
+                                __nv_bfloat16*, __nv_bfloat16*);                                                     \
+  template int launch_update_bwd1<T>(int64_t, int, const T*, const T*, const T*, const T*, T*, T*, cudaStream_t,     \
+                                     __nv_bfloat16*);                                                                \
+  template int launch_update_bwd2<T>(int64_t, int, const T*, const T*, T, T*, T*, cudaStream_t, __nv_bfloat16*);     \
   template int launch_readout<T>(int64_t, int64_t, int, int, const T*, const int32_t*, const int32_t*,               \
                                  const int32_t*, const T*, const T*, const T*, const T*, T*, T*, T*, int*,           \
                                  cudaStream_t);                                                                      \

@@ -1,6 +1,7 @@
 // pnn_api.cu — the C ABI of include/pnn.h: model upload, workspace arena, and the launch sequences of the hot path
 // (SURVEY.md §8(a) a1..a7).  Every step of the path runs in this library's kernels; there is no CPU fallback.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -8,6 +9,7 @@
 
 #include "../../include/pnn.h"
 #include "common.cuh"
+#include "edge_mma.cuh"
 #include "gemm_tc.cuh"
 
 using namespace pnn;
@@ -80,6 +82,8 @@ struct pnn_model {
   std::vector<BlockW> blk;
   int64_t oW1t = 0, oW1 = 0, ob1 = 0, ow2 = 0, ob2 = 0; // heads: [H][F][Fh], [H][Fh][F], [H][Fh], [H][Fh], [H]
   __nv_bfloat16* d_wb = nullptr;                        // BF16 copy of d_w (same offsets): tcgen05 GEMM operands
+  __nv_bfloat16* d_fltP = nullptr;                      // BF16 model: per block, the filter packed for edge_mma.cu
+  int64_t fltP_stride = 0;                              // elements per block
 };
 
 struct pnn_workspace {
@@ -98,6 +102,13 @@ struct pnn_workspace {
   std::vector<Tape> tape;
   // adjoints
   void *sb, *vb, *vb2, *ab, *PQb, *kb, *zb, *phib, *hb, *fpart;
+  // BF16 model: BF16 copies that feed the tensor-core GEMMs and the edge gathers (reading Q19)
+  struct Mirror {
+    __nv_bfloat16 *s16, *h16, *sn16, *v1_16, *k16, *vping16[2];
+    __nv_bfloat16 *ab16, *kb16, *PQb16, *phib16, *hb16;
+  } mb{};
+  struct Tape16 { __nv_bfloat16 *vin16, *phi16; };
+  std::vector<Tape16> tape16;
   // staging for pnn_eval_host
   int32_t *st_Z, *st_sptr, *st_head;
   double *st_pos, *st_cell;
@@ -238,6 +249,21 @@ int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, 
     if (!cuda_ok(cudaDeviceSynchronize(), "bf16 weight conversion") || launch_failed()) {
       cudaFree(m->d_wb); cudaFree(m->d_w); delete m; return PNN_ERR_CUDA;
     }
+    // filters packed for the tensor-core edge kernels (edge_mma.cuh)
+    m->fltP_stride = 3 * F * edge_mma_kp(cfg->K);
+    std::vector<uint16_t> fp((size_t)cfg->T * m->fltP_stride);
+    {
+      const double* q = w + (int64_t)(cfg->Zmax + 1) * F;
+      const int64_t per_block = 11 * F * F + 3 * F * K + 11 * F;
+      for (int t = 0; t < cfg->T; ++t) {
+        const double* fW = q + t * per_block + (F * F + F + 3 * F * F + 3 * F);
+        pack_filter_bf16((int)F, (int)K, fW, fW + 3 * F * K, fp.data() + (size_t)t * m->fltP_stride);
+      }
+    }
+    if (!cuda_ok(cudaMalloc((void**)&m->d_fltP, fp.size() * 2), "cudaMalloc(packed filters)") ||
+        !cuda_ok(cudaMemcpy(m->d_fltP, fp.data(), fp.size() * 2, cudaMemcpyHostToDevice), "cudaMemcpy(packed filters)")) {
+      cudaFree(m->d_fltP); cudaFree(m->d_wb); cudaFree(m->d_w); delete m; return PNN_ERR_CUDA;
+    }
   }
   *out = m;
   return PNN_OK;
@@ -245,6 +271,7 @@ int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, 
 
 void pnn_model_destroy(pnn_model* m) {
   if (!m) return;
+  cudaFree(m->d_fltP);
   cudaFree(m->d_wb);
   cudaFree(m->d_w);
   delete m;
@@ -327,6 +354,26 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
       ws->vping[0] = carve(es * N * 3 * F);
       ws->vping[1] = carve(es * N * 3 * F);
       ws->sb = ws->vb = ws->vb2 = ws->ab = ws->PQb = ws->kb = ws->zb = ws->phib = ws->hb = ws->fpart = nullptr;
+    }
+    if (m->cfg.prec == PNN_BF16) {
+      auto c16 = [&](int64_t n) { return (__nv_bfloat16*)carve(2 * n); };
+      pnn_workspace::Mirror& b = ws->mb;
+      b.s16 = c16(N * F); b.h16 = c16(N * F); b.sn16 = c16(N * 2 * F); b.v1_16 = c16(N * 3 * F); b.k16 = c16(N * F);
+      ws->tape16.resize(want_forces ? T : 1);
+      if (want_forces) {
+        for (int t = 0; t < T; ++t) {
+          ws->tape16[t].vin16 = (t == 0) ? nullptr : c16(N * 3 * F);
+          ws->tape16[t].phi16 = c16(N * 3 * F);
+        }
+        b.vping16[0] = b.vping16[1] = nullptr;
+        b.ab16 = c16(N * 3 * F); b.kb16 = c16(N * F); b.PQb16 = c16(N * 6 * F); b.phib16 = c16(N * 3 * F);
+        b.hb16 = c16(N * F);
+      } else {
+        ws->tape16[0].vin16 = nullptr;
+        ws->tape16[0].phi16 = c16(N * 3 * F);
+        b.vping16[0] = c16(N * 3 * F); b.vping16[1] = c16(N * 3 * F);
+        b.ab16 = b.kb16 = b.PQb16 = b.phib16 = b.hb16 = nullptr;
+      }
     }
     ws->st_Z = (int32_t*)carve(4 * N);
     ws->st_sptr = (int32_t*)carve(4 * (S + 1));
@@ -492,7 +539,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       nl += l_; ps_.done(l_); }
     ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
     { ProfScope ps_(ws, st, "edge_fwd");
-    const int l_ = launch_edge_fwd<T>(ea, phi, s_cur, F, v_in, sn, 2 * F, v1, st);                // B3b -> s' in sn[:, :F], v'
+    const int l_ = launch_edge_fwd<T, T>(ea, phi, s_cur, F, v_in, v_in, sn, 2 * F, v1, EdgeMirror(), st); // B3b -> s' in sn[:, :F], v'
       nl += l_; ps_.done(l_); }
     GemmEpi<T> e3;
     { ProfScope ps_(ws, st, "gemm_3N");
@@ -549,8 +596,8 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       // R3 + R4
       ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
       { ProfScope ps_(ws, st, "edge_bwd");
-      const int l_ = launch_edge_bwd<T>(ea, (const T*)tp.phi, (const T*)tp.v_in, sb, vb, t > 0 ? phib : nullptr, vb2, fpart,
-                               last ? 1 : 0, st);
+      const int l_ = launch_edge_bwd<T, T>(ea, (const T*)tp.phi, (const T*)tp.v_in, sb, vb, t > 0 ? phib : nullptr, vb2,
+                                           fpart, last ? 1 : 0, nullptr, st);
         nl += l_; ps_.done(l_); }
       if (t > 0) {
         GemmEpi<T> g4; g4.act = ACT_MUL_DSILU; g4.aux = (const T*)tp.hpre; g4.ldaux = F;
@@ -570,6 +617,130 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
   }
   ws->launches += nl;
   return PNN_OK;
+}
+
+// The BF16 model (reading Q19): every Linear runs on the tcgen05 tensor cores with BF16 operands and FP32
+// accumulation (gemm_tc.cu); the gathered sender payloads phi_j, v_j are BF16; geometry, radial basis, cutoff,
+// segment sums, the residual streams s, v, the adjoint streams, energies and forces stay FP32.
+int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const int32_t* sptr,
+              const int32_t* head, int flags, float* energy, float* forces, cudaStream_t st) {
+  typedef float T;
+  typedef __nv_bfloat16 B;
+  const pnn_config& c = m->cfg;
+  const int F = c.F, T_ = c.T;
+  const bool want_f = (flags & PNN_FORCES) != 0;
+  const T* W = (const T*)m->d_w;
+  const B* Wb = m->d_wb;
+  int nl = 0;
+  bool tc_fail = false;
+  EdgeArgs<T> ea;
+  ea.N = N; ea.F = F; ea.K = c.K; ea.rc = c.cutoff;
+  ea.rowptr = ws->g.rowptr; ea.col = ws->g.col; ea.geom = (const Geom<T>*)ws->g.geom; ea.d_err = ws->g.d_err;
+  T* s_cur = (T*)ws->s_cur; T* sn = (T*)ws->sn; T* v1 = (T*)ws->v1;
+  pnn_workspace::Mirror& mb = ws->mb;
+  const bool taped = ws->want_forces != 0;
+  EdgeMmaArgs em;
+  em.N = N; em.F = F; em.K = c.K; em.rc = (float)c.cutoff; em.rowptr = ws->g.rowptr; em.col = ws->g.col;
+  em.geom = (const Geom<float>*)ws->g.geom; em.d_err = ws->g.d_err;
+  static const bool simt_edges = getenv("PNN_BF16_SIMT_EDGES") != nullptr; // debugging aid: the SIMT edge kernels
+  // C / Cb [M,N] = epi(A[M,K] . Wt[N,K]^T): A BF16 (row stride lda), Wt at element offset woff of the BF16 weight copy
+  auto tc = [&](const char* fam, int64_t M, int Nn, int K, const B* A, int64_t lda, int64_t woff, const TcEpi& e) {
+    ProfScope ps_(ws, st, fam);
+    const int l_ = launch_gemm_tc(M, Nn, K, A, lda, Wb + woff, K, e, st);
+    if (l_ < 0) { tc_fail = true; return; }
+    nl += l_; ps_.done(l_);
+  };
+
+  { ProfScope ps_(ws, st, "embed");
+    const int l_ = launch_embed<T>(N, F, c.Zmax, Z, W + m->emb, s_cur, ws->g.d_err, st, mb.s16);
+    nl += l_; ps_.done(l_); }
+  for (int t = 0; t < T_; ++t) {
+    const BlockW& b = m->blk[t];
+    const pnn_workspace::Tape& tp = ws->tape[taped ? t : 0];
+    const pnn_workspace::Tape16& tp16 = ws->tape16[taped ? t : 0];
+    const T* v_in; T* v_out; const B* v_in16; B* v_out16;
+    if (taped) {
+      v_in = (const T*)tp.v_in; v_in16 = tp16.vin16;
+      v_out = (t + 1 < T_) ? (T*)ws->tape[t + 1].v_in : nullptr;
+      v_out16 = (t + 1 < T_) ? ws->tape16[t + 1].vin16 : nullptr;
+    } else {
+      v_in = (t == 0) ? nullptr : (const T*)ws->vping[(t - 1) & 1];
+      v_in16 = (t == 0) ? nullptr : mb.vping16[(t - 1) & 1];
+      v_out = (t + 1 < T_) ? (T*)ws->vping[t & 1] : nullptr;
+      v_out16 = (t + 1 < T_) ? mb.vping16[t & 1] : nullptr;
+    }
+    T* PQ = (T*)tp.PQ; T* a = (T*)tp.a;
+    TcEpi e1; e1.bias = W + b.b1; e1.act = ACT_SILU; e1.pre = (T*)tp.hpre; e1.ldpre = F; e1.Cb = mb.h16; e1.ldcb = F;
+    tc("gemm_N", N, F, F, mb.s16, F, b.W1, e1);                                   // B3a: h = silu(W1 s + b1)
+    TcEpi e2; e2.bias = W + b.b2; e2.Cb = tp16.phi16; e2.ldcb = 3 * F;
+    tc("gemm_N", N, 3 * F, F, mb.h16, F, b.W2, e2);                               // B3a: phi = W2 h + b2
+    ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
+    { ProfScope ps_(ws, st, "edge_fwd");
+      EdgeMirror mir; mir.s1 = mb.sn16; mir.ld_s1 = 2 * F; mir.v1 = mb.v1_16;
+      em.fltP = m->d_fltP + (int64_t)t * m->fltP_stride;
+      const int l_ = simt_edges ? launch_edge_fwd<T, B>(ea, tp16.phi16, s_cur, F, v_in16, v_in, sn, 2 * F, v1, mir, st)
+                                : launch_edge_fwd_mma(em, tp16.phi16, s_cur, F, v_in16, v_in, sn, 2 * F, v1, mir, st); // B3b
+      nl += l_; ps_.done(l_); }
+    TcEpi e3; e3.C = PQ; e3.ldc = 2 * F;
+    tc("gemm_3N", 3 * N, 2 * F, F, mb.v1_16, F, b.UV, e3);                         // B4: P | Q
+    { ProfScope ps_(ws, st, "update_elementwise");
+      const int l_ = launch_norm<T>(N, F, PQ, sn, (T)c.norm_eps, st, mb.sn16);
+      nl += l_; ps_.done(l_); }
+    TcEpi e4; e4.bias = W + b.c1; e4.act = ACT_SILU; e4.pre = (T*)tp.kpre; e4.ldpre = F; e4.Cb = mb.k16; e4.ldcb = F;
+    tc("gemm_N", N, F, 2 * F, mb.sn16, 2 * F, b.A1, e4);
+    TcEpi e5; e5.bias = W + b.c2; e5.C = a; e5.ldc = 3 * F;
+    tc("gemm_N", N, 3 * F, F, mb.k16, F, b.A2, e5);
+    { ProfScope ps_(ws, st, "update_elementwise");
+      const int l_ = launch_update<T>(N, F, sn, v1, PQ, a, s_cur, v_out, st, mb.s16, v_out16);
+      nl += l_; ps_.done(l_); }
+  }
+  { ProfScope ps_(ws, st, "readout");
+    const int l_ = launch_readout<T>(N, S, F, c.H, s_cur, ws->g.a2s, head, sptr, W + m->oW1t, W + m->ob1, W + m->ow2,
+                                     W + m->ob2, (T*)ws->opre, (T*)ws->eatom, energy, ws->g.d_err, st);
+    nl += l_; ps_.done(l_); }
+  if (want_f) {
+    T* sb = (T*)ws->sb; T* vb = (T*)ws->vb; T* vb2 = (T*)ws->vb2; T* PQb = (T*)ws->PQb; T* zb = (T*)ws->zb;
+    T* fpart = (T*)ws->fpart;
+    { ProfScope ps_(ws, st, "readout_bwd");
+      const int l_ = launch_readout_bwd<T>(N, F, c.H, (const T*)ws->opre, ws->g.a2s, head, W + m->oW1, W + m->ow2, sb, st);
+      nl += l_; ps_.done(l_); }
+    for (int t = T_ - 1; t >= 0; --t) {
+      const BlockW& b = m->blk[t];
+      const pnn_workspace::Tape& tp = ws->tape[t];
+      const pnn_workspace::Tape16& tp16 = ws->tape16[t];
+      const bool last = (t == T_ - 1);
+      { ProfScope ps_(ws, st, "update_bwd_elementwise");
+        const int l_ = launch_update_bwd1<T>(N, F, sb, last ? nullptr : vb, (const T*)tp.a, (const T*)tp.PQ, nullptr, PQb,
+                                             st, mb.ab16);
+        nl += l_; ps_.done(l_); }
+      TcEpi g1; g1.act = ACT_MUL_DSILU; g1.aux = (const T*)tp.kpre; g1.ldaux = F; g1.Cb = mb.kb16; g1.ldcb = F;
+      tc("gemm_N", N, F, 3 * F, mb.ab16, 3 * F, b.A2t, g1);                        // k-bar = A2^T a-bar . silu'
+      TcEpi g2; g2.C = zb; g2.ldc = 2 * F;
+      tc("gemm_N", N, 2 * F, F, mb.kb16, F, b.A1t, g2);                            // z-bar = A1^T k-bar
+      { ProfScope ps_(ws, st, "update_bwd_elementwise");
+        const int l_ = launch_update_bwd2<T>(N, F, zb, (const T*)tp.PQ, (T)c.norm_eps, sb, PQb, st, mb.PQb16);
+        nl += l_; ps_.done(l_); }
+      TcEpi g3; g3.accumulate = last ? 0 : 1; g3.C = vb; g3.ldc = F;
+      tc("gemm_3N", 3 * N, F, 2 * F, mb.PQb16, 2 * F, b.UVt, g3);                  // v-bar' += U^T P-bar + V^T Q-bar
+      ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
+      { ProfScope ps_(ws, st, "edge_bwd");
+        const int l_ = launch_edge_bwd<T, B>(ea, tp16.phi16, tp16.vin16, sb, vb, nullptr, vb2, fpart, last ? 1 : 0,
+                                             t > 0 ? mb.phib16 : nullptr, st);
+        nl += l_; ps_.done(l_); }
+      if (t > 0) {
+        TcEpi g4; g4.act = ACT_MUL_DSILU; g4.aux = (const T*)tp.hpre; g4.ldaux = F; g4.Cb = mb.hb16; g4.ldcb = F;
+        tc("gemm_N", N, F, 3 * F, mb.phib16, 3 * F, b.W2t, g4);
+        TcEpi g5; g5.accumulate = 1; g5.C = sb; g5.ldc = F;
+        tc("gemm_N", N, F, F, mb.hb16, F, b.W1t, g5);
+        T* tmp = vb; vb = vb2; vb2 = tmp;
+      }
+    }
+    { ProfScope ps_(ws, st, "force_assemble");
+      const int l_ = launch_force_assemble<T>(N, edge_num_slabs(F), fpart, forces, st);
+      nl += l_; ps_.done(l_); }
+  }
+  ws->launches += nl;
+  return tc_fail ? PNN_ERR_UNSUPPORTED : PNN_OK;
 }
 
 } // namespace
@@ -592,7 +763,7 @@ int pnn_eval(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const 
   else if (m->cfg.prec == PNN_FP32)
     rc = eval_simt<float>(m, ws, N, S, Z, sptr, head, flags, (float*)energy, (float*)forces, st);
   else
-    return PNN_ERR_UNSUPPORTED;
+    rc = eval_bf16(m, ws, N, S, Z, sptr, head, flags, (float*)energy, (float*)forces, st);
   if (rc != PNN_OK) return rc;
   if (launch_failed()) return PNN_ERR_CUDA;
   PNN_TRY(cudaGetLastError());
