@@ -132,7 +132,8 @@ int pnn_profile_read(pnn_workspace* ws, int max_entries, char* names, double* to
  * tensor pipe): C[M,N] = act( A[M,K] . Wt[N,K]^T + bias ), A / Wt DEVICE BF16 row-major with row strides lda / ldw
  * (elements), FP32 accumulation on tcgen05 tensor cores.  bias DEVICE f32 [N] or NULL; act 0 = none, 1 = SiLU.
  * C DEVICE f32 (row stride ldc) and / or Cb DEVICE bf16 (row stride ldcb); either may be NULL.  N and K multiples of
- * 32, lda / ldw multiples of 8.  Asynchronous. */
+ * 32, lda / ldw / ldcb multiples of 8, ldc a multiple of 4, all base pointers 16-byte aligned (PNN_ERR_INVALID_ARG
+ * otherwise).  Asynchronous. */
 int pnn_gemm_bf16(int64_t M, int32_t N, int32_t K, const void* A, int64_t lda, const void* Wt, int64_t ldw,
                   const float* bias, int32_t act, float* C, int64_t ldc, void* Cb, int64_t ldcb, void* cuda_stream);
 

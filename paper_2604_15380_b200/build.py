@@ -16,7 +16,7 @@ LIB = os.path.join(HERE, "libpnn.so")
 SOURCES = ["pnn_api.cu", "graph.cu", "gemm_simt.cu", "gemm_tc.cu", "edge.cu", "edge_mma.cu", "node.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
-         "--expt-relaxed-constexpr", "-Xptxas", "-v"]
+         "--expt-relaxed-constexpr", "--extended-lambda", "-Xptxas", "-v"]
 
 
 def _newer(path: str, than: float) -> bool:

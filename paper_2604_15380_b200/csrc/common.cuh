@@ -143,7 +143,7 @@ int launch_update_bwd1(int64_t N, int F, const T* sb, const T* vb, const T* a, c
                        cudaStream_t st, __nv_bfloat16* ab16 = nullptr);
 template <typename T>
 int launch_update_bwd2(int64_t N, int F, const T* zb, const T* PQ, T eps, T* sb, T* PQb, cudaStream_t st,
-                       __nv_bfloat16* PQb16 = nullptr);
+                       __nv_bfloat16* PQb16 = nullptr, __nv_bfloat16* sb16 = nullptr);
 // readout (B5 / R1).  W1t: [H][F][F/2] (transposed), W1: [H][F/2][F], b1 [H][F/2], w2 [H][F/2], b2 [H].
 template <typename T>
 int launch_readout(int64_t N, int64_t S, int F, int H, const T* s, const int32_t* a2s, const int32_t* head,

@@ -30,4 +30,13 @@ int launch_edge_fwd_mma(const EdgeMmaArgs& a, const __nv_bfloat16* phi, const fl
                         const __nv_bfloat16* v_in, const float* v_res, float* s1, int64_t ld_s1, float* v1,
                         const EdgeMirror& mir, cudaStream_t st);
 
+// Reverse message step (R3 + R4 partial).  phi / v_in: forward tape (BF16); sb16 [N,F], vb16 [N,3F]: BF16 copies of the
+// incoming adjoints s-bar', v-bar' (gathered and own rows); vb1: the FP32 v-bar' (residual of v-bar_in).  Writes
+// phib16 [N,3F] (BF16) and vb_in [N,3F] (FP32) when v_in != NULL (blocks t > 0; for t = 0 only forces are produced) and
+// adds the block's force contribution into fpart [edge_mma_num_slabs(F)][N][3].
+int launch_edge_bwd_mma(const EdgeMmaArgs& a, const __nv_bfloat16* phi, const __nv_bfloat16* v_in,
+                        const __nv_bfloat16* sb16, const __nv_bfloat16* vb16, const float* vb1, __nv_bfloat16* phib16,
+                        float* vb_in, float* fpart, int first_block, cudaStream_t st);
+int edge_mma_num_slabs(int F);
+
 } // namespace pnn

@@ -170,37 +170,68 @@ tc_gemm_k(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
       umma_commit(acc_bar);
     }
   } else {
-    // epilogue warps 2..5: TMEM lane quadrant = warp % 4
+    // epilogue warps 2..5: TMEM lane quadrant = warp % 4; a thread owns one output row and walks it 32 columns at a
+    // time (tcgen05.ld 32x32b.x32), so every global access is a 16-byte vector of that row
     const int q = warp & 3;
     mbar_wait(acc_bar, 0);
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    float* Tb = reinterpret_cast<float*>(tiles_ptr) + (warp - 2) * 32 * 33; // stage ring is free once acc_bar fired
-    const int64_t mrow0 = m0 + q * 32;
+    const int64_t m = m0 + q * 32 + lane;
+    const bool row_ok = m < M;
 #pragma unroll 1
     for (int c0 = 0; c0 < BN; c0 += 32) {
       uint32_t r[32];
       tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)c0, r);
+      if (!row_ok) continue;
+      const int n = n0 + c0;
+      float x[32];
 #pragma unroll
-      for (int j = 0; j < 32; ++j) Tb[lane * 33 + j] = __uint_as_float(r[j]);
-      __syncwarp();
-      const int n = n0 + c0 + lane;
-      const float bv = epi.bias ? epi.bias[n] : 0.0f;
-#pragma unroll 4
-      for (int rr = 0; rr < 32; ++rr) {
-        const int64_t m = mrow0 + rr;
-        if (m >= M) break;
-        float x = Tb[rr * 33 + lane] + bv;
-        if (epi.act == ACT_SILU) {
-          if (epi.pre) epi.pre[m * epi.ldpre + n] = x;
-          x = silu_f<float>(x);
-        } else if (epi.act == ACT_MUL_DSILU) {
-          x *= dsilu_f<float>(epi.aux[m * epi.ldaux + n]);
+      for (int j = 0; j < 32; ++j) x[j] = __uint_as_float(r[j]);
+      if (epi.bias) {
+#pragma unroll
+        for (int j = 0; j < 32; j += 4) {
+          const float4 bv = __ldg(reinterpret_cast<const float4*>(epi.bias + n + j));
+          x[j] += bv.x; x[j + 1] += bv.y; x[j + 2] += bv.z; x[j + 3] += bv.w;
         }
-        if (epi.accumulate) x += epi.C[m * epi.ldc + n];
-        if (epi.C) epi.C[m * epi.ldc + n] = x;
-        if (epi.Cb) epi.Cb[m * epi.ldcb + n] = __float2bfloat16_rn(x);
       }
-      __syncwarp();
+      if (epi.act == ACT_SILU) {
+        if (epi.pre) {
+          float4* pp = reinterpret_cast<float4*>(epi.pre + m * epi.ldpre + n);
+#pragma unroll
+          for (int j = 0; j < 32; j += 4) pp[j >> 2] = make_float4(x[j], x[j + 1], x[j + 2], x[j + 3]);
+        }
+#pragma unroll
+        for (int j = 0; j < 32; ++j) x[j] = silu_f<float>(x[j]);
+      } else if (epi.act == ACT_MUL_DSILU) {
+        const float4* ap = reinterpret_cast<const float4*>(epi.aux + m * epi.ldaux + n);
+#pragma unroll
+        for (int j = 0; j < 32; j += 4) {
+          const float4 av = ap[j >> 2];
+          x[j] *= dsilu_f<float>(av.x); x[j + 1] *= dsilu_f<float>(av.y);
+          x[j + 2] *= dsilu_f<float>(av.z); x[j + 3] *= dsilu_f<float>(av.w);
+        }
+      }
+      if (epi.C) {
+        float4* cp = reinterpret_cast<float4*>(epi.C + m * epi.ldc + n);
+        if (epi.accumulate) {
+#pragma unroll
+          for (int j = 0; j < 32; j += 4) {
+            const float4 cv = cp[j >> 2];
+            x[j] += cv.x; x[j + 1] += cv.y; x[j + 2] += cv.z; x[j + 3] += cv.w;
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < 32; j += 4) cp[j >> 2] = make_float4(x[j], x[j + 1], x[j + 2], x[j + 3]);
+      }
+      if (epi.Cb) {
+        uint4* bp = reinterpret_cast<uint4*>(epi.Cb + m * epi.ldcb + n);
+#pragma unroll
+        for (int j = 0; j < 32; j += 8) {
+          __nv_bfloat162 h0 = __floats2bfloat162_rn(x[j], x[j + 1]), h1 = __floats2bfloat162_rn(x[j + 2], x[j + 3]);
+          __nv_bfloat162 h2 = __floats2bfloat162_rn(x[j + 4], x[j + 5]), h3 = __floats2bfloat162_rn(x[j + 6], x[j + 7]);
+          bp[j >> 3] = make_uint4(*reinterpret_cast<uint32_t*>(&h0), *reinterpret_cast<uint32_t*>(&h1),
+                                  *reinterpret_cast<uint32_t*>(&h2), *reinterpret_cast<uint32_t*>(&h3));
+        }
+      }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   }
@@ -297,7 +328,12 @@ int launch_cfg(int64_t M, int N, int K, const CUtensorMap& ta, const CUtensorMap
 int launch_gemm_tc(int64_t M, int N, int K, const __nv_bfloat16* A, int64_t lda, const __nv_bfloat16* Wt, int64_t ldw,
                    const TcEpi& epi, cudaStream_t st) {
   if (M <= 0) return 0;
-  const int bn = (N % 256 == 0) ? 256 : (N % 128 == 0) ? 128 : (N % 64 == 0) ? 64 : 32;
+  // Widest tile that still gives about two waves of CTAs: small problems (a few thousand rows) are bound by the
+  // serial load -> MMA -> epilogue latency of one CTA, so they are cut into more, narrower tiles.
+  const int64_t m_tiles = (M + BM - 1) / BM;
+  int bn = (N % 64 == 0) ? 64 : 32;
+  for (int cand = 256; cand > 64; cand >>= 1)
+    if (N % cand == 0 && m_tiles * (N / cand) >= 2 * 148) { bn = cand; break; }
   CUtensorMap ta, tb;
   if (!get_tensor_map(A, M, K, lda, BM, &ta) || !get_tensor_map(Wt, N, K, ldw, bn, &tb)) return -1;
   switch (bn) {

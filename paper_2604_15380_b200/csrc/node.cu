@@ -113,12 +113,15 @@ __global__ void __launch_bounds__(256) update_bwd1_k(int64_t N, int F, const T* 
 template <typename T>
 __global__ void __launch_bounds__(256) update_bwd2_k(int64_t N, int F, const T* __restrict__ zb,
                                                      const T* __restrict__ PQ, T eps, T* __restrict__ sb,
-                                                     T* __restrict__ PQb, __nv_bfloat16* __restrict__ PQb16) {
+                                                     T* __restrict__ PQb, __nv_bfloat16* __restrict__ PQb16,
+                                                     __nv_bfloat16* __restrict__ sb16) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= N * F) return;
   const int64_t i = idx / F;
   const int f = (int)(idx % F);
-  sb[idx] += zb[i * 2 * F + f];
+  const T sbn = sb[idx] + zb[i * 2 * F + f];
+  sb[idx] = sbn;
+  if (sb16) sb16[idx] = __float2bfloat16_rn((float)sbn);
   const T nb = zb[i * 2 * F + F + f];
   const T q0 = PQ[(i * 3 + 0) * 2 * F + F + f], q1 = PQ[(i * 3 + 1) * 2 * F + F + f], q2 = PQ[(i * 3 + 2) * 2 * F + F + f];
   const T r = nb / sqrt(q0 * q0 + q1 * q1 + q2 * q2 + eps);
@@ -301,9 +304,9 @@ int launch_update_bwd1(int64_t N, int F, const T* sb, const T* vb, const T* a, c
 }
 template <typename T>
 int launch_update_bwd2(int64_t N, int F, const T* zb, const T* PQ, T eps, T* sb, T* PQb, cudaStream_t st,
-                       __nv_bfloat16* PQb16) {
+                       __nv_bfloat16* PQb16, __nv_bfloat16* sb16) {
   if (N == 0) return 0;
-  update_bwd2_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, zb, PQ, eps, sb, PQb, PQb16); PNN_KCHECK("update_bwd2_k");
+  update_bwd2_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, zb, PQ, eps, sb, PQb, PQb16, sb16); PNN_KCHECK("update_bwd2_k");
   return 1;
 }
 template <typename T>
@@ -350,7 +353,8 @@ int launch_force_assemble(int64_t N, int nslab, const T* fpart, T* forces, cudaS
                                 __nv_bfloat16*, __nv_bfloat16*);                                                     \
   template int launch_update_bwd1<T>(int64_t, int, const T*, const T*, const T*, const T*, T*, T*, cudaStream_t,     \
                                      __nv_bfloat16*);                                                                \
-  template int launch_update_bwd2<T>(int64_t, int, const T*, const T*, T, T*, T*, cudaStream_t, __nv_bfloat16*);     \
+  template int launch_update_bwd2<T>(int64_t, int, const T*, const T*, T, T*, T*, cudaStream_t, __nv_bfloat16*,      \
+                                     __nv_bfloat16*);                                                                \
   template int launch_readout<T>(int64_t, int64_t, int, int, const T*, const int32_t*, const int32_t*,               \
                                  const int32_t*, const T*, const T*, const T*, const T*, T*, T*, T*, int*,           \
                                  cudaStream_t);                                                                      \

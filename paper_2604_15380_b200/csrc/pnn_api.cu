@@ -105,7 +105,7 @@ struct pnn_workspace {
   // BF16 model: BF16 copies that feed the tensor-core GEMMs and the edge gathers (reading Q19)
   struct Mirror {
     __nv_bfloat16 *s16, *h16, *sn16, *v1_16, *k16, *vping16[2];
-    __nv_bfloat16 *ab16, *kb16, *PQb16, *phib16, *hb16;
+    __nv_bfloat16 *ab16, *kb16, *PQb16, *phib16, *hb16, *sb16, *vb16;
   } mb{};
   struct Tape16 { __nv_bfloat16 *vin16, *phi16; };
   std::vector<Tape16> tape16;
@@ -341,7 +341,7 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
       ws->zb = carve(es * N * 2 * F);
       ws->phib = carve(es * N * 3 * F);
       ws->hb = carve(es * N * F);
-      ws->fpart = carve(es * N * 3 * edge_num_slabs((int)F));
+      ws->fpart = carve(es * N * 3 * 8); // one slab of partial forces per CTA column (at most F/32 = 8)
     } else {
       ws->opre = nullptr;
       pnn_workspace::Tape& tp = ws->tape[0];
@@ -367,12 +367,12 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
         }
         b.vping16[0] = b.vping16[1] = nullptr;
         b.ab16 = c16(N * 3 * F); b.kb16 = c16(N * F); b.PQb16 = c16(N * 6 * F); b.phib16 = c16(N * 3 * F);
-        b.hb16 = c16(N * F);
+        b.hb16 = c16(N * F); b.sb16 = c16(N * F); b.vb16 = c16(N * 3 * F);
       } else {
         ws->tape16[0].vin16 = nullptr;
         ws->tape16[0].phi16 = c16(N * 3 * F);
         b.vping16[0] = c16(N * 3 * F); b.vping16[1] = c16(N * 3 * F);
-        b.ab16 = b.kb16 = b.PQb16 = b.phib16 = b.hb16 = nullptr;
+        b.ab16 = b.kb16 = b.PQb16 = b.phib16 = b.hb16 = b.sb16 = b.vb16 = nullptr;
       }
     }
     ws->st_Z = (int32_t*)carve(4 * N);
@@ -718,14 +718,17 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       TcEpi g2; g2.C = zb; g2.ldc = 2 * F;
       tc("gemm_N", N, 2 * F, F, mb.kb16, F, b.A1t, g2);                            // z-bar = A1^T k-bar
       { ProfScope ps_(ws, st, "update_bwd_elementwise");
-        const int l_ = launch_update_bwd2<T>(N, F, zb, (const T*)tp.PQ, (T)c.norm_eps, sb, PQb, st, mb.PQb16);
+        const int l_ = launch_update_bwd2<T>(N, F, zb, (const T*)tp.PQ, (T)c.norm_eps, sb, PQb, st, mb.PQb16, mb.sb16);
         nl += l_; ps_.done(l_); }
-      TcEpi g3; g3.accumulate = last ? 0 : 1; g3.C = vb; g3.ldc = F;
+      TcEpi g3; g3.accumulate = last ? 0 : 1; g3.C = vb; g3.ldc = F; g3.Cb = mb.vb16; g3.ldcb = F;
       tc("gemm_3N", 3 * N, F, 2 * F, mb.PQb16, 2 * F, b.UVt, g3);                  // v-bar' += U^T P-bar + V^T Q-bar
       ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
       { ProfScope ps_(ws, st, "edge_bwd");
-        const int l_ = launch_edge_bwd<T, B>(ea, tp16.phi16, tp16.vin16, sb, vb, nullptr, vb2, fpart, last ? 1 : 0,
-                                             t > 0 ? mb.phib16 : nullptr, st);
+        em.fltP = m->d_fltP + (int64_t)t * m->fltP_stride;
+        const int l_ = simt_edges ? launch_edge_bwd<T, B>(ea, tp16.phi16, tp16.vin16, sb, vb, nullptr, vb2, fpart,
+                                                          last ? 1 : 0, t > 0 ? mb.phib16 : nullptr, st)
+                                  : launch_edge_bwd_mma(em, tp16.phi16, tp16.vin16, mb.sb16, mb.vb16, vb,
+                                                        t > 0 ? mb.phib16 : nullptr, vb2, fpart, last ? 1 : 0, st);
         nl += l_; ps_.done(l_); }
       if (t > 0) {
         TcEpi g4; g4.act = ACT_MUL_DSILU; g4.aux = (const T*)tp.hpre; g4.ldaux = F; g4.Cb = mb.hb16; g4.ldcb = F;
@@ -736,7 +739,7 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       }
     }
     { ProfScope ps_(ws, st, "force_assemble");
-      const int l_ = launch_force_assemble<T>(N, edge_num_slabs(F), fpart, forces, st);
+      const int l_ = launch_force_assemble<T>(N, simt_edges ? edge_num_slabs(F) : edge_mma_num_slabs(F), fpart, forces, st);
       nl += l_; ps_.done(l_); }
   }
   ws->launches += nl;
@@ -808,6 +811,9 @@ int pnn_gemm_bf16(int64_t M, int32_t N, int32_t K, const void* A, int64_t lda, c
   if (M < 0 || N < 32 || K < 32 || N % 32 || K % 32 || lda % 8 || ldw % 8 || lda < K || ldw < K) return PNN_ERR_INVALID_ARG;
   if (M > 0 && (!A || !Wt || (!C && !Cb))) return PNN_ERR_INVALID_ARG;
   if (act != ACT_NONE && act != ACT_SILU) return PNN_ERR_INVALID_ARG;
+  if ((C && (ldc % 4 || ldc < N || ((uintptr_t)C & 15))) || (Cb && (ldcb % 8 || ldcb < N || ((uintptr_t)Cb & 15))) ||
+      ((uintptr_t)A & 15) || ((uintptr_t)Wt & 15) || (bias && ((uintptr_t)bias & 15)))
+    return PNN_ERR_INVALID_ARG;
   TcEpi e;
   e.bias = bias; e.act = act; e.C = C; e.ldc = ldc; e.Cb = (__nv_bfloat16*)Cb; e.ldcb = ldcb;
   const int nl = launch_gemm_tc(M, N, K, (const __nv_bfloat16*)A, lda, (const __nv_bfloat16*)Wt, ldw, e,
