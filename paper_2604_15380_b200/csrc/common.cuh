@@ -133,22 +133,25 @@ int edge_num_slabs(int F);
 template <typename T>
 int launch_embed(int64_t N, int F, int Zmax, const int32_t* Z, const T* emb, T* s, int* d_err, cudaStream_t st,
                  __nv_bfloat16* s16 = nullptr);
-template <typename T>
-int launch_norm(int64_t N, int F, const T* PQ, T* sn, T eps, cudaStream_t st, __nv_bfloat16* sn16 = nullptr);
-template <typename T>
-int launch_update(int64_t N, int F, const T* sn, const T* v1, const T* PQ, const T* a, T* s_out, T* v_out,
+// IT: storage type of P | Q and of the gate values a (= T, or BF16 in the BF16 model)
+template <typename T, typename IT>
+int launch_norm(int64_t N, int F, const IT* PQ, T* sn, T eps, cudaStream_t st, __nv_bfloat16* sn16 = nullptr);
+template <typename T, typename IT>
+int launch_update(int64_t N, int F, const T* sn, const T* v1, const IT* PQ, const IT* a, T* s_out, T* v_out,
                   cudaStream_t st, __nv_bfloat16* s16 = nullptr, __nv_bfloat16* v16 = nullptr);
-template <typename T>
-int launch_update_bwd1(int64_t N, int F, const T* sb, const T* vb, const T* a, const T* PQ, T* ab, T* PQb,
+template <typename T, typename IT>
+int launch_update_bwd1(int64_t N, int F, const T* sb, const T* vb, const IT* a, const IT* PQ, T* ab, T* PQb,
                        cudaStream_t st, __nv_bfloat16* ab16 = nullptr);
-template <typename T>
-int launch_update_bwd2(int64_t N, int F, const T* zb, const T* PQ, T eps, T* sb, T* PQb, cudaStream_t st,
+template <typename T, typename IT>
+int launch_update_bwd2(int64_t N, int F, const T* zb, const IT* PQ, T eps, T* sb, T* PQb, cudaStream_t st,
                        __nv_bfloat16* PQb16 = nullptr, __nv_bfloat16* sb16 = nullptr);
 // readout (B5 / R1).  W1t: [H][F][F/2] (transposed), W1: [H][F/2][F], b1 [H][F/2], w2 [H][F/2], b2 [H].
 template <typename T>
 int launch_readout(int64_t N, int64_t S, int F, int H, const T* s, const int32_t* a2s, const int32_t* head,
                    const int32_t* struct_ptr, const T* W1t, const T* b1, const T* w2, const T* b2, T* opre, T* eatom,
                    T* energy, int* d_err, cudaStream_t st);
+template <typename T>
+int launch_struct_sum(int64_t S, const int32_t* struct_ptr, const T* eatom, T* energy, cudaStream_t st);
 template <typename T>
 int launch_readout_bwd(int64_t N, int F, int H, const T* opre, const int32_t* a2s, const int32_t* head, const T* W1,
                        const T* w2, T* sb, cudaStream_t st);

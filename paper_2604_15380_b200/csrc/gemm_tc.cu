@@ -123,6 +123,15 @@ tc_gemm_k(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   const int64_t m0 = m_tile * BM;
   const int n0 = n_tile * BN;
   const int nkb = (K + BK - 1) / BK;
+  if (epi.readout) { // column tile n_tile = head n_tile: leave if none of this tile's rows belongs to it
+    int match = 0;
+    if (threadIdx.x < BM && m0 + threadIdx.x < M) {
+      int h = epi.head[epi.a2s[m0 + threadIdx.x]];
+      if (h < 0 || h >= epi.H) { if (n_tile == 0) atomicOr(epi.d_err, ERRF_BAD_HEAD); h = 0; }
+      match = (h == n_tile);
+    }
+    if (!__syncthreads_or(match)) return;
+  }
 
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
@@ -176,12 +185,34 @@ tc_gemm_k(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     mbar_wait(acc_bar, 0);
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const int64_t m = m0 + q * 32 + lane;
-    const bool row_ok = m < M;
+    bool row_ok = m < M;
+    int hrow = 0;
+    float esum = 0.0f;
+    if (epi.readout && row_ok) {
+      hrow = epi.head[epi.a2s[m]];
+      if (hrow < 0 || hrow >= epi.H) hrow = 0;
+      row_ok = (hrow == n_tile);
+    }
 #pragma unroll 1
     for (int c0 = 0; c0 < BN; c0 += 32) {
       uint32_t r[32];
       tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)c0, r);
       if (!row_ok) continue;
+      if (epi.readout) {
+        const int n = n0 + c0;
+#pragma unroll
+        for (int j = 0; j < 32; j += 4) {
+          const float4 bv = __ldg(reinterpret_cast<const float4*>(epi.bias + n + j));
+          const float4 wv = __ldg(reinterpret_cast<const float4*>(epi.w2 + n + j));
+          const float p0 = __uint_as_float(r[j]) + bv.x, p1 = __uint_as_float(r[j + 1]) + bv.y,
+                      p2 = __uint_as_float(r[j + 2]) + bv.z, p3 = __uint_as_float(r[j + 3]) + bv.w;
+          if (epi.opre) *reinterpret_cast<float4*>(epi.opre + m * BN + c0 + j) = make_float4(p0, p1, p2, p3);
+          esum = fmaf(wv.x, silu_f<float>(p0), esum); esum = fmaf(wv.y, silu_f<float>(p1), esum);
+          esum = fmaf(wv.z, silu_f<float>(p2), esum); esum = fmaf(wv.w, silu_f<float>(p3), esum);
+        }
+        if (c0 + 32 >= BN) epi.eatom[m] = esum + epi.b2[hrow];
+        continue;
+      }
       const int n = n0 + c0;
       float x[32];
 #pragma unroll
@@ -341,6 +372,24 @@ int launch_gemm_tc(int64_t M, int N, int K, const __nv_bfloat16* A, int64_t lda,
     case 128: return launch_cfg<128, 3>(M, N, K, ta, tb, epi, st);
     case 64: return launch_cfg<64, 4>(M, N, K, ta, tb, epi, st);
     default: return launch_cfg<32, 4>(M, N, K, ta, tb, epi, st);
+  }
+}
+
+int launch_readout_tc(int64_t N, int F, int H, const __nv_bfloat16* s16, const __nv_bfloat16* W1all, const float* b1,
+                      const float* w2, const float* b2, const int32_t* a2s, const int32_t* head, float* opre,
+                      float* eatom, int* d_err, cudaStream_t st) {
+  if (N <= 0) return 0;
+  const int Fh = F / 2;
+  if (Fh != 32 && Fh != 64 && Fh != 128) return -1;
+  CUtensorMap ta, tb;
+  if (!get_tensor_map(s16, N, F, F, BM, &ta) || !get_tensor_map(W1all, (int64_t)H * Fh, F, F, Fh, &tb)) return -1;
+  TcEpi e;
+  e.bias = b1; e.readout = 1; e.a2s = a2s; e.head = head; e.w2 = w2; e.b2 = b2; e.eatom = eatom; e.opre = opre;
+  e.H = H; e.d_err = d_err;
+  switch (Fh) {
+    case 128: return launch_cfg<128, 3>(N, H * Fh, F, ta, tb, e, st);
+    case 64: return launch_cfg<64, 4>(N, H * Fh, F, ta, tb, e, st);
+    default: return launch_cfg<32, 4>(N, H * Fh, F, ta, tb, e, st);
   }
 }
 

@@ -22,11 +22,31 @@ struct TcEpi {
   int64_t ldc = 0;
   __nv_bfloat16* Cb = nullptr;
   int64_t ldcb = 0;
+  // Multi-head readout mode (launch_readout_tc): column tile = one head.  Rows whose structure has another head are
+  // skipped; for the others eatom[m] = sum_n w2[n] silu(x[m][n] + bias[n]) + b2[head], opre[m][n - n0] = x + bias.
+  int readout = 0;
+  const int32_t* a2s = nullptr;
+  const int32_t* head = nullptr;
+  const float* w2 = nullptr;
+  const float* b2 = nullptr;
+  float* eatom = nullptr;
+  float* opre = nullptr;
+  int H = 0;
+  int* d_err = nullptr;
 };
 
 // Returns the number of kernels launched (0 or 1); < 0 when the TMA descriptor could not be encoded.
 int launch_gemm_tc(int64_t M, int N, int K, const __nv_bfloat16* A, int64_t lda, const __nv_bfloat16* Wt, int64_t ldw,
                    const TcEpi& epi, cudaStream_t st);
+
+// a6 on the tensor cores: eatom[i] = w2^h . silu(W1^h s_i + b1^h) + b2^h with h = head[a2s[i]] as ONE GEMM against the
+// stacked first layers of all heads, W1all [H*Fh][F] (BF16): a column tile is exactly one head (Fh in {32, 64, 128}),
+// tiles none of whose 128 rows use that head exit before loading anything, and the epilogue keeps only the rows of
+// its head.  bias = b1 of all heads [H*Fh], w2 [H*Fh], b2 [H].  opre (FP32 [N][Fh], pre-activation for R1) may be NULL.
+// Returns kernels launched, or -1 if this shape is not supported (the caller then uses the SIMT readout).
+int launch_readout_tc(int64_t N, int F, int H, const __nv_bfloat16* s16, const __nv_bfloat16* W1all, const float* b1,
+                      const float* w2, const float* b2, const int32_t* a2s, const int32_t* head, float* opre,
+                      float* eatom, int* d_err, cudaStream_t st);
 
 // dst[i] = bf16(src[i])
 int launch_f32_to_bf16(int64_t n, const float* src, __nv_bfloat16* dst, cudaStream_t st);

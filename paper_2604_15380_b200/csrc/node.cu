@@ -11,6 +11,10 @@ namespace {
 
 constexpr int RT = 16; // atoms per readout tile
 
+// P | Q and the gate values a may be stored narrower than the arithmetic type (BF16 model: tensor-core GEMM outputs)
+template <typename T, typename IT> __device__ __forceinline__ T ldi(const IT* p) { return (T)(*p); }
+template <> __device__ __forceinline__ float ldi<float, __nv_bfloat16>(const __nv_bfloat16* p) { return __bfloat162float(*p); }
+
 template <typename T>
 __global__ void __launch_bounds__(256) embed_k(int64_t N, int F, int Zmax, const int32_t* __restrict__ Z,
                                                const T* __restrict__ emb, T* __restrict__ s, int* d_err,
@@ -30,34 +34,36 @@ __global__ void __launch_bounds__(256) embed_k(int64_t N, int F, int Zmax, const
 }
 
 // PQ [N][3][2F] (P | Q)  ->  sn[:, F:2F] = sqrt(sum_a Q_a^2 + eps)          (B4)
-template <typename T>
-__global__ void __launch_bounds__(256) norm_k(int64_t N, int F, const T* __restrict__ PQ, T* __restrict__ sn, T eps,
+template <typename T, typename IT>
+__global__ void __launch_bounds__(256) norm_k(int64_t N, int F, const IT* __restrict__ PQ, T* __restrict__ sn, T eps,
                                               __nv_bfloat16* __restrict__ sn16) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= N * F) return;
   const int64_t i = idx / F;
   const int f = (int)(idx % F);
-  const T q0 = PQ[(i * 3 + 0) * 2 * F + F + f], q1 = PQ[(i * 3 + 1) * 2 * F + F + f], q2 = PQ[(i * 3 + 2) * 2 * F + F + f];
+  const T q0 = ldi<T, IT>(PQ + (i * 3 + 0) * 2 * F + F + f), q1 = ldi<T, IT>(PQ + (i * 3 + 1) * 2 * F + F + f),
+          q2 = ldi<T, IT>(PQ + (i * 3 + 2) * 2 * F + F + f);
   const T n = sqrt(q0 * q0 + q1 * q1 + q2 * q2 + eps);
   if (sn16) sn16[i * 2 * F + F + f] = __float2bfloat16_rn((float)n);
   else sn[i * 2 * F + F + f] = n;
 }
 
 // s'' = s' + a_sv <P,Q> + a_ss ;  v'' = v' + a_vv P                          (B4)
-template <typename T>
+template <typename T, typename IT>
 __global__ void __launch_bounds__(256) update_k(int64_t N, int F, const T* __restrict__ sn, const T* __restrict__ v1,
-                                                const T* __restrict__ PQ, const T* __restrict__ a,
+                                                const IT* __restrict__ PQ, const IT* __restrict__ a,
                                                 T* __restrict__ s_out, T* __restrict__ v_out,
                                                 __nv_bfloat16* __restrict__ s16, __nv_bfloat16* __restrict__ v16) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= N * F) return;
   const int64_t i = idx / F;
   const int f = (int)(idx % F);
-  const T avv = a[i * 3 * F + f], asv = a[i * 3 * F + F + f], ass = a[i * 3 * F + 2 * F + f];
+  const T avv = ldi<T, IT>(a + i * 3 * F + f), asv = ldi<T, IT>(a + i * 3 * F + F + f),
+          ass = ldi<T, IT>(a + i * 3 * F + 2 * F + f);
   T dot = T(0);
 #pragma unroll
   for (int ax = 0; ax < 3; ++ax) {
-    const T p = PQ[(i * 3 + ax) * 2 * F + f], q = PQ[(i * 3 + ax) * 2 * F + F + f];
+    const T p = ldi<T, IT>(PQ + (i * 3 + ax) * 2 * F + f), q = ldi<T, IT>(PQ + (i * 3 + ax) * 2 * F + F + f);
     dot = fma(p, q, dot);
     if (v_out) {
       const T r = fma(avv, p, v1[(i * 3 + ax) * F + f]);
@@ -71,23 +77,23 @@ __global__ void __launch_bounds__(256) update_k(int64_t N, int F, const T* __res
 }
 
 // R2, first half: a-bar [N,3F] and the direct parts of P-bar, Q-bar [N][3][2F]
-template <typename T>
+template <typename T, typename IT>
 __global__ void __launch_bounds__(256) update_bwd1_k(int64_t N, int F, const T* __restrict__ sb,
-                                                     const T* __restrict__ vb, const T* __restrict__ a,
-                                                     const T* __restrict__ PQ, T* __restrict__ ab,
+                                                     const T* __restrict__ vb, const IT* __restrict__ a,
+                                                     const IT* __restrict__ PQ, T* __restrict__ ab,
                                                      T* __restrict__ PQb, __nv_bfloat16* __restrict__ ab16) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= N * F) return;
   const int64_t i = idx / F;
   const int f = (int)(idx % F);
   const T sbf = sb[idx];
-  const T avv = a[i * 3 * F + f], asv = a[i * 3 * F + F + f];
+  const T avv = ldi<T, IT>(a + i * 3 * F + f), asv = ldi<T, IT>(a + i * 3 * F + F + f);
   T p[3], q[3], vbf[3];
   T dot = T(0), avvb = T(0);
 #pragma unroll
   for (int ax = 0; ax < 3; ++ax) {
-    p[ax] = PQ[(i * 3 + ax) * 2 * F + f];
-    q[ax] = PQ[(i * 3 + ax) * 2 * F + F + f];
+    p[ax] = ldi<T, IT>(PQ + (i * 3 + ax) * 2 * F + f);
+    q[ax] = ldi<T, IT>(PQ + (i * 3 + ax) * 2 * F + F + f);
     vbf[ax] = vb ? vb[(i * 3 + ax) * F + f] : T(0);
     dot = fma(p[ax], q[ax], dot);
     avvb = fma(vbf[ax], p[ax], avvb);
@@ -110,9 +116,9 @@ __global__ void __launch_bounds__(256) update_bwd1_k(int64_t N, int F, const T* 
 }
 
 // R2, second half: s-bar' = s-bar'' + z-bar[0:F];  Q-bar += n-bar Q / n
-template <typename T>
+template <typename T, typename IT>
 __global__ void __launch_bounds__(256) update_bwd2_k(int64_t N, int F, const T* __restrict__ zb,
-                                                     const T* __restrict__ PQ, T eps, T* __restrict__ sb,
+                                                     const IT* __restrict__ PQ, T eps, T* __restrict__ sb,
                                                      T* __restrict__ PQb, __nv_bfloat16* __restrict__ PQb16,
                                                      __nv_bfloat16* __restrict__ sb16) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -123,7 +129,8 @@ __global__ void __launch_bounds__(256) update_bwd2_k(int64_t N, int F, const T* 
   sb[idx] = sbn;
   if (sb16) sb16[idx] = __float2bfloat16_rn((float)sbn);
   const T nb = zb[i * 2 * F + F + f];
-  const T q0 = PQ[(i * 3 + 0) * 2 * F + F + f], q1 = PQ[(i * 3 + 1) * 2 * F + F + f], q2 = PQ[(i * 3 + 2) * 2 * F + F + f];
+  const T q0 = ldi<T, IT>(PQ + (i * 3 + 0) * 2 * F + F + f), q1 = ldi<T, IT>(PQ + (i * 3 + 1) * 2 * F + F + f),
+          q2 = ldi<T, IT>(PQ + (i * 3 + 2) * 2 * F + F + f);
   const T r = nb / sqrt(q0 * q0 + q1 * q1 + q2 * q2 + eps);
   const T qq[3] = {q0, q1, q2};
 #pragma unroll
@@ -282,31 +289,31 @@ int launch_embed(int64_t N, int F, int Zmax, const int32_t* Z, const T* emb, T* 
   embed_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, Zmax, Z, emb, s, d_err, s16); PNN_KCHECK("embed_k");
   return 1;
 }
-template <typename T>
-int launch_norm(int64_t N, int F, const T* PQ, T* sn, T eps, cudaStream_t st, __nv_bfloat16* sn16) {
+template <typename T, typename IT>
+int launch_norm(int64_t N, int F, const IT* PQ, T* sn, T eps, cudaStream_t st, __nv_bfloat16* sn16) {
   if (N == 0) return 0;
-  norm_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, PQ, sn, eps, sn16); PNN_KCHECK("norm_k");
+  norm_k<T, IT><<<nblk(N * F, 256), 256, 0, st>>>(N, F, PQ, sn, eps, sn16); PNN_KCHECK("norm_k");
   return 1;
 }
-template <typename T>
-int launch_update(int64_t N, int F, const T* sn, const T* v1, const T* PQ, const T* a, T* s_out, T* v_out,
+template <typename T, typename IT>
+int launch_update(int64_t N, int F, const T* sn, const T* v1, const IT* PQ, const IT* a, T* s_out, T* v_out,
                   cudaStream_t st, __nv_bfloat16* s16, __nv_bfloat16* v16) {
   if (N == 0) return 0;
-  update_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, sn, v1, PQ, a, s_out, v_out, s16, v16); PNN_KCHECK("update_k");
+  update_k<T, IT><<<nblk(N * F, 256), 256, 0, st>>>(N, F, sn, v1, PQ, a, s_out, v_out, s16, v16); PNN_KCHECK("update_k");
   return 1;
 }
-template <typename T>
-int launch_update_bwd1(int64_t N, int F, const T* sb, const T* vb, const T* a, const T* PQ, T* ab, T* PQb,
+template <typename T, typename IT>
+int launch_update_bwd1(int64_t N, int F, const T* sb, const T* vb, const IT* a, const IT* PQ, T* ab, T* PQb,
                        cudaStream_t st, __nv_bfloat16* ab16) {
   if (N == 0) return 0;
-  update_bwd1_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, sb, vb, a, PQ, ab, PQb, ab16); PNN_KCHECK("update_bwd1_k");
+  update_bwd1_k<T, IT><<<nblk(N * F, 256), 256, 0, st>>>(N, F, sb, vb, a, PQ, ab, PQb, ab16); PNN_KCHECK("update_bwd1_k");
   return 1;
 }
-template <typename T>
-int launch_update_bwd2(int64_t N, int F, const T* zb, const T* PQ, T eps, T* sb, T* PQb, cudaStream_t st,
+template <typename T, typename IT>
+int launch_update_bwd2(int64_t N, int F, const T* zb, const IT* PQ, T eps, T* sb, T* PQb, cudaStream_t st,
                        __nv_bfloat16* PQb16, __nv_bfloat16* sb16) {
   if (N == 0) return 0;
-  update_bwd2_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, zb, PQ, eps, sb, PQb, PQb16, sb16); PNN_KCHECK("update_bwd2_k");
+  update_bwd2_k<T, IT><<<nblk(N * F, 256), 256, 0, st>>>(N, F, zb, PQ, eps, sb, PQb, PQb16, sb16); PNN_KCHECK("update_bwd2_k");
   return 1;
 }
 template <typename T>
@@ -331,6 +338,12 @@ int launch_readout(int64_t N, int64_t S, int F, int H, const T* s, const int32_t
   return nl;
 }
 template <typename T>
+int launch_struct_sum(int64_t S, const int32_t* struct_ptr, const T* eatom, T* energy, cudaStream_t st) {
+  if (S <= 0) return 0;
+  struct_sum_k<T><<<(unsigned)S, 128, 0, st>>>(struct_ptr, eatom, energy); PNN_KCHECK("struct_sum_k");
+  return 1;
+}
+template <typename T>
 int launch_readout_bwd(int64_t N, int F, int H, const T* opre, const int32_t* a2s, const int32_t* head, const T* W1,
                        const T* w2, T* sb, cudaStream_t st) {
   if (N == 0) return 0;
@@ -348,21 +361,27 @@ int launch_force_assemble(int64_t N, int nslab, const T* fpart, T* forces, cudaS
 #define PNN_INST(T)                                                                                                  \
   template int launch_embed<T>(int64_t, int, int, const int32_t*, const T*, T*, int*, cudaStream_t,                  \
                                __nv_bfloat16*);                                                                      \
-  template int launch_norm<T>(int64_t, int, const T*, T*, T, cudaStream_t, __nv_bfloat16*);                          \
-  template int launch_update<T>(int64_t, int, const T*, const T*, const T*, const T*, T*, T*, cudaStream_t,          \
-                                __nv_bfloat16*, __nv_bfloat16*);                                                     \
-  template int launch_update_bwd1<T>(int64_t, int, const T*, const T*, const T*, const T*, T*, T*, cudaStream_t,     \
-                                     __nv_bfloat16*);                                                                \
-  template int launch_update_bwd2<T>(int64_t, int, const T*, const T*, T, T*, T*, cudaStream_t, __nv_bfloat16*,      \
-                                     __nv_bfloat16*);                                                                \
   template int launch_readout<T>(int64_t, int64_t, int, int, const T*, const int32_t*, const int32_t*,               \
                                  const int32_t*, const T*, const T*, const T*, const T*, T*, T*, T*, int*,           \
                                  cudaStream_t);                                                                      \
+  template int launch_struct_sum<T>(int64_t, const int32_t*, const T*, T*, cudaStream_t);                            \
   template int launch_readout_bwd<T>(int64_t, int, int, const T*, const int32_t*, const int32_t*, const T*,          \
                                      const T*, T*, cudaStream_t);                                                    \
   template int launch_force_assemble<T>(int64_t, int, const T*, T*, cudaStream_t);
+#define PNN_INST2(T, IT)                                                                                             \
+  template int launch_norm<T, IT>(int64_t, int, const IT*, T*, T, cudaStream_t, __nv_bfloat16*);                     \
+  template int launch_update<T, IT>(int64_t, int, const T*, const T*, const IT*, const IT*, T*, T*, cudaStream_t,    \
+                                    __nv_bfloat16*, __nv_bfloat16*);                                                 \
+  template int launch_update_bwd1<T, IT>(int64_t, int, const T*, const T*, const IT*, const IT*, T*, T*,             \
+                                         cudaStream_t, __nv_bfloat16*);                                              \
+  template int launch_update_bwd2<T, IT>(int64_t, int, const T*, const IT*, T, T*, T*, cudaStream_t, __nv_bfloat16*, \
+                                         __nv_bfloat16*);
 PNN_INST(float)
 PNN_INST(double)
+PNN_INST2(float, float)
+PNN_INST2(double, double)
+PNN_INST2(float, __nv_bfloat16)
 #undef PNN_INST
+#undef PNN_INST2
 
 } // namespace pnn

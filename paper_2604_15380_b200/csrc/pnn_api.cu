@@ -546,7 +546,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     const int l_ = launch_gemm<T>(3 * N, 2 * F, F, v1, F, W + b.UVt, 2 * F, PQ, 2 * F, e3, st);   // B4: P | Q
       nl += l_; ps_.done(l_); }
     { ProfScope ps_(ws, st, "update_elementwise");
-    const int l_ = launch_norm<T>(N, F, PQ, sn, (T)c.norm_eps, st);                               // n -> sn[:, F:]
+    const int l_ = launch_norm<T, T>(N, F, PQ, sn, (T)c.norm_eps, st);                               // n -> sn[:, F:]
       nl += l_; ps_.done(l_); }
     GemmEpi<T> e4; e4.bias = W + b.c1; e4.act = ACT_SILU; e4.pre = (T*)tp.kpre; e4.ldpre = F;
     { ProfScope ps_(ws, st, "gemm_N");
@@ -557,7 +557,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     const int l_ = launch_gemm<T>(N, 3 * F, F, k, F, W + b.A2t, 3 * F, a, 3 * F, e5, st);
       nl += l_; ps_.done(l_); }
     { ProfScope ps_(ws, st, "update_elementwise");
-    const int l_ = launch_update<T>(N, F, sn, v1, PQ, a, s_cur, v_out, st);
+    const int l_ = launch_update<T, T>(N, F, sn, v1, PQ, a, s_cur, v_out, st);
       nl += l_; ps_.done(l_); }
   }
   { ProfScope ps_(ws, st, "readout");
@@ -576,7 +576,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       const bool last = (t == T_ - 1);
       // R2
       { ProfScope ps_(ws, st, "update_bwd_elementwise");
-      const int l_ = launch_update_bwd1<T>(N, F, sb, last ? nullptr : vb, (const T*)tp.a, (const T*)tp.PQ, ab, PQb, st);
+      const int l_ = launch_update_bwd1<T, T>(N, F, sb, last ? nullptr : vb, (const T*)tp.a, (const T*)tp.PQ, ab, PQb, st);
         nl += l_; ps_.done(l_); }
       GemmEpi<T> g1; g1.act = ACT_MUL_DSILU; g1.aux = (const T*)tp.kpre; g1.ldaux = F;
       { ProfScope ps_(ws, st, "gemm_N");
@@ -587,7 +587,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       const int l_ = launch_gemm<T>(N, 2 * F, F, kb, F, W + b.A1, 2 * F, zb, 2 * F, g2, st);
         nl += l_; ps_.done(l_); }
       { ProfScope ps_(ws, st, "update_bwd_elementwise");
-      const int l_ = launch_update_bwd2<T>(N, F, zb, (const T*)tp.PQ, (T)c.norm_eps, sb, PQb, st);
+      const int l_ = launch_update_bwd2<T, T>(N, F, zb, (const T*)tp.PQ, (T)c.norm_eps, sb, PQb, st);
         nl += l_; ps_.done(l_); }
       GemmEpi<T> g3; g3.accumulate = last ? 0 : 1;
       { ProfScope ps_(ws, st, "gemm_3N");
@@ -669,7 +669,7 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       v_out = (t + 1 < T_) ? (T*)ws->vping[t & 1] : nullptr;
       v_out16 = (t + 1 < T_) ? mb.vping16[t & 1] : nullptr;
     }
-    T* PQ = (T*)tp.PQ; T* a = (T*)tp.a;
+    B* PQ = (B*)tp.PQ; B* a = (B*)tp.a;   // P | Q and the gate values are kept in BF16 (tape included)
     TcEpi e1; e1.bias = W + b.b1; e1.act = ACT_SILU; e1.pre = (T*)tp.hpre; e1.ldpre = F; e1.Cb = mb.h16; e1.ldcb = F;
     tc("gemm_N", N, F, F, mb.s16, F, b.W1, e1);                                   // B3a: h = silu(W1 s + b1)
     TcEpi e2; e2.bias = W + b.b2; e2.Cb = tp16.phi16; e2.ldcb = 3 * F;
@@ -681,22 +681,25 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       const int l_ = simt_edges ? launch_edge_fwd<T, B>(ea, tp16.phi16, s_cur, F, v_in16, v_in, sn, 2 * F, v1, mir, st)
                                 : launch_edge_fwd_mma(em, tp16.phi16, s_cur, F, v_in16, v_in, sn, 2 * F, v1, mir, st); // B3b
       nl += l_; ps_.done(l_); }
-    TcEpi e3; e3.C = PQ; e3.ldc = 2 * F;
+    TcEpi e3; e3.Cb = PQ; e3.ldcb = 2 * F;
     tc("gemm_3N", 3 * N, 2 * F, F, mb.v1_16, F, b.UV, e3);                         // B4: P | Q
     { ProfScope ps_(ws, st, "update_elementwise");
-      const int l_ = launch_norm<T>(N, F, PQ, sn, (T)c.norm_eps, st, mb.sn16);
+      const int l_ = launch_norm<T, B>(N, F, PQ, sn, (T)c.norm_eps, st, mb.sn16);
       nl += l_; ps_.done(l_); }
     TcEpi e4; e4.bias = W + b.c1; e4.act = ACT_SILU; e4.pre = (T*)tp.kpre; e4.ldpre = F; e4.Cb = mb.k16; e4.ldcb = F;
     tc("gemm_N", N, F, 2 * F, mb.sn16, 2 * F, b.A1, e4);
-    TcEpi e5; e5.bias = W + b.c2; e5.C = a; e5.ldc = 3 * F;
+    TcEpi e5; e5.bias = W + b.c2; e5.Cb = a; e5.ldcb = 3 * F;
     tc("gemm_N", N, 3 * F, F, mb.k16, F, b.A2, e5);
     { ProfScope ps_(ws, st, "update_elementwise");
-      const int l_ = launch_update<T>(N, F, sn, v1, PQ, a, s_cur, v_out, st, mb.s16, v_out16);
+      const int l_ = launch_update<T, B>(N, F, sn, v1, PQ, a, s_cur, v_out, st, mb.s16, v_out16);
       nl += l_; ps_.done(l_); }
   }
-  { ProfScope ps_(ws, st, "readout");
-    const int l_ = launch_readout<T>(N, S, F, c.H, s_cur, ws->g.a2s, head, sptr, W + m->oW1t, W + m->ob1, W + m->ow2,
-                                     W + m->ob2, (T*)ws->opre, (T*)ws->eatom, energy, ws->g.d_err, st);
+  { ProfScope ps_(ws, st, "readout");   // B5: all heads as one tensor-core GEMM, rows filtered by head in the epilogue
+    int l_ = launch_readout_tc(N, F, c.H, mb.s16, Wb + m->oW1, W + m->ob1, W + m->ow2, W + m->ob2, ws->g.a2s, head,
+                               (T*)ws->opre, (T*)ws->eatom, ws->g.d_err, st);
+    if (l_ >= 0) l_ += launch_struct_sum<T>(S, sptr, (const T*)ws->eatom, energy, st);
+    else l_ = launch_readout<T>(N, S, F, c.H, s_cur, ws->g.a2s, head, sptr, W + m->oW1t, W + m->ob1, W + m->ow2,
+                                W + m->ob2, (T*)ws->opre, (T*)ws->eatom, energy, ws->g.d_err, st);
     nl += l_; ps_.done(l_); }
   if (want_f) {
     T* sb = (T*)ws->sb; T* vb = (T*)ws->vb; T* vb2 = (T*)ws->vb2; T* PQb = (T*)ws->PQb; T* zb = (T*)ws->zb;
@@ -710,15 +713,15 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       const pnn_workspace::Tape16& tp16 = ws->tape16[t];
       const bool last = (t == T_ - 1);
       { ProfScope ps_(ws, st, "update_bwd_elementwise");
-        const int l_ = launch_update_bwd1<T>(N, F, sb, last ? nullptr : vb, (const T*)tp.a, (const T*)tp.PQ, nullptr, PQb,
-                                             st, mb.ab16);
+        const int l_ = launch_update_bwd1<T, B>(N, F, sb, last ? nullptr : vb, (const B*)tp.a, (const B*)tp.PQ, nullptr,
+                                                PQb, st, mb.ab16);
         nl += l_; ps_.done(l_); }
       TcEpi g1; g1.act = ACT_MUL_DSILU; g1.aux = (const T*)tp.kpre; g1.ldaux = F; g1.Cb = mb.kb16; g1.ldcb = F;
       tc("gemm_N", N, F, 3 * F, mb.ab16, 3 * F, b.A2t, g1);                        // k-bar = A2^T a-bar . silu'
       TcEpi g2; g2.C = zb; g2.ldc = 2 * F;
       tc("gemm_N", N, 2 * F, F, mb.kb16, F, b.A1t, g2);                            // z-bar = A1^T k-bar
       { ProfScope ps_(ws, st, "update_bwd_elementwise");
-        const int l_ = launch_update_bwd2<T>(N, F, zb, (const T*)tp.PQ, (T)c.norm_eps, sb, PQb, st, mb.PQb16, mb.sb16);
+        const int l_ = launch_update_bwd2<T, B>(N, F, zb, (const B*)tp.PQ, (T)c.norm_eps, sb, PQb, st, mb.PQb16, mb.sb16);
         nl += l_; ps_.done(l_); }
       TcEpi g3; g3.accumulate = last ? 0 : 1; g3.C = vb; g3.ldc = F; g3.Cb = mb.vb16; g3.ldcb = F;
       tc("gemm_3N", 3 * N, F, 2 * F, mb.PQb16, 2 * F, b.UVt, g3);                  // v-bar' += U^T P-bar + V^T Q-bar
