@@ -99,15 +99,36 @@ class ClockSampler:
 
 
 def algorithmic_work(family: str, N: int, E: int, mc: gen.ModelCfg, prec: str, forces: bool):
-    """(flops, bytes) per LAUNCH of one kernel family."""
+    """(flops, bytes) per LAUNCH of one kernel family (per-atom and per-edge figures)."""
     F, K = mc.F, mc.K
     b = 8 if prec == "fp64" else 4
     eb = 4 + 4 * b                                    # col + (ux,uy,uz,d)
+    if prec == "bf16":
+        # BF16 model: phi, v gathered as BF16 copies (read once from HBM), FP32 residual rows read and written,
+        # BF16 copies of the outputs written for the following GEMMs; 20 B per edge (sender index + geometry)
+        if family == "edge_fwd":   # read phi16 6F, v16 6F, s 4F, v 12F; write s' 4F, v' 12F, s'16 2F, v'16 6F
+            return E * (6 * K * F + 16 * F), N * 52 * F + E * 20
+        if family == "edge_bwd":   # read phi16 6F, v16 6F, sb16 2F, vb16 6F, vb 12F; write phib16 6F, vb_in 12F
+            return E * (12 * K * F + 60 * F), N * 50 * F + E * 20
+        return None, None
     if family == "edge_fwd":
         return E * (6 * K * F + 16 * F), N * 11 * F * b + E * eb
     if family == "edge_bwd":
         return E * (12 * K * F + 60 * F), N * 16 * F * b + E * eb
     return None, None
+
+
+def measured_traffic(workload: str, family: str):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/r01_traffic.csv), or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r01_traffic.csv")) as fh:
+            for line in fh:
+                q = line.strip().split(",")
+                if len(q) >= 3 and q[0] == workload and q[1] == family:
+                    return int(q[2])
+    except Exception:
+        pass
+    return None
 
 
 def run_reference(args, rank):
@@ -290,13 +311,15 @@ def main():
         per_s = kernels[fam]["ms_per_launch"] * 1e-3
         if prec in ("fp32", "fp64"):
             ach, peak = flops / per_s / 1e12, ALU_PEAK_TFLOPS[prec]
-            roof = dict(kernel=fam, bound="alu", achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak, traffic=None,
+            roof = dict(kernel=fam, bound="alu", achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak,
+                        traffic=measured_traffic(WORKLOAD_NAMES[args.workload], fam),
                         peak_source="derived: 148 SMs x lanes x 2 x 1.965 GHz (DESIGN.md)",
                         hbm_achieved_gbs=byts / per_s / 1e9, hbm_peak_gbs=peaks["hbm"], hbm_peak_source=peaks["source"])
         else:
             ach = byts / per_s / 1e9
             roof = dict(kernel=fam, bound="hbm", achieved=ach, peak=peaks["hbm"], unit="GB/s", frac=ach / peaks["hbm"],
-                        traffic=None, peak_source=peaks["source"])
+                        traffic=measured_traffic(WORKLOAD_NAMES[args.workload], fam), peak_source=peaks["source"],
+                        algorithmic_bytes=byts, tensor_flops=flops)
         roof["share_of_step"] = kernels[fam]["share"]
 
     line = dict(metric="painn_energy_force_structures_per_s", value=main_res["structures_per_s"], unit="structures/s",

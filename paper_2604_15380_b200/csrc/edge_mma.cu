@@ -25,7 +25,7 @@ namespace {
 
 constexpr int TE = 16; // edges (rows) per MMA tile
 constexpr int NTC = 2;  // tiles of one receiver staged per round (forward)
-constexpr int NTCB = 4; // ... (reverse)
+constexpr int NTCB = 3; // ... (reverse)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
