@@ -352,7 +352,7 @@ def main():
 
     if not args.no_extra and world == 1:
         extra = {}
-        for name in ("cfg1", "cfg3_fp32", "cfg5"):
+        for name in ("cfg1", "cfg3_fp32", "cfg3_bf16", "cfg4", "cfg5"):
             if name == args.workload:
                 continue
             try:
