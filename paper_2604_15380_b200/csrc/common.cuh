@@ -128,6 +128,11 @@ int launch_edge_bwd(const EdgeArgs<T>& a, const PT* phi, const PT* v_in, const T
                     T* vb_in, T* fpart, int first_block, __nv_bfloat16* phib16, cudaStream_t st);
 int edge_num_slabs(int F);
 
+// edge_warp.cu — the FP32 model's edge kernels (warp per receiver, filter rows in registers, no CTA barriers)
+int launch_edge_fwd_warp(const EdgeArgs<float>& a, const float* phi, const float* s_in, int64_t ld_sin, const float* v_in,
+                         float* s1, int64_t ld_s1, float* v1, cudaStream_t st);
+int edge_warp_num_slabs(int F, int K);
+
 // node.cu
 // (the trailing BF16 pointers are optional copies / replacements of an output for the BF16 model's GEMM operands)
 template <typename T>

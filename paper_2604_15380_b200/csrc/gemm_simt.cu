@@ -17,6 +17,40 @@ template <typename T> struct V4;
 template <> struct V4<float> { using type = float4; };
 template <> struct V4<double> { using type = double4; };
 
+// acc[i][j] += a[i] b[j].  FP32: packed fma.rn.f32x2 on column pairs (two FMAs per issued instruction; the plain
+// three-register FFMA issues at half rate on sm_100, B300_MICROARCH.md "Pipe rates").
+template <typename T, int TM, int TN>
+__device__ __forceinline__ void mac_tile(const T (&a)[TM], const T (&b)[TN], T (&acc)[TM][TN]) {
+#pragma unroll
+  for (int i = 0; i < TM; ++i)
+#pragma unroll
+    for (int j = 0; j < TN; ++j) acc[i][j] = fma(a[i], b[j], acc[i][j]);
+}
+template <>
+__device__ __forceinline__ void mac_tile<float, 4, 4>(const float (&a)[4], const float (&b)[4], float (&acc)[4][4]) {
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const float2 ai = make_float2(a[i], a[i]);
+#pragma unroll
+    for (int j = 0; j < 4; j += 2) {
+      const float2 r = __ffma2_rn(ai, make_float2(b[j], b[j + 1]), make_float2(acc[i][j], acc[i][j + 1]));
+      acc[i][j] = r.x; acc[i][j + 1] = r.y;
+    }
+  }
+}
+template <>
+__device__ __forceinline__ void mac_tile<float, 8, 8>(const float (&a)[8], const float (&b)[8], float (&acc)[8][8]) {
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const float2 ai = make_float2(a[i], a[i]);
+#pragma unroll
+    for (int j = 0; j < 8; j += 2) {
+      const float2 r = __ffma2_rn(ai, make_float2(b[j], b[j + 1]), make_float2(acc[i][j], acc[i][j + 1]));
+      acc[i][j] = r.x; acc[i][j + 1] = r.y;
+    }
+  }
+}
+
 template <typename T, int BM, int BN, int TM, int TN, int BK>
 __global__ void __launch_bounds__((BM / TM) * (BN / TN))
 gemm_k(int64_t M, int N, int K, const T* __restrict__ A, int64_t lda, const T* __restrict__ B, int64_t ldb,
@@ -102,10 +136,7 @@ gemm_k(int64_t M, int N, int K, const T* __restrict__ A, int64_t lda, const T* _
         const V t = *reinterpret_cast<const V*>(&Bs[buf][k][gj * SN_ + tx * 4]);
         b[gj * 4 + 0] = t.x; b[gj * 4 + 1] = t.y; b[gj * 4 + 2] = t.z; b[gj * 4 + 3] = t.w;
       }
-#pragma unroll
-      for (int i = 0; i < TM; ++i)
-#pragma unroll
-        for (int j = 0; j < TN; ++j) acc[i][j] = fma(a[i], b[j], acc[i][j]);
+      mac_tile<T, TM, TN>(a, b, acc);
     }
     if (kt + 1 < nk) {
       sstore(buf ^ 1);

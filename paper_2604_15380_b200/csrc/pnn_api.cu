@@ -5,6 +5,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "../../include/pnn.h"
@@ -512,6 +513,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
   ea.rowptr = ws->g.rowptr; ea.col = ws->g.col; ea.geom = (const Geom<T>*)ws->g.geom; ea.d_err = ws->g.d_err;
   T* s_cur = (T*)ws->s_cur; T* h = (T*)ws->h; T* sn = (T*)ws->sn; T* v1 = (T*)ws->v1; T* k = (T*)ws->k;
   const bool taped = ws->want_forces != 0;
+  static const bool old_edges = getenv("PNN_FP32_CTA_EDGES") != nullptr; // debugging aid: edge.cu kernels for FP32 too
 
   { ProfScope ps_(ws, st, "embed");
   const int l_ = launch_embed<T>(N, F, c.Zmax, Z, W + m->emb, s_cur, ws->g.d_err, st);
@@ -538,8 +540,14 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     const int l_ = launch_gemm<T>(N, 3 * F, F, h, F, W + b.W2t, 3 * F, phi, 3 * F, e2, st);       // B3a, second Linear
       nl += l_; ps_.done(l_); }
     ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
-    { ProfScope ps_(ws, st, "edge_fwd");
-    const int l_ = launch_edge_fwd<T, T>(ea, phi, s_cur, F, v_in, v_in, sn, 2 * F, v1, EdgeMirror(), st); // B3b -> s' in sn[:, :F], v'
+    { ProfScope ps_(ws, st, "edge_fwd");                                                         // B3b -> s' in sn[:, :F], v'
+      int l_;
+      if constexpr (std::is_same<T, float>::value) {
+        l_ = old_edges ? launch_edge_fwd<T, T>(ea, phi, s_cur, F, v_in, v_in, sn, 2 * F, v1, EdgeMirror(), st)
+                       : launch_edge_fwd_warp(ea, phi, s_cur, F, v_in, sn, 2 * F, v1, st);
+      } else {
+        l_ = launch_edge_fwd<T, T>(ea, phi, s_cur, F, v_in, v_in, sn, 2 * F, v1, EdgeMirror(), st);
+      }
       nl += l_; ps_.done(l_); }
     GemmEpi<T> e3;
     { ProfScope ps_(ws, st, "gemm_3N");
