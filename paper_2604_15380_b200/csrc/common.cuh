@@ -129,8 +129,13 @@ int launch_edge_bwd(const EdgeArgs<T>& a, const PT* phi, const PT* v_in, const T
 int edge_num_slabs(int F);
 
 // edge_warp.cu — the FP32 model's edge kernels (warp per receiver, filter rows in registers, no CTA barriers)
+// wt, dt (both or neither): edge tape [E][3][F] that receives the filter value w and dw/dd of every edge; the reverse
+// kernel reads them back instead of recomputing the filter.
 int launch_edge_fwd_warp(const EdgeArgs<float>& a, const float* phi, const float* s_in, int64_t ld_sin, const float* v_in,
-                         float* s1, int64_t ld_s1, float* v1, cudaStream_t st);
+                         float* s1, int64_t ld_s1, float* v1, float* wt, float* dt, cudaStream_t st);
+int launch_edge_bwd_warp(const EdgeArgs<float>& a, const float* phi, const float* v_in, const float* sb1, const float* vb1,
+                         const float* wt, const float* dt, float* phib, float* vb_in, float* fpart, int first_block,
+                         cudaStream_t st);
 int edge_warp_num_slabs(int F, int K);
 
 // node.cu

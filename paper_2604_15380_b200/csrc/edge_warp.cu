@@ -88,13 +88,17 @@ __device__ __forceinline__ void load_rows(const EdgeArgs<float>& a, int f0, floa
 }
 
 // ------------------------------------------------------------------------------------------ forward
-template <int KP, int FPL, int NWARP>
+// TAPE: also evaluate dw/dd and keep w and dw/dd of every (edge, chunk, feature) for the reverse sweep
+// (wt, dt: [E][3][F]), so that the reverse edge kernel does no filter arithmetic at all.
+template <int KP, int FPL, int NWARP, bool TAPE>
 __global__ void __launch_bounds__(NWARP * 32, FPL == 1 ? 3 : 2)
 edge_fwd_w_k(EdgeArgs<float> a, int RB, const float* __restrict__ phi, const float* __restrict__ s_in, int64_t ld_sin,
-             const float* __restrict__ v_in, float* __restrict__ s1, int64_t ld_s1, float* __restrict__ v1) {
+             const float* __restrict__ v_in, float* __restrict__ s1, int64_t ld_s1, float* __restrict__ v1,
+             float* __restrict__ wt, float* __restrict__ dt) {
   if (*a.d_err & ERRF_EDGE_OVERFLOW) return;
   constexpr int PG = KP + 4;
   __shared__ __align__(16) float G1s[NWARP][TW * PG];
+  __shared__ __align__(16) float G2s[TAPE ? NWARP : 1][TAPE ? TW * PG : 4];
   __shared__ float4 Us[NWARP][TW];
   __shared__ float2 Cs[NWARP][TW];
   __shared__ int Js[NWARP][TW];
@@ -110,6 +114,7 @@ edge_fwd_w_k(EdgeArgs<float> a, int RB, const float* __restrict__ phi, const flo
   const float pi_rc = (float)(3.14159265358979323846 / a.rc);
   const bool has_v = v_in != nullptr;
   float* G1 = G1s[warp]; float4* U = Us[warp]; float2* C = Cs[warp]; int* J = Js[warp];
+  float* G2 = TAPE ? G2s[warp] : nullptr;
 
   const int64_t nchunk = (a.N + RB - 1) / RB;
   for (int64_t ch = blockIdx.x; ch < nchunk; ch += gridDim.x) {
@@ -132,7 +137,7 @@ edge_fwd_w_k(EdgeArgs<float> a, int RB, const float* __restrict__ phi, const flo
       }
       for (int t0 = ea; t0 < eb; t0 += TW) {
         const int nE = min(TW, eb - t0);
-        stage_tile_w<KP, false>(a, lane, t0, nE, G1, nullptr, U, C, J, dmu, gamma, pi_rc);
+        stage_tile_w<KP, TAPE>(a, lane, t0, nE, G1, G2, U, C, J, dmu, gamma, pi_rc);
         // software pipeline: the sender rows of edge q+1 are requested before edge q is consumed
         float ph[3][FPL], vj[3][FPL], phn[3][FPL], vjn[3][FPL];
         auto gather = [&](int q, float (&p_)[3][FPL], float (&v_)[3][FPL]) {
@@ -154,16 +159,33 @@ edge_fwd_w_k(EdgeArgs<float> a, int RB, const float* __restrict__ phi, const flo
           const float4 u = U[q];
           const float cc = C[q].x;
           const float* g = G1 + q * PG;
+          float wv[3][FPL];
+#pragma unroll
+          for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int p = 0; p < FPL; ++p)
+              wv[c][p] = (c < 2 || has_v) ? dot_pairs<KP>(w[c][p], g, bias[c][p] * cc) : 0.0f;
+          if (TAPE) {
+            const float cp = C[q].y;
+            const float* g2 = G2 + q * PG;
+            const int64_t eo = (int64_t)(t0 + q) * 3 * F + f0;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+              if (c == 2 && !has_v) break;
+              float dw[FPL];
+#pragma unroll
+              for (int p = 0; p < FPL; ++p) dw[p] = dot_pairs<KP>(w[c][p], g2, bias[c][p] * cp);
+              stv<FPL>(wt + eo + c * F, wv[c]);
+              stv<FPL>(dt + eo + c * F, dw);
+            }
+          }
 #pragma unroll
           for (int p = 0; p < FPL; ++p) {
-            const float w0 = dot_pairs<KP>(w[0][p], g, bias[0][p] * cc);
-            const float w1 = dot_pairs<KP>(w[1][p], g, bias[1][p] * cc);
-            as[p] = fmaf(ph[0][p], w0, as[p]);
-            const float x1 = ph[1][p] * w1;
+            as[p] = fmaf(ph[0][p], wv[0][p], as[p]);
+            const float x1 = ph[1][p] * wv[1][p];
             av[0][p] = fmaf(x1, u.x, av[0][p]); av[1][p] = fmaf(x1, u.y, av[1][p]); av[2][p] = fmaf(x1, u.z, av[2][p]);
             if (has_v) {
-              const float w2 = dot_pairs<KP>(w[2][p], g, bias[2][p] * cc);
-              const float x2 = ph[2][p] * w2;
+              const float x2 = ph[2][p] * wv[2][p];
               av[0][p] = fmaf(x2, vj[0][p], av[0][p]); av[1][p] = fmaf(x2, vj[1][p], av[1][p]);
               av[2][p] = fmaf(x2, vj[2][p], av[2][p]);
             }
@@ -180,6 +202,116 @@ edge_fwd_w_k(EdgeArgs<float> a, int RB, const float* __restrict__ phi, const flo
   }
 }
 
+// ------------------------------------------------------------------------------------------ reverse
+// R3 + R4 with the filter value w and its derivative dw/dd read from the edge tape the forward kernel wrote: no
+// radial basis, no filter arithmetic, no shared memory.  Per edge a lane streams 6*FPL tape values (coalesced),
+// gathers the sender's phi, s-bar', v-bar', v rows for its features and keeps the receiver's own rows in registers.
+template <int FPL, int NWARP>
+__global__ void __launch_bounds__(NWARP * 32)
+edge_bwd_w_k(EdgeArgs<float> a, int RB, const float* __restrict__ phi, const float* __restrict__ v_in,
+             const float* __restrict__ sb1, const float* __restrict__ vb1, const float* __restrict__ wt,
+             const float* __restrict__ dt, float* __restrict__ phib, float* __restrict__ vb_in,
+             float* __restrict__ fpart, int first_block) {
+  if (*a.d_err & ERRF_EDGE_OVERFLOW) return;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int F = a.F;
+  const int f0 = (blockIdx.y * 32 + lane) * FPL;
+  const bool has_v = v_in != nullptr;
+  const int64_t nchunk = (a.N + RB - 1) / RB;
+  for (int64_t ch = blockIdx.x; ch < nchunk; ch += gridDim.x) {
+    const int64_t i_end = min((int64_t)(ch + 1) * RB, a.N);
+    for (int64_t i = ch * RB + warp; i < i_end; i += NWARP) {
+      const int ea = a.rowptr[i], eb = a.rowptr[i + 1];
+      const int64_t io = i * 3 * F + f0;
+      // the receiver's own rows
+      float li0[FPL], li[3][FPL], lph[3][FPL], lv[3][FPL];
+      ldv<FPL>(sb1 + i * F + f0, li0);
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        ldv<FPL>(vb1 + io + c * F, li[c]);
+        ldv<FPL>(phi + io + c * F, lph[c]);
+        if (has_v) ldv<FPL>(v_in + io + c * F, lv[c]);
+        else {
+#pragma unroll
+          for (int p = 0; p < FPL; ++p) lv[c][p] = 0.f;
+        }
+      }
+      float A0[FPL], A1[FPL], A2[3][FPL];
+#pragma unroll
+      for (int p = 0; p < FPL; ++p) { A0[p] = A1[p] = 0.f; A2[0][p] = A2[1][p] = A2[2][p] = 0.f; }
+      float fp0 = 0.f, fp1 = 0.f, fp2 = 0.f;
+      for (int e = ea; e < eb; ++e) {
+        const int64_t j = __ldg(a.col + e);
+        const float4 u = __ldg(reinterpret_cast<const float4*>(a.geom) + e);
+        const int64_t jo = j * 3 * F + f0, eo = (int64_t)e * 3 * F + f0;
+        float ph[3][FPL], bj[3][FPL], vj[3][FPL], sbj[FPL], wv[3][FPL], dw[3][FPL];
+        ldv<FPL>(sb1 + j * F + f0, sbj);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          ldv<FPL>(phi + jo + c * F, ph[c]);
+          ldv<FPL>(vb1 + jo + c * F, bj[c]);
+          if (c < 2 || has_v) { ldv<FPL>(wt + eo + c * F, wv[c]); ldv<FPL>(dt + eo + c * F, dw[c]); }
+          if (has_v) ldv<FPL>(v_in + jo + c * F, vj[c]);
+        }
+        float D = 0.f, B0 = 0.f, B1 = 0.f, B2 = 0.f;
+#pragma unroll
+        for (int p = 0; p < FPL; ++p) {
+          // scalar chunk
+          A0[p] = fmaf(sbj[p], wv[0][p], A0[p]);
+          D = fmaf(fmaf(li0[p], ph[0][p], sbj[p] * lph[0][p]), dw[0][p], D);
+          // direction chunk
+          const float tj = bj[0][p] * u.x + bj[1][p] * u.y + bj[2][p] * u.z;
+          const float ti = li[0][p] * u.x + li[1][p] * u.y + li[2][p] * u.z;
+          A1[p] = fmaf(-tj, wv[1][p], A1[p]);
+          D = fmaf(ti * ph[1][p] - tj * lph[1][p], dw[1][p], D);
+          B0 = fmaf(li[0][p] * ph[1][p] - bj[0][p] * lph[1][p], wv[1][p], B0);
+          B1 = fmaf(li[1][p] * ph[1][p] - bj[1][p] * lph[1][p], wv[1][p], B1);
+          B2 = fmaf(li[2][p] * ph[1][p] - bj[2][p] * lph[1][p], wv[1][p], B2);
+          // vector chunk
+          if (has_v) {
+            A2[0][p] = fmaf(bj[0][p], wv[2][p], A2[0][p]);
+            A2[1][p] = fmaf(bj[1][p], wv[2][p], A2[1][p]);
+            A2[2][p] = fmaf(bj[2][p], wv[2][p], A2[2][p]);
+            const float liv = li[0][p] * vj[0][p] + li[1][p] * vj[1][p] + li[2][p] * vj[2][p];
+            const float blv = bj[0][p] * lv[0][p] + bj[1][p] * lv[1][p] + bj[2][p] * lv[2][p];
+            D = fmaf(liv * ph[2][p] + blv * lph[2][p], dw[2][p], D);
+          }
+        }
+        const float Bu = B0 * u.x + B1 * u.y + B2 * u.z;
+        const float invd = 1.0f / u.w;
+        fp0 += D * u.x + (B0 - Bu * u.x) * invd;
+        fp1 += D * u.y + (B1 - Bu * u.y) * invd;
+        fp2 += D * u.z + (B2 - Bu * u.z) * invd;
+      }
+      if (phib != nullptr) {
+        float o[FPL];
+        stv<FPL>(phib + io, A0);
+        stv<FPL>(phib + io + F, A1);
+#pragma unroll
+        for (int p = 0; p < FPL; ++p) o[p] = lv[0][p] * A2[0][p] + lv[1][p] * A2[1][p] + lv[2][p] * A2[2][p];
+        stv<FPL>(phib + io + 2 * F, o);
+#pragma unroll
+        for (int ax = 0; ax < 3; ++ax) {
+#pragma unroll
+          for (int p = 0; p < FPL; ++p) o[p] = li[ax][p] + lph[2][p] * A2[ax][p];
+          stv<FPL>(vb_in + io + ax * F, o);
+        }
+      }
+#pragma unroll
+      for (int o = 16; o; o >>= 1) {
+        fp0 += __shfl_xor_sync(0xffffffffu, fp0, o);
+        fp1 += __shfl_xor_sync(0xffffffffu, fp1, o);
+        fp2 += __shfl_xor_sync(0xffffffffu, fp2, o);
+      }
+      if (lane == 0) {
+        float* dst = fpart + ((int64_t)blockIdx.y * a.N + i) * 3;
+        if (first_block) { dst[0] = fp0; dst[1] = fp1; dst[2] = fp2; }
+        else { dst[0] += fp0; dst[1] += fp1; dst[2] += fp2; }
+      }
+    }
+  }
+}
+
 } // namespace
 
 // FPL = 2 needs 6 K-long filter rows per lane in registers: used up to K = 20.
@@ -189,14 +321,18 @@ static int pick_kp4(int K) { return K <= 8 ? 8 : K <= 12 ? 12 : K <= 16 ? 16 : K
 int edge_warp_num_slabs(int F, int K) { return F / (32 * pick_fpl(F, K)); }
 
 int launch_edge_fwd_warp(const EdgeArgs<float>& a, const float* phi, const float* s_in, int64_t ld_sin, const float* v_in,
-                         float* s1, int64_t ld_s1, float* v1, cudaStream_t st) {
+                         float* s1, int64_t ld_s1, float* v1, float* wt, float* dt, cudaStream_t st) {
   if (a.N == 0) return 0;
   const int FPL = pick_fpl(a.F, a.K), KP = pick_kp4(a.K);
   constexpr int NW = 4;
   const int RB = 16;
   const int64_t nchunk = (a.N + RB - 1) / RB;
   dim3 grid((unsigned)std::min<int64_t>(nchunk, 148 * 4), a.F / (32 * FPL));
-#define PNN_L(KPV, FPLV) edge_fwd_w_k<KPV, FPLV, NW><<<grid, NW * 32, 0, st>>>(a, RB, phi, s_in, ld_sin, v_in, s1, ld_s1, v1)
+#define PNN_L(KPV, FPLV)                                                                                              \
+  {                                                                                                                   \
+    if (wt) edge_fwd_w_k<KPV, FPLV, NW, true><<<grid, NW * 32, 0, st>>>(a, RB, phi, s_in, ld_sin, v_in, s1, ld_s1, v1, wt, dt); \
+    else edge_fwd_w_k<KPV, FPLV, NW, false><<<grid, NW * 32, 0, st>>>(a, RB, phi, s_in, ld_sin, v_in, s1, ld_s1, v1, wt, dt);   \
+  }
   if (FPL == 2) {
     switch (KP) {
       case 8: PNN_L(8, 2); break;
@@ -217,6 +353,23 @@ int launch_edge_fwd_warp(const EdgeArgs<float>& a, const float* phi, const float
   }
 #undef PNN_L
   PNN_KCHECK("edge_fwd_w_k");
+  return 1;
+}
+
+int launch_edge_bwd_warp(const EdgeArgs<float>& a, const float* phi, const float* v_in, const float* sb1, const float* vb1,
+                         const float* wt, const float* dt, float* phib, float* vb_in, float* fpart, int first_block,
+                         cudaStream_t st) {
+  if (a.N == 0) return 0;
+  const int FPL = pick_fpl(a.F, a.K);
+  constexpr int NW = 4;
+  const int RB = 16;
+  const int64_t nchunk = (a.N + RB - 1) / RB;
+  dim3 grid((unsigned)std::min<int64_t>(nchunk, 148 * 8), a.F / (32 * FPL));
+  if (FPL == 2)
+    edge_bwd_w_k<2, NW><<<grid, NW * 32, 0, st>>>(a, RB, phi, v_in, sb1, vb1, wt, dt, phib, vb_in, fpart, first_block);
+  else
+    edge_bwd_w_k<1, NW><<<grid, NW * 32, 0, st>>>(a, RB, phi, v_in, sb1, vb1, wt, dt, phib, vb_in, fpart, first_block);
+  PNN_KCHECK("edge_bwd_w_k");
   return 1;
 }
 

@@ -110,6 +110,10 @@ struct pnn_workspace {
   } mb{};
   struct Tape16 { __nv_bfloat16 *vin16, *phi16; };
   std::vector<Tape16> tape16;
+  // FP32 model with forces: per block, the filter value w and dw/dd of every edge ([E][3][F] each), written by the
+  // forward edge kernel and consumed by the reverse one (NULL when it would not fit: the filter is then recomputed)
+  float* etape = nullptr;
+  int64_t etape_block = 0; // floats per block (= 2 * maxE * 3F)
   // staging for pnn_eval_host
   int32_t *st_Z, *st_sptr, *st_head;
   double *st_pos, *st_cell;
@@ -392,12 +396,26 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
       }
     }
   }
+  if (m->cfg.prec == PNN_FP32 && want_forces && maxE > 0) {
+    const int64_t per_block = 2 * maxE * 3 * F;
+    const int64_t bytes = per_block * T * 4;
+    size_t free_b = 0, total_b = 0;
+    cudaMemGetInfo(&free_b, &total_b);
+    if (bytes <= (int64_t)(free_b / 2) && cudaMalloc((void**)&ws->etape, bytes) == cudaSuccess) {
+      ws->etape_block = per_block;
+      ws->arena_bytes += bytes;
+    } else {
+      ws->etape = nullptr;
+      cudaGetLastError();
+    }
+  }
   *out = ws;
   return PNN_OK;
 }
 
 void pnn_workspace_destroy(pnn_workspace* ws) {
   if (!ws) return;
+  cudaFree(ws->etape);
   for (auto& r : ws->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (auto e : ws->ev_pool) cudaEventDestroy(e);
   cudaFree(ws->arena);
@@ -543,8 +561,10 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     { ProfScope ps_(ws, st, "edge_fwd");                                                         // B3b -> s' in sn[:, :F], v'
       int l_;
       if constexpr (std::is_same<T, float>::value) {
+        float* wt = (want_f && ws->etape) ? ws->etape + (int64_t)t * ws->etape_block : nullptr;
         l_ = old_edges ? launch_edge_fwd<T, T>(ea, phi, s_cur, F, v_in, v_in, sn, 2 * F, v1, EdgeMirror(), st)
-                       : launch_edge_fwd_warp(ea, phi, s_cur, F, v_in, sn, 2 * F, v1, st);
+                       : launch_edge_fwd_warp(ea, phi, s_cur, F, v_in, sn, 2 * F, v1, wt,
+                                              wt ? wt + ws->etape_block / 2 : nullptr, st);
       } else {
         l_ = launch_edge_fwd<T, T>(ea, phi, s_cur, F, v_in, v_in, sn, 2 * F, v1, EdgeMirror(), st);
       }
@@ -604,8 +624,19 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       // R3 + R4
       ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
       { ProfScope ps_(ws, st, "edge_bwd");
-      const int l_ = launch_edge_bwd<T, T>(ea, (const T*)tp.phi, (const T*)tp.v_in, sb, vb, t > 0 ? phib : nullptr, vb2,
-                                           fpart, last ? 1 : 0, nullptr, st);
+        int l_;
+        bool taped_edges = false;
+        if constexpr (std::is_same<T, float>::value) taped_edges = !old_edges && ws->etape != nullptr;
+        if constexpr (std::is_same<T, float>::value) {
+          if (taped_edges) {
+            const float* wt = ws->etape + (int64_t)t * ws->etape_block;
+            l_ = launch_edge_bwd_warp(ea, (const T*)tp.phi, (const T*)tp.v_in, sb, vb, wt, wt + ws->etape_block / 2,
+                                      t > 0 ? phib : nullptr, vb2, fpart, last ? 1 : 0, st);
+          }
+        }
+        if (!taped_edges)
+          l_ = launch_edge_bwd<T, T>(ea, (const T*)tp.phi, (const T*)tp.v_in, sb, vb, t > 0 ? phib : nullptr, vb2, fpart,
+                                     last ? 1 : 0, nullptr, st);
         nl += l_; ps_.done(l_); }
       if (t > 0) {
         GemmEpi<T> g4; g4.act = ACT_MUL_DSILU; g4.aux = (const T*)tp.hpre; g4.ldaux = F;
@@ -620,7 +651,10 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       }
     }
     { ProfScope ps_(ws, st, "force_assemble");
-    const int l_ = launch_force_assemble<T>(N, edge_num_slabs(F), fpart, forces, st);
+      int nslab = edge_num_slabs(F);
+      if constexpr (std::is_same<T, float>::value)
+        if (!old_edges && ws->etape != nullptr) nslab = edge_warp_num_slabs(F, c.K);
+    const int l_ = launch_force_assemble<T>(N, nslab, fpart, forces, st);
       nl += l_; ps_.done(l_); }
   }
   ws->launches += nl;
