@@ -111,6 +111,13 @@ def algorithmic_work(family: str, N: int, E: int, mc: gen.ModelCfg, prec: str, f
         if family == "edge_bwd":   # read phi16 6F, v16 6F, sb16 2F, vb16 6F, vb 12F; write phib16 6F, vb_in 12F
             return E * (12 * K * F + 60 * F), N * 50 * F + E * 20
         return None, None
+    if prec == "fp32" and forces:
+        # FP32 model with forces: the forward kernel also evaluates dw/dd and writes the edge tape (w, dw/dd: 24 F bytes
+        # per edge); the reverse kernel reads the tape and does no filter arithmetic
+        if family == "edge_fwd":
+            return E * (12 * K * F + 16 * F), N * 11 * F * b + E * (eb + 24 * F)
+        if family == "edge_bwd":
+            return E * 60 * F, N * 16 * F * b + E * (eb + 24 * F)
     if family == "edge_fwd":
         return E * (6 * K * F + 16 * F), N * 11 * F * b + E * eb
     if family == "edge_bwd":
