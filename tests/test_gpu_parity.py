@@ -169,3 +169,21 @@ def test_host_entry_point_matches_device_entry_point():
     eh, fh = net.eval_host(b.Z, b.pos, b.struct_ptr, b.head)
     assert np.array_equal(e.cpu().numpy(), eh) and np.array_equal(f.cpu().numpy(), fh)
     net.close()
+
+
+def test_fp32_recompute_edge_kernels_subprocess():
+    """The FP32 model normally runs edge_warp.cu with the edge tape; PNN_FP32_CTA_EDGES=1 selects the recomputing
+    kernels of edge.cu (the path taken when the tape does not fit).  Both must meet the FP32 tolerance."""
+    import os
+    import subprocess
+    import sys
+    code = ("import sys, os; sys.path.insert(0, os.getcwd()); sys.path.insert(0, 'tests');"
+            "import gen, oracle; from gpu_common import run_gpu; from helpers import energy_rel_err, force_rel_err;"
+            "mc, b = gen.model_cfg(2), gen.make_batch(2, 3, 12); w = gen.make_weights(mc, 2);"
+            "out = run_gpu(mc, w, b, 'fp32'); ref = oracle.evaluate(mc, w, b);"
+            "assert energy_rel_err(out['energy'], ref['energy']).max() < 1e-5;"
+            "assert force_rel_err(out['forces'], ref['forces'], b.struct_ptr).max() < 1e-4; print('ok')")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, PNN_FP32_CTA_EDGES="1")
+    r = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "ok" in r.stdout, r.stderr[-2000:]
