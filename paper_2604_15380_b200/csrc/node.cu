@@ -3,6 +3,8 @@
 //   scalar-vector products) and of its adjoint (R2), a6 multi-head readout + per-structure segmented sum (B5)
 //   and its adjoint (R1), and the final force assembly (R4).  Formulas: SURVEY.md §8(c).
 // All are streaming kernels: one thread per (atom, feature), consecutive threads on consecutive features.
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace pnn {
@@ -74,6 +76,71 @@ __global__ void __launch_bounds__(256) update_k(int64_t N, int F, const T* __res
   const T r = sn[i * 2 * F + f] + asv * dot + ass;
   s_out[idx] = r;
   if (s16) s16[idx] = __float2bfloat16_rn((float)r);
+}
+
+// ---- FP32-arithmetic versions of norm_k / update_k with 4 features per thread (16-byte FP32 and 8-byte BF16 accesses):
+// these kernels are pure HBM streams, so the access width decides the achieved bandwidth.
+template <typename IT> struct Ld4;
+template <> struct Ld4<float> {
+  static __device__ __forceinline__ float4 ld(const float* p) { return *reinterpret_cast<const float4*>(p); }
+};
+template <> struct Ld4<__nv_bfloat16> {
+  static __device__ __forceinline__ float4 ld(const __nv_bfloat16* p) {
+    const uint2 r = *reinterpret_cast<const uint2*>(p);
+    return make_float4(__uint_as_float(r.x << 16), __uint_as_float(r.x & 0xffff0000u), __uint_as_float(r.y << 16),
+                       __uint_as_float(r.y & 0xffff0000u));
+  }
+};
+__device__ __forceinline__ void st4_bf16(__nv_bfloat16* p, float4 v) {
+  const __nv_bfloat162 a = __floats2bfloat162_rn(v.x, v.y), b = __floats2bfloat162_rn(v.z, v.w);
+  *reinterpret_cast<uint2*>(p) = make_uint2(*reinterpret_cast<const uint32_t*>(&a), *reinterpret_cast<const uint32_t*>(&b));
+}
+
+template <typename IT>
+__global__ void __launch_bounds__(256) norm4_k(int64_t N, int F, const IT* __restrict__ PQ, float* __restrict__ sn, float eps,
+                                               __nv_bfloat16* __restrict__ sn16) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int F4 = F / 4;
+  if (idx >= N * F4) return;
+  const int64_t i = idx / F4;
+  const int f = (int)(idx % F4) * 4;
+  const float4 q0 = Ld4<IT>::ld(PQ + (i * 3 + 0) * 2 * F + F + f), q1 = Ld4<IT>::ld(PQ + (i * 3 + 1) * 2 * F + F + f),
+               q2 = Ld4<IT>::ld(PQ + (i * 3 + 2) * 2 * F + F + f);
+  const float4 n = make_float4(sqrtf(q0.x * q0.x + q1.x * q1.x + q2.x * q2.x + eps), sqrtf(q0.y * q0.y + q1.y * q1.y + q2.y * q2.y + eps),
+                               sqrtf(q0.z * q0.z + q1.z * q1.z + q2.z * q2.z + eps), sqrtf(q0.w * q0.w + q1.w * q1.w + q2.w * q2.w + eps));
+  if (sn16) st4_bf16(sn16 + i * 2 * F + F + f, n);
+  else *reinterpret_cast<float4*>(sn + i * 2 * F + F + f) = n;
+}
+
+template <typename IT>
+__global__ void __launch_bounds__(256) update4_k(int64_t N, int F, const float* __restrict__ sn, const float* __restrict__ v1,
+                                                 const IT* __restrict__ PQ, const IT* __restrict__ a,
+                                                 float* __restrict__ s_out, float* __restrict__ v_out,
+                                                 __nv_bfloat16* __restrict__ s16, __nv_bfloat16* __restrict__ v16) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int F4 = F / 4;
+  if (idx >= N * F4) return;
+  const int64_t i = idx / F4;
+  const int f = (int)(idx % F4) * 4;
+  const float4 avv = Ld4<IT>::ld(a + i * 3 * F + f), asv = Ld4<IT>::ld(a + i * 3 * F + F + f),
+               ass = Ld4<IT>::ld(a + i * 3 * F + 2 * F + f);
+  float4 dot = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+  for (int ax = 0; ax < 3; ++ax) {
+    const float4 p = Ld4<IT>::ld(PQ + (i * 3 + ax) * 2 * F + f), q = Ld4<IT>::ld(PQ + (i * 3 + ax) * 2 * F + F + f);
+    dot.x = fmaf(p.x, q.x, dot.x); dot.y = fmaf(p.y, q.y, dot.y); dot.z = fmaf(p.z, q.z, dot.z); dot.w = fmaf(p.w, q.w, dot.w);
+    if (v_out) {
+      const float4 v = *reinterpret_cast<const float4*>(v1 + (i * 3 + ax) * F + f);
+      const float4 r = make_float4(fmaf(avv.x, p.x, v.x), fmaf(avv.y, p.y, v.y), fmaf(avv.z, p.z, v.z), fmaf(avv.w, p.w, v.w));
+      *reinterpret_cast<float4*>(v_out + (i * 3 + ax) * F + f) = r;
+      if (v16) st4_bf16(v16 + (i * 3 + ax) * F + f, r);
+    }
+  }
+  const float4 s1 = *reinterpret_cast<const float4*>(sn + i * 2 * F + f);
+  const float4 r = make_float4(s1.x + asv.x * dot.x + ass.x, s1.y + asv.y * dot.y + ass.y, s1.z + asv.z * dot.z + ass.z,
+                               s1.w + asv.w * dot.w + ass.w);
+  *reinterpret_cast<float4*>(s_out + idx * 4) = r;
+  if (s16) st4_bf16(s16 + idx * 4, r);
 }
 
 // R2, first half: a-bar [N,3F] and the direct parts of P-bar, Q-bar [N][3][2F]
@@ -292,6 +359,10 @@ int launch_embed(int64_t N, int F, int Zmax, const int32_t* Z, const T* emb, T* 
 template <typename T, typename IT>
 int launch_norm(int64_t N, int F, const IT* PQ, T* sn, T eps, cudaStream_t st, __nv_bfloat16* sn16) {
   if (N == 0) return 0;
+  if constexpr (std::is_same<T, float>::value) {
+    norm4_k<IT><<<nblk(N * (F / 4), 256), 256, 0, st>>>(N, F, PQ, sn, eps, sn16); PNN_KCHECK("norm4_k");
+    return 1;
+  }
   norm_k<T, IT><<<nblk(N * F, 256), 256, 0, st>>>(N, F, PQ, sn, eps, sn16); PNN_KCHECK("norm_k");
   return 1;
 }
@@ -299,6 +370,10 @@ template <typename T, typename IT>
 int launch_update(int64_t N, int F, const T* sn, const T* v1, const IT* PQ, const IT* a, T* s_out, T* v_out,
                   cudaStream_t st, __nv_bfloat16* s16, __nv_bfloat16* v16) {
   if (N == 0) return 0;
+  if constexpr (std::is_same<T, float>::value) {
+    update4_k<IT><<<nblk(N * (F / 4), 256), 256, 0, st>>>(N, F, sn, v1, PQ, a, s_out, v_out, s16, v16); PNN_KCHECK("update4_k");
+    return 1;
+  }
   update_k<T, IT><<<nblk(N * F, 256), 256, 0, st>>>(N, F, sn, v1, PQ, a, s_out, v_out, s16, v16); PNN_KCHECK("update_k");
   return 1;
 }
