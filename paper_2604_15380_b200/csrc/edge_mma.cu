@@ -52,29 +52,28 @@ __device__ __forceinline__ uint32_t pack_bf2(float lo, float hi) {
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ uint4 ldg16(const __nv_bfloat16* p) { return __ldg(reinterpret_cast<const uint4*>(p)); }
 
-// Sum the 32 per-thread partials over the 8 row groups of the fragment layout (lanes t, t+4, ..., t+28) through a
-// per-warp shared-memory buffer of 32 x RED_PITCH bytes, 16 values at a time.
+// Sum the 32 per-thread partials over the 8 row groups of the fragment layout (lanes t, t+4, ..., t+28): a 3-stage
+// shuffle reduce-scatter (16 + 8 + 4 exchanges).  Shuffles, not shared memory: the kernel's L1 / shared-memory data pipe
+// is its busiest unit (profiles/r01_bf16_kernels.md), and a transposition through shared memory measured slower.
 // In: acc[a], a = comp*8 + fi.  Out: lane (g, t) holds a = g*4 .. g*4+3, i.e. comp = g>>1, fi = (g&1)*4 + q.
-constexpr int RED_PITCH = 80; // 16 floats + 16 bytes: conflict-free 16-byte accesses
-__device__ __forceinline__ void reduce_scatter32(const float (&acc)[32], int lane, unsigned char* red, float (&out)[4]) {
-  const int g = lane >> 2, t = lane & 3;
+constexpr int RED_PITCH = 80; // (reverse kernel) 16 floats + 16 bytes: conflict-free 16-byte accesses
+__device__ __forceinline__ void reduce_scatter32(const float (&acc)[32], int lane, unsigned char*, float (&out)[4]) {
+  float s1[16], s2[8];
+  const bool b2 = (lane & 16) != 0, b1 = (lane & 8) != 0, b0 = (lane & 4) != 0;
 #pragma unroll
-  for (int h = 0; h < 2; ++h) {
+  for (int q = 0; q < 16; ++q) {
+    const float keep = b2 ? acc[q + 16] : acc[q], send = b2 ? acc[q] : acc[q + 16];
+    s1[q] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+  }
 #pragma unroll
-    for (int q = 0; q < 4; ++q)
-      *reinterpret_cast<float4*>(red + lane * RED_PITCH + q * 16) =
-          make_float4(acc[16 * h + 4 * q], acc[16 * h + 4 * q + 1], acc[16 * h + 4 * q + 2], acc[16 * h + 4 * q + 3]);
-    __syncwarp();
-    if ((g >> 2) == h) {
-      float4 s = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int q = 0; q < 8; ++q) {
+    const float keep = b1 ? s1[q + 8] : s1[q], send = b1 ? s1[q] : s1[q + 8];
+    s2[q] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+  }
 #pragma unroll
-      for (int gg = 0; gg < 8; ++gg) {
-        const float4 x = *reinterpret_cast<const float4*>(red + (gg * 4 + t) * RED_PITCH + (g & 3) * 16);
-        s.x += x.x; s.y += x.y; s.z += x.z; s.w += x.w;
-      }
-      out[0] = s.x; out[1] = s.y; out[2] = s.z; out[3] = s.w;
-    }
-    __syncwarp();
+  for (int q = 0; q < 4; ++q) {
+    const float keep = b0 ? s2[q + 4] : s2[q], send = b0 ? s2[q] : s2[q + 4];
+    out[q] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
   }
 }
 
