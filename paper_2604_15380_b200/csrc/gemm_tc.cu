@@ -15,6 +15,8 @@
 // 2 x <= 113 KB) so one tile's epilogue overlaps the other's loads and MMAs.
 #include <cuda.h>
 
+#include <algorithm>
+#include <cstdlib>
 #include <mutex>
 #include <unordered_map>
 
@@ -88,6 +90,60 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
       : "r"(taddr)
       : "memory");
   asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// Epilogue of one output row segment: 32 accumulator columns of row m starting at column n (bias, activation, optional
+// pre-activation store / silu' factor / accumulate, FP32 and / or BF16 stores as 16-byte vectors of the row).
+__device__ __forceinline__ void epi_chunk(const TcEpi& epi, int64_t m, int n, const uint32_t (&r)[32]) {
+  float x[32];
+#pragma unroll
+  for (int j = 0; j < 32; ++j) x[j] = __uint_as_float(r[j]);
+  if (epi.bias) {
+#pragma unroll
+    for (int j = 0; j < 32; j += 4) {
+      const float4 bv = __ldg(reinterpret_cast<const float4*>(epi.bias + n + j));
+      x[j] += bv.x; x[j + 1] += bv.y; x[j + 2] += bv.z; x[j + 3] += bv.w;
+    }
+  }
+  if (epi.act == ACT_SILU) {
+    if (epi.pre) {
+      float4* pp = reinterpret_cast<float4*>(epi.pre + m * epi.ldpre + n);
+#pragma unroll
+      for (int j = 0; j < 32; j += 4) pp[j >> 2] = make_float4(x[j], x[j + 1], x[j + 2], x[j + 3]);
+    }
+#pragma unroll
+    for (int j = 0; j < 32; ++j) x[j] = silu_f<float>(x[j]);
+  } else if (epi.act == ACT_MUL_DSILU) {
+    const float4* ap = reinterpret_cast<const float4*>(epi.aux + m * epi.ldaux + n);
+#pragma unroll
+    for (int j = 0; j < 32; j += 4) {
+      const float4 av = ap[j >> 2];
+      x[j] *= dsilu_f<float>(av.x); x[j + 1] *= dsilu_f<float>(av.y);
+      x[j + 2] *= dsilu_f<float>(av.z); x[j + 3] *= dsilu_f<float>(av.w);
+    }
+  }
+  if (epi.C) {
+    float4* cp = reinterpret_cast<float4*>(epi.C + m * epi.ldc + n);
+    if (epi.accumulate) {
+#pragma unroll
+      for (int j = 0; j < 32; j += 4) {
+        const float4 cv = cp[j >> 2];
+        x[j] += cv.x; x[j + 1] += cv.y; x[j + 2] += cv.z; x[j + 3] += cv.w;
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < 32; j += 4) cp[j >> 2] = make_float4(x[j], x[j + 1], x[j + 2], x[j + 3]);
+  }
+  if (epi.Cb) {
+    uint4* bp = reinterpret_cast<uint4*>(epi.Cb + m * epi.ldcb + n);
+#pragma unroll
+    for (int j = 0; j < 32; j += 8) {
+      __nv_bfloat162 h0 = __floats2bfloat162_rn(x[j], x[j + 1]), h1 = __floats2bfloat162_rn(x[j + 2], x[j + 3]);
+      __nv_bfloat162 h2 = __floats2bfloat162_rn(x[j + 4], x[j + 5]), h3 = __floats2bfloat162_rn(x[j + 6], x[j + 7]);
+      bp[j >> 3] = make_uint4(*reinterpret_cast<uint32_t*>(&h0), *reinterpret_cast<uint32_t*>(&h1),
+                              *reinterpret_cast<uint32_t*>(&h2), *reinterpret_cast<uint32_t*>(&h3));
+    }
+  }
 }
 
 template <int BN, int STAGES>
@@ -213,56 +269,7 @@ tc_gemm_k(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         if (c0 + 32 >= BN) epi.eatom[m] = esum + epi.b2[hrow];
         continue;
       }
-      const int n = n0 + c0;
-      float x[32];
-#pragma unroll
-      for (int j = 0; j < 32; ++j) x[j] = __uint_as_float(r[j]);
-      if (epi.bias) {
-#pragma unroll
-        for (int j = 0; j < 32; j += 4) {
-          const float4 bv = __ldg(reinterpret_cast<const float4*>(epi.bias + n + j));
-          x[j] += bv.x; x[j + 1] += bv.y; x[j + 2] += bv.z; x[j + 3] += bv.w;
-        }
-      }
-      if (epi.act == ACT_SILU) {
-        if (epi.pre) {
-          float4* pp = reinterpret_cast<float4*>(epi.pre + m * epi.ldpre + n);
-#pragma unroll
-          for (int j = 0; j < 32; j += 4) pp[j >> 2] = make_float4(x[j], x[j + 1], x[j + 2], x[j + 3]);
-        }
-#pragma unroll
-        for (int j = 0; j < 32; ++j) x[j] = silu_f<float>(x[j]);
-      } else if (epi.act == ACT_MUL_DSILU) {
-        const float4* ap = reinterpret_cast<const float4*>(epi.aux + m * epi.ldaux + n);
-#pragma unroll
-        for (int j = 0; j < 32; j += 4) {
-          const float4 av = ap[j >> 2];
-          x[j] *= dsilu_f<float>(av.x); x[j + 1] *= dsilu_f<float>(av.y);
-          x[j + 2] *= dsilu_f<float>(av.z); x[j + 3] *= dsilu_f<float>(av.w);
-        }
-      }
-      if (epi.C) {
-        float4* cp = reinterpret_cast<float4*>(epi.C + m * epi.ldc + n);
-        if (epi.accumulate) {
-#pragma unroll
-          for (int j = 0; j < 32; j += 4) {
-            const float4 cv = cp[j >> 2];
-            x[j] += cv.x; x[j + 1] += cv.y; x[j + 2] += cv.z; x[j + 3] += cv.w;
-          }
-        }
-#pragma unroll
-        for (int j = 0; j < 32; j += 4) cp[j >> 2] = make_float4(x[j], x[j + 1], x[j + 2], x[j + 3]);
-      }
-      if (epi.Cb) {
-        uint4* bp = reinterpret_cast<uint4*>(epi.Cb + m * epi.ldcb + n);
-#pragma unroll
-        for (int j = 0; j < 32; j += 8) {
-          __nv_bfloat162 h0 = __floats2bfloat162_rn(x[j], x[j + 1]), h1 = __floats2bfloat162_rn(x[j + 2], x[j + 3]);
-          __nv_bfloat162 h2 = __floats2bfloat162_rn(x[j + 4], x[j + 5]), h3 = __floats2bfloat162_rn(x[j + 6], x[j + 7]);
-          bp[j >> 3] = make_uint4(*reinterpret_cast<uint32_t*>(&h0), *reinterpret_cast<uint32_t*>(&h1),
-                                  *reinterpret_cast<uint32_t*>(&h2), *reinterpret_cast<uint32_t*>(&h3));
-        }
-      }
+      epi_chunk(epi, m, n0 + c0, r);
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   }
@@ -270,6 +277,111 @@ tc_gemm_k(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   if (warp == 2) {
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(BN) : "memory");
+  }
+}
+
+// Persistent variant for large M (the screening batches): one CTA per SM slot walks tiles t = blockIdx.x, + gridDim.x, ...
+// The shared-memory stage ring runs on across tiles, and the accumulator is double-buffered in TMEM (2 x BN columns), so
+// the TMA loads and MMAs of tile i+1 overlap the epilogue (global stores) of tile i: these GEMMs have K <= 768 and are
+// bound by HBM traffic, not by the tensor pipe, so what matters is that loads and stores never pause.
+template <int BN, int STAGES>
+__global__ void __launch_bounds__(NTHREADS)
+tc_gemm_pk(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int64_t M, int N, int K,
+           int n_tiles, int64_t total_tiles, TcEpi epi) {
+  constexpr int A_BYTES = BM * BK * 2, B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const uint32_t raw = smem_u32(smem_raw);
+  const uint32_t tiles = (raw + 1023u) & ~1023u;
+  unsigned char* tiles_ptr = smem_raw + (tiles - raw);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tiles_ptr + STAGES * STAGE_BYTES); // full[S], empty[S], accfull[2], accempty[2]
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 4);
+  const uint32_t bar0 = smem_u32(bars);
+  auto full_bar = [&](int s) { return bar0 + 8u * s; };
+  auto empty_bar = [&](int s) { return bar0 + 8u * (STAGES + s); };
+  auto accfull_bar = [&](int b) { return bar0 + 8u * (2 * STAGES + b); };
+  auto accempty_bar = [&](int b) { return bar0 + 8u * (2 * STAGES + 2 + b); };
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nkb = (K + BK - 1) / BK;
+
+  if (warp == 1 && lane == 0) {
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(accfull_bar(b), 1); mbar_init(accempty_bar(b), 4); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 2) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(2 * BN)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      uint32_t it = 0; // k-blocks issued so far: stage = it % STAGES, parity = (it / STAGES) & 1
+      for (int64_t tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+        const int m0 = (int)((tile / n_tiles) * BM), n0 = (int)(tile % n_tiles) * BN;
+        for (int kb = 0; kb < nkb; ++kb, ++it) {
+          const int s = it % STAGES;
+          mbar_wait(empty_bar(s), ((it / STAGES) & 1u) ^ 1u);
+          const uint32_t sa = tiles + s * STAGE_BYTES;
+          mbar_expect_tx(full_bar(s), STAGE_BYTES);
+          tma_load_2d(sa, &tmA, full_bar(s), kb * BK, m0);
+          tma_load_2d(sa + A_BYTES, &tmB, full_bar(s), kb * BK, n0);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+      uint32_t it = 0, j = 0; // j: tiles done by this CTA; accumulator buffer j & 1
+      for (int64_t tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++j) {
+        const uint32_t b = j & 1u;
+        mbar_wait(accempty_bar(b), ((j >> 1) & 1u) ^ 1u); // the epilogue has drained this buffer
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const uint32_t acc = tmem_base + b * BN;
+        for (int kb = 0; kb < nkb; ++kb, ++it) {
+          const int s = it % STAGES;
+          mbar_wait(full_bar(s), (it / STAGES) & 1u);
+          asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+          const uint32_t sa = tiles + s * STAGE_BYTES;
+          const uint64_t ad = umma_desc_sw128(sa), bd = umma_desc_sw128(sa + A_BYTES);
+#pragma unroll
+          for (int k = 0; k < BK / 16; ++k)
+            umma_bf16(acc, ad + (uint64_t)(k * 2), bd + (uint64_t)(k * 2), idesc, (kb | k) ? 1u : 0u);
+          umma_commit(empty_bar(s));
+        }
+        umma_commit(accfull_bar(b));
+      }
+    }
+  } else {
+    const int q = warp & 3;
+    uint32_t j = 0;
+    for (int64_t tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++j) {
+      const uint32_t b = j & 1u;
+      const int64_t m = (tile / n_tiles) * BM + q * 32 + lane;
+      const int n0 = (int)(tile % n_tiles) * BN;
+      mbar_wait(accfull_bar(b), (j >> 1) & 1u);
+      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll 1
+      for (int c0 = 0; c0 < BN; c0 += 32) {
+        uint32_t r[32];
+        tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + b * BN + (uint32_t)c0, r);
+        if (m < M) epi_chunk(epi, m, n0 + c0, r);
+      }
+      // all TMEM reads of this warp are complete (tcgen05.wait::ld in tmem_ld32): hand the buffer back to the MMA warp
+      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+      __syncwarp();
+      if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(accempty_bar(b)) : "memory");
+    }
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 2) {
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(2 * BN) : "memory");
   }
 }
 
@@ -339,6 +451,24 @@ bool get_tensor_map(const __nv_bfloat16* ptr, int64_t rows, int cols, int64_t ld
 }
 
 template <int BN, int STAGES>
+int launch_persistent(int64_t M, int N, int K, const CUtensorMap& ta, const CUtensorMap& tb, const TcEpi& epi,
+                      cudaStream_t st) {
+  constexpr int SMEM = STAGES * (BM * BK * 2 + BN * BK * 2) + 1024 + 256;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(tc_gemm_pk<BN, STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
+    attr_set = true;
+  }
+  const int n_tiles = N / BN;
+  const int64_t total = ((M + BM - 1) / BM) * n_tiles;
+  const int per_sm = (2 * BN <= 256 && SMEM <= 110 * 1024) ? 2 : 1; // TMEM: 512 columns per SM
+  const unsigned grid = (unsigned)std::min<int64_t>(total, 148 * per_sm);
+  tc_gemm_pk<BN, STAGES><<<grid, NTHREADS, SMEM, st>>>(ta, tb, M, N, K, n_tiles, total, epi);
+  PNN_KCHECK("tc_gemm_pk");
+  return 1;
+}
+
+template <int BN, int STAGES>
 int launch_cfg(int64_t M, int N, int K, const CUtensorMap& ta, const CUtensorMap& tb, const TcEpi& epi,
                cudaStream_t st) {
   using L = TcSmem<BN, STAGES>;
@@ -365,8 +495,20 @@ int launch_gemm_tc(int64_t M, int N, int K, const __nv_bfloat16* A, int64_t lda,
   int bn = (N % 64 == 0) ? 64 : 32;
   for (int cand = 256; cand > 64; cand >>= 1)
     if (N % cand == 0 && m_tiles * (N / cand) >= 2 * 148) { bn = cand; break; }
+  static const bool no_persist = getenv("PNN_TC_NO_PERSIST") != nullptr; // debugging aid
+  const bool persist = !no_persist && m_tiles * (N / bn) >= 8 * 148;
+  // persistent kernel: 128-wide tiles, so that two CTAs (eight epilogue warps) share an SM and its 512 TMEM columns
+  if (persist && bn == 256) bn = 128;
   CUtensorMap ta, tb;
   if (!get_tensor_map(A, M, K, lda, BM, &ta) || !get_tensor_map(Wt, N, K, ldw, bn, &tb)) return -1;
+  if (persist) { // many tiles per SM: the persistent, double-buffered kernel
+    switch (bn) {
+      case 256: return launch_persistent<256, 4>(M, N, K, ta, tb, epi, st);
+      case 128: return launch_persistent<128, 3>(M, N, K, ta, tb, epi, st);
+      case 64: return launch_persistent<64, 4>(M, N, K, ta, tb, epi, st);
+      default: return launch_persistent<32, 4>(M, N, K, ta, tb, epi, st);
+    }
+  }
   switch (bn) {
     case 256: return launch_cfg<256, 2>(M, N, K, ta, tb, epi, st);
     case 128: return launch_cfg<128, 3>(M, N, K, ta, tb, epi, st);

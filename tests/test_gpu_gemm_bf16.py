@@ -8,7 +8,9 @@ pytestmark = pytest.mark.gpu
 
 
 @pytest.mark.parametrize("M,N,K", [(128, 32, 32), (1000, 96, 96), (300, 128, 256), (4133, 384, 128), (2500, 768, 256),
-                                   (777, 256, 512), (129, 512, 768), (1, 64, 64)])
+                                   (777, 256, 512), (129, 512, 768), (1, 64, 64),
+                                   # >= 8 x 148 tiles: the persistent kernel (double-buffered TMEM accumulator)
+                                   (160001, 256, 128), (200003, 96, 64), (90000, 768, 256)])
 @pytest.mark.parametrize("act", [0, 1])
 def test_gemm_bf16_matches_fp64(M, N, K, act):
     import torch
