@@ -1,7 +1,7 @@
 // edge_warp.cu — a4 / a7 edge kernels of the FP32 model, exact FP32 arithmetic on the ordinary ALUs.
 //
 // Same mathematics as edge.cu (sender scatters rewritten as gathers over the receiver's own
-// CSR row), different mapping, chosen from the ncu stall profile of edge.cu (profiles/r01_edge_bwd_cfg2_fp32.md: gather
+// CSR row), different mapping, chosen from the ncu stall profile of edge.cu (profiles/r01_edge_fp32_cfg2.md: gather
 // latency and CTA barriers, not FMA throughput):
 //   * one WARP per receiver, no CTA barrier in the main loop;
 //   * a lane owns FPL (1 or 2) contiguous features of a 32*FPL-wide slab for the whole kernel and keeps the 3*FPL filter
