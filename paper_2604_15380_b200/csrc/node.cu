@@ -273,6 +273,127 @@ __global__ void __launch_bounds__(128) readout_k(int64_t N, int F, int H, const 
   }
 }
 
+// ---- readout, second version: all threads busy.  A CTA takes RT = 16 atoms; thread (og, rg) owns 4 consecutive hidden
+// units (og) of rows rg and rg + 8.  Per input feature k it reads its head's 4 weights as one vector (coalesced over og,
+// L1-resident across the 8 row groups) and the two activations from shared memory: 8 FMAs per 3 loads (readout_k: 16
+// per 17), and no thread idles when F/2 < blockDim.  Each row uses the first layer of its own head, so a tile may mix
+// heads freely.  blockDim = 8 * Fh / 4.
+template <typename T> struct Vec4;
+template <> struct Vec4<float> {
+  static __device__ __forceinline__ void ld(const float* p, float (&x)[4]) {
+    const float4 v = *reinterpret_cast<const float4*>(p); x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w;
+  }
+};
+template <> struct Vec4<double> {
+  static __device__ __forceinline__ void ld(const double* p, double (&x)[4]) {
+    const double2 a = *reinterpret_cast<const double2*>(p), b = *reinterpret_cast<const double2*>(p + 2);
+    x[0] = a.x; x[1] = a.y; x[2] = b.x; x[3] = b.y;
+  }
+};
+
+template <typename T>
+__global__ void __launch_bounds__(256) readout2_k(int64_t N, int F, int H, const T* __restrict__ s,
+                                                  const int32_t* __restrict__ a2s, const int32_t* __restrict__ head,
+                                                  const T* __restrict__ W1t, const T* __restrict__ b1,
+                                                  const T* __restrict__ w2, const T* __restrict__ b2,
+                                                  T* __restrict__ opre, T* __restrict__ eatom, int* d_err) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int Fh = F / 2, NOG = Fh / 4;
+  T* S = reinterpret_cast<T*>(smem_raw);  // [RT][F]
+  T* Ep = S + RT * F;                     // [RT][NOG] partial energies
+  __shared__ int Hs[RT];
+  const int64_t i0 = (int64_t)blockIdx.x * RT;
+  const int nt = (int)min((int64_t)RT, N - i0);
+  for (int q = threadIdx.x; q < RT * F; q += blockDim.x) S[q] = (q < nt * F) ? s[i0 * F + q] : T(0);
+  if (threadIdx.x < RT) {
+    int h = 0;
+    if (threadIdx.x < nt) {
+      h = head[a2s[i0 + threadIdx.x]];
+      if (h < 0 || h >= H) { atomicOr(d_err, ERRF_BAD_HEAD); h = 0; }
+    }
+    Hs[threadIdx.x] = h;
+  }
+  __syncthreads();
+  const int og = threadIdx.x % NOG, rg = threadIdx.x / NOG; // rg in 0..7
+  const int h0 = Hs[rg], h1 = Hs[rg + 8];
+  const T* W0 = W1t + (int64_t)h0 * F * Fh + og * 4;
+  const T* W1p = W1t + (int64_t)h1 * F * Fh + og * 4;
+  T acc0[4] = {T(0), T(0), T(0), T(0)}, acc1[4] = {T(0), T(0), T(0), T(0)};
+#pragma unroll 4
+  for (int k = 0; k < F; ++k) {
+    T wa[4], wb[4];
+    Vec4<T>::ld(W0 + (int64_t)k * Fh, wa);
+    Vec4<T>::ld(W1p + (int64_t)k * Fh, wb);
+    const T x0 = S[rg * F + k], x1 = S[(rg + 8) * F + k];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { acc0[j] = fma(wa[j], x0, acc0[j]); acc1[j] = fma(wb[j], x1, acc1[j]); }
+  }
+#pragma unroll
+  for (int r = 0; r < 2; ++r) {
+    const int row = rg + 8 * r, h = r ? h1 : h0;
+    T e = T(0);
+    if (row < nt) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int o = og * 4 + j;
+        const T pre = (r ? acc1[j] : acc0[j]) + b1[h * Fh + o];
+        if (opre) opre[(i0 + row) * Fh + o] = pre;
+        e = fma(w2[h * Fh + o], silu_f<T>(pre), e);
+      }
+    }
+    Ep[row * NOG + og] = e;
+  }
+  __syncthreads();
+  if (threadIdx.x < nt) {
+    T e = T(0);
+    for (int q = 0; q < NOG; ++q) e += Ep[threadIdx.x * NOG + q];
+    eatom[i0 + threadIdx.x] = e + b2[Hs[threadIdx.x]];
+  }
+}
+
+// R1, second version: thread (kg, rg) owns 4 consecutive input features of rows rg and rg + 8.  blockDim = 8 * F / 4.
+template <typename T>
+__global__ void __launch_bounds__(512) readout_bwd2_k(int64_t N, int F, int H, const T* __restrict__ opre,
+                                                      const int32_t* __restrict__ a2s, const int32_t* __restrict__ head,
+                                                      const T* __restrict__ W1, const T* __restrict__ w2,
+                                                      T* __restrict__ sb) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int Fh = F / 2, NKG = F / 4;
+  T* Pb = reinterpret_cast<T*>(smem_raw); // [RT][Fh]  p = w2 o silu'(pre)
+  __shared__ int Hs[RT];
+  const int64_t i0 = (int64_t)blockIdx.x * RT;
+  const int nt = (int)min((int64_t)RT, N - i0);
+  if (threadIdx.x < RT) {
+    int h = 0;
+    if (threadIdx.x < nt) { h = head[a2s[i0 + threadIdx.x]]; if (h < 0 || h >= H) h = 0; }
+    Hs[threadIdx.x] = h;
+  }
+  __syncthreads();
+  for (int q = threadIdx.x; q < RT * Fh; q += blockDim.x) {
+    const int r = q / Fh, o = q % Fh;
+    Pb[q] = (r < nt) ? w2[Hs[r] * Fh + o] * dsilu_f<T>(opre[(i0 + r) * Fh + o]) : T(0);
+  }
+  __syncthreads();
+  const int kg = threadIdx.x % NKG, rg = threadIdx.x / NKG;
+  const T* Wa = W1 + (int64_t)Hs[rg] * Fh * F + kg * 4;
+  const T* Wb = W1 + (int64_t)Hs[rg + 8] * Fh * F + kg * 4;
+  T acc0[4] = {T(0), T(0), T(0), T(0)}, acc1[4] = {T(0), T(0), T(0), T(0)};
+#pragma unroll 4
+  for (int o = 0; o < Fh; ++o) {
+    T wa[4], wb[4];
+    Vec4<T>::ld(Wa + (int64_t)o * F, wa);
+    Vec4<T>::ld(Wb + (int64_t)o * F, wb);
+    const T p0 = Pb[rg * Fh + o], p1 = Pb[(rg + 8) * Fh + o];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { acc0[j] = fma(wa[j], p0, acc0[j]); acc1[j] = fma(wb[j], p1, acc1[j]); }
+  }
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    if (rg < nt) sb[(i0 + rg) * F + kg * 4 + j] = acc0[j];
+    if (rg + 8 < nt) sb[(i0 + rg + 8) * F + kg * 4 + j] = acc1[j];
+  }
+}
+
 // E_g = sum of the structure's atom energies (segmented sum, fixed tree order)
 template <typename T>
 __global__ void __launch_bounds__(128) struct_sum_k(const int32_t* __restrict__ sptr, const T* __restrict__ eatom,
@@ -403,7 +524,14 @@ int launch_readout(int64_t N, int64_t S, int F, int H, const T* s, const int32_t
       cudaFuncSetAttribute(readout_k<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
       attr_set = true;
     }
-    readout_k<T><<<nblk(N, RT), 128, smem, st>>>(N, F, H, s, a2s, head, W1t, b1, w2, b2, opre, eatom, d_err); PNN_KCHECK("readout_k");
+    if (F % 8 == 0 && F <= 256) {
+      const size_t smem2 = sizeof(T) * (RT * F + RT * (F / 8));
+      static bool attr2 = false;
+      if (!attr2) { cudaFuncSetAttribute(readout2_k<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024); attr2 = true; }
+      readout2_k<T><<<nblk(N, RT), 8 * (F / 8), smem2, st>>>(N, F, H, s, a2s, head, W1t, b1, w2, b2, opre, eatom, d_err); PNN_KCHECK("readout2_k");
+    } else {
+      readout_k<T><<<nblk(N, RT), 128, smem, st>>>(N, F, H, s, a2s, head, W1t, b1, w2, b2, opre, eatom, d_err); PNN_KCHECK("readout_k");
+    }
     ++nl;
   }
   if (S > 0) {
@@ -423,6 +551,10 @@ int launch_readout_bwd(int64_t N, int F, int H, const T* opre, const int32_t* a2
                        const T* w2, T* sb, cudaStream_t st) {
   if (N == 0) return 0;
   const size_t smem = sizeof(T) * (RT * (F / 2));
+  if (F % 8 == 0 && F <= 256) {
+    readout_bwd2_k<T><<<nblk(N, RT), 8 * (F / 4), smem, st>>>(N, F, H, opre, a2s, head, W1, w2, sb); PNN_KCHECK("readout_bwd2_k");
+    return 1;
+  }
   readout_bwd_k<T><<<nblk(N, RT), F < 256 ? (F < 64 ? 64 : F) : 256, smem, st>>>(N, F, H, opre, a2s, head, W1, w2, sb); PNN_KCHECK("readout_bwd_k");
   return 1;
 }
