@@ -213,6 +213,84 @@ __global__ void __launch_bounds__(256) update_bwd2_k(int64_t N, int F, const T* 
   }
 }
 
+// ---- 4 features per thread versions of the two kernels above (FP32 arithmetic; same formulas)
+__device__ __forceinline__ float4 f4mul(float4 a, float4 b) { return make_float4(a.x * b.x, a.y * b.y, a.z * b.z, a.w * b.w); }
+__device__ __forceinline__ float4 f4fma(float4 a, float4 b, float4 c) {
+  return make_float4(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y), fmaf(a.z, b.z, c.z), fmaf(a.w, b.w, c.w));
+}
+template <typename IT>
+__global__ void __launch_bounds__(256) update_bwd1_4_k(int64_t N, int F, const float* __restrict__ sb,
+                                                       const float* __restrict__ vb, const IT* __restrict__ a,
+                                                       const IT* __restrict__ PQ, float* __restrict__ ab,
+                                                       float* __restrict__ PQb, __nv_bfloat16* __restrict__ ab16) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int F4 = F / 4;
+  if (idx >= N * F4) return;
+  const int64_t i = idx / F4;
+  const int f = (int)(idx % F4) * 4;
+  const float4 sbf = *reinterpret_cast<const float4*>(sb + i * F + f);
+  const float4 avv = Ld4<IT>::ld(a + i * 3 * F + f), asv = Ld4<IT>::ld(a + i * 3 * F + F + f);
+  float4 p[3], q[3], vbf[3];
+  float4 dot = make_float4(0.f, 0.f, 0.f, 0.f), avvb = dot;
+#pragma unroll
+  for (int ax = 0; ax < 3; ++ax) {
+    p[ax] = Ld4<IT>::ld(PQ + (i * 3 + ax) * 2 * F + f);
+    q[ax] = Ld4<IT>::ld(PQ + (i * 3 + ax) * 2 * F + F + f);
+    vbf[ax] = vb ? *reinterpret_cast<const float4*>(vb + (i * 3 + ax) * F + f) : make_float4(0.f, 0.f, 0.f, 0.f);
+    dot = f4fma(p[ax], q[ax], dot);
+    avvb = f4fma(vbf[ax], p[ax], avvb);
+  }
+  const float4 sd = f4mul(sbf, dot);
+  if (ab16) {
+    st4_bf16(ab16 + i * 3 * F + f, avvb); st4_bf16(ab16 + i * 3 * F + F + f, sd); st4_bf16(ab16 + i * 3 * F + 2 * F + f, sbf);
+  } else {
+    *reinterpret_cast<float4*>(ab + i * 3 * F + f) = avvb;
+    *reinterpret_cast<float4*>(ab + i * 3 * F + F + f) = sd;
+    *reinterpret_cast<float4*>(ab + i * 3 * F + 2 * F + f) = sbf;
+  }
+  const float4 dotb = f4mul(sbf, asv);
+#pragma unroll
+  for (int ax = 0; ax < 3; ++ax) {
+    *reinterpret_cast<float4*>(PQb + (i * 3 + ax) * 2 * F + f) = f4fma(dotb, q[ax], f4mul(vbf[ax], avv));
+    *reinterpret_cast<float4*>(PQb + (i * 3 + ax) * 2 * F + F + f) = f4mul(dotb, p[ax]);
+  }
+}
+
+template <typename IT>
+__global__ void __launch_bounds__(256) update_bwd2_4_k(int64_t N, int F, const float* __restrict__ zb,
+                                                       const IT* __restrict__ PQ, float eps, float* __restrict__ sb,
+                                                       float* __restrict__ PQb, __nv_bfloat16* __restrict__ PQb16,
+                                                       __nv_bfloat16* __restrict__ sb16) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int F4 = F / 4;
+  if (idx >= N * F4) return;
+  const int64_t i = idx / F4;
+  const int f = (int)(idx % F4) * 4;
+  const float4 s0 = *reinterpret_cast<const float4*>(sb + i * F + f), z0 = *reinterpret_cast<const float4*>(zb + i * 2 * F + f);
+  const float4 sbn = make_float4(s0.x + z0.x, s0.y + z0.y, s0.z + z0.z, s0.w + z0.w);
+  *reinterpret_cast<float4*>(sb + i * F + f) = sbn;
+  if (sb16) st4_bf16(sb16 + i * F + f, sbn);
+  const float4 nb = *reinterpret_cast<const float4*>(zb + i * 2 * F + F + f);
+  float4 q[3];
+#pragma unroll
+  for (int ax = 0; ax < 3; ++ax) q[ax] = Ld4<IT>::ld(PQ + (i * 3 + ax) * 2 * F + F + f);
+  const float4 r = make_float4(nb.x / sqrtf(q[0].x * q[0].x + q[1].x * q[1].x + q[2].x * q[2].x + eps),
+                               nb.y / sqrtf(q[0].y * q[0].y + q[1].y * q[1].y + q[2].y * q[2].y + eps),
+                               nb.z / sqrtf(q[0].z * q[0].z + q[1].z * q[1].z + q[2].z * q[2].z + eps),
+                               nb.w / sqrtf(q[0].w * q[0].w + q[1].w * q[1].w + q[2].w * q[2].w + eps));
+#pragma unroll
+  for (int ax = 0; ax < 3; ++ax) {
+    const int64_t o = (i * 3 + ax) * 2 * F + f;
+    const float4 qb = f4fma(r, q[ax], *reinterpret_cast<const float4*>(PQb + o + F));
+    if (PQb16) {
+      st4_bf16(PQb16 + o, *reinterpret_cast<const float4*>(PQb + o));
+      st4_bf16(PQb16 + o + F, qb);
+    } else {
+      *reinterpret_cast<float4*>(PQb + o + F) = qb;
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------ readout
 // One CTA per tile of RT consecutive atoms.  Atoms of a structure are contiguous and share a head, so the tile
 // splits into a few runs of equal head; each run is a small [run x F] x [F x F/2] product with the head's W1.
@@ -502,6 +580,10 @@ template <typename T, typename IT>
 int launch_update_bwd1(int64_t N, int F, const T* sb, const T* vb, const IT* a, const IT* PQ, T* ab, T* PQb,
                        cudaStream_t st, __nv_bfloat16* ab16) {
   if (N == 0) return 0;
+  if constexpr (std::is_same<T, float>::value) {
+    update_bwd1_4_k<IT><<<nblk(N * (F / 4), 256), 256, 0, st>>>(N, F, sb, vb, a, PQ, ab, PQb, ab16); PNN_KCHECK("update_bwd1_4_k");
+    return 1;
+  }
   update_bwd1_k<T, IT><<<nblk(N * F, 256), 256, 0, st>>>(N, F, sb, vb, a, PQ, ab, PQb, ab16); PNN_KCHECK("update_bwd1_k");
   return 1;
 }
@@ -509,6 +591,10 @@ template <typename T, typename IT>
 int launch_update_bwd2(int64_t N, int F, const T* zb, const IT* PQ, T eps, T* sb, T* PQb, cudaStream_t st,
                        __nv_bfloat16* PQb16, __nv_bfloat16* sb16) {
   if (N == 0) return 0;
+  if constexpr (std::is_same<T, float>::value) {
+    update_bwd2_4_k<IT><<<nblk(N * (F / 4), 256), 256, 0, st>>>(N, F, zb, PQ, eps, sb, PQb, PQb16, sb16); PNN_KCHECK("update_bwd2_4_k");
+    return 1;
+  }
   update_bwd2_k<T, IT><<<nblk(N * F, 256), 256, 0, st>>>(N, F, zb, PQ, eps, sb, PQb, PQb16, sb16); PNN_KCHECK("update_bwd2_k");
   return 1;
 }
