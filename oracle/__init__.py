@@ -148,3 +148,31 @@ def forces_dual(mc, weights, batch):
                            _p(cell, ctypes.c_double), _p(pbc, ctypes.c_uint8), _p(head, ctypes.c_int32),
                            _p(frc, ctypes.c_double))
     return frc
+
+
+def evaluate_blended(mc, weights, batch, head_weights, forces: bool = True, skip_below: float = 0.0):
+    """Blended multi-head evaluation of the paper's inference pipeline (Fig. 5 at :420): every
+    structure g gets E_g = sum_h w[g,h] E_g^(h), F = -dE/dx, where E^(h) is the energy with head h applied to the shared
+    trunk and w [S,H] are the per-structure branch weights (in the paper a softmax over a composition MLP; here an input).
+    Heads with w[g,h] < skip_below are dropped for that structure ("branch skipping").
+
+    Written as its definition: H single-head evaluations of the oracle above, combined linearly.  Slow on purpose."""
+    import dataclasses
+    hw = np.asarray(head_weights, np.float64)
+    S = batch.head.shape[0]
+    assert hw.shape == (S, mc.H)
+    hw = np.where(hw < skip_below, 0.0, hw)
+    energy = np.zeros(S, np.float64)
+    frc = np.zeros((batch.Z.shape[0], 3), np.float64) if forces else None
+    sof = np.repeat(np.arange(S), np.diff(batch.struct_ptr))
+    n_edges = 0
+    for h in range(mc.H):
+        if not np.any(hw[:, h] != 0.0):
+            continue
+        bh = dataclasses.replace(batch, head=np.full(S, h, np.int32))
+        out = evaluate(mc, weights, bh, forces=forces)
+        n_edges = out["n_edges"]
+        energy += hw[:, h] * out["energy"]
+        if forces:
+            frc += hw[sof, h][:, None] * out["forces"]
+    return dict(energy=energy, forces=frc, n_edges=n_edges)
