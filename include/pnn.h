@@ -110,6 +110,16 @@ int pnn_eval(const pnn_model* m, pnn_workspace* ws, int64_t n_atoms, int64_t n_s
              const double* pos, const int32_t* struct_ptr, const int32_t* head, int flags, void* energy,
              void* forces, void* cuda_stream);
 
+/* Blended multi-head evaluation — the paper's inference pipeline (PAPER.md:166-168 branch weights, :371-373 "encoder
+ * reuse", "branch skipping", "fused gradient", Fig. 5 at :420): the shared trunk runs ONCE, every
+ * structure g is read out by all heads h with head_weights[g][h] >= skip_below, E_g = sum_h w[g][h] E_g^(h), and ONE
+ * reverse sweep gives forces = -dE/dx of that blended energy.  head_weights DEVICE [S,H], f64 for a PNN_FP64 model, f32
+ * otherwise (in the paper: a softmax over a composition MLP; here an input).  Other arguments, graph requirement and
+ * error behaviour as pnn_eval.  Asynchronous. */
+int pnn_eval_blended(const pnn_model* m, pnn_workspace* ws, int64_t n_atoms, int64_t n_structs, const int32_t* Z,
+                     const double* pos, const int32_t* struct_ptr, const void* head_weights, double skip_below,
+                     int flags, void* energy, void* forces, void* cuda_stream);
+
 /* Convenience for callers with HOST buffers (bench.py's e2e leg): copies Z, pos, struct_ptr, head (and cell /
  * pbc when not NULL) to the device, runs pnn_build_graph + pnn_eval and copies energy [S] / forces [N,3] back.
  * energy_host / forces_host have the dtype pnn_eval documents.  Synchronous. */

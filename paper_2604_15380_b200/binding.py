@@ -16,7 +16,7 @@ __all__ = [
     "PNN_OK", "PNN_BF16", "PNN_FP32", "PNN_FP64", "PNN_ENERGY", "PNN_FORCES", "PnnError", "pnn_config", "lib",
     "lib_path", "pnn_status_string", "pnn_last_cuda_error", "pnn_weights_count", "pnn_model_create",
     "pnn_model_destroy", "pnn_workspace_create", "pnn_workspace_destroy", "pnn_workspace_bytes", "pnn_build_graph",
-    "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_eval_host", "pnn_check_async_errors", "pnn_launch_count", "pnn_profile_enable",
+    "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_eval_blended", "pnn_eval_host", "pnn_check_async_errors", "pnn_launch_count", "pnn_profile_enable",
     "pnn_profile_read", "pnn_gemm_bf16",
     "PaiNN", "PRECISIONS",
 ]
@@ -77,6 +77,7 @@ def lib():
                                      ctypes.POINTER(i64)]
         L.pnn_graph_copy.argtypes = [vp, vp, vp, vp]
         L.pnn_eval.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, i32, vp, vp, vp]
+        L.pnn_eval_blended.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, ctypes.c_double, i32, vp, vp, vp]
         L.pnn_eval_host.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp]
         L.pnn_check_async_errors.argtypes = [vp]
         L.pnn_profile_enable.argtypes = [vp, i32]
@@ -167,6 +168,13 @@ def pnn_eval(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, struct_p
              forces=None, stream=None):
     _check(lib().pnn_eval(model, ws, n_atoms, n_structs, _ptr(Z), _ptr(pos), _ptr(struct_ptr), _ptr(head), flags,
                           _ptr(energy), _ptr(forces), stream), "pnn_eval")
+
+
+def pnn_eval_blended(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, struct_ptr, head_weights,
+                     skip_below: float, flags: int, energy, forces=None, stream=None):
+    _check(lib().pnn_eval_blended(model, ws, n_atoms, n_structs, _ptr(Z), _ptr(pos), _ptr(struct_ptr),
+                                  _ptr(head_weights), float(skip_below), flags, _ptr(energy), _ptr(forces), stream),
+           "pnn_eval_blended")
 
 
 def pnn_eval_host(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, struct_ptr, head, cell, pbc,
@@ -278,6 +286,22 @@ class PaiNN:
         frc = torch.empty((N, 3), dtype=self.out_dtype, device=pos.device) if forces else None
         flags = PNN_ENERGY | (PNN_FORCES if forces else 0)
         pnn_eval(self.model, self.ws, N, S, Z, pos, struct_ptr, head, flags, energy, frc, self._stream())
+        return energy, frc
+
+    def eval_blended(self, Z, pos, struct_ptr, head_weights, cell=None, pbc=None, forces: Optional[bool] = None,
+                     skip_below: float = 0.0, build: bool = True):
+        """Blended multi-head evaluation: head_weights [S,H] CUDA tensor in the model's output dtype."""
+        import torch
+        forces = self.want_forces if forces is None else forces
+        N, S = int(Z.shape[0]), int(head_weights.shape[0])
+        self._last_N = N
+        if build:
+            self.build_graph(pos, struct_ptr, cell, pbc)
+        energy = torch.empty(S, dtype=self.out_dtype, device=pos.device)
+        frc = torch.empty((N, 3), dtype=self.out_dtype, device=pos.device) if forces else None
+        flags = PNN_ENERGY | (PNN_FORCES if forces else 0)
+        pnn_eval_blended(self.model, self.ws, N, S, Z, pos, struct_ptr, head_weights, skip_below, flags, energy, frc,
+                         self._stream())
         return energy, frc
 
     def eval_host(self, Z, pos, struct_ptr, head, cell=None, pbc=None, forces: Optional[bool] = None,

@@ -160,6 +160,14 @@ template <typename T>
 int launch_readout(int64_t N, int64_t S, int F, int H, const T* s, const int32_t* a2s, const int32_t* head,
                    const int32_t* struct_ptr, const T* W1t, const T* b1, const T* w2, const T* b2, T* opre, T* eatom,
                    T* energy, int* d_err, cudaStream_t st);
+// blended multi-head readout: hw [S][H] branch weights, heads with hw < thr skipped; opre_all [N][H][F/2]
+template <typename T>
+int launch_readout_blend(int64_t N, int64_t S, int F, int H, const T* s, const int32_t* a2s, const T* hw, T thr,
+                         const int32_t* struct_ptr, const T* W1t, const T* b1, const T* w2, const T* b2, T* opre_all,
+                         T* eatom, T* energy, cudaStream_t st);
+template <typename T>
+int launch_readout_blend_bwd(int64_t N, int F, int H, const T* opre_all, const int32_t* a2s, const T* hw, T thr,
+                             const T* W1, const T* w2, T* sb, cudaStream_t st);
 template <typename T>
 int launch_struct_sum(int64_t S, const int32_t* struct_ptr, const T* eatom, T* energy, cudaStream_t st);
 template <typename T>

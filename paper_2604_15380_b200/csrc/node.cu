@@ -472,6 +472,122 @@ __global__ void __launch_bounds__(512) readout_bwd2_k(int64_t N, int F, int H, c
   }
 }
 
+// ---- blended multi-head readout (Fig. 5): every atom is read out by
+// ALL heads whose branch weight w[g,h] for its structure g is >= thr ("branch skipping"), eatom_i = sum_h w[g,h] eps_i^h.
+// Same thread mapping as readout2_k; the two rows of a thread share the head inside the h loop, so one weight vector
+// serves both.  opre_all [N][H][Fh] keeps the pre-activations of the evaluated heads for the reverse sweep.
+template <typename T>
+__global__ void __launch_bounds__(256) readout_blend_k(int64_t N, int F, int H, const T* __restrict__ s,
+                                                       const int32_t* __restrict__ a2s, const T* __restrict__ hw, T thr,
+                                                       const T* __restrict__ W1t, const T* __restrict__ b1,
+                                                       const T* __restrict__ w2, const T* __restrict__ b2,
+                                                       T* __restrict__ opre_all, T* __restrict__ eatom) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int Fh = F / 2, NOG = Fh / 4;
+  T* S = reinterpret_cast<T*>(smem_raw);  // [RT][F]
+  T* Ep = S + RT * F;                     // [RT][NOG]
+  __shared__ int Gs[RT];
+  const int64_t i0 = (int64_t)blockIdx.x * RT;
+  const int nt = (int)min((int64_t)RT, N - i0);
+  for (int q = threadIdx.x; q < RT * F; q += blockDim.x) S[q] = (q < nt * F) ? s[i0 * F + q] : T(0);
+  if (threadIdx.x < RT) Gs[threadIdx.x] = threadIdx.x < nt ? a2s[i0 + threadIdx.x] : -1;
+  __syncthreads();
+  const int og = threadIdx.x % NOG, rg = threadIdx.x / NOG;
+  const int g0 = Gs[rg], g1 = Gs[rg + 8];
+  T e0 = T(0), e1 = T(0);
+  for (int h = 0; h < H; ++h) {
+    T w0 = g0 >= 0 ? hw[(int64_t)g0 * H + h] : T(0), w1 = g1 >= 0 ? hw[(int64_t)g1 * H + h] : T(0);
+    if (w0 < thr) w0 = T(0);
+    if (w1 < thr) w1 = T(0);
+    if (w0 == T(0) && w1 == T(0)) continue;
+    const T* Wp = W1t + (int64_t)h * F * Fh + og * 4;
+    T acc0[4] = {T(0), T(0), T(0), T(0)}, acc1[4] = {T(0), T(0), T(0), T(0)};
+#pragma unroll 4
+    for (int k = 0; k < F; ++k) {
+      T wa[4];
+      Vec4<T>::ld(Wp + (int64_t)k * Fh, wa);
+      const T x0 = S[rg * F + k], x1 = S[(rg + 8) * F + k];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { acc0[j] = fma(wa[j], x0, acc0[j]); acc1[j] = fma(wa[j], x1, acc1[j]); }
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int o = og * 4 + j;
+      const T bb = b1[h * Fh + o], ww = w2[h * Fh + o];
+      const T p0 = acc0[j] + bb, p1 = acc1[j] + bb;
+      if (w0 != T(0)) {
+        if (opre_all) opre_all[((i0 + rg) * H + h) * Fh + o] = p0;
+        e0 = fma(w0 * ww, silu_f<T>(p0), e0);
+      }
+      if (w1 != T(0)) {
+        if (opre_all) opre_all[((i0 + rg + 8) * H + h) * Fh + o] = p1;
+        e1 = fma(w1 * ww, silu_f<T>(p1), e1);
+      }
+    }
+  }
+  Ep[rg * NOG + og] = e0;
+  Ep[(rg + 8) * NOG + og] = e1;
+  __syncthreads();
+  if (threadIdx.x < nt) {
+    T e = T(0);
+    for (int q = 0; q < NOG; ++q) e += Ep[threadIdx.x * NOG + q];
+    const int g = Gs[threadIdx.x];
+    for (int h = 0; h < H; ++h) {
+      const T w = hw[(int64_t)g * H + h];
+      if (!(w < thr)) e = fma(w, b2[h], e);
+    }
+    eatom[i0 + threadIdx.x] = e;
+  }
+}
+
+// R1 of the blended readout: s-bar_i = sum_h w[g,h] out_W1^{hT} (out_w2^h o silu'(pre_i^h)) over the evaluated heads.
+template <typename T>
+__global__ void __launch_bounds__(512) readout_blend_bwd_k(int64_t N, int F, int H, const T* __restrict__ opre_all,
+                                                           const int32_t* __restrict__ a2s, const T* __restrict__ hw,
+                                                           T thr, const T* __restrict__ W1, const T* __restrict__ w2,
+                                                           T* __restrict__ sb) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int Fh = F / 2, NKG = F / 4;
+  T* Pb = reinterpret_cast<T*>(smem_raw); // [RT][Fh]  w[g,h] w2 o silu'(pre) of the current head
+  __shared__ int Gs[RT];
+  const int64_t i0 = (int64_t)blockIdx.x * RT;
+  const int nt = (int)min((int64_t)RT, N - i0);
+  if (threadIdx.x < RT) Gs[threadIdx.x] = threadIdx.x < nt ? a2s[i0 + threadIdx.x] : -1;
+  __syncthreads();
+  const int kg = threadIdx.x % NKG, rg = threadIdx.x / NKG;
+  T acc0[4] = {T(0), T(0), T(0), T(0)}, acc1[4] = {T(0), T(0), T(0), T(0)};
+  for (int h = 0; h < H; ++h) {
+    bool any = false; // tile-uniform: every thread scans the 16 rows
+    for (int r = 0; r < nt; ++r) any = any || !(hw[(int64_t)Gs[r] * H + h] < thr);
+    if (!any) continue;
+    __syncthreads();
+    for (int q = threadIdx.x; q < RT * Fh; q += blockDim.x) {
+      const int r = q / Fh, o = q % Fh;
+      T p = T(0);
+      if (r < nt) {
+        const T w = hw[(int64_t)Gs[r] * H + h];
+        if (!(w < thr)) p = w * w2[h * Fh + o] * dsilu_f<T>(opre_all[((i0 + r) * H + h) * Fh + o]);
+      }
+      Pb[q] = p;
+    }
+    __syncthreads();
+    const T* Wp = W1 + (int64_t)h * Fh * F + kg * 4;
+#pragma unroll 4
+    for (int o = 0; o < Fh; ++o) {
+      T wa[4];
+      Vec4<T>::ld(Wp + (int64_t)o * F, wa);
+      const T p0 = Pb[rg * Fh + o], p1 = Pb[(rg + 8) * Fh + o];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { acc0[j] = fma(wa[j], p0, acc0[j]); acc1[j] = fma(wa[j], p1, acc1[j]); }
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    if (rg < nt) sb[(i0 + rg) * F + kg * 4 + j] = acc0[j];
+    if (rg + 8 < nt) sb[(i0 + rg + 8) * F + kg * 4 + j] = acc1[j];
+  }
+}
+
 // E_g = sum of the structure's atom energies (segmented sum, fixed tree order)
 template <typename T>
 __global__ void __launch_bounds__(128) struct_sum_k(const int32_t* __restrict__ sptr, const T* __restrict__ eatom,
@@ -627,6 +743,34 @@ int launch_readout(int64_t N, int64_t S, int F, int H, const T* s, const int32_t
   return nl;
 }
 template <typename T>
+int launch_readout_blend(int64_t N, int64_t S, int F, int H, const T* s, const int32_t* a2s, const T* hw, T thr,
+                         const int32_t* struct_ptr, const T* W1t, const T* b1, const T* w2, const T* b2, T* opre_all,
+                         T* eatom, T* energy, cudaStream_t st) {
+  int nl = 0;
+  if (N > 0) {
+    const size_t smem = sizeof(T) * (RT * F + RT * (F / 8));
+    static bool attr = false;
+    if (!attr) { cudaFuncSetAttribute(readout_blend_k<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024); attr = true; }
+    readout_blend_k<T><<<nblk(N, RT), 8 * (F / 8), smem, st>>>(N, F, H, s, a2s, hw, thr, W1t, b1, w2, b2, opre_all, eatom);
+    PNN_KCHECK("readout_blend_k");
+    ++nl;
+  }
+  if (S > 0) {
+    struct_sum_k<T><<<(unsigned)S, 128, 0, st>>>(struct_ptr, eatom, energy); PNN_KCHECK("struct_sum_k");
+    ++nl;
+  }
+  return nl;
+}
+template <typename T>
+int launch_readout_blend_bwd(int64_t N, int F, int H, const T* opre_all, const int32_t* a2s, const T* hw, T thr,
+                             const T* W1, const T* w2, T* sb, cudaStream_t st) {
+  if (N == 0) return 0;
+  const size_t smem = sizeof(T) * (RT * (F / 2));
+  readout_blend_bwd_k<T><<<nblk(N, RT), 8 * (F / 4), smem, st>>>(N, F, H, opre_all, a2s, hw, thr, W1, w2, sb);
+  PNN_KCHECK("readout_blend_bwd_k");
+  return 1;
+}
+template <typename T>
 int launch_struct_sum(int64_t S, const int32_t* struct_ptr, const T* eatom, T* energy, cudaStream_t st) {
   if (S <= 0) return 0;
   struct_sum_k<T><<<(unsigned)S, 128, 0, st>>>(struct_ptr, eatom, energy); PNN_KCHECK("struct_sum_k");
@@ -658,6 +802,11 @@ int launch_force_assemble(int64_t N, int nslab, const T* fpart, T* forces, cudaS
                                  const int32_t*, const T*, const T*, const T*, const T*, T*, T*, T*, int*,           \
                                  cudaStream_t);                                                                      \
   template int launch_struct_sum<T>(int64_t, const int32_t*, const T*, T*, cudaStream_t);                            \
+  template int launch_readout_blend<T>(int64_t, int64_t, int, int, const T*, const int32_t*, const T*, T,            \
+                                       const int32_t*, const T*, const T*, const T*, const T*, T*, T*, T*,           \
+                                       cudaStream_t);                                                                \
+  template int launch_readout_blend_bwd<T>(int64_t, int, int, const T*, const int32_t*, const T*, T, const T*,       \
+                                           const T*, T*, cudaStream_t);                                              \
   template int launch_readout_bwd<T>(int64_t, int, int, const T*, const int32_t*, const int32_t*, const T*,          \
                                      const T*, T*, cudaStream_t);                                                    \
   template int launch_force_assemble<T>(int64_t, int, const T*, T*, cudaStream_t);

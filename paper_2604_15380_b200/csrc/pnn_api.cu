@@ -99,6 +99,7 @@ struct pnn_workspace {
   int64_t launches = 0;
   // activations (element type = model state type)
   void *s_cur, *h, *sn, *v1, *k, *vping[2], *eatom, *opre;
+  void* opre_all = nullptr; // blended readout: pre-activations of every head [N][H][F/2] (reverse sweep)
   struct Tape { void *v_in, *hpre, *phi, *PQ, *kpre, *a; };
   std::vector<Tape> tape;
   // adjoints
@@ -327,6 +328,7 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
     ws->tape.resize(want_forces ? T : 1);
     if (want_forces) {
       ws->opre = carve(es * N * (F / 2));
+      ws->opre_all = carve(es * N * m->cfg.H * (F / 2));
       for (int t = 0; t < T; ++t) {
         pnn_workspace::Tape& tp = ws->tape[t];
         tp.v_in = (t == 0) ? nullptr : carve(es * N * 3 * F);
@@ -520,7 +522,7 @@ namespace {
 
 template <typename T>
 int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const int32_t* sptr,
-              const int32_t* head, int flags, T* energy, T* forces, cudaStream_t st) {
+              const int32_t* head, const T* hw, double skip_below, int flags, T* energy, T* forces, cudaStream_t st) {
   const pnn_config& c = m->cfg;
   const int F = c.F, T_ = c.T;
   const bool want_f = (flags & PNN_FORCES) != 0;
@@ -589,14 +591,19 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       nl += l_; ps_.done(l_); }
   }
   { ProfScope ps_(ws, st, "readout");
-  const int l_ = launch_readout<T>(N, S, F, c.H, s_cur, ws->g.a2s, head, sptr, W + m->oW1t, W + m->ob1, W + m->ow2,
+  const int l_ = hw ? launch_readout_blend<T>(N, S, F, c.H, s_cur, ws->g.a2s, hw, (T)skip_below, sptr, W + m->oW1t,
+                                               W + m->ob1, W + m->ow2, W + m->ob2, (T*)ws->opre_all, (T*)ws->eatom,
+                                               energy, st)
+                    : launch_readout<T>(N, S, F, c.H, s_cur, ws->g.a2s, head, sptr, W + m->oW1t, W + m->ob1, W + m->ow2,
                           W + m->ob2, (T*)ws->opre, (T*)ws->eatom, energy, ws->g.d_err, st);
     nl += l_; ps_.done(l_); }
   if (want_f) {
     T* sb = (T*)ws->sb; T* vb = (T*)ws->vb; T* vb2 = (T*)ws->vb2; T* ab = (T*)ws->ab; T* PQb = (T*)ws->PQb;
     T* kb = (T*)ws->kb; T* zb = (T*)ws->zb; T* phib = (T*)ws->phib; T* hb = (T*)ws->hb; T* fpart = (T*)ws->fpart;
     { ProfScope ps_(ws, st, "readout_bwd");
-    const int l_ = launch_readout_bwd<T>(N, F, c.H, (const T*)ws->opre, ws->g.a2s, head, W + m->oW1, W + m->ow2, sb, st); // R1
+    const int l_ = hw ? launch_readout_blend_bwd<T>(N, F, c.H, (const T*)ws->opre_all, ws->g.a2s, hw, (T)skip_below,
+                                                     W + m->oW1, W + m->ow2, sb, st)
+                      : launch_readout_bwd<T>(N, F, c.H, (const T*)ws->opre, ws->g.a2s, head, W + m->oW1, W + m->ow2, sb, st); // R1
       nl += l_; ps_.done(l_); }
     for (int t = T_ - 1; t >= 0; --t) {
       const BlockW& b = m->blk[t];
@@ -665,7 +672,8 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
 // accumulation (gemm_tc.cu); the gathered sender payloads phi_j, v_j are BF16; geometry, radial basis, cutoff,
 // segment sums, the residual streams s, v, the adjoint streams, energies and forces stay FP32.
 int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const int32_t* sptr,
-              const int32_t* head, int flags, float* energy, float* forces, cudaStream_t st) {
+              const int32_t* head, const float* hw, double skip_below, int flags, float* energy, float* forces,
+              cudaStream_t st) {
   typedef float T;
   typedef __nv_bfloat16 B;
   const pnn_config& c = m->cfg;
@@ -737,17 +745,25 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       nl += l_; ps_.done(l_); }
   }
   { ProfScope ps_(ws, st, "readout");   // B5: all heads as one tensor-core GEMM, rows filtered by head in the epilogue
-    int l_ = launch_readout_tc(N, F, c.H, mb.s16, Wb + m->oW1, W + m->ob1, W + m->ow2, W + m->ob2, ws->g.a2s, head,
+    int l_;
+    if (hw) { // blended heads: FP32 readout of the FP32 residual stream (one structure may need every head)
+      l_ = launch_readout_blend<T>(N, S, F, c.H, s_cur, ws->g.a2s, hw, (T)skip_below, sptr, W + m->oW1t, W + m->ob1,
+                                   W + m->ow2, W + m->ob2, (T*)ws->opre_all, (T*)ws->eatom, energy, st);
+    } else {
+    l_ = launch_readout_tc(N, F, c.H, mb.s16, Wb + m->oW1, W + m->ob1, W + m->ow2, W + m->ob2, ws->g.a2s, head,
                                (T*)ws->opre, (T*)ws->eatom, ws->g.d_err, st);
     if (l_ >= 0) l_ += launch_struct_sum<T>(S, sptr, (const T*)ws->eatom, energy, st);
     else l_ = launch_readout<T>(N, S, F, c.H, s_cur, ws->g.a2s, head, sptr, W + m->oW1t, W + m->ob1, W + m->ow2,
                                 W + m->ob2, (T*)ws->opre, (T*)ws->eatom, energy, ws->g.d_err, st);
+    }
     nl += l_; ps_.done(l_); }
   if (want_f) {
     T* sb = (T*)ws->sb; T* vb = (T*)ws->vb; T* vb2 = (T*)ws->vb2; T* PQb = (T*)ws->PQb; T* zb = (T*)ws->zb;
     T* fpart = (T*)ws->fpart;
     { ProfScope ps_(ws, st, "readout_bwd");
-      const int l_ = launch_readout_bwd<T>(N, F, c.H, (const T*)ws->opre, ws->g.a2s, head, W + m->oW1, W + m->ow2, sb, st);
+      const int l_ = hw ? launch_readout_blend_bwd<T>(N, F, c.H, (const T*)ws->opre_all, ws->g.a2s, hw, (T)skip_below,
+                                                       W + m->oW1, W + m->ow2, sb, st)
+                        : launch_readout_bwd<T>(N, F, c.H, (const T*)ws->opre, ws->g.a2s, head, W + m->oW1, W + m->ow2, sb, st);
       nl += l_; ps_.done(l_); }
     for (int t = T_ - 1; t >= 0; --t) {
       const BlockW& b = m->blk[t];
@@ -795,27 +811,45 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
 
 extern "C" {
 
-int pnn_eval(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const double* pos,
-             const int32_t* sptr, const int32_t* head, int flags, void* energy, void* forces, void* stream) {
-  (void)pos;
+static int eval_common(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z,
+                       const int32_t* sptr, const int32_t* head, const void* head_w, double skip_below, int flags,
+                       void* energy, void* forces, void* stream) {
   if (!m || !ws || ws->model != m || N < 0 || S < 0) return PNN_ERR_INVALID_ARG;
   if (!(flags & (PNN_ENERGY | PNN_FORCES))) return PNN_ERR_INVALID_ARG;
   if (N > ws->maxN || S > ws->maxS) return PNN_ERR_CAPACITY;
-  if ((N > 0 && !Z) || !sptr || (S > 0 && (!head || !energy))) return PNN_ERR_INVALID_ARG;
+  if ((N > 0 && !Z) || !sptr || (S > 0 && ((!head && !head_w) || !energy))) return PNN_ERR_INVALID_ARG;
   if ((flags & PNN_FORCES) && (!ws->want_forces || (N > 0 && !forces))) return PNN_ERR_INVALID_ARG;
   if (ws->graph_N != N || ws->graph_S != S) return PNN_ERR_NO_GRAPH;
   cudaStream_t st = (cudaStream_t)stream;
   int rc;
   if (m->cfg.prec == PNN_FP64)
-    rc = eval_simt<double>(m, ws, N, S, Z, sptr, head, flags, (double*)energy, (double*)forces, st);
+    rc = eval_simt<double>(m, ws, N, S, Z, sptr, head, (const double*)head_w, skip_below, flags, (double*)energy,
+                           (double*)forces, st);
   else if (m->cfg.prec == PNN_FP32)
-    rc = eval_simt<float>(m, ws, N, S, Z, sptr, head, flags, (float*)energy, (float*)forces, st);
+    rc = eval_simt<float>(m, ws, N, S, Z, sptr, head, (const float*)head_w, skip_below, flags, (float*)energy,
+                          (float*)forces, st);
   else
-    rc = eval_bf16(m, ws, N, S, Z, sptr, head, flags, (float*)energy, (float*)forces, st);
+    rc = eval_bf16(m, ws, N, S, Z, sptr, head, (const float*)head_w, skip_below, flags, (float*)energy, (float*)forces, st);
   if (rc != PNN_OK) return rc;
   if (launch_failed()) return PNN_ERR_CUDA;
   PNN_TRY(cudaGetLastError());
   return PNN_OK;
+}
+
+int pnn_eval(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const double* pos,
+             const int32_t* sptr, const int32_t* head, int flags, void* energy, void* forces, void* stream) {
+  (void)pos;
+  if (S > 0 && !head) return PNN_ERR_INVALID_ARG;
+  return eval_common(m, ws, N, S, Z, sptr, head, nullptr, 0.0, flags, energy, forces, stream);
+}
+
+int pnn_eval_blended(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const double* pos,
+                     const int32_t* sptr, const void* head_weights, double skip_below, int flags, void* energy,
+                     void* forces, void* stream) {
+  (void)pos;
+  if (S > 0 && !head_weights) return PNN_ERR_INVALID_ARG;
+  if ((flags & PNN_FORCES) && ws && !ws->opre_all) return PNN_ERR_INVALID_ARG;
+  return eval_common(m, ws, N, S, Z, sptr, nullptr, head_weights, skip_below, flags, energy, forces, stream);
 }
 
 int pnn_eval_host(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const double* pos,
