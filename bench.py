@@ -27,6 +27,8 @@ WORKLOADS = {
     "cfg1": (1, "fp64", True, None),
     "cfg2": (2, "fp32", True, None),
     "cfg2_fp64": (2, "fp64", True, None),
+    # blended multi-head inference (Fig. 5): all 16 heads weighted per structure, branches below 0.01 skipped
+    "cfg2_blended": (2, "fp32", True, None),
     "cfg3_fp32": (3, "fp32", True, None),
     "cfg3_bf16": (3, "bf16", True, None),
     "cfg4": (4, "bf16", False, 16384),
@@ -34,6 +36,7 @@ WORKLOADS = {
     "cfg5": (5, "fp64", True, None),
 }
 WORKLOAD_NAMES = {"cfg1": "cfg1_tiny_fp64", "cfg2": "cfg2_molecular_fp32", "cfg2_fp64": "cfg2_molecular_fp64",
+                  "cfg2_blended": "cfg2_molecular_fp32_blended_heads",
                   "cfg3_fp32": "cfg3_crystals_fp32", "cfg3_bf16": "cfg3_crystals_bf16",
                   "cfg4": "cfg4_screening_bf16_batch16384", "cfg4_fp32": "cfg4_screening_fp32_batch16384",
                   "cfg5": "cfg5_large_fp64"}
@@ -214,7 +217,15 @@ def main():
         flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)  # 256 MB > 126 MB L2
         st = torch.cuda.current_stream()
 
+        blended = name.endswith("_blended")
+        if blended:
+            hw = gen.make_head_weights(cfg_id, np.arange(rank * S, rank * S + b.n_structs), mc.H)
+            d["hw"] = torch.from_numpy(hw).to(torch.float64 if prec == "fp64" else torch.float32).to(dev)
+
         def step():
+            if blended:
+                return net.eval_blended(d["Z"], d["pos"], d["sp"], d["hw"], d["cell"], d["pbc"], forces=forces,
+                                        skip_below=0.01)
             return net.eval(d["Z"], d["pos"], d["sp"], d["head"], d["cell"], d["pbc"], forces=forces)
 
         for _ in range(warmup):
@@ -359,7 +370,7 @@ def main():
 
     if not args.no_extra and world == 1:
         extra = {}
-        for name in ("cfg1", "cfg3_fp32", "cfg3_bf16", "cfg4", "cfg5"):
+        for name in ("cfg1", "cfg2_blended", "cfg3_fp32", "cfg3_bf16", "cfg4", "cfg5"):
             if name == args.workload:
                 continue
             try:

@@ -14,6 +14,7 @@ from .synth import (  # noqa: F401
     weights_count,
     weights_layout,
     make_weights,
+    make_head_weights,
     make_batch,
     make_molecules,
     make_crystals,

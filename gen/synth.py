@@ -27,7 +27,7 @@ _M2 = np.uint64(0x94D049BB133111EB)
 _GOLD = np.uint64(0x9E3779B97F4A7C15)
 
 # purpose tags (arbitrary distinct constants)
-_T_NATOMS, _T_HEAD, _T_POS, _T_Z, _T_SHUF, _T_JIT, _T_W = 11, 12, 13, 14, 15, 16, 17
+_T_NATOMS, _T_HEAD, _T_POS, _T_Z, _T_SHUF, _T_JIT, _T_W, _T_HW = 11, 12, 13, 14, 15, 16, 17, 18
 
 MARGIN = 1e-9
 
@@ -172,6 +172,17 @@ def make_weights(mc: ModelCfg, cfg_id: int = 0, seed: int = BASE_SEED) -> np.nda
         z = _normal(seed, cfg_id, _T_W, tid, np.arange(n, dtype=np.uint64))
         blob[off:off + n] = z / math.sqrt(fan_in)
     return blob
+
+
+def make_head_weights(cfg_id: int, struct_ids, H: int, sharpness: float = 6.0, seed: int = BASE_SEED) -> np.ndarray:
+    """Per-structure branch weights [S,H] for blended multi-head inference: a softmax of seeded normal logits scaled by
+    `sharpness`, rounded to 6 decimals.  Stands in for the paper's composition-MLP softmax, which on
+    real inputs leaves ~81 % of the branches negligible; the default sharpness gives a similar share."""
+    ids = np.asarray(struct_ids, np.uint64)
+    z = np.stack([_normal(seed, cfg_id, _T_HW, ids, np.full(ids.shape, h, np.uint64)) for h in range(H)], axis=1)
+    z = sharpness * z
+    e = np.exp(z - z.max(axis=1, keepdims=True))
+    return np.round(e / e.sum(axis=1, keepdims=True), 6)
 
 
 def unpack_weights(mc: ModelCfg, blob: np.ndarray) -> dict:
