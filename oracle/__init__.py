@@ -48,7 +48,8 @@ def _p(a, ct):
 
 
 def _cfg_arrays(mc):
-    ic = np.array([mc.F, mc.T, mc.K, mc.H, mc.Zmax], np.int32)
+    rbf = {"gaussian": 0, "bessel": 1}[getattr(mc, "rbf", "gaussian")]
+    ic = np.array([mc.F, mc.T, mc.K, mc.H, mc.Zmax, rbf], np.int32)
     dc = np.array([mc.cutoff, mc.norm_eps], np.float64)
     return ic, dc
 
@@ -71,6 +72,17 @@ def rbf_cutoff(d: float, K: int, rc: float):
     c = np.zeros(1, np.float64)
     lib.oracle_rbf_cutoff(ctypes.c_double(d), ctypes.c_int32(K), ctypes.c_double(rc), _p(g, ctypes.c_double),
                           _p(c, ctypes.c_double))
+    return g, float(c[0])
+
+
+def rbf_cutoff_typed(d: float, K: int, rc: float, rbf: str):
+    """(g_k(d) [K], c(d)) for the named radial basis ("gaussian" or "bessel")."""
+    lib = _load()
+    g = np.zeros(K, np.float64)
+    c = np.zeros(1, np.float64)
+    lib.oracle_rbf_cutoff_typed(ctypes.c_double(d), ctypes.c_int32(K), ctypes.c_double(rc),
+                                ctypes.c_int32({"gaussian": 0, "bessel": 1}[rbf]), _p(g, ctypes.c_double),
+                                _p(c, ctypes.c_double))
     return g, float(c[0])
 
 

@@ -49,14 +49,16 @@ inline Dual& operator+=(Dual& a, Dual b) { a = a + b; return a; }
 inline Dual s_exp(Dual a) { double e = std::exp(a.v); return Dual(e, e * a.d); }
 inline Dual s_sqrt(Dual a) { double r = std::sqrt(a.v); return Dual(r, a.d / (2.0 * r)); }
 inline Dual s_cos(Dual a) { return Dual(std::cos(a.v), -std::sin(a.v) * a.d); }
+inline Dual s_sin(Dual a) { return Dual(std::sin(a.v), std::cos(a.v) * a.d); }
 inline double s_exp(double a) { return std::exp(a); }
 inline double s_sqrt(double a) { return std::sqrt(a); }
 inline double s_cos(double a) { return std::cos(a); }
+inline double s_sin(double a) { return std::sin(a); }
 inline double value_of(double a) { return a; }
 inline double value_of(Dual a) { return a.v; }
 
 // ------------------------------------------------------------------ model = views into the blob
-struct Cfg { int F, T, K, H, Zmax; double rc, eps; };
+struct Cfg { int F, T, K, H, Zmax; double rc, eps; int rbf; };  // rbf: 0 Gaussian, 1 Bessel
 struct Block {
   const double *msg_W1, *msg_b1, *msg_W2, *msg_b2, *flt_W, *flt_b;
   const double *upd_U, *upd_V, *upd_A1, *upd_c1, *upd_A2, *upd_c2;
@@ -146,7 +148,10 @@ template <class S> inline S silu(S x) { return x / (S(1.0) + s_exp(-x)); }      
 inline double dsilu(double x) { const double sg = 1.0 / (1.0 + std::exp(-x)); return sg * (1.0 + x * (1.0 - sg)); }
 
 // Gaussian radial basis (Q2): centres mu_k = k rc/(K-1), gamma = 1/(2 dmu^2), dmu = rc/(K-1).
-template <class S> inline S rbf(S d, int k, int K, double rc) {
+// Bessel radial basis (the paper's lead model, "4 (Bessel)"; type 1): the zeroth-order spherical Bessel
+// functions b_n(d) = sqrt(2/rc) sin(n pi d / rc) / d, n = k + 1 = 1..K, orthonormal on [0, rc] with weight d^2.
+template <class S> inline S rbf(S d, int k, int K, double rc, int type = 0) {
+  if (type == 1) return S(std::sqrt(2.0 / rc)) * s_sin(S((k + 1) * M_PI / rc) * d) / d;
   const double dmu = (K > 1) ? rc / (K - 1) : rc;
   const double gamma = 1.0 / (2.0 * dmu * dmu), mu = k * dmu;
   return s_exp(S(-gamma) * (d - S(mu)) * (d - S(mu)));
@@ -227,7 +232,7 @@ void forward(const Model& m, int N, int nS, const int32_t* Z, const S* pos, cons
       for (int e = ed.rowptr[i]; e < ed.rowptr[i + 1]; ++e) {
         const int j = ed.send[e];
         const S d = tp.d[e];
-        for (int k = 0; k < K; ++k) g[k] = rbf(d, k, K, rc);
+        for (int k = 0; k < K; ++k) g[k] = rbf(d, k, K, rc, m.c.rbf);
         const S c = fcut(d, rc);
         for (int o = 0; o < 3 * F; ++o) {                     // w_e = (flt_W g + flt_b) c(d)
           S acc = S(w.flt_b[o]);
@@ -397,7 +402,15 @@ void reverse(const Model& m, int N, int nS, const int32_t* sptr, const int32_t* 
         const int i = ed.recv[e];
         const double d = tp.d[e];
         const double dmu = (K > 1) ? rc / (K - 1) : rc, gamma = 1.0 / (2.0 * dmu * dmu);
-        for (int k = 0; k < K; ++k) { g[k] = rbf(d, k, K, rc); gp[k] = -2.0 * gamma * (d - k * dmu) * g[k]; }
+        for (int k = 0; k < K; ++k) {
+          g[k] = rbf(d, k, K, rc, m.c.rbf);
+          if (m.c.rbf == 1) {  // d/dd [A sin(n pi d/rc) / d] = A (n pi/rc) cos(n pi d/rc) / d - g / d
+            const double wn = (k + 1) * M_PI / rc;
+            gp[k] = std::sqrt(2.0 / rc) * wn * std::cos(wn * d) / d - g[k] / d;
+          } else {
+            gp[k] = -2.0 * gamma * (d - k * dmu) * g[k];
+          }
+        }
         const double c = fcut(d, rc), cp = -(M_PI / (2.0 * rc)) * std::sin(M_PI * d / rc);
         for (int o = 0; o < 3 * F; ++o) {
           double lin = w.flt_b[o], dlin = 0.0;
@@ -459,7 +472,7 @@ void reverse(const Model& m, int N, int nS, const int32_t* sptr, const int32_t* 
   for (long q = 0; q < (long)N * 3; ++q) forces[q] = -gx[q];
 }
 
-Cfg make_cfg(const int32_t* ic, const double* dc) { return Cfg{ic[0], ic[1], ic[2], ic[3], ic[4], dc[0], dc[1]}; }
+Cfg make_cfg(const int32_t* ic, const double* dc) { return Cfg{ic[0], ic[1], ic[2], ic[3], ic[4], dc[0], dc[1], ic[5]}; }
 
 }  // namespace
 
@@ -536,6 +549,10 @@ void oracle_forces_dual(const int32_t* icfg, const double* dcfg, const double* w
 // Radial basis and cutoff envelope alone (for the closed-form pins): g [K], c [1].
 void oracle_rbf_cutoff(double d, int32_t K, double rc, double* g, double* c) {
   for (int k = 0; k < K; ++k) g[k] = rbf<double>(d, k, K, rc);
+  *c = fcut<double>(d, rc);
+}
+void oracle_rbf_cutoff_typed(double d, int32_t K, double rc, int32_t type, double* g, double* c) {
+  for (int k = 0; k < K; ++k) g[k] = rbf<double>(d, k, K, rc, type);
   *c = fcut<double>(d, rc);
 }
 
