@@ -45,13 +45,16 @@ extern "C" {
 
 typedef enum { PNN_BF16 = 0, PNN_FP32 = 1, PNN_FP64 = 2 } pnn_precision;
 
-/* F feature width (multiple of 32, 32..256), T interaction blocks, K Gaussian radial basis functions (2..32),
+/* F feature width (multiple of 32, 32..256), T interaction blocks, K radial basis functions (<= 32) of type rbf,
  * H heads, Zmax largest atomic number, cutoff r_c [A], norm_eps the epsilon under the sqrt of the update block. */
+#define PNN_RBF_GAUSSIAN 0 /* g_k(d) = exp(-gamma (d - k r_c/(K-1))^2), gamma = (K-1)^2 / (2 r_c^2), k = 0..K-1 (2 <= K) */
+#define PNN_RBF_BESSEL 1   /* b_n(d) = sqrt(2/r_c) sin(n pi d / r_c) / d, n = 1..K (the lead model's basis)  */
 typedef struct {
   int32_t F, T, K, H, Zmax;
   double cutoff;
   double norm_eps;
   int32_t prec; /* pnn_precision */
+  int32_t rbf;  /* PNN_RBF_GAUSSIAN or PNN_RBF_BESSEL; both are multiplied by the cosine cutoff */
 } pnn_config;
 
 typedef struct pnn_model pnn_model;         /* opaque; owns device copies of the weights in model precision */

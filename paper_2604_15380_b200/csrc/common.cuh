@@ -53,6 +53,38 @@ __device__ __forceinline__ float dsilu_f<float>(float x) {
   return sg * (1.0f + x * (1.0f - sg));
 }
 
+// Radial basis function k of type `rbf` at distance d and its derivative (SURVEY.md §8(c) B3 / reading Q2):
+//   rbf 0  Gaussian  g_k = exp(-gamma (d - k dmu)^2),  dmu = r_c / (K - 1), gamma = 1 / (2 dmu^2)
+//   rbf 1  Bessel    b_n = sqrt(2 / r_c) sin(n pi d / r_c) / d,  n = k + 1   (the paper's lead model)
+template <typename T>
+__device__ __forceinline__ void rbf_eval(int rbf, int k, T d, T rc, T dmu, T gamma, T& g, T& gd) {
+  if (rbf == 1) {
+    const T wn = T(k + 1) * T(3.14159265358979323846) / rc, A = sqrt(T(2) / rc);
+    T sn, cs;
+    sincos(wn * d, &sn, &cs);
+    g = A * sn / d;
+    gd = A * wn * cs / d - g / d;
+  } else {
+    const T dd = d - T(k) * dmu;
+    g = exp(-gamma * dd * dd);
+    gd = -T(2) * gamma * dd * g;
+  }
+}
+template <>
+__device__ __forceinline__ void rbf_eval<float>(int rbf, int k, float d, float rc, float dmu, float gamma, float& g, float& gd) {
+  if (rbf == 1) {
+    const float wn = (float)(k + 1) * 3.14159265358979323846f / rc, A = sqrtf(2.0f / rc);
+    float sn, cs;
+    sincosf(wn * d, &sn, &cs);
+    g = A * sn / d;
+    gd = A * wn * cs / d - g / d;
+  } else {
+    const float dd = d - (float)k * dmu;
+    g = expf(-gamma * dd * dd);
+    gd = -2.0f * gamma * dd * g;
+  }
+}
+
 // ---------------------------------------------------------------------------------------------
 // launch wrappers (one per kernel family); every wrapper returns the number of kernels launched
 // ---------------------------------------------------------------------------------------------
@@ -101,6 +133,7 @@ template <typename T>
 struct EdgeArgs {
   int64_t N;
   int F, K;
+  int rbf = 0; // 0 Gaussian, 1 Bessel (rbf_eval)
   double rc;
   const int32_t* rowptr;
   const int32_t* col;

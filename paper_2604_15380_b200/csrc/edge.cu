@@ -126,8 +126,9 @@ edge_fwd_k(EdgeArgs<T> a, int FS, int RB, const PT* __restrict__ phi, const T* _
       __syncthreads();
       for (int q = tid; q < nE * KP; q += nthr) {
         const int e = q / KP, k = q % KP;
-        const T dd = U[e * 4 + 3] - (T)k * dmu;
-        G[q] = (k < K) ? t_exp<T>(-gamma * dd * dd) * Cc[e] : T(0);
+        T g = T(0), gd = T(0);
+        if (k < K) rbf_eval<T>(a.rbf, k, U[e * 4 + 3], rc, dmu, gamma, g, gd);
+        G[q] = g * Cc[e];
       }
       __syncthreads();
       for (int q = 0; q < nE; ++q) {
@@ -257,10 +258,10 @@ edge_bwd_k(EdgeArgs<T> a, int FS, int RB, const PT* __restrict__ phi, const PT* 
       __syncthreads();
       for (int q = tid; q < nE * KP; q += nthr) {
         const int e = q / KP, k = q % KP;
-        const T dd = U[e * 4 + 3] - (T)k * dmu;
-        const T g = (k < K) ? t_exp<T>(-gamma * dd * dd) : T(0);
+        T g = T(0), gd = T(0);
+        if (k < K) rbf_eval<T>(a.rbf, k, U[e * 4 + 3], rc, dmu, gamma, g, gd);
         G1[q] = g * Cc[e];
-        G2[q] = (Cc[e] * (-T(2) * gamma * dd) + Cp[e]) * g;
+        G2[q] = Cc[e] * gd + Cp[e] * g;
       }
       __syncthreads();
       for (int q = 0; q < nE; ++q) {

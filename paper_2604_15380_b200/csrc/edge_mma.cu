@@ -132,15 +132,25 @@ __device__ __forceinline__ void stage_rows(const EdgeMmaArgs& a, int lane, int n
     const int row = idx / (KP / 2), k = (idx % (KP / 2)) * 2;
     const float d = Us[row].w;
     const float2 cc = Cs[row]; // (0, 0) on padded rows
-    const float d0 = d - (float)k * dmu, d1 = d0 - dmu;
-    const float r0 = (k < a.K) ? __expf(-gamma * d0 * d0) : 0.f;
-    const float r1 = (k + 1 < a.K) ? __expf(-gamma * d1 * d1) : 0.f;
+    float r0 = 0.f, r1 = 0.f, e0 = 0.f, e1 = 0.f; // basis functions k, k+1 and their derivatives
+    if (a.rbf == 1) { // Bessel: sqrt(2/rc) sin(n pi d / rc) / d, n = k + 1
+      const float A = sqrtf(2.0f / a.rc), id = 1.0f / d, w0 = (float)(k + 1) * pi_rc, w1 = w0 + pi_rc;
+      float s0, c0, s1, c1;
+      __sincosf(w0 * d, &s0, &c0);
+      __sincosf(w1 * d, &s1, &c1);
+      if (k < a.K) { r0 = A * s0 * id; e0 = (A * w0 * c0 - r0) * id; }
+      if (k + 1 < a.K) { r1 = A * s1 * id; e1 = (A * w1 * c1 - r1) * id; }
+    } else {          // Gaussian
+      const float d0 = d - (float)k * dmu, d1 = d0 - dmu;
+      if (k < a.K) { r0 = __expf(-gamma * d0 * d0); e0 = -2.0f * gamma * d0 * r0; }
+      if (k + 1 < a.K) { r1 = __expf(-gamma * d1 * d1); e1 = -2.0f * gamma * d1 * r1; }
+    }
     const float g0 = (k < a.K) ? r0 * cc.x : (k == a.K ? cc.x : 0.f);
     const float g1 = (k + 1 < a.K) ? r1 * cc.x : (k + 1 == a.K ? cc.x : 0.f);
     *reinterpret_cast<uint32_t*>(Gs + row * PA + k * 2) = pack_bf2(g0, g1);
     if (BWD) { // d/dd of the same columns
-      const float h0 = (k < a.K) ? r0 * (cc.y - 2.0f * gamma * d0 * cc.x) : (k == a.K ? cc.y : 0.f);
-      const float h1 = (k + 1 < a.K) ? r1 * (cc.y - 2.0f * gamma * d1 * cc.x) : (k + 1 == a.K ? cc.y : 0.f);
+      const float h0 = (k < a.K) ? e0 * cc.x + r0 * cc.y : (k == a.K ? cc.y : 0.f);
+      const float h1 = (k + 1 < a.K) ? e1 * cc.x + r1 * cc.y : (k + 1 == a.K ? cc.y : 0.f);
       *reinterpret_cast<uint32_t*>(G2s + row * PA + k * 2) = pack_bf2(h0, h1);
     }
   }

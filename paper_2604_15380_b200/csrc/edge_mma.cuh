@@ -11,6 +11,7 @@ namespace pnn {
 struct EdgeMmaArgs {
   int64_t N;
   int F, K;
+  int rbf = 0; // 0 Gaussian, 1 Bessel
   float rc;
   const int32_t* rowptr;
   const int32_t* col;

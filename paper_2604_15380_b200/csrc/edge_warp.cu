@@ -64,10 +64,10 @@ __device__ __forceinline__ void stage_tile_w(const EdgeArgs<float>& a, int lane,
     J[lane] = a.col[t0 + lane];
 #pragma unroll 4
     for (int k = 0; k < KP; ++k) {
-      const float dd = gq.d - (float)k * dmu;
-      const float g = (k < a.K) ? expf(-gamma * dd * dd) : 0.0f;
+      float g = 0.0f, gd = 0.0f;
+      if (k < a.K) rbf_eval<float>(a.rbf, k, gq.d, (float)a.rc, dmu, gamma, g, gd);
       G1[lane * PG + k] = g * cc;
-      if (BWD) G2[lane * PG + k] = (cc * (-2.0f * gamma * dd) + cp) * g;
+      if (BWD) G2[lane * PG + k] = cc * gd + cp * g;
     }
   }
   __syncwarp();

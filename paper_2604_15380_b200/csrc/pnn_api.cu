@@ -54,7 +54,8 @@ size_t elem_size(int prec) { return prec == PNN_FP64 ? 8 : 4; }
 bool config_ok(const pnn_config* c) {
   if (!c) return false;
   if (c->F < 32 || c->F > 256 || c->F % 32) return false;
-  if (c->T < 1 || c->T > 64 || c->K < 2 || c->K > 32 || c->H < 1 || c->Zmax < 1) return false;
+  if (c->rbf != PNN_RBF_GAUSSIAN && c->rbf != PNN_RBF_BESSEL) return false;
+  if (c->T < 1 || c->T > 64 || c->K < (c->rbf == PNN_RBF_BESSEL ? 1 : 2) || c->K > 32 || c->H < 1 || c->Zmax < 1) return false;
   if (!(c->cutoff > 0.0) || !(c->norm_eps >= 0.0)) return false;
   if (c->prec != PNN_BF16 && c->prec != PNN_FP32 && c->prec != PNN_FP64) return false;
   return true;
@@ -529,7 +530,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
   const T* W = (const T*)m->d_w;
   int nl = 0;
   EdgeArgs<T> ea;
-  ea.N = N; ea.F = F; ea.K = c.K; ea.rc = c.cutoff;
+  ea.N = N; ea.F = F; ea.K = c.K; ea.rc = c.cutoff; ea.rbf = c.rbf;
   ea.rowptr = ws->g.rowptr; ea.col = ws->g.col; ea.geom = (const Geom<T>*)ws->g.geom; ea.d_err = ws->g.d_err;
   T* s_cur = (T*)ws->s_cur; T* h = (T*)ws->h; T* sn = (T*)ws->sn; T* v1 = (T*)ws->v1; T* k = (T*)ws->k;
   const bool taped = ws->want_forces != 0;
@@ -684,13 +685,13 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
   int nl = 0;
   bool tc_fail = false;
   EdgeArgs<T> ea;
-  ea.N = N; ea.F = F; ea.K = c.K; ea.rc = c.cutoff;
+  ea.N = N; ea.F = F; ea.K = c.K; ea.rc = c.cutoff; ea.rbf = c.rbf;
   ea.rowptr = ws->g.rowptr; ea.col = ws->g.col; ea.geom = (const Geom<T>*)ws->g.geom; ea.d_err = ws->g.d_err;
   T* s_cur = (T*)ws->s_cur; T* sn = (T*)ws->sn; T* v1 = (T*)ws->v1;
   pnn_workspace::Mirror& mb = ws->mb;
   const bool taped = ws->want_forces != 0;
   EdgeMmaArgs em;
-  em.N = N; em.F = F; em.K = c.K; em.rc = (float)c.cutoff; em.rowptr = ws->g.rowptr; em.col = ws->g.col;
+  em.N = N; em.F = F; em.K = c.K; em.rbf = c.rbf; em.rc = (float)c.cutoff; em.rowptr = ws->g.rowptr; em.col = ws->g.col;
   em.geom = (const Geom<float>*)ws->g.geom; em.d_err = ws->g.d_err;
   static const bool simt_edges = getenv("PNN_BF16_SIMT_EDGES") != nullptr; // debugging aid: the SIMT edge kernels
   // C / Cb [M,N] = epi(A[M,K] . Wt[N,K]^T): A BF16 (row stride lda), Wt at element offset woff of the BF16 weight copy

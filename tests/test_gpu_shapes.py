@@ -58,3 +58,22 @@ def test_energy_only_shapes(precision):
     ref = oracle.evaluate(mc, w, b, forces=False)
     tol = 1e-5 if precision == "fp32" else 2e-2
     assert (energy_rel_err(out["energy"], ref["energy"]).max() if precision == "fp32" else l2_rel(out["energy"], ref["energy"])) < tol
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32", "bf16"])
+@pytest.mark.parametrize("F,K,kind", [(64, 4, "mol"), (256, 4, "xtal"), (128, 8, "mol"), (32, 1, "mol")])
+def test_bessel_basis(F, K, kind, precision):
+    """The paper's lead model uses 4 Bessel radial functions; pnn_config.rbf = PNN_RBF_BESSEL."""
+    rc = 5.0 if kind == "mol" else 6.0
+    mc = gen.ModelCfg(F=F, T=2, K=K, H=2, cutoff=rc, rbf="bessel")
+    w = gen.make_weights(mc, 300 + F + K)
+    b = batch_for(kind, 2)
+    out = run_gpu(mc, w, b, precision)
+    ref = oracle.evaluate(mc, w, b)
+    if precision == "bf16":
+        assert l2_rel(out["energy"], ref["energy"]) < 2e-2
+        assert l2_rel(out["forces"], ref["forces"]) < (2e-2 if kind == "mol" else 8e-2)
+    else:
+        te, tf = (1e-10, 1e-10) if precision == "fp64" else (1e-5, 1e-4)
+        assert energy_rel_err(out["energy"], ref["energy"]).max() < te
+        assert force_rel_err(out["forces"], ref["forces"], b.struct_ptr).max() < tf
