@@ -76,6 +76,7 @@ class ModelCfg:
     Zmax: int = 86
     cutoff: float = 5.0
     norm_eps: float = 1e-8
+    pbc_images: str = "minimum"  # or "all": every periodic image inside the cutoff (cells narrower than 2 r_c)
     rbf: str = "gaussian"   # or "bessel" (the paper's lead model uses 4 Bessel functions)
 
 

@@ -58,7 +58,7 @@ inline double value_of(double a) { return a; }
 inline double value_of(Dual a) { return a.v; }
 
 // ------------------------------------------------------------------ model = views into the blob
-struct Cfg { int F, T, K, H, Zmax; double rc, eps; int rbf; };  // rbf: 0 Gaussian, 1 Bessel
+struct Cfg { int F, T, K, H, Zmax; double rc, eps; int rbf; int images; };  // rbf: 0 Gaussian, 1 Bessel; images: 0 minimum image, 1 all
 struct Block {
   const double *msg_W1, *msg_b1, *msg_W2, *msg_b2, *flt_W, *flt_b;
   const double *upd_U, *upd_V, *upd_A1, *upd_c1, *upd_A2, *upd_c2;
@@ -109,13 +109,47 @@ void inverse3(const double* C, double* Ci) {
 }
 
 // SURVEY §8(c) B1.  Rows of C are the lattice vectors; positions are row vectors.
+// all_images = 0: one (minimum) image per ordered pair (reading Q13).  all_images = 1: the radius graph of the infinite
+// periodic structure — every ordered pair (i, j), i == j included, and every integer lattice shift s with
+// 0 < |x_j - x_i + s.C| < rc; needed when a cell is narrower than 2 rc.
 void neighbours(int N, int S, const double* pos, const int32_t* sptr, const double* cell,
-                const uint8_t* pbc, double rc, Edges* E) {
+                const uint8_t* pbc, double rc, Edges* E, int all_images = 0) {
   E->rowptr.assign(N + 1, 0);
   for (int g = 0; g < S; ++g) {
     const bool periodic = cell && pbc && (pbc[3 * g] || pbc[3 * g + 1] || pbc[3 * g + 2]);
     double C[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1}, Ci[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1};
     if (periodic) { std::memcpy(C, cell + 9 * g, sizeof C); inverse3(C, Ci); }
+    if (periodic && all_images) {
+      int M[3] = {0, 0, 0};   // shifts tried around the nearest image: enough to cover rc on every periodic axis
+      for (int a = 0; a < 3; ++a) {
+        const double cn = std::sqrt(Ci[0 + a] * Ci[0 + a] + Ci[3 + a] * Ci[3 + a] + Ci[6 + a] * Ci[6 + a]);
+        if (pbc[3 * g + a]) M[a] = (int)std::floor(rc * cn) + 1;   // 1/cn = distance between lattice planes of axis a
+      }
+      for (int i = sptr[g]; i < sptr[g + 1]; ++i)
+        for (int j = sptr[g]; j < sptr[g + 1]; ++j) {
+          const double D[3] = {pos[3 * j] - pos[3 * i], pos[3 * j + 1] - pos[3 * i + 1], pos[3 * j + 2] - pos[3 * i + 2]};
+          int n0[3] = {0, 0, 0};
+          for (int a = 0; a < 3; ++a)
+            if (pbc[3 * g + a]) n0[a] = (int)std::round(D[0] * Ci[0 + a] + D[1] * Ci[3 + a] + D[2] * Ci[6 + a]);
+          for (int s0 = -n0[0] - M[0]; s0 <= -n0[0] + M[0]; ++s0)      // ascending shift: the canonical edge order
+            for (int s1 = -n0[1] - M[1]; s1 <= -n0[1] + M[1]; ++s1)
+              for (int s2 = -n0[2] - M[2]; s2 <= -n0[2] + M[2]; ++s2) {
+                if (j == i && s0 == 0 && s1 == 0 && s2 == 0) continue;
+                const int sh[3] = {s0, s1, s2};
+                double sc[3], r[3];
+                for (int b = 0; b < 3; ++b) {
+                  sc[b] = sh[0] * C[0 + b] + sh[1] * C[3 + b] + sh[2] * C[6 + b];
+                  r[b] = D[b] + sc[b];
+                }
+                if (r[0] * r[0] + r[1] * r[1] + r[2] * r[2] < rc * rc) {
+                  E->recv.push_back(i); E->send.push_back(j);
+                  for (int b = 0; b < 3; ++b) { E->shift.push_back((int8_t)sh[b]); E->shift_cart.push_back(sc[b]); }
+                  E->rowptr[i + 1]++;
+                }
+              }
+        }
+      continue;
+    }
     for (int i = sptr[g]; i < sptr[g + 1]; ++i) {
       for (int j = sptr[g]; j < sptr[g + 1]; ++j) {
         if (j == i) continue;                                       // Q12: no self edge
@@ -472,7 +506,7 @@ void reverse(const Model& m, int N, int nS, const int32_t* sptr, const int32_t* 
   for (long q = 0; q < (long)N * 3; ++q) forces[q] = -gx[q];
 }
 
-Cfg make_cfg(const int32_t* ic, const double* dc) { return Cfg{ic[0], ic[1], ic[2], ic[3], ic[4], dc[0], dc[1], ic[5]}; }
+Cfg make_cfg(const int32_t* ic, const double* dc) { return Cfg{ic[0], ic[1], ic[2], ic[3], ic[4], dc[0], dc[1], ic[5], ic[6]}; }
 
 }  // namespace
 
@@ -486,11 +520,19 @@ int64_t oracle_weights_count(const int32_t* icfg /*F,T,K,H,Zmax*/) {
 }
 
 // B1 only.  Pass 1: call with recv == NULL to get the edge count.  Pass 2: fill arrays.
+int64_t oracle_neighbours_images(int32_t N, int32_t S, const double* pos, const int32_t* sptr, const double* cell,
+                                 const uint8_t* pbc, double rc, int32_t all_images, int32_t* rowptr, int32_t* recv,
+                                 int32_t* send, int8_t* shift, double* rvec);
 int64_t oracle_neighbours(int32_t N, int32_t S, const double* pos, const int32_t* sptr, const double* cell,
                           const uint8_t* pbc, double rc, int32_t* rowptr, int32_t* recv, int32_t* send,
                           int8_t* shift, double* rvec) {
+  return oracle_neighbours_images(N, S, pos, sptr, cell, pbc, rc, 0, rowptr, recv, send, shift, rvec);
+}
+int64_t oracle_neighbours_images(int32_t N, int32_t S, const double* pos, const int32_t* sptr, const double* cell,
+                                 const uint8_t* pbc, double rc, int32_t all_images, int32_t* rowptr, int32_t* recv,
+                                 int32_t* send, int8_t* shift, double* rvec) {
   Edges ed;
-  neighbours(N, S, pos, sptr, cell, pbc, rc, &ed);
+  neighbours(N, S, pos, sptr, cell, pbc, rc, &ed, all_images);
   const int64_t E = (int64_t)ed.recv.size();
   if (rowptr) std::memcpy(rowptr, ed.rowptr.data(), sizeof(int32_t) * (N + 1));
   if (recv) {
@@ -514,7 +556,7 @@ int64_t oracle_eval(const int32_t* icfg, const double* dcfg /*cutoff, eps*/, con
   Model m;
   parse_blob(make_cfg(icfg, dcfg), weights, &m);
   Edges ed;
-  neighbours(N, S, pos, sptr, cell, pbc, m.c.rc, &ed);
+  neighbours(N, S, pos, sptr, cell, pbc, m.c.rc, &ed, m.c.images);
   Tape<double> tp;
   forward<double>(m, N, S, Z, pos, sptr, head, ed, tp, energy);
   if (s_out) std::memcpy(s_out, tp.s_out.data(), sizeof(double) * tp.s_out.size());
@@ -533,7 +575,7 @@ void oracle_forces_dual(const int32_t* icfg, const double* dcfg, const double* w
   Model m;
   parse_blob(make_cfg(icfg, dcfg), weights, &m);
   Edges ed;
-  neighbours(N, S, pos, sptr, cell, pbc, m.c.rc, &ed);
+  neighbours(N, S, pos, sptr, cell, pbc, m.c.rc, &ed, m.c.images);
   std::vector<int> sof(N);
   for (int g = 0; g < S; ++g) for (int i = sptr[g]; i < sptr[g + 1]; ++i) sof[i] = g;
 #pragma omp parallel for schedule(dynamic, 1)

@@ -53,7 +53,7 @@ def edges_by_image_enumeration(batch: gen.Batch, rc: float, nimg: int = 2):
                 d2 = (d * d).sum(1)
                 for jj in np.nonzero(d2 < rc * rc)[0]:
                     j = sp[g] + jj
-                    if j == i:
+                    if j == i and not any(sh):
                         continue
                     out.add((int(i), int(j), int(sh[0]), int(sh[1]), int(sh[2])))
     return out
