@@ -47,6 +47,8 @@ typedef enum { PNN_BF16 = 0, PNN_FP32 = 1, PNN_FP64 = 2 } pnn_precision;
 
 /* F feature width (multiple of 32, 32..256), T interaction blocks, K radial basis functions (<= 32) of type rbf,
  * H heads, Zmax largest atomic number, cutoff r_c [A], norm_eps the epsilon under the sqrt of the update block. */
+#define PNN_IMAGES_MINIMUM 0 /* one (nearest) periodic image per ordered pair: exact only for cells >= 2 r_c wide        */
+#define PNN_IMAGES_ALL 1     /* every periodic image inside the cutoff, an atom's own images included (narrow cells)     */
 #define PNN_RBF_GAUSSIAN 0 /* g_k(d) = exp(-gamma (d - k r_c/(K-1))^2), gamma = (K-1)^2 / (2 r_c^2), k = 0..K-1 (2 <= K) */
 #define PNN_RBF_BESSEL 1   /* b_n(d) = sqrt(2/r_c) sin(n pi d / r_c) / d, n = 1..K (the lead model's basis)  */
 typedef struct {
@@ -55,6 +57,7 @@ typedef struct {
   double norm_eps;
   int32_t prec; /* pnn_precision */
   int32_t rbf;  /* PNN_RBF_GAUSSIAN or PNN_RBF_BESSEL; both are multiplied by the cosine cutoff */
+  int32_t pbc_images; /* PNN_IMAGES_MINIMUM or PNN_IMAGES_ALL (pnn_build_graph) */
 } pnn_config;
 
 typedef struct pnn_model pnn_model;         /* opaque; owns device copies of the weights in model precision */
@@ -79,7 +82,8 @@ int64_t pnn_workspace_bytes(const pnn_workspace* ws);
 
 /* a1 — radius graph (PAPER.md:230 cutoff, PAPER.md:269 PBC).  All ordered pairs (i, j),
  * i != j, in the same structure, with |x_j - x_i + shift.C| < r_c (strict, FP64); under PBC the shift is the
- * per-axis minimum-image rounding of the fractional difference.  Built by a cell list (cells >= r_c wide; a
+ * per-axis minimum-image rounding of the fractional difference (PNN_IMAGES_MINIMUM), or every shift that satisfies the
+ * predicate, pairs i == j with a non-zero shift included (PNN_IMAGES_ALL; several edges per ordered pair then).  Built by a cell list (cells >= r_c wide; a
  * structure narrower than 3 cells along an axis uses one cell on that axis) and emitted as receiver-sorted CSR
  * held inside the workspace, together with the per-edge unit vector and distance in model precision.
  *   pos        DEVICE [N,3] f64        struct_ptr DEVICE [S+1] i32

@@ -110,7 +110,7 @@ struct GraphBuffers {
   int* d_err;
 };
 int launch_graph_build(const GraphBuffers& g, int64_t N, int64_t S, const double* pos, const int32_t* struct_ptr,
-                       const double* cell, const uint8_t* pbc, double rc, int prec, cudaStream_t st);
+                       const double* cell, const uint8_t* pbc, double rc, int prec, int all_images, cudaStream_t st);
 
 // gemm_simt.cu :  C[M,N] (ldc) = epi( A[M,K] (lda) * B[K,N] (ldb) )
 enum : int { ACT_NONE = 0, ACT_SILU = 1, ACT_MUL_DSILU = 2 };

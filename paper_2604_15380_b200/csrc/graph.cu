@@ -249,7 +249,7 @@ __global__ void __launch_bounds__(256) sortcells_k(int64_t ncap, const int32_t* 
 }
 
 // ------------------------------------------------------------------------------------------ neighbour passes
-template <typename T, bool EMIT>
+template <typename T, bool EMIT, bool ALLIMG>
 __global__ void __launch_bounds__(256) neigh_k(int64_t N, const double* __restrict__ pos,
                                                const int32_t* __restrict__ a2s, const GridDesc* __restrict__ desc,
                                                const int32_t* __restrict__ cell_off, const int32_t* __restrict__ cid,
@@ -257,6 +257,7 @@ __global__ void __launch_bounds__(256) neigh_k(int64_t N, const double* __restri
                                                const int32_t* __restrict__ sorted, double rc2, int32_t* deg,
                                                const int32_t* __restrict__ rowptr, int32_t* col, int8_t* shift,
                                                Geom<T>* geom, int64_t max_edges) {
+  constexpr int all_images = ALLIMG ? 1 : 0;
   const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; // one warp per receiver
   const int lane = threadIdx.x & 31;
   if (i >= N) return;
@@ -276,6 +277,16 @@ __global__ void __launch_bounds__(256) neigh_k(int64_t N, const double* __restri
   const int cz = lc % dz; lc /= dz;
   const int cy = lc % dy;
   const int cx = lc / dy;
+  // all_images: on a periodic axis too narrow for a cell list (one cell), every image within the cutoff is an edge, the
+  // atom's own images included; M[a] shifts are tried on either side of the nearest image.  On an axis with >= 3 cells
+  // (each >= r_c wide) only the nearest image can be inside the cutoff.
+  int M0 = 0, M1 = 0, M2 = 0;
+  if (ALLIMG && periodic) {
+    const double rc = sqrt(rc2);
+    if (per[0] && dx == 1) M0 = (int)floor(rc * sqrt(Ci[0] * Ci[0] + Ci[3] * Ci[3] + Ci[6] * Ci[6])) + 1;
+    if (per[1] && dy == 1) M1 = (int)floor(rc * sqrt(Ci[1] * Ci[1] + Ci[4] * Ci[4] + Ci[7] * Ci[7])) + 1;
+    if (per[2] && dz == 1) M2 = (int)floor(rc * sqrt(Ci[2] * Ci[2] + Ci[5] * Ci[5] + Ci[8] * Ci[8])) + 1;
+  }
   int base = 0;
   bool ok_row = true;
   if (EMIT) {
@@ -296,39 +307,45 @@ __global__ void __launch_bounds__(256) neigh_k(int64_t N, const double* __restri
         const int pb = cell_start[c], pe = cell_start[c + 1];
         for (int p0 = pb; p0 < pe; p0 += 32) {
           const int p = p0 + lane;
-          bool hit = false;
           int j = -1, n0 = 0, n1 = 0, n2 = 0;
-          double r0 = 0, r1 = 0, r2 = 0;
-          if (p < pe) {
+          double D0 = 0, D1 = 0, D2 = 0;
+          const bool cand = p < pe;
+          if (cand) {
             j = sorted[p];
-            if (j != (int)i) {
-              // same operation order as the definition (oracle B1): D, f = D.C^-1, n = round(f), r = D - n.C
-              const double D0 = pos[3 * (int64_t)j] - xi, D1 = pos[3 * (int64_t)j + 1] - yi,
-                           D2 = pos[3 * (int64_t)j + 2] - zi;
-              if (periodic) {
-                if (per[0]) n0 = (int)round(D0 * Ci[0] + D1 * Ci[3] + D2 * Ci[6]);
-                if (per[1]) n1 = (int)round(D0 * Ci[1] + D1 * Ci[4] + D2 * Ci[7]);
-                if (per[2]) n2 = (int)round(D0 * Ci[2] + D1 * Ci[5] + D2 * Ci[8]);
+            // same operation order as the definition (oracle B1): D, f = D.C^-1, n = round(f), r = D - n.C
+            D0 = pos[3 * (int64_t)j] - xi; D1 = pos[3 * (int64_t)j + 1] - yi; D2 = pos[3 * (int64_t)j + 2] - zi;
+            if (periodic) {
+              if (per[0]) n0 = (int)round(D0 * Ci[0] + D1 * Ci[3] + D2 * Ci[6]);
+              if (per[1]) n1 = (int)round(D0 * Ci[1] + D1 * Ci[4] + D2 * Ci[7]);
+              if (per[2]) n2 = (int)round(D0 * Ci[2] + D1 * Ci[5] + D2 * Ci[8]);
+            }
+          }
+          for (int e0 = -M0; e0 <= M0; ++e0)
+            for (int e1 = -M1; e1 <= M1; ++e1)
+              for (int e2 = -M2; e2 <= M2; ++e2) { // warp-uniform trip counts: one ballot per image
+                bool hit = false;
+                const int m0 = n0 + e0, m1 = n1 + e1, m2 = n2 + e2;
+                double r0 = 0, r1 = 0, r2 = 0;
+                if (cand && (j != (int)i || (all_images && (m0 | m1 | m2) != 0))) {
+                  r0 = D0 + (-(m0 * C[0] + m1 * C[3] + m2 * C[6]));
+                  r1 = D1 + (-(m0 * C[1] + m1 * C[4] + m2 * C[7]));
+                  r2 = D2 + (-(m0 * C[2] + m1 * C[5] + m2 * C[8]));
+                  hit = (r0 * r0 + r1 * r1 + r2 * r2) < rc2;
+                }
+                const unsigned m = __ballot_sync(0xffffffffu, hit);
+                if (EMIT) {
+                  if (hit && ok_row) {
+                    const int64_t e = (int64_t)base + total + __popc(m & ((1u << lane) - 1u));
+                    col[e] = j;
+                    shift[3 * e] = (int8_t)(-m0); shift[3 * e + 1] = (int8_t)(-m1); shift[3 * e + 2] = (int8_t)(-m2);
+                    const double dd = sqrt(r0 * r0 + r1 * r1 + r2 * r2);
+                    Geom<T> q;
+                    q.ux = (T)(r0 / dd); q.uy = (T)(r1 / dd); q.uz = (T)(r2 / dd); q.d = (T)dd;
+                    geom[e] = q;
+                  }
+                }
+                total += __popc(m);
               }
-              r0 = D0 + (-(n0 * C[0] + n1 * C[3] + n2 * C[6]));
-              r1 = D1 + (-(n0 * C[1] + n1 * C[4] + n2 * C[7]));
-              r2 = D2 + (-(n0 * C[2] + n1 * C[5] + n2 * C[8]));
-              hit = (r0 * r0 + r1 * r1 + r2 * r2) < rc2;
-            }
-          }
-          const unsigned m = __ballot_sync(0xffffffffu, hit);
-          if (EMIT) {
-            if (hit && ok_row) {
-              const int64_t e = (int64_t)base + total + __popc(m & ((1u << lane) - 1u));
-              col[e] = j;
-              shift[3 * e] = (int8_t)(-n0); shift[3 * e + 1] = (int8_t)(-n1); shift[3 * e + 2] = (int8_t)(-n2);
-              const double dd = sqrt(r0 * r0 + r1 * r1 + r2 * r2);
-              Geom<T> q;
-              q.ux = (T)(r0 / dd); q.uy = (T)(r1 / dd); q.uz = (T)(r2 / dd); q.d = (T)dd;
-              geom[e] = q;
-            }
-          }
-          total += __popc(m);
         }
       }
     }
@@ -343,7 +360,7 @@ __global__ void check_edges_k(int64_t N, const int32_t* rowptr, int64_t max_edge
 } // namespace
 
 int launch_graph_build(const GraphBuffers& gb, int64_t N, int64_t S, const double* pos, const int32_t* sptr,
-                       const double* cell, const uint8_t* pbc, double rc, int prec, cudaStream_t st) {
+                       const double* cell, const uint8_t* pbc, double rc, int prec, int all_images, cudaStream_t st) {
   int nl = 0;
   if (N == 0 || S == 0) {
     cudaMemsetAsync(gb.rowptr, 0, sizeof(int32_t) * (N + 1), st);
@@ -361,19 +378,25 @@ int launch_graph_build(const GraphBuffers& gb, int64_t N, int64_t S, const doubl
   sortcells_k<<<(unsigned)((ncap + 255) / 256), 256, 0, st>>>(ncap, gb.cell_start, gb.sorted); PNN_KCHECK("sortcells_k"); ++nl;
   const unsigned nbW = (unsigned)((N * 32 + 255) / 256);
   const double rc2 = rc * rc;
-  neigh_k<float, false><<<nbW, 256, 0, st>>>(N, pos, gb.a2s, gb.desc, gb.cell_off, gb.cid, gb.cell_start, gb.sorted,
-                                             rc2, gb.deg, nullptr, nullptr, nullptr, nullptr, gb.max_edges); PNN_KCHECK("neigh_k"); ++nl;
+#define PNN_NEIGH(TT, EM, ...)                                                                          \
+  {                                                                                                     \
+    if (all_images) neigh_k<TT, EM, true><<<nbW, 256, 0, st>>>(__VA_ARGS__);                            \
+    else neigh_k<TT, EM, false><<<nbW, 256, 0, st>>>(__VA_ARGS__);                                      \
+    PNN_KCHECK("neigh_k");                                                                              \
+  }
+  PNN_NEIGH(float, false, N, pos, gb.a2s, gb.desc, gb.cell_off, gb.cid, gb.cell_start, gb.sorted, rc2, gb.deg, nullptr,
+            nullptr, nullptr, (Geom<float>*)nullptr, gb.max_edges)
+  ++nl;
   nl += exclusive_scan(gb.deg, N, gb.rowptr, gb.scan_tmp, st);
   check_edges_k<<<1, 1, 0, st>>>(N, gb.rowptr, gb.max_edges, gb.d_err); PNN_KCHECK("check_edges_k"); ++nl;
   if (prec == 2) {
-    neigh_k<double, true><<<nbW, 256, 0, st>>>(N, pos, gb.a2s, gb.desc, gb.cell_off, gb.cid, gb.cell_start,
-                                               gb.sorted, rc2, nullptr, gb.rowptr, gb.col, gb.shift,
-                                               (Geom<double>*)gb.geom, gb.max_edges); PNN_KCHECK("neigh_k");
+    PNN_NEIGH(double, true, N, pos, gb.a2s, gb.desc, gb.cell_off, gb.cid, gb.cell_start, gb.sorted, rc2, nullptr,
+              gb.rowptr, gb.col, gb.shift, (Geom<double>*)gb.geom, gb.max_edges)
   } else {
-    neigh_k<float, true><<<nbW, 256, 0, st>>>(N, pos, gb.a2s, gb.desc, gb.cell_off, gb.cid, gb.cell_start,
-                                              gb.sorted, rc2, nullptr, gb.rowptr, gb.col, gb.shift,
-                                              (Geom<float>*)gb.geom, gb.max_edges); PNN_KCHECK("neigh_k");
+    PNN_NEIGH(float, true, N, pos, gb.a2s, gb.desc, gb.cell_off, gb.cid, gb.cell_start, gb.sorted, rc2, nullptr,
+              gb.rowptr, gb.col, gb.shift, (Geom<float>*)gb.geom, gb.max_edges)
   }
+#undef PNN_NEIGH
   ++nl;
   return nl;
 }

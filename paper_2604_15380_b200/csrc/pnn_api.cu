@@ -55,6 +55,7 @@ bool config_ok(const pnn_config* c) {
   if (!c) return false;
   if (c->F < 32 || c->F > 256 || c->F % 32) return false;
   if (c->rbf != PNN_RBF_GAUSSIAN && c->rbf != PNN_RBF_BESSEL) return false;
+  if (c->pbc_images != PNN_IMAGES_MINIMUM && c->pbc_images != PNN_IMAGES_ALL) return false;
   if (c->T < 1 || c->T > 64 || c->K < (c->rbf == PNN_RBF_BESSEL ? 1 : 2) || c->K > 32 || c->H < 1 || c->Zmax < 1) return false;
   if (!(c->cutoff > 0.0) || !(c->norm_eps >= 0.0)) return false;
   if (c->prec != PNN_BF16 && c->prec != PNN_FP32 && c->prec != PNN_FP64) return false;
@@ -436,7 +437,8 @@ int pnn_build_graph(pnn_workspace* ws, int64_t N, int64_t S, const double* pos, 
   cudaStream_t st = (cudaStream_t)stream;
   {
     ProfScope ps(ws, st, "graph_build");
-    const int nl = launch_graph_build(ws->g, N, S, pos, sptr, cell, pbc, ws->model->cfg.cutoff, ws->model->cfg.prec, st);
+    const int nl = launch_graph_build(ws->g, N, S, pos, sptr, cell, pbc, ws->model->cfg.cutoff, ws->model->cfg.prec,
+                                      ws->model->cfg.pbc_images, st);
     ws->launches += nl;
     ps.done(nl);
   }
