@@ -86,12 +86,14 @@ def force_rel_err(Fc, Fref, struct_ptr):
 
 
 # ----------------------------------------------------------------------------- torch third opinion
-def torch_painn(mc: gen.ModelCfg, blob, batch: gen.Batch, edges, want_forces=True):
-    """Vectorised FP64 torch restatement with autograd forces.  `edges` = (recv, send, shift[E,3])
-    from an enumeration that does not come from the oracle."""
+def torch_painn(mc: gen.ModelCfg, blob, batch: gen.Batch, edges, want_forces=True, dtype=None):
+    """Vectorised torch restatement with autograd forces (FP64; `dtype=torch.float32` gives the plain library
+    FP32 evaluation used as the FP32 rounding floor).  `edges` = (recv, send, shift[E,3]) from an enumeration
+    that does not come from the oracle."""
     import torch
     torch.set_num_threads(max(1, torch.get_num_threads()))
-    W = {k: torch.tensor(v) for k, v in gen.synth.unpack_weights(mc, np.asarray(blob, np.float64)).items()}
+    DT = dtype or torch.float64
+    W = {k: torch.tensor(v).to(DT) for k, v in gen.synth.unpack_weights(mc, np.asarray(blob, np.float64)).items()}
     F, K, rc = mc.F, mc.K, mc.cutoff
     recv = torch.tensor(np.asarray(edges[0], np.int64))
     send = torch.tensor(np.asarray(edges[1], np.int64))
@@ -101,18 +103,18 @@ def torch_painn(mc: gen.ModelCfg, blob, batch: gen.Batch, edges, want_forces=Tru
         sc = np.einsum("ea,eab->eb", shift, batch.cell[sof[np.asarray(edges[0], np.int64)]])
     else:
         sc = np.zeros_like(shift)
-    pos = torch.tensor(batch.pos, requires_grad=True)
-    r = pos[send] - pos[recv] + torch.tensor(sc)
+    pos = torch.tensor(batch.pos).to(DT).requires_grad_(True)
+    r = pos[send] - pos[recv] + torch.tensor(sc).to(DT)
     d = r.norm(dim=1)
     u = r / d[:, None]
-    mu = torch.arange(K, dtype=torch.float64) * (rc / (K - 1) if K > 1 else rc)
+    mu = torch.arange(K, dtype=DT) * (rc / (K - 1) if K > 1 else rc)
     dmu = rc / (K - 1) if K > 1 else rc
     g = torch.exp(-(d[:, None] - mu[None, :]) ** 2 / (2 * dmu * dmu))
     c = 0.5 * (torch.cos(np.pi * d / rc) + 1.0)
     silu = torch.nn.functional.silu
     N = batch.n_atoms
     s = W["emb"][torch.tensor(batch.Z.astype(np.int64))]
-    v = torch.zeros(N, 3, F, dtype=torch.float64)
+    v = torch.zeros(N, 3, F, dtype=DT)
     for t in range(mc.T):
         p = f"b{t}."
         phi = silu(s @ W[p + "msg_W1"].T + W[p + "msg_b1"]) @ W[p + "msg_W2"].T + W[p + "msg_b2"]
@@ -136,9 +138,9 @@ def torch_painn(mc: gen.ModelCfg, blob, batch: gen.Batch, edges, want_forces=Tru
     w2 = torch.stack([W[f"h{h}.out_w2"] for h in range(mc.H)])[ha]
     b2 = torch.stack([W[f"h{h}.out_b2"] for h in range(mc.H)])[ha][:, 0]
     e = (w2 * silu(torch.einsum("nof,nf->no", W1, s) + b1)).sum(1) + b2
-    E = torch.zeros(batch.n_structs, dtype=torch.float64).index_add(0, torch.tensor(sof), e)
-    out = dict(energy=E.detach().numpy(), s=s.detach().numpy(), v=v.detach().numpy())
+    E = torch.zeros(batch.n_structs, dtype=DT).index_add(0, torch.tensor(sof), e)
+    out = dict(energy=E.detach().double().numpy(), s=s.detach().double().numpy(), v=v.detach().double().numpy())
     if want_forces:
         (gx,) = torch.autograd.grad(E.sum(), pos)
-        out["forces"] = -gx.numpy()
+        out["forces"] = -gx.double().numpy()
     return out

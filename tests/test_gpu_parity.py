@@ -105,6 +105,33 @@ def test_cfg3_crystals(precision):
     check_values(mc, w, b, out, precision)
 
 
+def test_cfg3_fp32_force_error_population_against_the_fp32_rounding_floor():
+    """DESIGN.md reading Q27.  BASELINE.json's FP32 force tolerance (1e-4) holds on the cfg3 sample above but not on
+    every cfg3 structure: the random-weight 128-wide, 60-neighbour network amplifies FP32 rounding to 1e-4...8e-4 of
+    the force scale in ANY FP32 evaluation.  What the kernels can be held to is (a) the energy tolerance on every
+    structure, (b) the force tolerance on the median structure, and (c) doing no worse than a plain library FP32
+    evaluation (torch CPU, autograd) of the same structures, which is the rounding floor of the arithmetic type."""
+    import torch
+    from helpers import torch_painn
+    mc = gen.model_cfg(3)
+    w = gen.make_weights(mc, 3)
+    eg, fg, ft = [], [], []
+    for start in (0, 4, 8):
+        b = gen.make_batch(3, start, 4)
+        ref = oracle.evaluate(mc, w, b)
+        nb = oracle.neighbours(b, mc.cutoff)
+        lib = torch_painn(mc, w, b, (nb["recv"], nb["send"], nb["shift"]), dtype=torch.float32)
+        out = run_gpu(mc, w, b, "fp32")
+        eg += list(energy_rel_err(out["energy"], ref["energy"]))
+        fg += list(force_rel_err(out["forces"], ref["forces"], b.struct_ptr))
+        ft += list(force_rel_err(lib["forces"], ref["forces"], b.struct_ptr))
+    eg, fg, ft = np.array(eg), np.array(fg), np.array(ft)
+    assert eg.max() < 1e-5
+    assert np.median(fg) < 1e-4
+    assert fg.max() < 1e-3
+    assert fg.max() <= 1.5 * ft.max() and np.median(fg) <= 1.5 * np.median(ft), (fg, ft)
+
+
 def test_cfg5_scaled_fp64():
     mc, b = gen.model_cfg(5), gen.make_batch(5, n_atoms=1200)
     w = gen.make_weights(mc, 5)
