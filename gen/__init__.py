@@ -15,6 +15,9 @@ from .synth import (  # noqa: F401
     weights_layout,
     make_weights,
     make_head_weights,
+    BRANCH_MLP_WIDTHS,
+    branch_mlp_count,
+    make_branch_mlp,
     make_batch,
     make_molecules,
     make_crystals,

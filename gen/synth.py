@@ -27,7 +27,7 @@ _M2 = np.uint64(0x94D049BB133111EB)
 _GOLD = np.uint64(0x9E3779B97F4A7C15)
 
 # purpose tags (arbitrary distinct constants)
-_T_NATOMS, _T_HEAD, _T_POS, _T_Z, _T_SHUF, _T_JIT, _T_W, _T_HW = 11, 12, 13, 14, 15, 16, 17, 18
+_T_NATOMS, _T_HEAD, _T_POS, _T_Z, _T_SHUF, _T_JIT, _T_W, _T_HW, _T_BW = 11, 12, 13, 14, 15, 16, 17, 18, 19
 
 MARGIN = 1e-9
 
@@ -185,6 +185,33 @@ def make_head_weights(cfg_id: int, struct_ids, H: int, sharpness: float = 6.0, s
     z = sharpness * z
     e = np.exp(z - z.max(axis=1, keepdims=True))
     return np.round(e / e.sum(axis=1, keepdims=True), 6)
+
+
+BRANCH_MLP_WIDTHS = (118, 128, 64, 16)      # 118*128+128 + 128*64+64 + 64*16+16 = 24,528 parameters ("24,500")
+
+
+def branch_mlp_count(widths: Sequence[int]) -> int:
+    return sum(widths[l + 1] * widths[l] + widths[l + 1] for l in range(len(widths) - 1))
+
+
+def make_branch_mlp(widths: Sequence[int] = BRANCH_MLP_WIDTHS, sharpness: float = 70.0, seed: int = BASE_SEED) -> np.ndarray:
+    """Flat FP64 parameter blob of the composition -> branch-weight MLP: per layer W [out, in] row-major, then b [out].
+    Seeded normals: first layer N(0,1) (its input is a composition vector whose entries sum to 1), later layers
+    N(0, 1/fan_in), biases N(0, 0.01); the last layer is scaled by `sharpness` so that the softmax is as peaked as the
+    paper's trained router (~81 % of the branches negligible).  No arithmetic of the method here."""
+    blob = np.empty(branch_mlp_count(widths), np.float64)
+    off = 0
+    L = len(widths) - 1
+    for l in range(L):
+        n_in, n_out = widths[l], widths[l + 1]
+        zw = _normal(seed, 0, _T_BW, 2 * l, np.arange(n_out * n_in, dtype=np.uint64))
+        zb = _normal(seed, 0, _T_BW, 2 * l + 1, np.arange(n_out, dtype=np.uint64))
+        gain = (1.0 if l == 0 else 1.0 / math.sqrt(n_in)) * (sharpness if l == L - 1 else 1.0)
+        blob[off:off + n_out * n_in] = zw * gain
+        off += n_out * n_in
+        blob[off:off + n_out] = zb * 0.1
+        off += n_out
+    return blob
 
 
 def unpack_weights(mc: ModelCfg, blob: np.ndarray) -> dict:

@@ -192,3 +192,46 @@ def evaluate_blended(mc, weights, batch, head_weights, forces: bool = True, skip
         if forces:
             frc += hw[sof, h][:, None] * out["forces"]
     return dict(energy=energy, forces=frc, n_edges=n_edges)
+
+
+def branch_weights(Z, struct_ptr, widths, params):
+    """Composition-conditioned branch weights ("the MLP maps the structure's chemical-composition vector
+    to softmax weights that blend these branch outputs"; "24,500 parameters ... maps per-element
+    chemical-composition vectors to per-branch blending weights ... softmax-normalized").
+
+    The paper gives neither the layer widths nor the activation nor the normalisation of the composition vector; DESIGN.md
+    reading Q28 fixes them: c_z = (number of atoms of the structure with atomic number z) / (number of atoms), z = 1 ...
+    widths[0] (an empty structure has c = 0); hidden layers x <- SiLU(W x + b) (the backbone's activation, SURVEY §8(c));
+    last layer linear; w = softmax over the widths[-1] heads.  `params` = per layer W [out, in] row-major then b [out],
+    FP64.  Returns [S, H] FP64.  Plain loops over structures and layers; written from the definition."""
+    Z = np.asarray(Z, np.int64)
+    sp = np.asarray(struct_ptr, np.int64)
+    widths = [int(x) for x in widths]
+    params = np.asarray(params, np.float64)
+    S = sp.shape[0] - 1
+    layers, off = [], 0
+    for l in range(len(widths) - 1):
+        n_in, n_out = widths[l], widths[l + 1]
+        W = params[off:off + n_out * n_in].reshape(n_out, n_in)
+        off += n_out * n_in
+        b = params[off:off + n_out]
+        off += n_out
+        layers.append((W, b))
+    assert off == params.shape[0]
+    out = np.zeros((S, widths[-1]), np.float64)
+    for g in range(S):
+        zs = Z[sp[g]:sp[g + 1]]
+        assert zs.size == 0 or (zs.min() >= 1 and zs.max() <= widths[0])
+        c = np.zeros(widths[0], np.float64)
+        for z in zs:
+            c[z - 1] += 1.0
+        if zs.size:
+            c /= zs.size
+        x = c
+        for l, (W, b) in enumerate(layers):
+            x = W @ x + b
+            if l + 1 < len(layers):
+                x = x / (1.0 + np.exp(-x))
+        e = np.exp(x - x.max())
+        out[g] = e / e.sum()
+    return out
