@@ -219,12 +219,13 @@ def main():
 
         blended = name.endswith("_blended")
         if blended:
-            hw = gen.make_head_weights(cfg_id, np.arange(rank * S, rank * S + b.n_structs), mc.H)
-            d["hw"] = torch.from_numpy(hw).to(torch.float64 if prec == "fp64" else torch.float32).to(dev)
+            # the composition -> softmax router runs on the device inside every step (Fig. 5)
+            net.set_branch_mlp(gen.BRANCH_MLP_WIDTHS, gen.make_branch_mlp())
 
         def step():
             if blended:
-                return net.eval_blended(d["Z"], d["pos"], d["sp"], d["hw"], d["cell"], d["pbc"], forces=forces,
+                hw = net.branch_weights(d["Z"], d["sp"])
+                return net.eval_blended(d["Z"], d["pos"], d["sp"], hw, d["cell"], d["pbc"], forces=forces,
                                         skip_below=0.01)
             return net.eval(d["Z"], d["pos"], d["sp"], d["head"], d["cell"], d["pbc"], forces=forces)
 

@@ -127,6 +127,27 @@ int pnn_eval_blended(const pnn_model* m, pnn_workspace* ws, int64_t n_atoms, int
                      const double* pos, const int32_t* struct_ptr, const void* head_weights, double skip_below,
                      int flags, void* energy, void* forces, void* cuda_stream);
 
+/* Composition-conditioned branch weights ("the MLP maps the structure's chemical-composition vector
+ * to softmax weights that blend these branch outputs"; "24,500 parameters ... per-element
+ * chemical-composition vectors ... softmax-normalized"; reading Q28 for what the paper leaves open):
+ *   c_z = (atoms of the structure with atomic number z) / (atoms of the structure), z = 1..widths[0] (c = 0 if empty);
+ *   x <- SiLU(W_l x + b_l) for the hidden layers, the last layer linear; w = softmax over the widths[n_layers] heads.
+ * pnn_branch_mlp_create: widths HOST [n_layers+1] (1 <= n_layers <= 8, every width in [1,256]); params HOST f64,
+ * per layer W [out,in] row-major then b [out], n_params = sum(out*in + out) (PNN_ERR_INVALID_ARG otherwise); copied to
+ * the device in FP64 (prec = PNN_FP64) or FP32 (PNN_FP32, PNN_BF16: the router is never evaluated in BF16).  The caller
+ * owns *out and frees it with pnn_branch_mlp_destroy. */
+typedef struct pnn_branch_mlp pnn_branch_mlp;
+int pnn_branch_mlp_create(int32_t n_layers, const int32_t* widths, const double* params, int64_t n_params, int prec,
+                          pnn_branch_mlp** out);
+void pnn_branch_mlp_destroy(pnn_branch_mlp* b);
+
+/* head_weights[g][h], DEVICE [S, widths[n_layers]] (f64 for a PNN_FP64 router, f32 otherwise) — the array
+ * pnn_eval_blended takes.  Z DEVICE [N] i32, struct_ptr DEVICE [S+1] i32.  An atomic number outside [1, widths[0]] is
+ * left out of the counts and sets the workspace's bad-input flag (pnn_check_async_errors -> PNN_ERR_BAD_INPUT).  The
+ * workspace is used for that flag and the launch count only; no graph is needed.  Asynchronous. */
+int pnn_branch_weights(const pnn_branch_mlp* b, pnn_workspace* ws, int64_t n_atoms, int64_t n_structs,
+                       const int32_t* Z, const int32_t* struct_ptr, void* head_weights, void* cuda_stream);
+
 /* Convenience for callers with HOST buffers (bench.py's e2e leg): copies Z, pos, struct_ptr, head (and cell /
  * pbc when not NULL) to the device, runs pnn_build_graph + pnn_eval and copies energy [S] / forces [N,3] back.
  * energy_host / forces_host have the dtype pnn_eval documents.  Synchronous. */

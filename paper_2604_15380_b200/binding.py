@@ -15,7 +15,8 @@ import numpy as np
 __all__ = [
     "PNN_OK", "PNN_BF16", "PNN_FP32", "PNN_FP64", "PNN_ENERGY", "PNN_FORCES", "PnnError", "pnn_config", "lib",
     "lib_path", "pnn_status_string", "pnn_last_cuda_error", "pnn_weights_count", "pnn_model_create",
-    "pnn_model_destroy", "pnn_workspace_create", "pnn_workspace_destroy", "pnn_workspace_bytes", "pnn_build_graph",
+    "pnn_model_destroy", "pnn_branch_mlp_create", "pnn_branch_mlp_destroy", "pnn_branch_weights",
+    "pnn_workspace_create", "pnn_workspace_destroy", "pnn_workspace_bytes", "pnn_build_graph",
     "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_eval_blended", "pnn_eval_host", "pnn_check_async_errors", "pnn_launch_count", "pnn_profile_enable",
     "pnn_profile_read", "pnn_gemm_bf16",
     "PaiNN", "PRECISIONS",
@@ -79,6 +80,10 @@ def lib():
         L.pnn_eval.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, i32, vp, vp, vp]
         L.pnn_eval_blended.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, ctypes.c_double, i32, vp, vp, vp]
         L.pnn_eval_host.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp]
+        L.pnn_branch_mlp_create.argtypes = [i32, vp, vp, i64, i32, ctypes.POINTER(vp)]
+        L.pnn_branch_mlp_destroy.argtypes = [vp]
+        L.pnn_branch_mlp_destroy.restype = None
+        L.pnn_branch_weights.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp]
         L.pnn_check_async_errors.argtypes = [vp]
         L.pnn_profile_enable.argtypes = [vp, i32]
         L.pnn_profile_read.argtypes = [vp, i32, vp, vp, vp, ctypes.POINTER(i32)]
@@ -177,6 +182,24 @@ def pnn_eval_blended(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, 
            "pnn_eval_blended")
 
 
+def pnn_branch_mlp_create(widths, params_host: np.ndarray, prec: int) -> int:
+    w = np.ascontiguousarray(widths, dtype=np.int32)
+    p = np.ascontiguousarray(params_host, dtype=np.float64)
+    out = ctypes.c_void_p()
+    _check(lib().pnn_branch_mlp_create(int(w.size) - 1, w.ctypes.data, p.ctypes.data, p.size, int(prec),
+                                       ctypes.byref(out)), "pnn_branch_mlp_create")
+    return out.value
+
+
+def pnn_branch_mlp_destroy(b: int) -> None:
+    lib().pnn_branch_mlp_destroy(b)
+
+
+def pnn_branch_weights(b: int, ws: int, n_atoms: int, n_structs: int, Z, struct_ptr, head_weights, stream=None):
+    _check(lib().pnn_branch_weights(b, ws, n_atoms, n_structs, _ptr(Z), _ptr(struct_ptr), _ptr(head_weights), stream),
+           "pnn_branch_weights")
+
+
 def pnn_eval_host(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, struct_ptr, head, cell, pbc,
                   flags: int, energy_host, forces_host=None, stream=None):
     _check(lib().pnn_eval_host(model, ws, n_atoms, n_structs, _ptr(Z), _ptr(pos), _ptr(struct_ptr), _ptr(head),
@@ -233,6 +256,9 @@ class PaiNN:
         self.max_atoms, self.max_edges, self.max_structs = max_atoms, max_edges, max_structs
 
     def close(self):
+        if getattr(self, "branch_mlp", None):
+            pnn_branch_mlp_destroy(self.branch_mlp)
+            self.branch_mlp = None
         if getattr(self, "ws", None):
             pnn_workspace_destroy(self.ws)
             self.ws = None
@@ -304,6 +330,24 @@ class PaiNN:
         pnn_eval_blended(self.model, self.ws, N, S, Z, pos, struct_ptr, head_weights, skip_below, flags, energy, frc,
                          self._stream())
         return energy, frc
+
+    def set_branch_mlp(self, widths, params: np.ndarray):
+        """Uploads the composition -> softmax router; widths[-1] must equal H."""
+        if int(widths[-1]) != self.cfg.H:
+            raise ValueError("the router's last width must equal the number of heads")
+        if getattr(self, "branch_mlp", None):
+            pnn_branch_mlp_destroy(self.branch_mlp)
+        self.branch_mlp = pnn_branch_mlp_create(widths, params, self.cfg.prec)
+
+    def branch_weights(self, Z, struct_ptr):
+        """[S,H] CUDA tensor of branch weights in the model's output dtype (the input of eval_blended)."""
+        import torch
+        if not getattr(self, "branch_mlp", None):
+            raise RuntimeError("set_branch_mlp first")
+        N, S = int(Z.shape[0]), int(struct_ptr.shape[0]) - 1
+        hw = torch.empty((S, self.cfg.H), dtype=self.out_dtype, device=Z.device)
+        pnn_branch_weights(self.branch_mlp, self.ws, N, S, Z, struct_ptr, hw, self._stream())
+        return hw
 
     def eval_host(self, Z, pos, struct_ptr, head, cell=None, pbc=None, forces: Optional[bool] = None,
                   energy_out=None, forces_out=None):

@@ -1,0 +1,99 @@
+// branch.cu — composition-conditioned branch weights (reading Q28): per structure
+// the element fractions c (histogram of Z over the structure's atoms), a small MLP with SiLU hidden layers, and a softmax
+// over the heads.  24.5 k parameters: the whole router lives in L2 / L1; one CTA evaluates SPB structures so that every
+// weight it reads is used SPB times, thread o owns output unit o of the current layer (weights stored input-major on the
+// device, so a warp reads 32 consecutive outputs of one input row).
+#include "common.cuh"
+
+namespace pnn {
+
+namespace {
+constexpr int BR_MAXW = 256;   // widest layer (include/pnn.h)
+constexpr int BR_SPB = 4;      // structures per CTA
+constexpr int BR_THREADS = 128;
+
+template <typename T>
+__global__ void __launch_bounds__(BR_THREADS) branch_mlp_k(int S, BranchMlpDims dm, const int32_t* __restrict__ Z,
+                                                           const int32_t* __restrict__ sptr,
+                                                           const T* __restrict__ params, T* __restrict__ out,
+                                                           int* __restrict__ d_err) {
+  __shared__ T xa[BR_SPB][BR_MAXW];
+  __shared__ T xb[BR_SPB][BR_MAXW];
+  __shared__ int cnt[BR_SPB][BR_MAXW];
+  const int tid = threadIdx.x;
+  const int g0 = blockIdx.x * BR_SPB;
+  const int W0 = dm.width[0];
+
+  for (int i = tid; i < BR_SPB * BR_MAXW; i += BR_THREADS) (&cnt[0][0])[i] = 0;
+  __syncthreads();
+  bool bad = false;
+  for (int s = 0; s < BR_SPB; ++s) {
+    const int g = g0 + s;
+    if (g >= S) break;
+    const int a0 = sptr[g], a1 = sptr[g + 1];
+    for (int a = a0 + tid; a < a1; a += BR_THREADS) {
+      const int z = Z[a];
+      if (z < 1 || z > W0) { bad = true; continue; }
+      atomicAdd(&cnt[s][z - 1], 1);
+    }
+  }
+  if (bad) atomicOr(d_err, ERRF_BAD_Z);
+  __syncthreads();
+  for (int s = 0; s < BR_SPB; ++s) {
+    const int g = g0 + s;
+    const int n = g < S ? sptr[g + 1] - sptr[g] : 0;
+    for (int i = tid; i < W0; i += BR_THREADS) xa[s][i] = n > 0 ? T(cnt[s][i]) / T(n) : T(0);
+  }
+  __syncthreads();
+
+  T(*xin)[BR_MAXW] = xa;
+  T(*xout)[BR_MAXW] = xb;
+  for (int l = 0; l < dm.n_layers; ++l) {
+    const int n_in = dm.width[l], n_out = dm.width[l + 1];
+    const T* __restrict__ Wt = params + dm.off_w[l];      // [n_in][n_out]
+    const T* __restrict__ bl = params + dm.off_b[l];
+    const bool last = l + 1 == dm.n_layers;
+    for (int o = tid; o < n_out; o += BR_THREADS) {
+      T acc[BR_SPB];
+#pragma unroll
+      for (int s = 0; s < BR_SPB; ++s) acc[s] = bl[o];
+      for (int i = 0; i < n_in; ++i) {
+        const T w = Wt[(size_t)i * n_out + o];
+#pragma unroll
+        for (int s = 0; s < BR_SPB; ++s) acc[s] = fma(w, xin[s][i], acc[s]);
+      }
+#pragma unroll
+      for (int s = 0; s < BR_SPB; ++s) xout[s][o] = last ? acc[s] : silu_f<T>(acc[s]);
+    }
+    __syncthreads();
+    T(*t)[BR_MAXW] = xin; xin = xout; xout = t;
+  }
+
+  // softmax over the heads (xin holds the logits): one thread per structure, H <= 256 terms
+  const int H = dm.width[dm.n_layers];
+  if (tid < BR_SPB && g0 + tid < S) {
+    const T* lg = xin[tid];
+    T mx = lg[0];
+    for (int h = 1; h < H; ++h) mx = lg[h] > mx ? lg[h] : mx;
+    T sum = T(0);
+    for (int h = 0; h < H; ++h) sum += exp(lg[h] - mx);
+    T* o = out + (size_t)(g0 + tid) * H;
+    for (int h = 0; h < H; ++h) o[h] = exp(lg[h] - mx) / sum;
+  }
+}
+} // namespace
+
+template <typename T>
+int launch_branch_mlp(int64_t S, const BranchMlpDims& dm, const int32_t* Z, const int32_t* sptr, const T* params,
+                      T* out, int* d_err, cudaStream_t st) {
+  if (S <= 0) return 0;
+  branch_mlp_k<T><<<(unsigned)((S + BR_SPB - 1) / BR_SPB), BR_THREADS, 0, st>>>((int)S, dm, Z, sptr, params, out, d_err);
+  PNN_KCHECK("branch_mlp_k");
+  return 1;
+}
+template int launch_branch_mlp<float>(int64_t, const BranchMlpDims&, const int32_t*, const int32_t*, const float*,
+                                      float*, int*, cudaStream_t);
+template int launch_branch_mlp<double>(int64_t, const BranchMlpDims&, const int32_t*, const int32_t*, const double*,
+                                       double*, int*, cudaStream_t);
+
+} // namespace pnn

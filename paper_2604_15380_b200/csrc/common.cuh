@@ -209,4 +209,16 @@ int launch_readout_bwd(int64_t N, int F, int H, const T* opre, const int32_t* a2
 template <typename T>
 int launch_force_assemble(int64_t N, int nslab, const T* fpart, T* forces, cudaStream_t st);
 
+// ---- branch.cu: composition -> softmax branch weights -------------------------------
+// Device parameter layout: per layer Wt [in][out] (input-major, i.e. the transpose of the C ABI's [out][in]) at off_w[l],
+// then b [out] at off_b[l].
+struct BranchMlpDims {
+  int n_layers;
+  int width[9];
+  int off_w[8], off_b[8];
+};
+template <typename T>
+int launch_branch_mlp(int64_t S, const BranchMlpDims& dm, const int32_t* Z, const int32_t* sptr, const T* params,
+                      T* out, int* d_err, cudaStream_t st);
+
 } // namespace pnn

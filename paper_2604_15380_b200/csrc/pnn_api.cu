@@ -855,6 +855,75 @@ int pnn_eval_blended(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S
   return eval_common(m, ws, N, S, Z, sptr, nullptr, head_weights, skip_below, flags, energy, forces, stream);
 }
 
+struct pnn_branch_mlp {
+  BranchMlpDims dm{};
+  int prec = PNN_FP32;
+  void* d_params = nullptr;
+};
+
+int pnn_branch_mlp_create(int32_t n_layers, const int32_t* widths, const double* params, int64_t n_params, int prec,
+                          pnn_branch_mlp** out) {
+  if (!widths || !params || !out || n_layers < 1 || n_layers > 8) return PNN_ERR_INVALID_ARG;
+  if (prec != PNN_BF16 && prec != PNN_FP32 && prec != PNN_FP64) return PNN_ERR_INVALID_ARG;
+  int64_t n = 0;
+  for (int l = 0; l <= n_layers; ++l)
+    if (widths[l] < 1 || widths[l] > 256) return PNN_ERR_INVALID_ARG;
+  for (int l = 0; l < n_layers; ++l) n += (int64_t)widths[l + 1] * widths[l] + widths[l + 1];
+  if (n != n_params) return PNN_ERR_INVALID_ARG;
+  pnn_branch_mlp* b = new (std::nothrow) pnn_branch_mlp;
+  if (!b) return PNN_ERR_INVALID_ARG;
+  b->prec = prec;
+  b->dm.n_layers = n_layers;
+  for (int l = 0; l <= n_layers; ++l) b->dm.width[l] = widths[l];
+  // device layout: per layer Wt [in][out], b [out] (branch.cu reads 32 consecutive outputs of one input per warp)
+  std::vector<double> t((size_t)n);
+  int64_t off = 0;
+  for (int l = 0; l < n_layers; ++l) {
+    const int ni = widths[l], no = widths[l + 1];
+    b->dm.off_w[l] = (int)off;
+    for (int o = 0; o < no; ++o)
+      for (int i = 0; i < ni; ++i) t[(size_t)off + (size_t)i * no + o] = params[off + (int64_t)o * ni + i];
+    off += (int64_t)no * ni;
+    b->dm.off_b[l] = (int)off;
+    for (int o = 0; o < no; ++o) t[(size_t)off + o] = params[off + o];
+    off += no;
+  }
+  const size_t es = prec == PNN_FP64 ? 8 : 4;
+  if (!cuda_ok(cudaMalloc(&b->d_params, (size_t)n * es), "cudaMalloc(branch mlp)")) { delete b; return PNN_ERR_CUDA; }
+  cudaError_t e;
+  if (prec == PNN_FP64) {
+    e = cudaMemcpy(b->d_params, t.data(), (size_t)n * 8, cudaMemcpyHostToDevice);
+  } else {
+    std::vector<float> tf((size_t)n);
+    for (size_t i = 0; i < (size_t)n; ++i) tf[i] = (float)t[i];
+    e = cudaMemcpy(b->d_params, tf.data(), (size_t)n * 4, cudaMemcpyHostToDevice);
+  }
+  if (!cuda_ok(e, "cudaMemcpy(branch mlp)")) { cudaFree(b->d_params); delete b; return PNN_ERR_CUDA; }
+  *out = b;
+  return PNN_OK;
+}
+
+void pnn_branch_mlp_destroy(pnn_branch_mlp* b) {
+  if (!b) return;
+  cudaFree(b->d_params);
+  delete b;
+}
+
+int pnn_branch_weights(const pnn_branch_mlp* b, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z,
+                       const int32_t* sptr, void* head_weights, void* stream) {
+  if (!b || !ws || N < 0 || S < 0 || S > 0x7fffffffLL / 4) return PNN_ERR_INVALID_ARG;
+  if ((N > 0 && !Z) || !sptr || (S > 0 && !head_weights)) return PNN_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  int nl;
+  if (b->prec == PNN_FP64)
+    nl = launch_branch_mlp<double>(S, b->dm, Z, sptr, (const double*)b->d_params, (double*)head_weights, ws->g.d_err, st);
+  else
+    nl = launch_branch_mlp<float>(S, b->dm, Z, sptr, (const float*)b->d_params, (float*)head_weights, ws->g.d_err, st);
+  ws->launches += nl;
+  if (launch_failed()) return PNN_ERR_CUDA;
+  return PNN_OK;
+}
+
 int pnn_eval_host(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const double* pos,
                   const int32_t* sptr, const int32_t* head, const double* cell, const uint8_t* pbc, int flags,
                   void* energy_host, void* forces_host, void* stream) {
