@@ -7,6 +7,7 @@
 // global->register->shared pipeline.  The BF16 model uses gemm_tc.cu (tcgen05 + TMA + TMEM) instead.
 // Epilogues fuse what follows each Linear in SURVEY.md §8(c): bias, SiLU (+ store of the pre-activation for the
 // reverse sweep), multiplication by silu'(stored pre-activation), and accumulation into C (residual adjoints).
+#include <cstdlib>
 #include "common.cuh"
 
 namespace pnn {
@@ -51,8 +52,8 @@ __device__ __forceinline__ void mac_tile<float, 8, 8>(const float (&a)[8], const
   }
 }
 
-template <typename T, int BM, int BN, int TM, int TN, int BK>
-__global__ void __launch_bounds__((BM / TM) * (BN / TN))
+template <typename T, int BM, int BN, int TM, int TN, int BK, int MINB = 0>
+__global__ void __launch_bounds__((BM / TM) * (BN / TN), MINB)
 gemm_k(int64_t M, int N, int K, const T* __restrict__ A, int64_t lda, const T* __restrict__ B, int64_t ldb,
        T* __restrict__ C, int64_t ldc, GemmEpi<T> epi) {
   constexpr int NT = (BM / TM) * (BN / TN);
@@ -67,7 +68,12 @@ gemm_k(int64_t M, int N, int K, const T* __restrict__ A, int64_t lda, const T* _
   __shared__ __align__(32) T Bs[2][BK][BN + PAD];
 
   const int tid = threadIdx.x;
-  const int tx = tid % (BN / TN), ty = tid / (BN / TN);
+  // A warp covers 8 x 4 threads (not 16 x 2): its LDS.128 of the B row touches 8 distinct 16-byte chunks (one 128-byte
+  // wavefront, not two) and its A read 4 chunks (one wavefront) — the shared-memory pipe is what binds the 4x4 tile.
+  constexpr int TXN = BN / TN;
+  static_assert(TXN % 8 == 0 && (BM / TM) % 4 == 0, "thread grid in units of 8 x 4 warps");
+  const int lane = tid & 31, wrp = tid >> 5;
+  const int tx = (wrp % (TXN / 8)) * 8 + (lane & 7), ty = (wrp / (TXN / 8)) * 4 + (lane >> 3);
   const int64_t m0 = (int64_t)blockIdx.x * BM;
   const int n0 = blockIdx.y * BN;
 
@@ -186,14 +192,29 @@ template <typename T>
 int launch_gemm(int64_t M, int N, int K, const T* A, int64_t lda, const T* B, int64_t ldb, T* C, int64_t ldc,
                 const GemmEpi<T>& epi, cudaStream_t st) {
   if (M <= 0) return 0;
-  // Large problems: 128x128 tiles (8x8 per thread).  Small ones (fewer than ~2 waves of big tiles): 64x64.
-  const int64_t big_tiles = ((M + 127) / 128) * ((N + 127) / 128);
-  if (big_tiles >= 2 * 148 && N >= 128) {
-    dim3 grid((unsigned)((M + 127) / 128), (unsigned)((N + 127) / 128));
-    gemm_k<T, 128, 128, 8, 8, (sizeof(T) == 8 ? 8 : 16)><<<grid, 256, 0, st>>>(M, N, K, A, lda, B, ldb, C, ldc, epi); PNN_KCHECK("gemm_k");
+  if constexpr (sizeof(T) == 4) {
+    // FP32: 64x128 tiles, 128 threads, 8x8 per thread (4 LDS.128 per 32 packed FMAs; 154 registers -> 3 CTAs per SM)
+    // once there are two CTAs per SM; below that 64x64 tiles with 4x4 per thread (four times the warps, but two
+    // LDS.128 per 8 packed FMAs: the shared-memory pipe binds it at ~28 TFLOP/s against ~50 for the 8x8 tile;
+    // B200 measurements in DESIGN.md section 10).
+    const int64_t wide_tiles = ((M + 63) / 64) * ((N + 127) / 128);
+    if (N >= 128 && wide_tiles >= 2 * 148) {
+      dim3 grid((unsigned)((M + 63) / 64), (unsigned)((N + 127) / 128));
+      gemm_k<T, 64, 128, 8, 8, 16, 3><<<grid, 128, 0, st>>>(M, N, K, A, lda, B, ldb, C, ldc, epi); PNN_KCHECK("gemm_k");
+    } else {
+      dim3 grid((unsigned)((M + 63) / 64), (unsigned)((N + 63) / 64));
+      gemm_k<T, 64, 64, 4, 4, 16><<<grid, 256, 0, st>>>(M, N, K, A, lda, B, ldb, C, ldc, epi); PNN_KCHECK("gemm_k");
+    }
   } else {
-    dim3 grid((unsigned)((M + 63) / 64), (unsigned)((N + 63) / 64));
-    gemm_k<T, 64, 64, 4, 4, 16><<<grid, 256, 0, st>>>(M, N, K, A, lda, B, ldb, C, ldc, epi); PNN_KCHECK("gemm_k");
+    // FP64: 128x128 tiles (8x8 per thread) for large problems, 64x64 (4x4) below ~2 waves of big tiles.
+    const int64_t big_tiles = ((M + 127) / 128) * ((N + 127) / 128);
+    if (big_tiles >= 2 * 148 && N >= 128) {
+      dim3 grid((unsigned)((M + 127) / 128), (unsigned)((N + 127) / 128));
+      gemm_k<T, 128, 128, 8, 8, 8><<<grid, 256, 0, st>>>(M, N, K, A, lda, B, ldb, C, ldc, epi); PNN_KCHECK("gemm_k");
+    } else {
+      dim3 grid((unsigned)((M + 63) / 64), (unsigned)((N + 63) / 64));
+      gemm_k<T, 64, 64, 4, 4, 16><<<grid, 256, 0, st>>>(M, N, K, A, lda, B, ldb, C, ldc, epi); PNN_KCHECK("gemm_k");
+    }
   }
   return 1;
 }
