@@ -7,7 +7,6 @@
 // global->register->shared pipeline.  The BF16 model uses gemm_tc.cu (tcgen05 + TMA + TMEM) instead.
 // Epilogues fuse what follows each Linear in SURVEY.md §8(c): bias, SiLU (+ store of the pre-activation for the
 // reverse sweep), multiplication by silu'(stored pre-activation), and accumulation into C (residual adjoints).
-#include <cstdlib>
 #include "common.cuh"
 
 namespace pnn {
@@ -27,30 +26,20 @@ __device__ __forceinline__ void mac_tile(const T (&a)[TM], const T (&b)[TN], T (
 #pragma unroll
     for (int j = 0; j < TN; ++j) acc[i][j] = fma(a[i], b[j], acc[i][j]);
 }
-template <>
-__device__ __forceinline__ void mac_tile<float, 4, 4>(const float (&a)[4], const float (&b)[4], float (&acc)[4][4]) {
+template <int TM, int TN>
+__device__ __forceinline__ void mac_tile_f2(const float (&a)[TM], const float (&b)[TN], float (&acc)[TM][TN]) {
 #pragma unroll
-  for (int i = 0; i < 4; ++i) {
+  for (int i = 0; i < TM; ++i) {
     const float2 ai = make_float2(a[i], a[i]);
 #pragma unroll
-    for (int j = 0; j < 4; j += 2) {
+    for (int j = 0; j < TN; j += 2) {
       const float2 r = __ffma2_rn(ai, make_float2(b[j], b[j + 1]), make_float2(acc[i][j], acc[i][j + 1]));
       acc[i][j] = r.x; acc[i][j + 1] = r.y;
     }
   }
 }
-template <>
-__device__ __forceinline__ void mac_tile<float, 8, 8>(const float (&a)[8], const float (&b)[8], float (&acc)[8][8]) {
-#pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    const float2 ai = make_float2(a[i], a[i]);
-#pragma unroll
-    for (int j = 0; j < 8; j += 2) {
-      const float2 r = __ffma2_rn(ai, make_float2(b[j], b[j + 1]), make_float2(acc[i][j], acc[i][j + 1]));
-      acc[i][j] = r.x; acc[i][j + 1] = r.y;
-    }
-  }
-}
+template <> __device__ __forceinline__ void mac_tile<float, 4, 4>(const float (&a)[4], const float (&b)[4], float (&acc)[4][4]) { mac_tile_f2<4, 4>(a, b, acc); }
+template <> __device__ __forceinline__ void mac_tile<float, 8, 8>(const float (&a)[8], const float (&b)[8], float (&acc)[8][8]) { mac_tile_f2<8, 8>(a, b, acc); }
 
 template <typename T, int BM, int BN, int TM, int TN, int BK, int MINB = 0>
 __global__ void __launch_bounds__((BM / TM) * (BN / TN), MINB)

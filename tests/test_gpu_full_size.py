@@ -1,0 +1,134 @@
+"""-m gpu: the CUDA path at BASELINE.json's FULL sizes, in the launch configurations bench.py times (same batch recipe,
+same workspace caps), checked on sampled structures the oracle can evaluate one by one (structures are independent, so a
+structure's energy and forces do not depend on the rest of the batch) and, for the single 100,000-atom structure of
+cfg5 that the oracle cannot finish in seconds, on properties that hold at any size."""
+
+import numpy as np
+import pytest
+
+import gen
+import oracle
+from gpu_common import make_model, to_device
+from helpers import energy_rel_err, force_rel_err
+
+pytestmark = pytest.mark.gpu
+
+
+def run_full(cfg_id, precision, forces, S=None, start=0):
+    import torch
+    mc = gen.model_cfg(cfg_id)
+    S = S or gen.CONFIGS[cfg_id]["S"]
+    b = gen.make_batch(cfg_id, start, S)
+    w = gen.make_weights(mc, cfg_id)
+    deg_cap = 96 if cfg_id in (3, 5) else 40                      # bench.py's workspace caps
+    net = make_model(mc, w, precision, b.n_atoms, b.n_atoms * deg_cap, b.n_structs, forces)
+    try:
+        t = to_device(b)
+        e, f = net.eval(t["Z"], t["pos"], t["struct_ptr"], t["head"], t["cell"], t["pbc"], forces=forces)
+        torch.cuda.synchronize()
+        net.check()
+        return mc, w, b, e.double().cpu().numpy(), None if f is None else f.double().cpu().numpy()
+    finally:
+        net.close()
+
+
+def sub_batch(b, ids):
+    parts = []
+    for g in ids:
+        a0, a1 = b.struct_ptr[g], b.struct_ptr[g + 1]
+        parts.append(gen.Batch(b.Z[a0:a1], b.pos[a0:a1], np.array([0, a1 - a0], np.int32), b.head[g:g + 1],
+                               None if b.cell is None else b.cell[g:g + 1], None if b.pbc is None else b.pbc[g:g + 1]))
+    return gen.concat_batches(parts)
+
+
+def sampled(b, e, f, ids):
+    sel = np.concatenate([np.arange(b.struct_ptr[g], b.struct_ptr[g + 1]) for g in ids])
+    return e[ids], None if f is None else f[sel]
+
+
+@pytest.mark.parametrize("precision,te,tf", [("fp32", 1e-5, 1e-4), ("fp64", 1e-10, 1e-10)])
+def test_cfg2_full_batch_sampled_structures(precision, te, tf):
+    """bench.py's headline workload: all 256 molecules in one call."""
+    mc, w, b, e, f = run_full(2, precision, True)
+    assert b.n_structs == 256
+    ids = [0, 37, 101, 128, 200, 255]
+    sb = sub_batch(b, ids)
+    ref = oracle.evaluate(mc, w, sb)
+    es, fs = sampled(b, e, f, ids)
+    # Q20 denominators over the sample
+    assert energy_rel_err(es, ref["energy"]).max() < te
+    assert force_rel_err(fs, ref["forces"], sb.struct_ptr).max() < tf
+    # every structure of the batch: finite, and zero net force (non-periodic) relative to its force scale
+    assert np.isfinite(e).all() and np.isfinite(f).all()
+    tol = 1e-4 if precision == "fp32" else 1e-10
+    for g in range(b.n_structs):
+        fg = f[b.struct_ptr[g]:b.struct_ptr[g + 1]]
+        assert np.abs(fg.sum(0)).max() < tol * max(np.abs(fg).sum(0).max(), 1e-30)
+
+
+def test_cfg3_full_batch_sampled_structures_fp64():
+    mc, w, b, e, f = run_full(3, "fp64", True)
+    assert b.n_structs == 64
+    ids = [5, 63]
+    sb = sub_batch(b, ids)
+    ref = oracle.evaluate(mc, w, sb)
+    es, fs = sampled(b, e, f, ids)
+    assert energy_rel_err(es, ref["energy"]).max() < 1e-10
+    assert force_rel_err(fs, ref["forces"], sb.struct_ptr).max() < 1e-10
+
+
+def test_cfg4_bench_batch_bf16_sampled_structures():
+    """bench.py --workload cfg4: 16,384 molecules per call, BF16, energy only."""
+    mc, w, b, e, _ = run_full(4, "bf16", False, S=16384)
+    ids = [0, 1, 4097, 8191, 12000, 16383, 3, 777, 9999, 15000, 2048, 6000]
+    sb = sub_batch(b, ids)
+    ref = oracle.evaluate(mc, w, sb, forces=False)
+    es = e[ids]
+    assert float(np.sqrt(((es - ref["energy"]) ** 2).sum() / (ref["energy"] ** 2).sum())) < 2e-2
+    assert energy_rel_err(es, ref["energy"]).max() < 6e-2
+    assert np.isfinite(e).all()
+
+
+def test_cfg5_full_size_fp64_properties():
+    """One periodic structure of 100,000 atoms (4.9 M edges): no oracle run at this size; properties that hold at any
+    size pin the result instead — (i) zero net force, (ii) invariance under a rigid translation and under moving atoms
+    by lattice vectors, (iii) forces = -dE/dx by central differences of the GPU energy on sampled atoms (the oracle's
+    own forces are pinned the same way on CPU)."""
+    import torch
+    cfg_id = 5
+    mc = gen.model_cfg(cfg_id)
+    b = gen.make_batch(cfg_id)
+    w = gen.make_weights(mc, cfg_id)
+    assert b.n_atoms == 100000
+    net = make_model(mc, w, "fp64", b.n_atoms, b.n_atoms * 96, 1, True)
+    try:
+        t = to_device(b)
+
+        def ev(pos, forces=True):
+            e, f = net.eval(t["Z"], pos, t["struct_ptr"], t["head"], t["cell"], t["pbc"], forces=forces)
+            torch.cuda.synchronize()
+            net.check()
+            return float(e[0]), None if f is None else f.cpu().numpy()
+
+        E0, F0 = ev(t["pos"])
+        assert np.isfinite(E0) and np.isfinite(F0).all()
+        scale = np.abs(F0).sum(0).max()
+        assert np.abs(F0.sum(0)).max() < 1e-10 * scale                                       # (i)
+        rng = np.random.default_rng(0)
+        shift = torch.tensor(rng.normal(size=3), device="cuda")
+        E1, F1 = ev(t["pos"] + shift)                                                          # (ii) translation
+        assert abs(E1 - E0) < 1e-9 * abs(E0) and np.abs(F1 - F0).max() < 1e-8 * np.abs(F0).max()
+        n = torch.tensor(rng.integers(-2, 3, (b.n_atoms, 3)).astype(np.float64), device="cuda")
+        E2, F2 = ev(t["pos"] + n @ t["cell"][0])                                               # (ii) lattice moves
+        assert abs(E2 - E0) < 1e-9 * abs(E0) and np.abs(F2 - F0).max() < 1e-8 * np.abs(F0).max()
+        h = 1e-5                                                                               # (iii)
+        for a, c in [(0, 0), (31415, 1), (99999, 2)]:
+            p = t["pos"].clone()
+            p[a, c] += h
+            Ep, _ = ev(p, forces=False)
+            p[a, c] -= 2 * h
+            Em, _ = ev(p, forces=False)
+            fd = -(Ep - Em) / (2 * h)
+            assert abs(fd - F0[a, c]) < 1e-5 * np.abs(F0).max(), (a, c, fd, F0[a, c])
+    finally:
+        net.close()
