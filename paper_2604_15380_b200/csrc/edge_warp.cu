@@ -91,7 +91,7 @@ __device__ __forceinline__ void load_rows(const EdgeArgs<float>& a, int f0, floa
 // TAPE: also evaluate dw/dd and keep w and dw/dd of every (edge, chunk, feature) for the reverse sweep
 // (wt, dt: [E][3][F]), so that the reverse edge kernel does no filter arithmetic at all.
 template <int KP, int FPL, int NWARP, bool TAPE>
-__global__ void __launch_bounds__(NWARP * 32, FPL == 1 ? 3 : 2)
+__global__ void __launch_bounds__(NWARP * 32, (FPL == 1 && KP <= 24) ? 3 : 2)
 edge_fwd_w_k(EdgeArgs<float> a, int RB, const float* __restrict__ phi, const float* __restrict__ s_in, int64_t ld_sin,
              const float* __restrict__ v_in, float* __restrict__ s1, int64_t ld_s1, float* __restrict__ v1,
              float* __restrict__ wt, float* __restrict__ dt) {
@@ -318,7 +318,11 @@ edge_bwd_w_k(EdgeArgs<float> a, int RB, const float* __restrict__ phi, const flo
 static int pick_fpl(int F, int K) { return (K <= 20 && F % 64 == 0) ? 2 : 1; }
 static int pick_kp4(int K) { return K <= 8 ? 8 : K <= 12 ? 12 : K <= 16 ? 16 : K <= 20 ? 20 : K <= 24 ? 24 : K <= 28 ? 28 : 32; }
 
-int edge_warp_num_slabs(int F, int K) { return F / (32 * pick_fpl(F, K)); }
+// The reverse kernel holds no filter rows: its lane width is chosen on its own (the tape layout [E][3][F] is lane-agnostic).
+// Two features (8-byte loads) per lane whenever F allows: cfg3 (F = 256, K = 32) 1.00 -> 0.76 ms against one feature.
+static int pick_fpl_bwd(int F) { return F % 64 == 0 ? 2 : 1; }
+
+int edge_warp_num_slabs(int F, int K) { (void)K; return F / (32 * pick_fpl_bwd(F)); }
 
 int launch_edge_fwd_warp(const EdgeArgs<float>& a, const float* phi, const float* s_in, int64_t ld_sin, const float* v_in,
                          float* s1, int64_t ld_s1, float* v1, float* wt, float* dt, cudaStream_t st) {
@@ -360,7 +364,7 @@ int launch_edge_bwd_warp(const EdgeArgs<float>& a, const float* phi, const float
                          const float* wt, const float* dt, float* phib, float* vb_in, float* fpart, int first_block,
                          cudaStream_t st) {
   if (a.N == 0) return 0;
-  const int FPL = pick_fpl(a.F, a.K);
+  const int FPL = pick_fpl_bwd(a.F);
   constexpr int NW = 4;
   const int RB = 16;
   const int64_t nchunk = (a.N + RB - 1) / RB;
