@@ -554,7 +554,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       v_out = (t + 1 < T_) ? (T*)ws->vping[t & 1] : nullptr;
     }
     T* phi = (T*)tp.phi; T* PQ = (T*)tp.PQ; T* a = (T*)tp.a;
-    GemmEpi<T> e1; e1.bias = W + b.b1; e1.act = ACT_SILU; e1.pre = (T*)tp.hpre; e1.ldpre = F;
+    GemmEpi<T> e1; e1.bias = W + b.b1; e1.act = ACT_SILU; e1.pre = want_f ? (T*)tp.hpre : nullptr; e1.ldpre = F;
     { ProfScope ps_(ws, st, "gemm_N");
     const int l_ = launch_gemm<T>(N, F, F, s_cur, F, W + b.W1t, F, h, F, e1, st);                 // B3a, first Linear + SiLU
       nl += l_; ps_.done(l_); }
@@ -581,7 +581,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     { ProfScope ps_(ws, st, "update_elementwise");
     const int l_ = launch_norm<T, T>(N, F, PQ, sn, (T)c.norm_eps, st);                               // n -> sn[:, F:]
       nl += l_; ps_.done(l_); }
-    GemmEpi<T> e4; e4.bias = W + b.c1; e4.act = ACT_SILU; e4.pre = (T*)tp.kpre; e4.ldpre = F;
+    GemmEpi<T> e4; e4.bias = W + b.c1; e4.act = ACT_SILU; e4.pre = want_f ? (T*)tp.kpre : nullptr; e4.ldpre = F;
     { ProfScope ps_(ws, st, "gemm_N");
     const int l_ = launch_gemm<T>(N, F, 2 * F, sn, 2 * F, W + b.A1t, F, k, F, e4, st);
       nl += l_; ps_.done(l_); }
@@ -723,7 +723,7 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       v_out16 = (t + 1 < T_) ? mb.vping16[t & 1] : nullptr;
     }
     B* PQ = (B*)tp.PQ; B* a = (B*)tp.a;   // P | Q and the gate values are kept in BF16 (tape included)
-    TcEpi e1; e1.bias = W + b.b1; e1.act = ACT_SILU; e1.pre = (T*)tp.hpre; e1.ldpre = F; e1.Cb = mb.h16; e1.ldcb = F;
+    TcEpi e1; e1.bias = W + b.b1; e1.act = ACT_SILU; e1.pre = want_f ? (T*)tp.hpre : nullptr; e1.ldpre = F; e1.Cb = mb.h16; e1.ldcb = F;
     tc("gemm_N", N, F, F, mb.s16, F, b.W1, e1);                                   // B3a: h = silu(W1 s + b1)
     TcEpi e2; e2.bias = W + b.b2; e2.Cb = tp16.phi16; e2.ldcb = 3 * F;
     tc("gemm_N", N, 3 * F, F, mb.h16, F, b.W2, e2);                               // B3a: phi = W2 h + b2
@@ -739,7 +739,7 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     { ProfScope ps_(ws, st, "update_elementwise");
       const int l_ = launch_norm<T, B>(N, F, PQ, sn, (T)c.norm_eps, st, mb.sn16);
       nl += l_; ps_.done(l_); }
-    TcEpi e4; e4.bias = W + b.c1; e4.act = ACT_SILU; e4.pre = (T*)tp.kpre; e4.ldpre = F; e4.Cb = mb.k16; e4.ldcb = F;
+    TcEpi e4; e4.bias = W + b.c1; e4.act = ACT_SILU; e4.pre = want_f ? (T*)tp.kpre : nullptr; e4.ldpre = F; e4.Cb = mb.k16; e4.ldcb = F;
     tc("gemm_N", N, F, 2 * F, mb.sn16, 2 * F, b.A1, e4);
     TcEpi e5; e5.bias = W + b.c2; e5.Cb = a; e5.ldcb = 3 * F;
     tc("gemm_N", N, 3 * F, F, mb.k16, F, b.A2, e5);
