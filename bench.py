@@ -357,17 +357,23 @@ def main():
         import oracle
         oracle.build()
         cfg_id, _, forces, _ = WORKLOADS[args.workload]
-        n_sample = {1: 8, 2: 64, 3: 2, 4: 128, 5: 1}[cfg_id]
+        # a bounded sample of the same workload, repeated until about 10 s of CPU work have been timed
+        n_sample = {1: 8, 2: 256, 3: 2, 4: 512, 5: 1}[cfg_id]
         sb = gen.make_batch(cfg_id, 0, n_sample) if cfg_id != 5 else gen.make_batch(5, n_atoms=3000)
         wts = gen.make_weights(mc, cfg_id)
         oracle.evaluate(mc, wts, sb.select([0]), forces=forces)   # page in
-        t0 = time.perf_counter()
-        o = oracle.evaluate(mc, wts, sb, forces=forces)
-        dt = time.perf_counter() - t0
-        line["cpu_baseline"] = dict(value=sb.n_structs / dt, unit="structures/s", cores=oracle.num_threads(),
-                                    kind="oracle", edges_per_s=o["n_edges"] / dt, seconds=dt,
-                                    sample=f"first {sb.n_structs} structures ({sb.n_atoms} atoms, {o['n_edges']} "
-                                           f"directed edges) of {WORKLOAD_NAMES[args.workload]}, FP64")
+        passes, t0 = 0, time.perf_counter()
+        while True:
+            o = oracle.evaluate(mc, wts, sb, forces=forces)
+            passes += 1
+            dt = time.perf_counter() - t0
+            if dt >= 10.0 or passes >= 1000:
+                break
+        line["cpu_baseline"] = dict(value=passes * sb.n_structs / dt, unit="structures/s", cores=oracle.num_threads(),
+                                    kind="oracle", edges_per_s=passes * o["n_edges"] / dt, seconds=dt,
+                                    sample=f"{passes} passes over the first {sb.n_structs} structures ({sb.n_atoms} "
+                                           f"atoms, {o['n_edges']} directed edges) of {WORKLOAD_NAMES[args.workload]}, "
+                                           f"FP64 oracle")
 
     if not args.no_extra and world == 1:
         extra = {}
