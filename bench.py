@@ -145,6 +145,16 @@ def run_reference(args, rank):
     """--impl reference: the CPU oracle, as it stands, on a bounded sample of the workload per step."""
     if rank != 0:
         return
+    # torchrun exports OMP_NUM_THREADS=1 to every rank; the other ranks have exited, so the oracle gets the host's cores
+    # here as it does in the N=1 launch (its OpenMP loops are unchanged: only the thread count is restored).
+    if os.environ.get("TORCHELASTIC_RUN_ID") and os.environ.get("OMP_NUM_THREADS") == "1":
+        try:
+            import ctypes
+            n_thr = len(os.sched_getaffinity(0))
+            os.environ["OMP_NUM_THREADS"] = str(n_thr)
+            ctypes.CDLL("libgomp.so.1").omp_set_num_threads(n_thr)
+        except Exception:
+            pass
     import oracle
     cfg_id, prec, forces, per_step = WORKLOADS[args.workload]
     mc = gen.model_cfg(cfg_id)
