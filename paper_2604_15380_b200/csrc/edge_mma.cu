@@ -706,7 +706,9 @@ int launch_edge_fwd_mma(const EdgeMmaArgs& a, const __nv_bfloat16* phi, const fl
                         const EdgeMirror& mir, cudaStream_t st) {
   if (a.N == 0) return 0;
   const int KP = edge_mma_kp(a.K), NSL = pick_nsl(a.F), NWARP = 8;
-  const int RB = 32;
+  // receivers per grid-stride chunk: ~8 chunks per CTA for small batches (cfg3, 8,192 atoms: 32 -> 8 receivers, 378 ->
+  // 337 us), 64 receivers for large ones (cfg4, 391 k atoms: 4.29 -> 4.26 ms)
+  const int RB = (int)std::min<int64_t>(64, std::max<int64_t>(NWARP, a.N / (148 * 2 * 8)));
   const int64_t nchunk = (a.N + RB - 1) / RB;
   dim3 grid((unsigned)std::min<int64_t>(nchunk, 148 * 2), a.F / 32 / NSL);
   const size_t smem = edge_mma_smem(KP, NSL, NWARP, false);
@@ -736,7 +738,7 @@ int launch_edge_bwd_mma(const EdgeMmaArgs& a, const __nv_bfloat16* phi, const __
                         float* vb_in, float* fpart, int first_block, cudaStream_t st) {
   if (a.N == 0) return 0;
   const int KP = edge_mma_kp(a.K), NSL = pick_nsl(a.F), NWARP = 4;
-  const int RB = 16;
+  const int RB = (int)std::min<int64_t>(16, std::max<int64_t>(8, a.N / (148 * 2 * 8)));   // cfg3: 16 -> 8, 930 -> 863 us
   const int64_t nchunk = (a.N + RB - 1) / RB;
   dim3 grid((unsigned)std::min<int64_t>(nchunk, 148 * 2), a.F / 32 / NSL);
   const size_t smem = edge_mma_smem(KP, NSL, NWARP, true);
