@@ -331,7 +331,12 @@ int launch_edge_fwd_warp(const EdgeArgs<float>& a, const float* phi, const float
   constexpr int NW = 4;
   const int RB = NW;   // one receiver per warp and chunk: finest grain for the grid-stride loop (16 measured 3 % slower)
   const int64_t nchunk = (a.N + RB - 1) / RB;
-  dim3 grid((unsigned)std::min<int64_t>(nchunk, 148 * 4), a.F / (32 * FPL));
+  // Persistent grid: a whole number of waves of resident CTAs (2 or 3 per SM by registers), shared out over the feature
+  // slabs — every extra CTA reloads its 3*FPL filter rows, and a partial wave leaves SMs idle.  Measured on B200, edge_fwd:
+  // cfg2 (F 128, K 20, 2 slabs) 148 x 2 CTAs 200 us, 111 x 2 255 us, 296 x 2 207 us, 592 x 2 220 us;
+  // cfg3 (F 256, K 32, 8 slabs) 37 x 8 CTAs 2.19 ms, 74 x 8 2.01 ms, 111 x 8 2.08 ms, 148 x 8 2.05 ms, 592 x 8 2.19 ms.
+  const int nslab = a.F / (32 * FPL), occ = (FPL == 1 && KP <= 24) ? 3 : 2, waves = FPL == 2 ? 1 : 2;
+  dim3 grid((unsigned)std::min<int64_t>(nchunk, std::max(1, 148 * occ * waves / nslab)), nslab);
 #define PNN_L(KPV, FPLV)                                                                                              \
   {                                                                                                                   \
     if (wt) edge_fwd_w_k<KPV, FPLV, NW, true><<<grid, NW * 32, 0, st>>>(a, RB, phi, s_in, ld_sin, v_in, s1, ld_s1, v1, wt, dt); \
@@ -368,7 +373,7 @@ int launch_edge_bwd_warp(const EdgeArgs<float>& a, const float* phi, const float
   constexpr int NW = 4;
   const int RB = NW;   // cfg2 0.160 -> 0.144 ms, cfg3 0.76 -> 0.73 ms against 16 receivers per chunk
   const int64_t nchunk = (a.N + RB - 1) / RB;
-  dim3 grid((unsigned)std::min<int64_t>(nchunk, 148 * 8), a.F / (32 * FPL));
+  dim3 grid((unsigned)std::min<int64_t>(nchunk, 148 * 16), a.F / (32 * FPL));
   if (FPL == 2)
     edge_bwd_w_k<2, NW><<<grid, NW * 32, 0, st>>>(a, RB, phi, v_in, sb1, vb1, wt, dt, phib, vb_in, fpart, first_block);
   else
