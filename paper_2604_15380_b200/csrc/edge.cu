@@ -355,7 +355,7 @@ int launch_edge_fwd(const EdgeArgs<T>& a, const PT* phi, const T* s_in, int64_t 
   if (a.N == 0) return 0;
   const int nslab = edge_num_slabs(a.F), FS = a.F / nslab, RB = pick_rb<T>(), KP = pick_kp(a.K);
   const int64_t nwork = (a.N + RB - 1) / RB;
-  dim3 grid((unsigned)std::min<int64_t>(nwork, 148 * 6), nslab);
+  dim3 grid((unsigned)std::min<int64_t>(nwork, 148 * 4), nslab);   // whole waves: cfg5 148*6 525 ms, 148*4 495 ms
   const size_t smem = sizeof(T) * (ET * KP + ET + ET * 4 + (size_t)RB * 7 * FS) + sizeof(int) * (ET + RB + 1);
 #define PNN_LAUNCH_FWD(KPV)                                                                                   \
   {                                                                                                           \
@@ -384,7 +384,7 @@ int launch_edge_bwd(const EdgeArgs<T>& a, const PT* phi, const PT* v_in, const T
   if (a.N == 0) return 0;
   const int nslab = edge_num_slabs(a.F), FS = a.F / nslab, RB = pick_rb<T>(), KP = pick_kp(a.K);
   const int64_t nwork = (a.N + RB - 1) / RB;
-  dim3 grid((unsigned)std::min<int64_t>(nwork, 148 * 6), nslab);
+  dim3 grid((unsigned)std::min<int64_t>(nwork, 148 * 4), nslab);   // whole waves: cfg5 148*6 525 ms, 148*4 495 ms
   const size_t smem = sizeof(T) * (2 * ET * KP + 2 * ET + ET * 4 + (size_t)RB * 5 * FS + RB * 12 * 3) +
                       sizeof(int) * (ET + RB + 1);
 #define PNN_LAUNCH_BWD(KPV)                                                                                   \
