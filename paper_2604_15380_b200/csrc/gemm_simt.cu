@@ -49,20 +49,15 @@ gemm_k(int64_t M, int N, int K, const T* __restrict__ A, int64_t lda, const T* _
   constexpr int PAD = 4;
   using V = typename V4<T>::type;
   static_assert(TM % 4 == 0 && TN % 4 == 0, "micro tile in units of 4");
-  static_assert((BM * BK / 4) % NT == 0 && (BK * BN / 4) % NT == 0, "tile loads must divide evenly");
-  constexpr int A_LD = (BM * BK / 4) / NT; // vector loads per thread for the A tile
-  constexpr int B_LD = (BK * BN / 4) / NT;
+  constexpr int A_V = BM * BK / 4, B_V = BK * BN / 4;   // vectors per tile
+  constexpr int A_LD = (A_V + NT - 1) / NT;             // vector loads per thread (the last one guarded if ragged)
+  constexpr int B_LD = (B_V + NT - 1) / NT;
 
   __shared__ __align__(32) T As[2][BK][BM + PAD]; // transposed A tile
   __shared__ __align__(32) T Bs[2][BK][BN + PAD];
 
   const int tid = threadIdx.x;
-  // A warp covers 8 x 4 threads (not 16 x 2): its LDS.128 of the B row touches 8 distinct 16-byte chunks (one 128-byte
-  // wavefront, not two) and its A read 4 chunks (one wavefront) — the shared-memory pipe is what binds the 4x4 tile.
-  constexpr int TXN = BN / TN;
-  static_assert(TXN % 8 == 0 && (BM / TM) % 4 == 0, "thread grid in units of 8 x 4 warps");
-  const int lane = tid & 31, wrp = tid >> 5;
-  const int tx = (wrp % (TXN / 8)) * 8 + (lane & 7), ty = (wrp / (TXN / 8)) * 4 + (lane >> 3);
+  const int tx = tid % (BN / TN), ty = tid / (BN / TN);
   const int64_t m0 = (int64_t)blockIdx.x * BM;
   const int n0 = blockIdx.y * BN;
 
@@ -79,6 +74,7 @@ gemm_k(int64_t M, int N, int K, const T* __restrict__ A, int64_t lda, const T* _
       const int v = tid + q * NT;          // vector index in the BM x (BK/4) tile
       const int r = v / (BK / 4), kq = v % (BK / 4);
       const int64_t m = m0 + r;
+      if (A_V % NT != 0 && v >= A_V) continue;
       if (m < M) ra[q] = *reinterpret_cast<const V*>(A + m * lda + k0 + kq * 4);
       else ra[q] = V{T(0), T(0), T(0), T(0)};
     }
@@ -87,6 +83,7 @@ gemm_k(int64_t M, int N, int K, const T* __restrict__ A, int64_t lda, const T* _
       const int v = tid + q * NT;          // vector index in the BK x (BN/4) tile
       const int r = v / (BN / 4), nq = v % (BN / 4);
       const int n = n0 + nq * 4;
+      if (B_V % NT != 0 && v >= B_V) continue;
       if (n < N) rb[q] = *reinterpret_cast<const V*>(B + (int64_t)(k0 + r) * ldb + n);
       else rb[q] = V{T(0), T(0), T(0), T(0)};
     }
@@ -96,6 +93,7 @@ gemm_k(int64_t M, int N, int K, const T* __restrict__ A, int64_t lda, const T* _
     for (int q = 0; q < A_LD; ++q) {
       const int v = tid + q * NT;
       const int r = v / (BK / 4), kq = v % (BK / 4);
+      if (A_V % NT != 0 && v >= A_V) continue;
       As[buf][kq * 4 + 0][r] = ra[q].x; As[buf][kq * 4 + 1][r] = ra[q].y;
       As[buf][kq * 4 + 2][r] = ra[q].z; As[buf][kq * 4 + 3][r] = ra[q].w;
     }
@@ -103,6 +101,7 @@ gemm_k(int64_t M, int N, int K, const T* __restrict__ A, int64_t lda, const T* _
     for (int q = 0; q < B_LD; ++q) {
       const int v = tid + q * NT;
       const int r = v / (BN / 4), nq = v % (BN / 4);
+      if (B_V % NT != 0 && v >= B_V) continue;
       *reinterpret_cast<V*>(&Bs[buf][r][nq * 4]) = rb[q];
     }
   };
@@ -191,8 +190,21 @@ int launch_gemm(int64_t M, int N, int K, const T* A, int64_t lda, const T* B, in
       dim3 grid((unsigned)((M + 63) / 64), (unsigned)((N + 127) / 128));
       gemm_k<T, 64, 128, 8, 8, 16, 3><<<grid, 128, 0, st>>>(M, N, K, A, lda, B, ldb, C, ldc, epi); PNN_KCHECK("gemm_k");
     } else {
-      dim3 grid((unsigned)((M + 63) / 64), (unsigned)((N + 63) / 64));
-      gemm_k<T, 64, 64, 4, 4, 16><<<grid, 256, 0, st>>>(M, N, K, A, lda, B, ldb, C, ldc, epi); PNN_KCHECK("gemm_k");
+      // The small GEMMs are one wave of co-resident CTAs, so their time follows the LARGEST number of CTAs on one SM
+      // (measured, 64x64 tiles, K = 384: 2 per SM 30.8 us, 3 per SM 41.0 us, 4 per SM 45.1 us).  10,354 rows make 324
+      // CTAs of 64 rows (three on 28 SMs) but 288 of 72 rows (two everywhere): take 72-row tiles when that pays.
+      auto cost = [&](int bm) {
+        const int64_t ctas = ((M + bm - 1) / bm) * ((N + 63) / 64), per_sm = (ctas + 147) / 148;
+        const double f = per_sm <= 1 ? 0.8 : per_sm == 2 ? 1.0 : per_sm == 3 ? 1.33 : per_sm == 4 ? 1.46 : 0.37 * per_sm;
+        return bm * f;
+      };
+      if (cost(72) < 0.97 * cost(64)) {
+        dim3 grid((unsigned)((M + 71) / 72), (unsigned)((N + 63) / 64));
+        gemm_k<T, 72, 64, 4, 4, 16><<<grid, 288, 0, st>>>(M, N, K, A, lda, B, ldb, C, ldc, epi); PNN_KCHECK("gemm_k");
+      } else {
+        dim3 grid((unsigned)((M + 63) / 64), (unsigned)((N + 63) / 64));
+        gemm_k<T, 64, 64, 4, 4, 16><<<grid, 256, 0, st>>>(M, N, K, A, lda, B, ldb, C, ldc, epi); PNN_KCHECK("gemm_k");
+      }
     }
   } else {
     // FP64: 128x128 tiles (8x8 per thread) for large problems, 64x64 (4x4) below ~2 waves of big tiles.
