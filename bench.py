@@ -128,6 +128,24 @@ def algorithmic_work(family: str, N: int, E: int, mc: gen.ModelCfg, prec: str, f
     return None, None
 
 
+def gemm_work(family: str, N: int, mc: gen.ModelCfg, prec: str, forces: bool):
+    """(flops, bytes) per launch, averaged over the launches of one GEMM family in a step: 2 M N K flop; operands and
+    result once (the SiLU GEMMs' stored pre-activation and the accumulating ones' read of C are not counted)."""
+    F, T = mc.F, mc.T
+    eb = 8 if prec == "fp64" else (2 if prec == "bf16" else 4)
+    if family == "gemm_N":
+        shapes = [(N, F, F), (N, 3 * F, F), (N, F, 2 * F), (N, 3 * F, F)] * T          # W1, W2, A1, A2
+        if forces:
+            shapes += [(N, F, 3 * F), (N, 2 * F, F)] * T + [(N, F, 3 * F), (N, F, F)] * (T - 1)
+    elif family == "gemm_3N":
+        shapes = [(3 * N, 2 * F, F)] * T + ([(3 * N, F, 2 * F)] * T if forces else [])  # U|V and its transpose
+    else:
+        return None, None, 0
+    fl = sum(2.0 * m * n * k for m, n, k in shapes)
+    by = sum(eb * (m * k + m * n + n * k) for m, n, k in shapes)
+    return fl / len(shapes), by / len(shapes), len(shapes)
+
+
 def measured_traffic(workload: str, family: str):
     """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/r01_traffic.csv), or None."""
     try:
@@ -333,22 +351,45 @@ def main():
         per = ms / max(nl, 1)
         kernels[fam] = dict(launches_per_step=nl / args.steps, ms_per_launch=per, share=ms / tot_ms)
     roof = None
-    edge_fams = [f for f in kernels if f.startswith("edge_")]
-    if edge_fams:
-        fam = max(edge_fams, key=lambda f: kernels[f]["share"])
-        flops, byts = algorithmic_work(fam, N, E, mc, prec, main_res["forces"])
+    cand = [f for f in kernels if f.startswith("edge_") or f.startswith("gemm_")]
+    if cand:
+        fam = max(cand, key=lambda f: kernels[f]["share"])      # the dominant kernel family of the step
         per_s = kernels[fam]["ms_per_launch"] * 1e-3
+        if fam.startswith("gemm_"):
+            flops, byts, _ = gemm_work(fam, N, mc, prec, main_res["forces"])
+        else:
+            flops, byts = algorithmic_work(fam, N, E, mc, prec, main_res["forces"])
         if prec in ("fp32", "fp64"):
             ach, peak = flops / per_s / 1e12, ALU_PEAK_TFLOPS[prec]
             roof = dict(kernel=fam, bound="alu", achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak,
                         traffic=measured_traffic(WORKLOAD_NAMES[args.workload], fam),
                         peak_source="derived: 148 SMs x lanes x 2 x 1.965 GHz (DESIGN.md)",
                         hbm_achieved_gbs=byts / per_s / 1e9, hbm_peak_gbs=peaks["hbm"], hbm_peak_source=peaks["source"])
+            try:   # the nominal ALU peak is also measured on the box (FMA micro-benchmark)
+                roof["alu_peak_measured"] = pnn.pnn_measure_alu_peak(pnn.PNN_FP64 if prec == "fp64" else pnn.PNN_FP32)
+                roof["frac_of_measured_peak"] = ach / roof["alu_peak_measured"]
+            except Exception as ex:
+                roof["alu_peak_measured"] = None
+        elif fam.startswith("gemm_"):
+            ach = flops / per_s / 1e12
+            roof = dict(kernel=fam, bound="tensor", achieved=ach, peak=peaks["bf16_sust"], unit="TFLOP/s",
+                        frac=ach / peaks["bf16_sust"], traffic=measured_traffic(WORKLOAD_NAMES[args.workload], fam),
+                        peak_source=peaks["source"] + " (sustained bf16)", algorithmic_bytes=byts)
         else:
             ach = byts / per_s / 1e9
             roof = dict(kernel=fam, bound="hbm", achieved=ach, peak=peaks["hbm"], unit="GB/s", frac=ach / peaks["hbm"],
                         traffic=measured_traffic(WORKLOAD_NAMES[args.workload], fam), peak_source=peaks["source"],
                         algorithmic_bytes=byts, tensor_flops=flops)
+        # the runner-up family, for context (the two are within a few percent of the step on cfg2)
+        others = sorted((f for f in cand if f != fam), key=lambda f: -kernels[f]["share"])
+        if others and prec in ("fp32", "fp64"):
+            f2 = others[0]
+            fl2 = gemm_work(f2, N, mc, prec, main_res["forces"])[0] if f2.startswith("gemm_") else \
+                algorithmic_work(f2, N, E, mc, prec, main_res["forces"])[0]
+            if fl2:
+                a2 = fl2 / (kernels[f2]["ms_per_launch"] * 1e-3) / 1e12
+                roof["runner_up"] = dict(kernel=f2, achieved=a2, frac=a2 / ALU_PEAK_TFLOPS[prec],
+                                         share_of_step=kernels[f2]["share"])
         roof["share_of_step"] = kernels[fam]["share"]
 
     line = dict(metric="painn_energy_force_structures_per_s", value=main_res["structures_per_s"], unit="structures/s",

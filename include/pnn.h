@@ -175,6 +175,12 @@ int pnn_profile_read(pnn_workspace* ws, int max_entries, char* names, double* to
 int pnn_gemm_bf16(int64_t M, int32_t N, int32_t K, const void* A, int64_t lda, const void* Wt, int64_t ldw,
                   const float* bias, int32_t act, float* C, int64_t ldc, void* Cb, int64_t ldcb, void* cuda_stream);
 
+/* Measured peak of the plain FMA pipe in TFLOP/s (the ALU roofs of the FP32 / FP64 edge kernels and
+ * GEMMs "must be measured on the box by a small FMA micro-benchmark"): independent register FMA chains, packed
+ * fma.rn.f32x2 for PNN_FP32 and DFMA for PNN_FP64, best of five launches timed with CUDA events.  *tflops is a host
+ * value.  PNN_BF16 -> PNN_ERR_INVALID_ARG (its roofs are HBM and the tensor pipe).  Synchronous. */
+int pnn_measure_alu_peak(int prec, double* tflops, void* cuda_stream);
+
 /* Number of kernels the library has launched on behalf of this workspace since it was created. */
 int64_t pnn_launch_count(const pnn_workspace* ws);
 

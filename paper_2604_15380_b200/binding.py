@@ -17,7 +17,7 @@ __all__ = [
     "lib_path", "pnn_status_string", "pnn_last_cuda_error", "pnn_weights_count", "pnn_model_create",
     "pnn_model_destroy", "pnn_branch_mlp_create", "pnn_branch_mlp_destroy", "pnn_branch_weights",
     "pnn_workspace_create", "pnn_workspace_destroy", "pnn_workspace_bytes", "pnn_build_graph",
-    "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_eval_blended", "pnn_eval_host", "pnn_check_async_errors", "pnn_launch_count", "pnn_profile_enable",
+    "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_eval_blended", "pnn_eval_host", "pnn_check_async_errors", "pnn_measure_alu_peak", "pnn_launch_count", "pnn_profile_enable",
     "pnn_profile_read", "pnn_gemm_bf16",
     "PaiNN", "PRECISIONS",
 ]
@@ -88,6 +88,7 @@ def lib():
         L.pnn_profile_enable.argtypes = [vp, i32]
         L.pnn_profile_read.argtypes = [vp, i32, vp, vp, vp, ctypes.POINTER(i32)]
         L.pnn_gemm_bf16.argtypes = [i64, i32, i32, vp, i64, vp, i64, vp, i32, vp, i64, vp, i64, vp]
+        L.pnn_measure_alu_peak.argtypes = [i32, ctypes.POINTER(ctypes.c_double), vp]
         L.pnn_launch_count.argtypes = [vp]
         L.pnn_launch_count.restype = i64
         _lib = L
@@ -209,6 +210,13 @@ def pnn_eval_host(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, str
 
 def pnn_check_async_errors(ws: int) -> None:
     _check(lib().pnn_check_async_errors(ws), "pnn_check_async_errors")
+
+
+def pnn_measure_alu_peak(prec: int, stream=None) -> float:
+    """Measured TFLOP/s of the FMA pipe (packed FP32 or FP64 chains)."""
+    out = ctypes.c_double()
+    _check(lib().pnn_measure_alu_peak(int(prec), ctypes.byref(out), stream), "pnn_measure_alu_peak")
+    return out.value
 
 
 def pnn_launch_count(ws: int) -> int:

@@ -3,6 +3,8 @@
 // over the heads.  24.5 k parameters: the whole router lives in L2 / L1; one CTA evaluates SPB structures so that every
 // weight it reads is used SPB times, thread o owns output unit o of the current layer (weights stored input-major on the
 // device, so a warp reads 32 consecutive outputs of one input row).
+#include <algorithm>
+
 #include "common.cuh"
 
 namespace pnn {
@@ -96,4 +98,62 @@ template int launch_branch_mlp<float>(int64_t, const BranchMlpDims&, const int32
 template int launch_branch_mlp<double>(int64_t, const BranchMlpDims&, const int32_t*, const int32_t*, const double*,
                                        double*, int*, cudaStream_t);
 
+} // namespace pnn
+
+// ---- plain-ALU peak ("FP32-ALU and FP64 peaks are nominal and must be measured on the box by a small
+// FMA micro-benchmark"): independent FMA chains in registers, nothing else in the loop.  FP32 uses the packed
+// fma.rn.f32x2 the kernels use (two FMAs per issued instruction).
+namespace pnn {
+namespace {
+constexpr int PK_CHAINS = 8, PK_ITERS = 4096;
+
+__global__ void __launch_bounds__(256) peak_f32_k(float2* out, float2 a, float2 b) {
+  float2 acc[PK_CHAINS];
+#pragma unroll
+  for (int c = 0; c < PK_CHAINS; ++c) acc[c] = make_float2(threadIdx.x * 1e-3f + c, blockIdx.x * 1e-3f - c);
+  for (int it = 0; it < PK_ITERS; ++it) {
+#pragma unroll
+    for (int c = 0; c < PK_CHAINS; ++c) acc[c] = __ffma2_rn(acc[c], a, b);
+  }
+  float2 s = make_float2(0.f, 0.f);
+#pragma unroll
+  for (int c = 0; c < PK_CHAINS; ++c) { s.x += acc[c].x; s.y += acc[c].y; }
+  if (s.x == 123.456f) out[0] = s;   // keeps the chains alive; never true for these inputs
+}
+
+__global__ void __launch_bounds__(256) peak_f64_k(double* out, double a, double b) {
+  double acc[PK_CHAINS];
+#pragma unroll
+  for (int c = 0; c < PK_CHAINS; ++c) acc[c] = threadIdx.x * 1e-3 + c;
+  for (int it = 0; it < PK_ITERS; ++it) {
+#pragma unroll
+    for (int c = 0; c < PK_CHAINS; ++c) acc[c] = fma(acc[c], a, b);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int c = 0; c < PK_CHAINS; ++c) s += acc[c];
+  if (s == 123.456) out[0] = s;
+}
+} // namespace
+
+// TFLOP/s of the FMA pipe, best of `reps` launches timed with CUDA events on `st`.  Synchronises.  Returns < 0 on error.
+double measure_alu_peak(bool fp64, void* scratch, cudaStream_t st) {
+  cudaEvent_t e0, e1;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return -1.0;
+  const int grid = 148 * 8, block = 256, reps = 5;
+  double best = 0.0;
+  for (int r = 0; r < reps + 1; ++r) {
+    cudaEventRecord(e0, st);
+    if (fp64) peak_f64_k<<<grid, block, 0, st>>>((double*)scratch, 0.999999, 1e-7);
+    else peak_f32_k<<<grid, block, 0, st>>>((float2*)scratch, make_float2(0.999999f, 0.999998f), make_float2(1e-7f, 2e-7f));
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { best = -1.0; break; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double flop = (double)grid * block * PK_ITERS * PK_CHAINS * (fp64 ? 2.0 : 4.0);
+    if (r > 0 && ms > 0.f) best = std::max(best, flop / (ms * 1e-3) * 1e-12);   // launch 0 is the warm-up
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  return best;
+}
 } // namespace pnn

@@ -220,5 +220,6 @@ struct BranchMlpDims {
 template <typename T>
 int launch_branch_mlp(int64_t S, const BranchMlpDims& dm, const int32_t* Z, const int32_t* sptr, const T* params,
                       T* out, int* d_err, cudaStream_t st);
+double measure_alu_peak(bool fp64, void* scratch, cudaStream_t st);   // TFLOP/s of the FMA pipe (packed FP32 / FP64)
 
 } // namespace pnn

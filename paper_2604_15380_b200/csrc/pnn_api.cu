@@ -924,6 +924,17 @@ int pnn_branch_weights(const pnn_branch_mlp* b, pnn_workspace* ws, int64_t N, in
   return PNN_OK;
 }
 
+int pnn_measure_alu_peak(int prec, double* tflops, void* stream) {
+  if (!tflops || (prec != PNN_FP32 && prec != PNN_FP64)) return PNN_ERR_INVALID_ARG;
+  void* scratch = nullptr;
+  PNN_TRY(cudaMalloc(&scratch, 64));
+  const double v = measure_alu_peak(prec == PNN_FP64, scratch, (cudaStream_t)stream);
+  cudaFree(scratch);
+  if (v <= 0.0) { cuda_ok(cudaGetLastError(), "pnn_measure_alu_peak"); return PNN_ERR_CUDA; }
+  *tflops = v;
+  return PNN_OK;
+}
+
 int pnn_eval_host(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const double* pos,
                   const int32_t* sptr, const int32_t* head, const double* cell, const uint8_t* pbc, int flags,
                   void* energy_host, void* forces_host, void* stream) {

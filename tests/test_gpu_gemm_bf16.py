@@ -48,3 +48,15 @@ def test_gemm_bf16_strided_and_outputs_optional():
     ref = Abig[:, 64:128].double() @ W.double().T
     assert (C[:, :N] == 0).all()
     assert ((C[:, N:].double() - ref).abs() <= 1e-4 * (1 + ref.abs())).all()
+
+
+def test_measured_alu_peak_is_near_the_derived_one():
+    """the plain-ALU roofs are measured on the box.  Derived: 148 SMs x 128 (64) lanes x 2 x 1.965 GHz =
+    74.4 (37.2) TFLOP/s; the packed-FMA micro-benchmark must land within 15 % of it and never above."""
+    from paper_2604_15380_b200 import binding as B
+    p32 = B.pnn_measure_alu_peak(B.PNN_FP32)
+    p64 = B.pnn_measure_alu_peak(B.PNN_FP64)
+    assert 0.85 * 74.45 < p32 < 1.02 * 74.45, p32
+    assert 0.85 * 37.22 < p64 < 1.02 * 37.22, p64
+    with pytest.raises(B.PnnError):
+        B.pnn_measure_alu_peak(B.PNN_BF16)
