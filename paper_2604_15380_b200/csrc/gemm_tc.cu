@@ -92,6 +92,27 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
   asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
+// 32-byte global store (STG.256 on sm_100: one full L2 sector per instruction; a row-owner thread otherwise writes its
+// row in 16-byte halves of a sector).  p must be 32-byte aligned.
+__device__ __forceinline__ void st256(void* p, uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t a4,
+                                      uint32_t a5, uint32_t a6, uint32_t a7) {
+  asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(p), "r"(a0), "r"(a1), "r"(a2), "r"(a3),
+               "r"(a4), "r"(a5), "r"(a6), "r"(a7)
+               : "memory");
+}
+__device__ __forceinline__ void ld256(const void* p, float (&v)[8]) {
+  uint32_t a[8];
+  asm volatile("ld.global.v8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(a[0]), "=r"(a[1]), "=r"(a[2]), "=r"(a[3]), "=r"(a[4]), "=r"(a[5]), "=r"(a[6]), "=r"(a[7])
+               : "l"(p)
+               : "memory");
+#pragma unroll
+  for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(a[i]);
+}
+__device__ __forceinline__ bool al32(const void* p, int64_t ld_bytes) {
+  return ((reinterpret_cast<uintptr_t>(p) | (uintptr_t)ld_bytes) & 31) == 0;
+}
+
 // Epilogue of one output row segment: 32 accumulator columns of row m starting at column n (bias, activation, optional
 // pre-activation store / silu' factor / accumulate, FP32 and / or BF16 stores as 16-byte vectors of the row).
 __device__ __forceinline__ void epi_chunk(const TcEpi& epi, int64_t m, int n, const uint32_t (&r)[32]) {
@@ -107,41 +128,84 @@ __device__ __forceinline__ void epi_chunk(const TcEpi& epi, int64_t m, int n, co
   }
   if (epi.act == ACT_SILU) {
     if (epi.pre) {
-      float4* pp = reinterpret_cast<float4*>(epi.pre + m * epi.ldpre + n);
+      float* pp = epi.pre + m * epi.ldpre + n;
+      if (al32(epi.pre, epi.ldpre * 4)) {
 #pragma unroll
-      for (int j = 0; j < 32; j += 4) pp[j >> 2] = make_float4(x[j], x[j + 1], x[j + 2], x[j + 3]);
+        for (int j = 0; j < 32; j += 8)
+          st256(pp + j, __float_as_uint(x[j]), __float_as_uint(x[j + 1]), __float_as_uint(x[j + 2]),
+                __float_as_uint(x[j + 3]), __float_as_uint(x[j + 4]), __float_as_uint(x[j + 5]),
+                __float_as_uint(x[j + 6]), __float_as_uint(x[j + 7]));
+      } else {
+#pragma unroll
+        for (int j = 0; j < 32; j += 4)
+          reinterpret_cast<float4*>(pp)[j >> 2] = make_float4(x[j], x[j + 1], x[j + 2], x[j + 3]);
+      }
     }
 #pragma unroll
     for (int j = 0; j < 32; ++j) x[j] = silu_f<float>(x[j]);
   } else if (epi.act == ACT_MUL_DSILU) {
-    const float4* ap = reinterpret_cast<const float4*>(epi.aux + m * epi.ldaux + n);
+    const float* ap = epi.aux + m * epi.ldaux + n;
+    if (al32(epi.aux, epi.ldaux * 4)) {
 #pragma unroll
-    for (int j = 0; j < 32; j += 4) {
-      const float4 av = ap[j >> 2];
-      x[j] *= dsilu_f<float>(av.x); x[j + 1] *= dsilu_f<float>(av.y);
-      x[j + 2] *= dsilu_f<float>(av.z); x[j + 3] *= dsilu_f<float>(av.w);
+      for (int j = 0; j < 32; j += 8) {
+        float av[8];
+        ld256(ap + j, av);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) x[j + i] *= dsilu_f<float>(av[i]);
+      }
+    } else {
+#pragma unroll
+      for (int j = 0; j < 32; j += 4) {
+        const float4 av = reinterpret_cast<const float4*>(ap)[j >> 2];
+        x[j] *= dsilu_f<float>(av.x); x[j + 1] *= dsilu_f<float>(av.y);
+        x[j + 2] *= dsilu_f<float>(av.z); x[j + 3] *= dsilu_f<float>(av.w);
+      }
     }
   }
   if (epi.C) {
     float4* cp = reinterpret_cast<float4*>(epi.C + m * epi.ldc + n);
     if (epi.accumulate) {
+      if (al32(epi.C, epi.ldc * 4)) {
 #pragma unroll
-      for (int j = 0; j < 32; j += 4) {
-        const float4 cv = cp[j >> 2];
-        x[j] += cv.x; x[j + 1] += cv.y; x[j + 2] += cv.z; x[j + 3] += cv.w;
+        for (int j = 0; j < 32; j += 8) {
+          float cv[8];
+          ld256(reinterpret_cast<const float*>(cp) + j, cv);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) x[j + i] += cv[i];
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 32; j += 4) {
+          const float4 cv = cp[j >> 2];
+          x[j] += cv.x; x[j + 1] += cv.y; x[j + 2] += cv.z; x[j + 3] += cv.w;
+        }
       }
     }
+    if (al32(epi.C, epi.ldc * 4)) {
 #pragma unroll
-    for (int j = 0; j < 32; j += 4) cp[j >> 2] = make_float4(x[j], x[j + 1], x[j + 2], x[j + 3]);
+      for (int j = 0; j < 32; j += 8)
+        st256(reinterpret_cast<float*>(cp) + j, __float_as_uint(x[j]), __float_as_uint(x[j + 1]),
+              __float_as_uint(x[j + 2]), __float_as_uint(x[j + 3]), __float_as_uint(x[j + 4]),
+              __float_as_uint(x[j + 5]), __float_as_uint(x[j + 6]), __float_as_uint(x[j + 7]));
+    } else {
+#pragma unroll
+      for (int j = 0; j < 32; j += 4) cp[j >> 2] = make_float4(x[j], x[j + 1], x[j + 2], x[j + 3]);
+    }
   }
   if (epi.Cb) {
     uint4* bp = reinterpret_cast<uint4*>(epi.Cb + m * epi.ldcb + n);
+    uint32_t h[16];
 #pragma unroll
-    for (int j = 0; j < 32; j += 8) {
-      __nv_bfloat162 h0 = __floats2bfloat162_rn(x[j], x[j + 1]), h1 = __floats2bfloat162_rn(x[j + 2], x[j + 3]);
-      __nv_bfloat162 h2 = __floats2bfloat162_rn(x[j + 4], x[j + 5]), h3 = __floats2bfloat162_rn(x[j + 6], x[j + 7]);
-      bp[j >> 3] = make_uint4(*reinterpret_cast<uint32_t*>(&h0), *reinterpret_cast<uint32_t*>(&h1),
-                              *reinterpret_cast<uint32_t*>(&h2), *reinterpret_cast<uint32_t*>(&h3));
+    for (int j = 0; j < 32; j += 2) {
+      __nv_bfloat162 t = __floats2bfloat162_rn(x[j], x[j + 1]);
+      h[j >> 1] = *reinterpret_cast<uint32_t*>(&t);
+    }
+    if (al32(epi.Cb, epi.ldcb * 2)) {
+      st256(bp, h[0], h[1], h[2], h[3], h[4], h[5], h[6], h[7]);
+      st256(bp + 2, h[8], h[9], h[10], h[11], h[12], h[13], h[14], h[15]);
+    } else {
+#pragma unroll
+      for (int q = 0; q < 4; ++q) bp[q] = make_uint4(h[4 * q], h[4 * q + 1], h[4 * q + 2], h[4 * q + 3]);
     }
   }
 }
