@@ -35,6 +35,27 @@ __global__ void __launch_bounds__(256) embed_k(int64_t N, int F, int Zmax, const
   if (s16) s16[idx] = __float2bfloat16_rn((float)e);
 }
 
+// FP32: four features per thread (16-byte loads / stores, 8-byte BF16 copy)
+__global__ void __launch_bounds__(256) embed4_k(int64_t N, int F4, int Zmax, const int32_t* __restrict__ Z,
+                                                const float4* __restrict__ emb, float4* __restrict__ s, int* d_err,
+                                                uint2* __restrict__ s16) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= N * F4) return;
+  const int64_t i = idx / F4;
+  const int q = (int)(idx - i * F4);
+  int z = Z[i];
+  if (z < 1 || z > Zmax) {
+    if (q == 0) atomicOr(d_err, ERRF_BAD_Z);
+    z = 1;
+  }
+  const float4 e = __ldg(emb + (int64_t)z * F4 + q);
+  s[idx] = e;
+  if (s16) {
+    __nv_bfloat162 lo = __floats2bfloat162_rn(e.x, e.y), hi = __floats2bfloat162_rn(e.z, e.w);
+    s16[idx] = make_uint2(*reinterpret_cast<uint32_t*>(&lo), *reinterpret_cast<uint32_t*>(&hi));
+  }
+}
+
 // PQ [N][3][2F] (P | Q)  ->  sn[:, F:2F] = sqrt(sum_a Q_a^2 + eps)          (B4)
 template <typename T, typename IT>
 __global__ void __launch_bounds__(256) norm_k(int64_t N, int F, const IT* __restrict__ PQ, T* __restrict__ sn, T eps,
@@ -668,6 +689,12 @@ template <typename T>
 int launch_embed(int64_t N, int F, int Zmax, const int32_t* Z, const T* emb, T* s, int* d_err, cudaStream_t st,
                  __nv_bfloat16* s16) {
   if (N == 0) return 0;
+  if constexpr (std::is_same<T, float>::value) {
+    embed4_k<<<nblk(N * (F / 4), 256), 256, 0, st>>>(N, F / 4, Zmax, Z, reinterpret_cast<const float4*>(emb),
+                                                     reinterpret_cast<float4*>(s), d_err, reinterpret_cast<uint2*>(s16));
+    PNN_KCHECK("embed4_k");
+    return 1;
+  }
   embed_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, Zmax, Z, emb, s, d_err, s16); PNN_KCHECK("embed_k");
   return 1;
 }
