@@ -30,6 +30,18 @@ __device__ __forceinline__ void ldv(const float* p, float (&x)[FPL]) {
   if (FPL == 1) x[0] = __ldg(p);
   else { const float2 t = __ldg(reinterpret_cast<const float2*>(p)); x[0] = t.x; x[FPL - 1] = t.y; }
 }
+// The edge tape is written once and read once, a whole sweep later: streaming (evict-first) accesses keep it from
+// displacing the gathered node rows in L2.
+template <int FPL>
+__device__ __forceinline__ void ldv_stream(const float* p, float (&x)[FPL]) {
+  if (FPL == 1) x[0] = __ldcs(p);
+  else { const float2 t = __ldcs(reinterpret_cast<const float2*>(p)); x[0] = t.x; x[FPL - 1] = t.y; }
+}
+template <int FPL>
+__device__ __forceinline__ void stv_stream(float* p, const float (&x)[FPL]) {
+  if (FPL == 1) __stcs(p, x[0]);
+  else __stcs(reinterpret_cast<float2*>(p), make_float2(x[0], x[FPL - 1]));
+}
 template <int FPL>
 __device__ __forceinline__ void stv(float* p, const float (&x)[FPL]) {
   if (FPL == 1) *p = x[0];
@@ -175,8 +187,8 @@ edge_fwd_w_k(EdgeArgs<float> a, int RB, const float* __restrict__ phi, const flo
               float dw[FPL];
 #pragma unroll
               for (int p = 0; p < FPL; ++p) dw[p] = dot_pairs<KP>(w[c][p], g2, bias[c][p] * cp);
-              stv<FPL>(wt + eo + c * F, wv[c]);
-              stv<FPL>(dt + eo + c * F, dw);
+              stv_stream<FPL>(wt + eo + c * F, wv[c]);
+              stv_stream<FPL>(dt + eo + c * F, dw);
             }
           }
 #pragma unroll
@@ -250,7 +262,7 @@ edge_bwd_w_k(EdgeArgs<float> a, int RB, const float* __restrict__ phi, const flo
         for (int c = 0; c < 3; ++c) {
           ldv<FPL>(phi + jo + c * F, ph[c]);
           ldv<FPL>(vb1 + jo + c * F, bj[c]);
-          if (c < 2 || has_v) { ldv<FPL>(wt + eo + c * F, wv[c]); ldv<FPL>(dt + eo + c * F, dw[c]); }
+          if (c < 2 || has_v) { ldv_stream<FPL>(wt + eo + c * F, wv[c]); ldv_stream<FPL>(dt + eo + c * F, dw[c]); }
           if (has_v) ldv<FPL>(v_in + jo + c * F, vj[c]);
         }
         float D = 0.f, B0 = 0.f, B1 = 0.f, B2 = 0.f;
