@@ -418,14 +418,25 @@ __global__ void __launch_bounds__(256) readout2_k(int64_t N, int F, int H, const
   const T* W0 = W1t + (int64_t)h0 * F * Fh + og * 4;
   const T* W1p = W1t + (int64_t)h1 * F * Fh + og * 4;
   T acc0[4] = {T(0), T(0), T(0), T(0)}, acc1[4] = {T(0), T(0), T(0), T(0)};
+  if (__all_sync(0xffffffffu, h0 == h1)) {   // the usual case (rows 8 apart in one structure): one weight vector for both
 #pragma unroll 4
-  for (int k = 0; k < F; ++k) {
-    T wa[4], wb[4];
-    Vec4<T>::ld(W0 + (int64_t)k * Fh, wa);
-    Vec4<T>::ld(W1p + (int64_t)k * Fh, wb);
-    const T x0 = S[rg * F + k], x1 = S[(rg + 8) * F + k];
+    for (int k = 0; k < F; ++k) {
+      T wa[4];
+      Vec4<T>::ld(W0 + (int64_t)k * Fh, wa);
+      const T x0 = S[rg * F + k], x1 = S[(rg + 8) * F + k];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) { acc0[j] = fma(wa[j], x0, acc0[j]); acc1[j] = fma(wb[j], x1, acc1[j]); }
+      for (int j = 0; j < 4; ++j) { acc0[j] = fma(wa[j], x0, acc0[j]); acc1[j] = fma(wa[j], x1, acc1[j]); }
+    }
+  } else {
+#pragma unroll 4
+    for (int k = 0; k < F; ++k) {
+      T wa[4], wb[4];
+      Vec4<T>::ld(W0 + (int64_t)k * Fh, wa);
+      Vec4<T>::ld(W1p + (int64_t)k * Fh, wb);
+      const T x0 = S[rg * F + k], x1 = S[(rg + 8) * F + k];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { acc0[j] = fma(wa[j], x0, acc0[j]); acc1[j] = fma(wb[j], x1, acc1[j]); }
+    }
   }
 #pragma unroll
   for (int r = 0; r < 2; ++r) {
@@ -477,14 +488,25 @@ __global__ void __launch_bounds__(512) readout_bwd2_k(int64_t N, int F, int H, c
   const T* Wa = W1 + (int64_t)Hs[rg] * Fh * F + kg * 4;
   const T* Wb = W1 + (int64_t)Hs[rg + 8] * Fh * F + kg * 4;
   T acc0[4] = {T(0), T(0), T(0), T(0)}, acc1[4] = {T(0), T(0), T(0), T(0)};
+  if (__all_sync(0xffffffffu, Hs[rg] == Hs[rg + 8])) {   // same head for both rows: one weight vector
 #pragma unroll 4
-  for (int o = 0; o < Fh; ++o) {
-    T wa[4], wb[4];
-    Vec4<T>::ld(Wa + (int64_t)o * F, wa);
-    Vec4<T>::ld(Wb + (int64_t)o * F, wb);
-    const T p0 = Pb[rg * Fh + o], p1 = Pb[(rg + 8) * Fh + o];
+    for (int o = 0; o < Fh; ++o) {
+      T wa[4];
+      Vec4<T>::ld(Wa + (int64_t)o * F, wa);
+      const T p0 = Pb[rg * Fh + o], p1 = Pb[(rg + 8) * Fh + o];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) { acc0[j] = fma(wa[j], p0, acc0[j]); acc1[j] = fma(wb[j], p1, acc1[j]); }
+      for (int j = 0; j < 4; ++j) { acc0[j] = fma(wa[j], p0, acc0[j]); acc1[j] = fma(wa[j], p1, acc1[j]); }
+    }
+  } else {
+#pragma unroll 4
+    for (int o = 0; o < Fh; ++o) {
+      T wa[4], wb[4];
+      Vec4<T>::ld(Wa + (int64_t)o * F, wa);
+      Vec4<T>::ld(Wb + (int64_t)o * F, wb);
+      const T p0 = Pb[rg * Fh + o], p1 = Pb[(rg + 8) * Fh + o];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { acc0[j] = fma(wa[j], p0, acc0[j]); acc1[j] = fma(wb[j], p1, acc1[j]); }
+    }
   }
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
