@@ -102,7 +102,55 @@ __global__ void __launch_bounds__(256) scan_apply_k(const int32_t* __restrict__ 
   if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 255) out[n] = bsum[gridDim.x];
 }
 
+// Small inputs (molecular batches: a few thousand cells / atoms): the whole scan in ONE block, 1024 threads x 4 items per
+// round with a running carry — one launch instead of three latency-bound ones.  out[n] = total.
+__global__ void __launch_bounds__(1024) scan_small_k(const int32_t* __restrict__ in, int n, int32_t* __restrict__ out) {
+  __shared__ int ws[32];
+  __shared__ int carry_s;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  for (int base = 0; base < n; base += 4096) {
+    const int i0 = base + threadIdx.x * 4;
+    int x[4], tsum = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      x[q] = (i0 + q < n) ? in[i0 + q] : 0;
+      tsum += x[q];
+    }
+    int incl = tsum;
+    for (int o = 1; o < 32; o <<= 1) {
+      const int y = __shfl_up_sync(0xffffffffu, incl, o);
+      if ((threadIdx.x & 31) >= o) incl += y;
+    }
+    if ((threadIdx.x & 31) == 31) ws[threadIdx.x >> 5] = incl;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+      int v = ws[threadIdx.x], iv = v;
+      for (int o = 1; o < 32; o <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, iv, o);
+        if (threadIdx.x >= o) iv += y;
+      }
+      ws[threadIdx.x] = iv - v; // exclusive warp offsets
+    }
+    __syncthreads();
+    int run = carry_s + ws[threadIdx.x >> 5] + incl - tsum;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      if (i0 + q < n) out[i0 + q] = run;
+      run += x[q];
+    }
+    __syncthreads();
+    if (threadIdx.x == 1023) carry_s = run;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[n] = carry_s;
+}
+
 int exclusive_scan(const int32_t* in, int64_t n, int32_t* out, int32_t* tmp, cudaStream_t st) {
+  if (n <= 16384) {
+    scan_small_k<<<1, 1024, 0, st>>>(in, (int)n, out); PNN_KCHECK("scan_small_k");
+    return 1;
+  }
   const int nb = (int)((n + SCAN_ITEMS - 1) / SCAN_ITEMS);
   scan_reduce_k<<<nb, 256, 0, st>>>(in, n, tmp); PNN_KCHECK("scan_reduce_k");
   scan_bsums_k<<<1, 1024, 0, st>>>(tmp, nb); PNN_KCHECK("scan_bsums_k");
