@@ -12,6 +12,7 @@
 //     the segment sums stay in registers and are written once per receiver: no cross-lane reduction, no atomics;
 //   * consecutive lanes own consecutive features, so every gather is one full 128- or 256-byte line per row.
 #include <algorithm>
+#include <cstdlib>
 
 #include "common.cuh"
 
@@ -324,6 +325,109 @@ edge_bwd_w_k(EdgeArgs<float> a, int RB, const float* __restrict__ phi, const flo
   }
 }
 
+// The same reverse step for two features per lane with every product on packed FMAs (fma.rn.f32x2): the two features of a
+// lane go through identical arithmetic, so each scalar FFMA / FMUL of edge_bwd_w_k<2> (130 per edge, half rate on sm_100)
+// becomes half a packed instruction.  Differences are folded into constants negated once per receiver; the direction
+// chunk's A1 is accumulated with the opposite sign and negated at the end.
+__device__ __forceinline__ float2 ld2(const float* p) { return __ldg(reinterpret_cast<const float2*>(p)); }
+__device__ __forceinline__ float2 ld2s(const float* p) { return __ldcs(reinterpret_cast<const float2*>(p)); }
+__device__ __forceinline__ float2 sp2(float x) { return make_float2(x, x); }
+
+template <int NWARP>
+__global__ void __launch_bounds__(NWARP * 32)
+edge_bwd_w2_k(EdgeArgs<float> a, int RB, const float* __restrict__ phi, const float* __restrict__ v_in,
+              const float* __restrict__ sb1, const float* __restrict__ vb1, const float* __restrict__ wt,
+              const float* __restrict__ dt, float* __restrict__ phib, float* __restrict__ vb_in,
+              float* __restrict__ fpart, int first_block) {
+  if (*a.d_err & ERRF_EDGE_OVERFLOW) return;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int F = a.F;
+  const int f0 = (blockIdx.y * 32 + lane) * 2;
+  const bool has_v = v_in != nullptr;
+  const float2 z2 = make_float2(0.f, 0.f);
+  const int64_t nchunk = (a.N + RB - 1) / RB;
+  for (int64_t ch = blockIdx.x; ch < nchunk; ch += gridDim.x) {
+    const int64_t i_end = min((int64_t)(ch + 1) * RB, a.N);
+    for (int64_t i = ch * RB + warp; i < i_end; i += NWARP) {
+      const int ea = a.rowptr[i], eb = a.rowptr[i + 1];
+      const int64_t io = i * 3 * F + f0;
+      // the receiver's own rows
+      const float2 li0 = ld2(sb1 + i * F + f0);
+      float2 li[3], lph[3], lv[3];
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        li[c] = ld2(vb1 + io + c * F);
+        lph[c] = ld2(phi + io + c * F);
+        lv[c] = has_v ? ld2(v_in + io + c * F) : z2;
+      }
+      const float2 nlph1 = make_float2(-lph[1].x, -lph[1].y);
+      float2 A0 = z2, A1n = z2, A2[3] = {z2, z2, z2};
+      float fp0 = 0.f, fp1 = 0.f, fp2 = 0.f;
+      for (int e = ea; e < eb; ++e) {
+        const int64_t j = __ldg(a.col + e);
+        const float4 u = __ldg(reinterpret_cast<const float4*>(a.geom) + e);
+        const int64_t jo = j * 3 * F + f0, eo = (int64_t)e * 3 * F + f0;
+        float2 ph[3], bj[3], vj[3], wv[3], dw[3];
+        const float2 sbj = ld2(sb1 + j * F + f0);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          ph[c] = ld2(phi + jo + c * F);
+          bj[c] = ld2(vb1 + jo + c * F);
+          if (c < 2 || has_v) { wv[c] = ld2s(wt + eo + c * F); dw[c] = ld2s(dt + eo + c * F); }
+          if (has_v) vj[c] = ld2(v_in + jo + c * F);
+        }
+        const float2 ux = sp2(u.x), uy = sp2(u.y), uz = sp2(u.z);
+        // scalar chunk
+        A0 = __ffma2_rn(sbj, wv[0], A0);
+        float2 D = __fmul2_rn(__ffma2_rn(li0, ph[0], __fmul2_rn(sbj, lph[0])), dw[0]);
+        // direction chunk
+        const float2 tj = __ffma2_rn(bj[2], uz, __ffma2_rn(bj[1], uy, __fmul2_rn(bj[0], ux)));
+        const float2 ti = __ffma2_rn(li[2], uz, __ffma2_rn(li[1], uy, __fmul2_rn(li[0], ux)));
+        A1n = __ffma2_rn(tj, wv[1], A1n);
+        D = __ffma2_rn(__ffma2_rn(ti, ph[1], __fmul2_rn(tj, nlph1)), dw[1], D);
+        const float2 B0 = __fmul2_rn(__ffma2_rn(li[0], ph[1], __fmul2_rn(bj[0], nlph1)), wv[1]);
+        const float2 B1 = __fmul2_rn(__ffma2_rn(li[1], ph[1], __fmul2_rn(bj[1], nlph1)), wv[1]);
+        const float2 B2 = __fmul2_rn(__ffma2_rn(li[2], ph[1], __fmul2_rn(bj[2], nlph1)), wv[1]);
+        // vector chunk
+        if (has_v) {
+          A2[0] = __ffma2_rn(bj[0], wv[2], A2[0]);
+          A2[1] = __ffma2_rn(bj[1], wv[2], A2[1]);
+          A2[2] = __ffma2_rn(bj[2], wv[2], A2[2]);
+          const float2 liv = __ffma2_rn(li[2], vj[2], __ffma2_rn(li[1], vj[1], __fmul2_rn(li[0], vj[0])));
+          const float2 blv = __ffma2_rn(bj[2], lv[2], __ffma2_rn(bj[1], lv[1], __fmul2_rn(bj[0], lv[0])));
+          D = __ffma2_rn(__ffma2_rn(liv, ph[2], __fmul2_rn(blv, lph[2])), dw[2], D);
+        }
+        const float Ds = D.x + D.y, b0 = B0.x + B0.y, b1 = B1.x + B1.y, b2 = B2.x + B2.y;
+        const float Bu = b0 * u.x + b1 * u.y + b2 * u.z;
+        const float invd = 1.0f / u.w;
+        fp0 += Ds * u.x + (b0 - Bu * u.x) * invd;
+        fp1 += Ds * u.y + (b1 - Bu * u.y) * invd;
+        fp2 += Ds * u.z + (b2 - Bu * u.z) * invd;
+      }
+      if (phib != nullptr) {
+        *reinterpret_cast<float2*>(phib + io) = A0;
+        *reinterpret_cast<float2*>(phib + io + F) = make_float2(-A1n.x, -A1n.y);
+        *reinterpret_cast<float2*>(phib + io + 2 * F) =
+            __ffma2_rn(lv[2], A2[2], __ffma2_rn(lv[1], A2[1], __fmul2_rn(lv[0], A2[0])));
+#pragma unroll
+        for (int ax = 0; ax < 3; ++ax)
+          *reinterpret_cast<float2*>(vb_in + io + ax * F) = __ffma2_rn(lph[2], A2[ax], li[ax]);
+      }
+#pragma unroll
+      for (int o = 16; o; o >>= 1) {
+        fp0 += __shfl_xor_sync(0xffffffffu, fp0, o);
+        fp1 += __shfl_xor_sync(0xffffffffu, fp1, o);
+        fp2 += __shfl_xor_sync(0xffffffffu, fp2, o);
+      }
+      if (lane == 0) {
+        float* dst = fpart + ((int64_t)blockIdx.y * a.N + i) * 3;
+        if (first_block) { dst[0] = fp0; dst[1] = fp1; dst[2] = fp2; }
+        else { dst[0] += fp0; dst[1] += fp1; dst[2] += fp2; }
+      }
+    }
+  }
+}
+
 } // namespace
 
 // FPL = 2 needs 6 K-long filter rows per lane in registers: used up to K = 20.
@@ -386,7 +490,10 @@ int launch_edge_bwd_warp(const EdgeArgs<float>& a, const float* phi, const float
   const int RB = NW;   // cfg2 0.160 -> 0.144 ms, cfg3 0.76 -> 0.73 ms against 16 receivers per chunk
   const int64_t nchunk = (a.N + RB - 1) / RB;
   dim3 grid((unsigned)std::min<int64_t>(nchunk, 148 * 16), a.F / (32 * FPL));
-  if (FPL == 2)
+  static const bool scalar_math = getenv("PNN_BWD_SCALAR") != nullptr;   // debugging aid: the unpacked kernel
+  if (FPL == 2 && !scalar_math)
+    edge_bwd_w2_k<NW><<<grid, NW * 32, 0, st>>>(a, RB, phi, v_in, sb1, vb1, wt, dt, phib, vb_in, fpart, first_block);
+  else if (FPL == 2)
     edge_bwd_w_k<2, NW><<<grid, NW * 32, 0, st>>>(a, RB, phi, v_in, sb1, vb1, wt, dt, phib, vb_in, fpart, first_block);
   else
     edge_bwd_w_k<1, NW><<<grid, NW * 32, 0, st>>>(a, RB, phi, v_in, sb1, vb1, wt, dt, phib, vb_in, fpart, first_block);
