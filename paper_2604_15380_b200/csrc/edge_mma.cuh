@@ -40,4 +40,12 @@ int launch_edge_bwd_mma(const EdgeMmaArgs& a, const __nv_bfloat16* phi, const __
                         float* vb_in, float* fpart, int first_block, cudaStream_t st);
 int edge_mma_num_slabs(int F);
 
+// edge_tc.cu — forward message step on tcgen05 (features on the TMEM lanes, 16 consecutive CSR edges per MMA tile).
+// fltT: one block's filter packed by pack_filter_tc (edge_tc_filter_elems(K) BF16 elements).
+int64_t edge_tc_filter_elems(int K);
+void pack_filter_tc(int F, int K, const double* fltW, const double* fltb, uint16_t* out);
+int launch_edge_fwd_tc(const EdgeMmaArgs& a, const __nv_bfloat16* fltT, const __nv_bfloat16* phi, const float* s_in,
+                       int64_t ld_sin, const __nv_bfloat16* v_in, const float* v_res, float* s1, int64_t ld_s1, float* v1,
+                       const EdgeMirror& mir, cudaStream_t st);
+
 } // namespace pnn

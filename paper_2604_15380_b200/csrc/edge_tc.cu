@@ -1,0 +1,453 @@
+// edge_tc.cu — a4 (forward message step) of the BF16 model with the filter contraction on the tcgen05 tensor cores.
+//
+// SURVEY.md §8(c) B3, per edge e = (i <- j):  w_e = (flt_W g(d_e) + flt_b) c(d_e),  x_e = phi_j o w_e,
+//   s'_i = s_i + sum_e x^ss,   v'_i[a] = v_i[a] + sum_e ( x^vs u_e[a] + x^vv o v_j[a] ).
+//
+// The filter is the small-K GEMM  W^T[3F x edges] = Wf[3F x (K+1)] . G^T[(K+1) x edges]  (SURVEY.md §7 hard part 3), run
+// TRANSPOSED on tcgen05.mma so that FEATURES lie on the 128 TMEM lanes and EDGES on the TMEM columns:
+//   A (shared memory, resident for the whole kernel): per accumulator a = chunk*2 + parity the 128 filter rows of the
+//       features f = 2*lane + parity, K-major, column K = flt_b, zero padded to KP = 16 ceil((K+1)/16);
+//   B (shared memory ring): a tile of 16 CONSECUTIVE CSR edges x KP: g_k(d) c(d), c(d) in column K (BF16);
+//   D (TMEM): 6 accumulators [128 lanes x 16 columns] FP32 per pipeline (4 in the first block, where v = 0).
+// A thread of an epilogue warp owns TMEM lane l of its quadrant = the feature PAIR (2l, 2l+1): one tcgen05.ld gives it
+// the filter values of its two features for the 16 edges of the tile; it then walks the edges, gathers the sender's
+// phi_j / v_j pair as one 32-bit word per chunk (a warp reads 128 contiguous bytes of the row: one L1 wavefront, the rows
+// of a molecule stay in L1 because neighbouring receivers are processed by the same CTA), multiplies with packed
+// FP32 FMAs and keeps the receiver's segment sum in registers: no cross-lane reduction, no atomics, and neither the MMA
+// nor its operand staging occupy the issue slots of the warps that do the gathers.
+//
+// One persistent CTA per SM, NGRP independent pipelines, each = 1 producer warp + 4 epilogue warps:
+//   producer  (per tile) radial basis x cutoff of 16 edges -> B slot; sender index, unit vector, receiver -> metadata slot;
+//             lane 0 then issues the 6 x KP/16 tcgen05.mma of the tile and commits them to the pipeline's "TMEM full"
+//             mbarrier; it also prefetches the next atom range's rows into L2 (cp.async.bulk.prefetch);
+//   epilogue  waits, tcgen05.ld's the tile into registers, frees the TMEM buffer at once (the next tile's MMAs overlap
+//             the arithmetic of this one), runs the edge loop, and at every change of receiver adds the residual row
+//             and writes s', v' (FP32) and their BF16 copies with coalesced 8-byte / 4-byte stores.
+#include <algorithm>
+#include <cstring>
+#include <vector>
+
+#include "common.cuh"
+#include "edge_mma.cuh"
+#include "tc_ptx.cuh"
+
+namespace pnn {
+
+namespace {
+
+using namespace tc;
+
+constexpr int NE = 16;   // edges per tile = N of the UMMA
+constexpr int NGRP = 2;  // pipelines per CTA
+constexpr int NSLOT = 4; // ring slots (B tile + metadata) per pipeline
+constexpr int SPLIT = 2; // epilogue warps per TMEM lane quadrant: they share the features and take alternate receivers
+constexpr int EPW = 4 * SPLIT; // epilogue warps per pipeline
+constexpr int NPROD = 2; // producer warps per pipeline (tile n is staged and issued by producer n % NPROD)
+constexpr int NTHR = NGRP * (EPW + NPROD) * 32;
+constexpr int ES = 4;    // edges per epilogue step (TMEM columns per tcgen05.ld)
+
+struct TileMeta {
+  float4 U[NE];        // unit vector; .w = receiver index (bit pattern)
+  uint32_t OFF[NE];    // sender row offset in 16-byte units (row = 3F BF16)
+  uint32_t mask[SPLIT]; // bit c: edge c of the tile is valid and its receiver belongs to epilogue half h
+  uint32_t pad[4 - SPLIT];
+};
+
+__device__ __forceinline__ float2 bf2(uint32_t x) {
+  return make_float2(__uint_as_float(x << 16), __uint_as_float(x & 0xffff0000u));
+}
+__device__ __forceinline__ uint32_t pack_bf2(float lo, float hi) {
+  const __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<const uint32_t*>(&h);
+}
+__device__ __forceinline__ uint32_t ldg_nc32(const void* p) { return __ldg(reinterpret_cast<const uint32_t*>(p)); }
+// streaming accesses that should not displace the gathered rows from L1
+__device__ __forceinline__ float2 ld_stream2(const float* p) {
+  float2 v;
+  asm volatile("ld.global.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ void st_stream2(float* p, float2 v) {
+  asm volatile("st.global.cs.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(v.x), "f"(v.y) : "memory");
+}
+__device__ __forceinline__ void st_stream1(void* p, uint32_t v) {
+  asm volatile("st.global.cs.b32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// 32 TMEM lanes x 4 columns, asynchronous
+__device__ __forceinline__ void tmem_ld4_async(uint32_t taddr, float (&r)[4]) {
+  uint32_t u[4];
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+               : "=r"(u[0]), "=r"(u[1]), "=r"(u[2]), "=r"(u[3])
+               : "r"(taddr)
+               : "memory");
+#pragma unroll
+  for (int i = 0; i < 4; ++i) r[i] = __uint_as_float(u[i]);
+}
+__device__ __forceinline__ void tmem_wait4(float (&r)[4], bool do_wait) {
+  if (do_wait) asm volatile("tcgen05.wait::ld.sync.aligned;" : "+f"(r[0]), "+f"(r[1]), "+f"(r[2]), "+f"(r[3]) : : "memory");
+  else asm volatile("" : "+f"(r[0]), "+f"(r[1]), "+f"(r[2]), "+f"(r[3]) : : "memory");
+}
+__device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+
+template <int KP, bool HASV>
+struct FwdSmem {
+  static constexpr int NACC = HASV ? 6 : 4;
+  static constexpr int A_BYTES = NACC * 128 * KP * 2;
+  static constexpr int B_TILE = NE * KP * 2;
+  static constexpr int GRP_BYTES = NSLOT * B_TILE + NSLOT * (int)sizeof(TileMeta);
+  static constexpr int BAR_OFF = A_BYTES + NGRP * GRP_BYTES;
+  static constexpr int NBAR_G = 2 * NSLOT + 4; // meta_full[NSLOT], meta_empty[NSLOT], tmem_full[2], tmem_empty[2]
+  static constexpr int NBAR = NGRP * NBAR_G;
+  static constexpr int TOTAL = BAR_OFF + NBAR * 8 + 32 + 128 /* alignment slack */;
+  static constexpr int TMEM_COLS = (NGRP * 2 * NACC * NE <= 256) ? 256 : 512;
+};
+
+// FT: the feature width when it is known at compile time (row offsets become immediates), 0 = use a.F
+template <int KP, bool HASV, int FT>
+__global__ void __launch_bounds__(NTHR, 1)
+edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, const __nv_bfloat16* __restrict__ phi,
+              const float* __restrict__ s_in, int64_t ld_sin, const __nv_bfloat16* __restrict__ v_in,
+              const float* __restrict__ v_res, float* __restrict__ s1, int64_t ld_s1, float* __restrict__ v1,
+              EdgeMirror mir) {
+  using L = FwdSmem<KP, HASV>;
+  constexpr int NACC = L::NACC, KS = KP / 16, KC = KP / 8;
+  if (*a.d_err & ERRF_EDGE_OVERFLOW) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const uint32_t raw = smem_u32(smem_raw);
+  const uint32_t base = (raw + 127u) & ~127u;
+  unsigned char* sm = smem_raw + (base - raw);
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sm + L::BAR_OFF);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + L::NBAR);
+  int* range = reinterpret_cast<int*>(tmem_slot + 1); // [2]: this CTA's atom range
+  const uint32_t bar0 = base + L::BAR_OFF;
+  auto meta_full = [&](int g, int s) { return bar0 + 8u * (g * L::NBAR_G + s); };
+  auto meta_empty = [&](int g, int s) { return bar0 + 8u * (g * L::NBAR_G + NSLOT + s); };
+  auto tmem_full = [&](int g, int b) { return bar0 + 8u * (g * L::NBAR_G + 2 * NSLOT + b); };
+  auto tmem_empty = [&](int g, int b) { return bar0 + 8u * (g * L::NBAR_G + 2 * NSLOT + 2 + b); };
+
+  // resident A operand: the packed filter image of this block, copied verbatim
+  {
+    const uint4* src = reinterpret_cast<const uint4*>(fltT);
+    uint4* dst = reinterpret_cast<uint4*>(sm);
+    for (int i = tid; i < L::A_BYTES / 16; i += NTHR) dst[i] = __ldg(src + i);
+  }
+  if (tid == 0) {
+    for (int g = 0; g < NGRP; ++g) {
+      for (int s = 0; s < NSLOT; ++s) { mbar_init(meta_full(g, s), 1); mbar_init(meta_empty(g, s), EPW); }
+      for (int b = 0; b < 2; ++b) { mbar_init(tmem_full(g, b), 1); mbar_init(tmem_empty(g, b), EPW); }
+    }
+    mbar_init_fence();
+  }
+  if (warp == 0 && lane < 2) {
+    // this CTA's contiguous atom range, balanced by edge count: [first atom with rowptr >= b E / nCTA, same for b + 1)
+    const int b = blockIdx.x + lane;
+    int res;
+    if (b == 0) res = 0;
+    else if (b >= (int)gridDim.x) res = (int)a.N;
+    else {
+      const int64_t E = __ldg(a.rowptr + a.N);
+      const int target = (int)(E * b / gridDim.x);
+      int lo = 0, hi = (int)a.N; // first i in [0, N] with rowptr[i] >= target
+      while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (__ldg(a.rowptr + mid) >= target) hi = mid; else lo = mid + 1;
+      }
+      res = lo;
+    }
+    range[lane] = res;
+  }
+  if (warp == NGRP * EPW) tmem_alloc<L::TMEM_COLS>(tmem_slot);
+  fence_proxy_async_smem(); // the A image was written with st.shared and is read by the MMA (async proxy)
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+  const int c_lo = range[0], c_hi = range[1];
+
+  const int F = FT ? FT : a.F;
+  // window w of this CTA = atoms [c_lo + w RA, min(c_lo + (w+1) RA, c_hi)), handled by pipeline w % NGRP
+
+  if (warp >= NGRP * EPW) {
+    // ================================================================== producer pp of pipeline g
+    const int g = (warp - NGRP * EPW) / NPROD, pp = (warp - NGRP * EPW) % NPROD;
+    unsigned char* grp = sm + L::A_BYTES + g * L::GRP_BYTES;
+    const uint32_t grp_u = base + L::A_BYTES + g * L::GRP_BYTES;
+    const int r = lane & 15, half = lane >> 4;
+    const float rc = a.rc;
+    const float dmu = (a.K > 1) ? rc / (float)(a.K - 1) : rc;
+    const float gamma = 1.0f / (2.0f * dmu * dmu);
+    const float pi_rc = 3.14159265358979323846f / rc;
+    const float bes_A = sqrtf(2.0f / rc);
+    const uint32_t row16 = (uint32_t)(3 * F / 8); // 16-byte units per row of phi / v_in
+    constexpr uint32_t idesc = umma_idesc_bf16(128, NE);
+    uint32_t n = 0; // tiles of this pipeline so far (both producers count all of them)
+    for (int64_t a0 = (int64_t)c_lo + (int64_t)g * RA; a0 < c_hi; a0 += (int64_t)NGRP * RA) {
+      const int64_t a1 = min(a0 + RA, (int64_t)c_hi);
+      const int na = (int)(a1 - a0);
+      const int rp = (lane <= na) ? __ldg(a.rowptr + a0 + lane) : 0x7fffffff; // RA <= 16
+      const int E0 = __shfl_sync(0xffffffffu, rp, 0), E1 = __shfl_sync(0xffffffffu, rp, na);
+      for (int e0 = E0; e0 < E1; e0 += NE, ++n) {
+        if ((n % NPROD) != (uint32_t)pp) continue;
+        const int slot = n % NSLOT;
+        mbar_wait_sleep(meta_empty(g, slot), ((n / NSLOT) & 1u) ^ 1u);
+        TileMeta* mt = reinterpret_cast<TileMeta*>(grp + NSLOT * L::B_TILE) + slot;
+        unsigned char* Bt = grp + slot * L::B_TILE;
+        const int e = e0 + r;
+        const bool ok = e < E1;
+        float4 gq = make_float4(0.f, 0.f, 0.f, 1.f);
+        int j = 0;
+        if (ok) { gq = __ldg(reinterpret_cast<const float4*>(a.geom) + e); j = __ldg(a.col + e); }
+        // receiver of edge e: a0 + max{l in 0..na-1 : rowptr[a0 + l] <= e} (binary search over the lanes' rowptr values)
+        int pos = 0;
+#pragma unroll
+        for (int step = 16; step >= 1; step >>= 1) {
+          const int t = pos + step;
+          const int val = __shfl_sync(0xffffffffu, rp, t & 31);
+          if (t < na && val <= e) pos = t;
+        }
+        const int rcv = (int)a0 + pos;
+        const float d = gq.w;
+        float sn_, cs_;
+        __sincosf(pi_rc * d, &sn_, &cs_);
+        const float cut = ok ? 0.5f * (cs_ + 1.0f) : 0.0f;
+        // this lane's KP/2 columns k = half*KP/2 ... : g_k(d) c(d) (k < K), c(d) (k == K), 0 (k > K)
+#pragma unroll
+        for (int q = 0; q < KP / 16; ++q) {
+          float v[8];
+#pragma unroll
+          for (int x = 0; x < 8; ++x) {
+            const int k = half * (KP / 2) + q * 8 + x;
+            float val;
+            if (a.rbf == 1) val = bes_A * __sinf((float)(k + 1) * pi_rc * d) / d;
+            else { const float dd = d - (float)k * dmu; val = __expf(-gamma * dd * dd); }
+            v[x] = (k < a.K) ? val * cut : (k == a.K ? cut : 0.0f);
+          }
+          const int kc = half * (KP / 16) + q;
+          *reinterpret_cast<uint4*>(Bt + (r >> 3) * (KC * 128) + kc * 128 + (r & 7) * 16) =
+              make_uint4(pack_bf2(v[0], v[1]), pack_bf2(v[2], v[3]), pack_bf2(v[4], v[5]), pack_bf2(v[6], v[7]));
+        }
+#pragma unroll
+        for (int hh = 0; hh < SPLIT; ++hh) {
+          const uint32_t m = __ballot_sync(0xffffffffu, ok && half == 0 && (rcv % SPLIT) == hh);
+          if (lane == 0) mt->mask[hh] = m;
+        }
+        if (half == 0) {
+          mt->U[r] = make_float4(gq.x, gq.y, gq.z, __int_as_float(rcv));
+          mt->OFF[r] = (uint32_t)j * row16;
+        }
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(meta_full(g, slot));
+          const uint32_t buf = n & 1u;
+          mbar_wait_sleep(tmem_empty(g, buf), ((n >> 1) & 1u) ^ 1u); // the epilogue has read tile n - 2 out of this buffer
+          tc_fence_after();
+          const uint32_t bt_u = grp_u + slot * L::B_TILE;
+#pragma unroll
+          for (int acc = 0; acc < NACC; ++acc)
+#pragma unroll
+            for (int ks = 0; ks < KS; ++ks)
+              umma_bf16(tmem_base + (uint32_t)(((g * 2 + buf) * NACC + acc) * NE),
+                        umma_desc_nosw(base + acc * (128 * KP * 2) + ks * 256, 128, KC * 128),
+                        umma_desc_nosw(bt_u + ks * 256, 128, KC * 128), idesc, ks ? 1u : 0u);
+          umma_commit(tmem_full(g, buf));
+        }
+        __syncwarp();
+      }
+    }
+  } else {
+    // ================================================================== epilogue warp (pipeline g, TMEM quadrant q)
+    const int g = warp / EPW, q = warp % 4, h = (warp % EPW) / 4; // h: takes the receivers with i % SPLIT == h
+    unsigned char* grp = sm + L::A_BYTES + g * L::GRP_BYTES;
+    const int p = q * 32 + lane;       // feature pair
+    const bool act = FT ? (2 * p < FT) : (2 * p < F);
+    const int f0 = act ? 2 * p : 0;    // inactive lanes compute on pair 0 and store nothing
+    const char* phi_f = reinterpret_cast<const char*>(phi) + f0 * 2;
+    const char* vin_f = reinterpret_cast<const char*>(v_in) + f0 * 2;
+    uint32_t n = 0;
+    for (int64_t a0 = (int64_t)c_lo + (int64_t)g * RA; a0 < c_hi; a0 += (int64_t)NGRP * RA) {
+      const int64_t a1 = min(a0 + RA, (int64_t)c_hi);
+      const int E0 = __ldg(a.rowptr + a0), E1 = __ldg(a.rowptr + a1);
+      int cur = (int)a0 + ((h - (int)(a0 % SPLIT) + SPLIT) % SPLIT); // my first atom of the window
+      float2 as = make_float2(0.f, 0.f), av[3], rs, rv[3];
+      av[0] = av[1] = av[2] = make_float2(0.f, 0.f);
+      rs = rv[0] = rv[1] = rv[2] = make_float2(0.f, 0.f);
+      auto begin_row = [&](int i) { // residual row of receiver i: loaded now, used when the receiver is complete
+        as = av[0] = av[1] = av[2] = make_float2(0.f, 0.f);
+        rs = ld_stream2(s_in + (int64_t)i * ld_sin + f0);
+        if (HASV) {
+#pragma unroll
+          for (int ax = 0; ax < 3; ++ax) rv[ax] = ld_stream2(v_res + ((int64_t)i * 3 + ax) * F + f0);
+        }
+      };
+      auto end_row = [&](int i) {
+        if (!act) return;
+        const float2 o = make_float2(rs.x + as.x, rs.y + as.y);
+        st_stream2(s1 + (int64_t)i * ld_s1 + f0, o);
+        if (mir.s1) st_stream1(mir.s1 + (int64_t)i * mir.ld_s1 + f0, pack_bf2(o.x, o.y));
+#pragma unroll
+        for (int ax = 0; ax < 3; ++ax) {
+          const float2 ov = make_float2(rv[ax].x + av[ax].x, rv[ax].y + av[ax].y);
+          const int64_t off = ((int64_t)i * 3 + ax) * F + f0;
+          st_stream2(v1 + off, ov);
+          if (mir.v1) st_stream1(mir.v1 + off, pack_bf2(ov.x, ov.y));
+        }
+      };
+      if (cur < (int)a1) begin_row(cur);
+      for (int e0 = E0; e0 < E1; e0 += NE, ++n) {
+        const int slot = n % NSLOT;
+        const uint32_t buf = n & 1u;
+        const TileMeta* mt = reinterpret_cast<const TileMeta*>(grp + NSLOT * L::B_TILE) + slot;
+        mbar_wait_sleep(meta_full(g, slot), (n / NSLOT) & 1u);
+        const uint32_t mymask = mt->mask[h];
+        // (every warp observes every phase of the barrier, also for tiles it has no edge in: a parity wait two phases
+        // behind would pass at once)
+        mbar_wait_sleep(tmem_full(g, buf), (n >> 1) & 1u);
+        if (mymask) {
+          tc_fence_after();
+          const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)((g * 2 + buf) * NACC * NE);
+#pragma unroll 1
+          for (int c0 = 0; c0 < NE; c0 += ES) {
+            const uint32_t m4 = (mymask >> c0) & ((1u << ES) - 1u);
+            if (!m4) continue;
+            float W[NACC][ES];
+#pragma unroll
+            for (int acc = 0; acc < NACC; ++acc) tmem_ld4_async(taddr + acc * NE + c0, W[acc]);
+            const uint4 oo = *reinterpret_cast<const uint4*>(mt->OFF + c0);
+            const uint32_t offs[4] = {oo.x, oo.y, oo.z, oo.w};
+            uint32_t gw[ES][6];
+#pragma unroll
+            for (int c = 0; c < ES; ++c) {
+              if (m4 & (1u << c)) {
+                const char* pr = phi_f + (uint64_t)offs[c] * 16u;
+                gw[c][0] = ldg_nc32(pr); gw[c][1] = ldg_nc32(pr + 2 * F);
+                if (HASV) {
+                  gw[c][2] = ldg_nc32(pr + 4 * F);
+                  const char* vr = vin_f + (uint64_t)offs[c] * 16u;
+                  gw[c][3] = ldg_nc32(vr); gw[c][4] = ldg_nc32(vr + 2 * F); gw[c][5] = ldg_nc32(vr + 4 * F);
+                }
+              }
+            }
+#pragma unroll
+            for (int acc = 0; acc < NACC; ++acc) tmem_wait4(W[acc], acc == 0);
+#pragma unroll
+            for (int c = 0; c < ES; ++c) {
+              if (m4 & (1u << c)) {
+                const float4 u = mt->U[c0 + c];
+                const int i = __float_as_int(u.w);
+                if (i != cur) { // receiver complete: write it (and any edge-less atoms of mine before the next one)
+                  end_row(cur);
+                  for (int k = cur + SPLIT; k < i; k += SPLIT) { begin_row(k); end_row(k); }
+                  cur = i;
+                  begin_row(cur);
+                }
+                as = __ffma2_rn(bf2(gw[c][0]), make_float2(W[0][c], W[1][c]), as);
+                const float2 xvs = __fmul2_rn(bf2(gw[c][1]), make_float2(W[2][c], W[3][c]));
+                av[0] = __ffma2_rn(xvs, make_float2(u.x, u.x), av[0]);
+                av[1] = __ffma2_rn(xvs, make_float2(u.y, u.y), av[1]);
+                av[2] = __ffma2_rn(xvs, make_float2(u.z, u.z), av[2]);
+                if (HASV) {
+                  const float2 xvv = __fmul2_rn(bf2(gw[c][2]), make_float2(W[NACC - 2][c], W[NACC - 1][c]));
+                  av[0] = __ffma2_rn(xvv, bf2(gw[c][3]), av[0]);
+                  av[1] = __ffma2_rn(xvv, bf2(gw[c][4]), av[1]);
+                  av[2] = __ffma2_rn(xvv, bf2(gw[c][5]), av[2]);
+                }
+              }
+            }
+          }
+          tc_fence_before();
+        }
+        __syncwarp();
+        if (lane == 0) { mbar_arrive(tmem_empty(g, buf)); mbar_arrive(meta_empty(g, slot)); }
+      }
+      if (cur < (int)a1) {
+        end_row(cur);
+        for (int k = cur + SPLIT; k < (int)a1; k += SPLIT) { begin_row(k); end_row(k); }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == NGRP * EPW) {
+    tc_fence_after();
+    tmem_dealloc<L::TMEM_COLS>(tmem_base);
+  }
+}
+
+uint16_t to_bf16_host(double x) {
+  float f = (float)x;
+  uint32_t u;
+  std::memcpy(&u, &f, 4);
+  const uint32_t r = u + 0x7fffu + ((u >> 16) & 1u); // round to nearest even
+  return (uint16_t)(r >> 16);
+}
+
+} // namespace
+
+// Host-side packing of one block's filter as the resident A operand of edge_fwd_tc_k: 6 accumulator tiles
+// a = chunk*2 + parity of 128 rows x KP columns, row l = filter row of feature 2l + parity (zero for 2l + parity >= F),
+// column k < K: flt_W, k == K: flt_b, then zeros; stored in the UMMA no-swizzle K-major layout
+// [16 row groups][KP/8 column chunks][8 rows][8 elements].
+int64_t edge_tc_filter_elems(int K) { return (int64_t)6 * 128 * edge_mma_kp(K); }
+
+void pack_filter_tc(int F, int K, const double* fltW, const double* fltb, uint16_t* out) {
+  const int KP = edge_mma_kp(K), KC = KP / 8;
+  std::memset(out, 0, sizeof(uint16_t) * (size_t)edge_tc_filter_elems(K));
+  for (int c = 0; c < 3; ++c)
+    for (int par = 0; par < 2; ++par)
+      for (int l = 0; l < 128; ++l) {
+        const int f = 2 * l + par;
+        if (f >= F) continue;
+        const int64_t src = (int64_t)c * F + f;
+        uint16_t* tile = out + (size_t)(c * 2 + par) * 128 * KP;
+        for (int k = 0; k <= K; ++k) {
+          const uint16_t val = k < K ? to_bf16_host(fltW[src * K + k]) : to_bf16_host(fltb[src]);
+          tile[((size_t)((l >> 3) * KC + (k >> 3)) * 8 + (l & 7)) * 8 + (k & 7)] = val;
+        }
+      }
+}
+
+int launch_edge_fwd_tc(const EdgeMmaArgs& a, const __nv_bfloat16* fltT, const __nv_bfloat16* phi, const float* s_in,
+                       int64_t ld_sin, const __nv_bfloat16* v_in, const float* v_res, float* s1, int64_t ld_s1, float* v1,
+                       const EdgeMirror& mir, cudaStream_t st) {
+  if (a.N == 0) return 0;
+  const int KP = edge_mma_kp(a.K);
+  // One persistent CTA per SM takes a contiguous, edge-balanced range of atoms and cuts it into windows of RA atoms that
+  // alternate between its pipelines: about 4 windows per pipeline, between 2 and 16 atoms each.
+  const int RA = (int)std::min<int64_t>(16, std::max<int64_t>(2, a.N / (148 * NGRP * 4)));
+  const unsigned grid = (unsigned)std::min<int64_t>(148, (a.N + RA * NGRP - 1) / (RA * NGRP));
+#define PNN_LAUNCH2(KPV, HV, FTV)                                                                                    \
+  {                                                                                                                  \
+    using L = FwdSmem<KPV, HV>;                                                                                      \
+    static bool attr_set = false;                                                                                    \
+    if (!attr_set) {                                                                                                 \
+      cudaFuncSetAttribute(edge_fwd_tc_k<KPV, HV, FTV>, cudaFuncAttributeMaxDynamicSharedMemorySize, L::TOTAL);      \
+      attr_set = true;                                                                                               \
+    }                                                                                                                \
+    edge_fwd_tc_k<KPV, HV, FTV><<<grid, NTHR, L::TOTAL, st>>>(a, RA, fltT, phi, s_in, ld_sin, v_in, v_res, s1, ld_s1, \
+                                                              v1, mir);                                              \
+    PNN_KCHECK("edge_fwd_tc_k");                                                                                     \
+  }
+#define PNN_LAUNCH(KPV, HV) { if (a.F == 256) PNN_LAUNCH2(KPV, HV, 256) else PNN_LAUNCH2(KPV, HV, 0) }
+  const bool hv = v_in != nullptr;
+  if (KP == 16) { if (hv) PNN_LAUNCH(16, true) else PNN_LAUNCH(16, false) }
+  else if (KP == 32) { if (hv) PNN_LAUNCH(32, true) else PNN_LAUNCH(32, false) }
+  else { if (hv) PNN_LAUNCH(48, true) else PNN_LAUNCH(48, false) }
+#undef PNN_LAUNCH2
+#undef PNN_LAUNCH
+  return 1;
+}
+
+} // namespace pnn

@@ -87,6 +87,8 @@ struct pnn_model {
   __nv_bfloat16* d_wb = nullptr;                        // BF16 copy of d_w (same offsets): tcgen05 GEMM operands
   __nv_bfloat16* d_fltP = nullptr;                      // BF16 model: per block, the filter packed for edge_mma.cu
   int64_t fltP_stride = 0;                              // elements per block
+  __nv_bfloat16* d_fltT = nullptr;                      // BF16 model: per block, the filter image of edge_tc.cu
+  int64_t fltT_stride = 0;
 };
 
 struct pnn_workspace {
@@ -268,9 +270,21 @@ int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, 
         pack_filter_bf16((int)F, (int)K, fW, fW + 3 * F * K, fp.data() + (size_t)t * m->fltP_stride);
       }
     }
+    m->fltT_stride = edge_tc_filter_elems(cfg->K);
+    std::vector<uint16_t> ft((size_t)cfg->T * m->fltT_stride);
+    {
+      const double* q = w + (int64_t)(cfg->Zmax + 1) * F;
+      const int64_t per_block = 11 * F * F + 3 * F * K + 11 * F;
+      for (int t = 0; t < cfg->T; ++t) {
+        const double* fW = q + t * per_block + (F * F + F + 3 * F * F + 3 * F);
+        pack_filter_tc((int)F, (int)K, fW, fW + 3 * F * K, ft.data() + (size_t)t * m->fltT_stride);
+      }
+    }
     if (!cuda_ok(cudaMalloc((void**)&m->d_fltP, fp.size() * 2), "cudaMalloc(packed filters)") ||
-        !cuda_ok(cudaMemcpy(m->d_fltP, fp.data(), fp.size() * 2, cudaMemcpyHostToDevice), "cudaMemcpy(packed filters)")) {
-      cudaFree(m->d_fltP); cudaFree(m->d_wb); cudaFree(m->d_w); delete m; return PNN_ERR_CUDA;
+        !cuda_ok(cudaMemcpy(m->d_fltP, fp.data(), fp.size() * 2, cudaMemcpyHostToDevice), "cudaMemcpy(packed filters)") ||
+        !cuda_ok(cudaMalloc((void**)&m->d_fltT, ft.size() * 2), "cudaMalloc(filter images)") ||
+        !cuda_ok(cudaMemcpy(m->d_fltT, ft.data(), ft.size() * 2, cudaMemcpyHostToDevice), "cudaMemcpy(filter images)")) {
+      cudaFree(m->d_fltT); cudaFree(m->d_fltP); cudaFree(m->d_wb); cudaFree(m->d_w); delete m; return PNN_ERR_CUDA;
     }
   }
   *out = m;
@@ -279,6 +293,7 @@ int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, 
 
 void pnn_model_destroy(pnn_model* m) {
   if (!m) return;
+  cudaFree(m->d_fltT);
   cudaFree(m->d_fltP);
   cudaFree(m->d_wb);
   cudaFree(m->d_w);
@@ -732,7 +747,8 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       EdgeMirror mir; mir.s1 = mb.sn16; mir.ld_s1 = 2 * F; mir.v1 = mb.v1_16;
       em.fltP = m->d_fltP + (int64_t)t * m->fltP_stride;
       const int l_ = simt_edges ? launch_edge_fwd<T, B>(ea, tp16.phi16, s_cur, F, v_in16, v_in, sn, 2 * F, v1, mir, st)
-                                : launch_edge_fwd_mma(em, tp16.phi16, s_cur, F, v_in16, v_in, sn, 2 * F, v1, mir, st); // B3b
+                                : launch_edge_fwd_tc(em, m->d_fltT + (int64_t)t * m->fltT_stride, tp16.phi16, s_cur, F,
+                                                     v_in16, v_in, sn, 2 * F, v1, mir, st); // B3b
       nl += l_; ps_.done(l_); }
     TcEpi e3; e3.Cb = PQ; e3.ldcb = 2 * F;
     tc("gemm_3N", 3 * N, 2 * F, F, mb.v1_16, F, b.UV, e3);                         // B4: P | Q
