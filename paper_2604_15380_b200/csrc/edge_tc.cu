@@ -46,10 +46,14 @@ constexpr int NPROD = 2; // producer warps per pipeline (tile n is staged and is
 constexpr int NTHR = NGRP * (EPW + NPROD) * 32;
 constexpr int ES = 4;    // edges per epilogue step (TMEM columns per tcgen05.ld)
 
+// A tile = 4 steps of 4 TMEM columns; a step holds up to 4 edges of ONE receiver (a receiver with d edges takes
+// ceil(d / 4) steps, the last one ragged), so a step is processed by exactly one epilogue half (receiver % SPLIT).
 struct TileMeta {
-  float4 U[NE];        // unit vector; .w = receiver index (bit pattern)
-  uint32_t OFF[NE];    // sender row offset in 16-byte units (row = 3F BF16)
-  uint32_t mask[SPLIT]; // bit c: edge c of the tile is valid and its receiver belongs to epilogue half h
+  float4 U[NE];         // per column: unit vector (w unused)
+  uint32_t OFF[NE];     // per column: sender row offset in 16-byte units (row = 3F BF16)
+  int srecv[NE / ES];   // per step: receiver
+  int scnt[NE / ES];    // per step: valid edges (0 = unused step)
+  uint32_t smask[SPLIT]; // bit s: step s is used and belongs to epilogue half h
   uint32_t pad[4 - SPLIT];
 };
 
@@ -196,28 +200,38 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
     for (int64_t a0 = (int64_t)c_lo + (int64_t)g * RA; a0 < c_hi; a0 += (int64_t)NGRP * RA) {
       const int64_t a1 = min(a0 + RA, (int64_t)c_hi);
       const int na = (int)(a1 - a0);
-      const int rp = (lane <= na) ? __ldg(a.rowptr + a0 + lane) : 0x7fffffff; // RA <= 16
-      const int E0 = __shfl_sync(0xffffffffu, rp, 0), E1 = __shfl_sync(0xffffffffu, rp, na);
-      for (int e0 = E0; e0 < E1; e0 += NE, ++n) {
+      // lane l < na: receiver a0 + l; so = exclusive prefix sum of its steps (lane na: the window's total)
+      const int rp = (lane <= na) ? __ldg(a.rowptr + a0 + lane) : 0;
+      const int rp1 = __shfl_down_sync(0xffffffffu, rp, 1);
+      const int nst = (lane < na) ? (rp1 - rp + ES - 1) / ES : 0;
+      int so = nst;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, so, o); if (lane >= o) so += t; }
+      so -= nst;
+      const int tot = __shfl_sync(0xffffffffu, so, na);
+      for (int s0 = 0; s0 < tot; s0 += NE / ES, ++n) {
         if ((n % NPROD) != (uint32_t)pp) continue;
         const int slot = n % NSLOT;
         mbar_wait_sleep(meta_empty(g, slot), ((n / NSLOT) & 1u) ^ 1u);
         TileMeta* mt = reinterpret_cast<TileMeta*>(grp + NSLOT * L::B_TILE) + slot;
         unsigned char* Bt = grp + slot * L::B_TILE;
-        const int e = e0 + r;
-        const bool ok = e < E1;
-        float4 gq = make_float4(0.f, 0.f, 0.f, 1.f);
-        int j = 0;
-        if (ok) { gq = __ldg(reinterpret_cast<const float4*>(a.geom) + e); j = __ldg(a.col + e); }
-        // receiver of edge e: a0 + max{l in 0..na-1 : rowptr[a0 + l] <= e} (binary search over the lanes' rowptr values)
+        // this lane's column r = step (r / 4), position (r % 4): receiver = last lane l < na with so[l] <= step
+        const int S = s0 + (r >> 2);
         int pos = 0;
 #pragma unroll
         for (int step = 16; step >= 1; step >>= 1) {
           const int t = pos + step;
-          const int val = __shfl_sync(0xffffffffu, rp, t & 31);
-          if (t < na && val <= e) pos = t;
+          const int val = __shfl_sync(0xffffffffu, so, t & 31);
+          if (t < na && val <= S) pos = t;
         }
+        const int so_p = __shfl_sync(0xffffffffu, so, pos), rp_p = __shfl_sync(0xffffffffu, rp, pos),
+                  rp_n = __shfl_sync(0xffffffffu, rp, pos + 1);
+        const int e = rp_p + (S - so_p) * ES + (r & 3);
+        const bool ok = S < tot && e < rp_n;
         const int rcv = (int)a0 + pos;
+        float4 gq = make_float4(0.f, 0.f, 0.f, 1.f);
+        int j = 0;
+        if (ok) { gq = __ldg(reinterpret_cast<const float4*>(a.geom) + e); j = __ldg(a.col + e); }
         const float d = gq.w;
         float sn_, cs_;
         __sincosf(pi_rc * d, &sn_, &cs_);
@@ -238,14 +252,20 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
           *reinterpret_cast<uint4*>(Bt + (r >> 3) * (KC * 128) + kc * 128 + (r & 7) * 16) =
               make_uint4(pack_bf2(v[0], v[1]), pack_bf2(v[2], v[3]), pack_bf2(v[4], v[5]), pack_bf2(v[6], v[7]));
         }
+        const uint32_t okm = __ballot_sync(0xffffffffu, ok && half == 0); // bit r: column r holds an edge
+        if (half == 0) {
+          mt->U[r] = gq;
+          mt->OFF[r] = (uint32_t)j * row16;
+          if ((r & 3) == 0) {
+            mt->srecv[r >> 2] = rcv;
+            mt->scnt[r >> 2] = __popc((okm >> r) & 15u);
+          }
+        }
 #pragma unroll
         for (int hh = 0; hh < SPLIT; ++hh) {
-          const uint32_t m = __ballot_sync(0xffffffffu, ok && half == 0 && (rcv % SPLIT) == hh);
-          if (lane == 0) mt->mask[hh] = m;
-        }
-        if (half == 0) {
-          mt->U[r] = make_float4(gq.x, gq.y, gq.z, __int_as_float(rcv));
-          mt->OFF[r] = (uint32_t)j * row16;
+          const uint32_t m = __ballot_sync(0xffffffffu, ok && half == 0 && (r & 3) == 0 && (rcv % SPLIT) == hh);
+          // bit 4 s of m -> bit s
+          if (lane == 0) mt->smask[hh] = (m & 1u) | ((m >> 3) & 2u) | ((m >> 6) & 4u) | ((m >> 9) & 8u);
         }
         fence_proxy_async_smem();
         __syncwarp();
@@ -279,7 +299,15 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
     uint32_t n = 0;
     for (int64_t a0 = (int64_t)c_lo + (int64_t)g * RA; a0 < c_hi; a0 += (int64_t)NGRP * RA) {
       const int64_t a1 = min(a0 + RA, (int64_t)c_hi);
-      const int E0 = __ldg(a.rowptr + a0), E1 = __ldg(a.rowptr + a1);
+      const int na = (int)(a1 - a0);
+      int tot; // steps of the window (as the producer counts them)
+      {
+        const int rp = (lane <= na) ? __ldg(a.rowptr + a0 + lane) : 0;
+        const int rp1 = __shfl_down_sync(0xffffffffu, rp, 1);
+        tot = (lane < na) ? (rp1 - rp + ES - 1) / ES : 0;
+#pragma unroll
+        for (int o = 16; o; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+      }
       int cur = (int)a0 + ((h - (int)(a0 % SPLIT) + SPLIT) % SPLIT); // my first atom of the window
       float2 as = make_float2(0.f, 0.f), av[3], rs, rv[3];
       av[0] = av[1] = av[2] = make_float2(0.f, 0.f);
@@ -306,12 +334,12 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
         }
       };
       if (cur < (int)a1) begin_row(cur);
-      for (int e0 = E0; e0 < E1; e0 += NE, ++n) {
+      for (int s0 = 0; s0 < tot; s0 += NE / ES, ++n) {
         const int slot = n % NSLOT;
         const uint32_t buf = n & 1u;
         const TileMeta* mt = reinterpret_cast<const TileMeta*>(grp + NSLOT * L::B_TILE) + slot;
         mbar_wait_sleep(meta_full(g, slot), (n / NSLOT) & 1u);
-        const uint32_t mymask = mt->mask[h];
+        const uint32_t mymask = mt->smask[h];
         // (every warp observes every phase of the barrier, also for tiles it has no edge in: a parity wait two phases
         // behind would pass at once)
         mbar_wait_sleep(tmem_full(g, buf), (n >> 1) & 1u);
@@ -319,18 +347,19 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
           tc_fence_after();
           const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)((g * 2 + buf) * NACC * NE);
 #pragma unroll 1
-          for (int c0 = 0; c0 < NE; c0 += ES) {
-            const uint32_t m4 = (mymask >> c0) & ((1u << ES) - 1u);
-            if (!m4) continue;
+          for (int si = 0; si < NE / ES; ++si) {
+            if (!((mymask >> si) & 1u)) continue;
+            const int c0 = si * ES;
             float W[NACC][ES];
 #pragma unroll
             for (int acc = 0; acc < NACC; ++acc) tmem_ld4_async(taddr + acc * NE + c0, W[acc]);
             const uint4 oo = *reinterpret_cast<const uint4*>(mt->OFF + c0);
             const uint32_t offs[4] = {oo.x, oo.y, oo.z, oo.w};
+            const int i = mt->srecv[si], cnt = mt->scnt[si];
             uint32_t gw[ES][6];
 #pragma unroll
             for (int c = 0; c < ES; ++c) {
-              if (m4 & (1u << c)) {
+              if (c < cnt) {
                 const char* pr = phi_f + (uint64_t)offs[c] * 16u;
                 gw[c][0] = ldg_nc32(pr); gw[c][1] = ldg_nc32(pr + 2 * F);
                 if (HASV) {
@@ -340,19 +369,18 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
                 }
               }
             }
+            if (i != cur) { // receiver complete: write it (and any edge-less atoms of mine before the next one)
+              end_row(cur);
+              for (int k = cur + SPLIT; k < i; k += SPLIT) { begin_row(k); end_row(k); }
+              cur = i;
+              begin_row(cur);
+            }
 #pragma unroll
             for (int acc = 0; acc < NACC; ++acc) tmem_wait4(W[acc], acc == 0);
 #pragma unroll
             for (int c = 0; c < ES; ++c) {
-              if (m4 & (1u << c)) {
+              if (c < cnt) {
                 const float4 u = mt->U[c0 + c];
-                const int i = __float_as_int(u.w);
-                if (i != cur) { // receiver complete: write it (and any edge-less atoms of mine before the next one)
-                  end_row(cur);
-                  for (int k = cur + SPLIT; k < i; k += SPLIT) { begin_row(k); end_row(k); }
-                  cur = i;
-                  begin_row(cur);
-                }
                 as = __ffma2_rn(bf2(gw[c][0]), make_float2(W[0][c], W[1][c]), as);
                 const float2 xvs = __fmul2_rn(bf2(gw[c][1]), make_float2(W[2][c], W[3][c]));
                 av[0] = __ffma2_rn(xvs, make_float2(u.x, u.x), av[0]);
