@@ -24,6 +24,7 @@
 //             the arithmetic of this one), runs the edge loop, and at every change of receiver adds the residual row
 //             and writes s', v' (FP32) and their BF16 copies with coalesced 8-byte / 4-byte stores.
 #include <algorithm>
+#include <cstddef>
 #include <cstring>
 #include <vector>
 
@@ -49,13 +50,48 @@ constexpr int ES = 4;    // edges per epilogue step (TMEM columns per tcgen05.ld
 // A tile = 4 steps of 4 TMEM columns; a step holds up to 4 edges of ONE receiver (a receiver with d edges takes
 // ceil(d / 4) steps, the last one ragged), so a step is processed by exactly one epilogue half (receiver % SPLIT).
 struct TileMeta {
-  float4 U[NE];         // per column: unit vector (w unused)
-  uint32_t OFF[NE];     // per column: sender row offset in 16-byte units (row = 3F BF16)
-  int srecv[NE / ES];   // per step: receiver
-  int scnt[NE / ES];    // per step: valid edges (0 = unused step)
-  uint32_t smask[SPLIT]; // bit s: step s is used and belongs to epilogue half h
+  float Ux[NE], Uy[NE], Uz[NE]; // per column: unit vector (0 in unused columns)
+  uint32_t OFF[NE];             // per column: sender row offset in 16-byte units (row = 3F BF16)
+  int2 sinfo[NE / ES];          // per step: (receiver, valid edges; 0 = unused step)
+  uint32_t smask[SPLIT];        // bit s: step s is used and belongs to epilogue half h
   uint32_t pad[4 - SPLIT];
 };
+// explicit shared-space loads from 32-bit shared addresses (no generic-to-shared conversions in the inner loops)
+__device__ __forceinline__ uint4 lds128(uint32_t a) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ float4 lds128f(uint32_t a) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ uint2 lds64(uint32_t a) {
+  uint2 v;
+  asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t a) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+  return v;
+}
+// backoff for the waits of warps that are ahead of their consumers (their polling would take issue slots)
+__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  for (;;) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    if (ok) break;
+    __nanosleep(128);
+  }
+}
 
 __device__ __forceinline__ float2 bf2(uint32_t x) {
   return make_float2(__uint_as_float(x << 16), __uint_as_float(x & 0xffff0000u));
@@ -212,7 +248,7 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
       for (int s0 = 0; s0 < tot; s0 += NE / ES, ++n) {
         if ((n % NPROD) != (uint32_t)pp) continue;
         const int slot = n % NSLOT;
-        mbar_wait_sleep(meta_empty(g, slot), ((n / NSLOT) & 1u) ^ 1u);
+        mbar_wait_backoff(meta_empty(g, slot), ((n / NSLOT) & 1u) ^ 1u);
         TileMeta* mt = reinterpret_cast<TileMeta*>(grp + NSLOT * L::B_TILE) + slot;
         unsigned char* Bt = grp + slot * L::B_TILE;
         // this lane's column r = step (r / 4), position (r % 4): receiver = last lane l < na with so[l] <= step
@@ -254,12 +290,9 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
         }
         const uint32_t okm = __ballot_sync(0xffffffffu, ok && half == 0); // bit r: column r holds an edge
         if (half == 0) {
-          mt->U[r] = gq;
+          mt->Ux[r] = ok ? gq.x : 0.f; mt->Uy[r] = ok ? gq.y : 0.f; mt->Uz[r] = ok ? gq.z : 0.f;
           mt->OFF[r] = (uint32_t)j * row16;
-          if ((r & 3) == 0) {
-            mt->srecv[r >> 2] = rcv;
-            mt->scnt[r >> 2] = __popc((okm >> r) & 15u);
-          }
+          if ((r & 3) == 0) mt->sinfo[r >> 2] = make_int2(rcv, __popc((okm >> r) & 15u));
         }
 #pragma unroll
         for (int hh = 0; hh < SPLIT; ++hh) {
@@ -272,7 +305,7 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
         if (lane == 0) {
           mbar_arrive(meta_full(g, slot));
           const uint32_t buf = n & 1u;
-          mbar_wait_sleep(tmem_empty(g, buf), ((n >> 1) & 1u) ^ 1u); // the epilogue has read tile n - 2 out of this buffer
+          mbar_wait_backoff(tmem_empty(g, buf), ((n >> 1) & 1u) ^ 1u); // the epilogue has read tile n - 2 out of this buffer
           tc_fence_after();
           const uint32_t bt_u = grp_u + slot * L::B_TILE;
 #pragma unroll
@@ -290,7 +323,7 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
   } else {
     // ================================================================== epilogue warp (pipeline g, TMEM quadrant q)
     const int g = warp / EPW, q = warp % 4, h = (warp % EPW) / 4; // h: takes the receivers with i % SPLIT == h
-    unsigned char* grp = sm + L::A_BYTES + g * L::GRP_BYTES;
+    const uint32_t grp_u = base + L::A_BYTES + g * L::GRP_BYTES;
     const int p = q * 32 + lane;       // feature pair
     const bool act = FT ? (2 * p < FT) : (2 * p < F);
     const int f0 = act ? 2 * p : 0;    // inactive lanes compute on pair 0 and store nothing
@@ -309,11 +342,18 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
         for (int o = 16; o; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
       }
       int cur = (int)a0 + ((h - (int)(a0 % SPLIT) + SPLIT) % SPLIT); // my first atom of the window
-      float2 as = make_float2(0.f, 0.f), av[3], rs, rv[3];
-      av[0] = av[1] = av[2] = make_float2(0.f, 0.f);
+      // Segment sums of the current receiver.  The packed FMAs pair two EDGES of one feature (component .x: even
+      // columns of the step, .y: odd columns), so that both operands of a packed product are adjacent registers
+      // (two TMEM columns of one accumulator; two unpacked halves): [feature parity] for s, [axis][feature parity] for v.
+      float2 as[2], av[3][2], rs, rv[3];
       rs = rv[0] = rv[1] = rv[2] = make_float2(0.f, 0.f);
+      auto zero_acc = [&]() {
+        as[0] = as[1] = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int ax = 0; ax < 3; ++ax) av[ax][0] = av[ax][1] = make_float2(0.f, 0.f);
+      };
       auto begin_row = [&](int i) { // residual row of receiver i: loaded now, used when the receiver is complete
-        as = av[0] = av[1] = av[2] = make_float2(0.f, 0.f);
+        zero_acc();
         rs = ld_stream2(s_in + (int64_t)i * ld_sin + f0);
         if (HASV) {
 #pragma unroll
@@ -322,24 +362,25 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
       };
       auto end_row = [&](int i) {
         if (!act) return;
-        const float2 o = make_float2(rs.x + as.x, rs.y + as.y);
+        const float2 o = make_float2(rs.x + (as[0].x + as[0].y), rs.y + (as[1].x + as[1].y));
         st_stream2(s1 + (int64_t)i * ld_s1 + f0, o);
         if (mir.s1) st_stream1(mir.s1 + (int64_t)i * mir.ld_s1 + f0, pack_bf2(o.x, o.y));
 #pragma unroll
         for (int ax = 0; ax < 3; ++ax) {
-          const float2 ov = make_float2(rv[ax].x + av[ax].x, rv[ax].y + av[ax].y);
+          const float2 ov = make_float2(rv[ax].x + (av[ax][0].x + av[ax][0].y), rv[ax].y + (av[ax][1].x + av[ax][1].y));
           const int64_t off = ((int64_t)i * 3 + ax) * F + f0;
           st_stream2(v1 + off, ov);
           if (mir.v1) st_stream1(mir.v1 + off, pack_bf2(ov.x, ov.y));
         }
       };
+      zero_acc();
       if (cur < (int)a1) begin_row(cur);
       for (int s0 = 0; s0 < tot; s0 += NE / ES, ++n) {
         const int slot = n % NSLOT;
         const uint32_t buf = n & 1u;
-        const TileMeta* mt = reinterpret_cast<const TileMeta*>(grp + NSLOT * L::B_TILE) + slot;
+        const uint32_t mt_u = grp_u + NSLOT * L::B_TILE + slot * (uint32_t)sizeof(TileMeta);
         mbar_wait_sleep(meta_full(g, slot), (n / NSLOT) & 1u);
-        const uint32_t mymask = mt->smask[h];
+        const uint32_t mymask = lds32(mt_u + (uint32_t)offsetof(TileMeta, smask) + 4u * h);
         // (every warp observes every phase of the barrier, also for tiles it has no edge in: a parity wait two phases
         // behind would pass at once)
         mbar_wait_sleep(tmem_full(g, buf), (n >> 1) & 1u);
@@ -349,16 +390,19 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
 #pragma unroll 1
           for (int si = 0; si < NE / ES; ++si) {
             if (!((mymask >> si) & 1u)) continue;
-            const int c0 = si * ES;
+            const uint32_t cb = (uint32_t)si * (ES * 4); // byte offset of the step's columns in the per-column arrays
             float W[NACC][ES];
 #pragma unroll
-            for (int acc = 0; acc < NACC; ++acc) tmem_ld4_async(taddr + acc * NE + c0, W[acc]);
-            const uint4 oo = *reinterpret_cast<const uint4*>(mt->OFF + c0);
+            for (int acc = 0; acc < NACC; ++acc) tmem_ld4_async(taddr + acc * NE + si * ES, W[acc]);
+            const uint4 oo = lds128(mt_u + (uint32_t)offsetof(TileMeta, OFF) + cb);
+            const uint2 inf = lds64(mt_u + (uint32_t)offsetof(TileMeta, sinfo) + 8u * si);
             const uint32_t offs[4] = {oo.x, oo.y, oo.z, oo.w};
-            const int i = mt->srecv[si], cnt = mt->scnt[si];
+            const int i = (int)inf.x, cnt = (int)inf.y;
             uint32_t gw[ES][6];
 #pragma unroll
             for (int c = 0; c < ES; ++c) {
+#pragma unroll
+              for (int x = 0; x < 6; ++x) gw[c][x] = 0u;
               if (c < cnt) {
                 const char* pr = phi_f + (uint64_t)offs[c] * 16u;
                 gw[c][0] = ldg_nc32(pr); gw[c][1] = ldg_nc32(pr + 2 * F);
@@ -375,22 +419,34 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
               cur = i;
               begin_row(cur);
             }
+            const float4 ux = lds128f(mt_u + (uint32_t)offsetof(TileMeta, Ux) + cb);
+            const float4 uy = lds128f(mt_u + (uint32_t)offsetof(TileMeta, Uy) + cb);
+            const float4 uz = lds128f(mt_u + (uint32_t)offsetof(TileMeta, Uz) + cb);
 #pragma unroll
             for (int acc = 0; acc < NACC; ++acc) tmem_wait4(W[acc], acc == 0);
+            // columns (0, 1) and (2, 3) of the step as packed pairs; unused columns have zero filter values and zero payloads
 #pragma unroll
-            for (int c = 0; c < ES; ++c) {
-              if (c < cnt) {
-                const float4 u = mt->U[c0 + c];
-                as = __ffma2_rn(bf2(gw[c][0]), make_float2(W[0][c], W[1][c]), as);
-                const float2 xvs = __fmul2_rn(bf2(gw[c][1]), make_float2(W[2][c], W[3][c]));
-                av[0] = __ffma2_rn(xvs, make_float2(u.x, u.x), av[0]);
-                av[1] = __ffma2_rn(xvs, make_float2(u.y, u.y), av[1]);
-                av[2] = __ffma2_rn(xvs, make_float2(u.z, u.z), av[2]);
+            for (int pr2 = 0; pr2 < ES / 2; ++pr2) {
+              const int c = 2 * pr2;
+              const float2 u0 = pr2 ? make_float2(ux.z, ux.w) : make_float2(ux.x, ux.y);
+              const float2 u1 = pr2 ? make_float2(uy.z, uy.w) : make_float2(uy.x, uy.y);
+              const float2 u2 = pr2 ? make_float2(uz.z, uz.w) : make_float2(uz.x, uz.y);
+#pragma unroll
+              for (int par = 0; par < 2; ++par) { // feature 2p + par: low / high halves of the gathered words
+                auto half2 = [&](int x) {
+                  return par ? make_float2(__uint_as_float(gw[c][x] & 0xffff0000u), __uint_as_float(gw[c + 1][x] & 0xffff0000u))
+                             : make_float2(__uint_as_float(gw[c][x] << 16), __uint_as_float(gw[c + 1][x] << 16));
+                };
+                as[par] = __ffma2_rn(half2(0), make_float2(W[par][c], W[par][c + 1]), as[par]);
+                const float2 xvs = __fmul2_rn(half2(1), make_float2(W[2 + par][c], W[2 + par][c + 1]));
+                av[0][par] = __ffma2_rn(xvs, u0, av[0][par]);
+                av[1][par] = __ffma2_rn(xvs, u1, av[1][par]);
+                av[2][par] = __ffma2_rn(xvs, u2, av[2][par]);
                 if (HASV) {
-                  const float2 xvv = __fmul2_rn(bf2(gw[c][2]), make_float2(W[NACC - 2][c], W[NACC - 1][c]));
-                  av[0] = __ffma2_rn(xvv, bf2(gw[c][3]), av[0]);
-                  av[1] = __ffma2_rn(xvv, bf2(gw[c][4]), av[1]);
-                  av[2] = __ffma2_rn(xvv, bf2(gw[c][5]), av[2]);
+                  const float2 xvv = __fmul2_rn(half2(2), make_float2(W[NACC - 2 + par][c], W[NACC - 2 + par][c + 1]));
+                  av[0][par] = __ffma2_rn(xvv, half2(3), av[0][par]);
+                  av[1][par] = __ffma2_rn(xvv, half2(4), av[1][par]);
+                  av[2][par] = __ffma2_rn(xvv, half2(5), av[2][par]);
                 }
               }
             }
