@@ -89,7 +89,7 @@ __device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity)
         : "r"(bar), "r"(parity)
         : "memory");
     if (ok) break;
-    __nanosleep(128);
+    __nanosleep(512);
   }
 }
 
@@ -289,9 +289,10 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
               make_uint4(pack_bf2(v[0], v[1]), pack_bf2(v[2], v[3]), pack_bf2(v[4], v[5]), pack_bf2(v[6], v[7]));
         }
         const uint32_t okm = __ballot_sync(0xffffffffu, ok && half == 0); // bit r: column r holds an edge
+        const int jfirst = __shfl_sync(0xffffffffu, j, lane & ~3);
         if (half == 0) {
           mt->Ux[r] = ok ? gq.x : 0.f; mt->Uy[r] = ok ? gq.y : 0.f; mt->Uz[r] = ok ? gq.z : 0.f;
-          mt->OFF[r] = (uint32_t)j * row16;
+          mt->OFF[r] = (uint32_t)(ok ? j : jfirst) * row16; // unused columns of a step gather a valid row (weight 0)
           if ((r & 3) == 0) mt->sinfo[r >> 2] = make_int2(rcv, __popc((okm >> r) & 15u));
         }
 #pragma unroll
@@ -345,23 +346,24 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
       // Segment sums of the current receiver.  The packed FMAs pair two EDGES of one feature (component .x: even
       // columns of the step, .y: odd columns), so that both operands of a packed product are adjacent registers
       // (two TMEM columns of one accumulator; two unpacked halves): [feature parity] for s, [axis][feature parity] for v.
-      float2 as[2], av[3][2], rs, rv[3];
-      rs = rv[0] = rv[1] = rv[2] = make_float2(0.f, 0.f);
-      auto zero_acc = [&]() {
+      float2 as[2], av[3][2];
+      auto begin_row = [&](int i) { // new receiver: zero sums; pull its residual row (read when it is complete) towards L2
         as[0] = as[1] = make_float2(0.f, 0.f);
 #pragma unroll
         for (int ax = 0; ax < 3; ++ax) av[ax][0] = av[ax][1] = make_float2(0.f, 0.f);
-      };
-      auto begin_row = [&](int i) { // residual row of receiver i: loaded now, used when the receiver is complete
-        zero_acc();
-        rs = ld_stream2(s_in + (int64_t)i * ld_sin + f0);
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(s_in + (int64_t)i * ld_sin + f0));
         if (HASV) {
 #pragma unroll
-          for (int ax = 0; ax < 3; ++ax) rv[ax] = ld_stream2(v_res + ((int64_t)i * 3 + ax) * F + f0);
+          for (int ax = 0; ax < 3; ++ax) asm volatile("prefetch.global.L2 [%0];" ::"l"(v_res + ((int64_t)i * 3 + ax) * F + f0));
         }
       };
       auto end_row = [&](int i) {
         if (!act) return;
+        const float2 rs = ld_stream2(s_in + (int64_t)i * ld_sin + f0);
+        float2 rv[3];
+#pragma unroll
+        for (int ax = 0; ax < 3; ++ax)
+          rv[ax] = HASV ? ld_stream2(v_res + ((int64_t)i * 3 + ax) * F + f0) : make_float2(0.f, 0.f);
         const float2 o = make_float2(rs.x + (as[0].x + as[0].y), rs.y + (as[1].x + as[1].y));
         st_stream2(s1 + (int64_t)i * ld_s1 + f0, o);
         if (mir.s1) st_stream1(mir.s1 + (int64_t)i * mir.ld_s1 + f0, pack_bf2(o.x, o.y));
@@ -373,8 +375,7 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
           if (mir.v1) st_stream1(mir.v1 + off, pack_bf2(ov.x, ov.y));
         }
       };
-      zero_acc();
-      if (cur < (int)a1) begin_row(cur);
+      begin_row(cur < (int)a1 ? cur : (int)a0);
       for (int s0 = 0; s0 < tot; s0 += NE / ES, ++n) {
         const int slot = n % NSLOT;
         const uint32_t buf = n & 1u;
@@ -387,23 +388,22 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
         if (mymask) {
           tc_fence_after();
           const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)((g * 2 + buf) * NACC * NE);
-#pragma unroll 1
+#pragma unroll
           for (int si = 0; si < NE / ES; ++si) {
-            if (!((mymask >> si) & 1u)) continue;
-            const uint32_t cb = (uint32_t)si * (ES * 4); // byte offset of the step's columns in the per-column arrays
-            float W[NACC][ES];
+            if ((mymask >> si) & 1u) {
+              constexpr uint32_t kOFF = (uint32_t)offsetof(TileMeta, OFF), kINF = (uint32_t)offsetof(TileMeta, sinfo),
+                                 kUX = (uint32_t)offsetof(TileMeta, Ux), kUY = (uint32_t)offsetof(TileMeta, Uy),
+                                 kUZ = (uint32_t)offsetof(TileMeta, Uz);
+              const uint32_t cb = (uint32_t)si * (ES * 4); // byte offset of the step's columns in the per-column arrays
+              float W[NACC][ES];
 #pragma unroll
-            for (int acc = 0; acc < NACC; ++acc) tmem_ld4_async(taddr + acc * NE + si * ES, W[acc]);
-            const uint4 oo = lds128(mt_u + (uint32_t)offsetof(TileMeta, OFF) + cb);
-            const uint2 inf = lds64(mt_u + (uint32_t)offsetof(TileMeta, sinfo) + 8u * si);
-            const uint32_t offs[4] = {oo.x, oo.y, oo.z, oo.w};
-            const int i = (int)inf.x, cnt = (int)inf.y;
-            uint32_t gw[ES][6];
+              for (int acc = 0; acc < NACC; ++acc) tmem_ld4_async(taddr + acc * NE + si * ES, W[acc]);
+              const uint4 oo = lds128(mt_u + kOFF + cb);
+              const uint32_t offs[4] = {oo.x, oo.y, oo.z, oo.w};
+              // all four columns gather: an unused column of a ragged step reads a valid row and has zero filter values
+              uint32_t gw[ES][6];
 #pragma unroll
-            for (int c = 0; c < ES; ++c) {
-#pragma unroll
-              for (int x = 0; x < 6; ++x) gw[c][x] = 0u;
-              if (c < cnt) {
+              for (int c = 0; c < ES; ++c) {
                 const char* pr = phi_f + (uint64_t)offs[c] * 16u;
                 gw[c][0] = ldg_nc32(pr); gw[c][1] = ldg_nc32(pr + 2 * F);
                 if (HASV) {
@@ -412,41 +412,41 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
                   gw[c][3] = ldg_nc32(vr); gw[c][4] = ldg_nc32(vr + 2 * F); gw[c][5] = ldg_nc32(vr + 4 * F);
                 }
               }
-            }
-            if (i != cur) { // receiver complete: write it (and any edge-less atoms of mine before the next one)
-              end_row(cur);
-              for (int k = cur + SPLIT; k < i; k += SPLIT) { begin_row(k); end_row(k); }
-              cur = i;
-              begin_row(cur);
-            }
-            const float4 ux = lds128f(mt_u + (uint32_t)offsetof(TileMeta, Ux) + cb);
-            const float4 uy = lds128f(mt_u + (uint32_t)offsetof(TileMeta, Uy) + cb);
-            const float4 uz = lds128f(mt_u + (uint32_t)offsetof(TileMeta, Uz) + cb);
+              const int i = (int)lds32(mt_u + kINF + 8u * si);
+              if (i != cur) { // receiver complete: write it (and any edge-less atoms of mine before the next one)
+                end_row(cur);
+                for (int k = cur + SPLIT; k < i; k += SPLIT) { begin_row(k); end_row(k); }
+                cur = i;
+                begin_row(cur);
+              }
 #pragma unroll
-            for (int acc = 0; acc < NACC; ++acc) tmem_wait4(W[acc], acc == 0);
-            // columns (0, 1) and (2, 3) of the step as packed pairs; unused columns have zero filter values and zero payloads
+              for (int acc = 0; acc < NACC; ++acc) tmem_wait4(W[acc], acc == 0);
+              // columns (0, 1) and (2, 3) of the step as packed pairs
 #pragma unroll
-            for (int pr2 = 0; pr2 < ES / 2; ++pr2) {
-              const int c = 2 * pr2;
-              const float2 u0 = pr2 ? make_float2(ux.z, ux.w) : make_float2(ux.x, ux.y);
-              const float2 u1 = pr2 ? make_float2(uy.z, uy.w) : make_float2(uy.x, uy.y);
-              const float2 u2 = pr2 ? make_float2(uz.z, uz.w) : make_float2(uz.x, uz.y);
+              for (int pr2 = 0; pr2 < ES / 2; ++pr2) {
+                const int c = 2 * pr2;
+                const uint2 u0b = lds64(mt_u + kUX + cb + 8u * pr2), u1b = lds64(mt_u + kUY + cb + 8u * pr2),
+                            u2b = lds64(mt_u + kUZ + cb + 8u * pr2);
+                const float2 u0 = make_float2(__uint_as_float(u0b.x), __uint_as_float(u0b.y));
+                const float2 u1 = make_float2(__uint_as_float(u1b.x), __uint_as_float(u1b.y));
+                const float2 u2 = make_float2(__uint_as_float(u2b.x), __uint_as_float(u2b.y));
 #pragma unroll
-              for (int par = 0; par < 2; ++par) { // feature 2p + par: low / high halves of the gathered words
-                auto half2 = [&](int x) {
-                  return par ? make_float2(__uint_as_float(gw[c][x] & 0xffff0000u), __uint_as_float(gw[c + 1][x] & 0xffff0000u))
-                             : make_float2(__uint_as_float(gw[c][x] << 16), __uint_as_float(gw[c + 1][x] << 16));
-                };
-                as[par] = __ffma2_rn(half2(0), make_float2(W[par][c], W[par][c + 1]), as[par]);
-                const float2 xvs = __fmul2_rn(half2(1), make_float2(W[2 + par][c], W[2 + par][c + 1]));
-                av[0][par] = __ffma2_rn(xvs, u0, av[0][par]);
-                av[1][par] = __ffma2_rn(xvs, u1, av[1][par]);
-                av[2][par] = __ffma2_rn(xvs, u2, av[2][par]);
-                if (HASV) {
-                  const float2 xvv = __fmul2_rn(half2(2), make_float2(W[NACC - 2 + par][c], W[NACC - 2 + par][c + 1]));
-                  av[0][par] = __ffma2_rn(xvv, half2(3), av[0][par]);
-                  av[1][par] = __ffma2_rn(xvv, half2(4), av[1][par]);
-                  av[2][par] = __ffma2_rn(xvv, half2(5), av[2][par]);
+                for (int par = 0; par < 2; ++par) { // feature 2p + par: low / high halves of the gathered words
+                  auto half2 = [&](int x) {
+                    return par ? make_float2(__uint_as_float(gw[c][x] & 0xffff0000u), __uint_as_float(gw[c + 1][x] & 0xffff0000u))
+                               : make_float2(__uint_as_float(gw[c][x] << 16), __uint_as_float(gw[c + 1][x] << 16));
+                  };
+                  as[par] = __ffma2_rn(half2(0), make_float2(W[par][c], W[par][c + 1]), as[par]);
+                  const float2 xvs = __fmul2_rn(half2(1), make_float2(W[2 + par][c], W[2 + par][c + 1]));
+                  av[0][par] = __ffma2_rn(xvs, u0, av[0][par]);
+                  av[1][par] = __ffma2_rn(xvs, u1, av[1][par]);
+                  av[2][par] = __ffma2_rn(xvs, u2, av[2][par]);
+                  if (HASV) {
+                    const float2 xvv = __fmul2_rn(half2(2), make_float2(W[NACC - 2 + par][c], W[NACC - 2 + par][c + 1]));
+                    av[0][par] = __ffma2_rn(xvv, half2(3), av[0][par]);
+                    av[1][par] = __ffma2_rn(xvv, half2(4), av[1][par]);
+                    av[2][par] = __ffma2_rn(xvv, half2(5), av[2][par]);
+                  }
                 }
               }
             }
