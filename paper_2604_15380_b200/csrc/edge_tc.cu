@@ -113,6 +113,43 @@ __device__ __forceinline__ void st_stream2(float* p, float2 v) {
 __device__ __forceinline__ void st_stream1(void* p, uint32_t v) {
   asm volatile("st.global.cs.b32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
+// NACC accumulators (16 columns apart) x 4 columns from one base address, asynchronous
+template <int NACC>
+__device__ __forceinline__ void tmem_ld4_accs(uint32_t taddr, float (&r)[NACC][4]) {
+  uint32_t u[NACC][4];
+  if constexpr (NACC == 6) {
+    asm volatile(
+        "{\n\t.reg .b32 t1, t2, t3, t4, t5;\n\t"
+        "add.u32 t1, %24, 16;\n\tadd.u32 t2, %24, 32;\n\tadd.u32 t3, %24, 48;\n\tadd.u32 t4, %24, 64;\n\tadd.u32 t5, %24, 80;\n\t"
+        "tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%24];\n\t"
+        "tcgen05.ld.sync.aligned.32x32b.x4.b32 {%4, %5, %6, %7}, [t1];\n\t"
+        "tcgen05.ld.sync.aligned.32x32b.x4.b32 {%8, %9, %10, %11}, [t2];\n\t"
+        "tcgen05.ld.sync.aligned.32x32b.x4.b32 {%12, %13, %14, %15}, [t3];\n\t"
+        "tcgen05.ld.sync.aligned.32x32b.x4.b32 {%16, %17, %18, %19}, [t4];\n\t"
+        "tcgen05.ld.sync.aligned.32x32b.x4.b32 {%20, %21, %22, %23}, [t5];\n\t}"
+        : "=r"(u[0][0]), "=r"(u[0][1]), "=r"(u[0][2]), "=r"(u[0][3]), "=r"(u[1][0]), "=r"(u[1][1]), "=r"(u[1][2]), "=r"(u[1][3]),
+          "=r"(u[2][0]), "=r"(u[2][1]), "=r"(u[2][2]), "=r"(u[2][3]), "=r"(u[3][0]), "=r"(u[3][1]), "=r"(u[3][2]), "=r"(u[3][3]),
+          "=r"(u[4][0]), "=r"(u[4][1]), "=r"(u[4][2]), "=r"(u[4][3]), "=r"(u[5][0]), "=r"(u[5][1]), "=r"(u[5][2]), "=r"(u[5][3])
+        : "r"(taddr)
+        : "memory");
+  } else {
+    asm volatile(
+        "{\n\t.reg .b32 t1, t2, t3;\n\t"
+        "add.u32 t1, %16, 16;\n\tadd.u32 t2, %16, 32;\n\tadd.u32 t3, %16, 48;\n\t"
+        "tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%16];\n\t"
+        "tcgen05.ld.sync.aligned.32x32b.x4.b32 {%4, %5, %6, %7}, [t1];\n\t"
+        "tcgen05.ld.sync.aligned.32x32b.x4.b32 {%8, %9, %10, %11}, [t2];\n\t"
+        "tcgen05.ld.sync.aligned.32x32b.x4.b32 {%12, %13, %14, %15}, [t3];\n\t}"
+        : "=r"(u[0][0]), "=r"(u[0][1]), "=r"(u[0][2]), "=r"(u[0][3]), "=r"(u[1][0]), "=r"(u[1][1]), "=r"(u[1][2]), "=r"(u[1][3]),
+          "=r"(u[2][0]), "=r"(u[2][1]), "=r"(u[2][2]), "=r"(u[2][3]), "=r"(u[3][0]), "=r"(u[3][1]), "=r"(u[3][2]), "=r"(u[3][3])
+        : "r"(taddr)
+        : "memory");
+  }
+#pragma unroll
+  for (int a = 0; a < NACC; ++a)
+#pragma unroll
+    for (int i = 0; i < 4; ++i) r[a][i] = __uint_as_float(u[a][i]);
+}
 // 32 TMEM lanes x 4 columns, asynchronous
 __device__ __forceinline__ void tmem_ld4_async(uint32_t taddr, float (&r)[4]) {
   uint32_t u[4];
@@ -379,7 +416,8 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
       for (int s0 = 0; s0 < tot; s0 += NE / ES, ++n) {
         const int slot = n % NSLOT;
         const uint32_t buf = n & 1u;
-        const uint32_t mt_u = grp_u + NSLOT * L::B_TILE + slot * (uint32_t)sizeof(TileMeta);
+        uint32_t mt_u = grp_u + NSLOT * L::B_TILE + slot * (uint32_t)sizeof(TileMeta);
+        asm volatile("" : "+r"(mt_u)); // keep it in a register (it is otherwise recomputed from scratch at every use)
         mbar_wait_sleep(meta_full(g, slot), (n / NSLOT) & 1u);
         const uint32_t mymask = lds32(mt_u + (uint32_t)offsetof(TileMeta, smask) + 4u * h);
         // (every warp observes every phase of the barrier, also for tiles it has no edge in: a parity wait two phases
@@ -387,7 +425,8 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
         mbar_wait_sleep(tmem_full(g, buf), (n >> 1) & 1u);
         if (mymask) {
           tc_fence_after();
-          const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)((g * 2 + buf) * NACC * NE);
+          uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)((g * 2 + buf) * NACC * NE);
+          asm volatile("" : "+r"(taddr));
 #pragma unroll
           for (int si = 0; si < NE / ES; ++si) {
             if ((mymask >> si) & 1u) {
@@ -396,8 +435,8 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
                                  kUZ = (uint32_t)offsetof(TileMeta, Uz);
               const uint32_t cb = (uint32_t)si * (ES * 4); // byte offset of the step's columns in the per-column arrays
               float W[NACC][ES];
-#pragma unroll
-              for (int acc = 0; acc < NACC; ++acc) tmem_ld4_async(taddr + acc * NE + si * ES, W[acc]);
+              static_assert(NE == 16, "tmem_ld4_accs assumes accumulators 16 columns apart");
+              tmem_ld4_accs<NACC>(taddr + si * ES, W);
               const uint4 oo = lds128(mt_u + kOFF + cb);
               const uint32_t offs[4] = {oo.x, oo.y, oo.z, oo.w};
               // all four columns gather: an unused column of a ragged step reads a valid row and has zero filter values
