@@ -72,13 +72,21 @@ int pnn_model_create(const pnn_config* cfg, const double* weights_host, int64_t 
 void pnn_model_destroy(pnn_model* m);
 
 /* Allocates all device memory needed for batches of up to max_atoms atoms, max_edges directed edges and
- * max_structs structures.  want_forces != 0 also allocates the per-block tape and the adjoint buffers
- * (SURVEY.md §8(a) a7).  Synchronous. */
+ * max_structs structures.  want_forces: 0, or PNN_WS_FORCES (also allocates the per-block tape and the adjoint buffers of
+ * the reverse sweep), optionally | PNN_WS_NO_EDGE_TAPE.  A PNN_FP32 model with forces keeps an EDGE
+ * TAPE (filter value and its derivative of every edge, feature and block: 24 F T bytes per edge of max_edges) that the
+ * reverse edge kernel streams back instead of recomputing the filter; PNN_WS_NO_EDGE_TAPE trades that memory for about 3x
+ * slower edge kernels of the reverse sweep.  If the tape (or anything else) cannot be allocated the call fails with
+ * PNN_ERR_CUDA: the library never changes kernels silently.  Any other bit in want_forces: PNN_ERR_INVALID_ARG.
+ * Synchronous. */
+#define PNN_WS_FORCES 1
+#define PNN_WS_NO_EDGE_TAPE 2
 int pnn_workspace_create(const pnn_model* m, int64_t max_atoms, int64_t max_edges, int64_t max_structs,
                          int want_forces, pnn_workspace** out);
 void pnn_workspace_destroy(pnn_workspace* ws);
-/* Bytes of device memory the workspace holds. */
+/* Bytes of device memory the workspace holds (the edge tape included), and the bytes of the edge tape alone (0: none). */
 int64_t pnn_workspace_bytes(const pnn_workspace* ws);
+int64_t pnn_workspace_edge_tape_bytes(const pnn_workspace* ws);
 
 /* a1 — radius graph (PAPER.md:230 cutoff, PAPER.md:269 PBC).  All ordered pairs (i, j),
  * i != j, in the same structure, with |x_j - x_i + shift.C| < r_c (strict, FP64); under PBC the shift is the
@@ -89,7 +97,9 @@ int64_t pnn_workspace_bytes(const pnn_workspace* ws);
  *   pos        DEVICE [N,3] f64        struct_ptr DEVICE [S+1] i32
  *   cell       DEVICE [S,3,3] f64 (rows = lattice vectors) or NULL    pbc DEVICE [S,3] u8 or NULL
  * Edge overflow (E > max_edges) is detected on the device and reported by pnn_check_async_errors /
- * pnn_graph_view.  Asynchronous. */
+ * pnn_graph_view / pnn_eval_host (PNN_ERR_CAPACITY); a truncated graph is never evaluated: until the next pnn_build_graph
+ * the edge kernels of pnn_eval do nothing, and once the overflow has been reported pnn_eval returns PNN_ERR_NO_GRAPH.
+ * Asynchronous. */
 int pnn_build_graph(pnn_workspace* ws, int64_t n_atoms, int64_t n_structs, const double* pos,
                     const int32_t* struct_ptr, const double* cell, const uint8_t* pbc, void* cuda_stream);
 
@@ -107,8 +117,10 @@ int pnn_graph_copy(const pnn_workspace* ws, int32_t* rowptr, int32_t* col, int8_
 #define PNN_FORCES 2
 
 /* a2..a7 — embedding, T x (message, update), multi-head readout, and (with PNN_FORCES) the analytic reverse
- * sweep.  Uses the graph last built in the workspace (same n_atoms, n_structs
- * and pos; PNN_ERR_NO_GRAPH otherwise).
+ * sweep.  Uses the graph last built in the workspace, which must have been built for
+ * the same n_atoms and n_structs (PNN_ERR_NO_GRAPH at once otherwise) and the same pos: pos DEVICE [N,3] f64 is
+ * checksummed on the device against the positions pnn_build_graph saw, and a mismatch (atoms moved without a rebuild)
+ * is reported as PNN_ERR_NO_GRAPH by pnn_check_async_errors; the results of that call are then undefined.
  *   Z DEVICE [N] i32 in [1,Zmax]     head DEVICE [S] i32 in [0,H)
  *   energy DEVICE [S], forces DEVICE [N,3]: f64 for a PNN_FP64 model, f32 for PNN_FP32 and PNN_BF16.
  *   forces may be NULL unless flags has PNN_FORCES (which needs a workspace created with want_forces).
@@ -150,13 +162,14 @@ int pnn_branch_weights(const pnn_branch_mlp* b, pnn_workspace* ws, int64_t n_ato
 
 /* Convenience for callers with HOST buffers (bench.py's e2e leg): copies Z, pos, struct_ptr, head (and cell /
  * pbc when not NULL) to the device, runs pnn_build_graph + pnn_eval and copies energy [S] / forces [N,3] back.
- * energy_host / forces_host have the dtype pnn_eval documents.  Synchronous. */
+ * energy_host / forces_host have the dtype pnn_eval documents.  Device-side errors of the call (edge overflow, bad Z /
+ * head) are returned by the call itself.  Synchronous. */
 int pnn_eval_host(const pnn_model* m, pnn_workspace* ws, int64_t n_atoms, int64_t n_structs, const int32_t* Z,
                   const double* pos, const int32_t* struct_ptr, const int32_t* head, const double* cell,
                   const uint8_t* pbc, int flags, void* energy_host, void* forces_host, void* cuda_stream);
 
-/* Reads the device error flags (edge overflow -> PNN_ERR_CAPACITY, bad Z / head -> PNN_ERR_BAD_INPUT) and
- * clears them.  Synchronises the device. */
+/* Reads the device error flags (edge overflow -> PNN_ERR_CAPACITY, positions changed since pnn_build_graph ->
+ * PNN_ERR_NO_GRAPH, bad Z / head -> PNN_ERR_BAD_INPUT) and clears them.  Synchronises the device. */
 int pnn_check_async_errors(pnn_workspace* ws);
 
 /* Optional per-kernel-family timing: when enabled, pnn_build_graph / pnn_eval bracket each kernel family with CUDA

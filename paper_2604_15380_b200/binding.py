@@ -16,7 +16,8 @@ __all__ = [
     "PNN_OK", "PNN_BF16", "PNN_FP32", "PNN_FP64", "PNN_ENERGY", "PNN_FORCES", "PnnError", "pnn_config", "lib",
     "lib_path", "pnn_status_string", "pnn_last_cuda_error", "pnn_weights_count", "pnn_model_create",
     "pnn_model_destroy", "pnn_branch_mlp_create", "pnn_branch_mlp_destroy", "pnn_branch_weights",
-    "pnn_workspace_create", "pnn_workspace_destroy", "pnn_workspace_bytes", "pnn_build_graph",
+    "pnn_workspace_create", "pnn_workspace_destroy", "pnn_workspace_bytes", "pnn_workspace_edge_tape_bytes",
+    "PNN_WS_FORCES", "PNN_WS_NO_EDGE_TAPE", "pnn_build_graph",
     "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_eval_blended", "pnn_eval_host", "pnn_check_async_errors", "pnn_measure_alu_peak", "pnn_launch_count", "pnn_profile_enable",
     "pnn_profile_read", "pnn_gemm_bf16",
     "PaiNN", "PRECISIONS",
@@ -73,6 +74,8 @@ def lib():
         L.pnn_workspace_destroy.restype = None
         L.pnn_workspace_bytes.argtypes = [vp]
         L.pnn_workspace_bytes.restype = i64
+        L.pnn_workspace_edge_tape_bytes.argtypes = [vp]
+        L.pnn_workspace_edge_tape_bytes.restype = i64
         L.pnn_build_graph.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
         L.pnn_graph_view.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp),
                                      ctypes.POINTER(i64)]
@@ -100,15 +103,35 @@ def _check(st: int, where: str):
         raise PnnError(st, where)
 
 
-def _ptr(x) -> Optional[int]:
-    """int / None pass through; numpy arrays give their host address; torch tensors their data_ptr()."""
+_NP_DTYPES = {"i32": np.int32, "f64": np.float64, "f32": np.float32, "u8": np.uint8, "i8": np.int8}
+
+
+def _ptr(x, dtype: Optional[str] = None, device: Optional[bool] = None) -> Optional[int]:
+    """int / None pass through; numpy arrays give their host address; torch tensors their data_ptr().
+    dtype ("i32", "f64", "f32", "u8", "i8", "bf16") and device (True: CUDA, False: host) are checked when given: the C ABI
+    takes untyped pointers, so a wrong element type or a host pointer where a device one is expected would be misread."""
     if x is None:
         return None
     if isinstance(x, int):
         return x
     if isinstance(x, np.ndarray):
-        assert x.flags["C_CONTIGUOUS"]
+        if not x.flags["C_CONTIGUOUS"]:
+            raise ValueError("array must be C-contiguous")
+        if dtype is not None and dtype != "bf16" and x.dtype != _NP_DTYPES[dtype]:
+            raise TypeError(f"expected a {dtype} array, got {x.dtype}")
+        if device:
+            raise TypeError("expected a CUDA tensor, got a host array")
         return x.ctypes.data
+    if not x.is_contiguous():
+        raise ValueError("tensor must be contiguous")
+    if dtype is not None:
+        import torch
+        want = {"i32": torch.int32, "f64": torch.float64, "f32": torch.float32, "u8": torch.uint8, "i8": torch.int8,
+                "bf16": torch.bfloat16}[dtype]
+        if x.dtype != want:
+            raise TypeError(f"expected a {dtype} tensor, got {x.dtype}")
+    if device is not None and bool(x.is_cuda) != device:
+        raise TypeError("expected a CUDA tensor" if device else "expected a host tensor")
     return x.data_ptr()
 
 
@@ -137,11 +160,20 @@ def pnn_model_destroy(model: int) -> None:
     lib().pnn_model_destroy(model)
 
 
-def pnn_workspace_create(model: int, max_atoms: int, max_edges: int, max_structs: int, want_forces: bool) -> int:
+PNN_WS_FORCES, PNN_WS_NO_EDGE_TAPE = 1, 2
+
+
+def pnn_workspace_create(model: int, max_atoms: int, max_edges: int, max_structs: int, want_forces) -> int:
+    """want_forces: bool, or the PNN_WS_* flags of include/pnn.h."""
     out = ctypes.c_void_p()
-    _check(lib().pnn_workspace_create(model, max_atoms, max_edges, max_structs, int(bool(want_forces)),
-                                      ctypes.byref(out)), "pnn_workspace_create")
+    flags = int(want_forces) if not isinstance(want_forces, bool) else int(want_forces)
+    _check(lib().pnn_workspace_create(model, max_atoms, max_edges, max_structs, flags, ctypes.byref(out)),
+           "pnn_workspace_create")
     return out.value
+
+
+def pnn_workspace_edge_tape_bytes(ws: int) -> int:
+    return lib().pnn_workspace_edge_tape_bytes(ws)
 
 
 def pnn_workspace_destroy(ws: int) -> None:
@@ -153,8 +185,8 @@ def pnn_workspace_bytes(ws: int) -> int:
 
 
 def pnn_build_graph(ws: int, n_atoms: int, n_structs: int, pos, struct_ptr, cell=None, pbc=None, stream=None):
-    _check(lib().pnn_build_graph(ws, n_atoms, n_structs, _ptr(pos), _ptr(struct_ptr), _ptr(cell), _ptr(pbc),
-                                 stream), "pnn_build_graph")
+    _check(lib().pnn_build_graph(ws, n_atoms, n_structs, _ptr(pos, "f64", True), _ptr(struct_ptr, "i32", True),
+                                 _ptr(cell, "f64", True), _ptr(pbc, "u8", True), stream), "pnn_build_graph")
 
 
 def pnn_graph_view(ws: int):
@@ -167,20 +199,21 @@ def pnn_graph_view(ws: int):
 
 
 def pnn_graph_copy(ws: int, rowptr=None, col=None, shift=None):
-    _check(lib().pnn_graph_copy(ws, _ptr(rowptr), _ptr(col), _ptr(shift)), "pnn_graph_copy")
+    _check(lib().pnn_graph_copy(ws, _ptr(rowptr, "i32"), _ptr(col, "i32"), _ptr(shift, "i8")), "pnn_graph_copy")
 
 
 def pnn_eval(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, struct_ptr, head, flags: int, energy,
              forces=None, stream=None):
-    _check(lib().pnn_eval(model, ws, n_atoms, n_structs, _ptr(Z), _ptr(pos), _ptr(struct_ptr), _ptr(head), flags,
-                          _ptr(energy), _ptr(forces), stream), "pnn_eval")
+    _check(lib().pnn_eval(model, ws, n_atoms, n_structs, _ptr(Z, "i32", True), _ptr(pos, "f64", True),
+                          _ptr(struct_ptr, "i32", True), _ptr(head, "i32", True), flags, _ptr(energy, None, True),
+                          _ptr(forces, None, True), stream), "pnn_eval")
 
 
 def pnn_eval_blended(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, struct_ptr, head_weights,
                      skip_below: float, flags: int, energy, forces=None, stream=None):
-    _check(lib().pnn_eval_blended(model, ws, n_atoms, n_structs, _ptr(Z), _ptr(pos), _ptr(struct_ptr),
-                                  _ptr(head_weights), float(skip_below), flags, _ptr(energy), _ptr(forces), stream),
-           "pnn_eval_blended")
+    _check(lib().pnn_eval_blended(model, ws, n_atoms, n_structs, _ptr(Z, "i32", True), _ptr(pos, "f64", True),
+                                  _ptr(struct_ptr, "i32", True), _ptr(head_weights, None, True), float(skip_below), flags,
+                                  _ptr(energy, None, True), _ptr(forces, None, True), stream), "pnn_eval_blended")
 
 
 def pnn_branch_mlp_create(widths, params_host: np.ndarray, prec: int) -> int:
@@ -197,15 +230,16 @@ def pnn_branch_mlp_destroy(b: int) -> None:
 
 
 def pnn_branch_weights(b: int, ws: int, n_atoms: int, n_structs: int, Z, struct_ptr, head_weights, stream=None):
-    _check(lib().pnn_branch_weights(b, ws, n_atoms, n_structs, _ptr(Z), _ptr(struct_ptr), _ptr(head_weights), stream),
-           "pnn_branch_weights")
+    _check(lib().pnn_branch_weights(b, ws, n_atoms, n_structs, _ptr(Z, "i32", True), _ptr(struct_ptr, "i32", True),
+                                    _ptr(head_weights, None, True), stream), "pnn_branch_weights")
 
 
 def pnn_eval_host(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, struct_ptr, head, cell, pbc,
                   flags: int, energy_host, forces_host=None, stream=None):
-    _check(lib().pnn_eval_host(model, ws, n_atoms, n_structs, _ptr(Z), _ptr(pos), _ptr(struct_ptr), _ptr(head),
-                               _ptr(cell), _ptr(pbc), flags, _ptr(energy_host), _ptr(forces_host), stream),
-           "pnn_eval_host")
+    _check(lib().pnn_eval_host(model, ws, n_atoms, n_structs, _ptr(Z, "i32", False), _ptr(pos, "f64", False),
+                               _ptr(struct_ptr, "i32", False), _ptr(head, "i32", False), _ptr(cell, "f64", False),
+                               _ptr(pbc, "u8", False), flags, _ptr(energy_host, None, False),
+                               _ptr(forces_host, None, False), stream), "pnn_eval_host")
 
 
 def pnn_check_async_errors(ws: int) -> None:
@@ -249,14 +283,16 @@ class PaiNN:
 
     def __init__(self, F: int, T: int, K: int, H: int, weights: np.ndarray, *, precision: str = "fp32",
                  cutoff: float = 5.0, Zmax: int = 86, norm_eps: float = 1e-8, max_atoms: int, max_edges: int,
-                 max_structs: int, forces: bool = True, rbf: str = "gaussian", pbc_images: str = "minimum"):
+                 max_structs: int, forces: bool = True, rbf: str = "gaussian", pbc_images: str = "minimum",
+                 edge_tape: bool = True):
         self.cfg = pnn_config(F, T, K, H, Zmax, cutoff, norm_eps, PRECISIONS[precision],
                               {"gaussian": 0, "bessel": 1}[rbf], {"minimum": 0, "all": 1}[pbc_images])
         self.precision = precision
         self.want_forces = bool(forces)
         self.model = pnn_model_create(self.cfg, weights)
         try:
-            self.ws = pnn_workspace_create(self.model, max_atoms, max_edges, max_structs, forces)
+            self.ws = pnn_workspace_create(self.model, max_atoms, max_edges, max_structs,
+                                           (PNN_WS_FORCES if forces else 0) | (0 if edge_tape else PNN_WS_NO_EDGE_TAPE))
         except Exception:
             pnn_model_destroy(self.model)
             self.model = None

@@ -13,7 +13,7 @@ void note_launch(const char* where);
 #define PNN_KCHECK(name) ::pnn::note_launch(name)
 
 // device-side error flags (workspace->d_err)
-enum : int { ERRF_EDGE_OVERFLOW = 1, ERRF_BAD_Z = 2, ERRF_BAD_HEAD = 4 };
+enum : int { ERRF_EDGE_OVERFLOW = 1, ERRF_BAD_Z = 2, ERRF_BAD_HEAD = 4, ERRF_STALE_GRAPH = 8 };
 
 // Per-edge geometry in model precision: unit vector receiver->sender image and distance.
 template <typename T>
@@ -107,8 +107,12 @@ struct GraphBuffers {
   void* geom;          // [Emax] Geom<T>
   int32_t* scan_tmp;   // scratch for the scans
   int64_t max_edges;
-  int* d_err;
+  int* d_err;   // sticky flags (ERRF_*), cleared by pnn_check_async_errors
+  int* d_ovf;   // ERRF_EDGE_OVERFLOW or 0 for the CURRENT graph: rewritten by every build, tested by the edge kernels
+  unsigned long long* d_poschk; // [2]: checksum of the positions the graph was built from / scratch for pnn_eval's check
 };
+// Flags ERRF_STALE_GRAPH when the checksum of pos differs from the one recorded by the last launch_graph_build.
+int launch_pos_check(const GraphBuffers& g, int64_t N, const double* pos, cudaStream_t st);
 int launch_graph_build(const GraphBuffers& g, int64_t N, int64_t S, const double* pos, const int32_t* struct_ptr,
                        const double* cell, const uint8_t* pbc, double rc, int prec, int all_images, cudaStream_t st);
 

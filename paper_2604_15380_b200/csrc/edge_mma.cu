@@ -1,18 +1,13 @@
-// edge_mma.cu — a4 / a7 edge kernels of the BF16 model: the filter contraction runs on the tensor cores.
+// edge_mma.cu — a7 reverse edge kernel of the BF16 model: the filter contraction runs on the tensor cores (mma.sync on
+// 16-edge tiles of one receiver).  The forward kernel of the BF16 model is edge_tc.cu (tcgen05).
 //
-// Forward: per edge e = (i <- j): w_e = (flt_W g(d_e) + flt_b) c(d_e), x_e = phi_j o w_e,
-// s'_i = s_i + sum x^ss, v'_i = v_i + sum (x^vs u_e + x^vv o v_j).
-//
-// The filter is a small-K GEMM [edges x K] . [K x 3F] (SURVEY.md §7 hard part 3).  Here a 16-edge tile of ONE receiver
-// is the M dimension of mma.sync.m16n8k16 (BF16 operands, FP32 accumulation): A = radial basis times cutoff, rounded
-// to BF16, with the cutoff itself as an extra column so that flt_b rides along as an extra weight row; B = filter
-// weights.  A warp owns a 32-feature slab of all three chunks.  The MMA columns are permuted (on the host, when the
-// model is created) so that thread (g, t) of the accumulator fragment owns the 8 CONTIGUOUS features t*8 .. t*8+7 of
-// the slab: the gathered sender rows phi_j / v_j (BF16) are then read with one 16-byte load per row and chunk, straight
-// into the fragment layout, and multiplied in registers with packed FP32 FMAs (fma.rn.f32x2).  Rows g and g+8 of a
-// tile belong to the same receiver, so every thread keeps a running FP32 sum; the 8 row groups meet once per receiver
-// in a 3-stage shuffle reduce-scatter after which lane (g, t) holds component g>>1 (s, v_x, v_y, v_z) of 4 contiguous
-// features and does the residual add and the coalesced FP32 + BF16 stores.  No atomics.
+// The filter is a small-K GEMM [edges x K] . [K x 3F] (SURVEY.md §7 hard part 3).  A 16-edge tile of ONE receiver is the M
+// dimension of mma.sync.m16n8k16 (BF16 operands, FP32 accumulation): A = radial basis times cutoff, rounded to BF16, with
+// the cutoff itself as an extra column so that flt_b rides along as an extra weight row; B = filter weights.  A warp owns a
+// 32-feature slab of all three chunks.  The MMA columns are permuted (on the host, when the model is created) so that
+// thread (g, t) of the accumulator fragment owns the 8 CONTIGUOUS features t*8 .. t*8+7 of the slab: the gathered sender
+// rows (BF16) are then read with one 16-byte load per row and chunk, straight into the fragment layout, and multiplied in
+// registers with packed FP32 FMAs (fma.rn.f32x2).  No atomics.
 #include <algorithm>
 #include <cstring>
 
@@ -24,8 +19,7 @@ namespace pnn {
 namespace {
 
 constexpr int TE = 16; // edges (rows) per MMA tile
-constexpr int NTC = 2;  // tiles of one receiver staged per round (forward)
-constexpr int NTCB = 3; // ... (reverse)
+constexpr int NTCB = 3; // tiles of one receiver staged per round
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -52,30 +46,7 @@ __device__ __forceinline__ uint32_t pack_bf2(float lo, float hi) {
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ uint4 ldg16(const __nv_bfloat16* p) { return __ldg(reinterpret_cast<const uint4*>(p)); }
 
-// Sum the 32 per-thread partials over the 8 row groups of the fragment layout (lanes t, t+4, ..., t+28): a 3-stage
-// shuffle reduce-scatter (16 + 8 + 4 exchanges).  Shuffles, not shared memory: the kernel's L1 / shared-memory data pipe
-// is its busiest unit (profiles/r01_bf16_kernels.md), and a transposition through shared memory measured slower.
-// In: acc[a], a = comp*8 + fi.  Out: lane (g, t) holds a = g*4 .. g*4+3, i.e. comp = g>>1, fi = (g&1)*4 + q.
-constexpr int RED_PITCH = 80; // (reverse kernel) 16 floats + 16 bytes: conflict-free 16-byte accesses
-__device__ __forceinline__ void reduce_scatter32(const float (&acc)[32], int lane, unsigned char*, float (&out)[4]) {
-  float s1[16], s2[8];
-  const bool b2 = (lane & 16) != 0, b1 = (lane & 8) != 0, b0 = (lane & 4) != 0;
-#pragma unroll
-  for (int q = 0; q < 16; ++q) {
-    const float keep = b2 ? acc[q + 16] : acc[q], send = b2 ? acc[q] : acc[q + 16];
-    s1[q] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-  }
-#pragma unroll
-  for (int q = 0; q < 8; ++q) {
-    const float keep = b1 ? s1[q + 8] : s1[q], send = b1 ? s1[q] : s1[q + 8];
-    s2[q] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-  }
-#pragma unroll
-  for (int q = 0; q < 4; ++q) {
-    const float keep = b0 ? s2[q + 4] : s2[q], send = b0 ? s2[q] : s2[q + 4];
-    out[q] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-  }
-}
+constexpr int RED_PITCH = 80; // 16 floats + 16 bytes: conflict-free 16-byte accesses
 
 // 16 per-thread partials -> sums over the 8 row groups.  Lanes with (g >> 2) == rh receive out[q] = sum of value
 // (g & 3) * 4 + q; the other lanes receive nothing.
@@ -155,188 +126,6 @@ __device__ __forceinline__ void stage_rows(const EdgeMmaArgs& a, int lane, int n
     }
   }
   __syncwarp();
-}
-
-// ------------------------------------------------------------------------------------------ forward
-// One warp per receiver (warps of a CTA take neighbouring receivers, so the gathered rows of a structure stay in
-// L1): the warp stages the A operand of up to NTC tiles once and then walks the CTA's NSL 32-feature slabs.
-// Receivers with more than NTC tiles are processed in rounds; a later round adds to the output of the previous one.
-template <int KP, bool HASV>
-__global__ void __launch_bounds__(256, 2)
-edge_fwd_mma_k(EdgeMmaArgs a, int NSL, int RB, const __nv_bfloat16* __restrict__ phi, const float* s_in,
-               int64_t ld_sin, const __nv_bfloat16* __restrict__ v_in, const float* v_res, float* s1, int64_t ld_s1,
-               float* v1, EdgeMirror mir) {
-  if (*a.d_err & ERRF_EDGE_OVERFLOW) return;
-  constexpr int PA = KP * 2 + 16; // padded row pitch (bytes): conflict-free ldmatrix
-  constexpr int KS = KP / 16;
-  constexpr int NR = NTC * TE;    // staged rows per round
-  extern __shared__ __align__(16) unsigned char smem[];
-  const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
-  unsigned char* Ws = smem;                                                     // [3][NSL][32 rows][PA]
-  unsigned char* Gs = Ws + (size_t)3 * NSL * 32 * PA + (size_t)warp * NR * PA;  // per warp [NR][PA]
-  float4* Us = reinterpret_cast<float4*>(Ws + (size_t)3 * NSL * 32 * PA + (size_t)nwarp * NR * PA) + warp * NR;
-  float2* Cs = reinterpret_cast<float2*>(reinterpret_cast<float4*>(Ws + (size_t)3 * NSL * 32 * PA +
-                                                                   (size_t)nwarp * NR * PA) + nwarp * NR) + warp * NR;
-  int* Js = reinterpret_cast<int*>(reinterpret_cast<float2*>(reinterpret_cast<float4*>(
-                Ws + (size_t)3 * NSL * 32 * PA + (size_t)nwarp * NR * PA) + nwarp * NR) + nwarp * NR) + warp * NR;
-
-  unsigned char* Rs = reinterpret_cast<unsigned char*>(
-      reinterpret_cast<int*>(reinterpret_cast<float2*>(reinterpret_cast<float4*>(
-          Ws + (size_t)3 * NSL * 32 * PA + (size_t)nwarp * NR * PA) + nwarp * NR) + nwarp * NR) + nwarp * NR) +
-      (size_t)warp * 32 * RED_PITCH;                                            // per warp [32][RED_PITCH]
-
-  const int F = a.F;
-  const int g = lane >> 2, t = lane & 3;
-  const int slab0 = blockIdx.y * NSL; // first 32-feature slab of this CTA
-  // filter weights of this CTA's slabs -> shared memory (packed rows are KP*2 bytes; smem rows are padded)
-  {
-    const int nslab_tot = F / 32;
-    constexpr int V = KP * 2 / 16; // 16-byte vectors per row
-    for (int idx = tid; idx < 3 * NSL * 32 * V; idx += nthr) {
-      const int v = idx % V, r = idx / V; // r = (c*NSL + w)*32 + row
-      const int c = r / (NSL * 32), w = (r / 32) % NSL, row = r % 32;
-      const uint4 val = __ldg(reinterpret_cast<const uint4*>(a.fltP) + ((size_t)((c * nslab_tot + slab0 + w) * 32 + row)) * V + v);
-      *reinterpret_cast<uint4*>(Ws + (size_t)r * PA + v * 16) = val;
-    }
-  }
-  __syncthreads();
-  const float rc = a.rc;
-  const float dmu = (a.K > 1) ? rc / (float)(a.K - 1) : rc;
-  const float gamma = 1.0f / (2.0f * dmu * dmu);
-  const float pi_rc = 3.14159265358979323846f / rc;
-  // ldmatrix lane addressing: A tile (rows = lane&15, k half = lane>>4), B tiles (row = lane&7, k half = (lane>>3)&1,
-  // n-tile of the pair = lane>>4)
-  const uint32_t a_off = (uint32_t)((lane & 15) * PA + (lane >> 4) * 16);
-  const uint32_t b_off = (uint32_t)(((lane >> 4) * 8 + (lane & 7)) * PA + ((lane >> 3) & 1) * 16);
-  const uint32_t Ws_u = smem_u32(Ws), Gs_u = smem_u32(Gs);
-
-  const int64_t nchunk = (a.N + RB - 1) / RB;
-  for (int64_t ch = blockIdx.x; ch < nchunk; ch += gridDim.x) {
-    const int64_t i_end = min((int64_t)(ch + 1) * RB, a.N);
-    for (int64_t i = ch * RB + warp; i < i_end; i += nwarp) {
-      const int ea = a.rowptr[i], eb = a.rowptr[i + 1];
-      // The warp's next receiver: pull its geometry, sender indices and own rows towards L2 now, so that the DRAM
-      // latency of these streaming reads overlaps the work on the current receiver.
-      if (i + nwarp < i_end) {
-        const int64_t in = i + nwarp;
-        const int en = __ldg(a.rowptr + in);
-        if (lane < 4) prefetch_l2(a.geom + en + lane * 8);
-        else if (lane == 4) prefetch_l2(a.col + en);
-        else if (lane < 5 + NSL) prefetch_l2(s_in + in * ld_sin + (slab0 + lane - 5) * 32);
-        else if (HASV && lane < 5 + 4 * NSL) {
-          const int q = lane - 5 - NSL;
-          prefetch_l2(v_res + (in * 3 + q / NSL) * F + (slab0 + q % NSL) * 32);
-        }
-      }
-      bool first = true;
-      for (int r0 = ea; first || r0 < eb; r0 += NR) {
-        const int ntile = min(NTC, (eb - r0 + TE - 1) / TE);
-        stage_rows<KP, false>(a, lane, ntile * TE, r0, eb, (int)i, Gs, nullptr, Us, Cs, Js, dmu, gamma, pi_rc);
-        for (int sl = 0; sl < NSL; ++sl) {
-          const int fbase = (slab0 + sl) * 32 + t * 8; // first of this thread's 8 contiguous features
-          float2 acc[16]; // [comp: s, v_x, v_y, v_z][n-tile]: the thread's 8 features as 4 pairs
-#pragma unroll
-          for (int q = 0; q < 16; ++q) acc[q] = make_float2(0.f, 0.f);
-          // the receiver's own row (residual input) is fetched now and used after the reduction
-          const int comp = g >> 1;
-          const int f = (slab0 + sl) * 32 + t * 8 + (g & 1) * 4;
-          const int64_t voff = (i * 3 + (comp - 1)) * F + f;
-          float4 own = make_float4(0.f, 0.f, 0.f, 0.f);
-          if (comp == 0) own = first ? *reinterpret_cast<const float4*>(s_in + i * ld_sin + f)
-                                     : *reinterpret_cast<const float4*>(s1 + i * ld_s1 + f);
-          else if (!first) own = *reinterpret_cast<const float4*>(v1 + voff);
-          else if (HASV) own = *reinterpret_cast<const float4*>(v_res + voff);
-          for (int tl = 0; tl < ntile; ++tl) {
-            uint32_t af[KS][4];
-#pragma unroll
-            for (int ks = 0; ks < KS; ++ks)
-              ldsm_x4(Gs_u + tl * TE * PA + a_off + ks * 32, af[ks][0], af[ks][1], af[ks][2], af[ks][3]);
-            // rows past the segment end have zero weights; their gathers are skipped (payload = 0)
-            const bool ok0 = r0 + tl * TE + g < eb, ok1 = r0 + tl * TE + g + 8 < eb;
-            const int64_t o0 = (int64_t)Js[tl * TE + g] * 3 * F + fbase, o1 = (int64_t)Js[tl * TE + g + 8] * 3 * F + fbase;
-            const float4 u0 = Us[tl * TE + g], u1 = Us[tl * TE + g + 8];
-            const uint4 zero4 = make_uint4(0u, 0u, 0u, 0u);
-            // all gathers of the tile are issued before the first MMA (one memory latency per tile and slab)
-            uint4 pp0[3], pp1[3], va0[3], va1[3];
-#pragma unroll
-            for (int c = 0; c < (HASV ? 3 : 2); ++c) {
-              pp0[c] = ok0 ? ldg16(phi + o0 + c * F) : zero4;
-              pp1[c] = ok1 ? ldg16(phi + o1 + c * F) : zero4;
-            }
-            if (HASV) {
-#pragma unroll
-              for (int ax = 0; ax < 3; ++ax) {
-                va0[ax] = ok0 ? ldg16(v_in + o0 + ax * F) : zero4;
-                va1[ax] = ok1 ? ldg16(v_in + o1 + ax * F) : zero4;
-              }
-            }
-#pragma unroll
-            for (int c = 0; c < (HASV ? 3 : 2); ++c) {
-              const uint4 p0 = pp0[c], p1 = pp1[c];
-              float C[4][4];
-#pragma unroll
-              for (int nt = 0; nt < 4; ++nt)
-#pragma unroll
-                for (int q = 0; q < 4; ++q) C[nt][q] = 0.f;
-              const uint32_t wbase = Ws_u + (uint32_t)((c * NSL + sl) * 32) * PA + b_off;
-#pragma unroll
-              for (int np = 0; np < 2; ++np)
-#pragma unroll
-                for (int ks = 0; ks < KS; ++ks) {
-                  uint32_t b0, b1, b2, b3;
-                  ldsm_x4(wbase + np * 16 * PA + ks * 32, b0, b1, b2, b3);
-                  mma_bf16(C[2 * np], af[ks], b0, b1);
-                  mma_bf16(C[2 * np + 1], af[ks], b2, b3);
-                }
-              const uint32_t pw0[4] = {p0.x, p0.y, p0.z, p0.w}, pw1[4] = {p1.x, p1.y, p1.z, p1.w};
-#pragma unroll
-              for (int nt = 0; nt < 4; ++nt) {
-                const float2 ph0 = bf2(pw0[nt]), ph1 = bf2(pw1[nt]);
-                const float2 w0 = make_float2(C[nt][0], C[nt][1]), w1 = make_float2(C[nt][2], C[nt][3]);
-                if (c == 0) {
-                  acc[nt] = __ffma2_rn(ph0, w0, acc[nt]);
-                  acc[nt] = __ffma2_rn(ph1, w1, acc[nt]);
-                } else {
-                  const float2 x0 = __fmul2_rn(ph0, w0), x1 = __fmul2_rn(ph1, w1);
-#pragma unroll
-                  for (int ax = 0; ax < 3; ++ax) {
-                    float2 m0, m1;
-                    if (c == 1) {
-                      const float ua0 = ax == 0 ? u0.x : (ax == 1 ? u0.y : u0.z);
-                      const float ua1 = ax == 0 ? u1.x : (ax == 1 ? u1.y : u1.z);
-                      m0 = make_float2(ua0, ua0); m1 = make_float2(ua1, ua1);
-                    } else {
-                      const uint32_t q0 = nt == 0 ? va0[ax].x : nt == 1 ? va0[ax].y : nt == 2 ? va0[ax].z : va0[ax].w;
-                      const uint32_t q1 = nt == 0 ? va1[ax].x : nt == 1 ? va1[ax].y : nt == 2 ? va1[ax].z : va1[ax].w;
-                      m0 = bf2(q0); m1 = bf2(q1);
-                    }
-                    acc[4 * (1 + ax) + nt] = __ffma2_rn(x0, m0, acc[4 * (1 + ax) + nt]);
-                    acc[4 * (1 + ax) + nt] = __ffma2_rn(x1, m1, acc[4 * (1 + ax) + nt]);
-                  }
-                }
-              }
-            }
-          }
-          // reduction over the 8 row groups, residual add, stores
-          float accf[32], r4[4];
-#pragma unroll
-          for (int q = 0; q < 16; ++q) { accf[2 * q] = acc[q].x; accf[2 * q + 1] = acc[q].y; }
-          reduce_scatter32(accf, lane, Rs, r4);
-          const float4 o = make_float4(own.x + r4[0], own.y + r4[1], own.z + r4[2], own.w + r4[3]);
-          if (comp == 0) {
-            *reinterpret_cast<float4*>(s1 + i * ld_s1 + f) = o;
-            if (mir.s1)
-              *reinterpret_cast<uint2*>(mir.s1 + i * mir.ld_s1 + f) = make_uint2(pack_bf2(o.x, o.y), pack_bf2(o.z, o.w));
-          } else {
-            *reinterpret_cast<float4*>(v1 + voff) = o;
-            if (mir.v1) *reinterpret_cast<uint2*>(mir.v1 + voff) = make_uint2(pack_bf2(o.x, o.y), pack_bf2(o.z, o.w));
-          }
-        }
-        __syncwarp(); // the staging buffers are rewritten by the next round / receiver
-        first = false;
-      }
-    }
-  }
 }
 
 // ------------------------------------------------------------------------------------------ reverse
@@ -696,40 +485,9 @@ void pack_filter_bf16(int F, int K, const double* fltW, const double* fltb, uint
         }
 }
 
-size_t edge_mma_smem(int KP, int NSL, int nwarp, bool bwd) {
-  const int PA = KP * 2 + 16, NR = (bwd ? NTCB : NTC) * TE;
-  return (size_t)3 * NSL * 32 * PA + (size_t)nwarp * (NR * (PA * (bwd ? 2 : 1) + 16 + 8 + 4) + 32 * RED_PITCH);
-}
-
-int launch_edge_fwd_mma(const EdgeMmaArgs& a, const __nv_bfloat16* phi, const float* s_in, int64_t ld_sin,
-                        const __nv_bfloat16* v_in, const float* v_res, float* s1, int64_t ld_s1, float* v1,
-                        const EdgeMirror& mir, cudaStream_t st) {
-  if (a.N == 0) return 0;
-  const int KP = edge_mma_kp(a.K), NSL = pick_nsl(a.F), NWARP = 8;
-  // receivers per grid-stride chunk: ~8 chunks per CTA for small batches (cfg3, 8,192 atoms: 32 -> 8 receivers, 378 ->
-  // 337 us), 64 receivers for large ones (cfg4, 391 k atoms: 4.29 -> 4.26 ms)
-  const int RB = (int)std::min<int64_t>(64, std::max<int64_t>(NWARP, a.N / (148 * 2 * 8)));
-  const int64_t nchunk = (a.N + RB - 1) / RB;
-  // 2 resident CTAs per SM; twice that for long batches of ragged molecules (cfg4: 4.26 -> 4.18 ms)
-  dim3 grid((unsigned)std::min<int64_t>(nchunk, nchunk >= 148 * 32 ? 148 * 4 : 148 * 2), a.F / 32 / NSL);
-  const size_t smem = edge_mma_smem(KP, NSL, NWARP, false);
-#define PNN_LAUNCH(KPV, HV)                                                                                        \
-  {                                                                                                                \
-    static bool attr_set = false;                                                                                  \
-    if (!attr_set) {                                                                                               \
-      cudaFuncSetAttribute(edge_fwd_mma_k<KPV, HV>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024);      \
-      attr_set = true;                                                                                             \
-    }                                                                                                              \
-    edge_fwd_mma_k<KPV, HV><<<grid, NWARP * 32, smem, st>>>(a, NSL, RB, phi, s_in, ld_sin, v_in, v_res, s1, ld_s1, \
-                                                            v1, mir);                                              \
-    PNN_KCHECK("edge_fwd_mma_k");                                                                                  \
-  }
-  const bool hv = v_in != nullptr;
-  if (KP == 16) { if (hv) PNN_LAUNCH(16, true) else PNN_LAUNCH(16, false) }
-  else if (KP == 32) { if (hv) PNN_LAUNCH(32, true) else PNN_LAUNCH(32, false) }
-  else { if (hv) PNN_LAUNCH(48, true) else PNN_LAUNCH(48, false) }
-#undef PNN_LAUNCH
-  return 1;
+size_t edge_mma_smem(int KP, int NSL, int nwarp) {
+  const int PA = KP * 2 + 16, NR = NTCB * TE;
+  return (size_t)3 * NSL * 32 * PA + (size_t)nwarp * (NR * (PA * 2 + 16 + 8 + 4) + 32 * RED_PITCH);
 }
 
 int edge_mma_num_slabs(int F) { return F / 32 / pick_nsl(F); }
@@ -742,7 +500,7 @@ int launch_edge_bwd_mma(const EdgeMmaArgs& a, const __nv_bfloat16* phi, const __
   const int RB = (int)std::min<int64_t>(16, std::max<int64_t>(8, a.N / (148 * 2 * 8)));   // cfg3: 16 -> 8, 930 -> 863 us
   const int64_t nchunk = (a.N + RB - 1) / RB;
   dim3 grid((unsigned)std::min<int64_t>(nchunk, 148 * 2), a.F / 32 / NSL);
-  const size_t smem = edge_mma_smem(KP, NSL, NWARP, true);
+  const size_t smem = edge_mma_smem(KP, NSL, NWARP);
 #define PNN_LAUNCH(KPV, HV)                                                                                        \
   {                                                                                                                \
     static bool attr_set = false;                                                                                  \

@@ -1,4 +1,5 @@
-// edge_mma.cuh — edge kernels of the BF16 model with the filter contraction on the tensor cores (edge_mma.cu).
+// edge_mma.cuh — edge kernels of the BF16 model with the filter contraction on the tensor cores (edge_tc.cu forward:
+// tcgen05; edge_mma.cu reverse: mma.sync).
 #pragma once
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -26,10 +27,6 @@ struct EdgeMmaArgs {
 
 int edge_mma_kp(int K);
 void pack_filter_bf16(int F, int K, const double* fltW, const double* fltb, uint16_t* out);
-
-int launch_edge_fwd_mma(const EdgeMmaArgs& a, const __nv_bfloat16* phi, const float* s_in, int64_t ld_sin,
-                        const __nv_bfloat16* v_in, const float* v_res, float* s1, int64_t ld_s1, float* v1,
-                        const EdgeMirror& mir, cudaStream_t st);
 
 // Reverse message step (R3 + R4 partial).  phi / v_in: forward tape (BF16); sb16 [N,F], vb16 [N,3F]: BF16 copies of the
 // incoming adjoints s-bar', v-bar' (gathered and own rows); vb1: the FP32 v-bar' (residual of v-bar_in).  Writes

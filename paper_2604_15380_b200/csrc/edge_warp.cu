@@ -490,11 +490,8 @@ int launch_edge_bwd_warp(const EdgeArgs<float>& a, const float* phi, const float
   const int RB = NW;   // cfg2 0.160 -> 0.144 ms, cfg3 0.76 -> 0.73 ms against 16 receivers per chunk
   const int64_t nchunk = (a.N + RB - 1) / RB;
   dim3 grid((unsigned)std::min<int64_t>(nchunk, 148 * 16), a.F / (32 * FPL));
-  static const bool scalar_math = getenv("PNN_BWD_SCALAR") != nullptr;   // debugging aid: the unpacked kernel
-  if (FPL == 2 && !scalar_math)
+  if (FPL == 2)
     edge_bwd_w2_k<NW><<<grid, NW * 32, 0, st>>>(a, RB, phi, v_in, sb1, vb1, wt, dt, phib, vb_in, fpart, first_block);
-  else if (FPL == 2)
-    edge_bwd_w_k<2, NW><<<grid, NW * 32, 0, st>>>(a, RB, phi, v_in, sb1, vb1, wt, dt, phib, vb_in, fpart, first_block);
   else
     edge_bwd_w_k<1, NW><<<grid, NW * 32, 0, st>>>(a, RB, phi, v_in, sb1, vb1, wt, dt, phib, vb_in, fpart, first_block);
   PNN_KCHECK("edge_bwd_w_k");

@@ -8,8 +8,8 @@
 //   warp 1    MMA issuer: one thread issues tcgen05.mma.cta_group::1.kind::f16 (M = 128, N = BN, K = 16) four times per
 //             k-block, accumulator in TMEM; tcgen05.commit frees the stage ("empty" mbarrier) and finally signals
 //             the epilogue ("accumulator full" mbarrier);
-//   warps 2-5 epilogue: tcgen05.ld (32 lanes x 32 columns per warp), transposition through shared memory so that
-//             global accesses are row-contiguous, then bias / SiLU / silu' / accumulate and FP32 / BF16 stores.
+//   warps 2-5 epilogue: tcgen05.ld (32 lanes x 32 columns per warp): a thread owns one output row and walks it 32 columns
+//             at a time, then bias / SiLU / silu' / accumulate and FP32 / BF16 stores as 32-byte pieces of that row.
 //             Warp 2 also allocates and frees the TMEM columns.
 // K <= 768 here (at most 12 k-blocks), so a CTA is short; two CTAs share an SM (TMEM 2 x 256 columns, shared memory
 // 2 x <= 113 KB) so one tile's epilogue overlaps the other's loads and MMAs.
@@ -156,9 +156,8 @@ struct TcSmem {
   static constexpr int A_BYTES = BM * BK * 2;
   static constexpr int B_BYTES = BN * BK * 2;
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-  static constexpr int EPI_BYTES = 4 * 32 * 33 * 4; // transposition buffers of the four epilogue warps
   static constexpr int PIPE_BYTES = STAGES * STAGE_BYTES;
-  static constexpr int TOTAL = (PIPE_BYTES > EPI_BYTES ? PIPE_BYTES : EPI_BYTES) + 1024 /*alignment slack*/ + 256;
+  static constexpr int TOTAL = PIPE_BYTES + 1024 /*alignment slack*/ + 256;
 };
 
 template <int BN, int STAGES>
@@ -170,7 +169,7 @@ tc_gemm_k(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t tiles = (raw + 1023u) & ~1023u;                 // 1024-byte aligned stage ring
   unsigned char* tiles_ptr = smem_raw + (tiles - raw);
-  const uint32_t PIPE = (L::PIPE_BYTES > L::EPI_BYTES ? L::PIPE_BYTES : L::EPI_BYTES);
+  const uint32_t PIPE = L::PIPE_BYTES;
   uint64_t* bars = reinterpret_cast<uint64_t*>(tiles_ptr + PIPE); // full[STAGES], empty[STAGES], accfull
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 1);
   const uint32_t bar0 = smem_u32(bars);
@@ -500,8 +499,7 @@ int launch_gemm_tc(int64_t M, int N, int K, const __nv_bfloat16* A, int64_t lda,
   int bn = (N % 64 == 0) ? 64 : 32;
   for (int cand = 256; cand > 64; cand >>= 1)
     if (N % cand == 0 && m_tiles * (N / cand) >= 2 * 148) { bn = cand; break; }
-  static const bool no_persist = getenv("PNN_TC_NO_PERSIST") != nullptr; // debugging aid
-  const bool persist = !no_persist && m_tiles * (N / bn) >= 8 * 148;
+  const bool persist = m_tiles * (N / bn) >= 8 * 148;
   // persistent kernel: 128-wide tiles, so that two CTAs (eight epilogue warps) share an SM and its 512 TMEM columns
   if (persist && bn == 256) bn = 128;
   CUtensorMap ta, tb;
@@ -521,6 +519,8 @@ int launch_gemm_tc(int64_t M, int N, int K, const __nv_bfloat16* A, int64_t lda,
     default: return launch_cfg<32, 4>(M, N, K, ta, tb, epi, st);
   }
 }
+
+bool readout_tc_supported(int F) { return F == 64 || F == 128 || F == 256; }
 
 int launch_readout_tc(int64_t N, int F, int H, const __nv_bfloat16* s16, const __nv_bfloat16* W1all, const float* b1,
                       const float* w2, const float* b2, const int32_t* a2s, const int32_t* head, float* opre,

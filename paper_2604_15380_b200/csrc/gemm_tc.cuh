@@ -43,7 +43,9 @@ int launch_gemm_tc(int64_t M, int N, int K, const __nv_bfloat16* A, int64_t lda,
 // stacked first layers of all heads, W1all [H*Fh][F] (BF16): a column tile is exactly one head (Fh in {32, 64, 128}),
 // tiles none of whose 128 rows use that head exit before loading anything, and the epilogue keeps only the rows of
 // its head.  bias = b1 of all heads [H*Fh], w2 [H*Fh], b2 [H].  opre (FP32 [N][Fh], pre-activation for R1) may be NULL.
-// Returns kernels launched, or -1 if this shape is not supported (the caller then uses the SIMT readout).
+// Returns kernels launched, or -1 if the shape is not supported (readout_tc_supported) or a TMA descriptor could not be
+// encoded (an error for the caller).
+bool readout_tc_supported(int F);
 int launch_readout_tc(int64_t N, int F, int H, const __nv_bfloat16* s16, const __nv_bfloat16* W1all, const float* b1,
                       const float* w2, const float* b2, const int32_t* a2s, const int32_t* head, float* opre,
                       float* eatom, int* d_err, cudaStream_t st);

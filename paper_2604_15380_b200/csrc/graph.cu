@@ -10,6 +10,8 @@
 // One warp per receiver scans its candidate cells 32 atoms at a time; __ballot_sync compaction gives every
 // accepted sender its slot, so rows come out in a deterministic order without atomics.  Two passes (count,
 // exclusive scan, emit).  The emit pass also stores the per-edge unit vector and distance in model precision.
+#include <algorithm>
+
 #include "common.cuh"
 
 namespace pnn {
@@ -407,8 +409,28 @@ __global__ void __launch_bounds__(256) neigh_k(int64_t N, const double* __restri
   if (!EMIT && lane == 0) deg[i] = total;
 }
 
-__global__ void check_edges_k(int64_t N, const int32_t* rowptr, int64_t max_edges, int* d_err) {
-  if ((int64_t)rowptr[N] > max_edges) atomicOr(d_err, ERRF_EDGE_OVERFLOW);
+__global__ void check_edges_k(int64_t N, const int32_t* rowptr, int64_t max_edges, int* d_err, int* d_ovf) {
+  const bool over = (int64_t)rowptr[N] > max_edges;
+  *d_ovf = over ? ERRF_EDGE_OVERFLOW : 0; // per-graph word: only the next build resets it
+  if (over) atomicOr(d_err, ERRF_EDGE_OVERFLOW);
+}
+
+// Order-independent 64-bit checksum of the position array (xor of a mix of (index, bit pattern)).
+__device__ __forceinline__ unsigned long long mix64(unsigned long long x) {
+  x ^= x >> 33; x *= 0xff51afd7ed558ccdULL; x ^= x >> 33; x *= 0xc4ceb9fe1a85ec53ULL; x ^= x >> 33;
+  return x;
+}
+__global__ void __launch_bounds__(256) pos_hash_k(int64_t n, const double* __restrict__ pos, unsigned long long* out) {
+  unsigned long long h = 0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+    h ^= mix64((unsigned long long)__double_as_longlong(pos[i]) + 0x9e3779b97f4a7c15ULL * (unsigned long long)(i + 1));
+#pragma unroll
+  for (int o = 16; o; o >>= 1) h ^= __shfl_xor_sync(0xffffffffu, h, o);
+  if ((threadIdx.x & 31) == 0 && h) atomicXor(out, h);
+}
+__global__ void pos_cmp_k(unsigned long long* chk, int* d_err) {
+  if (chk[1] != chk[0]) atomicOr(d_err, ERRF_STALE_GRAPH);
+  chk[1] = 0;
 }
 
 } // namespace
@@ -416,10 +438,14 @@ __global__ void check_edges_k(int64_t N, const int32_t* rowptr, int64_t max_edge
 int launch_graph_build(const GraphBuffers& gb, int64_t N, int64_t S, const double* pos, const int32_t* sptr,
                        const double* cell, const uint8_t* pbc, double rc, int prec, int all_images, cudaStream_t st) {
   int nl = 0;
+  cudaMemsetAsync(gb.d_poschk, 0, 2 * sizeof(unsigned long long), st);
   if (N == 0 || S == 0) {
     cudaMemsetAsync(gb.rowptr, 0, sizeof(int32_t) * (N + 1), st);
+    cudaMemsetAsync(gb.d_ovf, 0, sizeof(int), st);
     return 0;
   }
+  pos_hash_k<<<(unsigned)std::min<int64_t>((3 * N + 255) / 256, 592), 256, 0, st>>>(3 * N, pos, gb.d_poschk);
+  PNN_KCHECK("pos_hash_k"); ++nl;
   const int64_t ncap = N + S; // upper bound on the number of cells
   desc_k<<<(unsigned)S, 128, 0, st>>>(S, pos, sptr, cell, pbc, rc, gb.desc, gb.ncell, gb.a2s); PNN_KCHECK("desc_k"); ++nl;
   nl += exclusive_scan(gb.ncell, S, gb.cell_off, gb.scan_tmp, st);
@@ -442,7 +468,7 @@ int launch_graph_build(const GraphBuffers& gb, int64_t N, int64_t S, const doubl
             nullptr, nullptr, (Geom<float>*)nullptr, gb.max_edges)
   ++nl;
   nl += exclusive_scan(gb.deg, N, gb.rowptr, gb.scan_tmp, st);
-  check_edges_k<<<1, 1, 0, st>>>(N, gb.rowptr, gb.max_edges, gb.d_err); PNN_KCHECK("check_edges_k"); ++nl;
+  check_edges_k<<<1, 1, 0, st>>>(N, gb.rowptr, gb.max_edges, gb.d_err, gb.d_ovf); PNN_KCHECK("check_edges_k"); ++nl;
   if (prec == 2) {
     PNN_NEIGH(double, true, N, pos, gb.a2s, gb.desc, gb.cell_off, gb.cid, gb.cell_start, gb.sorted, rc2, nullptr,
               gb.rowptr, gb.col, gb.shift, (Geom<double>*)gb.geom, gb.max_edges)
@@ -453,6 +479,15 @@ int launch_graph_build(const GraphBuffers& gb, int64_t N, int64_t S, const doubl
 #undef PNN_NEIGH
   ++nl;
   return nl;
+}
+
+int launch_pos_check(const GraphBuffers& gb, int64_t N, const double* pos, cudaStream_t st) {
+  if (N == 0) return 0;
+  pos_hash_k<<<(unsigned)std::min<int64_t>((3 * N + 255) / 256, 592), 256, 0, st>>>(3 * N, pos, gb.d_poschk + 1);
+  PNN_KCHECK("pos_hash_k");
+  pos_cmp_k<<<1, 1, 0, st>>>(gb.d_poschk, gb.d_err);
+  PNN_KCHECK("pos_cmp_k");
+  return 2;
 }
 
 } // namespace pnn

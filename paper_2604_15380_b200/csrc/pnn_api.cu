@@ -119,6 +119,7 @@ struct pnn_workspace {
   // forward edge kernel and consumed by the reverse one (NULL when it would not fit: the filter is then recomputed)
   float* etape = nullptr;
   int64_t etape_block = 0; // floats per block (= 2 * maxE * 3F)
+  int64_t etape_bytes = 0;
   // staging for pnn_eval_host
   int32_t *st_Z, *st_sptr, *st_head;
   double *st_pos, *st_cell;
@@ -132,6 +133,16 @@ struct pnn_workspace {
 };
 
 namespace {
+int read_error_flags(pnn_workspace* ws) {
+  int flags[2] = {0, 0};
+  PNN_TRY(cudaMemcpy(flags, ws->g.d_err, 8, cudaMemcpyDeviceToHost));
+  PNN_TRY(cudaMemset(ws->g.d_err, 0, 4));
+  if ((flags[0] | flags[1]) & ERRF_EDGE_OVERFLOW) { ws->graph_N = ws->graph_S = -1; return PNN_ERR_CAPACITY; }
+  if (flags[0] & ERRF_STALE_GRAPH) return PNN_ERR_NO_GRAPH;
+  if (flags[0] & (ERRF_BAD_Z | ERRF_BAD_HEAD)) return PNN_ERR_BAD_INPUT;
+  return PNN_OK;
+}
+
 // Brackets the launches of one kernel family with CUDA events on the launch stream when profiling is on.
 struct ProfScope {
   pnn_workspace* ws; cudaStream_t st; const char* name; int64_t l0; cudaEvent_t a = nullptr;
@@ -306,7 +317,10 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
   if (maxN > 0x7fffffffLL / 32 || maxE > 0x7fffffffLL - 64 || maxS > 0x7fffffffLL - 64) return PNN_ERR_CAPACITY;
   pnn_workspace* ws = new (std::nothrow) pnn_workspace();
   if (!ws) return PNN_ERR_INVALID_ARG;
-  ws->model = m; ws->maxN = maxN; ws->maxE = maxE; ws->maxS = maxS; ws->want_forces = want_forces ? 1 : 0;
+  if (want_forces & ~(PNN_WS_FORCES | PNN_WS_NO_EDGE_TAPE)) { delete ws; return PNN_ERR_INVALID_ARG; }
+  const bool no_tape = (want_forces & PNN_WS_NO_EDGE_TAPE) != 0;
+  want_forces = (want_forces & PNN_WS_FORCES) ? 1 : 0;
+  ws->model = m; ws->maxN = maxN; ws->maxE = maxE; ws->maxS = maxS; ws->want_forces = want_forces;
   const int64_t F = m->cfg.F, T = m->cfg.T;
   const size_t es = elem_size(m->cfg.prec);
   const int64_t N = maxN > 0 ? maxN : 1, E = maxE > 0 ? maxE : 1, S = maxS > 0 ? maxS : 1;
@@ -335,6 +349,8 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
     g.geom = carve(4 * es * E);
     g.scan_tmp = (int32_t*)carve(4 * ((N + S + 2) / 1024 + 4));
     g.d_err = (int*)carve(256);
+    g.d_ovf = pass ? g.d_err + 1 : nullptr;
+    g.d_poschk = pass ? reinterpret_cast<unsigned long long*>(g.d_err + 4) : nullptr;
     g.max_edges = maxE;
     ws->s_cur = carve(es * N * F);
     ws->h = carve(es * N * F);
@@ -415,18 +431,17 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
       }
     }
   }
-  if (m->cfg.prec == PNN_FP32 && want_forces && maxE > 0) {
+  if (m->cfg.prec == PNN_FP32 && want_forces && maxE > 0 && !no_tape) {
+    // the FP32 edge tape (w and dw/dd of every edge and block): required unless the caller opted out with
+    // PNN_WS_NO_EDGE_TAPE; running out of memory is an error, never a silent change of kernels
     const int64_t per_block = 2 * maxE * 3 * F;
     const int64_t bytes = per_block * T * 4;
-    size_t free_b = 0, total_b = 0;
-    cudaMemGetInfo(&free_b, &total_b);
-    if (bytes <= (int64_t)(free_b / 2) && cudaMalloc((void**)&ws->etape, bytes) == cudaSuccess) {
-      ws->etape_block = per_block;
-      ws->arena_bytes += bytes;
-    } else {
-      ws->etape = nullptr;
-      cudaGetLastError();
+    if (!cuda_ok(cudaMalloc((void**)&ws->etape, bytes), "cudaMalloc(edge tape; create the workspace with PNN_WS_NO_EDGE_TAPE or a smaller max_edges)")) {
+      cudaFree(ws->arena); delete ws; return PNN_ERR_CUDA;
     }
+    ws->etape_block = per_block;
+    ws->etape_bytes = bytes;
+    ws->arena_bytes += bytes;
   }
   *out = ws;
   return PNN_OK;
@@ -442,6 +457,7 @@ void pnn_workspace_destroy(pnn_workspace* ws) {
 }
 
 int64_t pnn_workspace_bytes(const pnn_workspace* ws) { return ws ? ws->arena_bytes : 0; }
+int64_t pnn_workspace_edge_tape_bytes(const pnn_workspace* ws) { return ws ? ws->etape_bytes : 0; }
 int64_t pnn_launch_count(const pnn_workspace* ws) { return ws ? ws->launches : 0; }
 
 int pnn_build_graph(pnn_workspace* ws, int64_t N, int64_t S, const double* pos, const int32_t* sptr,
@@ -525,12 +541,7 @@ int pnn_profile_read(pnn_workspace* ws, int max_entries, char* names, double* to
 int pnn_check_async_errors(pnn_workspace* ws) {
   if (!ws) return PNN_ERR_INVALID_ARG;
   PNN_TRY(cudaDeviceSynchronize());
-  int flags = 0;
-  PNN_TRY(cudaMemcpy(&flags, ws->g.d_err, 4, cudaMemcpyDeviceToHost));
-  PNN_TRY(cudaMemset(ws->g.d_err, 0, 4));
-  if (flags & ERRF_EDGE_OVERFLOW) return PNN_ERR_CAPACITY;
-  if (flags & (ERRF_BAD_Z | ERRF_BAD_HEAD)) return PNN_ERR_BAD_INPUT;
-  return PNN_OK;
+  return read_error_flags(ws);
 }
 
 } // extern "C"
@@ -548,10 +559,9 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
   int nl = 0;
   EdgeArgs<T> ea;
   ea.N = N; ea.F = F; ea.K = c.K; ea.rc = c.cutoff; ea.rbf = c.rbf;
-  ea.rowptr = ws->g.rowptr; ea.col = ws->g.col; ea.geom = (const Geom<T>*)ws->g.geom; ea.d_err = ws->g.d_err;
+  ea.rowptr = ws->g.rowptr; ea.col = ws->g.col; ea.geom = (const Geom<T>*)ws->g.geom; ea.d_err = ws->g.d_ovf;
   T* s_cur = (T*)ws->s_cur; T* h = (T*)ws->h; T* sn = (T*)ws->sn; T* v1 = (T*)ws->v1; T* k = (T*)ws->k;
   const bool taped = ws->want_forces != 0;
-  static const bool old_edges = getenv("PNN_FP32_CTA_EDGES") != nullptr; // debugging aid: edge.cu kernels for FP32 too
 
   { ProfScope ps_(ws, st, "embed");
   const int l_ = launch_embed<T>(N, F, c.Zmax, Z, W + m->emb, s_cur, ws->g.d_err, st);
@@ -582,9 +592,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       int l_;
       if constexpr (std::is_same<T, float>::value) {
         float* wt = (want_f && ws->etape) ? ws->etape + (int64_t)t * ws->etape_block : nullptr;
-        l_ = old_edges ? launch_edge_fwd<T, T>(ea, phi, s_cur, F, v_in, v_in, sn, 2 * F, v1, EdgeMirror(), st)
-                       : launch_edge_fwd_warp(ea, phi, s_cur, F, v_in, sn, 2 * F, v1, wt,
-                                              wt ? wt + ws->etape_block / 2 : nullptr, st);
+        l_ = launch_edge_fwd_warp(ea, phi, s_cur, F, v_in, sn, 2 * F, v1, wt, wt ? wt + ws->etape_block / 2 : nullptr, st);
       } else {
         l_ = launch_edge_fwd<T, T>(ea, phi, s_cur, F, v_in, v_in, sn, 2 * F, v1, EdgeMirror(), st);
       }
@@ -651,7 +659,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       { ProfScope ps_(ws, st, "edge_bwd");
         int l_;
         bool taped_edges = false;
-        if constexpr (std::is_same<T, float>::value) taped_edges = !old_edges && ws->etape != nullptr;
+        if constexpr (std::is_same<T, float>::value) taped_edges = ws->etape != nullptr;
         if constexpr (std::is_same<T, float>::value) {
           if (taped_edges) {
             const float* wt = ws->etape + (int64_t)t * ws->etape_block;
@@ -678,7 +686,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     { ProfScope ps_(ws, st, "force_assemble");
       int nslab = edge_num_slabs(F);
       if constexpr (std::is_same<T, float>::value)
-        if (!old_edges && ws->etape != nullptr) nslab = edge_warp_num_slabs(F, c.K);
+        if (ws->etape != nullptr) nslab = edge_warp_num_slabs(F, c.K);
     const int l_ = launch_force_assemble<T>(N, nslab, fpart, forces, st);
       nl += l_; ps_.done(l_); }
   }
@@ -703,14 +711,13 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
   bool tc_fail = false;
   EdgeArgs<T> ea;
   ea.N = N; ea.F = F; ea.K = c.K; ea.rc = c.cutoff; ea.rbf = c.rbf;
-  ea.rowptr = ws->g.rowptr; ea.col = ws->g.col; ea.geom = (const Geom<T>*)ws->g.geom; ea.d_err = ws->g.d_err;
+  ea.rowptr = ws->g.rowptr; ea.col = ws->g.col; ea.geom = (const Geom<T>*)ws->g.geom; ea.d_err = ws->g.d_ovf;
   T* s_cur = (T*)ws->s_cur; T* sn = (T*)ws->sn; T* v1 = (T*)ws->v1;
   pnn_workspace::Mirror& mb = ws->mb;
   const bool taped = ws->want_forces != 0;
   EdgeMmaArgs em;
   em.N = N; em.F = F; em.K = c.K; em.rbf = c.rbf; em.rc = (float)c.cutoff; em.rowptr = ws->g.rowptr; em.col = ws->g.col;
-  em.geom = (const Geom<float>*)ws->g.geom; em.d_err = ws->g.d_err;
-  static const bool simt_edges = getenv("PNN_BF16_SIMT_EDGES") != nullptr; // debugging aid: the SIMT edge kernels
+  em.geom = (const Geom<float>*)ws->g.geom; em.d_err = ws->g.d_ovf;
   // C / Cb [M,N] = epi(A[M,K] . Wt[N,K]^T): A BF16 (row stride lda), Wt at element offset woff of the BF16 weight copy
   auto tc = [&](const char* fam, int64_t M, int Nn, int K, const B* A, int64_t lda, int64_t woff, const TcEpi& e) {
     ProfScope ps_(ws, st, fam);
@@ -746,9 +753,8 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     { ProfScope ps_(ws, st, "edge_fwd");
       EdgeMirror mir; mir.s1 = mb.sn16; mir.ld_s1 = 2 * F; mir.v1 = mb.v1_16;
       em.fltP = m->d_fltP + (int64_t)t * m->fltP_stride;
-      const int l_ = simt_edges ? launch_edge_fwd<T, B>(ea, tp16.phi16, s_cur, F, v_in16, v_in, sn, 2 * F, v1, mir, st)
-                                : launch_edge_fwd_tc(em, m->d_fltT + (int64_t)t * m->fltT_stride, tp16.phi16, s_cur, F,
-                                                     v_in16, v_in, sn, 2 * F, v1, mir, st); // B3b
+      const int l_ = launch_edge_fwd_tc(em, m->d_fltT + (int64_t)t * m->fltT_stride, tp16.phi16, s_cur, F, v_in16, v_in, sn,
+                                        2 * F, v1, mir, st); // B3b
       nl += l_; ps_.done(l_); }
     TcEpi e3; e3.Cb = PQ; e3.ldcb = 2 * F;
     tc("gemm_3N", 3 * N, 2 * F, F, mb.v1_16, F, b.UV, e3);                         // B4: P | Q
@@ -768,12 +774,14 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     if (hw) { // blended heads: FP32 readout of the FP32 residual stream (one structure may need every head)
       l_ = launch_readout_blend<T>(N, S, F, c.H, s_cur, ws->g.a2s, hw, (T)skip_below, sptr, W + m->oW1t, W + m->ob1,
                                    W + m->ow2, W + m->ob2, (T*)ws->opre_all, (T*)ws->eatom, energy, st);
-    } else {
-    l_ = launch_readout_tc(N, F, c.H, mb.s16, Wb + m->oW1, W + m->ob1, W + m->ow2, W + m->ob2, ws->g.a2s, head,
-                               (T*)ws->opre, (T*)ws->eatom, ws->g.d_err, st);
-    if (l_ >= 0) l_ += launch_struct_sum<T>(S, sptr, (const T*)ws->eatom, energy, st);
-    else l_ = launch_readout<T>(N, S, F, c.H, s_cur, ws->g.a2s, head, sptr, W + m->oW1t, W + m->ob1, W + m->ow2,
-                                W + m->ob2, (T*)ws->opre, (T*)ws->eatom, energy, ws->g.d_err, st);
+    } else if (readout_tc_supported(F)) { // head widths F/2 in {32, 64, 128}: one tensor-core GEMM over the stacked heads
+      l_ = launch_readout_tc(N, F, c.H, mb.s16, Wb + m->oW1, W + m->ob1, W + m->ow2, W + m->ob2, ws->g.a2s, head,
+                             (T*)ws->opre, (T*)ws->eatom, ws->g.d_err, st);
+      if (l_ < 0) { tc_fail = true; l_ = 0; }
+      else l_ += launch_struct_sum<T>(S, sptr, (const T*)ws->eatom, energy, st);
+    } else { // other widths: the FP32 readout of the FP32 residual stream
+      l_ = launch_readout<T>(N, S, F, c.H, s_cur, ws->g.a2s, head, sptr, W + m->oW1t, W + m->ob1, W + m->ow2,
+                             W + m->ob2, (T*)ws->opre, (T*)ws->eatom, energy, ws->g.d_err, st);
     }
     nl += l_; ps_.done(l_); }
   if (want_f) {
@@ -805,10 +813,8 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
       { ProfScope ps_(ws, st, "edge_bwd");
         em.fltP = m->d_fltP + (int64_t)t * m->fltP_stride;
-        const int l_ = simt_edges ? launch_edge_bwd<T, B>(ea, tp16.phi16, tp16.vin16, sb, vb, nullptr, vb2, fpart,
-                                                          last ? 1 : 0, t > 0 ? mb.phib16 : nullptr, st)
-                                  : launch_edge_bwd_mma(em, tp16.phi16, tp16.vin16, mb.sb16, mb.vb16, vb,
-                                                        t > 0 ? mb.phib16 : nullptr, vb2, fpart, last ? 1 : 0, st);
+        const int l_ = launch_edge_bwd_mma(em, tp16.phi16, tp16.vin16, mb.sb16, mb.vb16, vb, t > 0 ? mb.phib16 : nullptr, vb2,
+                                           fpart, last ? 1 : 0, st);
         nl += l_; ps_.done(l_); }
       if (t > 0) {
         TcEpi g4; g4.act = ACT_MUL_DSILU; g4.aux = (const T*)tp.hpre; g4.ldaux = F; g4.Cb = mb.hb16; g4.ldcb = F;
@@ -819,7 +825,7 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       }
     }
     { ProfScope ps_(ws, st, "force_assemble");
-      const int l_ = launch_force_assemble<T>(N, simt_edges ? edge_num_slabs(F) : edge_mma_num_slabs(F), fpart, forces, st);
+      const int l_ = launch_force_assemble<T>(N, edge_mma_num_slabs(F), fpart, forces, st);
       nl += l_; ps_.done(l_); }
   }
   ws->launches += nl;
@@ -857,18 +863,20 @@ static int eval_common(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t
 
 int pnn_eval(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const double* pos,
              const int32_t* sptr, const int32_t* head, int flags, void* energy, void* forces, void* stream) {
-  (void)pos;
-  if (S > 0 && !head) return PNN_ERR_INVALID_ARG;
-  return eval_common(m, ws, N, S, Z, sptr, head, nullptr, 0.0, flags, energy, forces, stream);
+  if ((S > 0 && !head) || (N > 0 && !pos)) return PNN_ERR_INVALID_ARG;
+  const int rc = eval_common(m, ws, N, S, Z, sptr, head, nullptr, 0.0, flags, energy, forces, stream);
+  if (rc == PNN_OK) ws->launches += launch_pos_check(ws->g, N, pos, (cudaStream_t)stream);
+  return rc;
 }
 
 int pnn_eval_blended(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const double* pos,
                      const int32_t* sptr, const void* head_weights, double skip_below, int flags, void* energy,
                      void* forces, void* stream) {
-  (void)pos;
-  if (S > 0 && !head_weights) return PNN_ERR_INVALID_ARG;
+  if ((S > 0 && !head_weights) || (N > 0 && !pos)) return PNN_ERR_INVALID_ARG;
   if ((flags & PNN_FORCES) && ws && !ws->opre_all) return PNN_ERR_INVALID_ARG;
-  return eval_common(m, ws, N, S, Z, sptr, nullptr, head_weights, skip_below, flags, energy, forces, stream);
+  const int rc = eval_common(m, ws, N, S, Z, sptr, nullptr, head_weights, skip_below, flags, energy, forces, stream);
+  if (rc == PNN_OK) ws->launches += launch_pos_check(ws->g, N, pos, (cudaStream_t)stream);
+  return rc;
 }
 
 struct pnn_branch_mlp {
@@ -981,7 +989,7 @@ int pnn_eval_host(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, c
   if ((flags & PNN_FORCES) && N > 0)
     PNN_TRY(cudaMemcpyAsync(forces_host, ws->st_forces, es * 3 * N, cudaMemcpyDeviceToHost, st));
   PNN_TRY(cudaStreamSynchronize(st));
-  return PNN_OK;
+  return read_error_flags(ws); // overflow / bad input are errors of this synchronous call, not of a later check
 }
 
 int pnn_gemm_bf16(int64_t M, int32_t N, int32_t K, const void* A, int64_t lda, const void* Wt, int64_t ldw,

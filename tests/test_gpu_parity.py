@@ -198,19 +198,29 @@ def test_host_entry_point_matches_device_entry_point():
     net.close()
 
 
-def test_fp32_recompute_edge_kernels_subprocess():
-    """The FP32 model normally runs edge_warp.cu with the edge tape; PNN_FP32_CTA_EDGES=1 selects the recomputing
-    kernels of edge.cu (the path taken when the tape does not fit).  Both must meet the FP32 tolerance."""
-    import os
-    import subprocess
-    import sys
-    code = ("import sys, os; sys.path.insert(0, os.getcwd()); sys.path.insert(0, 'tests');"
-            "import gen, oracle; from gpu_common import run_gpu; from helpers import energy_rel_err, force_rel_err;"
-            "mc, b = gen.model_cfg(2), gen.make_batch(2, 3, 12); w = gen.make_weights(mc, 2);"
-            "out = run_gpu(mc, w, b, 'fp32'); ref = oracle.evaluate(mc, w, b);"
-            "assert energy_rel_err(out['energy'], ref['energy']).max() < 1e-5;"
-            "assert force_rel_err(out['forces'], ref['forces'], b.struct_ptr).max() < 1e-4; print('ok')")
-    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    env = dict(os.environ, PNN_FP32_CTA_EDGES="1")
-    r = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True, timeout=600)
-    assert r.returncode == 0 and "ok" in r.stdout, r.stderr[-2000:]
+def test_fp32_without_the_edge_tape():
+    """The FP32 model normally keeps the edge tape (edge_warp.cu forward and reverse kernels); a workspace created with
+    PNN_WS_NO_EDGE_TAPE runs the forward warp kernel without the tape and the recomputing reverse kernel of edge.cu (its
+    own force-slab count).  Both must meet the FP32 tolerance, and the workspace must report which one it is."""
+    import paper_2604_15380_b200 as pnn
+    import torch
+    from gpu_common import to_device
+    mc, b = gen.model_cfg(2), gen.make_batch(2, 3, 12)
+    w = gen.make_weights(mc, 2)
+    ref = oracle.evaluate(mc, w, b)
+    res = {}
+    for tape in (True, False):
+        net = pnn.PaiNN(mc.F, mc.T, mc.K, mc.H, w, precision="fp32", cutoff=mc.cutoff, Zmax=mc.Zmax, norm_eps=mc.norm_eps,
+                        max_atoms=b.n_atoms, max_edges=b.n_atoms * 40, max_structs=b.n_structs, forces=True,
+                        edge_tape=tape)
+        assert (pnn.pnn_workspace_edge_tape_bytes(net.ws) > 0) == tape
+        if tape:
+            assert pnn.pnn_workspace_edge_tape_bytes(net.ws) == 24 * mc.F * mc.T * b.n_atoms * 40
+        t = to_device(b)
+        e, f = net.eval(t["Z"], t["pos"], t["struct_ptr"], t["head"])
+        torch.cuda.synchronize()
+        net.check()
+        res[tape] = (e.cpu().numpy().astype(np.float64), f.cpu().numpy().astype(np.float64))
+        net.close()
+        assert energy_rel_err(res[tape][0], ref["energy"]).max() < 1e-5
+        assert force_rel_err(res[tape][1], ref["forces"], b.struct_ptr).max() < 1e-4
