@@ -168,6 +168,34 @@ int pnn_eval_host(const pnn_model* m, pnn_workspace* ws, int64_t n_atoms, int64_
                   const double* pos, const int32_t* struct_ptr, const int32_t* head, const double* cell,
                   const uint8_t* pbc, int flags, void* energy_host, void* forces_host, void* cuda_stream);
 
+/* Streaming driver for screening runs ("1.1 billion atomistic structures in 50 seconds", the per-GPU
+ * throughput of PAPER.md:422-426; BASELINE.json configs[3]: 1,048,576 structures "streamed in batches of 16,384";
+ * SURVEY.md §7 step 8): `depth` pipeline slots, each with its own workspace, staging buffers and CUDA stream, so that the
+ * host-to-device copies of batch k+1 and the device-to-host copies of batch k-1 overlap the kernels of batch k.
+ *   pnn_stream_create  flags = PNN_ENERGY [| PNN_FORCES] for every batch; sizes are per batch; 1 <= depth <= 8
+ *                      (2 = double buffering).  Device memory: depth workspaces (pnn_stream_bytes).
+ *   pnn_stream_submit  enqueues one batch (arguments as pnn_eval_host, all HOST pointers; pinned memory is needed for the
+ *                      copies to overlap) into slot (number of batches submitted so far) mod depth and returns without
+ *                      waiting for it; the input and output buffers must stay valid and untouched until the batch has been
+ *                      waited for.  If that slot still holds an unfinished batch the call first waits for it, and a device
+ *                      error of THAT batch is what it returns.
+ *   pnn_stream_wait    blocks until the oldest batch not yet waited for is complete (its energy_host / forces_host are
+ *                      then valid) and returns its device-side status (PNN_ERR_CAPACITY, PNN_ERR_BAD_INPUT); PNN_OK when
+ *                      nothing is in flight.
+ *   pnn_stream_drain   waits for everything in flight; returns the first error.
+ * Results are bit-identical to pnn_eval_host on the same batch (same kernels, same launch configuration). */
+typedef struct pnn_stream pnn_stream;
+int pnn_stream_create(const pnn_model* m, int64_t max_atoms, int64_t max_edges, int64_t max_structs, int flags,
+                      int depth, pnn_stream** out);
+void pnn_stream_destroy(pnn_stream* s);
+int pnn_stream_submit(pnn_stream* s, int64_t n_atoms, int64_t n_structs, const int32_t* Z, const double* pos,
+                      const int32_t* struct_ptr, const int32_t* head, const double* cell, const uint8_t* pbc,
+                      void* energy_host, void* forces_host);
+int pnn_stream_wait(pnn_stream* s);
+int pnn_stream_drain(pnn_stream* s);
+int64_t pnn_stream_launch_count(const pnn_stream* s); /* kernels launched on behalf of the stream so far */
+int64_t pnn_stream_bytes(const pnn_stream* s);        /* device memory held by its workspaces          */
+
 /* Reads the device error flags (edge overflow -> PNN_ERR_CAPACITY, positions changed since pnn_build_graph ->
  * PNN_ERR_NO_GRAPH, bad Z / head -> PNN_ERR_BAD_INPUT) and clears them.  Synchronises the device. */
 int pnn_check_async_errors(pnn_workspace* ws);

@@ -18,7 +18,8 @@ __all__ = [
     "pnn_model_destroy", "pnn_branch_mlp_create", "pnn_branch_mlp_destroy", "pnn_branch_weights",
     "pnn_workspace_create", "pnn_workspace_destroy", "pnn_workspace_bytes", "pnn_workspace_edge_tape_bytes",
     "PNN_WS_FORCES", "PNN_WS_NO_EDGE_TAPE", "pnn_build_graph",
-    "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_eval_blended", "pnn_eval_host", "pnn_check_async_errors", "pnn_measure_alu_peak", "pnn_launch_count", "pnn_profile_enable",
+    "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_eval_blended", "pnn_eval_host", "pnn_stream_create", "pnn_stream_destroy", "pnn_stream_submit", "pnn_stream_wait",
+    "pnn_stream_drain", "pnn_stream_launch_count", "pnn_stream_bytes", "pnn_check_async_errors", "pnn_measure_alu_peak", "pnn_launch_count", "pnn_profile_enable",
     "pnn_profile_read", "pnn_gemm_bf16",
     "PaiNN", "PRECISIONS",
 ]
@@ -87,6 +88,16 @@ def lib():
         L.pnn_branch_mlp_destroy.argtypes = [vp]
         L.pnn_branch_mlp_destroy.restype = None
         L.pnn_branch_weights.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp]
+        L.pnn_stream_create.argtypes = [vp, i64, i64, i64, i32, i32, ctypes.POINTER(vp)]
+        L.pnn_stream_destroy.argtypes = [vp]
+        L.pnn_stream_destroy.restype = None
+        L.pnn_stream_submit.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.pnn_stream_wait.argtypes = [vp]
+        L.pnn_stream_drain.argtypes = [vp]
+        L.pnn_stream_launch_count.argtypes = [vp]
+        L.pnn_stream_launch_count.restype = i64
+        L.pnn_stream_bytes.argtypes = [vp]
+        L.pnn_stream_bytes.restype = i64
         L.pnn_check_async_errors.argtypes = [vp]
         L.pnn_profile_enable.argtypes = [vp, i32]
         L.pnn_profile_read.argtypes = [vp, i32, vp, vp, vp, ctypes.POINTER(i32)]
@@ -240,6 +251,42 @@ def pnn_eval_host(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, str
                                _ptr(struct_ptr, "i32", False), _ptr(head, "i32", False), _ptr(cell, "f64", False),
                                _ptr(pbc, "u8", False), flags, _ptr(energy_host, None, False),
                                _ptr(forces_host, None, False), stream), "pnn_eval_host")
+
+
+def pnn_stream_create(model: int, max_atoms: int, max_edges: int, max_structs: int, flags: int, depth: int = 2) -> int:
+    out = ctypes.c_void_p()
+    _check(lib().pnn_stream_create(model, max_atoms, max_edges, max_structs, flags, depth, ctypes.byref(out)),
+           "pnn_stream_create")
+    return out.value
+
+
+def pnn_stream_destroy(s: int) -> None:
+    lib().pnn_stream_destroy(s)
+
+
+def pnn_stream_submit(s: int, n_atoms: int, n_structs: int, Z, pos, struct_ptr, head, cell, pbc, energy_host,
+                      forces_host=None) -> None:
+    """All HOST arrays (numpy or pinned torch CPU tensors); they must stay alive until the batch has been waited for."""
+    _check(lib().pnn_stream_submit(s, n_atoms, n_structs, _ptr(Z, "i32", False), _ptr(pos, "f64", False),
+                                   _ptr(struct_ptr, "i32", False), _ptr(head, "i32", False), _ptr(cell, "f64", False),
+                                   _ptr(pbc, "u8", False), _ptr(energy_host, None, False), _ptr(forces_host, None, False)),
+           "pnn_stream_submit")
+
+
+def pnn_stream_wait(s: int) -> None:
+    _check(lib().pnn_stream_wait(s), "pnn_stream_wait")
+
+
+def pnn_stream_drain(s: int) -> None:
+    _check(lib().pnn_stream_drain(s), "pnn_stream_drain")
+
+
+def pnn_stream_launch_count(s: int) -> int:
+    return lib().pnn_stream_launch_count(s)
+
+
+def pnn_stream_bytes(s: int) -> int:
+    return lib().pnn_stream_bytes(s)
 
 
 def pnn_check_async_errors(ws: int) -> None:

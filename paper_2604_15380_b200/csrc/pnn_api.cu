@@ -959,9 +959,10 @@ int pnn_measure_alu_peak(int prec, double* tflops, void* stream) {
   return PNN_OK;
 }
 
-int pnn_eval_host(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const double* pos,
-                  const int32_t* sptr, const int32_t* head, const double* cell, const uint8_t* pbc, int flags,
-                  void* energy_host, void* forces_host, void* stream) {
+// H2D copies + pnn_build_graph + pnn_eval + D2H copies of one batch, all enqueued on `stream`; nothing is waited for.
+static int enqueue_host_batch(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z,
+                              const double* pos, const int32_t* sptr, const int32_t* head, const double* cell,
+                              const uint8_t* pbc, int flags, void* energy_host, void* forces_host, void* stream) {
   if (!m || !ws || N < 0 || S < 0) return PNN_ERR_INVALID_ARG;
   if (N > ws->maxN || S > ws->maxS) return PNN_ERR_CAPACITY;
   if ((N > 0 && (!Z || !pos)) || !sptr || (S > 0 && (!head || !energy_host))) return PNN_ERR_INVALID_ARG;
@@ -982,14 +983,121 @@ int pnn_eval_host(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, c
   int rc = pnn_build_graph(ws, N, S, ws->st_pos, ws->st_sptr, periodic ? ws->st_cell : nullptr,
                            periodic ? ws->st_pbc : nullptr, stream);
   if (rc != PNN_OK) return rc;
-  rc = pnn_eval(m, ws, N, S, ws->st_Z, ws->st_pos, ws->st_sptr, ws->st_head, flags, ws->st_energy, ws->st_forces,
-                stream);
+  rc = eval_common(m, ws, N, S, ws->st_Z, ws->st_sptr, ws->st_head, nullptr, 0.0, flags, ws->st_energy, ws->st_forces,
+                   stream);
   if (rc != PNN_OK) return rc;
   if (S > 0) PNN_TRY(cudaMemcpyAsync(energy_host, ws->st_energy, es * S, cudaMemcpyDeviceToHost, st));
   if ((flags & PNN_FORCES) && N > 0)
     PNN_TRY(cudaMemcpyAsync(forces_host, ws->st_forces, es * 3 * N, cudaMemcpyDeviceToHost, st));
-  PNN_TRY(cudaStreamSynchronize(st));
+  return PNN_OK;
+}
+
+int pnn_eval_host(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const double* pos,
+                  const int32_t* sptr, const int32_t* head, const double* cell, const uint8_t* pbc, int flags,
+                  void* energy_host, void* forces_host, void* stream) {
+  const int rc = enqueue_host_batch(m, ws, N, S, Z, pos, sptr, head, cell, pbc, flags, energy_host, forces_host, stream);
+  if (rc != PNN_OK) return rc;
+  PNN_TRY(cudaStreamSynchronize((cudaStream_t)stream));
   return read_error_flags(ws); // overflow / bad input are errors of this synchronous call, not of a later check
+}
+
+// ------------------------------------------------------------------------------------------------ streaming driver
+struct pnn_stream {
+  const pnn_model* model = nullptr;
+  int depth = 0, flags = 0;
+  struct Slot { pnn_workspace* ws = nullptr; cudaStream_t st = nullptr; bool busy = false; int* err_host = nullptr; };
+  std::vector<Slot> slot;
+  int64_t submitted = 0, waited = 0;
+};
+
+int pnn_stream_create(const pnn_model* m, int64_t max_atoms, int64_t max_edges, int64_t max_structs, int flags,
+                      int depth, pnn_stream** out) {
+  if (!m || !out || depth < 1 || depth > 8 || !(flags & (PNN_ENERGY | PNN_FORCES))) return PNN_ERR_INVALID_ARG;
+  pnn_stream* s = new (std::nothrow) pnn_stream();
+  if (!s) return PNN_ERR_INVALID_ARG;
+  s->model = m; s->depth = depth; s->flags = flags;
+  s->slot.resize(depth);
+  for (int i = 0; i < depth; ++i) {
+    int rc = pnn_workspace_create(m, max_atoms, max_edges, max_structs, (flags & PNN_FORCES) ? PNN_WS_FORCES : 0,
+                                  &s->slot[i].ws);
+    if (rc == PNN_OK && !cuda_ok(cudaStreamCreateWithFlags(&s->slot[i].st, cudaStreamNonBlocking), "cudaStreamCreate"))
+      rc = PNN_ERR_CUDA;
+    if (rc == PNN_OK && !cuda_ok(cudaMallocHost((void**)&s->slot[i].err_host, 16), "cudaMallocHost")) rc = PNN_ERR_CUDA;
+    if (rc != PNN_OK) { pnn_stream_destroy(s); return rc; }
+  }
+  *out = s;
+  return PNN_OK;
+}
+
+void pnn_stream_destroy(pnn_stream* s) {
+  if (!s) return;
+  for (auto& sl : s->slot) {
+    if (sl.st) { cudaStreamSynchronize(sl.st); cudaStreamDestroy(sl.st); }
+    if (sl.err_host) cudaFreeHost(sl.err_host);
+    pnn_workspace_destroy(sl.ws);
+  }
+  delete s;
+}
+
+static int stream_finish_slot(pnn_stream* s, int i) {
+  pnn_stream::Slot& sl = s->slot[i];
+  PNN_TRY(cudaStreamSynchronize(sl.st));
+  sl.busy = false;
+  ++s->waited;
+  const int f0 = sl.err_host[0], f1 = sl.err_host[1];
+  if ((f0 | f1) & (ERRF_EDGE_OVERFLOW | ERRF_BAD_Z | ERRF_BAD_HEAD | ERRF_STALE_GRAPH)) {
+    PNN_TRY(cudaMemsetAsync(sl.ws->g.d_err, 0, 4, sl.st));
+    if ((f0 | f1) & ERRF_EDGE_OVERFLOW) { sl.ws->graph_N = sl.ws->graph_S = -1; return PNN_ERR_CAPACITY; }
+    return PNN_ERR_BAD_INPUT;
+  }
+  return PNN_OK;
+}
+
+int pnn_stream_submit(pnn_stream* s, int64_t N, int64_t S, const int32_t* Z, const double* pos, const int32_t* sptr,
+                      const int32_t* head, const double* cell, const uint8_t* pbc, void* energy_host, void* forces_host) {
+  if (!s) return PNN_ERR_INVALID_ARG;
+  const int i = (int)(s->submitted % s->depth);
+  pnn_stream::Slot& sl = s->slot[i];
+  if (sl.busy) { // the slot's previous batch must have left the device before its staging buffers are rewritten
+    const int rc = stream_finish_slot(s, i);
+    if (rc != PNN_OK) return rc;
+  }
+  const int rc = enqueue_host_batch(s->model, sl.ws, N, S, Z, pos, sptr, head, cell, pbc, s->flags, energy_host,
+                                    forces_host, sl.st);
+  if (rc != PNN_OK) return rc;
+  PNN_TRY(cudaMemcpyAsync(sl.err_host, sl.ws->g.d_err, 8, cudaMemcpyDeviceToHost, sl.st));
+  sl.busy = true;
+  ++s->submitted;
+  return PNN_OK;
+}
+
+int pnn_stream_wait(pnn_stream* s) {
+  if (!s) return PNN_ERR_INVALID_ARG;
+  if (s->waited >= s->submitted) return PNN_OK;
+  const int i = (int)(s->waited % s->depth);
+  if (!s->slot[i].busy) return PNN_ERR_INVALID_ARG; // cannot happen: batches leave their slots in submission order
+  return stream_finish_slot(s, i);
+}
+
+int pnn_stream_drain(pnn_stream* s) {
+  if (!s) return PNN_ERR_INVALID_ARG;
+  int first = PNN_OK;
+  while (s->waited < s->submitted) {
+    const int rc = pnn_stream_wait(s);
+    if (rc != PNN_OK && first == PNN_OK) first = rc;
+  }
+  return first;
+}
+
+int64_t pnn_stream_launch_count(const pnn_stream* s) {
+  int64_t n = 0;
+  if (s) for (auto& sl : s->slot) n += sl.ws ? sl.ws->launches : 0;
+  return n;
+}
+int64_t pnn_stream_bytes(const pnn_stream* s) {
+  int64_t n = 0;
+  if (s) for (auto& sl : s->slot) n += sl.ws ? sl.ws->arena_bytes : 0;
+  return n;
 }
 
 int pnn_gemm_bf16(int64_t M, int32_t N, int32_t K, const void* A, int64_t lda, const void* Wt, int64_t ldw,
