@@ -1,10 +1,15 @@
 #!/usr/bin/env python
 """bench.py — PaiNN energy+force throughput of the B200 path (BASELINE.json metric) on synthetic input.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2|cfg3_fp32|cfg4|cfg5|...] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2|cfg3_fp32|cfg3_bf16|cfg4|cfg5|...]
+                  [--impl reference] [--only-headline]
 
-One step = one pass of the whole hot path (graph build + forward + analytic adjoint) over
-one batch.  Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every definition used here.
+One step = one pass of the whole hot path (graph build + forward + analytic adjoint) over one batch.
+Prints ONE JSON line (rank 0): the headline workload's contract keys plus `workloads`, one full record (>= 20 timed
+steps, median of per-step CUDA-event times, clocks, per-kernel-family times, roofline of the dominant kernel family,
+whole-step fraction of the SURVEY.md §8(d) roof, end-to-end leg) for each of BASELINE.json's configs: cfg2 FP32,
+cfg3 FP32, cfg3 BF16, cfg4 BF16 (one resident batch, and the WHOLE 64-batch stream from pinned host memory through the
+streaming driver), cfg5 FP64.  See DESIGN.md "Measurement" for every definition used here.
 """
 from __future__ import annotations
 
@@ -40,11 +45,13 @@ WORKLOAD_NAMES = {"cfg1": "cfg1_tiny_fp64", "cfg2": "cfg2_molecular_fp32", "cfg2
                   "cfg3_fp32": "cfg3_crystals_fp32", "cfg3_bf16": "cfg3_crystals_bf16",
                   "cfg4": "cfg4_screening_bf16_batch16384", "cfg4_fp32": "cfg4_screening_fp32_batch16384",
                   "cfg5": "cfg5_large_fp64"}
+FULL_RECORDS = ("cfg2", "cfg3_fp32", "cfg3_bf16", "cfg4", "cfg5")   # BASELINE.json configs[1..4] (cfg3 in both precisions)
+CFG4_STREAM_BATCHES = 64                                            # 1,048,576 structures / 16,384
 DTYPE = {"fp64": "f64", "fp32": "f32", "bf16": "bf16"}
 # plain-ALU peaks derived from the guide's unit counts and clocks:
 # 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz; FP64 at half the FP32 lane count.
-ALU_PEAK_TFLOPS = {"fp32": 148 * 128 * 2 * 1.965e9 / 1e12, "fp64": 148 * 64 * 2 * 1.965e9 / 1e12,
-                   "bf16": 148 * 128 * 2 * 1.965e9 / 1e12}
+ALU_PEAK_TFLOPS = {"fp32": 148 * 128 * 2 * 1.965e9 / 1e12, "fp64": 148 * 64 * 2 * 1.965e9 / 1e12}
+TRAFFIC_FILE = os.path.join("profiles", "r02_traffic.csv")
 
 
 def measured_peaks():
@@ -101,36 +108,26 @@ class ClockSampler:
         return out
 
 
-def algorithmic_work(family: str, N: int, E: int, mc: gen.ModelCfg, prec: str, forces: bool):
-    """(flops, bytes) per LAUNCH of one kernel family (per-atom and per-edge figures)."""
+# ------------------------------------------------------------------------------------------------ algorithmic work
+def edge_work(family: str, N: int, E: int, mc: gen.ModelCfg, prec: str):
+    """(flops, bytes) per LAUNCH of an edge kernel: what the METHOD requires (:461-469), not what the
+    implementation chose to move.  flops: a4 6KF + 16F per edge, a7 12KF + 60F (filter value and derivative, the
+    transposed contraction, the adjoint products); bytes: a4 N 11 F b + 20 E, a7 N 16 F b + 20 E (FP32 / FP64: b = 4 / 8);
+    BF16 model (reading Q19: BF16 gathered payloads, FP32 residual and adjoint streams): a4 N 52 F + 20 E, a7 N 50 F + 20 E.
+    The FP32 edge tape (24 F bytes per edge written by a4, read by a7) is NOT algorithmic: it appears in `traffic`."""
     F, K = mc.F, mc.K
-    b = 8 if prec == "fp64" else 4
-    eb = 4 + 4 * b                                    # col + (ux,uy,uz,d)
+    fl = E * (6 * K * F + 16 * F) if family == "edge_fwd" else E * (12 * K * F + 60 * F)
     if prec == "bf16":
-        # BF16 model: phi, v gathered as BF16 copies (read once from HBM), FP32 residual rows read and written,
-        # BF16 copies of the outputs written for the following GEMMs; 20 B per edge (sender index + geometry)
-        if family == "edge_fwd":   # read phi16 6F, v16 6F, s 4F, v 12F; write s' 4F, v' 12F, s'16 2F, v'16 6F
-            return E * (6 * K * F + 16 * F), N * 52 * F + E * 20
-        if family == "edge_bwd":   # read phi16 6F, v16 6F, sb16 2F, vb16 6F, vb 12F; write phib16 6F, vb_in 12F
-            return E * (12 * K * F + 60 * F), N * 50 * F + E * 20
-        return None, None
-    if prec == "fp32" and forces:
-        # FP32 model with forces: the forward kernel also evaluates dw/dd and writes the edge tape (w, dw/dd: 24 F bytes
-        # per edge); the reverse kernel reads the tape and does no filter arithmetic
-        if family == "edge_fwd":
-            return E * (12 * K * F + 16 * F), N * 11 * F * b + E * (eb + 24 * F)
-        if family == "edge_bwd":
-            return E * 60 * F, N * 16 * F * b + E * (eb + 24 * F)
-    if family == "edge_fwd":
-        return E * (6 * K * F + 16 * F), N * 11 * F * b + E * eb
-    if family == "edge_bwd":
-        return E * (12 * K * F + 60 * F), N * 16 * F * b + E * eb
-    return None, None
+        by = N * (52 if family == "edge_fwd" else 50) * F + 20 * E
+    else:
+        b = 8 if prec == "fp64" else 4
+        by = N * (11 if family == "edge_fwd" else 16) * F * b + (4 + 4 * b) * E
+    return float(fl), float(by)
 
 
 def gemm_work(family: str, N: int, mc: gen.ModelCfg, prec: str, forces: bool):
-    """(flops, bytes) per launch, averaged over the launches of one GEMM family in a step: 2 M N K flop; operands and
-    result once (the SiLU GEMMs' stored pre-activation and the accumulating ones' read of C are not counted)."""
+    """(flops, bytes, launches) per launch, averaged over the launches of one GEMM family in a step: 2 M N K flop; operands
+    and result once (the SiLU GEMMs' stored pre-activation and the accumulating ones' read of C are not counted)."""
     F, T = mc.F, mc.T
     eb = 8 if prec == "fp64" else (2 if prec == "bf16" else 4)
     if family == "gemm_N":
@@ -146,17 +143,68 @@ def gemm_work(family: str, N: int, mc: gen.ModelCfg, prec: str, forces: bool):
     return fl / len(shapes), by / len(shapes), len(shapes)
 
 
+def step_roof(N: int, E: int, mc: gen.ModelCfg, prec: str, forces: bool, peaks, alu_peak_tflops):
+    """SURVEY.md §8(d) whole-step roof (the table at :474-480): forward flops T (30 F^2 N + (6KF + 16F) E) + (F^2 + F) N and
+    compulsory bytes T (23 F b N + 20 E), x3 for energy + forces; t_roof = max over the applicable roofs (HBM; plain ALU
+    for FP32 / FP64; BF16 tensor pipe for the BF16 model)."""
+    F, T, K = mc.F, mc.T, mc.K
+    b = {"fp64": 8, "fp32": 4, "bf16": 2}[prec]
+    mult = 3 if forces else 1
+    flops = mult * (T * (30.0 * F * F * N + (6 * K * F + 16 * F) * E) + (F * F + F) * N)
+    byts = mult * T * (23.0 * F * b * N + 20.0 * E)
+    gather = mult * T * 6.0 * F * b * E
+    t_hbm = byts / (peaks["hbm"] * 1e9)
+    if prec == "bf16":
+        t_c, cname, cpeak = flops / (peaks["bf16_sust"] * 1e12), "tensor", peaks["bf16_sust"]
+    else:
+        t_c, cname, cpeak = flops / (alu_peak_tflops * 1e12), "alu", alu_peak_tflops
+    binds = "hbm" if t_hbm >= t_c else cname
+    return dict(flops=flops, compulsory_bytes=byts, gather_bytes=gather, t_hbm_ms=1e3 * t_hbm, t_compute_ms=1e3 * t_c,
+                compute_roof=cname, compute_peak_tflops=cpeak, t_roof_ms=1e3 * max(t_hbm, t_c), binds=binds,
+                t_hbm_if_all_gathers_miss_ms=1e3 * (byts + gather) / (peaks["hbm"] * 1e9))
+
+
 def measured_traffic(workload: str, family: str):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/r01_traffic.csv), or None."""
+    """(DRAM bytes per launch of a kernel family, source) from the committed ncu capture, or (None, None).  The number is
+    a constant of that capture, not measured in this run: `traffic_source` says so."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r01_traffic.csv")) as fh:
+        with open(os.path.join(ROOT, TRAFFIC_FILE)) as fh:
             for line in fh:
                 q = line.strip().split(",")
-                if len(q) >= 3 and q[0] == workload and q[1] == family:
-                    return int(q[2])
+                if len(q) >= 4 and q[0] == workload and q[1] == family:
+                    return int(q[2]), f"{TRAFFIC_FILE}: ncu --set full capture of {q[3]} (dram__bytes_read.sum + dram__bytes_write.sum, constant, not measured in this run)"
     except Exception:
         pass
-    return None
+    return None, None
+
+
+def family_roofline(fam: str, per_s: float, N: int, E: int, mc, prec: str, forces: bool, peaks, wname: str,
+                    alu_meas):
+    if fam.startswith("gemm_"):
+        flops, byts, _ = gemm_work(fam, N, mc, prec, forces)
+    else:
+        flops, byts = edge_work(fam, N, E, mc, prec)
+    traffic, tsrc = measured_traffic(wname, fam)
+    if prec in ("fp32", "fp64"):
+        ach, peak = flops / per_s / 1e12, ALU_PEAK_TFLOPS[prec]
+        r = dict(kernel=fam, bound="alu", achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak, traffic=traffic,
+                 traffic_source=tsrc, peak_source="derived: 148 SMs x lanes x 2 x 1.965 GHz (DESIGN.md)",
+                 algorithmic_flops=flops, algorithmic_bytes=byts, hbm_achieved_gbs=byts / per_s / 1e9,
+                 hbm_frac=byts / per_s / 1e9 / peaks["hbm"], hbm_peak_gbs=peaks["hbm"], hbm_peak_source=peaks["source"])
+        if alu_meas:
+            r["alu_peak_measured"] = alu_meas
+            r["frac_of_measured_peak"] = ach / alu_meas
+        return r
+    if fam.startswith("gemm_"):
+        ach = flops / per_s / 1e12
+        return dict(kernel=fam, bound="tensor", achieved=ach, peak=peaks["bf16_sust"], unit="TFLOP/s",
+                    frac=ach / peaks["bf16_sust"], traffic=traffic, traffic_source=tsrc,
+                    peak_source=peaks["source"] + " (sustained bf16)", algorithmic_flops=flops, algorithmic_bytes=byts,
+                    hbm_achieved_gbs=byts / per_s / 1e9, hbm_frac=byts / per_s / 1e9 / peaks["hbm"])
+    ach = byts / per_s / 1e9
+    return dict(kernel=fam, bound="hbm", achieved=ach, peak=peaks["hbm"], unit="GB/s", frac=ach / peaks["hbm"],
+                traffic=traffic, traffic_source=tsrc, peak_source=peaks["source"], algorithmic_bytes=byts,
+                tensor_flops=flops)
 
 
 def run_reference(args, rank):
@@ -208,7 +256,9 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="cfg2", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-extra", action="store_true", help="skip the context timings of the other configs")
+    ap.add_argument("--no-extra", "--only-headline", dest="no_extra", action="store_true",
+                    help="only the headline workload (skip the per-config records of the other configs)")
+    ap.add_argument("--stream-batches", type=int, default=CFG4_STREAM_BATCHES)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
     rank = int(os.environ.get("RANK", "0"))
@@ -227,6 +277,12 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     peaks = measured_peaks()
+    alu_meas = {}
+    for pr, code in (("fp32", pnn.PNN_FP32), ("fp64", pnn.PNN_FP64)):
+        try:   # the nominal ALU peak is also measured on the box (FMA micro-benchmark)
+            alu_meas[pr] = pnn.pnn_measure_alu_peak(code)
+        except Exception:
+            alu_meas[pr] = None
 
     def run_workload(name: str, steps: int, warmup: int, full: bool):
         cfg_id, prec, forces, per_step = WORKLOADS[name]
@@ -236,12 +292,23 @@ def main():
         # weak scaling: rank r evaluates its own structures [r*S, (r+1)*S) of the same recipe
         b = gen.make_batch(cfg_id, rank * S, S)
         w = gen.make_weights(mc, cfg_id)
-        deg_cap = 96 if cfg_id in (3, 5) else 40
-        net = pnn.PaiNN(mc.F, mc.T, mc.K, mc.H, w, precision=prec, cutoff=mc.cutoff, Zmax=mc.Zmax,
-                        norm_eps=mc.norm_eps, max_atoms=b.n_atoms, max_edges=b.n_atoms * deg_cap,
-                        max_structs=b.n_structs, forces=forces)
         tt = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev)
         d = dict(Z=tt(b.Z), pos=tt(b.pos), sp=tt(b.struct_ptr), head=tt(b.head), cell=tt(b.cell), pbc=tt(b.pbc))
+        # the workspace is sized from the batch's real edge count (a cheap graph-only pass with a generous bound), so that
+        # the FP32 edge tape is as large as the workload needs and no larger
+        deg_cap = 96 if cfg_id in (3, 5) else 40
+        probe = pnn.PaiNN(mc.F, mc.T, mc.K, mc.H, w, precision=prec, cutoff=mc.cutoff, Zmax=mc.Zmax,
+                          norm_eps=mc.norm_eps, max_atoms=b.n_atoms, max_edges=b.n_atoms * deg_cap,
+                          max_structs=b.n_structs, forces=False)
+        probe.build_graph(d["pos"], d["sp"], d["cell"], d["pbc"])
+        _, _, _, E = pnn.pnn_graph_view(probe.ws)
+        probe.close()
+        del probe
+        torch.cuda.empty_cache()
+        max_edges = int(E * 1.02) + 1024
+        net = pnn.PaiNN(mc.F, mc.T, mc.K, mc.H, w, precision=prec, cutoff=mc.cutoff, Zmax=mc.Zmax,
+                        norm_eps=mc.norm_eps, max_atoms=b.n_atoms, max_edges=max_edges,
+                        max_structs=b.n_structs, forces=forces)
         flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)  # 256 MB > 126 MB L2
         st = torch.cuda.current_stream()
 
@@ -262,7 +329,6 @@ def main():
             e, f = step()
         torch.cuda.synchronize()
         net.check()
-        _, _, _, E = pnn.pnn_graph_view(net.ws)
         # ---- device-resident timing: L2 flushed (untimed) before every step, CUDA events on the launch stream
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
         sampler = ClockSampler(local_rank)
@@ -283,19 +349,20 @@ def main():
             dist.barrier()
         t_wall = time.perf_counter() - t_wall0
         launches = net.launches - l0
-        clocks = sampler.stop() if full else None
-        ms = sum(a.elapsed_time(z) for a, z in ev)
-        tmax = torch.tensor([ms], dtype=torch.float64, device=dev)
+        per_step_ms = [a.elapsed_time(z) for a, z in ev]
+        ms = sum(per_step_ms)
+        tmax = torch.tensor([ms, float(np.median(per_step_ms))], dtype=torch.float64, device=dev)
         tot = torch.tensor([float(b.n_structs), float(E), float(b.n_atoms)], dtype=torch.float64, device=dev)
         if world > 1:
             dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
             dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-        ms = float(tmax.item())
+        ms, med = float(tmax[0].item()), float(tmax[1].item())
         S_tot, E_tot, N_tot = (float(x) for x in tot.tolist())
         res = dict(name=name, prec=prec, forces=forces, mc=mc, batch=b, n_structs=S_tot, n_edges=E_tot, n_atoms=N_tot,
-                   ms_per_step=ms / steps, structures_per_s=S_tot * steps / (ms * 1e-3),
-                   edges_per_s=E_tot * steps / (ms * 1e-3), launches=launches, clocks=clocks, wall_s=t_wall,
-                   ws_bytes=pnn.pnn_workspace_bytes(net.ws))
+                   ms_per_step=ms / steps, ms_per_step_median=med, ms_per_step_min=min(per_step_ms), steps=steps,
+                   structures_per_s=S_tot * steps / (ms * 1e-3), edges_per_s=E_tot * steps / (ms * 1e-3),
+                   launches=launches, wall_s=t_wall, ws_bytes=pnn.pnn_workspace_bytes(net.ws),
+                   tape_bytes=pnn.pnn_workspace_edge_tape_bytes(net.ws))
         if full:
             # ---- end to end through the host entry point: pinned host buffers, H2D + D2H inside the timed region
             pin = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -320,6 +387,7 @@ def main():
                 step_host()
                 z.record(st)
             torch.cuda.synchronize()
+            res["clocks"] = sampler.stop()
             ms2 = torch.tensor([sum(a.elapsed_time(z) for a, z in ev2)], dtype=torch.float64, device=dev)
             if world > 1:
                 dist.all_reduce(ms2, op=dist.ReduceOp.MAX)
@@ -327,7 +395,8 @@ def main():
             d2h = sum(x.numel() * x.element_size() for x in (eo, fo) if x is not None)
             res["e2e"] = dict(value=S_tot * steps / (float(ms2.item()) * 1e-3), unit="structures/s",
                               h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
-                              ms_per_step=float(ms2.item()) / steps)
+                              ms_per_step=float(ms2.item()) / steps,
+                              api="pnn_eval_host (pinned host buffers; H2D, graph build, evaluation, D2H, synchronise)")
             # ---- per-kernel-family CUDA-event timing (separate pass: the event pairs would perturb the step time)
             pnn.pnn_profile_enable(net.ws, True)
             for _ in range(steps):
@@ -336,73 +405,112 @@ def main():
             prof = pnn.pnn_profile_read(net.ws)
             pnn.pnn_profile_enable(net.ws, False)
             res["profile"] = prof
-        net.close()
+        res["net"] = net
         del flush
-        torch.cuda.empty_cache()
         return res
 
+    def cfg4_stream(res, n_batches: int):
+        """The WHOLE cfg4 stream (BASELINE.json configs[3]: 1,048,576 molecules in 64 batches of 16,384) from pinned host
+        memory through the double-buffered streaming driver: host wall clock around submit ... drain."""
+        net, mc = res["net"], res["mc"]
+        S = 16384
+        t_gen = time.perf_counter()
+        try:
+            import multiprocessing as mp
+            with mp.get_context("spawn").Pool(min(16, os.cpu_count() or 1, n_batches)) as pool:
+                batches = pool.starmap(gen.make_batch, [(4, k * S, S) for k in range(n_batches)])
+        except Exception:
+            batches = [gen.make_batch(4, k * S, S) for k in range(n_batches)]
+        t_gen = time.perf_counter() - t_gen
+        maxN = max(b.n_atoms for b in batches)
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        hin = [(pin(b.Z), pin(b.pos), pin(b.struct_ptr), pin(b.head)) for b in batches]
+        eo = [torch.empty(S, dtype=torch.float32).pin_memory() for _ in batches]
+        sh = pnn.pnn_stream_create(net.model, maxN, int(maxN * 12.5), S, pnn.PNN_ENERGY, 2)
+        try:
+            def run(n):
+                for k in range(n):
+                    z, p, sp, h = hin[k]
+                    pnn.pnn_stream_submit(sh, batches[k].n_atoms, S, z.numpy(), p.numpy(), sp.numpy(), h.numpy(), None,
+                                          None, eo[k].numpy())
+                pnn.pnn_stream_drain(sh)
+            run(min(3, n_batches))                       # warm-up
+            torch.cuda.synchronize()
+            l0 = pnn.pnn_stream_launch_count(sh)
+            t0 = time.perf_counter()
+            run(n_batches)
+            dt = time.perf_counter() - t0
+            launches = pnn.pnn_stream_launch_count(sh) - l0
+        finally:
+            pnn.pnn_stream_destroy(sh)
+        n_struct = S * n_batches
+        h2d = sum(x.numel() * x.element_size() for hb in hin for x in hb)
+        assert all(np.isfinite(e.numpy()).all() for e in eo)
+        return dict(api="pnn_stream_submit / pnn_stream_drain (depth 2: two workspaces, two CUDA streams, pinned host buffers)",
+                    batches=n_batches, structures=n_struct, atoms=int(sum(b.n_atoms for b in batches)), seconds=dt,
+                    structures_per_s=n_struct / dt, ms_per_batch=1e3 * dt / n_batches,
+                    resident_ms_per_batch=res["ms_per_step_median"],
+                    ratio_to_resident_batches=(1e3 * dt / n_batches) / res["ms_per_step_median"],
+                    h2d_bytes=h2d, d2h_bytes=4 * n_struct, gpu_launches=int(launches), input_generation_s=t_gen,
+                    timing="host wall clock around submit ... drain after a device synchronise")
+
+    def record(name: str, res) -> dict:
+        """The full per-config record (the headline's contract keys are derived from the same dict)."""
+        mc, prec, forces = res["mc"], res["prec"], res["forces"]
+        N, E = int(res["n_atoms"] / world), int(res["n_edges"] / world)
+        wname = WORKLOAD_NAMES[name]
+        kernels, tot_ms = {}, sum(v[0] for v in res["profile"].values())
+        for fam, (ms, nl) in sorted(res["profile"].items(), key=lambda kv: -kv[1][0]):
+            kernels[fam] = dict(launches_per_step=nl / res["steps"], ms_per_launch=ms / max(nl, 1), share=ms / tot_ms)
+        cand = [f for f in kernels if f.startswith("edge_") or f.startswith("gemm_")]
+        roof, per_kernel = None, {}
+        for fam in cand:
+            per_kernel[fam] = family_roofline(fam, kernels[fam]["ms_per_launch"] * 1e-3, N, E, mc, prec, forces, peaks,
+                                              wname, alu_meas.get(prec))
+            per_kernel[fam]["share_of_step"] = kernels[fam]["share"]
+        if cand:
+            roof = per_kernel[max(cand, key=lambda f: kernels[f]["share"])]   # the dominant kernel family of the step
+        sr = step_roof(N, E, mc, prec, forces, peaks, ALU_PEAK_TFLOPS.get(prec, 0.0))
+        sr["frac"] = sr["t_roof_ms"] / res["ms_per_step_median"]
+        out = dict(workload=wname, dtype=DTYPE[prec], outputs="energy+forces" if forces else "energy",
+                   structures_per_step=int(res["n_structs"]), atoms_per_step=int(res["n_atoms"]),
+                   directed_edges_per_step=int(res["n_edges"]), mean_degree=res["n_edges"] / max(res["n_atoms"], 1),
+                   F=mc.F, T=mc.T, K=mc.K, H=mc.H, cutoff=mc.cutoff, steps=res["steps"],
+                   ms_per_step=res["ms_per_step_median"], ms_per_step_mean=res["ms_per_step"],
+                   ms_per_step_min=res["ms_per_step_min"], timing="median of per-step CUDA-event times, L2 flushed",
+                   structures_per_s=res["n_structs"] / (res["ms_per_step_median"] * 1e-3),
+                   edges_per_s=res["n_edges"] / (res["ms_per_step_median"] * 1e-3), clocks=res.get("clocks"),
+                   e2e=res.get("e2e"), gpu_launches_per_step=res["launches"] / res["steps"], roofline=roof,
+                   roofline_per_kernel=per_kernel, step_roofline=sr, kernels=kernels,
+                   workspace_bytes=res["ws_bytes"], edge_tape_bytes=res["tape_bytes"])
+        return out
+
+    def close(res):
+        res["net"].close()
+        res.pop("net")
+        torch.cuda.empty_cache()
+
     main_res = run_workload(args.workload, args.steps, args.warmup, full=True)
+    main_rec = record(args.workload, main_res)
+    if args.workload == "cfg4" and world == 1 and not args.no_extra:
+        main_rec["stream"] = cfg4_stream(main_res, args.stream_batches)
+    close(main_res)
     mc, prec = main_res["mc"], main_res["prec"]
-    N, E = int(main_res["n_atoms"] / world), int(main_res["n_edges"] / world)
 
-    # roofline of the dominant kernel family
-    kernels, tot_ms = {}, sum(v[0] for v in main_res["profile"].values())
-    for fam, (ms, nl) in sorted(main_res["profile"].items(), key=lambda kv: -kv[1][0]):
-        per = ms / max(nl, 1)
-        kernels[fam] = dict(launches_per_step=nl / args.steps, ms_per_launch=per, share=ms / tot_ms)
-    roof = None
-    cand = [f for f in kernels if f.startswith("edge_") or f.startswith("gemm_")]
-    if cand:
-        fam = max(cand, key=lambda f: kernels[f]["share"])      # the dominant kernel family of the step
-        per_s = kernels[fam]["ms_per_launch"] * 1e-3
-        if fam.startswith("gemm_"):
-            flops, byts, _ = gemm_work(fam, N, mc, prec, main_res["forces"])
-        else:
-            flops, byts = algorithmic_work(fam, N, E, mc, prec, main_res["forces"])
-        if prec in ("fp32", "fp64"):
-            ach, peak = flops / per_s / 1e12, ALU_PEAK_TFLOPS[prec]
-            roof = dict(kernel=fam, bound="alu", achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak,
-                        traffic=measured_traffic(WORKLOAD_NAMES[args.workload], fam),
-                        peak_source="derived: 148 SMs x lanes x 2 x 1.965 GHz (DESIGN.md)",
-                        hbm_achieved_gbs=byts / per_s / 1e9, hbm_peak_gbs=peaks["hbm"], hbm_peak_source=peaks["source"])
-            try:   # the nominal ALU peak is also measured on the box (FMA micro-benchmark)
-                roof["alu_peak_measured"] = pnn.pnn_measure_alu_peak(pnn.PNN_FP64 if prec == "fp64" else pnn.PNN_FP32)
-                roof["frac_of_measured_peak"] = ach / roof["alu_peak_measured"]
-            except Exception as ex:
-                roof["alu_peak_measured"] = None
-        elif fam.startswith("gemm_"):
-            ach = flops / per_s / 1e12
-            roof = dict(kernel=fam, bound="tensor", achieved=ach, peak=peaks["bf16_sust"], unit="TFLOP/s",
-                        frac=ach / peaks["bf16_sust"], traffic=measured_traffic(WORKLOAD_NAMES[args.workload], fam),
-                        peak_source=peaks["source"] + " (sustained bf16)", algorithmic_bytes=byts)
-        else:
-            ach = byts / per_s / 1e9
-            roof = dict(kernel=fam, bound="hbm", achieved=ach, peak=peaks["hbm"], unit="GB/s", frac=ach / peaks["hbm"],
-                        traffic=measured_traffic(WORKLOAD_NAMES[args.workload], fam), peak_source=peaks["source"],
-                        algorithmic_bytes=byts, tensor_flops=flops)
-        # the runner-up family, for context (the two are within a few percent of the step on cfg2)
-        others = sorted((f for f in cand if f != fam), key=lambda f: -kernels[f]["share"])
-        if others and prec in ("fp32", "fp64"):
-            f2 = others[0]
-            fl2 = gemm_work(f2, N, mc, prec, main_res["forces"])[0] if f2.startswith("gemm_") else \
-                algorithmic_work(f2, N, E, mc, prec, main_res["forces"])[0]
-            if fl2:
-                a2 = fl2 / (kernels[f2]["ms_per_launch"] * 1e-3) / 1e12
-                roof["runner_up"] = dict(kernel=f2, achieved=a2, frac=a2 / ALU_PEAK_TFLOPS[prec],
-                                         share_of_step=kernels[f2]["share"])
-        roof["share_of_step"] = kernels[fam]["share"]
-
-    line = dict(metric="painn_energy_force_structures_per_s", value=main_res["structures_per_s"], unit="structures/s",
-                n_gpus=world, steps=args.steps, warmup=args.warmup, ms_per_step=main_res["ms_per_step"],
+    line = dict(metric="painn_energy_force_structures_per_s", value=main_rec["structures_per_s"], unit="structures/s",
+                n_gpus=world, steps=args.steps, warmup=args.warmup, ms_per_step=main_rec["ms_per_step"],
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype=DTYPE[prec], data="synthetic",
-                config=dict(workload=WORKLOAD_NAMES[args.workload], structures_per_step=int(main_res["n_structs"]),
-                            atoms_per_step=int(main_res["n_atoms"]), directed_edges_per_step=int(main_res["n_edges"]),
-                            mean_degree=main_res["n_edges"] / max(main_res["n_atoms"], 1), F=mc.F, T=mc.T, K=mc.K,
-                            H=mc.H, cutoff=mc.cutoff, outputs="energy+forces" if main_res["forces"] else "energy",
-                            l2="flushed between timed steps (256 MB write)", parallelism=f"replica x{world}"),
-                edges_per_s=main_res["edges_per_s"], clocks=main_res["clocks"], e2e=main_res["e2e"],
-                gpu_launches=int(main_res["launches"]), roofline=roof, kernels=kernels,
-                workspace_bytes=main_res["ws_bytes"])
+                config=dict(workload=WORKLOAD_NAMES[args.workload], structures_per_step=main_rec["structures_per_step"],
+                            atoms_per_step=main_rec["atoms_per_step"],
+                            directed_edges_per_step=main_rec["directed_edges_per_step"],
+                            mean_degree=main_rec["mean_degree"], F=mc.F, T=mc.T, K=mc.K, H=mc.H, cutoff=mc.cutoff,
+                            outputs=main_rec["outputs"], l2="flushed between timed steps (256 MB write)",
+                            timing="median of the per-step CUDA-event times", parallelism=f"replica x{world}"),
+                edges_per_s=main_rec["edges_per_s"], clocks=main_rec["clocks"], e2e=main_rec["e2e"],
+                gpu_launches=int(main_res["launches"]), roofline=main_rec["roofline"],
+                roofline_per_kernel=main_rec["roofline_per_kernel"], step_roofline=main_rec["step_roofline"],
+                kernels=main_rec["kernels"], workspace_bytes=main_rec["workspace_bytes"],
+                edge_tape_bytes=main_rec["edge_tape_bytes"])
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
@@ -427,16 +535,34 @@ def main():
                                            f"FP64 oracle")
 
     if not args.no_extra and world == 1:
-        extra = {}
-        for name in ("cfg1", "cfg2_blended", "cfg3_fp32", "cfg3_bf16", "cfg4", "cfg5"):
+        # one full record per BASELINE.json config (per kernel per config the binding roof)
+        recs = {WORKLOAD_NAMES[args.workload]: main_rec}
+        for name in FULL_RECORDS:
             if name == args.workload:
                 continue
             try:
+                r = run_workload(name, 20, 3, full=True)
+                rec = record(name, r)
+                if name == "cfg4":
+                    try:
+                        rec["stream"] = cfg4_stream(r, args.stream_batches)
+                    except Exception as ex:
+                        rec["stream"] = dict(error=str(ex)[:300])
+                close(r)
+                recs[WORKLOAD_NAMES[name]] = rec
+            except Exception as ex:  # never fail the headline line
+                recs[WORKLOAD_NAMES[name]] = dict(error=str(ex)[:300])
+        line["workloads"] = recs
+        extra = {}
+        for name in ("cfg1", "cfg2_blended"):   # context only: short timings
+            try:
                 r = run_workload(name, 5, 3, full=False)
-                extra[WORKLOAD_NAMES[name]] = dict(ms_per_step=r["ms_per_step"], structures_per_s=r["structures_per_s"],
-                                                   edges_per_s=r["edges_per_s"], atoms=int(r["n_atoms"]),
-                                                   directed_edges=int(r["n_edges"]), launches_per_step=r["launches"] / 5)
-            except Exception as ex:  # context only: never fail the headline line
+                extra[WORKLOAD_NAMES[name]] = dict(ms_per_step=r["ms_per_step_median"],
+                                                   structures_per_s=r["n_structs"] / (r["ms_per_step_median"] * 1e-3),
+                                                   atoms=int(r["n_atoms"]), directed_edges=int(r["n_edges"]),
+                                                   launches_per_step=r["launches"] / 5)
+                close(r)
+            except Exception as ex:
                 extra[WORKLOAD_NAMES[name]] = dict(error=str(ex)[:200])
         line["other_workloads"] = extra
 

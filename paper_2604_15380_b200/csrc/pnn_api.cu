@@ -426,7 +426,10 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
     if (pass == 0) {
       ws->arena_bytes = off;
       if (!cuda_ok(cudaMalloc((void**)&ws->arena, off), "cudaMalloc(workspace)")) { delete ws; return PNN_ERR_CUDA; }
-      if (!cuda_ok(cudaMemset(ws->arena, 0, off), "cudaMemset(workspace)")) {
+      // (cudaMemset on device memory may return before it has run: wait for it, so that work on non-blocking streams —
+      // the streaming driver's — cannot overtake the zero fill)
+      if (!cuda_ok(cudaMemset(ws->arena, 0, off), "cudaMemset(workspace)") ||
+          !cuda_ok(cudaDeviceSynchronize(), "cudaMemset(workspace)")) {
         cudaFree(ws->arena); delete ws; return PNN_ERR_CUDA;
       }
     }
