@@ -132,3 +132,36 @@ def test_cfg5_full_size_fp64_properties():
             assert abs(fd - F0[a, c]) < 1e-5 * np.abs(F0).max(), (a, c, fd, F0[a, c])
     finally:
         net.close()
+
+
+def test_cfg5_full_size_fp64_against_the_oracle_golden():
+    """cfg5 at FULL size (100,000 atoms, 4.95 M edges, the launch configuration bench.py times) against the ORACLE:
+    tests/golden/cfg5_oracle.npz is written by tests/golden/make_cfg5_golden.py, which calls only gen/ and oracle/
+    (about 20 minutes of CPU).  Whole CSR rowptr (degrees) and edge count bit-exact, sender lists of the sampled atoms by
+    checksum, energy and the forces of 2,000 sampled atoms to BASELINE.json's 1e-10."""
+    import os
+    import torch
+    g = np.load(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg5_oracle.npz"))
+    mc = gen.model_cfg(5)
+    b = gen.make_batch(5)
+    w = gen.make_weights(mc, 5)
+    net = make_model(mc, w, "fp64", b.n_atoms, int(g["n_edges"]) + 1024, 1, True)
+    try:
+        t = to_device(b)
+        e, f = net.eval(t["Z"], t["pos"], t["struct_ptr"], t["head"], t["cell"], t["pbc"])
+        torch.cuda.synchronize()
+        net.check()
+        rowptr, col, _ = net.graph()
+        assert int(rowptr[-1]) == int(g["n_edges"])
+        assert np.array_equal(np.diff(rowptr), g["degree"].astype(np.int64))
+        ssum = np.array([col[rowptr[i]:rowptr[i + 1]].astype(np.int64).sum() for i in g["sample"]])
+        assert np.array_equal(ssum, g["sender_sum_sample"])
+        e, f = e.cpu().numpy(), f.cpu().numpy()
+        assert abs(e[0] - g["energy"][0]) < 1e-10 * abs(g["energy"][0])
+        err = np.abs(f[g["sample"]] - g["forces_sample"]).max() / float(g["force_rms"])
+        print("cfg5 full size: energy rel err %.2e, sampled force err / RMS force %.2e"
+              % (abs(e[0] - g["energy"][0]) / abs(g["energy"][0]), err))
+        assert err < 1e-10
+        assert np.abs(f.sum(0) - g["force_sum"]).max() < 1e-9 * float(g["force_rms"]) * np.sqrt(b.n_atoms)
+    finally:
+        net.close()
