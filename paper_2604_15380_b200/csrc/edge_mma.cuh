@@ -45,4 +45,11 @@ int launch_edge_fwd_tc(const EdgeMmaArgs& a, const __nv_bfloat16* fltT, const __
                        int64_t ld_sin, const __nv_bfloat16* v_in, const float* v_res, float* s1, int64_t ld_s1, float* v1,
                        const EdgeMirror& mir, cudaStream_t st);
 
+// edge_tc_bwd.cu — reverse message step on tcgen05 (same arguments as launch_edge_bwd_mma plus the filter image fltT);
+// adds the block's force contribution into fpart [edge_tc_bwd_num_slabs()][N][3].
+int launch_edge_bwd_tc(const EdgeMmaArgs& a, const __nv_bfloat16* fltT, const __nv_bfloat16* phi, const __nv_bfloat16* v_in,
+                       const __nv_bfloat16* sb16, const __nv_bfloat16* vb16, const float* vb1, __nv_bfloat16* phib16,
+                       float* vb_in, float* fpart, int first_block, cudaStream_t st);
+int edge_tc_bwd_num_slabs();
+
 } // namespace pnn

@@ -816,8 +816,8 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
       { ProfScope ps_(ws, st, "edge_bwd");
         em.fltP = m->d_fltP + (int64_t)t * m->fltP_stride;
-        const int l_ = launch_edge_bwd_mma(em, tp16.phi16, tp16.vin16, mb.sb16, mb.vb16, vb, t > 0 ? mb.phib16 : nullptr, vb2,
-                                           fpart, last ? 1 : 0, st);
+        const int l_ = launch_edge_bwd_tc(em, m->d_fltT + (int64_t)t * m->fltT_stride, tp16.phi16, tp16.vin16, mb.sb16,
+                                          mb.vb16, vb, t > 0 ? mb.phib16 : nullptr, vb2, fpart, last ? 1 : 0, st);
         nl += l_; ps_.done(l_); }
       if (t > 0) {
         TcEpi g4; g4.act = ACT_MUL_DSILU; g4.aux = (const T*)tp.hpre; g4.ldaux = F; g4.Cb = mb.hb16; g4.ldcb = F;
@@ -828,7 +828,7 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       }
     }
     { ProfScope ps_(ws, st, "force_assemble");
-      const int l_ = launch_force_assemble<T>(N, edge_mma_num_slabs(F), fpart, forces, st);
+      const int l_ = launch_force_assemble<T>(N, edge_tc_bwd_num_slabs(), fpart, forces, st);
       nl += l_; ps_.done(l_); }
   }
   ws->launches += nl;
