@@ -117,7 +117,7 @@ def _check(st: int, where: str):
 _NP_DTYPES = {"i32": np.int32, "f64": np.float64, "f32": np.float32, "u8": np.uint8, "i8": np.int8}
 
 
-def _ptr(x, dtype: Optional[str] = None, device: Optional[bool] = None) -> Optional[int]:
+def _ptr(x, dtype: Optional[str] = None, device: Optional[bool] = None, contiguous: bool = True) -> Optional[int]:
     """int / None pass through; numpy arrays give their host address; torch tensors their data_ptr().
     dtype ("i32", "f64", "f32", "u8", "i8", "bf16") and device (True: CUDA, False: host) are checked when given: the C ABI
     takes untyped pointers, so a wrong element type or a host pointer where a device one is expected would be misread."""
@@ -133,7 +133,7 @@ def _ptr(x, dtype: Optional[str] = None, device: Optional[bool] = None) -> Optio
         if device:
             raise TypeError("expected a CUDA tensor, got a host array")
         return x.ctypes.data
-    if not x.is_contiguous():
+    if contiguous and not x.is_contiguous():
         raise ValueError("tensor must be contiguous")
     if dtype is not None:
         import torch
@@ -321,8 +321,9 @@ def pnn_profile_read(ws: int, max_entries: int = 32) -> dict:
 
 def pnn_gemm_bf16(M: int, N: int, K: int, A, lda: int, Wt, ldw: int, bias=None, act: int = 0, C=None, ldc: int = 0,
                   Cb=None, ldcb: int = 0, stream=None) -> None:
-    _check(lib().pnn_gemm_bf16(M, N, K, _ptr(A), lda, _ptr(Wt), ldw, _ptr(bias), act, _ptr(C), ldc, _ptr(Cb), ldcb,
-                               stream), "pnn_gemm_bf16")
+    sp = lambda t, dt: _ptr(t, dt, True, contiguous=False)   # row strides are explicit arguments here
+    _check(lib().pnn_gemm_bf16(M, N, K, sp(A, "bf16"), lda, sp(Wt, "bf16"), ldw, sp(bias, "f32"), act, sp(C, "f32"), ldc,
+                               sp(Cb, "bf16"), ldcb, stream), "pnn_gemm_bf16")
 
 
 class PaiNN:

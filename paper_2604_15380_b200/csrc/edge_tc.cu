@@ -29,7 +29,7 @@
 #include <vector>
 
 #include "common.cuh"
-#include "edge_mma.cuh"
+#include "edge_tc.cuh"
 #include "tc_ptx.cuh"
 
 namespace pnn {
@@ -269,6 +269,9 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
     const float bes_A = sqrtf(2.0f / rc);
     const uint32_t row16 = (uint32_t)(3 * F / 8); // 16-byte units per row of phi / v_in
     constexpr uint32_t idesc = umma_idesc_bf16(128, NE);
+    // UMMA shared-memory descriptors (no swizzle, K-major): high word constant, low word = start address >> 4 | LBO field
+    const uint32_t d_hi = (uint32_t)(umma_desc_nosw(0, 128, KC * 128) >> 32);
+    const uint32_t a_lo0 = (uint32_t)umma_desc_nosw(base, 128, KC * 128);
     uint32_t n = 0; // tiles of this pipeline so far (both producers count all of them)
     for (int64_t a0 = (int64_t)c_lo + (int64_t)g * RA; a0 < c_hi; a0 += (int64_t)NGRP * RA) {
       const int64_t a1 = min(a0 + RA, (int64_t)c_hi);
@@ -345,14 +348,14 @@ edge_fwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
           const uint32_t buf = n & 1u;
           mbar_wait_backoff(tmem_empty(g, buf), ((n >> 1) & 1u) ^ 1u); // the epilogue has read tile n - 2 out of this buffer
           tc_fence_after();
-          const uint32_t bt_u = grp_u + slot * L::B_TILE;
+          const uint32_t b_lo0 = (uint32_t)umma_desc_nosw(grp_u + slot * L::B_TILE, 128, KC * 128);
+          const uint32_t tmem_t = tmem_base + (uint32_t)((g * 2 + buf) * NACC * NE);
 #pragma unroll
           for (int acc = 0; acc < NACC; ++acc)
 #pragma unroll
             for (int ks = 0; ks < KS; ++ks)
-              umma_bf16(tmem_base + (uint32_t)(((g * 2 + buf) * NACC + acc) * NE),
-                        umma_desc_nosw(base + acc * (128 * KP * 2) + ks * 256, 128, KC * 128),
-                        umma_desc_nosw(bt_u + ks * 256, 128, KC * 128), idesc, ks ? 1u : 0u);
+              umma_bf16_lohi(tmem_t + (uint32_t)(acc * NE), a_lo0 + (uint32_t)((acc * (128 * KP * 2) + ks * 256) >> 4), d_hi,
+                             b_lo0 + (uint32_t)((ks * 256) >> 4), d_hi, idesc, ks != 0);
           umma_commit(tmem_full(g, buf));
         }
         __syncwarp();
@@ -519,6 +522,8 @@ uint16_t to_bf16_host(double x) {
 
 } // namespace
 
+int edge_mma_kp(int K) { return (K + 1 + 15) / 16 * 16; }
+
 // Host-side packing of one block's filter as the resident A operand of edge_fwd_tc_k: 6 accumulator tiles
 // a = chunk*2 + parity of 128 rows x KP columns, row l = filter row of feature 2l + parity (zero for 2l + parity >= F),
 // column k < K: flt_W, k == K: flt_b, then zeros; stored in the UMMA no-swizzle K-major layout
@@ -549,7 +554,7 @@ int launch_edge_fwd_tc(const EdgeMmaArgs& a, const __nv_bfloat16* fltT, const __
   const int KP = edge_mma_kp(a.K);
   // One persistent CTA per SM takes a contiguous, edge-balanced range of atoms and cuts it into windows of RA atoms that
   // alternate between its pipelines: about 4 windows per pipeline, between 2 and 16 atoms each.
-  const int RA = (int)std::min<int64_t>(16, std::max<int64_t>(2, a.N / (148 * NGRP * 4)));
+  const int RA = (int)std::min<int64_t>(16, std::max<int64_t>(2, a.N / (148 * NGRP * 8)));
   const unsigned grid = (unsigned)std::min<int64_t>(148, (a.N + RA * NGRP - 1) / (RA * NGRP));
 #define PNN_LAUNCH2(KPV, HV, FTV)                                                                                    \
   {                                                                                                                  \

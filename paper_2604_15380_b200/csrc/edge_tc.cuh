@@ -1,5 +1,5 @@
-// edge_mma.cuh — edge kernels of the BF16 model with the filter contraction on the tensor cores (edge_tc.cu forward:
-// tcgen05; edge_mma.cu reverse: mma.sync).
+// edge_tc.cuh — edge kernels of the BF16 model with the filter contraction on the tcgen05 tensor cores (edge_tc.cu forward,
+// edge_tc_bwd.cu reverse).
 #pragma once
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -17,25 +17,10 @@ struct EdgeMmaArgs {
   const int32_t* rowptr;
   const int32_t* col;
   const Geom<float>* geom;
-  // Filter of one block packed for the MMA B operand, BF16: KP = edge_mma_kp(K) columns per row
-  // (k < K: flt_W[row][k]; k == K: flt_b[row]; then zeros), rows ordered [chunk c][32-feature slab s][n-tile nt][g]
-  // with feature f = s*32 + (g>>1)*8 + nt*2 + (g&1)  — the column permutation that gives every thread of the
-  // accumulator fragment 8 contiguous features.
-  const __nv_bfloat16* fltP;
   const int* d_err;
 };
 
-int edge_mma_kp(int K);
-void pack_filter_bf16(int F, int K, const double* fltW, const double* fltb, uint16_t* out);
-
-// Reverse message step (R3 + R4 partial).  phi / v_in: forward tape (BF16); sb16 [N,F], vb16 [N,3F]: BF16 copies of the
-// incoming adjoints s-bar', v-bar' (gathered and own rows); vb1: the FP32 v-bar' (residual of v-bar_in).  Writes
-// phib16 [N,3F] (BF16) and vb_in [N,3F] (FP32) when v_in != NULL (blocks t > 0; for t = 0 only forces are produced) and
-// adds the block's force contribution into fpart [edge_mma_num_slabs(F)][N][3].
-int launch_edge_bwd_mma(const EdgeMmaArgs& a, const __nv_bfloat16* phi, const __nv_bfloat16* v_in,
-                        const __nv_bfloat16* sb16, const __nv_bfloat16* vb16, const float* vb1, __nv_bfloat16* phib16,
-                        float* vb_in, float* fpart, int first_block, cudaStream_t st);
-int edge_mma_num_slabs(int F);
+int edge_mma_kp(int K); // columns of the MMA operands: K radial functions + 1 (flt_b), padded to a multiple of 16
 
 // edge_tc.cu — forward message step on tcgen05 (features on the TMEM lanes, 16 consecutive CSR edges per MMA tile).
 // fltT: one block's filter packed by pack_filter_tc (edge_tc_filter_elems(K) BF16 elements).

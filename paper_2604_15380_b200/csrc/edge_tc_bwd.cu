@@ -24,7 +24,7 @@
 #include <cstring>
 
 #include "common.cuh"
-#include "edge_mma.cuh"
+#include "edge_tc.cuh"
 #include "tc_ptx.cuh"
 
 namespace pnn {
@@ -110,6 +110,8 @@ __device__ __forceinline__ void tmem_wait2(float (&r)[2], bool do_wait) {
 __device__ __forceinline__ float2 add2(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
 __device__ __forceinline__ float2 splat(float x) { return make_float2(x, x); }
+
+struct Gath { uint32_t gp[ES][3], gs[ES], gb[ES][3], gv[ES][3]; }; // gathered words of one step
 
 template <int KP, bool HASV>
 struct BwdSmem {
@@ -200,6 +202,11 @@ edge_bwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
     const float bes_A = sqrtf(2.0f / rc);
     const uint32_t row16 = (uint32_t)(3 * F / 8), rows16 = (uint32_t)(F / 8);
     constexpr uint32_t idesc = umma_idesc_bf16(128, NE);
+    // UMMA shared-memory descriptors (no swizzle, K-major): high word constant, low word = start address >> 4 | LBO field
+    const uint32_t d_hi = (uint32_t)(umma_desc_nosw(0, 128, KC * 128) >> 32);
+    const uint32_t a_lo0 = (uint32_t)umma_desc_nosw(base, 128, KC * 128);
+    const uint32_t tmem_g = tmem_base + (uint32_t)(g * 2 * NACC * NE);
+    static_assert(BwdSmem<48, true>::TOTAL < (1 << 18), "descriptor start addresses are 18-bit");
     uint32_t n = 0;
     for (int64_t a0 = (int64_t)c_lo + (int64_t)g * RA; a0 < c_hi; a0 += (int64_t)NGRP * RA) {
       const int64_t a1 = min(a0 + RA, (int64_t)c_hi);
@@ -285,16 +292,16 @@ edge_bwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
           if (n >= 2) mbar_wait_backoff(tmem_empty(g), n & 1u);
           mbar_wait_backoff(tmem_empty(g), (n & 1u) ^ 1u);
           tc_fence_after();
-          const uint32_t bt_u = grp_u + slot * 2 * L::B_TILE;
+          const uint32_t b_lo0 = (uint32_t)umma_desc_nosw(grp_u + slot * 2 * L::B_TILE, 128, KC * 128);
 #pragma unroll
           for (int part = 0; part < 2; ++part) // W from G, D from G'
 #pragma unroll
             for (int acc = 0; acc < NACC; ++acc)
 #pragma unroll
               for (int ks = 0; ks < KS; ++ks)
-                umma_bf16(tmem_base + (uint32_t)((g * 2 * NACC + part * NACC + acc) * NE),
-                          umma_desc_nosw(base + acc * (128 * KP * 2) + ks * 256, 128, KC * 128),
-                          umma_desc_nosw(bt_u + part * L::B_TILE + ks * 256, 128, KC * 128), idesc, ks ? 1u : 0u);
+                umma_bf16_lohi(tmem_g + (uint32_t)((part * NACC + acc) * NE),
+                               a_lo0 + (uint32_t)((acc * (128 * KP * 2) + ks * 256) >> 4), d_hi,
+                               b_lo0 + (uint32_t)((part * L::B_TILE + ks * 256) >> 4), d_hi, idesc, ks != 0);
           umma_commit(tmem_full(g));
         }
         __syncwarp();
@@ -378,10 +385,31 @@ edge_bwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
         mbar_wait(meta_full(g, slot), (n / NSLOT) & 1u);
         mbar_wait(tmem_full(g), n & 1u);
         tc_fence_after();
-#pragma unroll 1
-        for (int si = 0; si < NSTEP; ++si) {
-          const uint2 inf = lds64(mt_u + (uint32_t)offsetof(TileMetaB, sinfo) + 8u * si);
-          if (inf.y == 0u) break; // the used steps of a tile are its first ones
+        // The gathers of step si + 1 are issued before the arithmetic of step si (two register sets, the loop is unrolled
+        // by two steps): with two epilogue warps per scheduler there is little else to hide their latency behind.
+        auto load_step = [&](int si, Gath& G) {
+          const uint32_t cb = (uint32_t)si * (ES * 4);
+          const uint2 oo = lds64(mt_u + (uint32_t)offsetof(TileMetaB, OFF) + cb);
+          const uint2 os = lds64(mt_u + (uint32_t)offsetof(TileMetaB, OFS) + cb);
+          const uint32_t offs[2] = {oo.x, oo.y}, ofss[2] = {os.x, os.y};
+#pragma unroll
+          for (int c = 0; c < ES; ++c) {
+            const char* pr = phi_f + (uint64_t)offs[c] * 16u;
+            G.gp[c][0] = ldg_nc32(pr); G.gp[c][1] = ldg_nc32(pr + 2 * F);
+            G.gs[c] = ldg_nc32(sb_f + (uint64_t)ofss[c] * 16u);
+            const char* br = vb_f + (uint64_t)offs[c] * 16u;
+            G.gb[c][0] = ldg_nc32(br); G.gb[c][1] = ldg_nc32(br + 2 * F); G.gb[c][2] = ldg_nc32(br + 4 * F);
+            if (HASV) {
+              G.gp[c][2] = ldg_nc32(pr + 4 * F);
+              const char* vr = vin_f + (uint64_t)offs[c] * 16u;
+              G.gv[c][0] = ldg_nc32(vr); G.gv[c][1] = ldg_nc32(vr + 2 * F); G.gv[c][2] = ldg_nc32(vr + 4 * F);
+            }
+          }
+        };
+        auto used = [&](int si) {
+          return si < NSTEP && lds64(mt_u + (uint32_t)offsetof(TileMetaB, sinfo) + 8u * si).y != 0u;
+        };
+        auto process = [&](int si, const Gath& G) {
           const uint32_t cb = (uint32_t)si * (ES * 4);
           float W[NACC][ES], D[NACC][ES];
 #pragma unroll
@@ -389,24 +417,7 @@ edge_bwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
             tmem_ld2_async(taddr + acc * NE + si * ES, W[acc]);
             tmem_ld2_async(taddr + (NACC + acc) * NE + si * ES, D[acc]);
           }
-          const uint2 oo = lds64(mt_u + (uint32_t)offsetof(TileMetaB, OFF) + cb);
-          const uint2 os = lds64(mt_u + (uint32_t)offsetof(TileMetaB, OFS) + cb);
-          const uint32_t offs[2] = {oo.x, oo.y}, ofss[2] = {os.x, os.y};
-          uint32_t gp[ES][3], gs[ES], gb[ES][3], gv[ES][3];
-#pragma unroll
-          for (int c = 0; c < ES; ++c) {
-            const char* pr = phi_f + (uint64_t)offs[c] * 16u;
-            gp[c][0] = ldg_nc32(pr); gp[c][1] = ldg_nc32(pr + 2 * F);
-            gs[c] = ldg_nc32(sb_f + (uint64_t)ofss[c] * 16u);
-            const char* br = vb_f + (uint64_t)offs[c] * 16u;
-            gb[c][0] = ldg_nc32(br); gb[c][1] = ldg_nc32(br + 2 * F); gb[c][2] = ldg_nc32(br + 4 * F);
-            if (HASV) {
-              gp[c][2] = ldg_nc32(pr + 4 * F);
-              const char* vr = vin_f + (uint64_t)offs[c] * 16u;
-              gv[c][0] = ldg_nc32(vr); gv[c][1] = ldg_nc32(vr + 2 * F); gv[c][2] = ldg_nc32(vr + 4 * F);
-            }
-          }
-          const int i = (int)inf.x;
+          const int i = (int)lds64(mt_u + (uint32_t)offsetof(TileMetaB, sinfo) + 8u * si).x;
           if (i != cur) { // receiver complete: write it and any edge-less atoms before the next one
             end_row(cur);
             for (int k = cur + 1; k < i; ++k) { begin_row(k); end_row(k); }
@@ -424,13 +435,13 @@ edge_bwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
             const float u0 = c ? ux.y : ux.x, u1 = c ? uy.y : uy.x, u2 = c ? uz.y : uz.x, invd = c ? idd.y : idd.x;
             // ---- ss
             const float2 wss = make_float2(W[0][c], W[1][c]), dss = make_float2(D[0][c], D[1][c]);
-            const float2 pj0 = bf2(gp[c][0]), sj = bf2(gs[c]);
+            const float2 pj0 = bf2(G.gp[c][0]), sj = bf2(G.gs[c]);
             A0 = __ffma2_rn(sj, wss, A0);
             float2 y = __fmul2_rn(__ffma2_rn(lsb, pj0, __fmul2_rn(sj, lph[0])), dss);
             // ---- vs
             const float2 wvs = make_float2(W[2][c], W[3][c]), dvs = make_float2(D[2][c], D[3][c]);
-            const float2 pj1 = bf2(gp[c][1]);
-            const float2 b0 = bf2(gb[c][0]), b1 = bf2(gb[c][1]), b2 = bf2(gb[c][2]);
+            const float2 pj1 = bf2(G.gp[c][1]);
+            const float2 b0 = bf2(G.gb[c][0]), b1 = bf2(G.gb[c][1]), b2 = bf2(G.gb[c][2]);
             const float2 tj = __ffma2_rn(b2, splat(u2), __ffma2_rn(b1, splat(u1), __fmul2_rn(b0, splat(u0))));
             const float2 ti = __ffma2_rn(lvb[2], splat(u2), __ffma2_rn(lvb[1], splat(u1), __fmul2_rn(lvb[0], splat(u0))));
             const float2 ntj = neg2(tj), nlph = neg2(lph[1]);
@@ -446,8 +457,8 @@ edge_bwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
             // ---- vv
             if (HASV) {
               const float2 wvv = make_float2(W[NACC - 2][c], W[NACC - 1][c]), dvv = make_float2(D[NACC - 2][c], D[NACC - 1][c]);
-              const float2 pj2 = bf2(gp[c][2]);
-              const float2 v0 = bf2(gv[c][0]), v1 = bf2(gv[c][1]), v2 = bf2(gv[c][2]);
+              const float2 pj2 = bf2(G.gp[c][2]);
+              const float2 v0 = bf2(G.gv[c][0]), v1 = bf2(G.gv[c][1]), v2 = bf2(G.gv[c][2]);
               A2[0] = __ffma2_rn(b0, wvv, A2[0]);
               A2[1] = __ffma2_rn(b1, wvv, A2[1]);
               A2[2] = __ffma2_rn(b2, wvv, A2[2]);
@@ -461,6 +472,19 @@ edge_bwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
             fpp[1] = __ffma2_rn(y, splat(u1), fpp[1]);
             fpp[2] = __ffma2_rn(y, splat(u2), fpp[2]);
           }
+        };
+        Gath Ga, Gb;
+        load_step(0, Ga); // (the first step of a tile is always used)
+#pragma unroll 1
+        for (int si = 0; si < NSTEP; si += 2) {
+          const bool u1 = used(si + 1);
+          if (u1) load_step(si + 1, Gb);
+          process(si, Ga);
+          if (!u1) break;
+          const bool u2 = used(si + 2);
+          if (u2) load_step(si + 2, Ga);
+          process(si + 1, Gb);
+          if (!u2) break;
         }
         tc_fence_before();
         __syncwarp();
@@ -487,7 +511,7 @@ int launch_edge_bwd_tc(const EdgeMmaArgs& a, const __nv_bfloat16* fltT, const __
                        float* vb_in, float* fpart, int first_block, cudaStream_t st) {
   if (a.N == 0) return 0;
   const int KP = edge_mma_kp(a.K);
-  const int RA = (int)std::min<int64_t>(16, std::max<int64_t>(2, a.N / (148 * NGRP * 4)));
+  const int RA = (int)std::min<int64_t>(16, std::max<int64_t>(2, a.N / (148 * NGRP * 8)));
   const unsigned grid = (unsigned)std::min<int64_t>(148, (a.N + RA * NGRP - 1) / (RA * NGRP));
 #define PNN_LAUNCH2(KPV, HV, FTV)                                                                                     \
   {                                                                                                                   \

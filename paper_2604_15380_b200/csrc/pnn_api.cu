@@ -10,7 +10,7 @@
 
 #include "../../include/pnn.h"
 #include "common.cuh"
-#include "edge_mma.cuh"
+#include "edge_tc.cuh"
 #include "gemm_tc.cuh"
 
 using namespace pnn;
@@ -85,8 +85,6 @@ struct pnn_model {
   std::vector<BlockW> blk;
   int64_t oW1t = 0, oW1 = 0, ob1 = 0, ow2 = 0, ob2 = 0; // heads: [H][F][Fh], [H][Fh][F], [H][Fh], [H][Fh], [H]
   __nv_bfloat16* d_wb = nullptr;                        // BF16 copy of d_w (same offsets): tcgen05 GEMM operands
-  __nv_bfloat16* d_fltP = nullptr;                      // BF16 model: per block, the filter packed for edge_mma.cu
-  int64_t fltP_stride = 0;                              // elements per block
   __nv_bfloat16* d_fltT = nullptr;                      // BF16 model: per block, the filter image of edge_tc.cu
   int64_t fltT_stride = 0;
 };
@@ -270,17 +268,7 @@ int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, 
     if (!cuda_ok(cudaDeviceSynchronize(), "bf16 weight conversion") || launch_failed()) {
       cudaFree(m->d_wb); cudaFree(m->d_w); delete m; return PNN_ERR_CUDA;
     }
-    // filters packed for the tensor-core edge kernels (edge_mma.cuh)
-    m->fltP_stride = 3 * F * edge_mma_kp(cfg->K);
-    std::vector<uint16_t> fp((size_t)cfg->T * m->fltP_stride);
-    {
-      const double* q = w + (int64_t)(cfg->Zmax + 1) * F;
-      const int64_t per_block = 11 * F * F + 3 * F * K + 11 * F;
-      for (int t = 0; t < cfg->T; ++t) {
-        const double* fW = q + t * per_block + (F * F + F + 3 * F * F + 3 * F);
-        pack_filter_bf16((int)F, (int)K, fW, fW + 3 * F * K, fp.data() + (size_t)t * m->fltP_stride);
-      }
-    }
+    // filter images of the tensor-core edge kernels (edge_tc.cuh)
     m->fltT_stride = edge_tc_filter_elems(cfg->K);
     std::vector<uint16_t> ft((size_t)cfg->T * m->fltT_stride);
     {
@@ -291,11 +279,9 @@ int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, 
         pack_filter_tc((int)F, (int)K, fW, fW + 3 * F * K, ft.data() + (size_t)t * m->fltT_stride);
       }
     }
-    if (!cuda_ok(cudaMalloc((void**)&m->d_fltP, fp.size() * 2), "cudaMalloc(packed filters)") ||
-        !cuda_ok(cudaMemcpy(m->d_fltP, fp.data(), fp.size() * 2, cudaMemcpyHostToDevice), "cudaMemcpy(packed filters)") ||
-        !cuda_ok(cudaMalloc((void**)&m->d_fltT, ft.size() * 2), "cudaMalloc(filter images)") ||
+    if (!cuda_ok(cudaMalloc((void**)&m->d_fltT, ft.size() * 2), "cudaMalloc(filter images)") ||
         !cuda_ok(cudaMemcpy(m->d_fltT, ft.data(), ft.size() * 2, cudaMemcpyHostToDevice), "cudaMemcpy(filter images)")) {
-      cudaFree(m->d_fltT); cudaFree(m->d_fltP); cudaFree(m->d_wb); cudaFree(m->d_w); delete m; return PNN_ERR_CUDA;
+      cudaFree(m->d_fltT); cudaFree(m->d_wb); cudaFree(m->d_w); delete m; return PNN_ERR_CUDA;
     }
   }
   *out = m;
@@ -305,7 +291,6 @@ int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, 
 void pnn_model_destroy(pnn_model* m) {
   if (!m) return;
   cudaFree(m->d_fltT);
-  cudaFree(m->d_fltP);
   cudaFree(m->d_wb);
   cudaFree(m->d_w);
   delete m;
@@ -755,7 +740,6 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
     { ProfScope ps_(ws, st, "edge_fwd");
       EdgeMirror mir; mir.s1 = mb.sn16; mir.ld_s1 = 2 * F; mir.v1 = mb.v1_16;
-      em.fltP = m->d_fltP + (int64_t)t * m->fltP_stride;
       const int l_ = launch_edge_fwd_tc(em, m->d_fltT + (int64_t)t * m->fltT_stride, tp16.phi16, s_cur, F, v_in16, v_in, sn,
                                         2 * F, v1, mir, st); // B3b
       nl += l_; ps_.done(l_); }
@@ -815,8 +799,7 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       tc("gemm_3N", 3 * N, F, 2 * F, mb.PQb16, 2 * F, b.UVt, g3);                  // v-bar' += U^T P-bar + V^T Q-bar
       ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
       { ProfScope ps_(ws, st, "edge_bwd");
-        em.fltP = m->d_fltP + (int64_t)t * m->fltP_stride;
-        const int l_ = launch_edge_bwd_tc(em, m->d_fltT + (int64_t)t * m->fltT_stride, tp16.phi16, tp16.vin16, mb.sb16,
+          const int l_ = launch_edge_bwd_tc(em, m->d_fltT + (int64_t)t * m->fltT_stride, tp16.phi16, tp16.vin16, mb.sb16,
                                           mb.vb16, vb, t > 0 ? mb.phib16 : nullptr, vb2, fpart, last ? 1 : 0, st);
         nl += l_; ps_.done(l_); }
       if (t > 0) {
