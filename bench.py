@@ -418,9 +418,9 @@ def main():
         try:
             import multiprocessing as mp
             with mp.get_context("spawn").Pool(min(16, os.cpu_count() or 1, n_batches)) as pool:
-                batches = pool.starmap(gen.make_batch, [(4, k * S, S) for k in range(n_batches)])
+                batches = pool.starmap(gen.make_batch, [(4, (rank * n_batches + k) * S, S) for k in range(n_batches)])
         except Exception:
-            batches = [gen.make_batch(4, k * S, S) for k in range(n_batches)]
+            batches = [gen.make_batch(4, (rank * n_batches + k) * S, S) for k in range(n_batches)]
         t_gen = time.perf_counter() - t_gen
         maxN = max(b.n_atoms for b in batches)
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -436,18 +436,24 @@ def main():
                 pnn.pnn_stream_drain(sh)
             run(min(3, n_batches))                       # warm-up
             torch.cuda.synchronize()
+            if world > 1:
+                dist.barrier()
             l0 = pnn.pnn_stream_launch_count(sh)
             t0 = time.perf_counter()
             run(n_batches)
             dt = time.perf_counter() - t0
+            if world > 1:   # replica streaming (P independent replicas): every rank streams its own
+                tm = torch.tensor([dt], dtype=torch.float64, device=dev)   # batches; the job's time is the slowest rank's
+                dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+                dt = float(tm.item())
             launches = pnn.pnn_stream_launch_count(sh) - l0
         finally:
             pnn.pnn_stream_destroy(sh)
-        n_struct = S * n_batches
+        n_struct = S * n_batches * world
         h2d = sum(x.numel() * x.element_size() for hb in hin for x in hb)
         assert all(np.isfinite(e.numpy()).all() for e in eo)
         return dict(api="pnn_stream_submit / pnn_stream_drain (depth 2: two workspaces, two CUDA streams, pinned host buffers)",
-                    batches=n_batches, structures=n_struct, atoms=int(sum(b.n_atoms for b in batches)), seconds=dt,
+                    batches=n_batches * world, ranks=world, structures=n_struct, atoms=int(sum(b.n_atoms for b in batches)), seconds=dt,
                     structures_per_s=n_struct / dt, ms_per_batch=1e3 * dt / n_batches,
                     resident_ms_per_batch=res["ms_per_step_median"],
                     ratio_to_resident_batches=(1e3 * dt / n_batches) / res["ms_per_step_median"],
@@ -492,7 +498,7 @@ def main():
 
     main_res = run_workload(args.workload, args.steps, args.warmup, full=True)
     main_rec = record(args.workload, main_res)
-    if args.workload == "cfg4" and world == 1 and not args.no_extra:
+    if args.workload == "cfg4" and not args.no_extra:
         main_rec["stream"] = cfg4_stream(main_res, args.stream_batches)
     close(main_res)
     mc, prec = main_res["mc"], main_res["prec"]

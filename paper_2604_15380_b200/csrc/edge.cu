@@ -57,13 +57,16 @@ __device__ __forceinline__ float dotK(const float (&w)[KP], const float* __restr
 }
 template <int KP>
 __device__ __forceinline__ double dotK(const double (&w)[KP], const double* __restrict__ g) {
-  double acc = 0.0;
+  // four independent chains: a single DFMA chain of KP links is bound by the FP64 pipe's latency, not its rate
+  double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
 #pragma unroll
-  for (int k = 0; k < KP; k += 2) {
+  for (int k = 0; k < KP; k += 4) {
     const double2 t = *reinterpret_cast<const double2*>(g + k);
-    acc = fma(w[k], t.x, acc); acc = fma(w[k + 1], t.y, acc);
+    const double2 u = *reinterpret_cast<const double2*>(g + k + 2);
+    a0 = fma(w[k], t.x, a0); a1 = fma(w[k + 1], t.y, a1);
+    a2 = fma(w[k + 2], u.x, a2); a3 = fma(w[k + 3], u.y, a3);
   }
-  return acc;
+  return (a0 + a1) + (a2 + a3);
 }
 
 // ------------------------------------------------------------------------------------------ forward

@@ -183,16 +183,6 @@ tc_gemm_k(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   const int64_t m0 = m_tile * BM;
   const int n0 = n_tile * BN;
   const int nkb = (K + BK - 1) / BK;
-  if (epi.readout) { // column tile n_tile = head n_tile: leave if none of this tile's rows belongs to it
-    int match = 0;
-    if (threadIdx.x < BM && m0 + threadIdx.x < M) {
-      int h = epi.head[epi.a2s[m0 + threadIdx.x]];
-      if (h < 0 || h >= epi.H) { if (n_tile == 0) atomicOr(epi.d_err, ERRF_BAD_HEAD); h = 0; }
-      match = (h == n_tile);
-    }
-    if (!__syncthreads_or(match)) return;
-  }
-
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
     mbar_init(acc_bar, 1);
@@ -245,34 +235,12 @@ tc_gemm_k(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     mbar_wait(acc_bar, 0);
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const int64_t m = m0 + q * 32 + lane;
-    bool row_ok = m < M;
-    int hrow = 0;
-    float esum = 0.0f;
-    if (epi.readout && row_ok) {
-      hrow = epi.head[epi.a2s[m]];
-      if (hrow < 0 || hrow >= epi.H) hrow = 0;
-      row_ok = (hrow == n_tile);
-    }
+    const bool row_ok = m < M;
 #pragma unroll 1
     for (int c0 = 0; c0 < BN; c0 += 32) {
       uint32_t r[32];
       tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)c0, r);
       if (!row_ok) continue;
-      if (epi.readout) {
-        const int n = n0 + c0;
-#pragma unroll
-        for (int j = 0; j < 32; j += 4) {
-          const float4 bv = __ldg(reinterpret_cast<const float4*>(epi.bias + n + j));
-          const float4 wv = __ldg(reinterpret_cast<const float4*>(epi.w2 + n + j));
-          const float p0 = __uint_as_float(r[j]) + bv.x, p1 = __uint_as_float(r[j + 1]) + bv.y,
-                      p2 = __uint_as_float(r[j + 2]) + bv.z, p3 = __uint_as_float(r[j + 3]) + bv.w;
-          if (epi.opre) *reinterpret_cast<float4*>(epi.opre + m * BN + c0 + j) = make_float4(p0, p1, p2, p3);
-          esum = fmaf(wv.x, silu_f<float>(p0), esum); esum = fmaf(wv.y, silu_f<float>(p1), esum);
-          esum = fmaf(wv.z, silu_f<float>(p2), esum); esum = fmaf(wv.w, silu_f<float>(p3), esum);
-        }
-        if (c0 + 32 >= BN) epi.eatom[m] = esum + epi.b2[hrow];
-        continue;
-      }
       epi_chunk(epi, m, n0 + c0, r);
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -322,11 +290,25 @@ tc_gemm_pk(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   const uint32_t tmem_base = *tmem_slot;
 
+  // Tile sequence of this CTA, identical in the three roles.  Plain GEMM: tiles blockIdx.x, + gridDim.x, ... of the
+  // (row tile, column tile) grid.  Readout mode: row tiles blockIdx.x, + gridDim.x, ..., and per row tile the heads
+  // (column tiles) that occur in it (epi.head_mask).
+  const int64_t m_tiles = (M + BM - 1) / BM;
+  auto for_each_tile = [&](auto&& body) {
+    if (epi.readout) {
+      for (int64_t mt = blockIdx.x; mt < m_tiles; mt += gridDim.x) {
+        unsigned long long msk = epi.head_mask[mt];
+        while (msk) { const int h = __ffsll((long long)msk) - 1; msk &= msk - 1; body(mt, h); }
+      }
+    } else {
+      for (int64_t tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) body(tile / n_tiles, (int)(tile % n_tiles));
+    }
+  };
   if (warp == 0) {
     if (lane == 0) {
       uint32_t it = 0; // k-blocks issued so far: stage = it % STAGES, parity = (it / STAGES) & 1
-      for (int64_t tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-        const int m0 = (int)((tile / n_tiles) * BM), n0 = (int)(tile % n_tiles) * BN;
+      for_each_tile([&](int64_t mt, int nt) {
+        const int m0 = (int)(mt * BM), n0 = nt * BN;
         for (int kb = 0; kb < nkb; ++kb, ++it) {
           const int s = it % STAGES;
           mbar_wait(empty_bar(s), ((it / STAGES) & 1u) ^ 1u);
@@ -335,13 +317,13 @@ tc_gemm_pk(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
           tma_load_2d(sa, &tmA, full_bar(s), kb * BK, m0);
           tma_load_2d(sa + A_BYTES, &tmB, full_bar(s), kb * BK, n0);
         }
-      }
+      });
     }
   } else if (warp == 1) {
     if (lane == 0) {
       const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
       uint32_t it = 0, j = 0; // j: tiles done by this CTA; accumulator buffer j & 1
-      for (int64_t tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++j) {
+      for_each_tile([&](int64_t, int) {
         const uint32_t b = j & 1u;
         mbar_wait(accempty_bar(b), ((j >> 1) & 1u) ^ 1u); // the epilogue has drained this buffer
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -358,28 +340,53 @@ tc_gemm_pk(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
           umma_commit(empty_bar(s));
         }
         umma_commit(accfull_bar(b));
-      }
+        ++j;
+      });
     }
   } else {
     const int q = warp & 3;
     uint32_t j = 0;
-    for (int64_t tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++j) {
+    for_each_tile([&](int64_t mt, int nt) {
       const uint32_t b = j & 1u;
-      const int64_t m = (tile / n_tiles) * BM + q * 32 + lane;
-      const int n0 = (int)(tile % n_tiles) * BN;
+      const int64_t m = mt * BM + q * 32 + lane;
+      const int n0 = nt * BN;
       mbar_wait(accfull_bar(b), (j >> 1) & 1u);
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+      bool row_ok = m < M;
+      int hrow = 0;
+      float esum = 0.0f;
+      if (epi.readout && row_ok) { // column tile nt = head nt: only the rows of that head are read out
+        hrow = epi.head[epi.a2s[m]];
+        row_ok = (hrow == nt);
+      }
 #pragma unroll 1
       for (int c0 = 0; c0 < BN; c0 += 32) {
         uint32_t r[32];
         tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + b * BN + (uint32_t)c0, r);
-        if (m < M) epi_chunk(epi, m, n0 + c0, r);
+        if (!row_ok) continue;
+        if (epi.readout) {
+          const int n = n0 + c0;
+#pragma unroll
+          for (int jj = 0; jj < 32; jj += 4) {
+            const float4 bv = __ldg(reinterpret_cast<const float4*>(epi.bias + n + jj));
+            const float4 wv = __ldg(reinterpret_cast<const float4*>(epi.w2 + n + jj));
+            const float p0 = __uint_as_float(r[jj]) + bv.x, p1 = __uint_as_float(r[jj + 1]) + bv.y,
+                        p2 = __uint_as_float(r[jj + 2]) + bv.z, p3 = __uint_as_float(r[jj + 3]) + bv.w;
+            if (epi.opre) *reinterpret_cast<float4*>(epi.opre + m * BN + c0 + jj) = make_float4(p0, p1, p2, p3);
+            esum = fmaf(wv.x, silu_f<float>(p0), esum); esum = fmaf(wv.y, silu_f<float>(p1), esum);
+            esum = fmaf(wv.z, silu_f<float>(p2), esum); esum = fmaf(wv.w, silu_f<float>(p3), esum);
+          }
+          if (c0 + 32 >= BN) epi.eatom[m] = esum + epi.b2[hrow];
+          continue;
+        }
+        epi_chunk(epi, m, n0 + c0, r);
       }
       // all TMEM reads of this warp are complete (tcgen05.wait::ld in tmem_ld32): hand the buffer back to the MMA warp
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
       __syncwarp();
       if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(accempty_bar(b)) : "memory");
-    }
+      ++j;
+    });
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
@@ -520,23 +527,47 @@ int launch_gemm_tc(int64_t M, int N, int K, const __nv_bfloat16* A, int64_t lda,
   }
 }
 
-bool readout_tc_supported(int F) { return F == 64 || F == 128 || F == 256; }
+bool readout_tc_supported(int F, int H) { return (F == 64 || F == 128 || F == 256) && H <= 64; }
+
+// mask[t] = set of heads used by the rows of the 128-row tile t (one warp per tile); bad head indices are flagged
+__global__ void __launch_bounds__(256) head_mask_k(int64_t N, int H, const int32_t* __restrict__ a2s,
+                                                   const int32_t* __restrict__ head, unsigned long long* mask, int* d_err) {
+  const int64_t t = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (t * BM >= N) return;
+  unsigned long long m = 0;
+  bool bad = false;
+  for (int r = lane; r < BM; r += 32) {
+    const int64_t row = t * BM + r;
+    if (row < N) {
+      const int h = head[a2s[row]];
+      if (h < 0 || h >= H) bad = true; else m |= 1ull << h;
+    }
+  }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) m |= __shfl_xor_sync(0xffffffffu, m, o);
+  if (__any_sync(0xffffffffu, bad) && lane == 0) atomicOr(d_err, ERRF_BAD_HEAD);
+  if (lane == 0) mask[t] = m;
+}
 
 int launch_readout_tc(int64_t N, int F, int H, const __nv_bfloat16* s16, const __nv_bfloat16* W1all, const float* b1,
                       const float* w2, const float* b2, const int32_t* a2s, const int32_t* head, float* opre,
-                      float* eatom, int* d_err, cudaStream_t st) {
+                      float* eatom, int* d_err, unsigned long long* head_mask, cudaStream_t st) {
   if (N <= 0) return 0;
   const int Fh = F / 2;
-  if (Fh != 32 && Fh != 64 && Fh != 128) return -1;
+  if (!readout_tc_supported(F, H)) return -1;
   CUtensorMap ta, tb;
   if (!get_tensor_map(s16, N, F, F, BM, &ta) || !get_tensor_map(W1all, (int64_t)H * Fh, F, F, Fh, &tb)) return -1;
+  const int64_t m_tiles = (N + BM - 1) / BM;
+  head_mask_k<<<(unsigned)((m_tiles * 32 + 255) / 256), 256, 0, st>>>(N, H, a2s, head, head_mask, d_err);
+  PNN_KCHECK("head_mask_k");
   TcEpi e;
   e.bias = b1; e.readout = 1; e.a2s = a2s; e.head = head; e.w2 = w2; e.b2 = b2; e.eatom = eatom; e.opre = opre;
-  e.H = H; e.d_err = d_err;
+  e.H = H; e.d_err = d_err; e.head_mask = head_mask;
   switch (Fh) {
-    case 128: return launch_cfg<128, 3>(N, H * Fh, F, ta, tb, e, st);
-    case 64: return launch_cfg<64, 4>(N, H * Fh, F, ta, tb, e, st);
-    default: return launch_cfg<32, 4>(N, H * Fh, F, ta, tb, e, st);
+    case 128: return 1 + launch_persistent<128, 3>(N, H * Fh, F, ta, tb, e, st);
+    case 64: return 1 + launch_persistent<64, 4>(N, H * Fh, F, ta, tb, e, st);
+    default: return 1 + launch_persistent<32, 4>(N, H * Fh, F, ta, tb, e, st);
   }
 }
 

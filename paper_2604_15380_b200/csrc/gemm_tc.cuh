@@ -33,6 +33,7 @@ struct TcEpi {
   float* opre = nullptr;
   int H = 0;
   int* d_err = nullptr;
+  const unsigned long long* head_mask = nullptr; // [row tiles of 128]: bit h = some row of the tile uses head h
 };
 
 // Returns the number of kernels launched (0 or 1); < 0 when the TMA descriptor could not be encoded.
@@ -40,15 +41,16 @@ int launch_gemm_tc(int64_t M, int N, int K, const __nv_bfloat16* A, int64_t lda,
                    const TcEpi& epi, cudaStream_t st);
 
 // a6 on the tensor cores: eatom[i] = w2^h . silu(W1^h s_i + b1^h) + b2^h with h = head[a2s[i]] as ONE GEMM against the
-// stacked first layers of all heads, W1all [H*Fh][F] (BF16): a column tile is exactly one head (Fh in {32, 64, 128}),
-// tiles none of whose 128 rows use that head exit before loading anything, and the epilogue keeps only the rows of
-// its head.  bias = b1 of all heads [H*Fh], w2 [H*Fh], b2 [H].  opre (FP32 [N][Fh], pre-activation for R1) may be NULL.
+// stacked first layers of all heads, W1all [H*Fh][F] (BF16): a column tile is exactly one head (Fh in {32, 64, 128}); a
+// persistent CTA walks row tiles and, per row tile, only the heads that occur in it; the epilogue keeps the rows of its head.  bias = b1 of all heads [H*Fh], w2 [H*Fh], b2 [H].  opre (FP32 [N][Fh], pre-activation for R1) may be NULL.
 // Returns kernels launched, or -1 if the shape is not supported (readout_tc_supported) or a TMA descriptor could not be
 // encoded (an error for the caller).
-bool readout_tc_supported(int F);
+bool readout_tc_supported(int F, int H);
+// head_mask: scratch of ceil(N / 128) 64-bit words (which heads occur in each 128-row tile; written by a small kernel
+// first, so that only the (row tile, head) pairs that exist are computed).  H <= 64.
 int launch_readout_tc(int64_t N, int F, int H, const __nv_bfloat16* s16, const __nv_bfloat16* W1all, const float* b1,
                       const float* w2, const float* b2, const int32_t* a2s, const int32_t* head, float* opre,
-                      float* eatom, int* d_err, cudaStream_t st);
+                      float* eatom, int* d_err, unsigned long long* head_mask, cudaStream_t st);
 
 // dst[i] = bf16(src[i])
 int launch_f32_to_bf16(int64_t n, const float* src, __nv_bfloat16* dst, cudaStream_t st);

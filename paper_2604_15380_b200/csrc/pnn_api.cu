@@ -101,6 +101,7 @@ struct pnn_workspace {
   int64_t launches = 0;
   // activations (element type = model state type)
   void *s_cur, *h, *sn, *v1, *k, *vping[2], *eatom, *opre;
+  unsigned long long* head_mask = nullptr; // BF16 readout GEMM: heads present per 128-row tile
   void* opre_all = nullptr; // blended readout: pre-activations of every head [N][H][F/2] (reverse sweep)
   struct Tape { void *v_in, *hpre, *phi, *PQ, *kpre, *a; };
   std::vector<Tape> tape;
@@ -343,6 +344,7 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
     ws->v1 = carve(es * N * 3 * F);
     ws->k = carve(es * N * F);
     ws->eatom = carve(es * N);
+    ws->head_mask = (unsigned long long*)carve(8 * ((N + 127) / 128 + 1));
     ws->tape.resize(want_forces ? T : 1);
     if (want_forces) {
       ws->opre = carve(es * N * (F / 2));
@@ -761,9 +763,9 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     if (hw) { // blended heads: FP32 readout of the FP32 residual stream (one structure may need every head)
       l_ = launch_readout_blend<T>(N, S, F, c.H, s_cur, ws->g.a2s, hw, (T)skip_below, sptr, W + m->oW1t, W + m->ob1,
                                    W + m->ow2, W + m->ob2, (T*)ws->opre_all, (T*)ws->eatom, energy, st);
-    } else if (readout_tc_supported(F)) { // head widths F/2 in {32, 64, 128}: one tensor-core GEMM over the stacked heads
+    } else if (readout_tc_supported(F, c.H)) { // head widths F/2 in {32, 64, 128}: one tensor-core GEMM over the stacked heads
       l_ = launch_readout_tc(N, F, c.H, mb.s16, Wb + m->oW1, W + m->ob1, W + m->ow2, W + m->ob2, ws->g.a2s, head,
-                             (T*)ws->opre, (T*)ws->eatom, ws->g.d_err, st);
+                             (T*)ws->opre, (T*)ws->eatom, ws->g.d_err, ws->head_mask, st);
       if (l_ < 0) { tc_fail = true; l_ = 0; }
       else l_ += launch_struct_sum<T>(S, sptr, (const T*)ws->eatom, energy, st);
     } else { // other widths: the FP32 readout of the FP32 residual stream
