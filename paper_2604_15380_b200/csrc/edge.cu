@@ -418,7 +418,6 @@ int launch_edge_bwd(const EdgeArgs<T>& a, const PT* phi, const PT* v_in, const T
                                       int, __nv_bfloat16*, cudaStream_t);
 PNN_INST_EDGE(float, float)
 PNN_INST_EDGE(double, double)
-PNN_INST_EDGE(float, __nv_bfloat16)
 #undef PNN_INST_EDGE
 
 } // namespace pnn
