@@ -78,6 +78,7 @@ class ModelCfg:
     norm_eps: float = 1e-8
     pbc_images: str = "minimum"  # or "all": every periodic image inside the cutoff (cells narrower than 2 r_c)
     rbf: str = "gaussian"   # or "bessel" (the paper's lead model uses 4 Bessel functions)
+    max_neighbors: int = 0  # > 0: every receiver keeps its nearest max_neighbors senders ("Max neighbors 20")
 
 
 @dataclasses.dataclass

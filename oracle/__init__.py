@@ -50,7 +50,7 @@ def _p(a, ct):
 def _cfg_arrays(mc):
     rbf = {"gaussian": 0, "bessel": 1}[getattr(mc, "rbf", "gaussian")]
     images = {"minimum": 0, "all": 1}[getattr(mc, "pbc_images", "minimum")]
-    ic = np.array([mc.F, mc.T, mc.K, mc.H, mc.Zmax, rbf, images], np.int32)
+    ic = np.array([mc.F, mc.T, mc.K, mc.H, mc.Zmax, rbf, images, int(getattr(mc, "max_neighbors", 0))], np.int32)
     dc = np.array([mc.cutoff, mc.norm_eps], np.float64)
     return ic, dc
 
@@ -102,24 +102,26 @@ def _prep(batch):
     return Z, pos, sp, head, cell, pbc
 
 
-def neighbours(batch, cutoff: float, all_images: bool = False):
+def neighbours(batch, cutoff: float, all_images: bool = False, max_neighbors: int = 0):
     """Brute-force radius graph. Returns dict(rowptr, recv, send, shift, rvec).
-    all_images: every periodic image inside the cutoff (self images included) instead of the minimum image only."""
+    all_images: every periodic image inside the cutoff (self images included) instead of the minimum image only.
+    max_neighbors > 0: every receiver keeps its nearest max_neighbors senders only."""
     lib = _load()
     Z, pos, sp, head, cell, pbc = _prep(batch)
     N, S = Z.shape[0], head.shape[0]
     rowptr = np.zeros(N + 1, np.int32)
-    lib.oracle_neighbours_images.restype = ctypes.c_int64
+    lib.oracle_neighbours_capped.restype = ctypes.c_int64
     ai = ctypes.c_int32(1 if all_images else 0)
-    E = lib.oracle_neighbours_images(ctypes.c_int32(N), ctypes.c_int32(S), _p(pos, ctypes.c_double),
+    mn = ctypes.c_int32(int(max_neighbors))
+    E = lib.oracle_neighbours_capped(ctypes.c_int32(N), ctypes.c_int32(S), _p(pos, ctypes.c_double),
                                      _p(sp, ctypes.c_int32), _p(cell, ctypes.c_double), _p(pbc, ctypes.c_uint8),
-                                     ctypes.c_double(cutoff), ai, _p(rowptr, ctypes.c_int32), None, None, None, None)
+                                     ctypes.c_double(cutoff), ai, mn, _p(rowptr, ctypes.c_int32), None, None, None, None)
     recv = np.zeros(E, np.int32)
     send = np.zeros(E, np.int32)
     shift = np.zeros((E, 3), np.int8)
     rvec = np.zeros((E, 3), np.float64)
-    lib.oracle_neighbours_images(ctypes.c_int32(N), ctypes.c_int32(S), _p(pos, ctypes.c_double), _p(sp, ctypes.c_int32),
-                                 _p(cell, ctypes.c_double), _p(pbc, ctypes.c_uint8), ctypes.c_double(cutoff), ai,
+    lib.oracle_neighbours_capped(ctypes.c_int32(N), ctypes.c_int32(S), _p(pos, ctypes.c_double), _p(sp, ctypes.c_int32),
+                                 _p(cell, ctypes.c_double), _p(pbc, ctypes.c_uint8), ctypes.c_double(cutoff), ai, mn,
                                  _p(rowptr, ctypes.c_int32), _p(recv, ctypes.c_int32), _p(send, ctypes.c_int32),
                                  _p(shift, ctypes.c_int8), _p(rvec, ctypes.c_double))
     return dict(rowptr=rowptr, recv=recv, send=send, shift=shift, rvec=rvec)

@@ -26,6 +26,7 @@
 // "parity unpinned": the paper's trained-model figures (|dE| 0.021 / 0.080 eV, Table XV) —
 // the checkpoint and datasets are not available.
 
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstring>
@@ -58,7 +59,7 @@ inline double value_of(double a) { return a; }
 inline double value_of(Dual a) { return a.v; }
 
 // ------------------------------------------------------------------ model = views into the blob
-struct Cfg { int F, T, K, H, Zmax; double rc, eps; int rbf; int images; };  // rbf: 0 Gaussian, 1 Bessel; images: 0 minimum image, 1 all
+struct Cfg { int F, T, K, H, Zmax; double rc, eps; int rbf; int images; int max_nb; };  // rbf: 0 Gaussian, 1 Bessel; images: 0 minimum image, 1 all; max_nb: 0 = no cap
 struct Block {
   const double *msg_W1, *msg_b1, *msg_W2, *msg_b2, *flt_W, *flt_b;
   const double *upd_U, *upd_V, *upd_A1, *upd_c1, *upd_A2, *upd_c2;
@@ -112,8 +113,61 @@ void inverse3(const double* C, double* Ci) {
 // all_images = 0: one (minimum) image per ordered pair (reading Q13).  all_images = 1: the radius graph of the infinite
 // periodic structure — every ordered pair (i, j), i == j included, and every integer lattice shift s with
 // 0 < |x_j - x_i + s.C| < rc; needed when a cell is narrower than 2 rc.
+// max_nb > 0: the paper's "Max neighbors" (Table V: 20; 64 with periodic boundary conditions;
+// DESIGN.md reading Q16): every receiver keeps only its max_nb NEAREST senders inside the cutoff — smallest squared distance
+// first, ties broken by the sender index, then by the lattice shift — so the edge set is no longer symmetric.
+void cap_neighbours(int N, const double* pos, int max_nb, Edges* E);
+void neighbours_all(int N, int S, const double* pos, const int32_t* sptr, const double* cell,
+                    const uint8_t* pbc, double rc, Edges* E, int all_images);
 void neighbours(int N, int S, const double* pos, const int32_t* sptr, const double* cell,
-                const uint8_t* pbc, double rc, Edges* E, int all_images = 0) {
+                const uint8_t* pbc, double rc, Edges* E, int all_images = 0, int max_nb = 0) {
+  neighbours_all(N, S, pos, sptr, cell, pbc, rc, E, all_images);
+  if (max_nb > 0) cap_neighbours(N, pos, max_nb, E);
+}
+void cap_neighbours(int N, const double* pos, int max_nb, Edges* E) {
+  Edges out;
+  out.rowptr.assign(N + 1, 0);
+  for (int i = 0; i < N; ++i) {
+    const int a = E->rowptr[i], b = E->rowptr[i + 1];
+    std::vector<int> idx(b - a);
+    std::vector<double> d2(b - a);
+    for (int e = a; e < b; ++e) {
+      idx[e - a] = e;
+      double q = 0.0;
+      for (int c = 0; c < 3; ++c) {
+        const double r = pos[3 * E->send[e] + c] - pos[3 * i + c] + E->shift_cart[3 * e + c];
+        q += r * r;
+      }
+      d2[e - a] = q;
+    }
+    // plain selection sort of the row by (d^2, sender, shift): the first max_nb entries are kept
+    for (int x = 0; x < (int)idx.size(); ++x)
+      for (int y = x + 1; y < (int)idx.size(); ++y) {
+        const int ex = idx[x], ey = idx[y];
+        bool less = d2[ey - a] < d2[ex - a];
+        if (d2[ey - a] == d2[ex - a]) {
+          if (E->send[ey] != E->send[ex]) less = E->send[ey] < E->send[ex];
+          else
+            for (int c = 0; c < 3; ++c)
+              if (E->shift[3 * ey + c] != E->shift[3 * ex + c]) { less = E->shift[3 * ey + c] < E->shift[3 * ex + c]; break; }
+        }
+        if (less) { idx[x] = ey; idx[y] = ex; }
+      }
+    const int keep = std::min<int>(max_nb, (int)idx.size());
+    std::vector<int> kept(idx.begin(), idx.begin() + keep);
+    for (int x = 0; x < keep; ++x)          // back to the original (ascending sender) order within the row
+      for (int y = x + 1; y < keep; ++y)
+        if (kept[y] < kept[x]) { const int t = kept[x]; kept[x] = kept[y]; kept[y] = t; }
+    for (int e : kept) {
+      out.recv.push_back(i); out.send.push_back(E->send[e]);
+      for (int c = 0; c < 3; ++c) { out.shift.push_back(E->shift[3 * e + c]); out.shift_cart.push_back(E->shift_cart[3 * e + c]); }
+    }
+    out.rowptr[i + 1] = out.rowptr[i] + keep;
+  }
+  *E = out;
+}
+void neighbours_all(int N, int S, const double* pos, const int32_t* sptr, const double* cell,
+                    const uint8_t* pbc, double rc, Edges* E, int all_images) {
   E->rowptr.assign(N + 1, 0);
   for (int g = 0; g < S; ++g) {
     const bool periodic = cell && pbc && (pbc[3 * g] || pbc[3 * g + 1] || pbc[3 * g + 2]);
@@ -506,7 +560,9 @@ void reverse(const Model& m, int N, int nS, const int32_t* sptr, const int32_t* 
   for (long q = 0; q < (long)N * 3; ++q) forces[q] = -gx[q];
 }
 
-Cfg make_cfg(const int32_t* ic, const double* dc) { return Cfg{ic[0], ic[1], ic[2], ic[3], ic[4], dc[0], dc[1], ic[5], ic[6]}; }
+Cfg make_cfg(const int32_t* ic, const double* dc) {
+  return Cfg{ic[0], ic[1], ic[2], ic[3], ic[4], dc[0], dc[1], ic[5], ic[6], ic[7]};
+}
 
 }  // namespace
 
@@ -528,11 +584,19 @@ int64_t oracle_neighbours(int32_t N, int32_t S, const double* pos, const int32_t
                           int8_t* shift, double* rvec) {
   return oracle_neighbours_images(N, S, pos, sptr, cell, pbc, rc, 0, rowptr, recv, send, shift, rvec);
 }
+int64_t oracle_neighbours_capped(int32_t N, int32_t S, const double* pos, const int32_t* sptr, const double* cell,
+                                 const uint8_t* pbc, double rc, int32_t all_images, int32_t max_nb, int32_t* rowptr,
+                                 int32_t* recv, int32_t* send, int8_t* shift, double* rvec);
 int64_t oracle_neighbours_images(int32_t N, int32_t S, const double* pos, const int32_t* sptr, const double* cell,
                                  const uint8_t* pbc, double rc, int32_t all_images, int32_t* rowptr, int32_t* recv,
                                  int32_t* send, int8_t* shift, double* rvec) {
+  return oracle_neighbours_capped(N, S, pos, sptr, cell, pbc, rc, all_images, 0, rowptr, recv, send, shift, rvec);
+}
+int64_t oracle_neighbours_capped(int32_t N, int32_t S, const double* pos, const int32_t* sptr, const double* cell,
+                                 const uint8_t* pbc, double rc, int32_t all_images, int32_t max_nb, int32_t* rowptr,
+                                 int32_t* recv, int32_t* send, int8_t* shift, double* rvec) {
   Edges ed;
-  neighbours(N, S, pos, sptr, cell, pbc, rc, &ed, all_images);
+  neighbours(N, S, pos, sptr, cell, pbc, rc, &ed, all_images, max_nb);
   const int64_t E = (int64_t)ed.recv.size();
   if (rowptr) std::memcpy(rowptr, ed.rowptr.data(), sizeof(int32_t) * (N + 1));
   if (recv) {
@@ -556,7 +620,7 @@ int64_t oracle_eval(const int32_t* icfg, const double* dcfg /*cutoff, eps*/, con
   Model m;
   parse_blob(make_cfg(icfg, dcfg), weights, &m);
   Edges ed;
-  neighbours(N, S, pos, sptr, cell, pbc, m.c.rc, &ed, m.c.images);
+  neighbours(N, S, pos, sptr, cell, pbc, m.c.rc, &ed, m.c.images, m.c.max_nb);
   Tape<double> tp;
   forward<double>(m, N, S, Z, pos, sptr, head, ed, tp, energy);
   if (s_out) std::memcpy(s_out, tp.s_out.data(), sizeof(double) * tp.s_out.size());
@@ -575,7 +639,7 @@ void oracle_forces_dual(const int32_t* icfg, const double* dcfg, const double* w
   Model m;
   parse_blob(make_cfg(icfg, dcfg), weights, &m);
   Edges ed;
-  neighbours(N, S, pos, sptr, cell, pbc, m.c.rc, &ed, m.c.images);
+  neighbours(N, S, pos, sptr, cell, pbc, m.c.rc, &ed, m.c.images, m.c.max_nb);
   std::vector<int> sof(N);
   for (int g = 0; g < S; ++g) for (int i = sptr[g]; i < sptr[g + 1]; ++i) sof[i] = g;
 #pragma omp parallel for schedule(dynamic, 1)
