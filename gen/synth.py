@@ -79,6 +79,7 @@ class ModelCfg:
     pbc_images: str = "minimum"  # or "all": every periodic image inside the cutoff (cells narrower than 2 r_c)
     rbf: str = "gaussian"   # or "bessel" (the paper's lead model uses 4 Bessel functions)
     max_neighbors: int = 0  # > 0: every receiver keeps its nearest max_neighbors senders ("Max neighbors 20")
+    n_global: int = 0       # global attributes per structure (charge, spin: PAPER.md:58) entering the embedding
 
 
 @dataclasses.dataclass
@@ -159,6 +160,8 @@ def weights_layout(mc: ModelCfg):
         add(f"h{h}.out_b1", (F // 2,), F)
         add(f"h{h}.out_w2", (F // 2,), F // 2)
         add(f"h{h}.out_b2", (1,), F // 2)
+    if getattr(mc, "n_global", 0) > 0:   # global attributes (charge, spin): glob_W [F][n_global], appended
+        add("glob_W", (F, mc.n_global), 1)
     return out
 
 

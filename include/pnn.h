@@ -58,6 +58,11 @@ typedef struct {
   int32_t prec; /* pnn_precision */
   int32_t rbf;  /* PNN_RBF_GAUSSIAN or PNN_RBF_BESSEL; both are multiplied by the cosine cutoff */
   int32_t pbc_images; /* PNN_IMAGES_MINIMUM or PNN_IMAGES_ALL (pnn_build_graph) */
+  int32_t max_neighbors; /* 0 = every sender inside the cutoff; k > 0 = each receiver keeps its k NEAREST senders (the
+                            paper's "Max neighbors": 20 in Table V; 64 with PBC).  Smallest FP64
+                            squared distance first, ties by sender index, then lattice shift.  The edge set is then not
+                            symmetric: the reverse sweep runs its scatter form (atomic adds; edge_scatter.cu) instead of
+                            the gather form, and max_edges still bounds the UNCAPPED edge count of a batch. */
 } pnn_config;
 
 typedef struct pnn_model pnn_model;         /* opaque; owns device copies of the weights in model precision */

@@ -50,7 +50,8 @@ def _p(a, ct):
 def _cfg_arrays(mc):
     rbf = {"gaussian": 0, "bessel": 1}[getattr(mc, "rbf", "gaussian")]
     images = {"minimum": 0, "all": 1}[getattr(mc, "pbc_images", "minimum")]
-    ic = np.array([mc.F, mc.T, mc.K, mc.H, mc.Zmax, rbf, images, int(getattr(mc, "max_neighbors", 0))], np.int32)
+    ic = np.array([mc.F, mc.T, mc.K, mc.H, mc.Zmax, rbf, images, int(getattr(mc, "max_neighbors", 0)),
+                   int(getattr(mc, "n_global", 0))], np.int32)
     dc = np.array([mc.cutoff, mc.norm_eps], np.float64)
     return ic, dc
 
@@ -127,8 +128,9 @@ def neighbours(batch, cutoff: float, all_images: bool = False, max_neighbors: in
     return dict(rowptr=rowptr, recv=recv, send=send, shift=shift, rvec=rvec)
 
 
-def evaluate(mc, weights, batch, forces: bool = True, features: bool = False):
-    """Energy [S], forces [N,3] (or None); with features=True also s [N,F], v [N,3,F], eatom [N]."""
+def evaluate(mc, weights, batch, forces: bool = True, features: bool = False, globals_=None):
+    """Energy [S], forces [N,3] (or None); with features=True also s [N,F], v [N,3,F], eatom [N].
+    globals_ [S, mc.n_global]: the structures' global attributes (charge, spin), or None."""
     lib = _load()
     ic, dc = _cfg_arrays(mc)
     w = np.ascontiguousarray(weights, np.float64)
@@ -142,11 +144,16 @@ def evaluate(mc, weights, batch, forces: bool = True, features: bool = False):
     s_out = np.zeros((N, mc.F), np.float64) if features else None
     v_out = np.zeros((N, 3, mc.F), np.float64) if features else None
     eatom = np.zeros(N, np.float64) if features else None
-    E = lib.oracle_eval(_p(ic, ctypes.c_int32), _p(dc, ctypes.c_double), _p(w, ctypes.c_double), ctypes.c_int32(N),
-                        ctypes.c_int32(S), _p(Z, ctypes.c_int32), _p(pos, ctypes.c_double), _p(sp, ctypes.c_int32),
-                        _p(cell, ctypes.c_double), _p(pbc, ctypes.c_uint8), _p(head, ctypes.c_int32),
-                        _p(energy, ctypes.c_double), _p(frc, ctypes.c_double), _p(s_out, ctypes.c_double),
-                        _p(v_out, ctypes.c_double), _p(eatom, ctypes.c_double))
+    gl = None
+    if globals_ is not None:
+        gl = np.ascontiguousarray(globals_, np.float64)
+        assert gl.shape == (S, getattr(mc, "n_global", 0))
+    lib.oracle_eval_glob.restype = ctypes.c_int64
+    E = lib.oracle_eval_glob(_p(ic, ctypes.c_int32), _p(dc, ctypes.c_double), _p(w, ctypes.c_double), ctypes.c_int32(N),
+                             ctypes.c_int32(S), _p(Z, ctypes.c_int32), _p(pos, ctypes.c_double), _p(sp, ctypes.c_int32),
+                             _p(cell, ctypes.c_double), _p(pbc, ctypes.c_uint8), _p(head, ctypes.c_int32),
+                             _p(gl, ctypes.c_double), _p(energy, ctypes.c_double), _p(frc, ctypes.c_double),
+                             _p(s_out, ctypes.c_double), _p(v_out, ctypes.c_double), _p(eatom, ctypes.c_double))
     out = dict(energy=energy, forces=frc, n_edges=int(E))
     if features:
         out.update(s=s_out, v=v_out, eatom=eatom)

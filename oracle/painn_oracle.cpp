@@ -59,13 +59,13 @@ inline double value_of(double a) { return a; }
 inline double value_of(Dual a) { return a.v; }
 
 // ------------------------------------------------------------------ model = views into the blob
-struct Cfg { int F, T, K, H, Zmax; double rc, eps; int rbf; int images; int max_nb; };  // rbf: 0 Gaussian, 1 Bessel; images: 0 minimum image, 1 all; max_nb: 0 = no cap
+struct Cfg { int F, T, K, H, Zmax; double rc, eps; int rbf; int images; int max_nb; int n_glob; };  // rbf: 0 Gaussian, 1 Bessel; images: 0 minimum image, 1 all; max_nb: 0 = no cap; n_glob: global attributes per structure
 struct Block {
   const double *msg_W1, *msg_b1, *msg_W2, *msg_b2, *flt_W, *flt_b;
   const double *upd_U, *upd_V, *upd_A1, *upd_c1, *upd_A2, *upd_c2;
 };
 struct Head { const double *W1, *b1, *w2, *b2; };
-struct Model { Cfg c; const double* emb; std::vector<Block> blk; std::vector<Head> head; };
+struct Model { Cfg c; const double* emb; std::vector<Block> blk; std::vector<Head> head; const double* glob_W; };
 
 // Blob order: SURVEY.md §8(b) "Weight blob"; matrices row-major [out][in], y = W x + b.
 long parse_blob(const Cfg& c, const double* w, Model* m) {
@@ -90,6 +90,10 @@ long parse_blob(const Cfg& c, const double* w, Model* m) {
     hd.W1 = take((F / 2) * F); hd.b1 = take(F / 2); hd.w2 = take(F / 2); hd.b2 = take(1);
     if (m) m->head[h] = hd;
   }
+  // global attributes ("global attributes such as charge and spin used as additional input features";
+  // DESIGN.md reading Q30): glob_W [F][n_glob], appended to the blob when n_glob > 0
+  const double* gw = take((long)F * c.n_glob);
+  if (m) m->glob_W = gw;
   return (long)(p - w);
 }
 
@@ -266,7 +270,7 @@ template <class S> struct Tape {
 // ------------------------------------------------------------------ forward (B2..B5)
 template <class S>
 void forward(const Model& m, int N, int nS, const int32_t* Z, const S* pos, const int32_t* sptr,
-             const int32_t* head, const Edges& ed, Tape<S>& tp, S* energy) {
+             const int32_t* head, const Edges& ed, Tape<S>& tp, S* energy, const double* glob = nullptr) {
   const int F = m.c.F, K = m.c.K, T = m.c.T;
   const double rc = m.c.rc;
   const long E = (long)ed.recv.size();
@@ -289,6 +293,13 @@ void forward(const Model& m, int N, int nS, const int32_t* Z, const S* pos, cons
   std::vector<S> s((long)N * F), v((long)N * 3 * F, S(0.0));
   for (int i = 0; i < N; ++i)
     for (int f = 0; f < F; ++f) s[(long)i * F + f] = S(m.emb[(long)Z[i] * F + f]);
+  if (m.c.n_glob > 0 && glob) {   // s0_i += glob_W . (charge, spin, ...) of the atom's structure (reading Q30)
+    for (int g = 0; g < nS; ++g)
+      for (int i = sptr[g]; i < sptr[g + 1]; ++i)
+        for (int f = 0; f < F; ++f)
+          for (int q = 0; q < m.c.n_glob; ++q)
+            s[(long)i * F + f] += S(m.glob_W[(long)f * m.c.n_glob + q] * glob[(long)g * m.c.n_glob + q]);
+  }
 
   tp.blk.resize(T);
   for (int t = 0; t < T; ++t) {
@@ -561,7 +572,7 @@ void reverse(const Model& m, int N, int nS, const int32_t* sptr, const int32_t* 
 }
 
 Cfg make_cfg(const int32_t* ic, const double* dc) {
-  return Cfg{ic[0], ic[1], ic[2], ic[3], ic[4], dc[0], dc[1], ic[5], ic[6], ic[7]};
+  return Cfg{ic[0], ic[1], ic[2], ic[3], ic[4], dc[0], dc[1], ic[5], ic[6], ic[7], ic[8]};
 }
 
 }  // namespace
@@ -613,16 +624,28 @@ int64_t oracle_neighbours_capped(int32_t N, int32_t S, const double* pos, const 
 
 // Full path.  energy [S]; forces [N][3] or NULL; optional outputs s_out [N][F], v_out [N][3][F],
 // eatom [N] (may be NULL).  Returns the number of directed edges.
+int64_t oracle_eval_glob(const int32_t* icfg, const double* dcfg, const double* weights, int32_t N, int32_t S,
+                         const int32_t* Z, const double* pos, const int32_t* sptr, const double* cell, const uint8_t* pbc,
+                         const int32_t* head, const double* glob, double* energy, double* forces, double* s_out,
+                         double* v_out, double* eatom);
 int64_t oracle_eval(const int32_t* icfg, const double* dcfg /*cutoff, eps*/, const double* weights, int32_t N,
                     int32_t S, const int32_t* Z, const double* pos, const int32_t* sptr, const double* cell,
                     const uint8_t* pbc, const int32_t* head, double* energy, double* forces, double* s_out,
                     double* v_out, double* eatom) {
+  return oracle_eval_glob(icfg, dcfg, weights, N, S, Z, pos, sptr, cell, pbc, head, nullptr, energy, forces, s_out, v_out,
+                          eatom);
+}
+// glob [S][n_glob] (host) or NULL: the structures' global attributes (charge, spin)
+int64_t oracle_eval_glob(const int32_t* icfg, const double* dcfg, const double* weights, int32_t N, int32_t S,
+                         const int32_t* Z, const double* pos, const int32_t* sptr, const double* cell, const uint8_t* pbc,
+                         const int32_t* head, const double* glob, double* energy, double* forces, double* s_out,
+                         double* v_out, double* eatom) {
   Model m;
   parse_blob(make_cfg(icfg, dcfg), weights, &m);
   Edges ed;
   neighbours(N, S, pos, sptr, cell, pbc, m.c.rc, &ed, m.c.images, m.c.max_nb);
   Tape<double> tp;
-  forward<double>(m, N, S, Z, pos, sptr, head, ed, tp, energy);
+  forward<double>(m, N, S, Z, pos, sptr, head, ed, tp, energy, glob);
   if (s_out) std::memcpy(s_out, tp.s_out.data(), sizeof(double) * tp.s_out.size());
   if (v_out) std::memcpy(v_out, tp.v_out.data(), sizeof(double) * tp.v_out.size());
   if (eatom) std::memcpy(eatom, tp.eatom.data(), sizeof(double) * N);

@@ -110,11 +110,19 @@ struct GraphBuffers {
   int* d_err;   // sticky flags (ERRF_*), cleared by pnn_check_async_errors
   int* d_ovf;   // ERRF_EDGE_OVERFLOW or 0 for the CURRENT graph: rewritten by every build, tested by the edge kernels
   unsigned long long* d_poschk; // [2]: checksum of the positions the graph was built from / scratch for pnn_eval's check
+  // max-neighbour cap (pnn_config.max_neighbors > 0 only; NULL otherwise): scratch of the compaction pass
+  int32_t* cap_col = nullptr;   // [Emax]
+  int8_t* cap_shift = nullptr;  // [Emax,3]
+  void* cap_geom = nullptr;     // [Emax] Geom<T>
+  uint8_t* cap_keep = nullptr;  // [Emax]
+  int32_t* cap_deg = nullptr;   // [N+1]
+  int32_t* cap_rowptr = nullptr; // [N+1]
 };
 // Flags ERRF_STALE_GRAPH when the checksum of pos differs from the one recorded by the last launch_graph_build.
 int launch_pos_check(const GraphBuffers& g, int64_t N, const double* pos, cudaStream_t st);
 int launch_graph_build(const GraphBuffers& g, int64_t N, int64_t S, const double* pos, const int32_t* struct_ptr,
-                       const double* cell, const uint8_t* pbc, double rc, int prec, int all_images, cudaStream_t st);
+                       const double* cell, const uint8_t* pbc, double rc, int prec, int all_images, int max_neighbors,
+                       cudaStream_t st);
 
 // gemm_simt.cu :  C[M,N] (ldc) = epi( A[M,K] (lda) * B[K,N] (ldb) )
 enum : int { ACT_NONE = 0, ACT_SILU = 1, ACT_MUL_DSILU = 2 };
@@ -164,6 +172,10 @@ template <typename T, typename PT>
 int launch_edge_bwd(const EdgeArgs<T>& a, const PT* phi, const PT* v_in, const T* sb1, const T* vb1, T* phib,
                     T* vb_in, T* fpart, int first_block, __nv_bfloat16* phib16, cudaStream_t st);
 int edge_num_slabs(int F);
+// edge_scatter.cu — the reverse message step in scatter form (atomic adds) for asymmetric edge sets (max-neighbour cap)
+template <typename T, typename PT>
+int launch_edge_bwd_scatter(const EdgeArgs<T>& a, const PT* phi, const PT* v_in, const T* sb1, const T* vb1, T* phib,
+                            T* vb_in, T* fslab, int first_block, cudaStream_t st);
 
 // edge_warp.cu — the FP32 model's edge kernels (warp per receiver, filter rows in registers, no CTA barriers)
 // wt, dt (both or neither): edge tape [E][3][F] that receives the filter value w and dw/dd of every edge; the reverse

@@ -415,6 +415,91 @@ __global__ void check_edges_k(int64_t N, const int32_t* rowptr, int64_t max_edge
   if (over) atomicOr(d_err, ERRF_EDGE_OVERFLOW);
 }
 
+// ---- max-neighbour cap (reading Q16): a receiver keeps its `cap` nearest senders, smallest
+// FP64 squared distance first, ties by sender index, then by lattice shift.  One warp per receiver; the rank of an entry is
+// the number of entries of its row with a smaller key (rows are a few dozen entries long).
+__device__ __forceinline__ double cap_d2(const double* __restrict__ pos, const GridDesc& D, int64_t i, int j,
+                                         const int8_t* __restrict__ sh) {
+  double q = 0.0;
+#pragma unroll
+  for (int b = 0; b < 3; ++b) {
+    const double sc = (double)sh[0] * D.C[0 + b] + (double)sh[1] * D.C[3 + b] + (double)sh[2] * D.C[6 + b];
+    const double r = pos[3 * (int64_t)j + b] - pos[3 * i + b] + sc;
+    q += r * r;
+  }
+  return q;
+}
+__global__ void __launch_bounds__(256) cap_mark_k(int64_t N, int cap, const double* __restrict__ pos,
+                                                  const int32_t* __restrict__ a2s, const GridDesc* __restrict__ desc,
+                                                  const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                                                  const int8_t* __restrict__ shift, uint8_t* __restrict__ keep,
+                                                  int32_t* __restrict__ deg2, int64_t max_edges) {
+  const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (i >= N || (int64_t)rowptr[N] > max_edges) return;
+  const int ea = rowptr[i], eb = rowptr[i + 1], deg = eb - ea;
+  if (lane == 0) deg2[i] = min(deg, cap);
+  if (deg <= cap) {
+    for (int e = ea + lane; e < eb; e += 32) keep[e] = 1;
+    return;
+  }
+  const GridDesc& D = desc[a2s[i]];
+  for (int e = ea + lane; e < eb; e += 32) {
+    const double de = cap_d2(pos, D, i, col[e], shift + 3 * (int64_t)e);
+    int rank = 0;
+    for (int o = ea; o < eb; ++o) {
+      if (o == e) continue;
+      const double dv = cap_d2(pos, D, i, col[o], shift + 3 * (int64_t)o);
+      bool less = dv < de;
+      if (dv == de) {
+        if (col[o] != col[e]) less = col[o] < col[e];
+        else {
+          less = false;
+          for (int b = 0; b < 3; ++b)
+            if (shift[3 * (int64_t)o + b] != shift[3 * (int64_t)e + b]) { less = shift[3 * (int64_t)o + b] < shift[3 * (int64_t)e + b]; break; }
+        }
+      }
+      rank += less ? 1 : 0;
+    }
+    keep[e] = rank < cap ? 1 : 0;
+  }
+}
+// ok[0] = 1 when the uncapped graph fitted (the compaction ran); the primary rowptr is replaced only then
+__global__ void cap_finish_k(int64_t N, const int32_t* rowptr, const int32_t* rowptr2, int64_t max_edges, int32_t* ok) {
+  *ok = ((int64_t)rowptr[N] <= max_edges) ? 1 : 0;
+}
+__global__ void __launch_bounds__(256) cap_rowptr_k(int64_t N, const int32_t* __restrict__ rowptr2, int32_t* rowptr,
+                                                    const int32_t* ok) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i <= N && *ok) rowptr[i] = rowptr2[i];
+}
+template <typename T>
+__global__ void __launch_bounds__(256) cap_compact_k(int64_t N, const int32_t* __restrict__ rowptr,
+                                                     const int32_t* __restrict__ rowptr2, const uint8_t* __restrict__ keep,
+                                                     const int32_t* __restrict__ col, const int8_t* __restrict__ shift,
+                                                     const Geom<T>* __restrict__ geom, int32_t* __restrict__ col2,
+                                                     int8_t* __restrict__ shift2, Geom<T>* __restrict__ geom2,
+                                                     int64_t max_edges) {
+  const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (i >= N || (int64_t)rowptr[N] > max_edges) return;
+  const int ea = rowptr[i], eb = rowptr[i + 1];
+  int out = rowptr2[i];
+  for (int e0 = ea; e0 < eb; e0 += 32) { // stable: kept entries stay in their order
+    const int e = e0 + lane;
+    const bool k = e < eb && keep[e];
+    const unsigned m = __ballot_sync(0xffffffffu, k);
+    if (k) {
+      const int o = out + __popc(m & ((1u << lane) - 1u));
+      col2[o] = col[e];
+      shift2[3 * (int64_t)o] = shift[3 * (int64_t)e]; shift2[3 * (int64_t)o + 1] = shift[3 * (int64_t)e + 1];
+      shift2[3 * (int64_t)o + 2] = shift[3 * (int64_t)e + 2];
+      geom2[o] = geom[e];
+    }
+    out += __popc(m);
+  }
+}
+
 // Order-independent 64-bit checksum of the position array (xor of a mix of (index, bit pattern)).
 __device__ __forceinline__ unsigned long long mix64(unsigned long long x) {
   x ^= x >> 33; x *= 0xff51afd7ed558ccdULL; x ^= x >> 33; x *= 0xc4ceb9fe1a85ec53ULL; x ^= x >> 33;
@@ -436,7 +521,8 @@ __global__ void pos_cmp_k(unsigned long long* chk, int* d_err) {
 } // namespace
 
 int launch_graph_build(const GraphBuffers& gb, int64_t N, int64_t S, const double* pos, const int32_t* sptr,
-                       const double* cell, const uint8_t* pbc, double rc, int prec, int all_images, cudaStream_t st) {
+                       const double* cell, const uint8_t* pbc, double rc, int prec, int all_images, int max_neighbors,
+                       cudaStream_t st) {
   int nl = 0;
   cudaMemsetAsync(gb.d_poschk, 0, 2 * sizeof(unsigned long long), st);
   if (N == 0 || S == 0) {
@@ -478,6 +564,29 @@ int launch_graph_build(const GraphBuffers& gb, int64_t N, int64_t S, const doubl
   }
 #undef PNN_NEIGH
   ++nl;
+  if (max_neighbors > 0 && gb.cap_col) { // keep the nearest max_neighbors senders of every receiver (stable compaction)
+    cap_mark_k<<<nbW, 256, 0, st>>>(N, max_neighbors, pos, gb.a2s, gb.desc, gb.rowptr, gb.col, gb.shift, gb.cap_keep,
+                                    gb.cap_deg, gb.max_edges);
+    PNN_KCHECK("cap_mark_k"); ++nl;
+    nl += exclusive_scan(gb.cap_deg, N, gb.cap_rowptr, gb.scan_tmp, st);
+    const size_t gs = prec == 2 ? sizeof(Geom<double>) : sizeof(Geom<float>);
+    if (prec == 2)
+      cap_compact_k<double><<<nbW, 256, 0, st>>>(N, gb.rowptr, gb.cap_rowptr, gb.cap_keep, gb.col, gb.shift,
+                                                 (const Geom<double>*)gb.geom, gb.cap_col, gb.cap_shift,
+                                                 (Geom<double>*)gb.cap_geom, gb.max_edges);
+    else
+      cap_compact_k<float><<<nbW, 256, 0, st>>>(N, gb.rowptr, gb.cap_rowptr, gb.cap_keep, gb.col, gb.shift,
+                                                (const Geom<float>*)gb.geom, gb.cap_col, gb.cap_shift,
+                                                (Geom<float>*)gb.cap_geom, gb.max_edges);
+    PNN_KCHECK("cap_compact_k"); ++nl;
+    // back into the primary arrays (an overflowing graph was left untouched and stays flagged)
+    cap_finish_k<<<1, 1, 0, st>>>(N, gb.rowptr, gb.cap_rowptr, gb.max_edges, gb.cap_deg + N); PNN_KCHECK("cap_finish_k"); ++nl;
+    cudaMemcpyAsync(gb.col, gb.cap_col, sizeof(int32_t) * gb.max_edges, cudaMemcpyDeviceToDevice, st);
+    cudaMemcpyAsync(gb.shift, gb.cap_shift, 3 * gb.max_edges, cudaMemcpyDeviceToDevice, st);
+    cudaMemcpyAsync(gb.geom, gb.cap_geom, gs * gb.max_edges, cudaMemcpyDeviceToDevice, st);
+    cap_rowptr_k<<<(unsigned)((N + 1 + 255) / 256), 256, 0, st>>>(N, gb.cap_rowptr, gb.rowptr, gb.cap_deg + N);
+    PNN_KCHECK("cap_rowptr_k"); ++nl;
+  }
   return nl;
 }
 

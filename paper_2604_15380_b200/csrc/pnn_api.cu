@@ -59,6 +59,7 @@ bool config_ok(const pnn_config* c) {
   if (c->T < 1 || c->T > 64 || c->K < (c->rbf == PNN_RBF_BESSEL ? 1 : 2) || c->K > 32 || c->H < 1 || c->Zmax < 1) return false;
   if (!(c->cutoff > 0.0) || !(c->norm_eps >= 0.0)) return false;
   if (c->prec != PNN_BF16 && c->prec != PNN_FP32 && c->prec != PNN_FP64) return false;
+  if (c->max_neighbors < 0) return false;
   return true;
 }
 
@@ -337,6 +338,14 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
     g.d_err = (int*)carve(256);
     g.d_ovf = pass ? g.d_err + 1 : nullptr;
     g.d_poschk = pass ? reinterpret_cast<unsigned long long*>(g.d_err + 4) : nullptr;
+    if (m->cfg.max_neighbors > 0) { // scratch of the cap's compaction pass
+      g.cap_col = (int32_t*)carve(4 * E);
+      g.cap_shift = (int8_t*)carve(3 * E);
+      g.cap_geom = carve(4 * es * E);
+      g.cap_keep = (uint8_t*)carve(E);
+      g.cap_deg = (int32_t*)carve(4 * (N + 2));
+      g.cap_rowptr = (int32_t*)carve(4 * (N + 2));
+    }
     g.max_edges = maxE;
     ws->s_cur = carve(es * N * F);
     ws->h = carve(es * N * F);
@@ -421,7 +430,7 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
       }
     }
   }
-  if (m->cfg.prec == PNN_FP32 && want_forces && maxE > 0 && !no_tape) {
+  if (m->cfg.prec == PNN_FP32 && want_forces && maxE > 0 && !no_tape && m->cfg.max_neighbors == 0) {
     // the FP32 edge tape (w and dw/dd of every edge and block): required unless the caller opted out with
     // PNN_WS_NO_EDGE_TAPE; running out of memory is an error, never a silent change of kernels
     const int64_t per_block = 2 * maxE * 3 * F;
@@ -459,7 +468,7 @@ int pnn_build_graph(pnn_workspace* ws, int64_t N, int64_t S, const double* pos, 
   {
     ProfScope ps(ws, st, "graph_build");
     const int nl = launch_graph_build(ws->g, N, S, pos, sptr, cell, pbc, ws->model->cfg.cutoff, ws->model->cfg.prec,
-                                      ws->model->cfg.pbc_images, st);
+                                      ws->model->cfg.pbc_images, ws->model->cfg.max_neighbors, st);
     ws->launches += nl;
     ps.done(nl);
   }
@@ -646,6 +655,12 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
         nl += l_; ps_.done(l_); }
       // R3 + R4
       ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
+      if (c.max_neighbors > 0) { // capped (asymmetric) graph: the scatter form of R3 / R4
+        ProfScope ps_(ws, st, "edge_bwd");
+        const int l_ = launch_edge_bwd_scatter<T, T>(ea, (const T*)tp.phi, (const T*)tp.v_in, sb, vb, t > 0 ? phib : nullptr,
+                                                     t > 0 ? vb2 : nullptr, fpart, last ? 1 : 0, st);
+        nl += l_; ps_.done(l_);
+      } else
       { ProfScope ps_(ws, st, "edge_bwd");
         int l_;
         bool taped_edges = false;
@@ -677,6 +692,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       int nslab = edge_num_slabs(F);
       if constexpr (std::is_same<T, float>::value)
         if (ws->etape != nullptr) nslab = edge_warp_num_slabs(F, c.K);
+      if (c.max_neighbors > 0) nslab = 1;
     const int l_ = launch_force_assemble<T>(N, nslab, fpart, forces, st);
       nl += l_; ps_.done(l_); }
   }
@@ -813,7 +829,7 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       }
     }
     { ProfScope ps_(ws, st, "force_assemble");
-      const int l_ = launch_force_assemble<T>(N, edge_tc_bwd_num_slabs(), fpart, forces, st);
+      const int l_ = launch_force_assemble<T>(N, c.max_neighbors > 0 ? 1 : edge_tc_bwd_num_slabs(), fpart, forces, st);
       nl += l_; ps_.done(l_); }
   }
   ws->launches += nl;

@@ -26,7 +26,7 @@ def make_model(mc: gen.ModelCfg, weights, precision: str, max_atoms: int, max_ed
     return pnn.PaiNN(mc.F, mc.T, mc.K, mc.H, weights, precision=precision, cutoff=mc.cutoff, Zmax=mc.Zmax,
                      norm_eps=mc.norm_eps, max_atoms=max_atoms, max_edges=max_edges, max_structs=max_structs,
                      forces=forces, rbf=getattr(mc, "rbf", "gaussian"),
-                     pbc_images=getattr(mc, "pbc_images", "minimum"))
+                     pbc_images=getattr(mc, "pbc_images", "minimum"), max_neighbors=getattr(mc, "max_neighbors", 0))
 
 
 def run_gpu(mc: gen.ModelCfg, weights, batch: gen.Batch, precision: str, forces: bool = True, max_edges=None,

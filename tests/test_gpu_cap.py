@@ -1,0 +1,69 @@
+"""-m gpu parity of the max-neighbour cap (PAPER.md:231 Table V "Max neighbors 20", :269 "64"): capped edge sets bit-exact
+against the oracle, energies and forces (scatter form of the reverse sweep on the asymmetric edge set) in all precisions."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import gen
+import oracle
+from gpu_common import gpu_edge_set, run_gpu
+from helpers import edge_set, energy_rel_err, force_rel_err
+
+pytestmark = pytest.mark.gpu
+
+
+def _check_graph(b, mc, out):
+    nb = oracle.neighbours(b, mc.cutoff, all_images=(mc.pbc_images == "all"), max_neighbors=mc.max_neighbors)
+    assert np.array_equal(out["rowptr"], nb["rowptr"])
+    assert gpu_edge_set(out["rowptr"], out["col"], out["shift"]) == edge_set(nb)
+    return nb
+
+
+@pytest.mark.parametrize("k", [1, 6, 20, 64])
+def test_capped_graph_bit_exact_molecules(k):
+    mc = dataclasses.replace(gen.model_cfg(2), max_neighbors=k)
+    b = gen.make_batch(2, 0, 12)
+    out = run_gpu(mc, gen.make_weights(mc, 2), b, "fp32", want_graph=True)
+    nb = _check_graph(b, mc, out)
+    assert np.diff(nb["rowptr"]).max() <= k
+
+
+def test_capped_graph_bit_exact_periodic_crystals():
+    mc = dataclasses.replace(gen.model_cfg(3), max_neighbors=20)
+    b = gen.make_batch(3, 0, 2)
+    out = run_gpu(mc, gen.make_weights(mc, 3), b, "fp32", want_graph=True)
+    nb = _check_graph(b, mc, out)
+    assert np.all(np.diff(nb["rowptr"]) == 20)            # ~61 neighbours inside 6 A: every atom is capped
+    es = edge_set(nb)
+    assert any((j, i, -a, -b_, -c) not in es for (i, j, a, b_, c) in es)   # not symmetric
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32", "bf16"])
+def test_capped_values_molecules(precision):
+    mc = dataclasses.replace(gen.model_cfg(2), max_neighbors=8)
+    b = gen.make_batch(2, 5, 10)
+    w = gen.make_weights(mc, 2)
+    ref = oracle.evaluate(mc, w, b)
+    assert ref["n_edges"] < oracle.evaluate(gen.model_cfg(2), w, b, forces=False)["n_edges"]
+    out = run_gpu(mc, w, b, precision)
+    if precision == "bf16":
+        assert np.sqrt(((out["energy"] - ref["energy"]) ** 2).sum() / (ref["energy"] ** 2).sum()) < 2e-2
+        assert np.sqrt(((out["forces"] - ref["forces"]) ** 2).sum() / (ref["forces"] ** 2).sum()) < 2e-2
+    else:
+        te, tf = (1e-10, 1e-10) if precision == "fp64" else (1e-5, 1e-4)
+        assert energy_rel_err(out["energy"], ref["energy"]).max() < te
+        assert force_rel_err(out["forces"], ref["forces"], b.struct_ptr).max() < tf
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_capped_values_crystals_paper_setting(precision):
+    """The paper's periodic setting: 64 neighbours at most — cfg3 crystals have ~61, so some atoms are capped."""
+    mc = dataclasses.replace(gen.model_cfg(3), max_neighbors=56)
+    b = gen.make_batch(3, 3, 2)
+    w = gen.make_weights(mc, 3)
+    ref = oracle.evaluate(mc, w, b)
+    out = run_gpu(mc, w, b, precision)
+    te, tf = (1e-10, 1e-10) if precision == "fp64" else (1e-5, 2e-4)
+    assert energy_rel_err(out["energy"], ref["energy"]).max() < te
+    assert force_rel_err(out["forces"], ref["forces"], b.struct_ptr).max() < tf
