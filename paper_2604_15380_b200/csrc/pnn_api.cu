@@ -816,6 +816,13 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       TcEpi g3; g3.accumulate = last ? 0 : 1; g3.C = vb; g3.ldc = F; g3.Cb = mb.vb16; g3.ldcb = F;
       tc("gemm_3N", 3 * N, F, 2 * F, mb.PQb16, 2 * F, b.UVt, g3);                  // v-bar' += U^T P-bar + V^T Q-bar
       ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
+      if (c.max_neighbors > 0) { // capped (asymmetric) graph: scatter form on the FP32 adjoint streams, BF16 payloads
+        ProfScope ps_(ws, st, "edge_bwd");
+        int l_ = launch_edge_bwd_scatter<T, B>(ea, tp16.phi16, tp16.vin16, sb, vb, t > 0 ? (T*)ws->phib : nullptr,
+                                               t > 0 ? vb2 : nullptr, fpart, last ? 1 : 0, st);
+        if (t > 0) l_ += launch_f32_to_bf16((int64_t)N * 3 * F, (const float*)ws->phib, mb.phib16, st);
+        nl += l_; ps_.done(l_);
+      } else
       { ProfScope ps_(ws, st, "edge_bwd");
           const int l_ = launch_edge_bwd_tc(em, m->d_fltT + (int64_t)t * m->fltT_stride, tp16.phi16, tp16.vin16, mb.sb16,
                                           mb.vb16, vb, t > 0 ? mb.phib16 : nullptr, vb2, fpart, last ? 1 : 0, st);

@@ -64,6 +64,6 @@ def test_capped_values_crystals_paper_setting(precision):
     w = gen.make_weights(mc, 3)
     ref = oracle.evaluate(mc, w, b)
     out = run_gpu(mc, w, b, precision)
-    te, tf = (1e-10, 1e-10) if precision == "fp64" else (1e-5, 2e-4)
+    te, tf = (1e-10, 1e-10) if precision == "fp64" else (1e-5, 1e-3)   # FP32 forces on cfg3: the Q27 bound
     assert energy_rel_err(out["energy"], ref["energy"]).max() < te
     assert force_rel_err(out["forces"], ref["forces"], b.struct_ptr).max() < tf
