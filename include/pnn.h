@@ -63,6 +63,10 @@ typedef struct {
                             squared distance first, ties by sender index, then lattice shift.  The edge set is then not
                             symmetric: the reverse sweep runs its scatter form (atomic adds; edge_scatter.cu) instead of
                             the gather form, and max_edges still bounds the UNCAPPED edge count of a batch. */
+  int32_t n_global; /* global attributes per structure entering the embedding ("global attributes such as charge
+                       and spin used as additional input features"; reading Q30): 0 = none; G > 0 appends
+                       glob_W[F][G] to the weight blob, s0_i = emb[Z_i] + glob_W . attributes of the atom's structure
+                       (pnn_set_globals). */
 } pnn_config;
 
 typedef struct pnn_model pnn_model;         /* opaque; owns device copies of the weights in model precision */
@@ -133,6 +137,12 @@ int pnn_graph_copy(const pnn_workspace* ws, int32_t* rowptr, int32_t* col, int8_
 int pnn_eval(const pnn_model* m, pnn_workspace* ws, int64_t n_atoms, int64_t n_structs, const int32_t* Z,
              const double* pos, const int32_t* struct_ptr, const int32_t* head, int flags, void* energy,
              void* forces, void* cuda_stream);
+
+/* Global attributes of the structures of the NEXT evaluations of this workspace (pnn_config.n_global = G > 0): glob DEVICE
+ * [n_structs, G] f64 (e.g. total charge, spin multiplicity), read by pnn_eval / pnn_eval_blended when they run — the buffer
+ * stays owned by the caller and must stay valid until then; NULL = all attributes zero.  PNN_ERR_INVALID_ARG when the model
+ * has n_global = 0 and glob is not NULL.  pnn_eval_host and the streaming driver evaluate with zero attributes. */
+int pnn_set_globals(pnn_workspace* ws, int64_t n_structs, const double* glob);
 
 /* Blended multi-head evaluation — the paper's inference pipeline (PAPER.md:166-168 branch weights, :371-373 "encoder
  * reuse", "branch skipping", "fused gradient", Fig. 5 at :420): the shared trunk runs ONCE, every

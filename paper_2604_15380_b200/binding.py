@@ -18,7 +18,7 @@ __all__ = [
     "pnn_model_destroy", "pnn_branch_mlp_create", "pnn_branch_mlp_destroy", "pnn_branch_weights",
     "pnn_workspace_create", "pnn_workspace_destroy", "pnn_workspace_bytes", "pnn_workspace_edge_tape_bytes",
     "PNN_WS_FORCES", "PNN_WS_NO_EDGE_TAPE", "pnn_build_graph",
-    "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_eval_blended", "pnn_eval_host", "pnn_stream_create", "pnn_stream_destroy", "pnn_stream_submit", "pnn_stream_wait",
+    "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_set_globals", "pnn_eval_blended", "pnn_eval_host", "pnn_stream_create", "pnn_stream_destroy", "pnn_stream_submit", "pnn_stream_wait",
     "pnn_stream_drain", "pnn_stream_launch_count", "pnn_stream_bytes", "pnn_check_async_errors", "pnn_measure_alu_peak", "pnn_launch_count", "pnn_profile_enable",
     "pnn_profile_read", "pnn_gemm_bf16",
     "PaiNN", "PRECISIONS",
@@ -47,7 +47,7 @@ class pnn_config(ctypes.Structure):
     _fields_ = [("F", ctypes.c_int32), ("T", ctypes.c_int32), ("K", ctypes.c_int32), ("H", ctypes.c_int32),
                 ("Zmax", ctypes.c_int32), ("cutoff", ctypes.c_double), ("norm_eps", ctypes.c_double),
                 ("prec", ctypes.c_int32), ("rbf", ctypes.c_int32), ("pbc_images", ctypes.c_int32),
-                ("max_neighbors", ctypes.c_int32)]
+                ("max_neighbors", ctypes.c_int32), ("n_global", ctypes.c_int32)]
 
 
 def lib_path() -> str:
@@ -83,6 +83,7 @@ def lib():
                                      ctypes.POINTER(i64)]
         L.pnn_graph_copy.argtypes = [vp, vp, vp, vp]
         L.pnn_eval.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, i32, vp, vp, vp]
+        L.pnn_set_globals.argtypes = [vp, i64, vp]
         L.pnn_eval_blended.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, ctypes.c_double, i32, vp, vp, vp]
         L.pnn_eval_host.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp]
         L.pnn_branch_mlp_create.argtypes = [i32, vp, vp, i64, i32, ctypes.POINTER(vp)]
@@ -221,6 +222,10 @@ def pnn_eval(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, struct_p
                           _ptr(forces, None, True), stream), "pnn_eval")
 
 
+def pnn_set_globals(ws: int, n_structs: int, glob) -> None:
+    _check(lib().pnn_set_globals(ws, n_structs, _ptr(glob, "f64", True)), "pnn_set_globals")
+
+
 def pnn_eval_blended(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, struct_ptr, head_weights,
                      skip_below: float, flags: int, energy, forces=None, stream=None):
     _check(lib().pnn_eval_blended(model, ws, n_atoms, n_structs, _ptr(Z, "i32", True), _ptr(pos, "f64", True),
@@ -333,9 +338,10 @@ class PaiNN:
     def __init__(self, F: int, T: int, K: int, H: int, weights: np.ndarray, *, precision: str = "fp32",
                  cutoff: float = 5.0, Zmax: int = 86, norm_eps: float = 1e-8, max_atoms: int, max_edges: int,
                  max_structs: int, forces: bool = True, rbf: str = "gaussian", pbc_images: str = "minimum",
-                 edge_tape: bool = True, max_neighbors: int = 0):
+                 edge_tape: bool = True, max_neighbors: int = 0, n_global: int = 0):
         self.cfg = pnn_config(F, T, K, H, Zmax, cutoff, norm_eps, PRECISIONS[precision],
-                              {"gaussian": 0, "bessel": 1}[rbf], {"minimum": 0, "all": 1}[pbc_images], int(max_neighbors))
+                              {"gaussian": 0, "bessel": 1}[rbf], {"minimum": 0, "all": 1}[pbc_images], int(max_neighbors),
+                              int(n_global))
         self.precision = precision
         self.want_forces = bool(forces)
         self.model = pnn_model_create(self.cfg, weights)
@@ -394,12 +400,16 @@ class PaiNN:
         pnn_graph_copy(self.ws, rowptr, col, shift)
         return rowptr, col, shift
 
-    def eval(self, Z, pos, struct_ptr, head, cell=None, pbc=None, forces: Optional[bool] = None, build: bool = True):
-        """CUDA tensors in, CUDA tensors out: (energy [S], forces [N,3] or None)."""
+    def eval(self, Z, pos, struct_ptr, head, cell=None, pbc=None, forces: Optional[bool] = None, build: bool = True,
+             globals_=None):
+        """CUDA tensors in, CUDA tensors out: (energy [S], forces [N,3] or None).  globals_: [S, n_global] f64 CUDA tensor
+        of global attributes (charge, spin), or None."""
         import torch
         forces = self.want_forces if forces is None else forces
         N, S = int(Z.shape[0]), int(head.shape[0])
         self._last_N = N
+        if self.cfg.n_global > 0:
+            pnn_set_globals(self.ws, S, globals_)
         if build:
             self.build_graph(pos, struct_ptr, cell, pbc)
         energy = torch.empty(S, dtype=self.out_dtype, device=pos.device)

@@ -192,6 +192,10 @@ int edge_warp_num_slabs(int F, int K);
 template <typename T>
 int launch_embed(int64_t N, int F, int Zmax, const int32_t* Z, const T* emb, T* s, int* d_err, cudaStream_t st,
                  __nv_bfloat16* s16 = nullptr);
+// s[i][f] += sum_q globW[f][q] glob[a2s[i]][q] (global attributes: charge, spin; reading Q30); s16: BF16 copy rewritten
+template <typename T>
+int launch_embed_globals(int64_t N, int F, int G, const int32_t* a2s, const double* glob, const T* globW, T* s,
+                         __nv_bfloat16* s16, cudaStream_t st);
 // IT: storage type of P | Q and of the gate values a (= T, or BF16 in the BF16 model)
 template <typename T, typename IT>
 int launch_norm(int64_t N, int F, const IT* PQ, T* sn, T eps, cudaStream_t st, __nv_bfloat16* sn16 = nullptr);

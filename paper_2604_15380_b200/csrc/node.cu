@@ -35,6 +35,21 @@ __global__ void __launch_bounds__(256) embed_k(int64_t N, int F, int Zmax, const
   if (s16) s16[idx] = __float2bfloat16_rn((float)e);
 }
 
+template <typename T>
+__global__ void __launch_bounds__(256) embed_globals_k(int64_t N, int F, int G, const int32_t* __restrict__ a2s,
+                                                       const double* __restrict__ glob, const T* __restrict__ globW,
+                                                       T* __restrict__ s, __nv_bfloat16* __restrict__ s16) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= N * F) return;
+  const int64_t i = idx / F;
+  const int f = (int)(idx % F);
+  const double* gq = glob + (int64_t)a2s[i] * G;
+  T acc = s[idx];
+  for (int q = 0; q < G; ++q) acc += globW[(int64_t)f * G + q] * (T)gq[q];
+  s[idx] = acc;
+  if (s16) s16[idx] = __float2bfloat16_rn((float)acc);
+}
+
 // FP32: four features per thread (16-byte loads / stores, 8-byte BF16 copy)
 __global__ void __launch_bounds__(256) embed4_k(int64_t N, int F4, int Zmax, const int32_t* __restrict__ Z,
                                                 const float4* __restrict__ emb, float4* __restrict__ s, int* d_err,
@@ -708,6 +723,15 @@ inline unsigned nblk(int64_t n, int b) { return (unsigned)((n + b - 1) / b); }
 } // namespace
 
 template <typename T>
+int launch_embed_globals(int64_t N, int F, int G, const int32_t* a2s, const double* glob, const T* globW, T* s,
+                         __nv_bfloat16* s16, cudaStream_t st) {
+  if (N == 0) return 0;
+  embed_globals_k<T><<<nblk(N * F, 256), 256, 0, st>>>(N, F, G, a2s, glob, globW, s, s16);
+  PNN_KCHECK("embed_globals_k");
+  return 1;
+}
+
+template <typename T>
 int launch_embed(int64_t N, int F, int Zmax, const int32_t* Z, const T* emb, T* s, int* d_err, cudaStream_t st,
                  __nv_bfloat16* s16) {
   if (N == 0) return 0;
@@ -858,7 +882,9 @@ int launch_force_assemble(int64_t N, int nslab, const T* fpart, T* forces, cudaS
                                            const T*, T*, cudaStream_t);                                              \
   template int launch_readout_bwd<T>(int64_t, int, int, const T*, const int32_t*, const int32_t*, const T*,          \
                                      const T*, T*, cudaStream_t);                                                    \
-  template int launch_force_assemble<T>(int64_t, int, const T*, T*, cudaStream_t);
+  template int launch_force_assemble<T>(int64_t, int, const T*, T*, cudaStream_t);                                  \
+  template int launch_embed_globals<T>(int64_t, int, int, const int32_t*, const double*, const T*, T*,              \
+                                       __nv_bfloat16*, cudaStream_t);
 #define PNN_INST2(T, IT)                                                                                             \
   template int launch_norm<T, IT>(int64_t, int, const IT*, T*, T, cudaStream_t, __nv_bfloat16*);                     \
   template int launch_update<T, IT>(int64_t, int, const T*, const T*, const IT*, const IT*, T*, T*, cudaStream_t,    \

@@ -59,7 +59,7 @@ bool config_ok(const pnn_config* c) {
   if (c->T < 1 || c->T > 64 || c->K < (c->rbf == PNN_RBF_BESSEL ? 1 : 2) || c->K > 32 || c->H < 1 || c->Zmax < 1) return false;
   if (!(c->cutoff > 0.0) || !(c->norm_eps >= 0.0)) return false;
   if (c->prec != PNN_BF16 && c->prec != PNN_FP32 && c->prec != PNN_FP64) return false;
-  if (c->max_neighbors < 0) return false;
+  if (c->max_neighbors < 0 || c->n_global < 0 || c->n_global > 16) return false;
   return true;
 }
 
@@ -67,7 +67,7 @@ int64_t weights_count(const pnn_config* c) {
   const int64_t F = c->F, K = c->K;
   const int64_t per_block = 11 * F * F + 3 * F * K + 11 * F;
   const int64_t per_head = (F / 2) * F + (F / 2) + (F / 2) + 1;
-  return (int64_t)(c->Zmax + 1) * F + c->T * per_block + c->H * per_head;
+  return (int64_t)(c->Zmax + 1) * F + c->T * per_block + c->H * per_head + F * (int64_t)c->n_global;
 }
 
 // element offsets of one block's arrays inside the device weight buffer
@@ -84,6 +84,7 @@ struct pnn_model {
   int64_t n_elem = 0;
   int64_t emb = 0;
   std::vector<BlockW> blk;
+  int64_t globW = 0;                                    // [F][n_global] (global attributes -> embedding)
   int64_t oW1t = 0, oW1 = 0, ob1 = 0, ow2 = 0, ob2 = 0; // heads: [H][F][Fh], [H][Fh][F], [H][Fh], [H][Fh], [H]
   __nv_bfloat16* d_wb = nullptr;                        // BF16 copy of d_w (same offsets): tcgen05 GEMM operands
   __nv_bfloat16* d_fltT = nullptr;                      // BF16 model: per block, the filter image of edge_tc.cu
@@ -102,6 +103,7 @@ struct pnn_workspace {
   int64_t launches = 0;
   // activations (element type = model state type)
   void *s_cur, *h, *sn, *v1, *k, *vping[2], *eatom, *opre;
+  const double* glob = nullptr;            // global attributes of the next evaluations (pnn_set_globals), DEVICE [S][G]
   unsigned long long* head_mask = nullptr; // BF16 readout GEMM: heads present per 128-row tile
   void* opre_all = nullptr; // blended readout: pre-activations of every head [N][H][F/2] (reverse sweep)
   struct Tape { void *v_in, *hpre, *phi, *PQ, *kpre, *a; };
@@ -250,6 +252,7 @@ int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, 
       for (int64_t o = 0; o < Fh; ++o) { hb[m->ob1 + h * Fh + o] = b1[o]; hb[m->ow2 + h * Fh + o] = w2[o]; }
       hb[m->ob2 + h] = b2[0];
     }
+    if (cfg->n_global > 0) m->globW = put(take(F * cfg->n_global), F * cfg->n_global);
   }
   m->n_elem = (int64_t)hb.size();
   const size_t es = elem_size(cfg->prec);
@@ -563,7 +566,9 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
   const bool taped = ws->want_forces != 0;
 
   { ProfScope ps_(ws, st, "embed");
-  const int l_ = launch_embed<T>(N, F, c.Zmax, Z, W + m->emb, s_cur, ws->g.d_err, st);
+  int l_ = launch_embed<T>(N, F, c.Zmax, Z, W + m->emb, s_cur, ws->g.d_err, st);
+    if (c.n_global > 0 && ws->glob)
+      l_ += launch_embed_globals<T>(N, F, c.n_global, ws->g.a2s, ws->glob, W + m->globW, s_cur, nullptr, st);
     nl += l_; ps_.done(l_); }
   for (int t = 0; t < T_; ++t) {
     const BlockW& b = m->blk[t];
@@ -733,7 +738,9 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
   };
 
   { ProfScope ps_(ws, st, "embed");
-    const int l_ = launch_embed<T>(N, F, c.Zmax, Z, W + m->emb, s_cur, ws->g.d_err, st, mb.s16);
+    int l_ = launch_embed<T>(N, F, c.Zmax, Z, W + m->emb, s_cur, ws->g.d_err, st, mb.s16);
+    if (c.n_global > 0 && ws->glob)
+      l_ += launch_embed_globals<T>(N, F, c.n_global, ws->g.a2s, ws->glob, W + m->globW, s_cur, mb.s16, st);
     nl += l_; ps_.done(l_); }
   for (int t = 0; t < T_; ++t) {
     const BlockW& b = m->blk[t];
@@ -880,6 +887,13 @@ int pnn_eval(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const 
   return rc;
 }
 
+int pnn_set_globals(pnn_workspace* ws, int64_t S, const double* glob) {
+  if (!ws || S < 0 || S > ws->maxS) return PNN_ERR_INVALID_ARG;
+  if (glob && ws->model->cfg.n_global == 0) return PNN_ERR_INVALID_ARG;
+  ws->glob = glob;
+  return PNN_OK;
+}
+
 int pnn_eval_blended(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const double* pos,
                      const int32_t* sptr, const void* head_weights, double skip_below, int flags, void* energy,
                      void* forces, void* stream) {
@@ -994,6 +1008,7 @@ static int enqueue_host_batch(const pnn_model* m, pnn_workspace* ws, int64_t N, 
   int rc = pnn_build_graph(ws, N, S, ws->st_pos, ws->st_sptr, periodic ? ws->st_cell : nullptr,
                            periodic ? ws->st_pbc : nullptr, stream);
   if (rc != PNN_OK) return rc;
+  ws->glob = nullptr; // the host entry points evaluate with zero global attributes
   rc = eval_common(m, ws, N, S, ws->st_Z, ws->st_sptr, ws->st_head, nullptr, 0.0, flags, ws->st_energy, ws->st_forces,
                    stream);
   if (rc != PNN_OK) return rc;

@@ -26,11 +26,12 @@ def make_model(mc: gen.ModelCfg, weights, precision: str, max_atoms: int, max_ed
     return pnn.PaiNN(mc.F, mc.T, mc.K, mc.H, weights, precision=precision, cutoff=mc.cutoff, Zmax=mc.Zmax,
                      norm_eps=mc.norm_eps, max_atoms=max_atoms, max_edges=max_edges, max_structs=max_structs,
                      forces=forces, rbf=getattr(mc, "rbf", "gaussian"),
-                     pbc_images=getattr(mc, "pbc_images", "minimum"), max_neighbors=getattr(mc, "max_neighbors", 0))
+                     pbc_images=getattr(mc, "pbc_images", "minimum"), max_neighbors=getattr(mc, "max_neighbors", 0),
+                     n_global=getattr(mc, "n_global", 0))
 
 
 def run_gpu(mc: gen.ModelCfg, weights, batch: gen.Batch, precision: str, forces: bool = True, max_edges=None,
-            want_graph: bool = False):
+            want_graph: bool = False, globals_=None):
     """Returns dict(energy, forces, [rowptr, col, shift]) as numpy arrays."""
     import torch
     if max_edges is None:
@@ -38,7 +39,8 @@ def run_gpu(mc: gen.ModelCfg, weights, batch: gen.Batch, precision: str, forces:
     net = make_model(mc, weights, precision, max(batch.n_atoms, 1), max_edges, max(batch.n_structs, 1), forces)
     try:
         t = to_device(batch)
-        e, f = net.eval(t["Z"], t["pos"], t["struct_ptr"], t["head"], t["cell"], t["pbc"], forces=forces)
+        gl = None if globals_ is None else torch.from_numpy(np.ascontiguousarray(globals_, np.float64)).cuda()
+        e, f = net.eval(t["Z"], t["pos"], t["struct_ptr"], t["head"], t["cell"], t["pbc"], forces=forces, globals_=gl)
         torch.cuda.synchronize()
         net.check()
         out = dict(energy=e.cpu().numpy().astype(np.float64),
