@@ -172,7 +172,8 @@ def measured_traffic(workload: str, family: str):
             for line in fh:
                 q = line.strip().split(",")
                 if len(q) >= 4 and q[0] == workload and q[1] == family:
-                    return int(q[2]), f"{TRAFFIC_FILE}: ncu --set full capture of {q[3]} (dram__bytes_read.sum + dram__bytes_write.sum, constant, not measured in this run)"
+                    return int(q[2]), (f"{TRAFFIC_FILE}: ncu --set full capture of {','.join(q[3:])} (dram__bytes_read.sum + "
+                                       "dram__bytes_write.sum; a constant of that capture, not measured in this run)")
     except Exception:
         pass
     return None, None
