@@ -80,6 +80,9 @@ class ModelCfg:
     rbf: str = "gaussian"   # or "bessel" (the paper's lead model uses 4 Bessel functions)
     max_neighbors: int = 0  # > 0: every receiver keeps its nearest max_neighbors senders ("Max neighbors 20")
     n_global: int = 0       # global attributes per structure (charge, spin: PAPER.md:58) entering the embedding
+    head_type: str = "atomwise"  # or "pooled": the paper's graph-level head, mean pool -> 2 shared
+    head_d1: int = 50            # layers of width head_d1 -> per head 2 layers of width head_d2 -> 1
+    head_d2: int = 776
 
 
 @dataclasses.dataclass
@@ -155,7 +158,15 @@ def weights_layout(mc: ModelCfg):
         add(f"b{t}.upd_c1", (F,), 2 * F)
         add(f"b{t}.upd_A2", (3 * F, F), F)
         add(f"b{t}.upd_c2", (3 * F,), F)
-    for h in range(H):
+    if getattr(mc, "head_type", "atomwise") == "pooled":
+        d1, d2 = mc.head_d1, mc.head_d2
+        add("pool.W1", (d1, F), F); add("pool.b1", (d1,), F)
+        add("pool.W2", (d1, d1), d1); add("pool.b2", (d1,), d1)
+        for h in range(H):
+            add(f"h{h}.br_W1", (d2, d1), d1); add(f"h{h}.br_b1", (d2,), d1)
+            add(f"h{h}.br_W2", (d2, d2), d2); add(f"h{h}.br_b2", (d2,), d2)
+            add(f"h{h}.br_w3", (d2,), d2); add(f"h{h}.br_b3", (1,), d2)
+    for h in range(H if getattr(mc, "head_type", "atomwise") != "pooled" else 0):
         add(f"h{h}.out_W1", (F // 2, F), F)
         add(f"h{h}.out_b1", (F // 2,), F)
         add(f"h{h}.out_w2", (F // 2,), F // 2)

@@ -51,7 +51,8 @@ def _cfg_arrays(mc):
     rbf = {"gaussian": 0, "bessel": 1}[getattr(mc, "rbf", "gaussian")]
     images = {"minimum": 0, "all": 1}[getattr(mc, "pbc_images", "minimum")]
     ic = np.array([mc.F, mc.T, mc.K, mc.H, mc.Zmax, rbf, images, int(getattr(mc, "max_neighbors", 0)),
-                   int(getattr(mc, "n_global", 0))], np.int32)
+                   int(getattr(mc, "n_global", 0)), {"atomwise": 0, "pooled": 1}[getattr(mc, "head_type", "atomwise")],
+                   int(getattr(mc, "head_d1", 50)), int(getattr(mc, "head_d2", 776))], np.int32)
     dc = np.array([mc.cutoff, mc.norm_eps], np.float64)
     return ic, dc
 

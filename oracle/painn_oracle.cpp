@@ -59,13 +59,21 @@ inline double value_of(double a) { return a; }
 inline double value_of(Dual a) { return a.v; }
 
 // ------------------------------------------------------------------ model = views into the blob
-struct Cfg { int F, T, K, H, Zmax; double rc, eps; int rbf; int images; int max_nb; int n_glob; };  // rbf: 0 Gaussian, 1 Bessel; images: 0 minimum image, 1 all; max_nb: 0 = no cap; n_glob: global attributes per structure
+struct Cfg { int F, T, K, H, Zmax; double rc, eps; int rbf; int images; int max_nb; int n_glob; int head_type, d1, d2; };  // rbf: 0 Gaussian, 1 Bessel; images: 0 minimum image, 1 all; max_nb: 0 = no cap; n_glob: global attributes per structure
 struct Block {
   const double *msg_W1, *msg_b1, *msg_W2, *msg_b2, *flt_W, *flt_b;
   const double *upd_U, *upd_V, *upd_A1, *upd_c1, *upd_A2, *upd_c2;
 };
 struct Head { const double *W1, *b1, *w2, *b2; };
-struct Model { Cfg c; const double* emb; std::vector<Block> blk; std::vector<Head> head; const double* glob_W; };
+// Pooled graph-level head of the paper's lead model ("Output heads 16 (graph-level)", "2 shared layers
+// (dim 50) + 2 branch layers (dim 776)"; reading Q29): x_g = mean_i s_i, two shared Linear+SiLU layers of width
+// d1, then per head two Linear+SiLU layers of width d2 and a linear output.
+struct PoolShared { const double *W1, *b1, *W2, *b2; };                 // [d1][F], [d1], [d1][d1], [d1]
+struct PoolBranch { const double *W1, *b1, *W2, *b2, *w3, *b3; };       // [d2][d1], [d2], [d2][d2], [d2], [d2], [1]
+struct Model {
+  Cfg c; const double* emb; std::vector<Block> blk; std::vector<Head> head; const double* glob_W;
+  PoolShared ps; std::vector<PoolBranch> pb;
+};
 
 // Blob order: SURVEY.md §8(b) "Weight blob"; matrices row-major [out][in], y = W x + b.
 long parse_blob(const Cfg& c, const double* w, Model* m) {
@@ -85,6 +93,17 @@ long parse_blob(const Cfg& c, const double* w, Model* m) {
     b.upd_A2 = take(3 * F * F); b.upd_c2 = take(3 * F);
     if (m) m->blk[t] = b;
   }
+  if (c.head_type == 1) {
+    const long d1 = c.d1, d2 = c.d2;
+    PoolShared ps;
+    ps.W1 = take(d1 * F); ps.b1 = take(d1); ps.W2 = take(d1 * d1); ps.b2 = take(d1);
+    if (m) { m->ps = ps; m->pb.resize(c.H); }
+    for (int h = 0; h < c.H; ++h) {
+      PoolBranch b;
+      b.W1 = take(d2 * d1); b.b1 = take(d2); b.W2 = take(d2 * d2); b.b2 = take(d2); b.w3 = take(d2); b.b3 = take(1);
+      if (m) m->pb[h] = b;
+    }
+  } else
   for (int h = 0; h < c.H; ++h) {
     Head hd;
     hd.W1 = take((F / 2) * F); hd.b1 = take(F / 2); hd.w2 = take(F / 2); hd.b2 = take(1);
@@ -265,6 +284,7 @@ template <class S> struct Tape {
   std::vector<S> s_out, v_out;     // final features
   std::vector<S> opre;             // readout pre-activation [N][F/2]
   std::vector<S> eatom;            // per-atom energy
+  std::vector<S> pool_pre;         // pooled head: pre-activations per structure [S][2 d1 + 2 d2]
 };
 
 // ------------------------------------------------------------------ forward (B2..B5)
@@ -395,6 +415,27 @@ void forward(const Model& m, int N, int nS, const int32_t* Z, const S* pos, cons
   }
   tp.s_out = s; tp.v_out = v;
 
+  if (m.c.head_type == 1) {   // pooled graph-level head (reading Q29)
+    const int d1 = m.c.d1, d2 = m.c.d2, W = 2 * d1 + 2 * d2;
+    tp.pool_pre.assign((long)nS * W, S(0.0)); tp.eatom.assign(N, S(0.0)); tp.opre.clear();
+    for (int g = 0; g < nS; ++g) {
+      const int n = sptr[g + 1] - sptr[g];
+      std::vector<S> x(F, S(0.0)), y1(d1), y2(d1), z1(d2), z2(d2);
+      for (int i = sptr[g]; i < sptr[g + 1]; ++i)
+        for (int f = 0; f < F; ++f) x[f] += s[(long)i * F + f];
+      if (n > 0) for (int f = 0; f < F; ++f) x[f] = x[f] / S((double)n);          // mean over the structure's atoms
+      S* pre = tp.pool_pre.data() + (long)g * W;
+      const PoolBranch& b = m.pb[head[g]];
+      for (int o = 0; o < d1; ++o) { S a = S(m.ps.b1[o]); for (int k = 0; k < F; ++k) a += S(m.ps.W1[(long)o * F + k]) * x[k]; pre[o] = a; y1[o] = silu(a); }
+      for (int o = 0; o < d1; ++o) { S a = S(m.ps.b2[o]); for (int k = 0; k < d1; ++k) a += S(m.ps.W2[(long)o * d1 + k]) * y1[k]; pre[d1 + o] = a; y2[o] = silu(a); }
+      for (int o = 0; o < d2; ++o) { S a = S(b.b1[o]); for (int k = 0; k < d1; ++k) a += S(b.W1[(long)o * d1 + k]) * y2[k]; pre[2 * d1 + o] = a; z1[o] = silu(a); }
+      for (int o = 0; o < d2; ++o) { S a = S(b.b2[o]); for (int k = 0; k < d2; ++k) a += S(b.W2[(long)o * d2 + k]) * z1[k]; pre[2 * d1 + d2 + o] = a; z2[o] = silu(a); }
+      S Eg = S(b.b3[0]);
+      for (int o = 0; o < d2; ++o) Eg += S(b.w3[o]) * z2[o];
+      energy[g] = Eg;
+    }
+    return;
+  }
   // B5 readout: eps_i = out_w2 . silu(out_W1 s_i + out_b1) + out_b2 with the structure's head; E_g = sum_i eps_i
   const int Fh = F / 2;
   tp.opre.assign((long)N * Fh, S(0.0)); tp.eatom.assign(N, S(0.0));
@@ -439,6 +480,23 @@ void reverse(const Model& m, int N, int nS, const int32_t* sptr, const int32_t* 
   // R1 readout: p-bar = out_w2 . silu'(pre) ; s-bar_i = out_W1^T p-bar ; v-bar_i = 0
   std::vector<int> sof(N, 0);
   for (int g = 0; g < nS; ++g) for (int i = sptr[g]; i < sptr[g + 1]; ++i) sof[i] = g;
+  if (m.c.head_type == 1) {   // pooled head: back through the branch and shared layers to x-bar_g; s-bar_i = x-bar_g / n_g
+    const int d1 = m.c.d1, d2 = m.c.d2, W = 2 * d1 + 2 * d2;
+    for (int g = 0; g < nS; ++g) {
+      const int n = sptr[g + 1] - sptr[g];
+      if (n == 0) continue;
+      const double* pre = tp.pool_pre.data() + (long)g * W;
+      const PoolBranch& b = m.pb[head[g]];
+      std::vector<double> z2b(d2), z1b(d2), y2b(d1), y1b(d1), xb(F);
+      for (int o = 0; o < d2; ++o) z2b[o] = b.w3[o] * dsilu(pre[2 * d1 + d2 + o]);
+      for (int k = 0; k < d2; ++k) { double a = 0.0; for (int o = 0; o < d2; ++o) a += b.W2[(long)o * d2 + k] * z2b[o]; z1b[k] = a * dsilu(pre[2 * d1 + k]); }
+      for (int k = 0; k < d1; ++k) { double a = 0.0; for (int o = 0; o < d2; ++o) a += b.W1[(long)o * d1 + k] * z1b[o]; y2b[k] = a * dsilu(pre[d1 + k]); }
+      for (int k = 0; k < d1; ++k) { double a = 0.0; for (int o = 0; o < d1; ++o) a += m.ps.W2[(long)o * d1 + k] * y2b[o]; y1b[k] = a * dsilu(pre[k]); }
+      for (int k = 0; k < F; ++k) { double a = 0.0; for (int o = 0; o < d1; ++o) a += m.ps.W1[(long)o * F + k] * y1b[o]; xb[k] = a; }
+      for (int i = sptr[g]; i < sptr[g + 1]; ++i)
+        for (int k = 0; k < F; ++k) sb[(long)i * F + k] = xb[k] / (double)n;
+    }
+  } else {
 #pragma omp parallel for schedule(static)
   for (int i = 0; i < N; ++i) {
     const Head& hd = m.head[head[sof[i]]];
@@ -446,6 +504,7 @@ void reverse(const Model& m, int N, int nS, const int32_t* sptr, const int32_t* 
       const double pb = hd.w2[o] * dsilu(tp.opre[(long)i * Fh + o]);
       for (int k = 0; k < F; ++k) sb[(long)i * F + k] += hd.W1[(long)o * F + k] * pb;
     }
+  }
   }
 
   for (int t = T - 1; t >= 0; --t) {
@@ -572,7 +631,7 @@ void reverse(const Model& m, int N, int nS, const int32_t* sptr, const int32_t* 
 }
 
 Cfg make_cfg(const int32_t* ic, const double* dc) {
-  return Cfg{ic[0], ic[1], ic[2], ic[3], ic[4], dc[0], dc[1], ic[5], ic[6], ic[7], ic[8]};
+  return Cfg{ic[0], ic[1], ic[2], ic[3], ic[4], dc[0], dc[1], ic[5], ic[6], ic[7], ic[8], ic[9], ic[10], ic[11]};
 }
 
 }  // namespace
