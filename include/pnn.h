@@ -51,6 +51,8 @@ typedef enum { PNN_BF16 = 0, PNN_FP32 = 1, PNN_FP64 = 2 } pnn_precision;
 #define PNN_IMAGES_ALL 1     /* every periodic image inside the cutoff, an atom's own images included (narrow cells)     */
 #define PNN_RBF_GAUSSIAN 0 /* g_k(d) = exp(-gamma (d - k r_c/(K-1))^2), gamma = (K-1)^2 / (2 r_c^2), k = 0..K-1 (2 <= K) */
 #define PNN_RBF_BESSEL 1   /* b_n(d) = sqrt(2/r_c) sin(n pi d / r_c) / d, n = 1..K (the lead model's basis)  */
+#define PNN_HEAD_ATOMWISE 0 /* per-atom readout MLP of the structure's head, summed over the atoms      */
+#define PNN_HEAD_POOLED 1   /* mean pooling, shared layers, per-head branch layers (the paper's graph-level heads)         */
 typedef struct {
   int32_t F, T, K, H, Zmax;
   double cutoff;
@@ -67,6 +69,15 @@ typedef struct {
                        and spin used as additional input features"; reading Q30): 0 = none; G > 0 appends
                        glob_W[F][G] to the weight blob, s0_i = emb[Z_i] + glob_W . attributes of the atom's structure
                        (pnn_set_globals). */
+  int32_t head_type; /* PNN_HEAD_ATOMWISE (0): E_g = sum_i MLP_h(s_i), the blob's heads as listed above.
+                        PNN_HEAD_POOLED (1): the paper's graph-level heads ("Output heads 16 (graph-level)",
+                        "2 shared layers (dim 50) + 2 branch layers (dim 776)"; reading Q29): x_g = mean_i s_i,
+                        y = silu(P2 silu(P1 x_g + p1) + p2), z = silu(B2_h silu(B1_h y + q1_h) + q2_h), E_g = w3_h . z + q3_h.
+                        The blob then holds, in place of the atom-wise heads: P1[d1][F] p1[d1] P2[d1][d1] p2[d1], then per
+                        head B1[d2][d1] q1[d2] B2[d2][d2] q2[d2] w3[d2] q3[1].  pnn_eval_blended returns PNN_ERR_UNSUPPORTED
+                        for such a model. */
+  int32_t head_d1;   /* pooled head: width of the two shared layers (paper: 50); ignored for atom-wise heads */
+  int32_t head_d2;   /* pooled head: width of the two branch layers (paper: 776) */
 } pnn_config;
 
 typedef struct pnn_model pnn_model;         /* opaque; owns device copies of the weights in model precision */

@@ -47,7 +47,8 @@ class pnn_config(ctypes.Structure):
     _fields_ = [("F", ctypes.c_int32), ("T", ctypes.c_int32), ("K", ctypes.c_int32), ("H", ctypes.c_int32),
                 ("Zmax", ctypes.c_int32), ("cutoff", ctypes.c_double), ("norm_eps", ctypes.c_double),
                 ("prec", ctypes.c_int32), ("rbf", ctypes.c_int32), ("pbc_images", ctypes.c_int32),
-                ("max_neighbors", ctypes.c_int32), ("n_global", ctypes.c_int32)]
+                ("max_neighbors", ctypes.c_int32), ("n_global", ctypes.c_int32), ("head_type", ctypes.c_int32),
+                ("head_d1", ctypes.c_int32), ("head_d2", ctypes.c_int32)]
 
 
 def lib_path() -> str:
@@ -338,10 +339,11 @@ class PaiNN:
     def __init__(self, F: int, T: int, K: int, H: int, weights: np.ndarray, *, precision: str = "fp32",
                  cutoff: float = 5.0, Zmax: int = 86, norm_eps: float = 1e-8, max_atoms: int, max_edges: int,
                  max_structs: int, forces: bool = True, rbf: str = "gaussian", pbc_images: str = "minimum",
-                 edge_tape: bool = True, max_neighbors: int = 0, n_global: int = 0):
+                 edge_tape: bool = True, max_neighbors: int = 0, n_global: int = 0, head_type: str = "atomwise",
+                 head_d1: int = 50, head_d2: int = 776):
         self.cfg = pnn_config(F, T, K, H, Zmax, cutoff, norm_eps, PRECISIONS[precision],
                               {"gaussian": 0, "bessel": 1}[rbf], {"minimum": 0, "all": 1}[pbc_images], int(max_neighbors),
-                              int(n_global))
+                              int(n_global), {"atomwise": 0, "pooled": 1}[head_type], int(head_d1), int(head_d2))
         self.precision = precision
         self.want_forces = bool(forces)
         self.model = pnn_model_create(self.cfg, weights)

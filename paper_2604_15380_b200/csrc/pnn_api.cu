@@ -60,14 +60,20 @@ bool config_ok(const pnn_config* c) {
   if (!(c->cutoff > 0.0) || !(c->norm_eps >= 0.0)) return false;
   if (c->prec != PNN_BF16 && c->prec != PNN_FP32 && c->prec != PNN_FP64) return false;
   if (c->max_neighbors < 0 || c->n_global < 0 || c->n_global > 16) return false;
+  if (c->head_type != PNN_HEAD_ATOMWISE && c->head_type != PNN_HEAD_POOLED) return false;
+  if (c->head_type == PNN_HEAD_POOLED && !pool_head_supported(c->F, c->head_d1, c->head_d2, c->H, c->prec == PNN_FP64 ? 8 : 4))
+    return false;
   return true;
 }
 
 int64_t weights_count(const pnn_config* c) {
   const int64_t F = c->F, K = c->K;
   const int64_t per_block = 11 * F * F + 3 * F * K + 11 * F;
-  const int64_t per_head = (F / 2) * F + (F / 2) + (F / 2) + 1;
-  return (int64_t)(c->Zmax + 1) * F + c->T * per_block + c->H * per_head + F * (int64_t)c->n_global;
+  const int64_t d1 = c->head_d1, d2 = c->head_d2;
+  const int64_t heads = c->head_type == PNN_HEAD_POOLED
+                            ? d1 * F + d1 + d1 * d1 + d1 + c->H * (d2 * d1 + d2 + d2 * d2 + d2 + d2 + 1)
+                            : c->H * ((F / 2) * F + (F / 2) + (F / 2) + 1);
+  return (int64_t)(c->Zmax + 1) * F + c->T * per_block + heads + F * (int64_t)c->n_global;
 }
 
 // element offsets of one block's arrays inside the device weight buffer
@@ -86,6 +92,7 @@ struct pnn_model {
   std::vector<BlockW> blk;
   int64_t globW = 0;                                    // [F][n_global] (global attributes -> embedding)
   int64_t oW1t = 0, oW1 = 0, ob1 = 0, ow2 = 0, ob2 = 0; // heads: [H][F][Fh], [H][Fh][F], [H][Fh], [H][Fh], [H]
+  int64_t pP1 = 0, pp1 = 0, pP2 = 0, pp2 = 0, pbr = 0, pbr_stride = 0; // pooled head (pool_head.cu), original [out][in]
   __nv_bfloat16* d_wb = nullptr;                        // BF16 copy of d_w (same offsets): tcgen05 GEMM operands
   __nv_bfloat16* d_fltT = nullptr;                      // BF16 model: per block, the filter image of edge_tc.cu
   int64_t fltT_stride = 0;
@@ -104,6 +111,7 @@ struct pnn_workspace {
   // activations (element type = model state type)
   void *s_cur, *h, *sn, *v1, *k, *vping[2], *eatom, *opre;
   const double* glob = nullptr;            // global attributes of the next evaluations (pnn_set_globals), DEVICE [S][G]
+  void* pool_scratch = nullptr;            // pooled head: x, x-bar, head permutation, tile table
   unsigned long long* head_mask = nullptr; // BF16 readout GEMM: heads present per 128-row tile
   void* opre_all = nullptr; // blended readout: pre-activations of every head [N][H][F/2] (reverse sweep)
   struct Tape { void *v_in, *hpre, *phi, *PQ, *kpre, *a; };
@@ -237,7 +245,14 @@ int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, 
     b.A2t = put_t(A2, 3 * F, F); b.c2 = put(c2, 3 * F);
     b.A2 = put(A2, 3 * F * F); b.A1 = put(A1, 2 * F * F); b.W2 = put(W2, 3 * F * F); b.W1 = put(W1, F * F);
   }
-  {
+  if (cfg->head_type == PNN_HEAD_POOLED) {
+    const int64_t d1 = cfg->head_d1, d2 = cfg->head_d2;
+    m->pP1 = put(take(d1 * F), d1 * F);   m->pp1 = put(take(d1), d1);
+    m->pP2 = put(take(d1 * d1), d1 * d1); m->pp2 = put(take(d1), d1);
+    m->pbr_stride = d2 * d1 + d2 + d2 * d2 + d2 + d2 + 1;
+    m->pbr = put(take(cfg->H * m->pbr_stride), cfg->H * m->pbr_stride);
+    if (cfg->n_global > 0) m->globW = put(take(F * cfg->n_global), F * cfg->n_global);
+  } else {
     const int H = cfg->H;
     m->oW1t = reserve(H * F * Fh); m->oW1 = reserve(H * Fh * F);
     m->ob1 = reserve(H * Fh); m->ow2 = reserve(H * Fh); m->ob2 = reserve(H);
@@ -357,6 +372,7 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
     ws->k = carve(es * N * F);
     ws->eatom = carve(es * N);
     ws->head_mask = (unsigned long long*)carve(8 * ((N + 127) / 128 + 1));
+    if (m->cfg.head_type == PNN_HEAD_POOLED) ws->pool_scratch = carve(pool_head_scratch_bytes(S, (int)F, m->cfg.H, es));
     ws->tape.resize(want_forces ? T : 1);
     if (want_forces) {
       ws->opre = carve(es * N * (F / 2));
@@ -620,6 +636,16 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     const int l_ = launch_update<T, T>(N, F, sn, v1, PQ, a, s_cur, v_out, st);
       nl += l_; ps_.done(l_); }
   }
+  const bool pooled = c.head_type == PNN_HEAD_POOLED;
+  if (pooled && hw) return PNN_ERR_UNSUPPORTED;
+  if (pooled) { // graph-level head: forward and, with forces, its adjoint s-bar (R1) in one go
+    ProfScope ps_(ws, st, "readout");
+    const int l_ = launch_pool_head<T>(N, S, F, c.H, c.head_d1, c.head_d2, s_cur, ws->g.a2s, sptr, head, W, m->pP1, m->pp1,
+                                       m->pP2, m->pp2, m->pbr, m->pbr_stride, ws->pool_scratch, energy,
+                                       want_f ? (T*)ws->sb : nullptr, ws->g.d_err, st);
+    if (l_ < 0) return PNN_ERR_UNSUPPORTED;
+    nl += l_; ps_.done(l_);
+  } else
   { ProfScope ps_(ws, st, "readout");
   const int l_ = hw ? launch_readout_blend<T>(N, S, F, c.H, s_cur, ws->g.a2s, hw, (T)skip_below, sptr, W + m->oW1t,
                                                W + m->ob1, W + m->ow2, W + m->ob2, (T*)ws->opre_all, (T*)ws->eatom,
@@ -630,6 +656,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
   if (want_f) {
     T* sb = (T*)ws->sb; T* vb = (T*)ws->vb; T* vb2 = (T*)ws->vb2; T* ab = (T*)ws->ab; T* PQb = (T*)ws->PQb;
     T* kb = (T*)ws->kb; T* zb = (T*)ws->zb; T* phib = (T*)ws->phib; T* hb = (T*)ws->hb; T* fpart = (T*)ws->fpart;
+    if (!pooled)
     { ProfScope ps_(ws, st, "readout_bwd");
     const int l_ = hw ? launch_readout_blend_bwd<T>(N, F, c.H, (const T*)ws->opre_all, ws->g.a2s, hw, (T)skip_below,
                                                      W + m->oW1, W + m->ow2, sb, st)
@@ -781,9 +808,16 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       const int l_ = launch_update<T, B>(N, F, sn, v1, PQ, a, s_cur, v_out, st, mb.s16, v_out16);
       nl += l_; ps_.done(l_); }
   }
+  const bool pooled = c.head_type == PNN_HEAD_POOLED;
+  if (pooled && hw) return PNN_ERR_UNSUPPORTED;
   { ProfScope ps_(ws, st, "readout");   // B5: all heads as one tensor-core GEMM, rows filtered by head in the epilogue
     int l_;
-    if (hw) { // blended heads: FP32 readout of the FP32 residual stream (one structure may need every head)
+    if (pooled) { // graph-level head in FP32 on the FP32 residual stream (S rows, not N: no tensor-core case)
+      l_ = launch_pool_head<T>(N, S, F, c.H, c.head_d1, c.head_d2, s_cur, ws->g.a2s, sptr, head, W, m->pP1, m->pp1, m->pP2,
+                               m->pp2, m->pbr, m->pbr_stride, ws->pool_scratch, energy, want_f ? (T*)ws->sb : nullptr,
+                               ws->g.d_err, st);
+      if (l_ < 0) return PNN_ERR_UNSUPPORTED;
+    } else if (hw) { // blended heads: FP32 readout of the FP32 residual stream (one structure may need every head)
       l_ = launch_readout_blend<T>(N, S, F, c.H, s_cur, ws->g.a2s, hw, (T)skip_below, sptr, W + m->oW1t, W + m->ob1,
                                    W + m->ow2, W + m->ob2, (T*)ws->opre_all, (T*)ws->eatom, energy, st);
     } else if (readout_tc_supported(F, c.H)) { // head widths F/2 in {32, 64, 128}: one tensor-core GEMM over the stacked heads
@@ -799,6 +833,7 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
   if (want_f) {
     T* sb = (T*)ws->sb; T* vb = (T*)ws->vb; T* vb2 = (T*)ws->vb2; T* PQb = (T*)ws->PQb; T* zb = (T*)ws->zb;
     T* fpart = (T*)ws->fpart;
+    if (!pooled)
     { ProfScope ps_(ws, st, "readout_bwd");
       const int l_ = hw ? launch_readout_blend_bwd<T>(N, F, c.H, (const T*)ws->opre_all, ws->g.a2s, hw, (T)skip_below,
                                                        W + m->oW1, W + m->ow2, sb, st)
@@ -862,6 +897,7 @@ static int eval_common(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t
   if (N > ws->maxN || S > ws->maxS) return PNN_ERR_CAPACITY;
   if ((N > 0 && !Z) || !sptr || (S > 0 && ((!head && !head_w) || !energy))) return PNN_ERR_INVALID_ARG;
   if ((flags & PNN_FORCES) && (!ws->want_forces || (N > 0 && !forces))) return PNN_ERR_INVALID_ARG;
+  if (head_w && m->cfg.head_type == PNN_HEAD_POOLED) return PNN_ERR_UNSUPPORTED;
   if (ws->graph_N != N || ws->graph_S != S) return PNN_ERR_NO_GRAPH;
   cudaStream_t st = (cudaStream_t)stream;
   int rc;

@@ -1,0 +1,268 @@
+// pool_head.cu — the paper's graph-level output heads ("Output heads 16 (graph-level)", "Head architecture
+// 2 shared layers (dim 50) + 2 branch layers (dim 776)"; reading Q29):
+//   x_g = mean_{i in g} s_i                                  (mean pooling of the final scalar features)
+//   y1 = silu(P1 x_g + p1) ; y2 = silu(P2 y1 + p2)           (shared trunk, width d1)
+//   z1 = silu(B1_h y2 + q1_h) ; z2 = silu(B2_h z1 + q2_h)    (branch of the structure's head h, width d2)
+//   E_g = w3_h . z2 + q3_h
+// and its adjoint for forces: x-bar_g = P1^T (P2^T (B1_h^T (B2_h^T (w3_h . silu'(.)) . silu'(.)) . silu'(.)) . silu'(.)),
+// s-bar_i = x-bar_{g(i)} / n_g.
+//
+// The branch layers are the cost (d2 x d2 weights per head, one matrix-vector product per structure), so structures are
+// counting-sorted by head first and a CTA takes G structures of ONE head: every weight row read from L2 is used G times.
+// Forward and adjoint run back to back in the same CTA with the pre-activations in shared memory: no tape, one launch.
+#include <algorithm>
+
+#include "common.cuh"
+
+namespace pnn {
+
+namespace {
+
+constexpr int POOL_THREADS = 256;
+constexpr int POOL_MAXH = 1024;
+
+// x[g][f] = mean_i s[i][f]; one CTA per structure (grid-stride), threads over (atom slice, feature)
+template <typename T>
+__global__ void __launch_bounds__(POOL_THREADS)
+pool_mean_k(int64_t S, int F, const int32_t* __restrict__ sptr, const T* __restrict__ s, T* __restrict__ x) {
+  __shared__ T part[POOL_THREADS];
+  const int f = threadIdx.x % F, a0 = threadIdx.x / F, na = POOL_THREADS / F; // F in {32..256}, multiple of 32
+  for (int64_t g = blockIdx.x; g < S; g += gridDim.x) {
+    const int i0 = sptr[g], i1 = sptr[g + 1];
+    T acc = T(0);
+    if (a0 < na)
+      for (int i = i0 + a0; i < i1; i += na) acc += s[(int64_t)i * F + f];
+    part[threadIdx.x] = acc;
+    __syncthreads();
+    if (threadIdx.x < F) {
+      T t = T(0);
+      for (int a = 0; a < na; ++a) t += part[a * F + f];
+      x[g * F + f] = (i1 > i0) ? t / (T)(i1 - i0) : T(0);
+    }
+    __syncthreads();
+  }
+}
+
+// Counting sort of the structures by head (one CTA): perm[] lists the structures head by head, tiles[] = (head, first
+// position in perm, count <= G) for every CTA of pooled_head_k, *ntiles their number.  Structures with a head index out
+// of range raise ERRF_BAD_HEAD and are left out (their energy stays 0).
+__global__ void __launch_bounds__(1024)
+head_sort_k(int64_t S, int H, int G, const int32_t* __restrict__ head, int32_t* __restrict__ perm, int4* __restrict__ tiles,
+            int32_t* __restrict__ ntiles, int* __restrict__ d_err) {
+  __shared__ int cnt[POOL_MAXH], start[POOL_MAXH], tstart[POOL_MAXH], cur[POOL_MAXH];
+  for (int h = threadIdx.x; h < H; h += blockDim.x) { cnt[h] = 0; cur[h] = 0; }
+  __syncthreads();
+  for (int64_t g = threadIdx.x; g < S; g += blockDim.x) {
+    const int h = head[g];
+    if (h < 0 || h >= H) atomicOr(d_err, ERRF_BAD_HEAD);
+    else atomicAdd(&cnt[h], 1);
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int a = 0, t = 0;
+    for (int h = 0; h < H; ++h) { start[h] = a; tstart[h] = t; a += cnt[h]; t += (cnt[h] + G - 1) / G; }
+    *ntiles = t;
+  }
+  __syncthreads();
+  for (int64_t g = threadIdx.x; g < S; g += blockDim.x) {
+    const int h = head[g];
+    if (h >= 0 && h < H) perm[start[h] + atomicAdd(&cur[h], 1)] = (int32_t)g;
+  }
+  for (int h = threadIdx.x; h < H; h += blockDim.x)
+    for (int t = 0, c = cnt[h]; c > 0; ++t, c -= G) tiles[tstart[h] + t] = make_int4(h, start[h] + t * G, min(c, G), 0);
+}
+
+template <typename T> __device__ __forceinline__ T silu_f(T x) { return x / (T(1) + exp(-x)); }
+template <typename T> __device__ __forceinline__ T dsilu_f(T x) {
+  const T sg = T(1) / (T(1) + exp(-x));
+  return sg * (T(1) + x * (T(1) - sg));
+}
+
+// out[g][o] = sum_i W[o][i] in[g][i] + b[o] for the CTA's G structures: a warp per output row, lanes over the inputs
+template <typename T, int G>
+__device__ __forceinline__ void layer_fwd(int n_out, int n_in, const T* __restrict__ W, const T* __restrict__ b,
+                                          const T* in, int ld_in, T* pre, int ld_pre) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = POOL_THREADS / 32;
+  for (int o = warp; o < n_out; o += nw) {
+    T acc[G];
+#pragma unroll
+    for (int g = 0; g < G; ++g) acc[g] = T(0);
+    const T* row = W + (int64_t)o * n_in;
+    for (int i = lane; i < n_in; i += 32) {
+      const T w = row[i];
+#pragma unroll
+      for (int g = 0; g < G; ++g) acc[g] = fma(w, in[g * ld_in + i], acc[g]);
+    }
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+#pragma unroll
+      for (int m = 16; m; m >>= 1) acc[g] += __shfl_xor_sync(0xffffffffu, acc[g], m);
+    }
+    if (lane == 0) {
+      const T bo = b[o];
+#pragma unroll
+      for (int g = 0; g < G; ++g) pre[g * ld_pre + o] = acc[g] + bo;
+    }
+  }
+}
+
+// out[g][i] = (sum_o W[o][i] gb[g][o]) * (dpre ? silu'(dpre[g][i]) : 1): threads over the inputs, rows read coalesced
+template <typename T, int G>
+__device__ __forceinline__ void layer_bwd(int n_out, int n_in, const T* __restrict__ W, const T* gb, int ld_gb,
+                                          const T* dpre, int ld_dpre, T* out, int ld_out) {
+  for (int i = threadIdx.x; i < n_in; i += POOL_THREADS) {
+    T acc[G];
+#pragma unroll
+    for (int g = 0; g < G; ++g) acc[g] = T(0);
+    for (int o = 0; o < n_out; ++o) {
+      const T w = W[(int64_t)o * n_in + i];
+#pragma unroll
+      for (int g = 0; g < G; ++g) acc[g] = fma(w, gb[g * ld_gb + o], acc[g]);
+    }
+#pragma unroll
+    for (int g = 0; g < G; ++g) out[g * ld_out + i] = dpre ? acc[g] * dsilu_f<T>(dpre[g * ld_dpre + i]) : acc[g];
+  }
+}
+
+struct PoolW { int64_t P1, p1, P2, p2, br, br_stride; }; // element offsets; one head's branch: B1 q1 B2 q2 w3 q3
+
+// One CTA per tile of <= G structures of one head.  Shared memory, per structure: x [F] | pre1 [d1] | pre2 [d1] |
+// pre3 [d2] | pre4 [d2] | act [max(F,d1,d2)] | gb [max(F,d1,d2)].
+template <typename T, int G>
+__global__ void __launch_bounds__(POOL_THREADS)
+pooled_head_k(int F, int d1, int d2, const T* __restrict__ Wt, PoolW pw, const int32_t* __restrict__ perm,
+              const int4* __restrict__ tiles, const int32_t* __restrict__ ntiles, const T* __restrict__ x,
+              T* __restrict__ energy, T* __restrict__ xbar) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  if ((int)blockIdx.x >= *ntiles) return;
+  const int4 tl = tiles[blockIdx.x];
+  const int h = tl.x, p0 = tl.y, cnt = tl.z;
+  const int dm = max(F, max(d1, d2));
+  const int ld = F + 2 * d1 + 2 * d2 + 2 * dm;
+  T* sm = reinterpret_cast<T*>(smem_raw);
+  T* X = sm; T* PRE1 = X + F; T* PRE2 = PRE1 + d1; T* PRE3 = PRE2 + d1; T* PRE4 = PRE3 + d2; T* ACT = PRE4 + d2;
+  T* GB = ACT + dm;
+  const T* B1 = Wt + pw.br + (int64_t)h * pw.br_stride;
+  const T* q1 = B1 + (int64_t)d2 * d1; const T* B2 = q1 + d2; const T* q2 = B2 + (int64_t)d2 * d2;
+  const T* w3 = q2 + d2; const T* q3 = w3 + d2;
+  for (int g = 0; g < G; ++g) {
+    const int64_t sg = perm[p0 + min(g, cnt - 1)]; // padding slots repeat the last structure (results not written)
+    for (int f = threadIdx.x; f < F; f += POOL_THREADS) X[g * ld + f] = x[sg * F + f];
+  }
+  __syncthreads();
+  auto act = [&](const T* pre, int n) {
+    __syncthreads();
+    for (int t = threadIdx.x; t < G * n; t += POOL_THREADS) { const int g = t / n, o = t - g * n; ACT[g * ld + o] = silu_f<T>(pre[g * ld + o]); }
+    __syncthreads();
+  };
+  layer_fwd<T, G>(d1, F, Wt + pw.P1, Wt + pw.p1, X, ld, PRE1, ld);    act(PRE1, d1);
+  layer_fwd<T, G>(d1, d1, Wt + pw.P2, Wt + pw.p2, ACT, ld, PRE2, ld); act(PRE2, d1);
+  layer_fwd<T, G>(d2, d1, B1, q1, ACT, ld, PRE3, ld);                 act(PRE3, d2);
+  layer_fwd<T, G>(d2, d2, B2, q2, ACT, ld, PRE4, ld);                 act(PRE4, d2);
+  { // E_g = w3 . z2 + q3: a warp per structure
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int g = warp; g < cnt; g += POOL_THREADS / 32) {
+      T a = T(0);
+      for (int o = lane; o < d2; o += 32) a = fma(w3[o], ACT[g * ld + o], a);
+#pragma unroll
+      for (int m = 16; m; m >>= 1) a += __shfl_xor_sync(0xffffffffu, a, m);
+      if (lane == 0) energy[perm[p0 + g]] = a + q3[0];
+    }
+  }
+  if (!xbar) return;
+  __syncthreads();
+  for (int t = threadIdx.x; t < G * d2; t += POOL_THREADS) { // z2-bar (pre-activation adjoint)
+    const int g = t / d2, o = t - g * d2;
+    GB[g * ld + o] = w3[o] * dsilu_f<T>(PRE4[g * ld + o]);
+  }
+  __syncthreads();
+  layer_bwd<T, G>(d2, d2, B2, GB, ld, PRE3, ld, ACT, ld);             __syncthreads(); // z1-bar in ACT
+  layer_bwd<T, G>(d2, d1, B1, ACT, ld, PRE2, ld, GB, ld);             __syncthreads(); // y2-bar in GB
+  layer_bwd<T, G>(d1, d1, Wt + pw.P2, GB, ld, PRE1, ld, ACT, ld);     __syncthreads(); // y1-bar in ACT
+  layer_bwd<T, G>(d1, F, Wt + pw.P1, ACT, ld, (const T*)nullptr, 0, GB, ld); __syncthreads(); // x-bar in GB
+  for (int g = 0; g < cnt; ++g) {
+    const int64_t sg = perm[p0 + g];
+    for (int f = threadIdx.x; f < F; f += POOL_THREADS) xbar[sg * F + f] = GB[g * ld + f];
+  }
+}
+
+// s-bar_i = x-bar_{g(i)} / n_g
+template <typename T>
+__global__ void __launch_bounds__(256)
+pool_bcast_k(int64_t n, int F, const int32_t* __restrict__ a2s, const int32_t* __restrict__ sptr, const T* __restrict__ xbar,
+             T* __restrict__ sb) {
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t i = t / F;
+    const int f = (int)(t - i * F), g = a2s[i];
+    sb[t] = xbar[(int64_t)g * F + f] / (T)(sptr[g + 1] - sptr[g]);
+  }
+}
+
+template <typename T> constexpr int pool_group() { return sizeof(T) == 8 ? 4 : 8; }
+
+} // namespace
+
+int64_t pool_head_scratch_bytes(int64_t maxS, int F, int H, size_t elem) {
+  const int64_t G = elem == 8 ? 4 : 8;
+  return 2 * ((maxS * F * (int64_t)elem + 255) / 256 * 256) + (maxS * 4 + 255) / 256 * 256 +
+         (((maxS + G - 1) / G + H) * 16 + 255) / 256 * 256 + 256;
+}
+
+bool pool_head_supported(int F, int d1, int d2, int H, size_t elem) {
+  if (d1 < 1 || d2 < 1 || d1 > 4096 || d2 > 4096 || H > POOL_MAXH) return false;
+  const int64_t G = elem == 8 ? 4 : 8, dm = std::max(F, std::max(d1, d2));
+  return G * (F + 2 * d1 + 2 * d2 + 2 * dm) * (int64_t)elem <= 227 * 1024;
+}
+
+// energy [S] and, when sb != NULL, s-bar [N][F] of the pooled head.  scratch: pool_head_scratch_bytes().  Returns the
+// number of launches, -1 when the shapes are not supported.
+template <typename T>
+int launch_pool_head(int64_t N, int64_t S, int F, int H, int d1, int d2, const T* s, const int32_t* a2s,
+                     const int32_t* sptr, const int32_t* head, const T* W, int64_t oP1, int64_t op1, int64_t oP2,
+                     int64_t op2, int64_t obr, int64_t br_stride, void* scratch, T* energy, T* sb, int* d_err,
+                     cudaStream_t st) {
+  if (S == 0) return 0;
+  if (!pool_head_supported(F, d1, d2, H, sizeof(T))) return -1;
+  constexpr int G = pool_group<T>();
+  char* p = (char*)scratch;
+  auto carve = [&](int64_t b) { char* q = p; p += (b + 255) / 256 * 256; return q; };
+  T* x = (T*)carve(S * F * (int64_t)sizeof(T));
+  T* xbar = (T*)carve(S * F * (int64_t)sizeof(T));
+  int32_t* perm = (int32_t*)carve(S * 4);
+  const int64_t max_tiles = (S + G - 1) / G + H;
+  int4* tiles = (int4*)carve(max_tiles * 16);
+  int32_t* ntiles = (int32_t*)carve(4);
+  cudaMemsetAsync(energy, 0, sizeof(T) * S, st);
+  pool_mean_k<T><<<(unsigned)std::min<int64_t>(S, 148 * 8), POOL_THREADS, 0, st>>>(S, F, sptr, s, x);
+  PNN_KCHECK("pool_mean_k");
+  head_sort_k<<<1, 1024, 0, st>>>(S, H, G, head, perm, tiles, ntiles, d_err);
+  PNN_KCHECK("head_sort_k");
+  const int dm = std::max(F, std::max(d1, d2));
+  const size_t smem = (size_t)G * (F + 2 * d1 + 2 * d2 + 2 * dm) * sizeof(T);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(pooled_head_k<T, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    attr_set = true;
+  }
+  PoolW pw{oP1, op1, oP2, op2, obr, br_stride};
+  pooled_head_k<T, G><<<(unsigned)max_tiles, POOL_THREADS, smem, st>>>(F, d1, d2, W, pw, perm, tiles, ntiles, x, energy,
+                                                                       sb ? xbar : nullptr);
+  PNN_KCHECK("pooled_head_k");
+  int nl = 3;
+  if (sb && N > 0) {
+    const int64_t n = N * F;
+    pool_bcast_k<T><<<(unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16), 256, 0, st>>>(n, F, a2s, sptr, xbar, sb);
+    PNN_KCHECK("pool_bcast_k");
+    ++nl;
+  }
+  return nl;
+}
+
+template int launch_pool_head<float>(int64_t, int64_t, int, int, int, int, const float*, const int32_t*, const int32_t*,
+                                     const int32_t*, const float*, int64_t, int64_t, int64_t, int64_t, int64_t, int64_t,
+                                     void*, float*, float*, int*, cudaStream_t);
+template int launch_pool_head<double>(int64_t, int64_t, int, int, int, int, const double*, const int32_t*, const int32_t*,
+                                      const int32_t*, const double*, int64_t, int64_t, int64_t, int64_t, int64_t, int64_t,
+                                      void*, double*, double*, int*, cudaStream_t);
+
+} // namespace pnn

@@ -27,7 +27,8 @@ def make_model(mc: gen.ModelCfg, weights, precision: str, max_atoms: int, max_ed
                      norm_eps=mc.norm_eps, max_atoms=max_atoms, max_edges=max_edges, max_structs=max_structs,
                      forces=forces, rbf=getattr(mc, "rbf", "gaussian"),
                      pbc_images=getattr(mc, "pbc_images", "minimum"), max_neighbors=getattr(mc, "max_neighbors", 0),
-                     n_global=getattr(mc, "n_global", 0))
+                     n_global=getattr(mc, "n_global", 0), head_type=getattr(mc, "head_type", "atomwise"),
+                     head_d1=getattr(mc, "head_d1", 50), head_d2=getattr(mc, "head_d2", 776))
 
 
 def run_gpu(mc: gen.ModelCfg, weights, batch: gen.Batch, precision: str, forces: bool = True, max_edges=None,

@@ -44,6 +44,13 @@ def test_weight_blob_size_matches_generators(pnn):
             assert pnn.pnn_weights_count(cfg) == gen.weights_count(mc)
     # F=256, T=4, K=32, H=16, Zmax=86 -> 3,543,824 scalars
     assert pnn.pnn_weights_count(pnn.pnn_config(256, 4, 32, 16, 86, 6.0, 1e-8, pnn.PNN_FP32)) == 3543824
+    # pooled graph-level heads and global attribute columns change the blob the same way on both sides
+    import dataclasses
+    mc = dataclasses.replace(gen.model_cfg(2), head_type="pooled", head_d1=50, head_d2=776, n_global=2)
+    cfg = pnn.pnn_config(mc.F, mc.T, mc.K, mc.H, mc.Zmax, mc.cutoff, mc.norm_eps, pnn.PNN_FP32, 0, 0, 0, 2, 1, 50, 776)
+    assert pnn.pnn_weights_count(cfg) == gen.weights_count(mc)
+    with pytest.raises(pnn.PnnError):   # widths whose activations do not fit one CTA's shared memory
+        pnn.pnn_weights_count(pnn.pnn_config(64, 2, 20, 2, 86, 5.0, 1e-8, pnn.PNN_FP64, 0, 0, 0, 0, 1, 50, 4000))
 
 
 @pytest.mark.parametrize("bad", [dict(F=48), dict(F=512), dict(F=0), dict(K=1), dict(K=33), dict(T=0), dict(H=0),
