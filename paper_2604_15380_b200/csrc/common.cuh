@@ -197,13 +197,15 @@ template <typename T>
 int launch_embed_globals(int64_t N, int F, int G, const int32_t* a2s, const double* glob, const T* globW, T* s,
                          __nv_bfloat16* s16, cudaStream_t st);
 // pool_head.cu: the paper's graph-level heads (mean pooling -> shared layers -> per-head branch layers; reading Q29)
+// element offsets in the device weight buffer: shared layers P1 [d1][F], p1, P2 [d1][d1], p2 and their transposes; per head
+// (stride br_stride, blob order) B1 [d2][d1] q1 B2 [d2][d2] q2 w3 q3; per head (stride brT_stride) B1^T [d1][d2] B2^T [d2][d2]
+struct PoolHeadW { int64_t P1, p1, P2, p2, P1t, P2t, br, br_stride, brT, brT_stride; };
 int64_t pool_head_scratch_bytes(int64_t maxS, int F, int H, size_t elem);
 bool pool_head_supported(int F, int d1, int d2, int H, size_t elem);
 template <typename T>
 int launch_pool_head(int64_t N, int64_t S, int F, int H, int d1, int d2, const T* s, const int32_t* a2s,
-                     const int32_t* sptr, const int32_t* head, const T* W, int64_t oP1, int64_t op1, int64_t oP2,
-                     int64_t op2, int64_t obr, int64_t br_stride, void* scratch, T* energy, T* sb, int* d_err,
-                     cudaStream_t st);
+                     const int32_t* sptr, const int32_t* head, const T* W, const PoolHeadW& pw, void* scratch, T* energy,
+                     T* sb, int* d_err, cudaStream_t st);
 // IT: storage type of P | Q and of the gate values a (= T, or BF16 in the BF16 model)
 template <typename T, typename IT>
 int launch_norm(int64_t N, int F, const IT* PQ, T* sn, T eps, cudaStream_t st, __nv_bfloat16* sn16 = nullptr);

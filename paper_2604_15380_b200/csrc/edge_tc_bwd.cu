@@ -121,7 +121,7 @@ struct BwdSmem {
   static constexpr int B_TILE = NE * KP * 2;    // one of the two B tiles (G, G') of a slot
   static constexpr int GRP_BYTES = NSLOT * 2 * B_TILE + NSLOT * (int)sizeof(TileMetaB);
   static constexpr int BAR_OFF = A_BYTES + NGRP * GRP_BYTES;
-  static constexpr int NBAR_G = 2 * NSLOT + 2;  // meta_full[NSLOT], meta_empty[NSLOT], tmem_full, tmem_empty
+  static constexpr int NBAR_G = 2 * NSLOT + 3;  // meta_full[NSLOT], meta_empty[NSLOT], tmem_full, tmem_empty[2]
   static constexpr int NBAR = NGRP * NBAR_G;
   static constexpr int TOTAL = BAR_OFF + NBAR * 8 + 32 + 128;
   static constexpr int TMEM_COLS = (NGRP * 2 * NACC * NE <= 256) ? 256 : 512;
@@ -148,7 +148,7 @@ edge_bwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
   auto meta_full = [&](int g, int s) { return bar0 + 8u * (g * L::NBAR_G + s); };
   auto meta_empty = [&](int g, int s) { return bar0 + 8u * (g * L::NBAR_G + NSLOT + s); };
   auto tmem_full = [&](int g) { return bar0 + 8u * (g * L::NBAR_G + 2 * NSLOT); };
-  auto tmem_empty = [&](int g) { return bar0 + 8u * (g * L::NBAR_G + 2 * NSLOT + 1); };
+  auto tmem_empty = [&](int g, uint32_t b) { return bar0 + 8u * (g * L::NBAR_G + 2 * NSLOT + 1 + b); };
 
   { // resident A operand: the packed filter image of this block (the first NACC accumulator tiles), copied verbatim
     const uint4* src = reinterpret_cast<const uint4*>(fltT);
@@ -159,7 +159,7 @@ edge_bwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
     for (int g = 0; g < NGRP; ++g) {
       for (int s = 0; s < NSLOT; ++s) { mbar_init(meta_full(g, s), 1); mbar_init(meta_empty(g, s), EPW); }
       mbar_init(tmem_full(g), 1);
-      mbar_init(tmem_empty(g), EPW);
+      mbar_init(tmem_empty(g, 0), EPW); mbar_init(tmem_empty(g, 1), EPW);
     }
     mbar_init_fence();
   }
@@ -287,10 +287,11 @@ edge_bwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
         __syncwarp();
         if (lane == 0) {
           mbar_arrive(meta_full(g, slot));
-          // the epilogue has finished the previous tile.  The two producers alternate on ONE barrier, so this one has not
-          // observed phase n - 2 yet: a parity wait for phase n - 1 alone would pass while n - 2 is still open.
-          if (n >= 2) mbar_wait_backoff(tmem_empty(g), n & 1u);
-          mbar_wait_backoff(tmem_empty(g), (n & 1u) ^ 1u);
+          // the epilogue has finished tile n - 1 (one TMEM buffer per group).  Tiles alternate between two barriers by
+          // parity, so that this producer (which owns one parity) sees EVERY phase of the other parity's barrier in order:
+          // on a single barrier it would skip every other phase, and a parity wait for a phase two behind the barrier's
+          // current one never returns.
+          if (n >= 1) mbar_wait_backoff(tmem_empty(g, (n - 1u) & 1u), ((n - 1u) >> 1) & 1u);
           tc_fence_after();
           const uint32_t b_lo0 = (uint32_t)umma_desc_nosw(grp_u + slot * 2 * L::B_TILE, 128, KC * 128);
 #pragma unroll
@@ -488,7 +489,7 @@ edge_bwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
         }
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) { mbar_arrive(tmem_empty(g)); mbar_arrive(meta_empty(g, slot)); }
+        if (lane == 0) { mbar_arrive(tmem_empty(g, n & 1u)); mbar_arrive(meta_empty(g, slot)); }
       }
       end_row(cur);
       for (int k = cur + 1; k < (int)a1; ++k) { begin_row(k); end_row(k); }

@@ -92,7 +92,7 @@ struct pnn_model {
   std::vector<BlockW> blk;
   int64_t globW = 0;                                    // [F][n_global] (global attributes -> embedding)
   int64_t oW1t = 0, oW1 = 0, ob1 = 0, ow2 = 0, ob2 = 0; // heads: [H][F][Fh], [H][Fh][F], [H][Fh], [H][Fh], [H]
-  int64_t pP1 = 0, pp1 = 0, pP2 = 0, pp2 = 0, pbr = 0, pbr_stride = 0; // pooled head (pool_head.cu), original [out][in]
+  PoolHeadW pool{};                                     // pooled head (pool_head.cu)
   __nv_bfloat16* d_wb = nullptr;                        // BF16 copy of d_w (same offsets): tcgen05 GEMM operands
   __nv_bfloat16* d_fltT = nullptr;                      // BF16 model: per block, the filter image of edge_tc.cu
   int64_t fltT_stride = 0;
@@ -247,10 +247,24 @@ int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, 
   }
   if (cfg->head_type == PNN_HEAD_POOLED) {
     const int64_t d1 = cfg->head_d1, d2 = cfg->head_d2;
-    m->pP1 = put(take(d1 * F), d1 * F);   m->pp1 = put(take(d1), d1);
-    m->pP2 = put(take(d1 * d1), d1 * d1); m->pp2 = put(take(d1), d1);
-    m->pbr_stride = d2 * d1 + d2 + d2 * d2 + d2 + d2 + 1;
-    m->pbr = put(take(cfg->H * m->pbr_stride), cfg->H * m->pbr_stride);
+    PoolHeadW& pw = m->pool;
+    const double* P1 = take(d1 * F);  pw.P1 = put(P1, d1 * F);  pw.P1t = put_t(P1, d1, F);  pw.p1 = put(take(d1), d1);
+    const double* P2 = take(d1 * d1); pw.P2 = put(P2, d1 * d1); pw.P2t = put_t(P2, d1, d1); pw.p2 = put(take(d1), d1);
+    pw.br_stride = d2 * d1 + d2 + d2 * d2 + d2 + d2 + 1;
+    pw.brT_stride = d1 * d2 + d2 * d2;
+    const double* br = take(cfg->H * pw.br_stride);
+    pw.br = put(br, cfg->H * pw.br_stride);
+    pw.brT = reserve(cfg->H * pw.brT_stride);
+    for (int h = 0; h < cfg->H; ++h) {
+      const double* B1 = br + h * pw.br_stride;
+      const double* B2 = B1 + d2 * d1 + d2;
+      double* t1 = hb.data() + pw.brT + h * pw.brT_stride;
+      double* t2 = t1 + d1 * d2;
+      for (int64_t o = 0; o < d2; ++o) {
+        for (int64_t i = 0; i < d1; ++i) t1[i * d2 + o] = B1[o * d1 + i];
+        for (int64_t i = 0; i < d2; ++i) t2[i * d2 + o] = B2[o * d2 + i];
+      }
+    }
     if (cfg->n_global > 0) m->globW = put(take(F * cfg->n_global), F * cfg->n_global);
   } else {
     const int H = cfg->H;
@@ -640,9 +654,8 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
   if (pooled && hw) return PNN_ERR_UNSUPPORTED;
   if (pooled) { // graph-level head: forward and, with forces, its adjoint s-bar (R1) in one go
     ProfScope ps_(ws, st, "readout");
-    const int l_ = launch_pool_head<T>(N, S, F, c.H, c.head_d1, c.head_d2, s_cur, ws->g.a2s, sptr, head, W, m->pP1, m->pp1,
-                                       m->pP2, m->pp2, m->pbr, m->pbr_stride, ws->pool_scratch, energy,
-                                       want_f ? (T*)ws->sb : nullptr, ws->g.d_err, st);
+    const int l_ = launch_pool_head<T>(N, S, F, c.H, c.head_d1, c.head_d2, s_cur, ws->g.a2s, sptr, head, W, m->pool,
+                                       ws->pool_scratch, energy, want_f ? (T*)ws->sb : nullptr, ws->g.d_err, st);
     if (l_ < 0) return PNN_ERR_UNSUPPORTED;
     nl += l_; ps_.done(l_);
   } else
@@ -813,9 +826,8 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
   { ProfScope ps_(ws, st, "readout");   // B5: all heads as one tensor-core GEMM, rows filtered by head in the epilogue
     int l_;
     if (pooled) { // graph-level head in FP32 on the FP32 residual stream (S rows, not N: no tensor-core case)
-      l_ = launch_pool_head<T>(N, S, F, c.H, c.head_d1, c.head_d2, s_cur, ws->g.a2s, sptr, head, W, m->pP1, m->pp1, m->pP2,
-                               m->pp2, m->pbr, m->pbr_stride, ws->pool_scratch, energy, want_f ? (T*)ws->sb : nullptr,
-                               ws->g.d_err, st);
+      l_ = launch_pool_head<T>(N, S, F, c.H, c.head_d1, c.head_d2, s_cur, ws->g.a2s, sptr, head, W, m->pool,
+                               ws->pool_scratch, energy, want_f ? (T*)ws->sb : nullptr, ws->g.d_err, st);
       if (l_ < 0) return PNN_ERR_UNSUPPORTED;
     } else if (hw) { // blended heads: FP32 readout of the FP32 residual stream (one structure may need every head)
       l_ = launch_readout_blend<T>(N, S, F, c.H, s_cur, ws->g.a2s, hw, (T)skip_below, sptr, W + m->oW1t, W + m->ob1,

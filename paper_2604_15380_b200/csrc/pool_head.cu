@@ -8,7 +8,9 @@
 // s-bar_i = x-bar_{g(i)} / n_g.
 //
 // The branch layers are the cost (d2 x d2 weights per head, one matrix-vector product per structure), so structures are
-// counting-sorted by head first and a CTA takes G structures of ONE head: every weight row read from L2 is used G times.
+// counting-sorted by head first and a CTA takes G structures (16 in FP32, 8 in FP64) of ONE head: every weight read from L2 is
+// used G times.  A layer is a thread-per-output matrix-vector product over weights stored [in][out] (coalesced), the G input
+// vectors broadcast from shared memory; the adjoint is the same routine over the original [out][in] weights.
 // Forward and adjoint run back to back in the same CTA with the pre-activations in shared memory: no tape, one launch.
 #include <algorithm>
 
@@ -19,6 +21,7 @@ namespace pnn {
 namespace {
 
 constexpr int POOL_THREADS = 256;
+constexpr int POOL_MAXT = 1024; // threads of pooled_head_k: one per output feature of the widest layer
 constexpr int POOL_MAXH = 1024;
 
 // x[g][f] = mean_i s[i][f]; one CTA per structure (grid-stride), threads over (atom slice, feature)
@@ -78,59 +81,40 @@ template <typename T> __device__ __forceinline__ T dsilu_f(T x) {
   return sg * (T(1) + x * (T(1) - sg));
 }
 
-// out[g][o] = sum_i W[o][i] in[g][i] + b[o] for the CTA's G structures: a warp per output row, lanes over the inputs
-template <typename T, int G>
-__device__ __forceinline__ void layer_fwd(int n_out, int n_in, const T* __restrict__ W, const T* __restrict__ b,
-                                          const T* in, int ld_in, T* pre, int ld_pre) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = POOL_THREADS / 32;
-  for (int o = warp; o < n_out; o += nw) {
+template <typename T> struct alignas(16) Vec16 { T v[16 / sizeof(T)]; };
+
+// acc[r][g] = sum_c M[c][r] v[c][g] for the CTA's G structures, then epi(r, acc): a thread per output r, the matrix row c
+// read coalesced over r, v[c][0..G) broadcast from shared memory with 16-byte loads.  Serves the forward layers with the
+// transposed weights (M = W^T [in][out]) and the adjoint with the original ones (M = W [out][in]).
+template <typename T, int G, typename Epi>
+__device__ __forceinline__ void matvec(int n_r, int n_c, const T* __restrict__ M, const T* v, Epi epi) {
+  constexpr int VW = 16 / sizeof(T);
+  for (int r = threadIdx.x; r < n_r; r += blockDim.x) {
     T acc[G];
 #pragma unroll
     for (int g = 0; g < G; ++g) acc[g] = T(0);
-    const T* row = W + (int64_t)o * n_in;
-    for (int i = lane; i < n_in; i += 32) {
-      const T w = row[i];
+    const T* col = M + r;
+#pragma unroll 4
+    for (int c = 0; c < n_c; ++c) {
+      const T w = __ldg(col + (int64_t)c * n_r);
+      const Vec16<T>* vc = reinterpret_cast<const Vec16<T>*>(v + c * G);
 #pragma unroll
-      for (int g = 0; g < G; ++g) acc[g] = fma(w, in[g * ld_in + i], acc[g]);
+      for (int q = 0; q < G / VW; ++q) {
+        const Vec16<T> x = vc[q];
+#pragma unroll
+        for (int e = 0; e < VW; ++e) acc[q * VW + e] = fma(w, x.v[e], acc[q * VW + e]);
+      }
     }
-#pragma unroll
-    for (int g = 0; g < G; ++g) {
-#pragma unroll
-      for (int m = 16; m; m >>= 1) acc[g] += __shfl_xor_sync(0xffffffffu, acc[g], m);
-    }
-    if (lane == 0) {
-      const T bo = b[o];
-#pragma unroll
-      for (int g = 0; g < G; ++g) pre[g * ld_pre + o] = acc[g] + bo;
-    }
+    epi(r, acc);
   }
 }
 
-// out[g][i] = (sum_o W[o][i] gb[g][o]) * (dpre ? silu'(dpre[g][i]) : 1): threads over the inputs, rows read coalesced
+// One CTA per tile of <= G structures of one head.  Shared memory ([feature][G], the G structures of a feature side by
+// side): PRE1 [d1] | PRE2 [d1] | PRE3 [d2] | PRE4 [d2] | A [dm] | B [dm], dm = max(F, d1, d2); A and B ping-pong as the
+// input and output of consecutive layers, forward and reverse.
 template <typename T, int G>
-__device__ __forceinline__ void layer_bwd(int n_out, int n_in, const T* __restrict__ W, const T* gb, int ld_gb,
-                                          const T* dpre, int ld_dpre, T* out, int ld_out) {
-  for (int i = threadIdx.x; i < n_in; i += POOL_THREADS) {
-    T acc[G];
-#pragma unroll
-    for (int g = 0; g < G; ++g) acc[g] = T(0);
-    for (int o = 0; o < n_out; ++o) {
-      const T w = W[(int64_t)o * n_in + i];
-#pragma unroll
-      for (int g = 0; g < G; ++g) acc[g] = fma(w, gb[g * ld_gb + o], acc[g]);
-    }
-#pragma unroll
-    for (int g = 0; g < G; ++g) out[g * ld_out + i] = dpre ? acc[g] * dsilu_f<T>(dpre[g * ld_dpre + i]) : acc[g];
-  }
-}
-
-struct PoolW { int64_t P1, p1, P2, p2, br, br_stride; }; // element offsets; one head's branch: B1 q1 B2 q2 w3 q3
-
-// One CTA per tile of <= G structures of one head.  Shared memory, per structure: x [F] | pre1 [d1] | pre2 [d1] |
-// pre3 [d2] | pre4 [d2] | act [max(F,d1,d2)] | gb [max(F,d1,d2)].
-template <typename T, int G>
-__global__ void __launch_bounds__(POOL_THREADS)
-pooled_head_k(int F, int d1, int d2, const T* __restrict__ Wt, PoolW pw, const int32_t* __restrict__ perm,
+__global__ void __launch_bounds__(POOL_MAXT)
+pooled_head_k(int F, int d1, int d2, const T* __restrict__ Wt, PoolHeadW pw, const int32_t* __restrict__ perm,
               const int4* __restrict__ tiles, const int32_t* __restrict__ ntiles, const T* __restrict__ x,
               T* __restrict__ energy, T* __restrict__ xbar) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -138,51 +122,56 @@ pooled_head_k(int F, int d1, int d2, const T* __restrict__ Wt, PoolW pw, const i
   const int4 tl = tiles[blockIdx.x];
   const int h = tl.x, p0 = tl.y, cnt = tl.z;
   const int dm = max(F, max(d1, d2));
-  const int ld = F + 2 * d1 + 2 * d2 + 2 * dm;
-  T* sm = reinterpret_cast<T*>(smem_raw);
-  T* X = sm; T* PRE1 = X + F; T* PRE2 = PRE1 + d1; T* PRE3 = PRE2 + d1; T* PRE4 = PRE3 + d2; T* ACT = PRE4 + d2;
-  T* GB = ACT + dm;
-  const T* B1 = Wt + pw.br + (int64_t)h * pw.br_stride;
-  const T* q1 = B1 + (int64_t)d2 * d1; const T* B2 = q1 + d2; const T* q2 = B2 + (int64_t)d2 * d2;
+  T* PRE1 = reinterpret_cast<T*>(smem_raw);
+  T* PRE2 = PRE1 + d1 * G; T* PRE3 = PRE2 + d1 * G; T* PRE4 = PRE3 + d2 * G; T* A = PRE4 + d2 * G; T* B = A + dm * G;
+  const T* hb = Wt + pw.br + (int64_t)h * pw.br_stride; // B1 q1 B2 q2 w3 q3 (blob order)
+  const T* B1 = hb; const T* q1 = B1 + (int64_t)d2 * d1; const T* B2 = q1 + d2; const T* q2 = B2 + (int64_t)d2 * d2;
   const T* w3 = q2 + d2; const T* q3 = w3 + d2;
-  for (int g = 0; g < G; ++g) {
-    const int64_t sg = perm[p0 + min(g, cnt - 1)]; // padding slots repeat the last structure (results not written)
-    for (int f = threadIdx.x; f < F; f += POOL_THREADS) X[g * ld + f] = x[sg * F + f];
+  const T* B1t = Wt + pw.brT + (int64_t)h * pw.brT_stride; const T* B2t = B1t + (int64_t)d1 * d2;
+  for (int t = threadIdx.x; t < F * G; t += blockDim.x) { // padding slots repeat the last structure (results not written)
+    const int f = t / G, g = t - f * G;
+    B[t] = x[(int64_t)perm[p0 + min(g, cnt - 1)] * F + f];
   }
   __syncthreads();
-  auto act = [&](const T* pre, int n) {
-    __syncthreads();
-    for (int t = threadIdx.x; t < G * n; t += POOL_THREADS) { const int g = t / n, o = t - g * n; ACT[g * ld + o] = silu_f<T>(pre[g * ld + o]); }
+  auto fwd = [&](int n_out, int n_in, const T* Mt, const T* bias, const T* in, T* pre, T* out) {
+    matvec<T, G>(n_out, n_in, Mt, in, [&](int o, const T* acc) {
+      const T bo = bias[o];
+#pragma unroll
+      for (int g = 0; g < G; ++g) { const T p = acc[g] + bo; pre[o * G + g] = p; out[o * G + g] = silu_f<T>(p); }
+    });
     __syncthreads();
   };
-  layer_fwd<T, G>(d1, F, Wt + pw.P1, Wt + pw.p1, X, ld, PRE1, ld);    act(PRE1, d1);
-  layer_fwd<T, G>(d1, d1, Wt + pw.P2, Wt + pw.p2, ACT, ld, PRE2, ld); act(PRE2, d1);
-  layer_fwd<T, G>(d2, d1, B1, q1, ACT, ld, PRE3, ld);                 act(PRE3, d2);
-  layer_fwd<T, G>(d2, d2, B2, q2, ACT, ld, PRE4, ld);                 act(PRE4, d2);
+  fwd(d1, F, Wt + pw.P1t, Wt + pw.p1, B, PRE1, A);
+  fwd(d1, d1, Wt + pw.P2t, Wt + pw.p2, A, PRE2, B);
+  fwd(d2, d1, B1t, q1, B, PRE3, A);
+  fwd(d2, d2, B2t, q2, A, PRE4, B);
   { // E_g = w3 . z2 + q3: a warp per structure
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int g = warp; g < cnt; g += POOL_THREADS / 32) {
+    for (int g = warp; g < cnt; g += blockDim.x / 32) {
       T a = T(0);
-      for (int o = lane; o < d2; o += 32) a = fma(w3[o], ACT[g * ld + o], a);
+      for (int o = lane; o < d2; o += 32) a = fma(w3[o], B[o * G + g], a);
 #pragma unroll
       for (int m = 16; m; m >>= 1) a += __shfl_xor_sync(0xffffffffu, a, m);
       if (lane == 0) energy[perm[p0 + g]] = a + q3[0];
     }
   }
   if (!xbar) return;
+  for (int t = threadIdx.x; t < G * d2; t += blockDim.x) A[t] = w3[t / G] * dsilu_f<T>(PRE4[t]); // z2-bar (pre-activation)
   __syncthreads();
-  for (int t = threadIdx.x; t < G * d2; t += POOL_THREADS) { // z2-bar (pre-activation adjoint)
-    const int g = t / d2, o = t - g * d2;
-    GB[g * ld + o] = w3[o] * dsilu_f<T>(PRE4[g * ld + o]);
-  }
-  __syncthreads();
-  layer_bwd<T, G>(d2, d2, B2, GB, ld, PRE3, ld, ACT, ld);             __syncthreads(); // z1-bar in ACT
-  layer_bwd<T, G>(d2, d1, B1, ACT, ld, PRE2, ld, GB, ld);             __syncthreads(); // y2-bar in GB
-  layer_bwd<T, G>(d1, d1, Wt + pw.P2, GB, ld, PRE1, ld, ACT, ld);     __syncthreads(); // y1-bar in ACT
-  layer_bwd<T, G>(d1, F, Wt + pw.P1, ACT, ld, (const T*)nullptr, 0, GB, ld); __syncthreads(); // x-bar in GB
-  for (int g = 0; g < cnt; ++g) {
-    const int64_t sg = perm[p0 + g];
-    for (int f = threadIdx.x; f < F; f += POOL_THREADS) xbar[sg * F + f] = GB[g * ld + f];
+  auto bwd = [&](int n_out, int n_in, const T* M, const T* gb, const T* dpre, T* out) {
+    matvec<T, G>(n_in, n_out, M, gb, [&](int i, const T* acc) {
+#pragma unroll
+      for (int g = 0; g < G; ++g) out[i * G + g] = dpre ? acc[g] * dsilu_f<T>(dpre[i * G + g]) : acc[g];
+    });
+    __syncthreads();
+  };
+  bwd(d2, d2, B2, A, PRE3, B);                      // z1-bar
+  bwd(d2, d1, B1, B, PRE2, A);                      // y2-bar
+  bwd(d1, d1, Wt + pw.P2, A, PRE1, B);              // y1-bar
+  bwd(d1, F, Wt + pw.P1, B, (const T*)nullptr, A);  // x-bar
+  for (int t = threadIdx.x; t < F * G; t += blockDim.x) {
+    const int f = t / G, g = t - f * G;
+    if (g < cnt) xbar[(int64_t)perm[p0 + g] * F + f] = A[t];
   }
 }
 
@@ -198,29 +187,28 @@ pool_bcast_k(int64_t n, int F, const int32_t* __restrict__ a2s, const int32_t* _
   }
 }
 
-template <typename T> constexpr int pool_group() { return sizeof(T) == 8 ? 4 : 8; }
+template <typename T> constexpr int pool_group() { return sizeof(T) == 8 ? 8 : 16; }
 
 } // namespace
 
 int64_t pool_head_scratch_bytes(int64_t maxS, int F, int H, size_t elem) {
-  const int64_t G = elem == 8 ? 4 : 8;
+  const int64_t G = elem == 8 ? 8 : 16;
   return 2 * ((maxS * F * (int64_t)elem + 255) / 256 * 256) + (maxS * 4 + 255) / 256 * 256 +
          (((maxS + G - 1) / G + H) * 16 + 255) / 256 * 256 + 256;
 }
 
 bool pool_head_supported(int F, int d1, int d2, int H, size_t elem) {
   if (d1 < 1 || d2 < 1 || d1 > 4096 || d2 > 4096 || H > POOL_MAXH) return false;
-  const int64_t G = elem == 8 ? 4 : 8, dm = std::max(F, std::max(d1, d2));
-  return G * (F + 2 * d1 + 2 * d2 + 2 * dm) * (int64_t)elem <= 227 * 1024;
+  const int64_t G = elem == 8 ? 8 : 16, dm = std::max(F, std::max(d1, d2));
+  return G * (2 * d1 + 2 * d2 + 2 * dm) * (int64_t)elem <= 227 * 1024;
 }
 
 // energy [S] and, when sb != NULL, s-bar [N][F] of the pooled head.  scratch: pool_head_scratch_bytes().  Returns the
 // number of launches, -1 when the shapes are not supported.
 template <typename T>
 int launch_pool_head(int64_t N, int64_t S, int F, int H, int d1, int d2, const T* s, const int32_t* a2s,
-                     const int32_t* sptr, const int32_t* head, const T* W, int64_t oP1, int64_t op1, int64_t oP2,
-                     int64_t op2, int64_t obr, int64_t br_stride, void* scratch, T* energy, T* sb, int* d_err,
-                     cudaStream_t st) {
+                     const int32_t* sptr, const int32_t* head, const T* W, const PoolHeadW& pw, void* scratch, T* energy,
+                     T* sb, int* d_err, cudaStream_t st) {
   if (S == 0) return 0;
   if (!pool_head_supported(F, d1, d2, H, sizeof(T))) return -1;
   constexpr int G = pool_group<T>();
@@ -238,14 +226,15 @@ int launch_pool_head(int64_t N, int64_t S, int F, int H, int d1, int d2, const T
   head_sort_k<<<1, 1024, 0, st>>>(S, H, G, head, perm, tiles, ntiles, d_err);
   PNN_KCHECK("head_sort_k");
   const int dm = std::max(F, std::max(d1, d2));
-  const size_t smem = (size_t)G * (F + 2 * d1 + 2 * d2 + 2 * dm) * sizeof(T);
+  const size_t smem = (size_t)G * (2 * d1 + 2 * d2 + 2 * dm) * sizeof(T);
+  const int rounds = (dm + POOL_MAXT - 1) / POOL_MAXT;
+  const int nthr = std::max(64, ((dm + rounds - 1) / rounds + 31) / 32 * 32);
   static bool attr_set = false;
   if (!attr_set) {
     cudaFuncSetAttribute(pooled_head_k<T, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     attr_set = true;
   }
-  PoolW pw{oP1, op1, oP2, op2, obr, br_stride};
-  pooled_head_k<T, G><<<(unsigned)max_tiles, POOL_THREADS, smem, st>>>(F, d1, d2, W, pw, perm, tiles, ntiles, x, energy,
+  pooled_head_k<T, G><<<(unsigned)max_tiles, nthr, smem, st>>>(F, d1, d2, W, pw, perm, tiles, ntiles, x, energy,
                                                                        sb ? xbar : nullptr);
   PNN_KCHECK("pooled_head_k");
   int nl = 3;
@@ -259,10 +248,10 @@ int launch_pool_head(int64_t N, int64_t S, int F, int H, int d1, int d2, const T
 }
 
 template int launch_pool_head<float>(int64_t, int64_t, int, int, int, int, const float*, const int32_t*, const int32_t*,
-                                     const int32_t*, const float*, int64_t, int64_t, int64_t, int64_t, int64_t, int64_t,
-                                     void*, float*, float*, int*, cudaStream_t);
+                                     const int32_t*, const float*, const PoolHeadW&, void*, float*, float*, int*,
+                                     cudaStream_t);
 template int launch_pool_head<double>(int64_t, int64_t, int, int, int, int, const double*, const int32_t*, const int32_t*,
-                                      const int32_t*, const double*, int64_t, int64_t, int64_t, int64_t, int64_t, int64_t,
-                                      void*, double*, double*, int*, cudaStream_t);
+                                      const int32_t*, const double*, const PoolHeadW&, void*, double*, double*, int*,
+                                      cudaStream_t);
 
 } // namespace pnn
