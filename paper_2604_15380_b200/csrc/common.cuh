@@ -197,9 +197,13 @@ template <typename T>
 int launch_embed_globals(int64_t N, int F, int G, const int32_t* a2s, const double* glob, const T* globW, T* s,
                          __nv_bfloat16* s16, cudaStream_t st);
 // pool_head.cu: the paper's graph-level heads (mean pooling -> shared layers -> per-head branch layers; reading Q29)
-// element offsets in the device weight buffer: shared layers P1 [d1][F], p1, P2 [d1][d1], p2 and their transposes; per head
-// (stride br_stride, blob order) B1 [d2][d1] q1 B2 [d2][d2] q2 w3 q3; per head (stride brT_stride) B1^T [d1][d2] B2^T [d2][d2]
-struct PoolHeadW { int64_t P1, p1, P2, p2, P1t, P2t, br, br_stride, brT, brT_stride; };
+// element offsets in the device weight buffer (every array starts on a multiple of 4 elements: 16-byte loads): shared
+// layers P1 [d1][F], p1, P2 [d1][d1], p2 and the transposes P1t [F][d1], P2t [d1][d1]; per head, at br + h * br_stride:
+// B1 [d2][d1] at 0, q1, B2 [d2][d2], q2, w3, q3, B1t [d1][d2], B2t [d2][d2] at the o* offsets
+struct PoolHeadW {
+  int64_t P1, p1, P2, p2, P1t, P2t, br, br_stride;
+  int64_t oq1, oB2, oq2, ow3, oq3, oB1t, oB2t;
+};
 int64_t pool_head_scratch_bytes(int64_t maxS, int F, int H, size_t elem);
 bool pool_head_supported(int F, int d1, int d2, int H, size_t elem);
 template <typename T>

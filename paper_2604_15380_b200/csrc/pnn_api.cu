@@ -250,19 +250,22 @@ int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, 
     PoolHeadW& pw = m->pool;
     const double* P1 = take(d1 * F);  pw.P1 = put(P1, d1 * F);  pw.P1t = put_t(P1, d1, F);  pw.p1 = put(take(d1), d1);
     const double* P2 = take(d1 * d1); pw.P2 = put(P2, d1 * d1); pw.P2t = put_t(P2, d1, d1); pw.p2 = put(take(d1), d1);
-    pw.br_stride = d2 * d1 + d2 + d2 * d2 + d2 + d2 + 1;
-    pw.brT_stride = d1 * d2 + d2 * d2;
-    const double* br = take(cfg->H * pw.br_stride);
-    pw.br = put(br, cfg->H * pw.br_stride);
-    pw.brT = reserve(cfg->H * pw.brT_stride);
+    auto up4 = [](int64_t n) { return (n + 3) / 4 * 4; };
+    pw.oq1 = up4(d2 * d1);          pw.oB2 = pw.oq1 + up4(d2);      pw.oq2 = pw.oB2 + up4(d2 * d2);
+    pw.ow3 = pw.oq2 + up4(d2);      pw.oq3 = pw.ow3 + up4(d2);      pw.oB1t = pw.oq3 + 4;
+    pw.oB2t = pw.oB1t + up4(d1 * d2); pw.br_stride = pw.oB2t + up4(d2 * d2);
+    pw.br = reserve(cfg->H * pw.br_stride);
     for (int h = 0; h < cfg->H; ++h) {
-      const double* B1 = br + h * pw.br_stride;
-      const double* B2 = B1 + d2 * d1 + d2;
-      double* t1 = hb.data() + pw.brT + h * pw.brT_stride;
-      double* t2 = t1 + d1 * d2;
-      for (int64_t o = 0; o < d2; ++o) {
-        for (int64_t i = 0; i < d1; ++i) t1[i * d2 + o] = B1[o * d1 + i];
-        for (int64_t i = 0; i < d2; ++i) t2[i * d2 + o] = B2[o * d2 + i];
+      const double* B1 = take(d2 * d1); const double* q1 = take(d2);
+      const double* B2 = take(d2 * d2); const double* q2 = take(d2);
+      const double* w3 = take(d2);      const double* q3 = take(1);
+      double* o = hb.data() + pw.br + h * pw.br_stride;
+      std::memcpy(o, B1, sizeof(double) * d2 * d1);          std::memcpy(o + pw.oq1, q1, sizeof(double) * d2);
+      std::memcpy(o + pw.oB2, B2, sizeof(double) * d2 * d2); std::memcpy(o + pw.oq2, q2, sizeof(double) * d2);
+      std::memcpy(o + pw.ow3, w3, sizeof(double) * d2);      o[pw.oq3] = q3[0];
+      for (int64_t r = 0; r < d2; ++r) {
+        for (int64_t i = 0; i < d1; ++i) o[pw.oB1t + i * d2 + r] = B1[r * d1 + i];
+        for (int64_t i = 0; i < d2; ++i) o[pw.oB2t + i * d2 + r] = B2[r * d2 + i];
       }
     }
     if (cfg->n_global > 0) m->globW = put(take(F * cfg->n_global), F * cfg->n_global);

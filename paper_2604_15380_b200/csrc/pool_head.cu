@@ -21,7 +21,9 @@ namespace pnn {
 namespace {
 
 constexpr int POOL_THREADS = 256;
-constexpr int POOL_MAXT = 1024; // threads of pooled_head_k: one per output feature of the widest layer
+constexpr int POOL_RT = 2;      // outputs per thread of pooled_head_k (register tile POOL_RT x G)
+constexpr int POOL_U = 16;      // weight loads in flight per thread
+constexpr int POOL_MAXT = 512;  // threads of pooled_head_k: one per POOL_RT output features of the widest layer
 constexpr int POOL_MAXH = 1024;
 
 // x[g][f] = mean_i s[i][f]; one CTA per structure (grid-stride), threads over (atom slice, feature)
@@ -82,30 +84,99 @@ template <typename T> __device__ __forceinline__ T dsilu_f(T x) {
 }
 
 template <typename T> struct alignas(16) Vec16 { T v[16 / sizeof(T)]; };
+template <typename T, int RT> struct alignas(RT * sizeof(T) >= 16 ? 16 : RT * sizeof(T)) VecR { T v[RT]; };
 
-// acc[r][g] = sum_c M[c][r] v[c][g] for the CTA's G structures, then epi(r, acc): a thread per output r, the matrix row c
-// read coalesced over r, v[c][0..G) broadcast from shared memory with 16-byte loads.  Serves the forward layers with the
-// transposed weights (M = W^T [in][out]) and the adjoint with the original ones (M = W [out][in]).
-template <typename T, int G, typename Epi>
-__device__ __forceinline__ void matvec(int n_r, int n_c, const T* __restrict__ M, const T* v, Epi epi) {
-  constexpr int VW = 16 / sizeof(T);
-  for (int r = threadIdx.x; r < n_r; r += blockDim.x) {
-    T acc[G];
+template <typename T, int G, int RT, int U>
+struct MatTile {
+  static constexpr int VW = 16 / sizeof(T);
+  T acc[RT][G];
+  __device__ __forceinline__ void zero() {
 #pragma unroll
-    for (int g = 0; g < G; ++g) acc[g] = T(0);
-    const T* col = M + r;
-#pragma unroll 4
-    for (int c = 0; c < n_c; ++c) {
-      const T w = __ldg(col + (int64_t)c * n_r);
+    for (int i = 0; i < RT; ++i)
+#pragma unroll
+      for (int j = 0; j < G; ++j) acc[i][j] = T(0);
+  }
+  // acc += sum_{c in [c0, c1)} M[c][r0 .. r0+4) (x) v[c][0..G); the weight loads of the next U rows are in flight while
+  // the FMAs of the current U rows issue
+  __device__ __forceinline__ void run(int r0, int n_r, int c0, int c1, const T* __restrict__ M, const T* v) {
+    const bool vec = (n_r % RT) == 0;
+    const T* col = M + r0;
+    auto load_w = [&](int c, VecR<T, RT>& w) {
+      if (vec) { w = *reinterpret_cast<const VecR<T, RT>*>(col + (int64_t)c * n_r); }
+      else {
+#pragma unroll
+        for (int i = 0; i < RT; ++i) w.v[i] = (r0 + i < n_r) ? __ldg(col + (int64_t)c * n_r + i) : T(0);
+      }
+    };
+    auto fmas = [&](const VecR<T, RT>& w, int c) {
       const Vec16<T>* vc = reinterpret_cast<const Vec16<T>*>(v + c * G);
 #pragma unroll
       for (int q = 0; q < G / VW; ++q) {
         const Vec16<T> x = vc[q];
 #pragma unroll
-        for (int e = 0; e < VW; ++e) acc[q * VW + e] = fma(w, x.v[e], acc[q * VW + e]);
+        for (int i = 0; i < RT; ++i)
+#pragma unroll
+          for (int e = 0; e < VW; ++e) acc[i][q * VW + e] = fma(w.v[i], x.v[e], acc[i][q * VW + e]);
       }
+    };
+    int c = c0;
+    for (; c + U <= c1; c += U) { // U weight loads in flight per thread, then their FMAs
+      VecR<T, RT> w[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) load_w(c + u, w[u]);
+#pragma unroll
+      for (int u = 0; u < U; ++u) fmas(w[u], c + u);
     }
-    epi(r, acc);
+    for (; c < c1; ++c) {
+      VecR<T, RT> w;
+      load_w(c, w);
+      fmas(w, c);
+    }
+  }
+};
+
+// out[r][g] = sum_c M[c][r] v[c][g] for the CTA's G structures, then epi(r, g, value).  A thread owns RT = POOL_RT consecutive
+// outputs r for all G structures (an RT x G register tile): per c one 16-byte (float) weight load, coalesced over r, and
+// G values of v broadcast from shared memory for RT * G FMAs (a thread per output would spend G broadcast loads on G FMAs
+// and is bound by the shared-memory return path).  Narrow layers (all outputs inside one warp) split the sum over c
+// between the warps and add the partial tiles in warp order through `scratch` (deterministic).
+// Serves the forward layers with the transposed weights (M = W^T [in][out]) and the adjoint with the original ones
+// (M = W [out][in]).  M must be 16-byte aligned; rows are loaded as vectors when n_r is a multiple of RT.
+template <typename T, int G, typename Epi>
+__device__ __forceinline__ void matvec(int n_r, int n_c, const T* __restrict__ M, const T* v, T* scratch, int scratch_elems,
+                                       Epi epi) {
+  constexpr int RT = POOL_RT;
+  const int nw = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  MatTile<T, G, RT, POOL_U> t;
+  if (n_r <= 32 * RT && n_c >= 64 && nw * n_r * G <= scratch_elems) { // split over c
+    const int per = (n_c + nw - 1) / nw, c0 = warp * per, c1 = min(n_c, c0 + per), r0 = lane * RT;
+    if (r0 < n_r) {
+      t.zero();
+      t.run(r0, n_r, c0, c1, M, v);
+#pragma unroll
+      for (int i = 0; i < RT; ++i)
+        if (r0 + i < n_r) {
+#pragma unroll
+          for (int j = 0; j < G; ++j) scratch[(warp * n_r + r0 + i) * G + j] = t.acc[i][j];
+        }
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < n_r * G; e += blockDim.x) {
+      T sum = T(0);
+      for (int w = 0; w < nw; ++w) sum += scratch[w * n_r * G + e];
+      epi(e / G, e % G, sum);
+    }
+    return;
+  }
+  for (int r0 = threadIdx.x * RT; r0 < n_r; r0 += blockDim.x * RT) {
+    t.zero();
+    t.run(r0, n_r, 0, n_c, M, v);
+#pragma unroll
+    for (int i = 0; i < RT; ++i)
+      if (r0 + i < n_r) {
+#pragma unroll
+        for (int j = 0; j < G; ++j) epi(r0 + i, j, t.acc[i][j]);
+      }
   }
 }
 
@@ -124,27 +195,26 @@ pooled_head_k(int F, int d1, int d2, const T* __restrict__ Wt, PoolHeadW pw, con
   const int dm = max(F, max(d1, d2));
   T* PRE1 = reinterpret_cast<T*>(smem_raw);
   T* PRE2 = PRE1 + d1 * G; T* PRE3 = PRE2 + d1 * G; T* PRE4 = PRE3 + d2 * G; T* A = PRE4 + d2 * G; T* B = A + dm * G;
-  const T* hb = Wt + pw.br + (int64_t)h * pw.br_stride; // B1 q1 B2 q2 w3 q3 (blob order)
-  const T* B1 = hb; const T* q1 = B1 + (int64_t)d2 * d1; const T* B2 = q1 + d2; const T* q2 = B2 + (int64_t)d2 * d2;
-  const T* w3 = q2 + d2; const T* q3 = w3 + d2;
-  const T* B1t = Wt + pw.brT + (int64_t)h * pw.brT_stride; const T* B2t = B1t + (int64_t)d1 * d2;
+  const T* B1 = Wt + pw.br + (int64_t)h * pw.br_stride;
+  const T* q1 = B1 + pw.oq1; const T* B2 = B1 + pw.oB2; const T* q2 = B1 + pw.oq2; const T* w3 = B1 + pw.ow3;
+  const T* q3 = B1 + pw.oq3; const T* B1t = B1 + pw.oB1t; const T* B2t = B1 + pw.oB2t;
   for (int t = threadIdx.x; t < F * G; t += blockDim.x) { // padding slots repeat the last structure (results not written)
     const int f = t / G, g = t - f * G;
     B[t] = x[(int64_t)perm[p0 + min(g, cnt - 1)] * F + f];
   }
   __syncthreads();
-  auto fwd = [&](int n_out, int n_in, const T* Mt, const T* bias, const T* in, T* pre, T* out) {
-    matvec<T, G>(n_out, n_in, Mt, in, [&](int o, const T* acc) {
-      const T bo = bias[o];
-#pragma unroll
-      for (int g = 0; g < G; ++g) { const T p = acc[g] + bo; pre[o * G + g] = p; out[o * G + g] = silu_f<T>(p); }
+  // split: PRE3 | PRE4 are free (not yet written / already consumed) and may hold the partial tiles of a narrow layer
+  auto fwd = [&](int n_out, int n_in, const T* Mt, const T* bias, const T* in, T* pre, T* out, bool split) {
+    matvec<T, G>(n_out, n_in, Mt, in, PRE3, split ? 2 * d2 * G : 0, [&](int o, int g, T acc) {
+      const T p = acc + bias[o];
+      pre[o * G + g] = p; out[o * G + g] = silu_f<T>(p);
     });
     __syncthreads();
   };
-  fwd(d1, F, Wt + pw.P1t, Wt + pw.p1, B, PRE1, A);
-  fwd(d1, d1, Wt + pw.P2t, Wt + pw.p2, A, PRE2, B);
-  fwd(d2, d1, B1t, q1, B, PRE3, A);
-  fwd(d2, d2, B2t, q2, A, PRE4, B);
+  fwd(d1, F, Wt + pw.P1t, Wt + pw.p1, B, PRE1, A, true);
+  fwd(d1, d1, Wt + pw.P2t, Wt + pw.p2, A, PRE2, B, true);
+  fwd(d2, d1, B1t, q1, B, PRE3, A, false);
+  fwd(d2, d2, B2t, q2, A, PRE4, B, false);
   { // E_g = w3 . z2 + q3: a warp per structure
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int g = warp; g < cnt; g += blockDim.x / 32) {
@@ -158,17 +228,16 @@ pooled_head_k(int F, int d1, int d2, const T* __restrict__ Wt, PoolHeadW pw, con
   if (!xbar) return;
   for (int t = threadIdx.x; t < G * d2; t += blockDim.x) A[t] = w3[t / G] * dsilu_f<T>(PRE4[t]); // z2-bar (pre-activation)
   __syncthreads();
-  auto bwd = [&](int n_out, int n_in, const T* M, const T* gb, const T* dpre, T* out) {
-    matvec<T, G>(n_in, n_out, M, gb, [&](int i, const T* acc) {
-#pragma unroll
-      for (int g = 0; g < G; ++g) out[i * G + g] = dpre ? acc[g] * dsilu_f<T>(dpre[i * G + g]) : acc[g];
+  auto bwd = [&](int n_out, int n_in, const T* M, const T* gb, const T* dpre, T* out, bool split) {
+    matvec<T, G>(n_in, n_out, M, gb, PRE3, split ? 2 * d2 * G : 0, [&](int i, int g, T acc) {
+      out[i * G + g] = dpre ? acc * dsilu_f<T>(dpre[i * G + g]) : acc;
     });
     __syncthreads();
   };
-  bwd(d2, d2, B2, A, PRE3, B);                      // z1-bar
-  bwd(d2, d1, B1, B, PRE2, A);                      // y2-bar
-  bwd(d1, d1, Wt + pw.P2, A, PRE1, B);              // y1-bar
-  bwd(d1, F, Wt + pw.P1, B, (const T*)nullptr, A);  // x-bar
+  bwd(d2, d2, B2, A, PRE3, B, false);                      // z1-bar
+  bwd(d2, d1, B1, B, PRE2, A, true);                       // y2-bar
+  bwd(d1, d1, Wt + pw.P2, A, PRE1, B, true);               // y1-bar
+  bwd(d1, F, Wt + pw.P1, B, (const T*)nullptr, A, true);   // x-bar
   for (int t = threadIdx.x; t < F * G; t += blockDim.x) {
     const int f = t / G, g = t - f * G;
     if (g < cnt) xbar[(int64_t)perm[p0 + g] * F + f] = A[t];
@@ -227,8 +296,9 @@ int launch_pool_head(int64_t N, int64_t S, int F, int H, int d1, int d2, const T
   PNN_KCHECK("head_sort_k");
   const int dm = std::max(F, std::max(d1, d2));
   const size_t smem = (size_t)G * (2 * d1 + 2 * d2 + 2 * dm) * sizeof(T);
-  const int rounds = (dm + POOL_MAXT - 1) / POOL_MAXT;
-  const int nthr = std::max(64, ((dm + rounds - 1) / rounds + 31) / 32 * 32);
+  const int nq = (dm + POOL_RT - 1) / POOL_RT; // a thread per POOL_RT outputs
+  const int rounds = (nq + POOL_MAXT - 1) / POOL_MAXT;
+  const int nthr = std::max(64, ((nq + rounds - 1) / rounds + 31) / 32 * 32);
   static bool attr_set = false;
   if (!attr_set) {
     cudaFuncSetAttribute(pooled_head_k<T, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
