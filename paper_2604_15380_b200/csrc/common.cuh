@@ -196,6 +196,13 @@ int launch_embed(int64_t N, int F, int Zmax, const int32_t* Z, const T* emb, T* 
 template <typename T>
 int launch_embed_globals(int64_t N, int F, int G, const int32_t* a2s, const double* glob, const T* globW, T* s,
                          __nv_bfloat16* s16, cudaStream_t st);
+// edge_dmma.cu: FP64 edge kernels with the filter contraction on the FP64 tensor cores (F a multiple of 64)
+bool edge_dmma_supported(int F, int K);
+int launch_edge_fwd_dmma(const EdgeArgs<double>& a, const double* phi, const double* s_in, int64_t ld_sin, const double* v_in,
+                         const double* v_res, double* s1, int64_t ld_s1, double* v1, cudaStream_t st);
+int launch_edge_bwd_dmma(const EdgeArgs<double>& a, const double* phi, const double* v_in, const double* sb1,
+                         const double* vb1, double* phib, double* vb_in, double* fpart, int first_block, cudaStream_t st);
+int edge_dmma_num_slabs(int F);
 // pool_head.cu: the paper's graph-level heads (mean pooling -> shared layers -> per-head branch layers; reading Q29)
 // element offsets in the device weight buffer (every array starts on a multiple of 4 elements: 16-byte loads): shared
 // layers P1 [d1][F], p1, P2 [d1][d1], p2 and the transposes P1t [F][d1], P2t [d1][d1]; per head, at br + h * br_stride:

@@ -630,6 +630,9 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       if constexpr (std::is_same<T, float>::value) {
         float* wt = (want_f && ws->etape) ? ws->etape + (int64_t)t * ws->etape_block : nullptr;
         l_ = launch_edge_fwd_warp(ea, phi, s_cur, F, v_in, sn, 2 * F, v1, wt, wt ? wt + ws->etape_block / 2 : nullptr, st);
+      } else if constexpr (std::is_same<T, double>::value) {
+        l_ = edge_dmma_supported(F, c.K) ? launch_edge_fwd_dmma(ea, phi, s_cur, F, v_in, v_in, sn, 2 * F, v1, st)
+                                         : launch_edge_fwd<T, T>(ea, phi, s_cur, F, v_in, v_in, sn, 2 * F, v1, EdgeMirror(), st);
       } else {
         l_ = launch_edge_fwd<T, T>(ea, phi, s_cur, F, v_in, v_in, sn, 2 * F, v1, EdgeMirror(), st);
       }
@@ -720,7 +723,14 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
                                       t > 0 ? phib : nullptr, vb2, fpart, last ? 1 : 0, st);
           }
         }
-        if (!taped_edges)
+        bool dmma_edges = false;
+        if constexpr (std::is_same<T, double>::value) {
+          dmma_edges = edge_dmma_supported(F, c.K);
+          if (dmma_edges)
+            l_ = launch_edge_bwd_dmma(ea, (const T*)tp.phi, (const T*)tp.v_in, sb, vb, t > 0 ? phib : nullptr, vb2, fpart,
+                                      last ? 1 : 0, st);
+        }
+        if (!taped_edges && !dmma_edges)
           l_ = launch_edge_bwd<T, T>(ea, (const T*)tp.phi, (const T*)tp.v_in, sb, vb, t > 0 ? phib : nullptr, vb2, fpart,
                                      last ? 1 : 0, nullptr, st);
         nl += l_; ps_.done(l_); }
@@ -738,6 +748,8 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     }
     { ProfScope ps_(ws, st, "force_assemble");
       int nslab = edge_num_slabs(F);
+      if constexpr (std::is_same<T, double>::value)
+        if (edge_dmma_supported(F, c.K)) nslab = edge_dmma_num_slabs(F);
       if constexpr (std::is_same<T, float>::value)
         if (ws->etape != nullptr) nslab = edge_warp_num_slabs(F, c.K);
       if (c.max_neighbors > 0) nslab = 1;
