@@ -36,6 +36,16 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
 
 __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
 
+// 16-byte asynchronous global -> shared copies (LDGSTS): the gathers of the next tile land in the warp's shared-memory slots
+// while the tensor cores work on the current one, without holding registers
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+  const uint32_t s_ = (uint32_t)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s_), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+constexpr int GSLOTS = 8; // gather slots (16 bytes per lane each) per tile and warp
+
 // --------------------------------------------------------------------------------------------------- forward
 // Staged pass (double-buffered): G = radial basis WITHOUT the cutoff (the epilogue multiplies by c(d): w = c (D + b)), so
 // that staging G needs d only and runs in the same phase as staging u, c, j — one CTA barrier per pass.
@@ -254,6 +264,7 @@ edge_bwd_dmma_k(EdgeArgs<double> a, int RB, const double* __restrict__ phi, cons
   double* const sm = reinterpret_cast<double*>(smem_raw);
   double* const FW = sm + 2 * BUF_D;                               // [2][12][3]
   int* const Jb = reinterpret_cast<int*>(FW + 2 * 12 * 3);         // [2][DPASS]
+  double2* const GS = reinterpret_cast<double2*>(Jb + 2 * DPASS);  // [12 warps][2 stages][GSLOTS][32 lanes]
   auto G1 = [&](int b) { return sm + b * BUF_D; };
   auto G2 = [&](int b) { return sm + b * BUF_D + DPASS * LD; };
   auto Ub = [&](int b) { return sm + b * BUF_D + 2 * DPASS * LD; };              // ux uy uz c
@@ -403,23 +414,35 @@ edge_bwd_dmma_k(EdgeArgs<double> a, int RB, const double* __restrict__ phi, cons
       const int64_t this_i = i;
       const double* g1 = G1(cur); const double* g2 = G2(cur); const double* ub = Ub(cur); const double* vb = Vb(cur);
       const int* jb = Jb + cur * DPASS;
-      for (int t = 0; t < nT; ++t) {
-        const int slot = t * DT + row;
-        const int64_t j = jb[slot];
-        // gathers first, the DMMAs do not depend on them
-        double2 gq[8];
+      double2* const gsw = GS + (warp * 2 * GSLOTS) * 32 + lane; // this lane's slots: [stage][slot] at stride 32
+      auto issue = [&](int t) { // asynchronous gathers of tile t into stage t & 1
+        const int64_t j = jb[t * DT + row];
+        double2* dst = gsw + (t & 1) * GSLOTS * 32;
         if (ss) {
-          gq[0] = ldg2(phi + j * 3 * F + fo); gq[1] = ldg2(phi + j * 3 * F + fo + 8);
-          gq[2] = ldg2(sb1 + j * F + fo);     gq[3] = ldg2(sb1 + j * F + fo + 8);
+          cp_async16(dst, phi + j * 3 * F + fo);      cp_async16(dst + 32, phi + j * 3 * F + fo + 8);
+          cp_async16(dst + 64, sb1 + j * F + fo);     cp_async16(dst + 96, sb1 + j * F + fo + 8);
         } else {
-          gq[0] = ldg2(phi + j * 3 * F + F + fo); gq[1] = ldg2(phi + j * 3 * F + 2 * F + fo);
+          cp_async16(dst, phi + j * 3 * F + F + fo);  cp_async16(dst + 32, phi + j * 3 * F + 2 * F + fo);
 #pragma unroll
-          for (int q = 0; q < 3; ++q) gq[2 + q] = ldg2(vb1 + (j * 3 + q) * F + fo);
+          for (int q = 0; q < 3; ++q) cp_async16(dst + (2 + q) * 32, vb1 + (j * 3 + q) * F + fo);
           if (has_v) {
 #pragma unroll
-            for (int q = 0; q < 3; ++q) gq[5 + q] = ldg2(v_in + (j * 3 + q) * F + fo);
+            for (int q = 0; q < 3; ++q) cp_async16(dst + (5 + q) * 32, v_in + (j * 3 + q) * F + fo);
           }
         }
+        cp_async_commit();
+      };
+      issue(0);
+      // stage the next pass into the other buffer behind the first tile's gathers
+      if (last) ni = find_pass(i + 1, np0, neb);
+      if (ni < i1) stage(cur ^ 1, np0, min(DPASS, neb - np0));
+      for (int t = 0; t < nT; ++t) {
+        const int slot = t * DT + row;
+        if (t + 1 < nT) { issue(t + 1); cp_async_wait<1>(); } else cp_async_wait<0>();
+        const double2* src = gsw + (t & 1) * GSLOTS * 32;
+        double2 gq[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) gq[q] = ((ss && q >= 4) || (!ss && !has_v && q >= 5)) ? make_double2(0.0, 0.0) : src[q * 32];
         const double4 uc = *reinterpret_cast<const double4*>(ub + slot * 4);
         const double2 cd = *reinterpret_cast<const double2*>(vb + slot * 2); // c', 1/d
         double d1[2][2] = {}, d2[2][2] = {};
@@ -481,10 +504,6 @@ edge_bwd_dmma_k(EdgeArgs<double> a, int RB, const double* __restrict__ phi, cons
           const double bu = fma(bs[0], u[0], fma(bs[1], u[1], bs[2] * u[2]));
 #pragma unroll
           for (int q = 0; q < 3; ++q) fp[q] += fma(dps, u[q], (bs[q] - bu * u[q]) * cd.y);
-        }
-        if (t == 0) { // stage the next pass into the other buffer behind the first tile
-          if (last) ni = find_pass(i + 1, np0, neb);
-          if (ni < i1) stage(cur ^ 1, np0, min(DPASS, neb - np0));
         }
       }
       if (last) {
@@ -553,12 +572,13 @@ int launch_edge_bwd_dmma(const EdgeArgs<double>& a, const double* phi, const dou
   const int64_t nwork = (a.N + RB - 1) / RB;
   dim3 grid((unsigned)std::min<int64_t>(nwork, 148 * 8), a.F / DFS);
   const int KS = (a.K + 3) / 4, LD = 4 * KS + GPAD;
-  const size_t smem = sizeof(double) * (2 * (2 * DPASS * LD + DPASS * 6) + 2 * 12 * 3) + sizeof(int) * 2 * DPASS;
+  const size_t smem = sizeof(double) * (2 * (2 * DPASS * LD + DPASS * 6) + 2 * 12 * 3) + sizeof(int) * 2 * DPASS +
+                      (size_t)12 * 2 * GSLOTS * 32 * 16;
 #define PNN_LAUNCH_DB(KSV)                                                                                              \
   {                                                                                                                     \
     static bool attr_set = false;                                                                                       \
     if (!attr_set) {                                                                                                    \
-      cudaFuncSetAttribute(edge_bwd_dmma_k<KSV>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);              \
+      cudaFuncSetAttribute(edge_bwd_dmma_k<KSV>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);              \
       attr_set = true;                                                                                                  \
     }                                                                                                                   \
     edge_bwd_dmma_k<KSV><<<grid, DTHR, smem, st>>>(a, RB, phi, v_in, sb1, vb1, phib, vb_in, fpart, first_block);        \
