@@ -140,6 +140,11 @@ template <typename T>
 int launch_gemm(int64_t M, int N, int K, const T* A, int64_t lda, const T* B, int64_t ldb, T* C, int64_t ldc,
                 const GemmEpi<T>& epi, cudaStream_t st);
 
+// gemm_dmma.cu: the FP64 contraction on the FP64 tensor cores (N a multiple of 64, K of 16)
+bool gemm_dmma_supported(int64_t M, int N, int K);
+int launch_gemm_dmma(int64_t M, int N, int K, const double* A, int64_t lda, const double* B, int64_t ldb, double* C,
+                     int64_t ldc, const GemmEpi<double>& epi, cudaStream_t st);
+
 // edge.cu
 template <typename T>
 struct EdgeArgs {

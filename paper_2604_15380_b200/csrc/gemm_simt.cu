@@ -207,6 +207,8 @@ int launch_gemm(int64_t M, int N, int K, const T* A, int64_t lda, const T* B, in
       }
     }
   } else {
+    // FP64: the tensor-core kernel (gemm_dmma.cu) whenever the shape allows; the ALU kernel takes the rest (N < 64, ...)
+    if (gemm_dmma_supported(M, N, K)) return launch_gemm_dmma(M, N, K, A, lda, B, ldb, C, ldc, epi, st);
     // FP64: 128x128 tiles (8x8 per thread) for large problems, 64x64 (4x4) below ~2 waves of big tiles.
     const int64_t big_tiles = ((M + 127) / 128) * ((N + 127) / 128);
     if (big_tiles >= 2 * 148 && N >= 128) {
