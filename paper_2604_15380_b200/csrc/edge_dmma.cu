@@ -16,6 +16,7 @@
 // warp.  A pass = the next <= 64 edges of ONE receiver in tiles of 8 (rows past the end carry cutoff 0, i.e. weight 0, and
 // gather a valid row).  Used by the FP64 model whenever F is a multiple of 64.
 #include <algorithm>
+#include <type_traits>
 
 #include "common.cuh"
 
@@ -44,7 +45,8 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-constexpr int GSLOTS = 8; // gather slots (16 bytes per lane each) per tile and warp
+constexpr int GSLOTS = 8; // gather slots (16 bytes per lane each) per tile and warp, reverse kernel
+constexpr int FSLOTS = 5; // ... forward kernel
 
 // --------------------------------------------------------------------------------------------------- forward
 // Staged pass (double-buffered): G = radial basis WITHOUT the cutoff (the epilogue multiplies by c(d): w = c (D + b)), so
@@ -56,9 +58,11 @@ edge_fwd_dmma_k(EdgeArgs<double> a, int RB, const double* __restrict__ phi, cons
                 double* __restrict__ v1) {
   if (*a.d_err & ERRF_EDGE_OVERFLOW) return;
   constexpr int KP = 4 * KS, LD = KP + GPAD;
-  __shared__ __align__(16) double Gs[2][DPASS * LD]; // radial basis (no cutoff)
-  __shared__ __align__(16) double Us[2][DPASS * 4];  // ux uy uz c(d); c = 0 on rows past the end of the pass
-  __shared__ int Js[2][DPASS];
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double (*const Gs)[DPASS * LD] = reinterpret_cast<double (*)[DPASS * LD]>(smem_raw);                 // [2] radial basis (no cutoff)
+  double (*const Us)[DPASS * 4] = reinterpret_cast<double (*)[DPASS * 4]>(smem_raw + sizeof(double) * 2 * DPASS * LD); // [2] ux uy uz c(d)
+  int (*const Js)[DPASS] = reinterpret_cast<int (*)[DPASS]>(smem_raw + sizeof(double) * 2 * DPASS * (LD + 4));       // [2]
+  double2* const GS = reinterpret_cast<double2*>(smem_raw + sizeof(double) * 2 * DPASS * (LD + 4) + sizeof(int) * 2 * DPASS); // gathers
   const int F = a.F, K = a.K;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int row = lane >> 2, cp = lane & 3;
@@ -159,69 +163,85 @@ edge_fwd_dmma_k(EdgeArgs<double> a, int RB, const double* __restrict__ phi, cons
       int64_t ni = i;
       int np0 = p0 + DPASS, neb = eb;
       const int64_t this_i = i;
-      // gathers run one tile ahead of the arithmetic (two register sets, loop unrolled by two)
-      struct Gath { double2 pa, pb, v0, v1, v2; };
-      auto load_tile = [&](int t, Gath& g) {
+      // Gathers of tile t + 1 travel as asynchronous copies into the warp's shared-memory slots and its DMMAs are issued
+      // in the same basic block as the epilogue of tile t (independent instruction streams the scheduler can interleave:
+      // the tensor pipe is then fed while the FP64 ALUs finish the previous tile).
+      auto consume = [&](auto ss_c, auto hv_c) {
+      constexpr bool SS_ = decltype(ss_c)::value, HV_ = decltype(hv_c)::value;
+      double2* const gsw = GS + (warp * 2 * FSLOTS) * 32 + lane;
+      auto issue = [&](int t) {
         const int64_t j = Js[cur][t * DT + row];
         const double* pj = phi + j * 3 * F + f0 + 2 * cp;
-        if (ss) { g.pa = ldg2(pj); g.pb = ldg2(pj + 8); }
+        double2* dst = gsw + (t & 1) * FSLOTS * 32;
+        if (SS_) { cp_async16(dst, pj); cp_async16(dst + 32, pj + 8); }
         else {
-          g.pa = ldg2(pj + F);
-          if (has_v) {
-            g.pb = ldg2(pj + 2 * F);
+          cp_async16(dst, pj + F);
+          if (HV_) {
+            cp_async16(dst + 32, pj + 2 * F);
             const double* vp = v_in + j * 3 * F + f0 + 2 * cp;
-            g.v0 = ldg2(vp); g.v1 = ldg2(vp + F); g.v2 = ldg2(vp + 2 * F);
+            cp_async16(dst + 64, vp); cp_async16(dst + 96, vp + F); cp_async16(dst + 128, vp + 2 * F);
           }
         }
+        cp_async_commit();
       };
-      auto compute = [&](int t, const Gath& g) {
-        const int slot = t * DT + row;
-        const double4 uc = *reinterpret_cast<const double4*>(&Us[cur][slot * 4]); // ux uy uz c
-        const double* Ar = &Gs[cur][slot * LD + cp];
-        double d[2][2][2] = {}; // [block][chain][half]: two chains over the k-steps per accumulator
-        if (ss || has_v) {
+      auto mma = [&](int t, double (&d)[2][2]) {
+        const double* Ar = &Gs[cur][(t * DT + row) * LD + cp];
+        d[0][0] = d[0][1] = d[1][0] = d[1][1] = 0.0;
+        if (SS_ || HV_) {
 #pragma unroll
           for (int ks = 0; ks < KS; ++ks) {
             const double av = Ar[4 * ks];
-            dmma884(d[0][ks & 1][0], d[0][ks & 1][1], av, wf[0][ks]);
-            dmma884(d[1][ks & 1][0], d[1][ks & 1][1], av, wf[1][ks]);
+            dmma884(d[0][0], d[0][1], av, wf[0][ks]);
+            dmma884(d[1][0], d[1][1], av, wf[1][ks]);
           }
         } else {
 #pragma unroll
-          for (int ks = 0; ks < KS; ++ks) dmma884(d[0][ks & 1][0], d[0][ks & 1][1], Ar[4 * ks], wf[0][ks]);
+          for (int ks = 0; ks < KS; ++ks) dmma884(d[0][0], d[0][1], Ar[4 * ks], wf[0][ks]);
         }
-        const double w00 = uc.w * (d[0][0][0] + d[0][1][0] + bias[0][0]), w01 = uc.w * (d[0][0][1] + d[0][1][1] + bias[0][1]);
-        const double w10 = uc.w * (d[1][0][0] + d[1][1][0] + bias[1][0]), w11 = uc.w * (d[1][0][1] + d[1][1][1] + bias[1][1]);
-        if (ss) {
-          acc[0][0][0] = fma(g.pa.x, w00, acc[0][0][0]); acc[0][0][1] = fma(g.pa.y, w01, acc[0][0][1]);
-          acc[0][1][0] = fma(g.pb.x, w10, acc[0][1][0]); acc[0][1][1] = fma(g.pb.y, w11, acc[0][1][1]);
+      };
+      auto epi = [&](int t, const double (&d)[2][2]) {
+        const int slot = t * DT + row;
+        const double4 uc = *reinterpret_cast<const double4*>(&Us[cur][slot * 4]); // ux uy uz c
+        const double2* src = gsw + (t & 1) * FSLOTS * 32;
+        const double w00 = uc.w * (d[0][0] + bias[0][0]), w01 = uc.w * (d[0][1] + bias[0][1]);
+        const double w10 = uc.w * (d[1][0] + bias[1][0]), w11 = uc.w * (d[1][1] + bias[1][1]);
+        const double2 pa = src[0];
+        if (SS_) {
+          const double2 pb = src[32];
+          acc[0][0][0] = fma(pa.x, w00, acc[0][0][0]); acc[0][0][1] = fma(pa.y, w01, acc[0][0][1]);
+          acc[0][1][0] = fma(pb.x, w10, acc[0][1][0]); acc[0][1][1] = fma(pb.y, w11, acc[0][1][1]);
         } else {
-          const double xs0 = g.pa.x * w00, xs1 = g.pa.y * w01;
+          const double xs0 = pa.x * w00, xs1 = pa.y * w01;
           acc[0][0][0] = fma(xs0, uc.x, acc[0][0][0]); acc[0][0][1] = fma(xs1, uc.x, acc[0][0][1]);
           acc[1][0][0] = fma(xs0, uc.y, acc[1][0][0]); acc[1][0][1] = fma(xs1, uc.y, acc[1][0][1]);
           acc[2][0][0] = fma(xs0, uc.z, acc[2][0][0]); acc[2][0][1] = fma(xs1, uc.z, acc[2][0][1]);
-          if (has_v) {
-            const double xv0 = g.pb.x * w10, xv1 = g.pb.y * w11;
-            acc[0][0][0] = fma(xv0, g.v0.x, acc[0][0][0]); acc[0][0][1] = fma(xv1, g.v0.y, acc[0][0][1]);
-            acc[1][0][0] = fma(xv0, g.v1.x, acc[1][0][0]); acc[1][0][1] = fma(xv1, g.v1.y, acc[1][0][1]);
-            acc[2][0][0] = fma(xv0, g.v2.x, acc[2][0][0]); acc[2][0][1] = fma(xv1, g.v2.y, acc[2][0][1]);
+          if (HV_) {
+            const double2 pb = src[32], v0 = src[64], v1_ = src[96], v2 = src[128];
+            const double xv0 = pb.x * w10, xv1 = pb.y * w11;
+            acc[0][0][0] = fma(xv0, v0.x, acc[0][0][0]);  acc[0][0][1] = fma(xv1, v0.y, acc[0][0][1]);
+            acc[1][0][0] = fma(xv0, v1_.x, acc[1][0][0]); acc[1][0][1] = fma(xv1, v1_.y, acc[1][0][1]);
+            acc[2][0][0] = fma(xv0, v2.x, acc[2][0][0]);  acc[2][0][1] = fma(xv1, v2.y, acc[2][0][1]);
           }
         }
       };
-      Gath g0, g1;
-      load_tile(0, g0);
-      for (int t = 0; t < nT; t += 2) {
-        if (t + 1 < nT) load_tile(t + 1, g1);
-        compute(t, g0);
-        if (t == 0) { // stage the next pass into the other buffer behind the first tile
-          if (last) ni = find_pass(i + 1, np0, neb);
-          if (ni < i1) stage(cur ^ 1, np0, min(DPASS, neb - np0));
-        }
-        if (t + 1 < nT) {
-          if (t + 2 < nT) load_tile(t + 2, g0);
-          compute(t + 1, g1);
-        }
+      issue(0);
+      // stage the next pass into the other buffer behind the first tile's gathers
+      if (last) ni = find_pass(i + 1, np0, neb);
+      if (ni < i1) stage(cur ^ 1, np0, min(DPASS, neb - np0));
+      double dA[2][2], dB[2][2];
+      mma(0, dA);
+      for (int t = 0;;) { // DMMAs of tile t + 1 and epilogue of tile t in ONE basic block (two register sets, unrolled by two)
+        if (t + 1 >= nT) { cp_async_wait<0>(); epi(t, dA); break; }
+        issue(t + 1); cp_async_wait<1>(); mma(t + 1, dB); epi(t, dA);
+        ++t;
+        if (t + 1 >= nT) { cp_async_wait<0>(); epi(t, dB); break; }
+        issue(t + 1); cp_async_wait<1>(); mma(t + 1, dA); epi(t, dB);
+        ++t;
       }
+      };
+      if (ss) consume(std::true_type(), std::true_type());
+      else if (has_v) consume(std::false_type(), std::true_type());
+      else consume(std::false_type(), std::false_type());
       if (last) { // the eight edge rows of the warp meet; lanes 0-3 (row 0) write the receiver's row
 #pragma unroll
         for (int q = 0; q < 3; ++q)
@@ -548,8 +568,16 @@ int launch_edge_fwd_dmma(const EdgeArgs<double>& a, const double* phi, const dou
   const int64_t nwork = (a.N + RB - 1) / RB;
   dim3 grid((unsigned)std::min<int64_t>(nwork, 148 * 8), a.F / DFS);
   const int KS = (a.K + 3) / 4;
+  const size_t smem = sizeof(double) * 2 * DPASS * (4 * KS + GPAD + 4) + sizeof(int) * 2 * DPASS + (size_t)12 * 2 * FSLOTS * 32 * 16;
 #define PNN_LAUNCH_DF(KSV)                                                                                              \
-  edge_fwd_dmma_k<KSV><<<grid, DTHR, 0, st>>>(a, RB, phi, s_in, ld_sin, v_in, v_res, s1, ld_s1, v1);
+  {                                                                                                                     \
+    static bool attr_set = false;                                                                                       \
+    if (!attr_set) {                                                                                                    \
+      cudaFuncSetAttribute(edge_fwd_dmma_k<KSV>, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * 1024);              \
+      attr_set = true;                                                                                                  \
+    }                                                                                                                   \
+    edge_fwd_dmma_k<KSV><<<grid, DTHR, smem, st>>>(a, RB, phi, s_in, ld_sin, v_in, v_res, s1, ld_s1, v1);               \
+  }
   switch (KS) {
     case 1: PNN_LAUNCH_DF(1) break;
     case 2: PNN_LAUNCH_DF(2) break;
