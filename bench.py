@@ -195,6 +195,8 @@ def family_roofline(fam: str, per_s: float, N: int, E: int, mc, prec: str, force
         if alu_meas:
             r["alu_peak_measured"] = alu_meas
             r["frac_of_measured_peak"] = ach / alu_meas
+        if prec == "fp64":   # edge_dmma.cu / gemm_dmma.cu: the FP64 tensor instruction (DMMA) has the FP64 FMA peak
+            r["pipe"] = "fp64 tensor path (mma.sync m8n8k4 f64) where F % 64 == 0; its measured peak equals the FP64 FMA peak (DESIGN.md section 6)"
         return r
     if fam.startswith("gemm_"):
         ach = flops / per_s / 1e12
