@@ -2,9 +2,10 @@
 //
 //   C[M,N] = epi( A[M,K] * B[K,N] ),  all row-major, K a multiple of 16, N a multiple of 4.
 //
-// tcgen05 has no FP64 kind and no true-FP32 kind (SURVEY.md §7 hard part 2), so the FP32 and FP64 models run
-// their Linear layers here: a register-blocked, shared-memory tiled FFMA / DFMA kernel with a double-buffered
-// global->register->shared pipeline.  The BF16 model uses gemm_tc.cu (tcgen05 + TMA + TMEM) instead.
+// tcgen05 has no true-FP32 kind (SURVEY.md §7 hard part 2), so the FP32 model runs its Linear layers here: a
+// register-blocked, shared-memory tiled FFMA kernel with a double-buffered global->register->shared pipeline.  The FP64
+// model uses the FP64 tensor-core kernel of gemm_dmma.cu whenever the shape allows and the DFMA instance of this kernel
+// otherwise (N not a multiple of 64); the BF16 model uses gemm_tc.cu (tcgen05 + TMA + TMEM).
 // Epilogues fuse what follows each Linear in SURVEY.md §8(c): bias, SiLU (+ store of the pre-activation for the
 // reverse sweep), multiplication by silu'(stored pre-activation), and accumulation into C (residual adjoints).
 #include "common.cuh"
