@@ -83,6 +83,7 @@ class ModelCfg:
     head_type: str = "atomwise"  # or "pooled": the paper's graph-level head, mean pool -> 2 shared
     head_d1: int = 50            # layers of width head_d1 -> per head 2 layers of width head_d2 -> 1
     head_d2: int = 776
+    backbone: str = "painn"      # or "schnet": the second backbone on the same graph
 
 
 @dataclasses.dataclass
@@ -145,6 +146,19 @@ def weights_layout(mc: ModelCfg):
         off += int(np.prod(shape))
 
     add("emb", (mc.Zmax + 1, F), 1)
+    if getattr(mc, "backbone", "painn") == "schnet":   # continuous-filter convolution blocks (reading Q31)
+        for t in range(T):
+            add(f"b{t}.flt_W1", (F, K), K); add(f"b{t}.flt_b1", (F,), K)
+            add(f"b{t}.flt_W2", (F, F), F); add(f"b{t}.flt_b2", (F,), F)
+            add(f"b{t}.in_W", (F, F), F)
+            add(f"b{t}.out_W1", (F, F), F); add(f"b{t}.out_b1", (F,), F)
+            add(f"b{t}.out_W2", (F, F), F); add(f"b{t}.out_b2", (F,), F)
+        for h in range(H):
+            add(f"h{h}.out_W1", (F // 2, F), F)
+            add(f"h{h}.out_b1", (F // 2,), F)
+            add(f"h{h}.out_w2", (F // 2,), F // 2)
+            add(f"h{h}.out_b2", (1,), F // 2)
+        return out
     for t in range(T):
         add(f"b{t}.msg_W1", (F, F), F)
         add(f"b{t}.msg_b1", (F,), F)
