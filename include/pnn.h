@@ -52,6 +52,8 @@ typedef enum { PNN_BF16 = 0, PNN_FP32 = 1, PNN_FP64 = 2 } pnn_precision;
 #define PNN_RBF_GAUSSIAN 0 /* g_k(d) = exp(-gamma (d - k r_c/(K-1))^2), gamma = (K-1)^2 / (2 r_c^2), k = 0..K-1 (2 <= K) */
 #define PNN_RBF_BESSEL 1   /* b_n(d) = sqrt(2/r_c) sin(n pi d / r_c) / d, n = 1..K (the lead model's basis)  */
 #define PNN_HEAD_ATOMWISE 0 /* per-atom readout MLP of the structure's head, summed over the atoms      */
+#define PNN_BACKBONE_PAINN 0
+#define PNN_BACKBONE_SCHNET 1
 #define PNN_HEAD_POOLED 1   /* mean pooling, shared layers, per-head branch layers (the paper's graph-level heads)         */
 typedef struct {
   int32_t F, T, K, H, Zmax;
@@ -78,6 +80,13 @@ typedef struct {
                         for such a model. */
   int32_t head_d1;   /* pooled head: width of the two shared layers (paper: 50); ignored for atom-wise heads */
   int32_t head_d2;   /* pooled head: width of the two branch layers (paper: 776) */
+  int32_t backbone;  /* PNN_BACKBONE_PAINN (0) or PNN_BACKBONE_SCHNET (1): the second backbone on the same graph (PAPER.md:147,
+                        212: SchNet is one of the six backbones of the paper's search; reading Q31).  Per block
+                        W_e = (F2 silu(F1 g(d_e) + f1) + f2) c(d_e), m_i = sum_{e=(i<-j)} (A x_j) o W_e,
+                        x_i += B2 silu(B1 m_i + b1) + b2; same embedding, radial basis, cutoff and atom-wise heads.  The blob then
+                        holds per block flt_W1[F][K] flt_b1[F] flt_W2[F][F] flt_b2[F] in_W[F][F] out_W1[F][F] out_b1[F]
+                        out_W2[F][F] out_b2[F] in place of the PaiNN block arrays.  PNN_FP32 / PNN_FP64 only; no neighbour cap,
+                        global attributes, pooled heads or blended evaluation (PNN_ERR_UNSUPPORTED / PNN_ERR_INVALID_ARG). */
 } pnn_config;
 
 typedef struct pnn_model pnn_model;         /* opaque; owns device copies of the weights in model precision */

@@ -48,7 +48,7 @@ class pnn_config(ctypes.Structure):
                 ("Zmax", ctypes.c_int32), ("cutoff", ctypes.c_double), ("norm_eps", ctypes.c_double),
                 ("prec", ctypes.c_int32), ("rbf", ctypes.c_int32), ("pbc_images", ctypes.c_int32),
                 ("max_neighbors", ctypes.c_int32), ("n_global", ctypes.c_int32), ("head_type", ctypes.c_int32),
-                ("head_d1", ctypes.c_int32), ("head_d2", ctypes.c_int32)]
+                ("head_d1", ctypes.c_int32), ("head_d2", ctypes.c_int32), ("backbone", ctypes.c_int32)]
 
 
 def lib_path() -> str:
@@ -340,10 +340,11 @@ class PaiNN:
                  cutoff: float = 5.0, Zmax: int = 86, norm_eps: float = 1e-8, max_atoms: int, max_edges: int,
                  max_structs: int, forces: bool = True, rbf: str = "gaussian", pbc_images: str = "minimum",
                  edge_tape: bool = True, max_neighbors: int = 0, n_global: int = 0, head_type: str = "atomwise",
-                 head_d1: int = 50, head_d2: int = 776):
+                 head_d1: int = 50, head_d2: int = 776, backbone: str = "painn"):
         self.cfg = pnn_config(F, T, K, H, Zmax, cutoff, norm_eps, PRECISIONS[precision],
                               {"gaussian": 0, "bessel": 1}[rbf], {"minimum": 0, "all": 1}[pbc_images], int(max_neighbors),
-                              int(n_global), {"atomwise": 0, "pooled": 1}[head_type], int(head_d1), int(head_d2))
+                              int(n_global), {"atomwise": 0, "pooled": 1}[head_type], int(head_d1), int(head_d2),
+                              {"painn": 0, "schnet": 1}[backbone])
         self.precision = precision
         self.want_forces = bool(forces)
         self.model = pnn_model_create(self.cfg, weights)

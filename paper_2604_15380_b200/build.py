@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpnn.so")
-SOURCES = ["pnn_api.cu", "graph.cu", "gemm_simt.cu", "gemm_dmma.cu", "gemm_tc.cu", "edge.cu", "edge_dmma.cu", "edge_tc.cu", "edge_tc_bwd.cu", "edge_warp.cu", "edge_scatter.cu", "pool_head.cu", "node.cu", "branch.cu"]
+SOURCES = ["pnn_api.cu", "graph.cu", "gemm_simt.cu", "gemm_dmma.cu", "gemm_tc.cu", "edge.cu", "edge_dmma.cu", "edge_tc.cu", "edge_tc_bwd.cu", "edge_warp.cu", "edge_scatter.cu", "pool_head.cu", "schnet.cu", "node.cu", "branch.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "--expt-relaxed-constexpr", "--extended-lambda", "-Xptxas", "-v"]

@@ -208,6 +208,17 @@ int launch_edge_fwd_dmma(const EdgeArgs<double>& a, const double* phi, const dou
 int launch_edge_bwd_dmma(const EdgeArgs<double>& a, const double* phi, const double* v_in, const double* sb1,
                          const double* vb1, double* phib, double* vb_in, double* fpart, int first_block, cudaStream_t st);
 int edge_dmma_num_slabs(int F);
+// schnet.cu: edge-side kernels of the second backbone (continuous-filter convolution; reading Q31)
+template <typename T>
+int launch_sch_rbf(int64_t N, int64_t maxE, int K, int KP, int rbf, double rc, const int32_t* rowptr, const void* geom, T* G,
+                   T* Gd, const int* d_ovf, cudaStream_t st);
+template <typename T>
+int launch_sch_conv_fwd(int64_t N, int F, double rc, const int32_t* rowptr, const int32_t* col, const void* geom, const T* Wf,
+                        const T* x1, T* m, const int* d_ovf, cudaStream_t st);
+template <typename T>
+int launch_sch_conv_bwd(int64_t N, int F, double rc, const int32_t* rowptr, const int32_t* col, const void* geom, const T* Wf,
+                        const T* dWf, const T* x1, const T* mb, T* x1b, T* forces, int first_block, const int* d_ovf,
+                        cudaStream_t st);
 // pool_head.cu: the paper's graph-level heads (mean pooling -> shared layers -> per-head branch layers; reading Q29)
 // element offsets in the device weight buffer (every array starts on a multiple of 4 elements: 16-byte loads): shared
 // layers P1 [d1][F], p1, P2 [d1][d1], p2 and the transposes P1t [F][d1], P2t [d1][d1]; per head, at br + h * br_stride:

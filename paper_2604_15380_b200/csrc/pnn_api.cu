@@ -61,6 +61,10 @@ bool config_ok(const pnn_config* c) {
   if (c->prec != PNN_BF16 && c->prec != PNN_FP32 && c->prec != PNN_FP64) return false;
   if (c->max_neighbors < 0 || c->n_global < 0 || c->n_global > 16) return false;
   if (c->head_type != PNN_HEAD_ATOMWISE && c->head_type != PNN_HEAD_POOLED) return false;
+  if (c->backbone != PNN_BACKBONE_PAINN && c->backbone != PNN_BACKBONE_SCHNET) return false;
+  if (c->backbone == PNN_BACKBONE_SCHNET &&
+      (c->prec == PNN_BF16 || c->max_neighbors > 0 || c->n_global > 0 || c->head_type != PNN_HEAD_ATOMWISE))
+    return false;
   if (c->head_type == PNN_HEAD_POOLED && !pool_head_supported(c->F, c->head_d1, c->head_d2, c->H, c->prec == PNN_FP64 ? 8 : 4))
     return false;
   return true;
@@ -69,6 +73,8 @@ bool config_ok(const pnn_config* c) {
 int64_t weights_count(const pnn_config* c) {
   const int64_t F = c->F, K = c->K;
   const int64_t per_block = 11 * F * F + 3 * F * K + 11 * F;
+  if (c->backbone == PNN_BACKBONE_SCHNET)
+    return (int64_t)(c->Zmax + 1) * F + c->T * (F * K + F + 4 * F * F + 3 * F) + c->H * ((F / 2) * F + (F / 2) + (F / 2) + 1);
   const int64_t d1 = c->head_d1, d2 = c->head_d2;
   const int64_t heads = c->head_type == PNN_HEAD_POOLED
                             ? d1 * F + d1 + d1 * d1 + d1 + c->H * (d2 * d1 + d2 + d2 * d2 + d2 + d2 + 1)
@@ -77,6 +83,9 @@ int64_t weights_count(const pnn_config* c) {
 }
 
 // element offsets of one block's arrays inside the device weight buffer
+// SchNet block (schnet.cu): filter network F1 [F][K] -> [KP][F] transposed and zero-padded to KP = 16 ceil(K / 16) rows,
+// F2^T, A^T and A, B1^T / B1, B2^T / B2 (forward: [in][out]; reverse: [out][in])
+struct SchBlockW { int64_t fW1t, fb1, fW2t, fb2, At, A, B1t, b1, B2t, b2, B1, B2; };
 struct BlockW {
   int64_t W1t, b1, W2t, b2, fltW, fltb, UVt, A1t, c1, A2t, c2; // forward (transposed: [in][out])
   int64_t A2, A1, UV, W2, W1;                                   // reverse (original: [out][in])
@@ -90,6 +99,7 @@ struct pnn_model {
   int64_t n_elem = 0;
   int64_t emb = 0;
   std::vector<BlockW> blk;
+  std::vector<SchBlockW> sblk; // backbone = PNN_BACKBONE_SCHNET
   int64_t globW = 0;                                    // [F][n_global] (global attributes -> embedding)
   int64_t oW1t = 0, oW1 = 0, ob1 = 0, ow2 = 0, ob2 = 0; // heads: [H][F][Fh], [H][Fh][F], [H][Fh], [H][Fh], [H]
   PoolHeadW pool{};                                     // pooled head (pool_head.cu)
@@ -111,6 +121,13 @@ struct pnn_workspace {
   // activations (element type = model state type)
   void *s_cur, *h, *sn, *v1, *k, *vping[2], *eatom, *opre;
   const double* glob = nullptr;            // global attributes of the next evaluations (pnn_set_globals), DEVICE [S][G]
+  // SchNet backbone (schnet.cu): node rows x1 = A x, m, y; edge rows G / G' [E][KP], H1 = silu(pre1), pre1, the tangent Ht,
+  // per block the filter Wf and its derivative dWf [E][F] and the node tape x1, pre2; adjoints yb, mb, x1b
+  struct Sch {
+    void *x1 = nullptr, *m = nullptr, *y = nullptr, *G = nullptr, *Gd = nullptr, *H1 = nullptr, *pre1 = nullptr, *Ht = nullptr;
+    void *yb = nullptr, *mb = nullptr, *x1b = nullptr;
+    std::vector<void*> Wf, dWf, x1t, pre2;
+  } sch;
   void* pool_scratch = nullptr;            // pooled head: x, x-bar, head permutation, tile table
   unsigned long long* head_mask = nullptr; // BF16 readout GEMM: heads present per 128-row tile
   void* opre_all = nullptr; // blended readout: pre-activations of every head [N][H][F/2] (reverse sweep)
@@ -222,8 +239,29 @@ int pnn_model_create(const pnn_config* cfg, const double* w, int64_t n_scalars, 
   const double* p = w;
   auto take = [&](int64_t n) { const double* q = p; p += n; return q; };
   m->emb = put(take((cfg->Zmax + 1) * F), (cfg->Zmax + 1) * F);
-  m->blk.resize(cfg->T);
-  for (int t = 0; t < cfg->T; ++t) {
+  const bool schnet = cfg->backbone == PNN_BACKBONE_SCHNET;
+  if (schnet) {
+    const int64_t KP = (K + 15) / 16 * 16;
+    m->sblk.resize(cfg->T);
+    for (int t = 0; t < cfg->T; ++t) {
+      SchBlockW& b = m->sblk[t];
+      const double* F1 = take(F * K); const double* f1 = take(F);
+      const double* F2 = take(F * F); const double* f2 = take(F);
+      const double* A = take(F * F);
+      const double* B1 = take(F * F); const double* b1 = take(F);
+      const double* B2 = take(F * F); const double* b2 = take(F);
+      b.fW1t = reserve(KP * F); // [KP][F], rows K..KP-1 zero
+      for (int64_t f = 0; f < F; ++f)
+        for (int64_t k = 0; k < K; ++k) hb[b.fW1t + k * F + f] = F1[f * K + k];
+      b.fb1 = put(f1, F);
+      b.fW2t = put_t(F2, F, F); b.fb2 = put(f2, F);
+      b.At = put_t(A, F, F); b.A = put(A, F * F);
+      b.B1t = put_t(B1, F, F); b.b1 = put(b1, F); b.B1 = put(B1, F * F);
+      b.B2t = put_t(B2, F, F); b.b2 = put(b2, F); b.B2 = put(B2, F * F);
+    }
+  }
+  m->blk.resize(schnet ? 0 : cfg->T);
+  for (int t = 0; t < (schnet ? 0 : cfg->T); ++t) {
     BlockW& b = m->blk[t];
     const double* W1 = take(F * F);     const double* b1 = take(F);
     const double* W2 = take(3 * F * F); const double* b2 = take(3 * F);
@@ -382,6 +420,29 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
       g.cap_rowptr = (int32_t*)carve(4 * (N + 2));
     }
     g.max_edges = maxE;
+    const bool schnet = m->cfg.backbone == PNN_BACKBONE_SCHNET;
+    if (schnet) {
+      const int64_t KP = (m->cfg.K + 15) / 16 * 16;
+      pnn_workspace::Sch& q = ws->sch;
+      ws->s_cur = carve(es * N * F);
+      ws->eatom = carve(es * N);
+      q.m = carve(es * N * F); q.y = carve(es * N * F);
+      q.G = carve(es * E * KP); q.H1 = carve(es * E * F);
+      const int nt = want_forces ? (int)T : 1;
+      q.Wf.assign(nt, nullptr); q.dWf.assign(nt, nullptr); q.x1t.assign(nt, nullptr); q.pre2.assign(nt, nullptr);
+      for (int t = 0; t < nt; ++t) {
+        q.Wf[t] = carve(es * E * F);
+        q.x1t[t] = carve(es * N * F);
+        if (want_forces) { q.dWf[t] = carve(es * E * F); q.pre2[t] = carve(es * N * F); }
+      }
+      ws->tape.resize(1);
+      if (want_forces) {
+        q.Gd = carve(es * E * KP); q.pre1 = carve(es * E * F); q.Ht = carve(es * E * F);
+        q.yb = carve(es * N * F); q.mb = carve(es * N * F); q.x1b = carve(es * N * F);
+        ws->opre = carve(es * N * (F / 2));
+        ws->sb = carve(es * N * F);
+      }
+    } else {
     ws->s_cur = carve(es * N * F);
     ws->h = carve(es * N * F);
     ws->sn = carve(es * N * 2 * F);
@@ -447,6 +508,7 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
         b.ab16 = b.kb16 = b.PQb16 = b.phib16 = b.hb16 = b.sb16 = b.vb16 = nullptr;
       }
     }
+    } // PaiNN arrays
     ws->st_Z = (int32_t*)carve(4 * N);
     ws->st_sptr = (int32_t*)carve(4 * (S + 1));
     ws->st_head = (int32_t*)carve(4 * S);
@@ -466,7 +528,8 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
       }
     }
   }
-  if (m->cfg.prec == PNN_FP32 && want_forces && maxE > 0 && !no_tape && m->cfg.max_neighbors == 0) {
+  if (m->cfg.prec == PNN_FP32 && want_forces && maxE > 0 && !no_tape && m->cfg.max_neighbors == 0 &&
+      m->cfg.backbone == PNN_BACKBONE_PAINN) {
     // the FP32 edge tape (w and dw/dd of every edge and block): required unless the caller opted out with
     // PNN_WS_NO_EDGE_TAPE; running out of memory is an error, never a silent change of kernels
     const int64_t per_block = 2 * maxE * 3 * F;
@@ -912,6 +975,90 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
   return tc_fail ? PNN_ERR_UNSUPPORTED : PNN_OK;
 }
 
+
+// The second backbone (schnet.cu): same graph, embedding, readout and reverse-sweep entry as the
+// PaiNN path; the filter-generating network runs as E-row GEMMs, the node layers as N-row GEMMs.
+template <typename T>
+int eval_schnet(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const int32_t* sptr,
+                const int32_t* head, int flags, T* energy, T* forces, cudaStream_t st) {
+  const pnn_config& c = m->cfg;
+  const int F = c.F, T_ = c.T, KP = (c.K + 15) / 16 * 16;
+  const bool want_f = (flags & PNN_FORCES) != 0;
+  const bool taped = ws->want_forces != 0;
+  const T* W = (const T*)m->d_w;
+  pnn_workspace::Sch& q = ws->sch;
+  const int64_t Emax = ws->maxE; // the GEMMs of the filter network run over the workspace's edge capacity (rows past the
+                                 // graph's edge count hold stale finite values nobody reads: E lives on the device)
+  T* x = (T*)ws->s_cur;
+  int nl = 0;
+  auto gemm = [&](const char* fam, int64_t M_, int N_, int K_, const T* A, int64_t lda, int64_t Boff, T* C, const GemmEpi<T>& e) {
+    ProfScope ps_(ws, st, fam);
+    const int l_ = launch_gemm<T>(M_, N_, K_, A, lda, W + Boff, N_, C, N_, e, st);
+    nl += l_; ps_.done(l_);
+  };
+  { ProfScope ps_(ws, st, "embed");
+    const int l_ = launch_embed<T>(N, F, c.Zmax, Z, W + m->emb, x, ws->g.d_err, st);
+    nl += l_; ps_.done(l_); }
+  { ProfScope ps_(ws, st, "edge_fwd");   // radial-basis rows g (and g' for the forces), once per evaluation
+    const int l_ = launch_sch_rbf<T>(N, Emax, c.K, KP, c.rbf, c.cutoff, ws->g.rowptr, ws->g.geom, (T*)q.G,
+                                     want_f ? (T*)q.Gd : nullptr, ws->g.d_ovf, st);
+    nl += l_; ps_.done(l_); }
+  for (int t = 0; t < T_; ++t) {
+    const SchBlockW& b = m->sblk[t];
+    const int tt = taped ? t : 0;
+    T* Wf = (T*)q.Wf[tt]; T* x1 = (T*)q.x1t[tt];
+    GemmEpi<T> e1; e1.bias = W + b.fb1; e1.act = ACT_SILU; e1.pre = want_f ? (T*)q.pre1 : nullptr; e1.ldpre = F;
+    gemm("gemm_E", Emax, F, KP, (const T*)q.G, KP, b.fW1t, (T*)q.H1, e1);                 // silu(F1 g + f1)
+    GemmEpi<T> e2; e2.bias = W + b.fb2;
+    gemm("gemm_E", Emax, F, F, (const T*)q.H1, F, b.fW2t, Wf, e2);                        // F = F2 . + f2 (cutoff applied later)
+    if (want_f) { // dF/dd by forward mode through the same two layers
+      GemmEpi<T> e3; e3.act = ACT_MUL_DSILU; e3.aux = (const T*)q.pre1; e3.ldaux = F;
+      gemm("gemm_E", Emax, F, KP, (const T*)q.Gd, KP, b.fW1t, (T*)q.Ht, e3);
+      GemmEpi<T> e4;
+      gemm("gemm_E", Emax, F, F, (const T*)q.Ht, F, b.fW2t, (T*)q.dWf[t], e4);
+    }
+    GemmEpi<T> e5;
+    gemm("gemm_N", N, F, F, x, F, b.At, x1, e5);                                           // x1 = A x
+    { ProfScope ps_(ws, st, "edge_fwd");
+      const int l_ = launch_sch_conv_fwd<T>(N, F, c.cutoff, ws->g.rowptr, ws->g.col, ws->g.geom, Wf, x1, (T*)q.m,
+                                            ws->g.d_ovf, st);
+      nl += l_; ps_.done(l_); }
+    GemmEpi<T> e6; e6.bias = W + b.b1; e6.act = ACT_SILU; e6.pre = want_f ? (T*)q.pre2[t] : nullptr; e6.ldpre = F;
+    gemm("gemm_N", N, F, F, (const T*)q.m, F, b.B1t, (T*)q.y, e6);
+    GemmEpi<T> e7; e7.bias = W + b.b2; e7.accumulate = 1;
+    gemm("gemm_N", N, F, F, (const T*)q.y, F, b.B2t, x, e7);                               // x += B2 silu(.) + b2
+  }
+  { ProfScope ps_(ws, st, "readout");
+    const int l_ = launch_readout<T>(N, S, F, c.H, x, ws->g.a2s, head, sptr, W + m->oW1t, W + m->ob1, W + m->ow2, W + m->ob2,
+                                     (T*)ws->opre, (T*)ws->eatom, energy, ws->g.d_err, st);
+    nl += l_; ps_.done(l_); }
+  if (want_f) {
+    T* xb = (T*)ws->sb;
+    { ProfScope ps_(ws, st, "readout_bwd");
+      const int l_ = launch_readout_bwd<T>(N, F, c.H, (const T*)ws->opre, ws->g.a2s, head, W + m->oW1, W + m->ow2, xb, st);
+      nl += l_; ps_.done(l_); }
+    if (T_ == 0 || N == 0) cudaMemsetAsync(forces, 0, sizeof(T) * 3 * N, st);
+    for (int t = T_ - 1; t >= 0; --t) {
+      const SchBlockW& b = m->sblk[t];
+      GemmEpi<T> g1; g1.act = ACT_MUL_DSILU; g1.aux = (const T*)q.pre2[t]; g1.ldaux = F;
+      gemm("gemm_N", N, F, F, xb, F, b.B2, (T*)q.yb, g1);                                  // y-bar = (B2^T x-bar) silu'
+      GemmEpi<T> g2;
+      gemm("gemm_N", N, F, F, (const T*)q.yb, F, b.B1, (T*)q.mb, g2);                     // m-bar = B1^T y-bar
+      { ProfScope ps_(ws, st, "edge_bwd");
+        const int l_ = launch_sch_conv_bwd<T>(N, F, c.cutoff, ws->g.rowptr, ws->g.col, ws->g.geom, (const T*)q.Wf[t],
+                                              (const T*)q.dWf[t], (const T*)q.x1t[t], (const T*)q.mb,
+                                              t > 0 ? (T*)q.x1b : nullptr, forces, t == T_ - 1 ? 1 : 0, ws->g.d_ovf, st);
+        nl += l_; ps_.done(l_); }
+      if (t > 0) {
+        GemmEpi<T> g3; g3.accumulate = 1;
+        gemm("gemm_N", N, F, F, (const T*)q.x1b, F, b.A, xb, g3);                          // x-bar += A^T x1-bar
+      }
+    }
+  }
+  ws->launches += nl;
+  return PNN_OK;
+}
+
 } // namespace
 
 extern "C" {
@@ -928,6 +1075,12 @@ static int eval_common(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t
   if (ws->graph_N != N || ws->graph_S != S) return PNN_ERR_NO_GRAPH;
   cudaStream_t st = (cudaStream_t)stream;
   int rc;
+  if (m->cfg.backbone == PNN_BACKBONE_SCHNET) {
+    if (head_w) return PNN_ERR_UNSUPPORTED;
+    rc = m->cfg.prec == PNN_FP64
+             ? eval_schnet<double>(m, ws, N, S, Z, sptr, head, flags, (double*)energy, (double*)forces, st)
+             : eval_schnet<float>(m, ws, N, S, Z, sptr, head, flags, (float*)energy, (float*)forces, st);
+  } else
   if (m->cfg.prec == PNN_FP64)
     rc = eval_simt<double>(m, ws, N, S, Z, sptr, head, (const double*)head_w, skip_below, flags, (double*)energy,
                            (double*)forces, st);

@@ -28,7 +28,8 @@ def make_model(mc: gen.ModelCfg, weights, precision: str, max_atoms: int, max_ed
                      forces=forces, rbf=getattr(mc, "rbf", "gaussian"),
                      pbc_images=getattr(mc, "pbc_images", "minimum"), max_neighbors=getattr(mc, "max_neighbors", 0),
                      n_global=getattr(mc, "n_global", 0), head_type=getattr(mc, "head_type", "atomwise"),
-                     head_d1=getattr(mc, "head_d1", 50), head_d2=getattr(mc, "head_d2", 776))
+                     head_d1=getattr(mc, "head_d1", 50), head_d2=getattr(mc, "head_d2", 776),
+                     backbone=getattr(mc, "backbone", "painn"))
 
 
 def run_gpu(mc: gen.ModelCfg, weights, batch: gen.Batch, precision: str, forces: bool = True, max_edges=None,

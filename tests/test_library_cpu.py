@@ -49,6 +49,12 @@ def test_weight_blob_size_matches_generators(pnn):
     mc = dataclasses.replace(gen.model_cfg(2), head_type="pooled", head_d1=50, head_d2=776, n_global=2)
     cfg = pnn.pnn_config(mc.F, mc.T, mc.K, mc.H, mc.Zmax, mc.cutoff, mc.norm_eps, pnn.PNN_FP32, 0, 0, 0, 2, 1, 50, 776)
     assert pnn.pnn_weights_count(cfg) == gen.weights_count(mc)
+    mcs = dataclasses.replace(gen.model_cfg(2), backbone="schnet")   # second backbone: other block arrays, same heads
+    cfgs = pnn.pnn_config(mcs.F, mcs.T, mcs.K, mcs.H, mcs.Zmax, mcs.cutoff, mcs.norm_eps, pnn.PNN_FP64, 0, 0, 0, 0, 0, 50, 776, 1)
+    assert pnn.pnn_weights_count(cfgs) == gen.weights_count(mcs)
+    with pytest.raises(pnn.PnnError):   # the second backbone has no BF16 path
+        pnn.pnn_weights_count(pnn.pnn_config(mcs.F, mcs.T, mcs.K, mcs.H, mcs.Zmax, mcs.cutoff, mcs.norm_eps, pnn.PNN_BF16, 0, 0,
+                                             0, 0, 0, 50, 776, 1))
     with pytest.raises(pnn.PnnError):   # widths whose activations do not fit one CTA's shared memory
         pnn.pnn_weights_count(pnn.pnn_config(64, 2, 20, 2, 86, 5.0, 1e-8, pnn.PNN_FP64, 0, 0, 0, 0, 1, 50, 4000))
 
