@@ -14,6 +14,7 @@ streaming driver), cfg5 FP64.  See DESIGN.md "Measurement" for every definition 
 from __future__ import annotations
 
 import argparse
+import dataclasses
 import json
 import os
 import subprocess
@@ -39,12 +40,21 @@ WORKLOADS = {
     "cfg4": (4, "bf16", False, 16384),
     "cfg4_fp32": (4, "fp32", False, 16384),
     "cfg5": (5, "fp64", True, None),
+    # the paper's own model settings and the second backbone on the cfg2 batch (context lines)
+    "cfg2_pooled": (2, "fp32", True, None),
+    "cfg2_cap20": (2, "fp32", True, None),
+    "cfg2_schnet": (2, "fp32", True, None),
 }
+# model options that differ from the config's BASELINE.json model (gen.ModelCfg fields)
+VARIANTS = {"cfg2_pooled": dict(head_type="pooled", head_d1=50, head_d2=776),
+            "cfg2_cap20": dict(max_neighbors=20),
+            "cfg2_schnet": dict(backbone="schnet")}
 WORKLOAD_NAMES = {"cfg1": "cfg1_tiny_fp64", "cfg2": "cfg2_molecular_fp32", "cfg2_fp64": "cfg2_molecular_fp64",
                   "cfg2_blended": "cfg2_molecular_fp32_blended_heads",
                   "cfg3_fp32": "cfg3_crystals_fp32", "cfg3_bf16": "cfg3_crystals_bf16",
                   "cfg4": "cfg4_screening_bf16_batch16384", "cfg4_fp32": "cfg4_screening_fp32_batch16384",
-                  "cfg5": "cfg5_large_fp64"}
+                  "cfg5": "cfg5_large_fp64", "cfg2_pooled": "cfg2_molecular_fp32_pooled_heads_50_776",
+                  "cfg2_cap20": "cfg2_molecular_fp32_max_neighbors_20", "cfg2_schnet": "cfg2_molecular_fp32_schnet"}
 FULL_RECORDS = ("cfg2", "cfg3_fp32", "cfg3_bf16", "cfg4", "cfg5")   # BASELINE.json configs[1..4] (cfg3 in both precisions)
 CFG4_STREAM_BATCHES = 64                                            # 1,048,576 structures / 16,384
 DTYPE = {"fp64": "f64", "fp32": "f32", "bf16": "bf16"}
@@ -290,7 +300,9 @@ def main():
     def run_workload(name: str, steps: int, warmup: int, full: bool):
         cfg_id, prec, forces, per_step = WORKLOADS[name]
         c = gen.CONFIGS[cfg_id]
-        mc = gen.model_cfg(cfg_id)
+        mc = dataclasses.replace(gen.model_cfg(cfg_id), **VARIANTS.get(name, {}))
+        opts = dict(max_neighbors=mc.max_neighbors, head_type=mc.head_type, head_d1=mc.head_d1, head_d2=mc.head_d2,
+                    backbone=mc.backbone)
         S = per_step or c["S"]
         # weak scaling: rank r evaluates its own structures [r*S, (r+1)*S) of the same recipe
         b = gen.make_batch(cfg_id, rank * S, S)
@@ -302,7 +314,7 @@ def main():
         deg_cap = 96 if cfg_id in (3, 5) else 40
         probe = pnn.PaiNN(mc.F, mc.T, mc.K, mc.H, w, precision=prec, cutoff=mc.cutoff, Zmax=mc.Zmax,
                           norm_eps=mc.norm_eps, max_atoms=b.n_atoms, max_edges=b.n_atoms * deg_cap,
-                          max_structs=b.n_structs, forces=False)
+                          max_structs=b.n_structs, forces=False, **dict(opts, max_neighbors=0))   # max_edges bounds the UNCAPPED count
         probe.build_graph(d["pos"], d["sp"], d["cell"], d["pbc"])
         _, _, _, E = pnn.pnn_graph_view(probe.ws)
         probe.close()
@@ -311,7 +323,7 @@ def main():
         max_edges = int(E * 1.02) + 1024
         net = pnn.PaiNN(mc.F, mc.T, mc.K, mc.H, w, precision=prec, cutoff=mc.cutoff, Zmax=mc.Zmax,
                         norm_eps=mc.norm_eps, max_atoms=b.n_atoms, max_edges=max_edges,
-                        max_structs=b.n_structs, forces=forces)
+                        max_structs=b.n_structs, forces=forces, **opts)
         flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)  # 256 MB > 126 MB L2
         st = torch.cuda.current_stream()
 
@@ -477,6 +489,20 @@ def main():
             per_kernel[fam] = family_roofline(fam, kernels[fam]["ms_per_launch"] * 1e-3, N, E, mc, prec, forces, peaks,
                                               wname, alu_meas.get(prec))
             per_kernel[fam]["share_of_step"] = kernels[fam]["share"]
+        if prec == "fp32" and "edge_fwd" in per_kernel and "edge_bwd" in per_kernel and res["tape_bytes"]:
+            # FP32 with the edge tape: the forward kernel also evaluates dw/dd (6KF of the reverse step's 12KF flop per edge)
+            # and the reverse kernel streams it back, so each family's own fraction is skewed (reverse can exceed 1):
+            # the pair is judged together
+            fw, bw = per_kernel["edge_fwd"], per_kernel["edge_bwd"]
+            t_pair = (kernels["edge_fwd"]["ms_per_launch"] + kernels["edge_bwd"]["ms_per_launch"]) * 1e-3
+            ach = (fw["algorithmic_flops"] + bw["algorithmic_flops"]) / t_pair / 1e12
+            note = ("edge tape: the forward kernel computes half of the reverse step's algorithmic flops; see "
+                    "roofline_per_kernel['edge_fwd+edge_bwd']")
+            fw["note"] = bw["note"] = note
+            per_kernel["edge_fwd+edge_bwd"] = dict(kernel="edge_fwd+edge_bwd", bound="alu", achieved=ach, peak=fw["peak"],
+                                                   unit="TFLOP/s", frac=ach / fw["peak"], peak_source=fw["peak_source"],
+                                                   algorithmic_flops=fw["algorithmic_flops"] + bw["algorithmic_flops"],
+                                                   share_of_step=kernels["edge_fwd"]["share"] + kernels["edge_bwd"]["share"])
         if cand:
             roof = per_kernel[max(cand, key=lambda f: kernels[f]["share"])]   # the dominant kernel family of the step
         sr = step_roof(N, E, mc, prec, forces, peaks, ALU_PEAK_TFLOPS.get(prec, 0.0))
@@ -563,7 +589,7 @@ def main():
                 recs[WORKLOAD_NAMES[name]] = dict(error=str(ex)[:300])
         line["workloads"] = recs
         extra = {}
-        for name in ("cfg1", "cfg2_blended"):   # context only: short timings
+        for name in ("cfg1", "cfg2_blended", "cfg2_pooled", "cfg2_cap20", "cfg2_schnet"):   # context only: short timings
             try:
                 r = run_workload(name, 5, 3, full=False)
                 extra[WORKLOAD_NAMES[name]] = dict(ms_per_step=r["ms_per_step_median"],
