@@ -180,7 +180,8 @@ int edge_num_slabs(int F);
 // edge_scatter.cu — the reverse message step in scatter form (atomic adds) for asymmetric edge sets (max-neighbour cap)
 template <typename T, typename PT>
 int launch_edge_bwd_scatter(const EdgeArgs<T>& a, const PT* phi, const PT* v_in, const T* sb1, const T* vb1, T* phib,
-                            T* vb_in, T* fslab, int first_block, cudaStream_t st);
+                            T* vb_in, T* fslab, int first_block, cudaStream_t st, const T* wt = nullptr,
+                            const T* dt = nullptr); // wt, dt: the FP32 edge tape (w, dw/dd [E][3][F]) or NULL = recompute
 
 // edge_warp.cu — the FP32 model's edge kernels (warp per receiver, filter rows in registers, no CTA barriers)
 // wt, dt (both or neither): edge tape [E][3][F] that receives the filter value w and dw/dd of every edge; the reverse

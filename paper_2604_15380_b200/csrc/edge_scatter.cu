@@ -8,8 +8,8 @@
 //   phi-bar_j^c += x-bar^c w_e^c ;  v-bar_j[a] += v-bar'_i[a] phi_j^vv w_e^vv
 //   dE/dd_e = sum_{c,f} x-bar^c phi_j^c dw_e^c/dd ;  u-bar_e[a] = sum_f v-bar'_i[a] phi_j^vs w_e^vs
 //   G_e = dE/dd_e u_e + (u-bar_e - (u-bar_e . u_e) u_e) / d_e ;  force_i += G_e ;  force_j -= G_e
-// One warp per receiver, lanes stride over the features, the filter is recomputed from the radial basis (K + 1 terms per
-// feature and chunk).  It is the plain path: correctness for the paper's own graph setting, not a tuned kernel.
+// One warp per receiver, lanes stride over the features; the filter value and derivative come from the FP32 edge tape of the
+// forward kernel when there is one, else they are recomputed from the radial basis (K + 1 terms per feature and chunk).  It is the plain path: correctness for the paper's own graph setting, not a tuned kernel.
 #include <algorithm>
 
 #include "common.cuh"
@@ -28,7 +28,8 @@ template <> __device__ __forceinline__ void sincos_t<double>(double x, double* s
 template <typename T, typename PT>
 __global__ void __launch_bounds__(128)
 edge_bwd_scatter_k(EdgeArgs<T> a, const PT* __restrict__ phi, const PT* __restrict__ v_in, const T* __restrict__ sb1,
-                   const T* __restrict__ vb1, T* phib, T* vb_in, T* fslab) {
+                   const T* __restrict__ vb1, T* phib, T* vb_in, T* fslab, const T* __restrict__ wt,
+                   const T* __restrict__ dt) {
   if (*a.d_err & ERRF_EDGE_OVERFLOW) return;
   __shared__ T Gs[4][2][36]; // per warp: g_k c (k < K), c at k = K; and their d/dd
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -47,6 +48,7 @@ edge_bwd_scatter_k(EdgeArgs<T> a, const PT* __restrict__ phi, const PT* __restri
       sincos_t<T>(pi_rc * gq.d, &sn, &cs);
       const T cc = T(0.5) * (cs + T(1)), cp = -T(0.5) * pi_rc * sn;
       __syncwarp();
+      if (!wt)
       for (int k = lane; k <= K; k += 32) {
         T g = T(1), gd = T(0);
         if (k < K) rbf_eval<T>(a.rbf, k, gq.d, rc, dmu, gamma, g, gd);
@@ -57,6 +59,14 @@ edge_bwd_scatter_k(EdgeArgs<T> a, const PT* __restrict__ phi, const PT* __restri
       T dEdd = T(0), ub0 = T(0), ub1 = T(0), ub2 = T(0);
       for (int f = lane; f < F; f += 32) {
         T w[3], dw[3];
+        if (wt) { // FP32 edge tape written by the forward kernel: w and dw/dd of this edge ([E][3][F]; vv only when v != 0)
+#pragma unroll
+          for (int c = 0; c < 3; ++c) {
+            const bool on = c < 2 || has_v;
+            w[c] = on ? wt[(int64_t)e * 3 * F + c * F + f] : T(0);
+            dw[c] = on ? dt[(int64_t)e * 3 * F + c * F + f] : T(0);
+          }
+        } else
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
           const T* row = a.fltW + ((int64_t)c * F + f) * K;
@@ -112,7 +122,7 @@ edge_bwd_scatter_k(EdgeArgs<T> a, const PT* __restrict__ phi, const PT* __restri
 // vb_in = vb1 + scatter sums.  fslab [N,3]: force slab, zeroed here when first_block, otherwise accumulated into.
 template <typename T, typename PT>
 int launch_edge_bwd_scatter(const EdgeArgs<T>& a, const PT* phi, const PT* v_in, const T* sb1, const T* vb1, T* phib,
-                            T* vb_in, T* fslab, int first_block, cudaStream_t st) {
+                            T* vb_in, T* fslab, int first_block, cudaStream_t st, const T* wt, const T* dt) {
   if (a.N == 0) return 0;
   if (phib) {
     cudaMemsetAsync(phib, 0, sizeof(T) * a.N * 3 * a.F, st);
@@ -120,17 +130,19 @@ int launch_edge_bwd_scatter(const EdgeArgs<T>& a, const PT* phi, const PT* v_in,
   }
   if (first_block) cudaMemsetAsync(fslab, 0, sizeof(T) * a.N * 3, st);
   const unsigned grid = (unsigned)std::min<int64_t>((a.N + 3) / 4, 148 * 16);
-  edge_bwd_scatter_k<T, PT><<<grid, 128, 0, st>>>(a, phi, v_in, sb1, vb1, phib, vb_in, fslab);
+  edge_bwd_scatter_k<T, PT><<<grid, 128, 0, st>>>(a, phi, v_in, sb1, vb1, phib, vb_in, fslab, wt, dt);
   PNN_KCHECK("edge_bwd_scatter_k");
   return 1;
 }
 
 template int launch_edge_bwd_scatter<float, float>(const EdgeArgs<float>&, const float*, const float*, const float*,
-                                                   const float*, float*, float*, float*, int, cudaStream_t);
+                                                   const float*, float*, float*, float*, int, cudaStream_t, const float*,
+                                                   const float*);
 template int launch_edge_bwd_scatter<double, double>(const EdgeArgs<double>&, const double*, const double*, const double*,
-                                                     const double*, double*, double*, double*, int, cudaStream_t);
+                                                     const double*, double*, double*, double*, int, cudaStream_t,
+                                                     const double*, const double*);
 template int launch_edge_bwd_scatter<float, __nv_bfloat16>(const EdgeArgs<float>&, const __nv_bfloat16*,
                                                            const __nv_bfloat16*, const float*, const float*, float*, float*,
-                                                           float*, int, cudaStream_t);
+                                                           float*, int, cudaStream_t, const float*, const float*);
 
 } // namespace pnn

@@ -528,8 +528,7 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
       }
     }
   }
-  if (m->cfg.prec == PNN_FP32 && want_forces && maxE > 0 && !no_tape && m->cfg.max_neighbors == 0 &&
-      m->cfg.backbone == PNN_BACKBONE_PAINN) {
+  if (m->cfg.prec == PNN_FP32 && want_forces && maxE > 0 && !no_tape && m->cfg.backbone == PNN_BACKBONE_PAINN) {
     // the FP32 edge tape (w and dw/dd of every edge and block): required unless the caller opted out with
     // PNN_WS_NO_EDGE_TAPE; running out of memory is an error, never a silent change of kernels
     const int64_t per_block = 2 * maxE * 3 * F;
@@ -771,8 +770,12 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
       if (c.max_neighbors > 0) { // capped (asymmetric) graph: the scatter form of R3 / R4
         ProfScope ps_(ws, st, "edge_bwd");
+        const T* wt = nullptr; // FP32: the edge tape of the forward kernel serves the scatter form too
+        if constexpr (std::is_same<T, float>::value)
+          if (ws->etape) wt = ws->etape + (int64_t)t * ws->etape_block;
         const int l_ = launch_edge_bwd_scatter<T, T>(ea, (const T*)tp.phi, (const T*)tp.v_in, sb, vb, t > 0 ? phib : nullptr,
-                                                     t > 0 ? vb2 : nullptr, fpart, last ? 1 : 0, st);
+                                                     t > 0 ? vb2 : nullptr, fpart, last ? 1 : 0, st, wt,
+                                                     wt ? wt + ws->etape_block / 2 : nullptr);
         nl += l_; ps_.done(l_);
       } else
       { ProfScope ps_(ws, st, "edge_bwd");
