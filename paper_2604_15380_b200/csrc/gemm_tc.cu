@@ -30,6 +30,8 @@ namespace {
 
 constexpr int BM = 128, BK = 64;
 constexpr int NTHREADS = 192;
+constexpr int EPI_PER_Q = 2;                      // persistent kernel: epilogue warps per TMEM lane quadrant
+constexpr int NTHREADS_PK = 64 + 128 * EPI_PER_Q; // TMA warp, MMA warp, 4 * EPI_PER_Q epilogue warps
 
 using namespace tc;
 
@@ -257,7 +259,7 @@ tc_gemm_k(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 // the TMA loads and MMAs of tile i+1 overlap the epilogue (global stores) of tile i: these GEMMs have K <= 768 and are
 // bound by HBM traffic, not by the tensor pipe, so what matters is that loads and stores never pause.
 template <int BN, int STAGES>
-__global__ void __launch_bounds__(NTHREADS)
+__global__ void __launch_bounds__(NTHREADS_PK)
 tc_gemm_pk(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int64_t M, int N, int K,
            int n_tiles, int64_t total_tiles, TcEpi epi) {
   constexpr int A_BYTES = BM * BK * 2, B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
@@ -277,7 +279,7 @@ tc_gemm_pk(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
 
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(accfull_bar(b), 1); mbar_init(accempty_bar(b), 4); }
+    for (int b = 0; b < 2; ++b) { mbar_init(accfull_bar(b), 1); mbar_init(accempty_bar(b), 4 * EPI_PER_Q); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 2) {
@@ -344,7 +346,14 @@ tc_gemm_pk(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
       });
     }
   } else {
-    const int q = warp & 3;
+    // Several warps share a TMEM lane quadrant (a warp reads the lanes 32 (warp % 4) ...) and split the tile's columns: these
+    // GEMMs are bound by the epilogue (a row per thread: bias / activation / conversions and 32-byte stores of 256+ columns),
+    // not by the tensor pipe or HBM, so more warps shorten it.  Readout mode sums over ALL columns of a head per row:
+    // there (and for narrow tiles) the surplus warps of a quadrant only hand the buffer back.
+    const int q = warp & 3, part = (warp - 2) >> 2;
+    constexpr int PARTS = (BN / 32 >= EPI_PER_Q) ? EPI_PER_Q : (BN >= 64 ? 2 : 1); // column groups of >= 32
+    const int parts = epi.readout ? 1 : PARTS;
+    const int c_lo = part < parts ? part * (BN / parts) : 0, c_hi = part < parts ? c_lo + BN / parts : 0;
     uint32_t j = 0;
     for_each_tile([&](int64_t mt, int nt) {
       const uint32_t b = j & 1u;
@@ -360,7 +369,7 @@ tc_gemm_pk(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
         row_ok = (hrow == nt);
       }
 #pragma unroll 1
-      for (int c0 = 0; c0 < BN; c0 += 32) {
+      for (int c0 = c_lo; c0 < c_hi; c0 += 32) {
         uint32_t r[32];
         tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + b * BN + (uint32_t)c0, r);
         if (!row_ok) continue;
@@ -474,7 +483,7 @@ int launch_persistent(int64_t M, int N, int K, const CUtensorMap& ta, const CUte
   const int64_t total = ((M + BM - 1) / BM) * n_tiles;
   const int per_sm = (2 * BN <= 256 && SMEM <= 110 * 1024) ? 2 : 1; // TMEM: 512 columns per SM
   const unsigned grid = (unsigned)std::min<int64_t>(total, 148 * per_sm);
-  tc_gemm_pk<BN, STAGES><<<grid, NTHREADS, SMEM, st>>>(ta, tb, M, N, K, n_tiles, total, epi);
+  tc_gemm_pk<BN, STAGES><<<grid, NTHREADS_PK, SMEM, st>>>(ta, tb, M, N, K, n_tiles, total, epi);
   PNN_KCHECK("tc_gemm_pk");
   return 1;
 }
