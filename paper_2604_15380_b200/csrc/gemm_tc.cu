@@ -29,7 +29,6 @@ namespace pnn {
 namespace {
 
 constexpr int BM = 128, BK = 64;
-constexpr int NTHREADS = 192;
 constexpr int EPI_PER_Q = 2;                      // persistent kernel: epilogue warps per TMEM lane quadrant
 constexpr int NTHREADS_PK = 64 + 128 * EPI_PER_Q; // TMA warp, MMA warp, 4 * EPI_PER_Q epilogue warps
 
@@ -163,7 +162,7 @@ struct TcSmem {
 };
 
 template <int BN, int STAGES>
-__global__ void __launch_bounds__(NTHREADS)
+__global__ void __launch_bounds__(NTHREADS_PK)
 tc_gemm_k(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int64_t M, int N, int K,
           int n_tiles, TcEpi epi) {
   using L = TcSmem<BN, STAGES>;
@@ -233,13 +232,16 @@ tc_gemm_k(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   } else {
     // epilogue warps 2..5: TMEM lane quadrant = warp % 4; a thread owns one output row and walks it 32 columns at a
     // time (tcgen05.ld 32x32b.x32), so every global access is a 16-byte vector of that row
-    const int q = warp & 3;
+    // (EPI_PER_Q warps per quadrant split the tile's columns, as in the persistent kernel)
+    const int q = warp & 3, part = (warp - 2) >> 2;
+    constexpr int PARTS = (BN / 32 >= EPI_PER_Q) ? EPI_PER_Q : (BN >= 64 ? 2 : 1);
+    const int c_lo = part < PARTS ? part * (BN / PARTS) : 0, c_hi = part < PARTS ? c_lo + BN / PARTS : 0;
     mbar_wait(acc_bar, 0);
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const int64_t m = m0 + q * 32 + lane;
     const bool row_ok = m < M;
 #pragma unroll 1
-    for (int c0 = 0; c0 < BN; c0 += 32) {
+    for (int c0 = c_lo; c0 < c_hi; c0 += 32) {
       uint32_t r[32];
       tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)c0, r);
       if (!row_ok) continue;
@@ -499,7 +501,7 @@ int launch_cfg(int64_t M, int N, int K, const CUtensorMap& ta, const CUtensorMap
   }
   const int n_tiles = N / BN;
   const int64_t m_tiles = (M + BM - 1) / BM;
-  tc_gemm_k<BN, STAGES><<<(unsigned)(m_tiles * n_tiles), NTHREADS, L::TOTAL, st>>>(ta, tb, M, N, K, n_tiles, epi);
+  tc_gemm_k<BN, STAGES><<<(unsigned)(m_tiles * n_tiles), NTHREADS_PK, L::TOTAL, st>>>(ta, tb, M, N, K, n_tiles, epi);
   PNN_KCHECK("tc_gemm_k");
   return 1;
 }
