@@ -142,6 +142,31 @@ int pnn_graph_view(const pnn_workspace* ws, const int32_t** rowptr, const int32_
  * rowptr [N+1] i32, col [E] i32, shift [E,3] i8.  Any pointer may be NULL.  Synchronous. */
 int pnn_graph_copy(const pnn_workspace* ws, int32_t* rowptr, int32_t* col, int8_t* shift);
 
+/* The radius graph WITHOUT any allocation — for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it): no model, no workspace.  Same builder and same result as pnn_build_graph (cell
+ * list, strict d < cutoff in FP64, receiver-sorted CSR, bit-identical rowptr / col / shift), but every scratch array of the
+ * build (cell lists, scan buffers, per-edge geometry) lives in ONE file-scope static device array of
+ * PNN_STATIC_SCRATCH_BYTES inside the library, which every GPU that loads libpnn.so holds until the process exits.  Limits,
+ * rejected with PNN_ERR_CAPACITY (pnn_last_cuda_error() then names the argument and the limit): n_atoms <=
+ * PNN_STATIC_MAX_ATOMS, n_structs <= PNN_STATIC_MAX_STRUCTS, max_edges <= PNN_STATIC_MAX_EDGES.
+ *   pos, struct_ptr, cell, pbc: DEVICE, as pnn_build_graph.  pbc_images: PNN_IMAGES_MINIMUM or PNN_IMAGES_ALL.
+ *   rowptr [n_atoms+1] i32, col [max_edges] i32, shift [max_edges,3] i8: DEVICE, caller-owned OUTPUTS; rowptr[n_atoms] is the
+ *   number of directed edges.  flags: DEVICE i32 [1] output or NULL: 0, or PNN_STATIC_EDGE_OVERFLOW when the graph has more
+ *   than max_edges edges (rowptr is then still complete, col / shift are unspecified).
+ * Asynchronous on cuda_stream; calls no cudaMalloc / cudaFree or allocating routine.  The address of the static array is
+ * resolved once per device, on the first call made with that device current (make that call outside graph capture).  ALL
+ * calls share the array: calls that overlap on the GPU (different streams, or another host thread's call on the same
+ * device) race; issue them on one stream or order them with events.  The array keeps the previous call's contents; what
+ * must start at zero is cleared on the stream by every call. */
+#define PNN_STATIC_MAX_ATOMS 16384
+#define PNN_STATIC_MAX_STRUCTS 4096
+#define PNN_STATIC_MAX_EDGES 262144
+#define PNN_STATIC_SCRATCH_BYTES (6 * 1024 * 1024)
+#define PNN_STATIC_EDGE_OVERFLOW 1
+int pnn_build_graph_static(int64_t n_atoms, int64_t n_structs, const double* pos, const int32_t* struct_ptr,
+                           const double* cell, const uint8_t* pbc, double cutoff, int32_t pbc_images, int64_t max_edges,
+                           int32_t* rowptr, int32_t* col, int8_t* shift, int32_t* flags, void* cuda_stream);
+
 #define PNN_ENERGY 1
 #define PNN_FORCES 2
 

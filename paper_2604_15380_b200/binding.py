@@ -18,7 +18,9 @@ __all__ = [
     "pnn_model_destroy", "pnn_branch_mlp_create", "pnn_branch_mlp_destroy", "pnn_branch_weights",
     "pnn_workspace_create", "pnn_workspace_destroy", "pnn_workspace_bytes", "pnn_workspace_edge_tape_bytes",
     "PNN_WS_FORCES", "PNN_WS_NO_EDGE_TAPE", "pnn_build_graph",
-    "pnn_graph_view", "pnn_graph_copy", "pnn_eval", "pnn_set_globals", "pnn_eval_blended", "pnn_eval_host", "pnn_stream_create", "pnn_stream_destroy", "pnn_stream_submit", "pnn_stream_wait",
+    "pnn_graph_view", "pnn_graph_copy", "pnn_build_graph_static", "PNN_STATIC_MAX_ATOMS", "PNN_STATIC_MAX_STRUCTS",
+    "PNN_STATIC_MAX_EDGES", "PNN_STATIC_SCRATCH_BYTES", "PNN_STATIC_EDGE_OVERFLOW", "PNN_IMAGES_MINIMUM", "PNN_IMAGES_ALL",
+    "pnn_eval", "pnn_set_globals", "pnn_eval_blended", "pnn_eval_host", "pnn_stream_create", "pnn_stream_destroy", "pnn_stream_submit", "pnn_stream_wait",
     "pnn_stream_drain", "pnn_stream_launch_count", "pnn_stream_bytes", "pnn_check_async_errors", "pnn_measure_alu_peak", "pnn_launch_count", "pnn_profile_enable",
     "pnn_profile_read", "pnn_gemm_bf16",
     "PaiNN", "PRECISIONS",
@@ -27,6 +29,9 @@ __all__ = [
 PNN_OK = 0
 PNN_BF16, PNN_FP32, PNN_FP64 = 0, 1, 2
 PNN_ENERGY, PNN_FORCES = 1, 2
+PNN_STATIC_MAX_ATOMS, PNN_STATIC_MAX_STRUCTS, PNN_STATIC_MAX_EDGES = 16384, 4096, 262144
+PNN_STATIC_SCRATCH_BYTES, PNN_STATIC_EDGE_OVERFLOW = 6 * 1024 * 1024, 1
+PNN_IMAGES_MINIMUM, PNN_IMAGES_ALL = 0, 1
 PRECISIONS = {"bf16": PNN_BF16, "fp32": PNN_FP32, "fp64": PNN_FP64}
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -83,6 +88,7 @@ def lib():
         L.pnn_graph_view.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp),
                                      ctypes.POINTER(i64)]
         L.pnn_graph_copy.argtypes = [vp, vp, vp, vp]
+        L.pnn_build_graph_static.argtypes = [i64, i64, vp, vp, vp, vp, ctypes.c_double, ctypes.c_int32, i64, vp, vp, vp, vp, vp]
         L.pnn_eval.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, i32, vp, vp, vp]
         L.pnn_set_globals.argtypes = [vp, i64, vp]
         L.pnn_eval_blended.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, ctypes.c_double, i32, vp, vp, vp]
@@ -214,6 +220,19 @@ def pnn_graph_view(ws: int):
 
 def pnn_graph_copy(ws: int, rowptr=None, col=None, shift=None):
     _check(lib().pnn_graph_copy(ws, _ptr(rowptr, "i32"), _ptr(col, "i32"), _ptr(shift, "i8")), "pnn_graph_copy")
+
+
+def pnn_build_graph_static(n_atoms: int, n_structs: int, pos, struct_ptr, cell, pbc, cutoff: float, pbc_images: int,
+                           max_edges: int, rowptr, col, shift, flags=None, stream=None) -> None:
+    """The radius graph into caller-owned DEVICE buffers with no allocation inside the library (include/pnn.h: scratch in a
+    static device array of PNN_STATIC_SCRATCH_BYTES; sizes beyond PNN_STATIC_MAX_* raise PnnError(-2) naming the limit)."""
+    st = lib().pnn_build_graph_static(n_atoms, n_structs, _ptr(pos, "f64", True), _ptr(struct_ptr, "i32", True),
+                                      _ptr(cell, "f64", True), _ptr(pbc, "u8", True), float(cutoff), int(pbc_images),
+                                      max_edges, _ptr(rowptr, "i32", True), _ptr(col, "i32", True),
+                                      _ptr(shift, "i8", True), _ptr(flags, "i32", True), stream)
+    if st == -2:
+        raise PnnError(st, "pnn_build_graph_static: " + pnn_last_cuda_error())
+    _check(st, "pnn_build_graph_static")
 
 
 def pnn_eval(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, struct_ptr, head, flags: int, energy,

@@ -3,6 +3,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <type_traits>
@@ -1358,6 +1359,85 @@ int pnn_gemm_bf16(int64_t M, int32_t N, int32_t K, const void* A, int64_t lda, c
   const int nl = launch_gemm_tc(M, N, K, (const __nv_bfloat16*)A, lda, (const __nv_bfloat16*)Wt, ldw, e,
                                 (cudaStream_t)stream);
   if (nl < 0) return PNN_ERR_UNSUPPORTED;
+  if (launch_failed()) return PNN_ERR_CUDA;
+  PNN_TRY(cudaGetLastError());
+  return PNN_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ no-allocation graph build
+// pnn_build_graph_static (include/pnn.h): the graph builder of graph.cu with every scratch array carved out of ONE file-scope
+// device array.  In HOST code the array's name is only a stand-in for the symbol, not a device address: the address the
+// kernels get is resolved here, once per device, with cudaGetSymbolAddress while that device is current.
+} // extern "C"
+
+namespace {
+static __device__ __align__(256) unsigned char g_static_scratch[PNN_STATIC_SCRATCH_BYTES];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mutex;
+unsigned char* g_static_ptr[STATIC_MAX_DEVICES] = {};
+
+// device address of g_static_scratch on the CURRENT device (NULL + last-error text on failure)
+unsigned char* static_scratch_ptr() {
+  int dev = -1;
+  if (!cuda_ok(cudaGetDevice(&dev), "cudaGetDevice") || dev < 0 || dev >= STATIC_MAX_DEVICES) return nullptr;
+  std::lock_guard<std::mutex> lk(g_static_mutex);
+  if (!g_static_ptr[dev]) {
+    void* p = nullptr;
+    if (!cuda_ok(cudaGetSymbolAddress(&p, g_static_scratch), "cudaGetSymbolAddress(static scratch)")) return nullptr;
+    g_static_ptr[dev] = (unsigned char*)p;
+  }
+  return g_static_ptr[dev];
+}
+} // namespace
+
+extern "C" {
+
+int pnn_build_graph_static(int64_t N, int64_t S, const double* pos, const int32_t* sptr, const double* cell,
+                           const uint8_t* pbc, double cutoff, int32_t pbc_images, int64_t max_edges, int32_t* rowptr,
+                           int32_t* col, int8_t* shift, int32_t* flags, void* stream) {
+  if (N < 0 || S < 0 || max_edges < 0 || !(cutoff > 0.0)) return PNN_ERR_INVALID_ARG;
+  if (pbc_images != PNN_IMAGES_MINIMUM && pbc_images != PNN_IMAGES_ALL) return PNN_ERR_INVALID_ARG;
+  if ((N > 0 && !pos) || !sptr || !rowptr || (max_edges > 0 && (!col || !shift))) return PNN_ERR_INVALID_ARG;
+  auto too_big = [&](const char* what, int64_t v, int64_t lim) {
+    g_last_cuda_error = std::string("pnn_build_graph_static: ") + what + " = " + std::to_string(v) +
+                        " exceeds the static scratch limit " + std::to_string(lim);
+    return PNN_ERR_CAPACITY;
+  };
+  if (N > PNN_STATIC_MAX_ATOMS) return too_big("n_atoms", N, PNN_STATIC_MAX_ATOMS);
+  if (S > PNN_STATIC_MAX_STRUCTS) return too_big("n_structs", S, PNN_STATIC_MAX_STRUCTS);
+  if (max_edges > PNN_STATIC_MAX_EDGES) return too_big("max_edges", max_edges, PNN_STATIC_MAX_EDGES);
+  unsigned char* base = static_scratch_ptr();
+  if (!base) return PNN_ERR_CUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  // carve the builder's scratch (sizes of THIS call; the limits above bound the total by PNN_STATIC_SCRATCH_BYTES)
+  const int64_t Nn = N > 0 ? N : 1, Sn = S > 0 ? S : 1, En = max_edges > 0 ? max_edges : 1;
+  int64_t off = 0;
+  auto carve = [&](int64_t bytes) { unsigned char* q = base + off; off += (bytes + 255) / 256 * 256; return (void*)q; };
+  GraphBuffers g{};
+  g.d_err = (int*)carve(256);
+  g.d_ovf = g.d_err + 1;
+  g.d_poschk = reinterpret_cast<unsigned long long*>(g.d_err + 4);
+  g.a2s = (int32_t*)carve(4 * Nn);
+  g.desc = (GridDesc*)carve((int64_t)sizeof(GridDesc) * Sn);
+  g.ncell = (int32_t*)carve(4 * (Sn + 1));
+  g.cell_off = (int32_t*)carve(4 * (Sn + 1));
+  g.cid = (int32_t*)carve(4 * Nn);
+  g.cell_cnt = (int32_t*)carve(4 * (Nn + Sn + 2));
+  g.cell_start = (int32_t*)carve(4 * (Nn + Sn + 2));
+  g.cell_fill = (int32_t*)carve(4 * (Nn + Sn + 2));
+  g.sorted = (int32_t*)carve(4 * Nn);
+  g.deg = (int32_t*)carve(4 * (Nn + 1));
+  g.scan_tmp = (int32_t*)carve(4 * ((Nn + Sn + 2) / 1024 + 4));
+  g.geom = carve((int64_t)sizeof(Geom<float>) * En); // per-edge geometry: written by the builder, not an output here
+  if (off > (int64_t)PNN_STATIC_SCRATCH_BYTES) return too_big("scratch bytes", off, PNN_STATIC_SCRATCH_BYTES);
+  g.rowptr = rowptr; g.col = col; g.shift = shift; // the caller's outputs
+  g.max_edges = max_edges;
+  // the array keeps the last call's contents: the sticky error word must start at zero (the builder clears the cell
+  // counters, the position checksum and the overflow word itself)
+  PNN_TRY(cudaMemsetAsync(g.d_err, 0, 256, st));
+  launch_graph_build(g, N, S, pos, sptr, cell, pbc, cutoff, PNN_FP32, pbc_images, 0, st);
+  if (flags) PNN_TRY(cudaMemcpyAsync(flags, g.d_ovf, sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
   if (launch_failed()) return PNN_ERR_CUDA;
   PNN_TRY(cudaGetLastError());
   return PNN_OK;
