@@ -57,6 +57,7 @@ WORKLOAD_NAMES = {"cfg1": "cfg1_tiny_fp64", "cfg2": "cfg2_molecular_fp32", "cfg2
                   "cfg2_cap20": "cfg2_molecular_fp32_max_neighbors_20", "cfg2_schnet": "cfg2_molecular_fp32_schnet"}
 FULL_RECORDS = ("cfg2", "cfg3_fp32", "cfg3_bf16", "cfg4", "cfg5")   # BASELINE.json configs[1..4] (cfg3 in both precisions)
 CFG4_STREAM_BATCHES = 64                                            # 1,048,576 structures / 16,384
+STREAM_DEPTH = 2   # pipeline slots of the streaming driver (measured: 3 slots are not faster, 1.073 against 1.062 of resident)
 DTYPE = {"fp64": "f64", "fp32": "f32", "bf16": "bf16"}
 # plain-ALU peaks derived from the guide's unit counts and clocks:
 # 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz; FP64 at half the FP32 lane count.
@@ -441,7 +442,7 @@ def main():
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
         hin = [(pin(b.Z), pin(b.pos), pin(b.struct_ptr), pin(b.head)) for b in batches]
         eo = [torch.empty(S, dtype=torch.float32).pin_memory() for _ in batches]
-        sh = pnn.pnn_stream_create(net.model, maxN, int(maxN * 12.5), S, pnn.PNN_ENERGY, 2)
+        sh = pnn.pnn_stream_create(net.model, maxN, int(maxN * 12.5), S, pnn.PNN_ENERGY, STREAM_DEPTH)
         try:
             def run(n):
                 for k in range(n):
@@ -467,7 +468,7 @@ def main():
         n_struct = S * n_batches * world
         h2d = sum(x.numel() * x.element_size() for hb in hin for x in hb)
         assert all(np.isfinite(e.numpy()).all() for e in eo)
-        return dict(api="pnn_stream_submit / pnn_stream_drain (depth 2: two workspaces, two CUDA streams, pinned host buffers)",
+        return dict(api=f"pnn_stream_submit / pnn_stream_drain (depth {STREAM_DEPTH}: one workspace and CUDA stream per slot, pinned host buffers)",
                     batches=n_batches * world, ranks=world, structures=n_struct, atoms=int(sum(b.n_atoms for b in batches)), seconds=dt,
                     structures_per_s=n_struct / dt, ms_per_batch=1e3 * dt / n_batches,
                     resident_ms_per_batch=res["ms_per_step_median"],
