@@ -333,12 +333,22 @@ def main():
             # the composition -> softmax router runs on the device inside every step (Fig. 5)
             net.set_branch_mlp(gen.BRANCH_MLP_WIDTHS, gen.make_branch_mlp())
 
-        def step():
+        def step_eager():
             if blended:
                 hw = net.branch_weights(d["Z"], d["sp"])
                 return net.eval_blended(d["Z"], d["pos"], d["sp"], hw, d["cell"], d["pbc"], forces=forces,
                                         skip_below=0.01)
             return net.eval(d["Z"], d["pos"], d["sp"], d["head"], d["cell"], d["pbc"], forces=forces)
+
+        # the timed step: graph build + evaluation replayed as ONE CUDA graph (pnn_eval_replay: same kernels, bit-identical
+        # results, fixed output buffers); the blended pipeline has no recorded form and stays eager
+        e_out = torch.empty(b.n_structs, dtype=net.out_dtype, device=dev)
+        f_out = torch.empty((b.n_atoms, 3), dtype=net.out_dtype, device=dev) if forces else None
+
+        def step():
+            if blended:
+                return step_eager()
+            return net.eval_replay(d["Z"], d["pos"], d["sp"], d["head"], e_out, f_out, d["cell"], d["pbc"])
 
         for _ in range(warmup):
             flush.zero_()
@@ -366,6 +376,15 @@ def main():
         t_wall = time.perf_counter() - t_wall0
         launches = net.launches - l0
         per_step_ms = [a.elapsed_time(z) for a, z in ev]
+        # the same step launched kernel by kernel (pnn_build_graph + pnn_eval), a few steps, for comparison
+        ev_e = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(min(steps, 10))]
+        for a, z in ev_e:
+            flush.zero_()
+            a.record(st)
+            step_eager()
+            z.record(st)
+        torch.cuda.synchronize()
+        eager_ms = float(np.median([a.elapsed_time(z) for a, z in ev_e]))
         ms = sum(per_step_ms)
         tmax = torch.tensor([ms, float(np.median(per_step_ms))], dtype=torch.float64, device=dev)
         tot = torch.tensor([float(b.n_structs), float(E), float(b.n_atoms)], dtype=torch.float64, device=dev)
@@ -377,7 +396,8 @@ def main():
         res = dict(name=name, prec=prec, forces=forces, mc=mc, batch=b, n_structs=S_tot, n_edges=E_tot, n_atoms=N_tot,
                    ms_per_step=ms / steps, ms_per_step_median=med, ms_per_step_min=min(per_step_ms), steps=steps,
                    structures_per_s=S_tot * steps / (ms * 1e-3), edges_per_s=E_tot * steps / (ms * 1e-3),
-                   launches=launches, wall_s=t_wall, ws_bytes=pnn.pnn_workspace_bytes(net.ws),
+                   launches=launches, wall_s=t_wall, ws_bytes=pnn.pnn_workspace_bytes(net.ws), eager_ms=eager_ms,
+                   launch_mode="eager" if blended else "CUDA graph replay (pnn_eval_replay)",
                    tape_bytes=pnn.pnn_workspace_edge_tape_bytes(net.ws))
         if full:
             # ---- end to end through the host entry point: pinned host buffers, H2D + D2H inside the timed region
@@ -417,7 +437,7 @@ def main():
             pnn.pnn_profile_enable(net.ws, True)
             for _ in range(steps):
                 flush.zero_()
-                step()
+                step_eager()
             prof = pnn.pnn_profile_read(net.ws)
             pnn.pnn_profile_enable(net.ws, False)
             res["profile"] = prof
@@ -514,6 +534,7 @@ def main():
                    F=mc.F, T=mc.T, K=mc.K, H=mc.H, cutoff=mc.cutoff, steps=res["steps"],
                    ms_per_step=res["ms_per_step_median"], ms_per_step_mean=res["ms_per_step"],
                    ms_per_step_min=res["ms_per_step_min"], timing="median of per-step CUDA-event times, L2 flushed",
+                   launch_mode=res["launch_mode"], ms_per_step_eager=res["eager_ms"],
                    structures_per_s=res["n_structs"] / (res["ms_per_step_median"] * 1e-3),
                    edges_per_s=res["n_edges"] / (res["ms_per_step_median"] * 1e-3), clocks=res.get("clocks"),
                    e2e=res.get("e2e"), gpu_launches_per_step=res["launches"] / res["steps"], roofline=roof,
@@ -541,7 +562,8 @@ def main():
                             directed_edges_per_step=main_rec["directed_edges_per_step"],
                             mean_degree=main_rec["mean_degree"], F=mc.F, T=mc.T, K=mc.K, H=mc.H, cutoff=mc.cutoff,
                             outputs=main_rec["outputs"], l2="flushed between timed steps (256 MB write)",
-                            timing="median of the per-step CUDA-event times", parallelism=f"replica x{world}"),
+                            timing="median of the per-step CUDA-event times", parallelism=f"replica x{world}",
+                            launch=main_rec["launch_mode"], ms_per_step_eager=main_rec["ms_per_step_eager"]),
                 edges_per_s=main_rec["edges_per_s"], clocks=main_rec["clocks"], e2e=main_rec["e2e"],
                 gpu_launches=int(main_res["launches"]), roofline=main_rec["roofline"],
                 roofline_per_kernel=main_rec["roofline_per_kernel"], step_roofline=main_rec["step_roofline"],

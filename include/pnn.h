@@ -183,6 +183,19 @@ int pnn_eval(const pnn_model* m, pnn_workspace* ws, int64_t n_atoms, int64_t n_s
              const double* pos, const int32_t* struct_ptr, const int32_t* head, int flags, void* energy,
              void* forces, void* cuda_stream);
 
+/* pnn_build_graph + pnn_eval as ONE replayed CUDA graph, for loops that evaluate the same (n_atoms, n_structs) again and again
+ * with positions updated IN PLACE (molecular dynamics, relaxations; small batches are bound by launch overhead: ~60-110
+ * launches per evaluation).  Every launch geometry of the path depends on n_atoms / n_structs only (the edge count lives on
+ * the device), so the recorded sequence stays valid when the atoms move.  The first call with a new signature — sizes, flags,
+ * stream and every pointer argument — runs the path eagerly (it also sets kernel attributes), the second records it into a CUDA
+ * graph on an internal stream, and from then on a call is one cudaGraphLaunch on cuda_stream.  Arguments and error behaviour
+ * as pnn_build_graph and pnn_eval; the edge-overflow / bad-input / stale-graph flags are still reported by
+ * pnn_check_async_errors.  A different signature drops the recorded graph and starts over.  Not available while
+ * pnn_profile_enable is on (PNN_ERR_UNSUPPORTED).  Asynchronous. */
+int pnn_eval_replay(const pnn_model* m, pnn_workspace* ws, int64_t n_atoms, int64_t n_structs, const int32_t* Z,
+                    const double* pos, const int32_t* struct_ptr, const int32_t* head, const double* cell,
+                    const uint8_t* pbc, int flags, void* energy, void* forces, void* cuda_stream);
+
 /* Global attributes of the structures of the NEXT evaluations of this workspace (pnn_config.n_global = G > 0): glob DEVICE
  * [n_structs, G] f64 (e.g. total charge, spin multiplicity), read by pnn_eval / pnn_eval_blended when they run — the buffer
  * stays owned by the caller and must stay valid until then; NULL = all attributes zero.  PNN_ERR_INVALID_ARG when the model

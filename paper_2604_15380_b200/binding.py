@@ -20,7 +20,7 @@ __all__ = [
     "PNN_WS_FORCES", "PNN_WS_NO_EDGE_TAPE", "pnn_build_graph",
     "pnn_graph_view", "pnn_graph_copy", "pnn_build_graph_static", "PNN_STATIC_MAX_ATOMS", "PNN_STATIC_MAX_STRUCTS",
     "PNN_STATIC_MAX_EDGES", "PNN_STATIC_SCRATCH_BYTES", "PNN_STATIC_EDGE_OVERFLOW", "PNN_IMAGES_MINIMUM", "PNN_IMAGES_ALL",
-    "pnn_eval", "pnn_set_globals", "pnn_eval_blended", "pnn_eval_host", "pnn_stream_create", "pnn_stream_destroy", "pnn_stream_submit", "pnn_stream_wait",
+    "pnn_eval", "pnn_eval_replay", "pnn_set_globals", "pnn_eval_blended", "pnn_eval_host", "pnn_stream_create", "pnn_stream_destroy", "pnn_stream_submit", "pnn_stream_wait",
     "pnn_stream_drain", "pnn_stream_launch_count", "pnn_stream_bytes", "pnn_check_async_errors", "pnn_measure_alu_peak", "pnn_launch_count", "pnn_profile_enable",
     "pnn_profile_read", "pnn_gemm_bf16",
     "PaiNN", "PRECISIONS",
@@ -91,6 +91,7 @@ def lib():
         L.pnn_build_graph_static.argtypes = [i64, i64, vp, vp, vp, vp, ctypes.c_double, ctypes.c_int32, i64, vp, vp, vp, vp, vp]
         L.pnn_eval.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, i32, vp, vp, vp]
         L.pnn_set_globals.argtypes = [vp, i64, vp]
+        L.pnn_eval_replay.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp]
         L.pnn_eval_blended.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, ctypes.c_double, i32, vp, vp, vp]
         L.pnn_eval_host.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, vp, vp, i32, vp, vp, vp]
         L.pnn_branch_mlp_create.argtypes = [i32, vp, vp, i64, i32, ctypes.POINTER(vp)]
@@ -240,6 +241,15 @@ def pnn_eval(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, struct_p
     _check(lib().pnn_eval(model, ws, n_atoms, n_structs, _ptr(Z, "i32", True), _ptr(pos, "f64", True),
                           _ptr(struct_ptr, "i32", True), _ptr(head, "i32", True), flags, _ptr(energy, None, True),
                           _ptr(forces, None, True), stream), "pnn_eval")
+
+
+def pnn_eval_replay(model: int, ws: int, n_atoms: int, n_structs: int, Z, pos, struct_ptr, head, cell, pbc, flags: int,
+                    energy, forces=None, stream=None):
+    """pnn_build_graph + pnn_eval as one replayed CUDA graph (include/pnn.h): same buffers, positions updated in place."""
+    _check(lib().pnn_eval_replay(model, ws, n_atoms, n_structs, _ptr(Z, "i32", True), _ptr(pos, "f64", True),
+                                 _ptr(struct_ptr, "i32", True), _ptr(head, "i32", True), _ptr(cell, "f64", True),
+                                 _ptr(pbc, "u8", True), flags, _ptr(energy, None, True), _ptr(forces, None, True), stream),
+           "pnn_eval_replay")
 
 
 def pnn_set_globals(ws: int, n_structs: int, glob) -> None:
@@ -439,6 +449,16 @@ class PaiNN:
         flags = PNN_ENERGY | (PNN_FORCES if forces else 0)
         pnn_eval(self.model, self.ws, N, S, Z, pos, struct_ptr, head, flags, energy, frc, self._stream())
         return energy, frc
+
+    def eval_replay(self, Z, pos, struct_ptr, head, energy, forces=None, cell=None, pbc=None):
+        """Graph build + evaluation as one replayed CUDA graph (pnn_eval_replay): the caller owns ALL buffers, inputs and
+        outputs (CUDA tensors), keeps them alive and updates `pos` in place between calls; forces=None: energy only."""
+        N, S = int(Z.shape[0]), int(head.shape[0])
+        self._last_N = N
+        flags = PNN_ENERGY | (PNN_FORCES if forces is not None else 0)
+        pnn_eval_replay(self.model, self.ws, N, S, Z, pos, struct_ptr, head, cell, pbc, flags, energy, forces,
+                        self._stream())
+        return energy, forces
 
     def eval_blended(self, Z, pos, struct_ptr, head_weights, cell=None, pbc=None, forces: Optional[bool] = None,
                      skip_below: float = 0.0, build: bool = True):

@@ -153,6 +153,15 @@ struct pnn_workspace {
   double *st_pos, *st_cell;
   uint8_t* st_pbc;
   void *st_energy, *st_forces;
+  // pnn_eval_replay: the recorded launch sequence (build + eval) of one call signature
+  struct Replay {
+    cudaGraphExec_t exec = nullptr;
+    cudaStream_t cap_stream = nullptr; // internal stream the sequence is recorded on (the legacy default stream cannot capture)
+    int seen = 0;                       // eager calls made with the current signature
+    int64_t N = -1, S = -1; int flags = 0;
+    const void* ptr[10] = {};           // Z, pos, sptr, head, cell, pbc, energy, forces, stream, global attributes
+    int64_t launches = 0;               // kernel launches of one replay
+  } replay;
   // optional per-kernel-family timing (pnn_profile_enable)
   bool profile = false;
   struct ProfRec { const char* name; cudaEvent_t a, b; int launches; };
@@ -547,6 +556,8 @@ int pnn_workspace_create(const pnn_model* m, int64_t maxN, int64_t maxE, int64_t
 
 void pnn_workspace_destroy(pnn_workspace* ws) {
   if (!ws) return;
+  if (ws->replay.exec) cudaGraphExecDestroy(ws->replay.exec);
+  if (ws->replay.cap_stream) cudaStreamDestroy(ws->replay.cap_stream);
   cudaFree(ws->etape);
   for (auto& r : ws->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (auto e : ws->ev_pool) cudaEventDestroy(e);
@@ -1105,6 +1116,56 @@ int pnn_eval(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const 
   const int rc = eval_common(m, ws, N, S, Z, sptr, head, nullptr, 0.0, flags, energy, forces, stream);
   if (rc == PNN_OK) ws->launches += launch_pos_check(ws->g, N, pos, (cudaStream_t)stream);
   return rc;
+}
+
+int pnn_eval_replay(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const int32_t* Z, const double* pos,
+                    const int32_t* sptr, const int32_t* head, const double* cell, const uint8_t* pbc, int flags,
+                    void* energy, void* forces, void* stream) {
+  if (!m || !ws || ws->model != m) return PNN_ERR_INVALID_ARG;
+  if (ws->profile) return PNN_ERR_UNSUPPORTED;
+  pnn_workspace::Replay& r = ws->replay;
+  const void* sig[10] = {Z, pos, sptr, head, cell, pbc, energy, forces, stream, ws->glob};
+  const bool same = r.N == N && r.S == S && r.flags == flags && std::memcmp(sig, r.ptr, sizeof(sig)) == 0;
+  if (!same) { // a new signature: forget the recorded graph
+    if (r.exec) { cudaGraphExecDestroy(r.exec); r.exec = nullptr; }
+    r.seen = 0; r.N = N; r.S = S; r.flags = flags;
+    std::memcpy(r.ptr, sig, sizeof(sig));
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  if (r.exec) { // replay: the graph, the build stream and the sizes are those of the recorded call
+    PNN_TRY(cudaGraphLaunch(r.exec, st));
+    ws->graph_N = N; ws->graph_S = S; ws->graph_stream = st;
+    ws->launches += r.launches;
+    return PNN_OK;
+  }
+  auto run = [&](void* on) {
+    int rc = pnn_build_graph(ws, N, S, pos, sptr, cell, pbc, on);
+    if (rc == PNN_OK) rc = pnn_eval(m, ws, N, S, Z, pos, sptr, head, flags, energy, forces, on);
+    return rc;
+  };
+  if (r.seen++ == 0) return run(stream); // eager: also sets kernel attributes and encodes the tensor maps
+  if (!r.cap_stream) PNN_TRY(cudaStreamCreateWithFlags(&r.cap_stream, cudaStreamNonBlocking));
+  const int64_t l0 = ws->launches;
+  PNN_TRY(cudaStreamBeginCapture(r.cap_stream, cudaStreamCaptureModeThreadLocal));
+  const int rc = run((void*)r.cap_stream);
+  cudaGraph_t graph = nullptr;
+  const cudaError_t ce = cudaStreamEndCapture(r.cap_stream, &graph);
+  r.launches = ws->launches - l0;
+  ws->launches = l0;
+  if (rc != PNN_OK || ce != cudaSuccess || !graph) {
+    if (graph) cudaGraphDestroy(graph);
+    r.seen = 0;
+    if (rc != PNN_OK) return rc;
+    cuda_ok(ce != cudaSuccess ? ce : cudaErrorUnknown, "cudaStreamEndCapture(pnn_eval_replay)");
+    return PNN_ERR_CUDA;
+  }
+  const cudaError_t ie = cudaGraphInstantiate(&r.exec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (!cuda_ok(ie, "cudaGraphInstantiate(pnn_eval_replay)")) { r.exec = nullptr; r.seen = 0; return PNN_ERR_CUDA; }
+  PNN_TRY(cudaGraphLaunch(r.exec, st));
+  ws->graph_N = N; ws->graph_S = S; ws->graph_stream = st;
+  ws->launches += r.launches;
+  return PNN_OK;
 }
 
 int pnn_set_globals(pnn_workspace* ws, int64_t S, const double* glob) {

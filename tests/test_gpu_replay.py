@@ -1,0 +1,56 @@
+"""-m gpu: pnn_eval_replay (graph build + evaluation recorded once into a CUDA graph and replayed while the atoms move in place)
+against the eager path pnn_build_graph + pnn_eval: bit for bit, over a short "trajectory" in which the edge set changes."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import gen
+import oracle
+from gpu_common import make_model, to_device
+from helpers import energy_rel_err, force_rel_err
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("precision,cfg_id,n", [("fp64", 1, 8), ("fp32", 2, 12), ("bf16", 2, 12), ("fp32", 3, 2)])
+def test_replay_matches_eager_along_a_trajectory(precision, cfg_id, n):
+    import torch
+    mc = gen.model_cfg(cfg_id)
+    w = gen.make_weights(mc, cfg_id)
+    b = gen.make_batch(cfg_id, 0, n)
+    net = make_model(mc, w, precision, b.n_atoms, b.n_atoms * 96, b.n_structs, True)
+    ref_net = make_model(mc, w, precision, b.n_atoms, b.n_atoms * 96, b.n_structs, True)
+    try:
+        t = to_device(b)
+        pos = t["pos"].clone()
+        energy = torch.empty(b.n_structs, dtype=net.out_dtype, device="cuda")
+        forces = torch.empty((b.n_atoms, 3), dtype=net.out_dtype, device="cuda")
+        rng = np.random.default_rng(1)
+        edge_counts = set()
+        for step in range(6):          # call 0 eager, call 1 records, calls 2.. replay
+            if step:
+                pos += torch.from_numpy(rng.normal(0, 0.15, (b.n_atoms, 3))).cuda()    # in place: same buffer
+            net.eval_replay(t["Z"], pos, t["struct_ptr"], t["head"], energy, forces, t["cell"], t["pbc"])
+            e_ref, f_ref = ref_net.eval(t["Z"], pos, t["struct_ptr"], t["head"], t["cell"], t["pbc"])
+            torch.cuda.synchronize()
+            net.check(); ref_net.check()
+            assert torch.equal(energy, e_ref), step
+            assert torch.equal(forces, f_ref), step
+            edge_counts.add(int(net.graph()[0][-1]))
+        assert len(edge_counts) > 1                                   # the graph really changed under the replayed launch list
+        # and the last frame against the oracle
+        bb = dataclasses.replace(b, pos=pos.cpu().numpy())
+        ref = oracle.evaluate(mc, w, bb)
+        te, tf = {"fp64": (1e-10, 1e-10), "fp32": (1e-5, 1e-3 if cfg_id == 3 else 1e-4), "bf16": (6e-2, 2e-1)}[precision]
+        assert energy_rel_err(energy.double().cpu().numpy(), ref["energy"]).max() < te
+        assert force_rel_err(forces.double().cpu().numpy(), ref["forces"], b.struct_ptr).max() < tf
+        # a new signature (energy only, other output buffer) drops the recorded graph and still works
+        e2 = torch.empty_like(energy)
+        for _ in range(3):
+            net.eval_replay(t["Z"], pos, t["struct_ptr"], t["head"], e2, None, t["cell"], t["pbc"])
+        torch.cuda.synchronize()
+        assert torch.equal(e2, energy)
+    finally:
+        net.close()
+        ref_net.close()
