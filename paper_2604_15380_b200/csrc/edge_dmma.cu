@@ -566,7 +566,7 @@ int launch_edge_fwd_dmma(const EdgeArgs<double>& a, const double* phi, const dou
   if (a.N == 0) return 0;
   const int RB = 16;
   const int64_t nwork = (a.N + RB - 1) / RB;
-  dim3 grid((unsigned)std::min<int64_t>(nwork, 148 * 8), a.F / DFS);
+  dim3 grid((unsigned)std::min<int64_t>(nwork, 148), a.F / DFS); // one CTA per SM and slab at a time; swept: 148 x 1..8 within 1 %
   const int KS = (a.K + 3) / 4;
   const size_t smem = sizeof(double) * 2 * DPASS * (4 * KS + GPAD + 4) + sizeof(int) * 2 * DPASS + (size_t)12 * 2 * FSLOTS * 32 * 16;
 #define PNN_LAUNCH_DF(KSV)                                                                                              \
@@ -598,7 +598,7 @@ int launch_edge_bwd_dmma(const EdgeArgs<double>& a, const double* phi, const dou
   if (a.N == 0) return 0;
   const int RB = 16;
   const int64_t nwork = (a.N + RB - 1) / RB;
-  dim3 grid((unsigned)std::min<int64_t>(nwork, 148 * 8), a.F / DFS);
+  dim3 grid((unsigned)std::min<int64_t>(nwork, 148), a.F / DFS); // one CTA per SM and slab at a time; swept: 148 x 1..8 within 1 %
   const int KS = (a.K + 3) / 4, LD = 4 * KS + GPAD;
   const size_t smem = sizeof(double) * (2 * (2 * DPASS * LD + DPASS * 6) + 2 * 12 * 3) + sizeof(int) * 2 * DPASS +
                       (size_t)12 * 2 * GSLOTS * 32 * 16;
