@@ -236,7 +236,9 @@ int pnn_branch_weights(const pnn_branch_mlp* b, pnn_workspace* ws, int64_t n_ato
 /* Convenience for callers with HOST buffers (bench.py's e2e leg): copies Z, pos, struct_ptr, head (and cell /
  * pbc when not NULL) to the device, runs pnn_build_graph + pnn_eval and copies energy [S] / forces [N,3] back.
  * energy_host / forces_host have the dtype pnn_eval documents.  Device-side errors of the call (edge overflow, bad Z /
- * head) are returned by the call itself.  Synchronous. */
+ * head) are returned by the call itself.  When consecutive calls on a workspace have the same n_atoms and n_structs the
+ * device part is replayed as one CUDA graph (pnn_eval_replay on the workspace's staging buffers; not while profiling is
+ * on); the streaming driver inherits this for batches of a fixed shape.  Synchronous. */
 int pnn_eval_host(const pnn_model* m, pnn_workspace* ws, int64_t n_atoms, int64_t n_structs, const int32_t* Z,
                   const double* pos, const int32_t* struct_ptr, const int32_t* head, const double* cell,
                   const uint8_t* pbc, int flags, void* energy_host, void* forces_host, void* cuda_stream);

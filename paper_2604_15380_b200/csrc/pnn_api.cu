@@ -1286,12 +1286,21 @@ static int enqueue_host_batch(const pnn_model* m, pnn_workspace* ws, int64_t N, 
     PNN_TRY(cudaMemcpyAsync(ws->st_cell, cell, 72 * S, cudaMemcpyHostToDevice, st));
     PNN_TRY(cudaMemcpyAsync(ws->st_pbc, pbc, 3 * S, cudaMemcpyHostToDevice, st));
   }
-  int rc = pnn_build_graph(ws, N, S, ws->st_pos, ws->st_sptr, periodic ? ws->st_cell : nullptr,
-                           periodic ? ws->st_pbc : nullptr, stream);
-  if (rc != PNN_OK) return rc;
   ws->glob = nullptr; // the host entry points evaluate with zero global attributes
-  rc = eval_common(m, ws, N, S, ws->st_Z, ws->st_sptr, ws->st_head, nullptr, 0.0, flags, ws->st_energy, ws->st_forces,
-                   stream);
+  int rc;
+  if (!ws->profile) {
+    // graph build + evaluation on the staging buffers: their addresses never change, so when the sizes repeat (a loop over
+    // one system, batches of a fixed shape) the launch sequence is replayed as one CUDA graph (pnn_eval_replay); ragged
+    // batches change the signature every time and run kernel by kernel as before
+    rc = pnn_eval_replay(m, ws, N, S, ws->st_Z, ws->st_pos, ws->st_sptr, ws->st_head, periodic ? ws->st_cell : nullptr,
+                         periodic ? ws->st_pbc : nullptr, flags, ws->st_energy, ws->st_forces, stream);
+  } else {
+    rc = pnn_build_graph(ws, N, S, ws->st_pos, ws->st_sptr, periodic ? ws->st_cell : nullptr,
+                         periodic ? ws->st_pbc : nullptr, stream);
+    if (rc == PNN_OK)
+      rc = eval_common(m, ws, N, S, ws->st_Z, ws->st_sptr, ws->st_head, nullptr, 0.0, flags, ws->st_energy, ws->st_forces,
+                       stream);
+  }
   if (rc != PNN_OK) return rc;
   if (S > 0) PNN_TRY(cudaMemcpyAsync(energy_host, ws->st_energy, es * S, cudaMemcpyDeviceToHost, st));
   if ((flags & PNN_FORCES) && N > 0)
