@@ -187,8 +187,8 @@ int pnn_eval(const pnn_model* m, pnn_workspace* ws, int64_t n_atoms, int64_t n_s
  * with positions updated IN PLACE (molecular dynamics, relaxations; small batches are bound by launch overhead: ~60-110
  * launches per evaluation).  Every launch geometry of the path depends on n_atoms / n_structs only (the edge count lives on
  * the device), so the recorded sequence stays valid when the atoms move.  The first call with a new signature — sizes, flags,
- * stream and every pointer argument — runs the path eagerly (it also sets kernel attributes), the second records it into a CUDA
- * graph on an internal stream, and from then on a call is one cudaGraphLaunch on cuda_stream.  Arguments and error behaviour
+ * stream and every pointer argument — and the one after it run the path eagerly (kernel attributes are set then), the third
+ * records it into a CUDA graph on an internal stream, and from then on a call is one cudaGraphLaunch on cuda_stream.  Arguments and error behaviour
  * as pnn_build_graph and pnn_eval; the edge-overflow / bad-input / stale-graph flags are still reported by
  * pnn_check_async_errors.  A different signature drops the recorded graph and starts over.  Not available while
  * pnn_profile_enable is on (PNN_ERR_UNSUPPORTED).  Asynchronous. */
