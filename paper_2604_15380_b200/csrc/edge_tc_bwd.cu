@@ -410,7 +410,7 @@ edge_bwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
         auto used = [&](int si) {
           return si < NSTEP && lds64(mt_u + (uint32_t)offsetof(TileMetaB, sinfo) + 8u * si).y != 0u;
         };
-        auto process = [&](int si, const Gath& G) {
+        auto process = [&](int si, const Gath& G, bool last) {
           const uint32_t cb = (uint32_t)si * (ES * 4);
           float W[NACC][ES], D[NACC][ES];
 #pragma unroll
@@ -431,6 +431,12 @@ edge_bwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
           const float2 idd = lds64f(mt_u + (uint32_t)offsetof(TileMetaB, Id) + cb);
 #pragma unroll
           for (int acc = 0; acc < NACC; ++acc) { tmem_wait2(W[acc], acc == 0); tmem_wait2(D[acc], false); }
+          if (last) { // the tile's last TMEM read is done: hand the buffer back now, so that the next tile's MMAs (there is
+                      // ONE buffer per pipeline) run under the arithmetic of this step instead of after it
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tmem_empty(g, n & 1u));
+          }
 #pragma unroll
           for (int c = 0; c < ES; ++c) {
             const float u0 = c ? ux.y : ux.x, u1 = c ? uy.y : uy.x, u2 = c ? uz.y : uz.x, invd = c ? idd.y : idd.x;
@@ -480,16 +486,15 @@ edge_bwd_tc_k(EdgeMmaArgs a, int RA, const __nv_bfloat16* __restrict__ fltT, con
         for (int si = 0; si < NSTEP; si += 2) {
           const bool u1 = used(si + 1);
           if (u1) load_step(si + 1, Gb);
-          process(si, Ga);
+          process(si, Ga, !u1);
           if (!u1) break;
           const bool u2 = used(si + 2);
           if (u2) load_step(si + 2, Ga);
-          process(si + 1, Gb);
+          process(si + 1, Gb, !u2);
           if (!u2) break;
         }
-        tc_fence_before();
         __syncwarp();
-        if (lane == 0) { mbar_arrive(tmem_empty(g, n & 1u)); mbar_arrive(meta_empty(g, slot)); }
+        if (lane == 0) mbar_arrive(meta_empty(g, slot)); // (tmem_empty was signalled inside the tile's last step)
       }
       end_row(cur);
       for (int k = cur + 1; k < (int)a1; ++k) { begin_row(k); end_row(k); }
