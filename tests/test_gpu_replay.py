@@ -54,3 +54,33 @@ def test_replay_matches_eager_along_a_trajectory(precision, cfg_id, n):
     finally:
         net.close()
         ref_net.close()
+
+
+@pytest.mark.parametrize("precision", ["fp32", "bf16"])
+def test_eval_host_replays_when_the_shape_repeats(precision):
+    """pnn_eval_host records its device part on the third call with the same batch shape: every call gives the same bits, a
+    batch of another shape in between runs eagerly, and moving the atoms (same shape) is picked up by the replayed graph."""
+    mc = gen.model_cfg(2)
+    w = gen.make_weights(mc, 2)
+    b1, b2 = gen.make_batch(2, 0, 10), gen.make_batch(2, 10, 7)
+    net = make_model(mc, w, precision, max(b1.n_atoms, b2.n_atoms), max(b1.n_atoms, b2.n_atoms) * 40, 10, True)
+    ref_net = make_model(mc, w, precision, max(b1.n_atoms, b2.n_atoms), max(b1.n_atoms, b2.n_atoms) * 40, 10, True)
+    try:
+        def host(n, b):
+            e, f = n.eval_host(b.Z, b.pos, b.struct_ptr, b.head, forces=True)
+            return e.copy(), f.copy()
+        e1, f1 = host(ref_net, b1)
+        e2, f2 = host(ref_net, b2)
+        for k in range(5):
+            e, f = host(net, b1)
+            assert np.array_equal(e, e1) and np.array_equal(f, f1), k
+        e, f = host(net, b2)
+        assert np.array_equal(e, e2) and np.array_equal(f, f2)
+        moved = dataclasses.replace(b1, pos=b1.pos + np.random.default_rng(0).normal(0, 0.1, b1.pos.shape))
+        em, fm = host(ref_net, moved)
+        for k in range(4):
+            e, f = host(net, moved if k != 1 else b1)     # same shape, other positions: the same recorded graph
+            assert np.array_equal(e, e1 if k == 1 else em) and np.array_equal(f, f1 if k == 1 else fm), k
+    finally:
+        net.close()
+        ref_net.close()
