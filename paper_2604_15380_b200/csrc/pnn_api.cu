@@ -161,7 +161,10 @@ struct pnn_workspace {
     int64_t N = -1, S = -1; int flags = 0;
     const void* ptr[10] = {};           // Z, pos, sptr, head, cell, pbc, energy, forces, stream, global attributes
     int64_t launches = 0;               // kernel launches of one replay
+    cudaStream_t cap_stream2 = nullptr; // the graph build is recorded on a forked stream: it runs beside the embedding and the
+    cudaEvent_t ev_fork = nullptr, ev_graph = nullptr; // first block's node GEMMs, which do not need the graph
   } replay;
+  cudaEvent_t graph_ready = nullptr;    // while recording: the event the first kernel that reads the graph must wait for
   // optional per-kernel-family timing (pnn_profile_enable)
   bool profile = false;
   struct ProfRec { const char* name; cudaEvent_t a, b; int launches; };
@@ -178,6 +181,11 @@ int read_error_flags(pnn_workspace* ws) {
   if (flags[0] & ERRF_STALE_GRAPH) return PNN_ERR_NO_GRAPH;
   if (flags[0] & (ERRF_BAD_Z | ERRF_BAD_HEAD)) return PNN_ERR_BAD_INPUT;
   return PNN_OK;
+}
+
+// pnn_eval_replay records the graph build on a forked stream: the first kernel that reads the graph waits for it here
+inline void wait_graph(pnn_workspace* ws, cudaStream_t st) {
+  if (ws->graph_ready) cudaStreamWaitEvent(st, ws->graph_ready, 0);
 }
 
 // Brackets the launches of one kernel family with CUDA events on the launch stream when profiling is on.
@@ -558,6 +566,9 @@ void pnn_workspace_destroy(pnn_workspace* ws) {
   if (!ws) return;
   if (ws->replay.exec) cudaGraphExecDestroy(ws->replay.exec);
   if (ws->replay.cap_stream) cudaStreamDestroy(ws->replay.cap_stream);
+  if (ws->replay.cap_stream2) cudaStreamDestroy(ws->replay.cap_stream2);
+  if (ws->replay.ev_fork) cudaEventDestroy(ws->replay.ev_fork);
+  if (ws->replay.ev_graph) cudaEventDestroy(ws->replay.ev_graph);
   cudaFree(ws->etape);
   for (auto& r : ws->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (auto e : ws->ev_pool) cudaEventDestroy(e);
@@ -674,8 +685,10 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
 
   { ProfScope ps_(ws, st, "embed");
   int l_ = launch_embed<T>(N, F, c.Zmax, Z, W + m->emb, s_cur, ws->g.d_err, st);
-    if (c.n_global > 0 && ws->glob)
+    if (c.n_global > 0 && ws->glob) {
+      wait_graph(ws, st);
       l_ += launch_embed_globals<T>(N, F, c.n_global, ws->g.a2s, ws->glob, W + m->globW, s_cur, nullptr, st);
+    }
     nl += l_; ps_.done(l_); }
   for (int t = 0; t < T_; ++t) {
     const BlockW& b = m->blk[t];
@@ -699,6 +712,7 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     const int l_ = launch_gemm<T>(N, 3 * F, F, h, F, W + b.W2t, 3 * F, phi, 3 * F, e2, st);       // B3a, second Linear
       nl += l_; ps_.done(l_); }
     ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
+    if (t == 0) wait_graph(ws, st);
     { ProfScope ps_(ws, st, "edge_fwd");                                                         // B3b -> s' in sn[:, :F], v'
       int l_;
       if constexpr (std::is_same<T, float>::value) {
@@ -872,8 +886,10 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
 
   { ProfScope ps_(ws, st, "embed");
     int l_ = launch_embed<T>(N, F, c.Zmax, Z, W + m->emb, s_cur, ws->g.d_err, st, mb.s16);
-    if (c.n_global > 0 && ws->glob)
+    if (c.n_global > 0 && ws->glob) {
+      wait_graph(ws, st);
       l_ += launch_embed_globals<T>(N, F, c.n_global, ws->g.a2s, ws->glob, W + m->globW, s_cur, mb.s16, st);
+    }
     nl += l_; ps_.done(l_); }
   for (int t = 0; t < T_; ++t) {
     const BlockW& b = m->blk[t];
@@ -896,6 +912,7 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     TcEpi e2; e2.bias = W + b.b2; e2.Cb = tp16.phi16; e2.ldcb = 3 * F;
     tc("gemm_N", N, 3 * F, F, mb.h16, F, b.W2, e2);                               // B3a: phi = W2 h + b2
     ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
+    if (t == 0) wait_graph(ws, st);
     { ProfScope ps_(ws, st, "edge_fwd");
       EdgeMirror mir; mir.s1 = mb.sn16; mir.ld_s1 = 2 * F; mir.v1 = mb.v1_16;
       const int l_ = launch_edge_fwd_tc(em, m->d_fltT + (int64_t)t * m->fltT_stride, tp16.phi16, s_cur, F, v_in16, v_in, sn,
@@ -1014,6 +1031,7 @@ int eval_schnet(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, con
   { ProfScope ps_(ws, st, "embed");
     const int l_ = launch_embed<T>(N, F, c.Zmax, Z, W + m->emb, x, ws->g.d_err, st);
     nl += l_; ps_.done(l_); }
+  wait_graph(ws, st);
   { ProfScope ps_(ws, st, "edge_fwd");   // radial-basis rows g (and g' for the forces), once per evaluation
     const int l_ = launch_sch_rbf<T>(N, Emax, c.K, KP, c.rbf, c.cutoff, ws->g.rowptr, ws->g.geom, (T*)q.G,
                                      want_f ? (T*)q.Gd : nullptr, ws->g.d_ovf, st);
@@ -1146,10 +1164,26 @@ int pnn_eval_replay(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S,
   // eager twice: the first call also sets kernel attributes and encodes the tensor maps; recording (about a millisecond of host
   // time) starts only when a signature has come three times in a row, so that ragged batch streams never pay for it
   if (r.seen++ < 2) return run(stream);
-  if (!r.cap_stream) PNN_TRY(cudaStreamCreateWithFlags(&r.cap_stream, cudaStreamNonBlocking));
+  if (!r.cap_stream) {
+    PNN_TRY(cudaStreamCreateWithFlags(&r.cap_stream, cudaStreamNonBlocking));
+    PNN_TRY(cudaStreamCreateWithFlags(&r.cap_stream2, cudaStreamNonBlocking));
+    PNN_TRY(cudaEventCreateWithFlags(&r.ev_fork, cudaEventDisableTiming));
+    PNN_TRY(cudaEventCreateWithFlags(&r.ev_graph, cudaEventDisableTiming));
+  }
   const int64_t l0 = ws->launches;
   PNN_TRY(cudaStreamBeginCapture(r.cap_stream, cudaStreamCaptureModeThreadLocal));
-  const int rc = run((void*)r.cap_stream);
+  // the graph build on a forked branch: it runs beside the embedding and the first block's node GEMMs, and joins where the
+  // evaluation first reads the graph (wait_graph) — and once more at the end, so that the branch is always joined
+  int rc = PNN_ERR_CUDA;
+  if (cuda_ok(cudaEventRecord(r.ev_fork, r.cap_stream), "cudaEventRecord") &&
+      cuda_ok(cudaStreamWaitEvent(r.cap_stream2, r.ev_fork, 0), "cudaStreamWaitEvent")) {
+    rc = pnn_build_graph(ws, N, S, pos, sptr, cell, pbc, (void*)r.cap_stream2);
+    if (!cuda_ok(cudaEventRecord(r.ev_graph, r.cap_stream2), "cudaEventRecord") && rc == PNN_OK) rc = PNN_ERR_CUDA;
+    ws->graph_ready = r.ev_graph;
+    if (rc == PNN_OK) rc = pnn_eval(m, ws, N, S, Z, pos, sptr, head, flags, energy, forces, (void*)r.cap_stream);
+    ws->graph_ready = nullptr;
+    cudaStreamWaitEvent(r.cap_stream, r.ev_graph, 0);
+  }
   cudaGraph_t graph = nullptr;
   const cudaError_t ce = cudaStreamEndCapture(r.cap_stream, &graph);
   r.launches = ws->launches - l0;
