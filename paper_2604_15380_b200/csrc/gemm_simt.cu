@@ -8,6 +8,8 @@
 // otherwise (N not a multiple of 64); the BF16 model uses gemm_tc.cu (tcgen05 + TMA + TMEM).
 // Epilogues fuse what follows each Linear in SURVEY.md §8(c): bias, SiLU (+ store of the pre-activation for the
 // reverse sweep), multiplication by silu'(stored pre-activation), and accumulation into C (residual adjoints).
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace pnn {
@@ -175,6 +177,162 @@ gemm_k(int64_t M, int N, int K, const T* __restrict__ A, int64_t lda, const T* _
     }
 }
 
+// ------------------------------------------------------------------------------------------ split-K over a CTA pair (FP32)
+// The 64 x 128 tile with 8 x 8 values per thread reaches about twice the rate of the 4 x 4 tiles (one LDS.128 per 8 packed
+// FMAs instead of per 4), but the small GEMMs of a molecular batch (10,354 x 128) make only 162 such tiles for 148 SMs.
+// Here a CLUSTER of two CTAs shares one tile: CTA r contracts k in [r K/2, (r+1) K/2), then each CTA keeps the 32 rows of the
+// tile that its threads hold in micro-tile group r, adds the partner's partial sums of those rows — read from the partner's
+// shared memory over DSMEM — and runs the epilogue on them: 324 CTAs of 128 threads, three per SM, one wave.  The order of
+// the sum is fixed (k-halves in rank order), so results are deterministic.
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cluster_sync() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ float4 ld_peer4(uint32_t local_addr, uint32_t peer_rank) {
+  uint32_t ra;
+  float4 v;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(local_addr), "r"(peer_rank));
+  asm volatile("ld.shared::cluster.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(ra) : "memory");
+  return v;
+}
+
+__global__ void __launch_bounds__(128, 3)
+gemm_sk_k(int64_t M, int N, int K, const float* __restrict__ A, int64_t lda, const float* __restrict__ B, int64_t ldb,
+          float* __restrict__ C, int64_t ldc, GemmEpi<float> epi) {
+  constexpr int BM = 64, BN = 128, BK = 16, TM = 8, TN = 8, NT = 128, PAD = 4;
+  constexpr int A_LD = BM * BK / 4 / NT, B_LD = BK * BN / 4 / NT; // 2 and 4 vector loads per thread and k-block
+  // one buffer: the double-buffered tiles of the main loop, then the 16 KB exchange area of the split-K reduction
+  __shared__ __align__(16) float smem[2 * BK * (BM + PAD) + 2 * BK * (BN + PAD)];
+  float (*As)[BK][BM + PAD] = reinterpret_cast<float (*)[BK][BM + PAD]>(smem);
+  float (*Bs)[BK][BN + PAD] = reinterpret_cast<float (*)[BK][BN + PAD]>(smem + 2 * BK * (BM + PAD));
+  static_assert(2 * BK * (BM + PAD) + 2 * BK * (BN + PAD) >= NT * 32, "exchange area");
+  const int tid = threadIdx.x;
+  const int tx = tid % (BN / TN), ty = tid / (BN / TN);
+  const int64_t m0 = (int64_t)blockIdx.x * BM;
+  const int n0 = blockIdx.y * BN;
+  const uint32_t rank = blockIdx.z; // rank in the cluster (1, 1, 2)
+  const int kb0 = (int)rank * (K / 2), kb1 = kb0 + K / 2;
+
+  float acc[TM][TN];
+#pragma unroll
+  for (int i = 0; i < TM; ++i)
+#pragma unroll
+    for (int j = 0; j < TN; ++j) acc[i][j] = 0.0f;
+  float4 ra[A_LD], rb[B_LD];
+  auto gload = [&](int k0) {
+#pragma unroll
+    for (int q = 0; q < A_LD; ++q) {
+      const int v = tid + q * NT, r = v / (BK / 4), kq = v % (BK / 4);
+      const int64_t m = m0 + r;
+      ra[q] = (m < M) ? *reinterpret_cast<const float4*>(A + m * lda + k0 + kq * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+#pragma unroll
+    for (int q = 0; q < B_LD; ++q) {
+      const int v = tid + q * NT, r = v / (BN / 4), nq = v % (BN / 4);
+      rb[q] = *reinterpret_cast<const float4*>(B + (int64_t)(k0 + r) * ldb + n0 + nq * 4);
+    }
+  };
+  auto sstore = [&](int buf) {
+#pragma unroll
+    for (int q = 0; q < A_LD; ++q) {
+      const int v = tid + q * NT, r = v / (BK / 4), kq = v % (BK / 4);
+      As[buf][kq * 4 + 0][r] = ra[q].x; As[buf][kq * 4 + 1][r] = ra[q].y;
+      As[buf][kq * 4 + 2][r] = ra[q].z; As[buf][kq * 4 + 3][r] = ra[q].w;
+    }
+#pragma unroll
+    for (int q = 0; q < B_LD; ++q) {
+      const int v = tid + q * NT, r = v / (BN / 4), nq = v % (BN / 4);
+      *reinterpret_cast<float4*>(&Bs[buf][r][nq * 4]) = rb[q];
+    }
+  };
+  gload(kb0);
+  sstore(0);
+  __syncthreads();
+  const int nk = (kb1 - kb0) / BK;
+  for (int kt = 0; kt < nk; ++kt) {
+    const int buf = kt & 1;
+    if (kt + 1 < nk) gload(kb0 + (kt + 1) * BK);
+#pragma unroll
+    for (int k = 0; k < BK; ++k) {
+      float a[TM], b[TN];
+#pragma unroll
+      for (int gi = 0; gi < 2; ++gi) {
+        const float4 t = *reinterpret_cast<const float4*>(&As[buf][k][gi * 32 + ty * 4]);
+        a[gi * 4 + 0] = t.x; a[gi * 4 + 1] = t.y; a[gi * 4 + 2] = t.z; a[gi * 4 + 3] = t.w;
+      }
+#pragma unroll
+      for (int gj = 0; gj < 2; ++gj) {
+        const float4 t = *reinterpret_cast<const float4*>(&Bs[buf][k][gj * 64 + tx * 4]);
+        b[gj * 4 + 0] = t.x; b[gj * 4 + 1] = t.y; b[gj * 4 + 2] = t.z; b[gj * 4 + 3] = t.w;
+      }
+      mac_tile<float, TM, TN>(a, b, acc);
+    }
+    if (kt + 1 < nk) {
+      sstore(buf ^ 1);
+      __syncthreads();
+    }
+  }
+  // exchange: a thread hands the partner the 4 x 8 sums of the micro-tile group the partner keeps (group 1 - rank) through
+  // its own shared memory ([value][thread]: conflict-free), and fetches the partner's sums of its own group over DSMEM
+  __syncthreads(); // the tiles are dead
+  float r[4][8];
+  auto exchange = [&](auto keep_c) { // compile-time group indices: acc stays in registers
+    constexpr int keep = decltype(keep_c)::value, give = 1 - keep;
+#pragma unroll
+    for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+      for (int j4 = 0; j4 < 2; ++j4)
+        *reinterpret_cast<float4*>(&smem[((ii * 2 + j4) * NT + tid) * 4]) =
+            make_float4(acc[give * 4 + ii][j4 * 4 + 0], acc[give * 4 + ii][j4 * 4 + 1], acc[give * 4 + ii][j4 * 4 + 2],
+                        acc[give * 4 + ii][j4 * 4 + 3]);
+    cluster_sync();
+#pragma unroll
+    for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+      for (int j4 = 0; j4 < 2; ++j4) {
+        const float4 p = ld_peer4(smem_addr(&smem[((ii * 2 + j4) * NT + tid) * 4]), (uint32_t)give);
+        // rank 0 holds the first k-half: the sum is always (first half) + (second half)
+        const float* mine = &acc[keep * 4 + ii][j4 * 4];
+        r[ii][j4 * 4 + 0] = keep == 0 ? mine[0] + p.x : p.x + mine[0];
+        r[ii][j4 * 4 + 1] = keep == 0 ? mine[1] + p.y : p.y + mine[1];
+        r[ii][j4 * 4 + 2] = keep == 0 ? mine[2] + p.z : p.z + mine[2];
+        r[ii][j4 * 4 + 3] = keep == 0 ? mine[3] + p.w : p.w + mine[3];
+      }
+  };
+  if (rank == 0) exchange(std::integral_constant<int, 0>()); else exchange(std::integral_constant<int, 1>());
+  const int keep = (int)rank;
+  cluster_sync(); // the partner has read my shared memory: it may be released
+  // epilogue on the kept rows (as gemm_k)
+#pragma unroll
+  for (int ii = 0; ii < 4; ++ii) {
+    const int64_t m = m0 + keep * 32 + ty * 4 + ii;
+    if (m >= M) continue;
+#pragma unroll
+    for (int gj = 0; gj < 2; ++gj) {
+      const int n = n0 + gj * 64 + tx * 4;
+      float x[4] = {r[ii][gj * 4 + 0], r[ii][gj * 4 + 1], r[ii][gj * 4 + 2], r[ii][gj * 4 + 3]};
+      if (epi.bias) {
+        const float4 bv = *reinterpret_cast<const float4*>(epi.bias + n);
+        x[0] += bv.x; x[1] += bv.y; x[2] += bv.z; x[3] += bv.w;
+      }
+      if (epi.act == ACT_SILU) {
+        if (epi.pre) *reinterpret_cast<float4*>(epi.pre + m * epi.ldpre + n) = make_float4(x[0], x[1], x[2], x[3]);
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) x[jj] = silu_f<float>(x[jj]);
+      } else if (epi.act == ACT_MUL_DSILU) {
+        const float4 xv = *reinterpret_cast<const float4*>(epi.aux + m * epi.ldaux + n);
+        x[0] *= dsilu_f<float>(xv.x); x[1] *= dsilu_f<float>(xv.y); x[2] *= dsilu_f<float>(xv.z); x[3] *= dsilu_f<float>(xv.w);
+      }
+      float4* cp = reinterpret_cast<float4*>(C + m * ldc + n);
+      if (epi.accumulate) {
+        const float4 cv = *cp;
+        x[0] += cv.x; x[1] += cv.y; x[2] += cv.z; x[3] += cv.w;
+      }
+      *cp = make_float4(x[0], x[1], x[2], x[3]);
+    }
+  }
+}
+
 } // namespace
 
 template <typename T>
@@ -190,6 +348,20 @@ int launch_gemm(int64_t M, int N, int K, const T* A, int64_t lda, const T* B, in
     if (N >= 128 && wide_tiles >= 2 * 148) {
       dim3 grid((unsigned)((M + 63) / 64), (unsigned)((N + 127) / 128));
       gemm_k<T, 64, 128, 8, 8, 16, 3><<<grid, 128, 0, st>>>(M, N, K, A, lda, B, ldb, C, ldc, epi); PNN_KCHECK("gemm_k");
+    } else if (N % 128 == 0 && K % 32 == 0 && K >= 256 && 2 * wide_tiles >= 148 * 3 && 2 * wide_tiles <= 148 * 4) {
+      // too few wide tiles for the SMs, but twice as many fill them (three CTAs of 128 threads per SM): two CTAs (a cluster)
+      // per tile, each contracting half of K (gemm_sk_k).  Measured: cfg3 FP32 (8,192 x 256 outputs, 512 CTAs) 78 -> 70 us per
+      // launch; cfg2 (10,354 x 128: 324 CTAs, 2.2 per SM) 31 -> 33 us, hence the lower bound
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)((M + 63) / 64), (unsigned)(N / 128), 2);
+      cfg.blockDim = dim3(128);
+      cfg.stream = st;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = 1; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 2;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      cudaLaunchKernelEx(&cfg, gemm_sk_k, M, N, K, (const float*)A, lda, (const float*)B, ldb, (float*)C, ldc, epi);
+      PNN_KCHECK("gemm_sk_k");
     } else {
       // The small GEMMs are one wave of co-resident CTAs, so their time follows the LARGEST number of CTAs on one SM
       // (measured, 64x64 tiles, K = 384: 2 per SM 30.8 us, 3 per SM 41.0 us, 4 per SM 45.1 us).  10,354 rows make 324
