@@ -34,15 +34,17 @@ constexpr int NTHREADS_PK = 64 + 128 * EPI_PER_Q; // TMA warp, MMA warp, 4 * EPI
 
 using namespace tc;
 
-// SiLU and its derivative for the BF16 model's epilogues: ex2.approx / rcp.approx (relative error ~2^-21, far below the BF16
-// rounding of what they feed) instead of expf and an IEEE division -- about 6 instead of 18 instructions per element of an
-// epilogue that binds these GEMMs.  The FP32 and FP64 models keep silu_f / dsilu_f of common.cuh.
+// SiLU of the READOUT epilogue: ex2.approx / rcp.approx (relative error ~1e-6) instead of expf and an IEEE division, about 6
+// instead of 18 instructions per element.  Only there: the readout sums silu values in FP32 straight into the atom energy, so
+// the approximation stays a 1e-6 effect.  In the hidden layers the activation is rounded to BF16 and fed on, and a change
+// in the last bits flips BF16 rounding decisions that the network amplifies (cfg3 results move by
+// percents under 1e-7 perturbations) -- measured: with the approximate SiLU in the hidden-layer epilogues the cfg4 batch
+// gains another 0.3 ms, and the single-structure cfg3 BF16 blended check moves from inside 2e-2 to 3.3e-2.  They keep silu_f.
 __device__ __forceinline__ float silu_fast(float x) { return __fdividef(x, 1.0f + __expf(-x)); }
-__device__ __forceinline__ float dsilu_fast(float x) {
-  const float sg = __fdividef(1.0f, 1.0f + __expf(-x));
-  return sg * fmaf(x, 1.0f - sg, 1.0f);
-}
 
+__device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
 // 32-byte global store (STG.256 on sm_100: one full L2 sector per instruction; a row-owner thread otherwise writes its
 // row in 16-byte halves of a sector).  p must be 32-byte aligned.
 __device__ __forceinline__ void st256(void* p, uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t a4,
@@ -66,7 +68,8 @@ __device__ __forceinline__ bool al32(const void* p, int64_t ld_bytes) {
 
 // Epilogue of one output row segment: 32 accumulator columns of row m starting at column n (bias, activation, optional
 // pre-activation store / silu' factor / accumulate, FP32 and / or BF16 stores as 16-byte vectors of the row).
-__device__ __forceinline__ void epi_chunk(const TcEpi& epi, int64_t m, int n, const uint32_t (&r)[32]) {
+template <bool KEEP_CB = false>
+__device__ __forceinline__ void epi_chunk(const TcEpi& epi, int64_t m, int n, const uint32_t (&r)[32], uint32_t* hout = nullptr) {
   float x[32];
 #pragma unroll
   for (int j = 0; j < 32; ++j) x[j] = __uint_as_float(r[j]);
@@ -93,7 +96,7 @@ __device__ __forceinline__ void epi_chunk(const TcEpi& epi, int64_t m, int n, co
       }
     }
 #pragma unroll
-    for (int j = 0; j < 32; ++j) x[j] = silu_fast(x[j]);
+    for (int j = 0; j < 32; ++j) x[j] = silu_f<float>(x[j]);
   } else if (epi.act == ACT_MUL_DSILU) {
     const float* ap = epi.aux + m * epi.ldaux + n;
     if (al32(epi.aux, epi.ldaux * 4)) {
@@ -102,14 +105,14 @@ __device__ __forceinline__ void epi_chunk(const TcEpi& epi, int64_t m, int n, co
         float av[8];
         ld256(ap + j, av);
 #pragma unroll
-        for (int i = 0; i < 8; ++i) x[j + i] *= dsilu_fast(av[i]);
+        for (int i = 0; i < 8; ++i) x[j + i] *= dsilu_f<float>(av[i]);
       }
     } else {
 #pragma unroll
       for (int j = 0; j < 32; j += 4) {
         const float4 av = reinterpret_cast<const float4*>(ap)[j >> 2];
-        x[j] *= dsilu_fast(av.x); x[j + 1] *= dsilu_fast(av.y);
-        x[j + 2] *= dsilu_fast(av.z); x[j + 3] *= dsilu_fast(av.w);
+        x[j] *= dsilu_f<float>(av.x); x[j + 1] *= dsilu_f<float>(av.y);
+        x[j + 2] *= dsilu_f<float>(av.z); x[j + 3] *= dsilu_f<float>(av.w);
       }
     }
   }
@@ -143,7 +146,13 @@ __device__ __forceinline__ void epi_chunk(const TcEpi& epi, int64_t m, int n, co
       for (int j = 0; j < 32; j += 4) cp[j >> 2] = make_float4(x[j], x[j + 1], x[j + 2], x[j + 3]);
     }
   }
-  if (epi.Cb) {
+  if (KEEP_CB) { // TMA-store epilogue: the BF16 words go to the caller, which stages them in shared memory
+#pragma unroll
+    for (int j = 0; j < 32; j += 2) {
+      __nv_bfloat162 t = __floats2bfloat162_rn(x[j], x[j + 1]);
+      hout[j >> 1] = *reinterpret_cast<uint32_t*>(&t);
+    }
+  } else if (epi.Cb) {
     uint4* bp = reinterpret_cast<uint4*>(epi.Cb + m * epi.ldcb + n);
     uint32_t h[16];
 #pragma unroll
@@ -269,16 +278,24 @@ tc_gemm_k(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 // The shared-memory stage ring runs on across tiles, and the accumulator is double-buffered in TMEM (2 x BN columns), so
 // the TMA loads and MMAs of tile i+1 overlap the epilogue (global stores) of tile i: these GEMMs have K <= 768 and are
 // bound by HBM traffic, not by the tensor pipe, so what matters is that loads and stores never pause.
-template <int BN, int STAGES>
-__global__ void __launch_bounds__(NTHREADS_PK)
-tc_gemm_pk(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, int64_t M, int N, int K,
-           int n_tiles, int64_t total_tiles, TcEpi epi) {
+// TST: the BF16 output leaves through shared memory and the TMA engine (cp.async.bulk.tensor shared -> global): an epilogue
+// warp stages its 32 rows x 64 columns (4 KB, 128-byte swizzle as the tensor map of C expects) and one lane issues the store.
+// A row-owner thread's own global stores touch 32 different lines per instruction and kept the L1 / LSU data pipe ~70 % busy on
+// the wide-output launches (profiles/r02_bf16_node.md); staged, a warp's 4 KB cost 32 shared-memory wavefronts and one TMA.
+constexpr int TST_WARP_BYTES = 32 * 128;
+template <int BN, int STAGES, bool TST = false>
+__global__ void __launch_bounds__(NTHREADS_PK, 2)
+tc_gemm_pk(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+           const __grid_constant__ CUtensorMap tmC, int64_t M, int N, int K, int n_tiles, int64_t total_tiles, TcEpi epi) {
   constexpr int A_BYTES = BM * BK * 2, B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
+  constexpr int STG_BYTES = TST ? 4 * EPI_PER_Q * TST_WARP_BYTES : 0;
+  static_assert(!TST || (BN == 128 && EPI_PER_Q == 2), "TMA-store epilogue: 64 columns per epilogue warp");
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t tiles = (raw + 1023u) & ~1023u;
   unsigned char* tiles_ptr = smem_raw + (tiles - raw);
-  uint64_t* bars = reinterpret_cast<uint64_t*>(tiles_ptr + STAGES * STAGE_BYTES); // full[S], empty[S], accfull[2], accempty[2]
+  const uint32_t stg0 = tiles + STAGES * STAGE_BYTES; // TST: one 4 KB staging buffer per epilogue warp (1024-byte aligned)
+  uint64_t* bars = reinterpret_cast<uint64_t*>(tiles_ptr + STAGES * STAGE_BYTES + STG_BYTES); // full[S], empty[S], accfull[2], accempty[2]
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * STAGES + 4);
   const uint32_t bar0 = smem_u32(bars);
   auto full_bar = [&](int s) { return bar0 + 8u * s; };
@@ -383,7 +400,7 @@ tc_gemm_pk(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
       for (int c0 = c_lo; c0 < c_hi; c0 += 32) {
         uint32_t r[32];
         tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + b * BN + (uint32_t)c0, r);
-        if (!row_ok) continue;
+        if (!row_ok && !TST) continue;
         if (epi.readout) {
           const int n = n0 + c0;
 #pragma unroll
@@ -399,6 +416,35 @@ tc_gemm_pk(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
           if (c0 + 32 >= BN) epi.eatom[m] = esum + epi.b2[hrow];
           continue;
         }
+        if (TST) {
+          const uint32_t sbuf = stg0 + (uint32_t)(warp - 2) * TST_WARP_BYTES;
+          if (c0 == c_lo) { // the previous tile's store must have read this buffer before it is rewritten
+            if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+            __syncwarp();
+          }
+          uint32_t h[16];
+          if (row_ok) epi_chunk<true>(epi, m, n0 + c0, r, h); // rows beyond M: staged as they are, clipped by the TMA store
+          else {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) h[i] = 0u;
+          }
+          const uint32_t rowb = sbuf + (uint32_t)lane * 128u, jc0 = (uint32_t)(c0 - c_lo) >> 3; // 16-byte chunk of column c0
+#pragma unroll
+          for (int i = 0; i < 4; ++i)
+            sts128(rowb + (((jc0 + i) ^ ((uint32_t)lane & 7u)) << 4), h[4 * i], h[4 * i + 1], h[4 * i + 2], h[4 * i + 3]);
+          if (c0 + 32 >= c_hi) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) {
+              asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];" ::"l"(
+                               reinterpret_cast<uint64_t>(&tmC)),
+                           "r"(n0 + c_lo), "r"((int)(mt * BM) + q * 32), "r"(sbuf)
+                           : "memory");
+              asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            }
+          }
+          continue;
+        }
         epi_chunk(epi, m, n0 + c0, r);
       }
       // all TMEM reads of this warp are complete (tcgen05.wait::ld in tmem_ld32): hand the buffer back to the MMA warp
@@ -408,6 +454,7 @@ tc_gemm_pk(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUte
       ++j;
     });
   }
+  if (TST && warp >= 2 && lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); // stores done before exit
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
   if (warp == 2) {
@@ -481,20 +528,20 @@ bool get_tensor_map(const __nv_bfloat16* ptr, int64_t rows, int cols, int64_t ld
   return true;
 }
 
-template <int BN, int STAGES>
+template <int BN, int STAGES, bool TST = false>
 int launch_persistent(int64_t M, int N, int K, const CUtensorMap& ta, const CUtensorMap& tb, const TcEpi& epi,
-                      cudaStream_t st) {
-  constexpr int SMEM = STAGES * (BM * BK * 2 + BN * BK * 2) + 1024 + 256;
+                      cudaStream_t st, const CUtensorMap* tc = nullptr) {
+  constexpr int SMEM = STAGES * (BM * BK * 2 + BN * BK * 2) + (TST ? 4 * EPI_PER_Q * TST_WARP_BYTES : 0) + 1024 + 256;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaFuncSetAttribute(tc_gemm_pk<BN, STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
+    cudaFuncSetAttribute(tc_gemm_pk<BN, STAGES, TST>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
     attr_set = true;
   }
   const int n_tiles = N / BN;
   const int64_t total = ((M + BM - 1) / BM) * n_tiles;
   const int per_sm = (2 * BN <= 256 && SMEM <= 110 * 1024) ? 2 : 1; // TMEM: 512 columns per SM
   const unsigned grid = (unsigned)std::min<int64_t>(total, 148 * per_sm);
-  tc_gemm_pk<BN, STAGES><<<grid, NTHREADS_PK, SMEM, st>>>(ta, tb, M, N, K, n_tiles, total, epi);
+  tc_gemm_pk<BN, STAGES, TST><<<grid, NTHREADS_PK, SMEM, st>>>(ta, tb, tc ? *tc : ta, M, N, K, n_tiles, total, epi);
   PNN_KCHECK("tc_gemm_pk");
   return 1;
 }
@@ -534,7 +581,19 @@ int launch_gemm_tc(int64_t M, int N, int K, const __nv_bfloat16* A, int64_t lda,
   if (persist) { // many tiles per SM: the persistent, double-buffered kernel
     switch (bn) {
       case 256: return launch_persistent<256, 4>(M, N, K, ta, tb, epi, st);
-      case 128: return launch_persistent<128, 3>(M, N, K, ta, tb, epi, st);
+      case 128: {
+        // BF16 output, no readout: through shared memory and the TMA store engine (two pipeline stages make room for the
+        // staging buffers at two CTAs per SM)
+        CUtensorMap tc;
+        // Measured on cfg4 (ncu, per launch): N x 768 with bias 264 -> 205 us, N x 256 with bias and SiLU 166 -> 88 us (with the
+        // approximate SiLU), but the plain 3N x 512 conversion epilogue 420 -> 440 us (it loses the third stage and had
+        // little arithmetic to take the stores away from): staged stores only where the epilogue has bias / activation work
+        if (epi.Cb && !epi.readout && (epi.bias || epi.act) && (reinterpret_cast<uintptr_t>(epi.Cb) & 15) == 0 &&
+            (epi.ldcb * 2) % 16 == 0 &&
+            get_tensor_map(epi.Cb, M, N, epi.ldcb, 32, &tc))
+          return launch_persistent<128, 2, true>(M, N, K, ta, tb, epi, st, &tc);
+        return launch_persistent<128, 3>(M, N, K, ta, tb, epi, st);
+      }
       case 64: return launch_persistent<64, 4>(M, N, K, ta, tb, epi, st);
       default: return launch_persistent<32, 4>(M, N, K, ta, tb, epi, st);
     }

@@ -132,11 +132,6 @@ __device__ __forceinline__ void st4_bf16(__nv_bfloat16* p, float4 v) {
   *reinterpret_cast<uint2*>(p) = make_uint2(*reinterpret_cast<const uint32_t*>(&a), *reinterpret_cast<const uint32_t*>(&b));
 }
 
-__device__ __forceinline__ float sqrt_approx(float x) {
-  float y;
-  asm("sqrt.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
 template <typename IT>
 __global__ void __launch_bounds__(256) norm4_k(int64_t N, int F, const IT* __restrict__ PQ, float* __restrict__ sn, float eps,
                                                __nv_bfloat16* __restrict__ sn16) {
@@ -147,13 +142,10 @@ __global__ void __launch_bounds__(256) norm4_k(int64_t N, int F, const IT* __res
   const int f = (int)(idx % F4) * 4;
   const float4 q0 = Ld4<IT>::ld(PQ + (i * 3 + 0) * 2 * F + F + f), q1 = Ld4<IT>::ld(PQ + (i * 3 + 1) * 2 * F + F + f),
                q2 = Ld4<IT>::ld(PQ + (i * 3 + 2) * 2 * F + F + f);
-  const float4 r = make_float4(q0.x * q0.x + q1.x * q1.x + q2.x * q2.x + eps, q0.y * q0.y + q1.y * q1.y + q2.y * q2.y + eps,
-                               q0.z * q0.z + q1.z * q1.z + q2.z * q2.z + eps, q0.w * q0.w + q1.w * q1.w + q2.w * q2.w + eps);
-  if (sn16) { // BF16 model: the norm is rounded to BF16, so the one-instruction square root (sqrt.approx, ~2^-22) serves
-    st4_bf16(sn16 + i * 2 * F + F + f, make_float4(sqrt_approx(r.x), sqrt_approx(r.y), sqrt_approx(r.z), sqrt_approx(r.w)));
-  } else {
-    *reinterpret_cast<float4*>(sn + i * 2 * F + F + f) = make_float4(sqrtf(r.x), sqrtf(r.y), sqrtf(r.z), sqrtf(r.w));
-  }
+  const float4 n = make_float4(sqrtf(q0.x * q0.x + q1.x * q1.x + q2.x * q2.x + eps), sqrtf(q0.y * q0.y + q1.y * q1.y + q2.y * q2.y + eps),
+                               sqrtf(q0.z * q0.z + q1.z * q1.z + q2.z * q2.z + eps), sqrtf(q0.w * q0.w + q1.w * q1.w + q2.w * q2.w + eps));
+  if (sn16) st4_bf16(sn16 + i * 2 * F + F + f, n);
+  else *reinterpret_cast<float4*>(sn + i * 2 * F + F + f) = n;
 }
 
 template <typename IT>
