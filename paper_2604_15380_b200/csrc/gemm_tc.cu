@@ -10,7 +10,10 @@
 //             the epilogue ("accumulator full" mbarrier);
 //   warps 2-5 epilogue: tcgen05.ld (32 lanes x 32 columns per warp): a thread owns one output row and walks it 32 columns
 //             at a time, then bias / SiLU / silu' / accumulate and FP32 / BF16 stores as 32-byte pieces of that row.
-//             Warp 2 also allocates and frees the TMEM columns.
+//             Warp 2 also allocates and frees the TMEM columns.  The persistent kernel (tc_gemm_pk) runs eight epilogue warps,
+//             two per TMEM lane quadrant splitting the tile's columns, and, where the epilogue has bias / activation work
+//             (TST), sends the BF16 output through shared memory and the TMA engine instead: a warp stages its 32 rows x 64
+//             columns (128-byte swizzle) and one lane issues cp.async.bulk.tensor shared -> global.
 // K <= 768 here (at most 12 k-blocks), so a CTA is short; two CTAs share an SM (TMEM 2 x 256 columns, shared memory
 // 2 x <= 113 KB) so one tile's epilogue overlaps the other's loads and MMAs.
 #include <cuda.h>
