@@ -709,7 +709,8 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       nl += l_; ps_.done(l_); }
     GemmEpi<T> e2; e2.bias = W + b.b2;
     { ProfScope ps_(ws, st, "gemm_N");
-    const int l_ = launch_gemm<T>(N, 3 * F, F, h, F, W + b.W2t, 3 * F, phi, 3 * F, e2, st);       // B3a, second Linear
+    // first block: v = 0, so the vv chunk of phi (its last F columns) multiplies zeros in B3b and is not computed
+    const int l_ = launch_gemm<T>(N, (t == 0 ? 2 : 3) * F, F, h, F, W + b.W2t, 3 * F, phi, 3 * F, e2, st); // B3a, second Linear
       nl += l_; ps_.done(l_); }
     ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
     if (t == 0) wait_graph(ws, st);
@@ -736,9 +737,11 @@ int eval_simt(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     { ProfScope ps_(ws, st, "gemm_N");
     const int l_ = launch_gemm<T>(N, F, 2 * F, sn, 2 * F, W + b.A1t, F, k, F, e4, st);
       nl += l_; ps_.done(l_); }
-    GemmEpi<T> e5; e5.bias = W + b.c2;
+    // last block: v is not carried on, so the a_vv gate (the first F columns of a) is not computed (its adjoint is zero too)
+    const int skip = (t + 1 == T_) ? F : 0;
+    GemmEpi<T> e5; e5.bias = W + b.c2 + skip;
     { ProfScope ps_(ws, st, "gemm_N");
-    const int l_ = launch_gemm<T>(N, 3 * F, F, k, F, W + b.A2t, 3 * F, a, 3 * F, e5, st);
+    const int l_ = launch_gemm<T>(N, 3 * F - skip, F, k, F, W + b.A2t + skip, 3 * F, a + skip, 3 * F, e5, st);
       nl += l_; ps_.done(l_); }
     { ProfScope ps_(ws, st, "update_elementwise");
     const int l_ = launch_update<T, T>(N, F, sn, v1, PQ, a, s_cur, v_out, st);
@@ -910,7 +913,7 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
     TcEpi e1; e1.bias = W + b.b1; e1.act = ACT_SILU; e1.pre = want_f ? (T*)tp.hpre : nullptr; e1.ldpre = F; e1.Cb = mb.h16; e1.ldcb = F;
     tc("gemm_N", N, F, F, mb.s16, F, b.W1, e1);                                   // B3a: h = silu(W1 s + b1)
     TcEpi e2; e2.bias = W + b.b2; e2.Cb = tp16.phi16; e2.ldcb = 3 * F;
-    tc("gemm_N", N, 3 * F, F, mb.h16, F, b.W2, e2);                               // B3a: phi = W2 h + b2
+    tc("gemm_N", N, (t == 0 ? 2 : 3) * F, F, mb.h16, F, b.W2, e2);                 // B3a: phi = W2 h + b2 (no vv chunk while v = 0)
     ea.fltW = W + b.fltW; ea.fltb = W + b.fltb;
     if (t == 0) wait_graph(ws, st);
     { ProfScope ps_(ws, st, "edge_fwd");
@@ -925,8 +928,9 @@ int eval_bf16(const pnn_model* m, pnn_workspace* ws, int64_t N, int64_t S, const
       nl += l_; ps_.done(l_); }
     TcEpi e4; e4.bias = W + b.c1; e4.act = ACT_SILU; e4.pre = want_f ? (T*)tp.kpre : nullptr; e4.ldpre = F; e4.Cb = mb.k16; e4.ldcb = F;
     tc("gemm_N", N, F, 2 * F, mb.sn16, 2 * F, b.A1, e4);
-    TcEpi e5; e5.bias = W + b.c2; e5.Cb = a; e5.ldcb = 3 * F;
-    tc("gemm_N", N, 3 * F, F, mb.k16, F, b.A2, e5);
+    const int skip = (t + 1 == T_) ? F : 0; // last block: v is not carried on, the a_vv gate (first F columns) is not computed
+    TcEpi e5; e5.bias = W + b.c2 + skip; e5.Cb = a + skip; e5.ldcb = 3 * F;
+    tc("gemm_N", N, 3 * F - skip, F, mb.k16, F, b.A2 + (int64_t)skip * F, e5);
     { ProfScope ps_(ws, st, "update_elementwise");
       const int l_ = launch_update<T, B>(N, F, sn, v1, PQ, a, s_cur, v_out, st, mb.s16, v_out16);
       nl += l_; ps_.done(l_); }
