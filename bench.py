@@ -190,8 +190,34 @@ def measured_traffic(workload: str, family: str):
     return None, None
 
 
+L2_PEAK_GBS = None   # measured once per run by pnn_measure_l2_peak (L2-resident reads, 512-byte rows per warp)
+
+
+def gather_context(fam: str, per_s: float, E: int, mc, prec: str):
+    """Context for the edge kernels, next to the SURVEY.md 8(d) roof: the sender rows a launch gathers (a4: phi_j and v_j,
+    6 F payload elements per edge; a7 also the adjoint rows s-bar_j, v-bar_j, 4 F more) and the rate at which it does, against
+    the measured bandwidth of L2-resident reads.  The rows are served by L1 and L2 (they are read deg times each), so this is
+    not DRAM traffic and not the roof of the contract -- it shows how far a gather-bound kernel is from the cache it lives in."""
+    pb = {"fp64": 8, "fp32": 4, "bf16": 2}[prec]
+    ab = 8 if prec == "fp64" else 4
+    g = E * mc.F * (6.0 * pb + (4.0 * ab if fam == "edge_bwd" else 0.0))
+    out = dict(gather_bytes=g, gather_gbs=g / per_s / 1e9)
+    if L2_PEAK_GBS:
+        out["l2_peak_gbs_measured"] = L2_PEAK_GBS
+        out["gather_frac_of_l2_peak"] = out["gather_gbs"] / L2_PEAK_GBS
+    return out
+
+
 def family_roofline(fam: str, per_s: float, N: int, E: int, mc, prec: str, forces: bool, peaks, wname: str,
                     alu_meas):
+    r = _family_roofline(fam, per_s, N, E, mc, prec, forces, peaks, wname, alu_meas)
+    if fam in ("edge_fwd", "edge_bwd"):
+        r.update(gather_context(fam, per_s, E, mc, prec))
+    return r
+
+
+def _family_roofline(fam: str, per_s: float, N: int, E: int, mc, prec: str, forces: bool, peaks, wname: str,
+                     alu_meas):
     if fam.startswith("gemm_"):
         flops, byts, _ = gemm_work(fam, N, mc, prec, forces)
     else:
@@ -297,6 +323,11 @@ def main():
             alu_meas[pr] = pnn.pnn_measure_alu_peak(code)
         except Exception:
             alu_meas[pr] = None
+    global L2_PEAK_GBS
+    try:   # context for the gather-bound edge kernels (gather_context)
+        L2_PEAK_GBS = pnn.pnn_measure_l2_peak()
+    except Exception:
+        L2_PEAK_GBS = None
 
     def run_workload(name: str, steps: int, warmup: int, full: bool):
         cfg_id, prec, forces, per_step = WORKLOADS[name]

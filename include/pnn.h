@@ -297,6 +297,13 @@ int pnn_gemm_bf16(int64_t M, int32_t N, int32_t K, const void* A, int64_t lda, c
  * value.  PNN_BF16 -> PNN_ERR_INVALID_ARG (its roofs are HBM and the tensor pipe).  Synchronous. */
 int pnn_measure_alu_peak(int prec, double* tflops, void* cuda_stream);
 
+/* Measured bandwidth of L2-resident reads in GB/s: a 32 MB buffer (a quarter of the L2, far larger than L1) streamed by
+ * every CTA in 512-byte rows per warp, the access shape of the edge kernels' sender-row gathers; best of five launches
+ * timed with CUDA events.  Context for the gather-bound edge kernels (cfg3: 61 neighbours per atom, the sender rows live
+ * in L2, and SURVEY.md 8(d)'s HBM roof says little about them).  *gbs is a host value.  Synchronous; allocates and frees
+ * its buffer. */
+int pnn_measure_l2_peak(double* gbs, void* cuda_stream);
+
 /* Number of kernels the library has launched on behalf of this workspace since it was created. */
 int64_t pnn_launch_count(const pnn_workspace* ws);
 

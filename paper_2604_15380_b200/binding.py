@@ -21,7 +21,7 @@ __all__ = [
     "pnn_graph_view", "pnn_graph_copy", "pnn_build_graph_static", "PNN_STATIC_MAX_ATOMS", "PNN_STATIC_MAX_STRUCTS",
     "PNN_STATIC_MAX_EDGES", "PNN_STATIC_SCRATCH_BYTES", "PNN_STATIC_EDGE_OVERFLOW", "PNN_IMAGES_MINIMUM", "PNN_IMAGES_ALL",
     "pnn_eval", "pnn_eval_replay", "pnn_set_globals", "pnn_eval_blended", "pnn_eval_host", "pnn_stream_create", "pnn_stream_destroy", "pnn_stream_submit", "pnn_stream_wait",
-    "pnn_stream_drain", "pnn_stream_launch_count", "pnn_stream_bytes", "pnn_check_async_errors", "pnn_measure_alu_peak", "pnn_launch_count", "pnn_profile_enable",
+    "pnn_stream_drain", "pnn_stream_launch_count", "pnn_stream_bytes", "pnn_check_async_errors", "pnn_measure_alu_peak", "pnn_measure_l2_peak", "pnn_launch_count", "pnn_profile_enable",
     "pnn_profile_read", "pnn_gemm_bf16",
     "PaiNN", "PRECISIONS",
 ]
@@ -113,6 +113,7 @@ def lib():
         L.pnn_profile_read.argtypes = [vp, i32, vp, vp, vp, ctypes.POINTER(i32)]
         L.pnn_gemm_bf16.argtypes = [i64, i32, i32, vp, i64, vp, i64, vp, i32, vp, i64, vp, i64, vp]
         L.pnn_measure_alu_peak.argtypes = [i32, ctypes.POINTER(ctypes.c_double), vp]
+        L.pnn_measure_l2_peak.argtypes = [ctypes.POINTER(ctypes.c_double), vp]
         L.pnn_launch_count.argtypes = [vp]
         L.pnn_launch_count.restype = i64
         _lib = L
@@ -333,6 +334,13 @@ def pnn_measure_alu_peak(prec: int, stream=None) -> float:
     """Measured TFLOP/s of the FMA pipe (packed FP32 or FP64 chains)."""
     out = ctypes.c_double()
     _check(lib().pnn_measure_alu_peak(int(prec), ctypes.byref(out), stream), "pnn_measure_alu_peak")
+    return out.value
+
+
+def pnn_measure_l2_peak(stream=None) -> float:
+    """Measured GB/s of L2-resident reads (512-byte rows per warp)."""
+    out = ctypes.c_double()
+    _check(lib().pnn_measure_l2_peak(ctypes.byref(out), stream), "pnn_measure_l2_peak")
     return out.value
 
 

@@ -156,4 +156,44 @@ double measure_alu_peak(bool fp64, void* scratch, cudaStream_t st) {
   cudaEventDestroy(e0); cudaEventDestroy(e1);
   return best;
 }
+// L2 read bandwidth: every CTA streams the whole buffer (32 MB, a quarter of the 126 MB L2; after the warm-up pass it is
+// L2-resident and far larger than L1) in 512-byte rows per warp, the access shape of the edge kernels' gathers.
+__global__ void __launch_bounds__(256) peak_l2_k(const float4* __restrict__ buf, int64_t n4, int passes, float* out) {
+  float acc = 0.f;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int p = 0; p < passes; ++p) {
+    // start offset differs per CTA and pass so that the CTAs do not walk the buffer in lockstep
+    int64_t i = ((int64_t)blockIdx.x * 7919 + p * 104729) % n4;
+    i = (i / 32) * 32 + threadIdx.x % 32 + (int64_t)(threadIdx.x / 32) * 32;
+    for (int64_t k = 0; k < n4; k += stride) {
+      int64_t j = i + k;
+      if (j >= n4) j -= n4;
+      const float4 v = __ldcg(buf + j);
+      acc += v.x + v.y + v.z + v.w;
+    }
+  }
+  if (acc == 12345.678f) out[0] = acc; // never true for the zero-filled buffer: keeps the loads alive
+}
+
+double measure_l2_peak(void* buf, int64_t bytes, cudaStream_t st) {
+  cudaEvent_t e0, e1;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return -1.0;
+  const int grid = 148 * 4, block = 256, passes = 8, reps = 5;
+  const int64_t n4 = bytes / 16;
+  double best = 0.0;
+  for (int r = 0; r < reps + 1; ++r) {
+    cudaEventRecord(e0, st);
+    peak_l2_k<<<grid, block, 0, st>>>((const float4*)buf, n4, passes, (float*)buf);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { best = -1.0; break; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    // per pass the grid reads ceil(n4 / stride) * stride vectors
+    const int64_t stride = (int64_t)grid * block;
+    const double moved = (double)((n4 + stride - 1) / stride) * stride * 16.0 * passes;
+    if (r > 0 && ms > 0.f) best = std::max(best, moved / (ms * 1e-3) * 1e-9);   // launch 0 is the warm-up; GB/s
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  return best;
+}
 } // namespace pnn

@@ -279,5 +279,6 @@ template <typename T>
 int launch_branch_mlp(int64_t S, const BranchMlpDims& dm, const int32_t* Z, const int32_t* sptr, const T* params,
                       T* out, int* d_err, cudaStream_t st);
 double measure_alu_peak(bool fp64, void* scratch, cudaStream_t st);   // TFLOP/s of the FMA pipe (packed FP32 / FP64)
+double measure_l2_peak(void* buf, int64_t bytes, cudaStream_t st);      // GB/s of L2-resident reads (512-byte rows per warp)
 
 } // namespace pnn

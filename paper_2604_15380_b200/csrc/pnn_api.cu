@@ -1294,6 +1294,19 @@ int pnn_branch_weights(const pnn_branch_mlp* b, pnn_workspace* ws, int64_t N, in
   return PNN_OK;
 }
 
+int pnn_measure_l2_peak(double* gbs, void* stream) {
+  if (!gbs) return PNN_ERR_INVALID_ARG;
+  const int64_t bytes = 32ll << 20;
+  void* buf = nullptr;
+  PNN_TRY(cudaMalloc(&buf, bytes));
+  if (!cuda_ok(cudaMemsetAsync(buf, 0, bytes, (cudaStream_t)stream), "pnn_measure_l2_peak")) { cudaFree(buf); return PNN_ERR_CUDA; }
+  const double v = measure_l2_peak(buf, bytes, (cudaStream_t)stream);
+  cudaFree(buf);
+  if (v <= 0.0) { cuda_ok(cudaGetLastError(), "pnn_measure_l2_peak"); return PNN_ERR_CUDA; }
+  *gbs = v;
+  return PNN_OK;
+}
+
 int pnn_measure_alu_peak(int prec, double* tflops, void* stream) {
   if (!tflops || (prec != PNN_FP32 && prec != PNN_FP64)) return PNN_ERR_INVALID_ARG;
   void* scratch = nullptr;

@@ -62,3 +62,12 @@ def test_measured_alu_peak_is_near_the_derived_one():
     assert 0.85 * 37.22 < p64 < 1.02 * 37.22, p64
     with pytest.raises(B.PnnError):
         B.pnn_measure_alu_peak(B.PNN_BF16)
+
+
+def test_measured_l2_read_bandwidth_is_above_hbm_and_plausible():
+    """pnn_measure_l2_peak (context for the gather-bound edge kernels in bench.py): L2-resident reads must be faster than
+    the HBM copy peak of MEASURED_PEAKS.json (about 6.5 TB/s on this pool) and below what 148 SMs can take in (64 bytes per
+    clock and SM at 1.965 GHz = 18.6 TB/s)."""
+    from paper_2604_15380_b200 import binding as B
+    v = max(B.pnn_measure_l2_peak() for _ in range(2))
+    assert 6500.0 < v < 18600.0, v
