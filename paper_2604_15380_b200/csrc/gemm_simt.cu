@@ -120,7 +120,9 @@ gemm_k(int64_t M, int N, int K, const T* __restrict__ A, int64_t lda, const T* _
   for (int kt = 0; kt < nk; ++kt) {
     const int buf = kt & 1;
     if (kt + 1 < nk) gload((kt + 1) * BK);
-#pragma unroll
+#pragma unroll 8 // not 16: the fully unrolled k-block (about 800 instructions) ran 16 % of its issue cycles short of
+                 // instructions (ncu: stall_no_instruction 0.46 per issue); halves measured: cfg2 gemm_3N 61.1 -> 58.0 us,
+                 // cfg3 split-K 67.6 -> 65.0 us
     for (int k = 0; k < BK; ++k) {
       T a[TM], b[TN];
 #pragma unroll
@@ -252,7 +254,7 @@ gemm_sk_k(int64_t M, int N, int K, const float* __restrict__ A, int64_t lda, con
   for (int kt = 0; kt < nk; ++kt) {
     const int buf = kt & 1;
     if (kt + 1 < nk) gload(kb0 + (kt + 1) * BK);
-#pragma unroll
+#pragma unroll 8
     for (int k = 0; k < BK; ++k) {
       float a[TM], b[TN];
 #pragma unroll
