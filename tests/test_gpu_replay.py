@@ -84,3 +84,34 @@ def test_eval_host_replays_when_the_shape_repeats(precision):
     finally:
         net.close()
         ref_net.close()
+
+
+@pytest.mark.parametrize("cfg_id,precision,n", [(2, "fp32", 256), (3, "fp32", 64), (3, "bf16", 64), (4, "bf16", 4096),
+                                                (5, "fp64", 1)])
+def test_replay_matches_eager_at_the_sizes_bench_times(cfg_id, precision, n):
+    """The launch configuration bench.py times (whole cfg2 / cfg3 / cfg5 batches, a quarter of a cfg4 batch): the replayed
+    step -- persistent tcgen05 GEMMs with TMA stores, the split-K cluster GEMM, the FP64 tensor-core kernels, the forked
+    graph build -- returns what the kernel-by-kernel path returns, bit for bit."""
+    import torch
+    mc = gen.model_cfg(cfg_id)
+    w = gen.make_weights(mc, cfg_id)
+    b = gen.make_batch(cfg_id, 0, n)
+    want_f = cfg_id != 4
+    net = make_model(mc, w, precision, b.n_atoms, b.n_atoms * (96 if cfg_id in (3, 5) else 40), b.n_structs, want_f)
+    try:
+        t = to_device(b)
+        e_ref, f_ref = net.eval(t["Z"], t["pos"], t["struct_ptr"], t["head"], t["cell"], t["pbc"])
+        e_ref = e_ref.clone()
+        f_ref = None if f_ref is None else f_ref.clone()
+        energy = torch.empty(b.n_structs, dtype=net.out_dtype, device="cuda")
+        forces = torch.empty((b.n_atoms, 3), dtype=net.out_dtype, device="cuda") if want_f else None
+        for _ in range(5):             # calls 0 and 1 eager, call 2 records, calls 3 and 4 replay
+            energy.fill_(float("nan"))
+            net.eval_replay(t["Z"], t["pos"], t["struct_ptr"], t["head"], energy, forces, t["cell"], t["pbc"])
+        torch.cuda.synchronize()
+        net.check()
+        assert torch.equal(energy, e_ref)
+        if want_f:
+            assert torch.equal(forces, f_ref)
+    finally:
+        net.close()
